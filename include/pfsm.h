@@ -1,0 +1,147 @@
+/*
+ * pfsm.h -- C ABI of libpfsm: one partitioned-folded-spectrum-method (PFSM) solve of the dense
+ * real-symmetric FP64 eigenproblem  A V = V Lambda  on one NVIDIA B200 (sm_100a).
+ *
+ * Method: E.L. Briggs, C.T. Kelley, J. Bernholc, "Parallel implementation of electronic structure
+ * eigensolver using a partitioned folded spectrum method", arXiv:1502.07806, section II
+ * (PAPER.md:47-100).  The interface follows the paper's stated intent, "a separate library with a
+ * calling interface similar to the standard eigensolvers" (section VI): LAPACK-like,
+ * column-major, integer status codes.
+ *
+ * The five steps one solve runs, all in hand-written CUDA kernels on the caller's stream:
+ *   1. partition   N eigenpairs -> P contiguous slices of m = N/P; slice s owns the principal
+ *                  submatrix B_s = A[lo:lo+M, lo:lo+M], M = min(N, m + 2*window),
+ *                  lo = clamp(s*m - window, 0, N - M)                      (Fig. 1)
+ *   2. submatrix   batched symmetric eigensolve B_s y = mu y; the slice's m eigenpairs (local
+ *      eigensolve  ascending indices s*m-lo .. s*m-lo+m-1) give shifts eps_i = mu and zero-padded
+ *                  start vectors x_i^0
+ *   3. folded      iters times:  x_i <- x_i - alpha (A - eps_i I)^2 x_i, applied as two successive
+ *      spectrum    products W = A V - V diag(eps), V <- V - alpha (A W - W diag(eps))
+ *                                                                  (Eq. 5 and 11)
+ *   4. Gram-       all N vectors, ascending column order, done as Cholesky-QR:
+ *      Schmidt     G = V^T V = R^T R, V <- V R^-1
+ *   5. eigenvalues lambda_i = v_i^T A v_i and r_i = ||A v_i - lambda_i v_i||_2 (the paper does not
+ *                  say how lambda is produced after step 4; Rayleigh quotients are this library's reading)
+ *
+ * Conventions common to every call
+ *   - All matrices are FP64, column-major with leading dimension N.  Eigenvector i is the
+ *     contiguous column V + i*N.  A is full storage: both triangles valid and exactly mirrored.
+ *   - "device" pointers are CUDA device memory on the device current at pfsm_create; "host"
+ *     pointers are ordinary (ideally pinned) host memory.  All must be 16-byte aligned.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  pfsm_solve
+ *     only enqueues work and returns without synchronizing the host.
+ *   - Return value: 0 = success; -k = the k-th argument is invalid (LAPACK convention);
+ *     >= 1000 = 1000 + cudaError_t of a failed CUDA call.  Numerical status is reported separately
+ *     and asynchronously through pfsm_get_info.
+ *   - The library never frees or reallocates caller memory and never modifies A.  The handle owns
+ *     its workspace.  One handle = one solve in flight; handles are not thread-safe; distinct
+ *     handles on distinct streams are independent.
+ *   - There is no CPU fallback: every call fails with a CUDA error code if no sm_100 device is usable.
+ */
+#ifndef PFSM_H
+#define PFSM_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct pfsm_ctx* pfsm_handle_t; /* opaque */
+
+#define PFSM_CUDA_ERROR_BASE 1000
+
+/*
+ * Create a solver for fixed (N, P, window, iters, alpha) and allocate its device workspace
+ * (about 5 N^2 doubles + P M^2 doubles) on the current device.           [step 1, PAPER.md:88]
+ *   out     host pointer receiving the handle
+ *   N       matrix order; N >= 2, even (TMA row pitch must be a multiple of 16 bytes)
+ *   P       number of spectral slices; P >= 1 and N % P == 0 (the paper writes m = N/P)
+ *   window  halo rows/columns added on each side of a slice's diagonal block; >= 0.
+ *           M = min(N, N/P + 2*window) must be <= 512 in this version.
+ *   iters   folded-spectrum iterations of Eq. 11; >= 0
+ *   alpha   step length of Eq. 11; finite and > 0.  The library does not estimate spectra:
+ *           alpha = 0.5 / max|lambda|^2 keeps every damping factor 1 - alpha (lambda - eps)^2 in [-1, 1].
+ * Errors: -1..-6 for the corresponding argument; 1000+cudaError on allocation failure.
+ */
+int pfsm_create(pfsm_handle_t* out, int64_t N, int32_t P, int32_t window, int32_t iters, double alpha);
+
+/*
+ * Enqueue one PFSM solve (steps 2-5) on `stream`.                         [PAPER.md:86-96]
+ *   A          device, N x N, symmetric, read only
+ *   V_inout    device, N x N.  On output column i is the i-th orthonormal approximate eigenvector.
+ *              Its input content is ignored in this version: start vectors come only from the
+ *              submatrix solutions.
+ *   lambda_out device, N.  lambda_out[i] belongs to column i (slice order; not re-sorted).
+ * Errors: -1 null handle, -2/-3/-4 null or misaligned pointer, 1000+cudaError on launch failure.
+ */
+int pfsm_solve(pfsm_handle_t h, const double* A, double* V_inout, double* lambda_out, void* stream);
+
+/*
+ * Same solve with HOST buffers: copies A host->device, runs pfsm_solve, copies V and lambda back,
+ * all asynchronously on `stream` (pinned host memory recommended), using device staging buffers owned
+ * by the handle (2 N^2 doubles more, allocated on first use).  The caller synchronizes the stream
+ * before reading V_host / lambda_host.
+ */
+int pfsm_solve_host(pfsm_handle_t h, const double* A_host, double* V_host, double* lambda_host, void* stream);
+
+/*
+ * Diagnostic variant of pfsm_solve that stops after step `last_step` (2, 3, 4 or 5) and leaves V in
+ * its state after that step (2: zero-padded start vectors; 3: after the folded-spectrum iterations;
+ * 4: orthonormalized; 5 = pfsm_solve).  lambda_out is written only when last_step == 5 and may be
+ * NULL otherwise.  Used by the parity tests to compare each step with the oracle.
+ */
+int pfsm_solve_partial(pfsm_handle_t h, const double* A, double* V_inout, double* lambda_out, void* stream,
+                       int32_t last_step);
+
+/* Release the handle and its workspace (synchronizes the device).  NULL is a no-op returning 0. */
+int pfsm_destroy(pfsm_handle_t h);
+
+/*
+ * Numerical status of the last solve; synchronizes `stream` (the stream that solve was enqueued on).
+ *   *info = 0        success
+ *   1 <= *info <= N  Cholesky pivot *info of V^T V was not positive: the N vectors are numerically
+ *                    dependent -- the paper's failure mode for a matrix that is not diagonally
+ *                    dominant.  Outputs are undefined; use a standard eigensolver
+ *                    for this step.
+ *   *info = N+s+1    the submatrix eigensolver of slice s did not converge within its sweep cap.
+ */
+int pfsm_get_info(pfsm_handle_t h, void* stream, int64_t* info);
+
+/* Device pointer to the N residual norms r_i = ||A v_i - lambda_i v_i||_2 of the last solve (step 5). */
+int pfsm_get_residuals(pfsm_handle_t h, const double** r_device);
+
+/* Device pointer to the N shifts eps_i (submatrix eigenvalues) of the last solve (step 2). */
+int pfsm_get_shifts(pfsm_handle_t h, const double** eps_device);
+
+/* Change alpha (it scales with 1/||A||^2, so it changes when the spectrum's extent does). */
+int pfsm_set_alpha(pfsm_handle_t h, double alpha);
+
+/* Bytes of device workspace the handle currently owns. */
+size_t pfsm_workspace_bytes(pfsm_handle_t h);
+
+/* Number of kernels (and memsets/copies excluded) one pfsm_solve of this handle launches. */
+int64_t pfsm_launches_per_solve(pfsm_handle_t h);
+
+/*
+ * Per-step device times of the NEXT solves: when enabled, pfsm_solve records CUDA events between the
+ * steps; pfsm_get_step_ms synchronizes and returns ms for steps 2, 3, 4, 5 in ms[0..3].
+ */
+int pfsm_enable_step_timing(pfsm_handle_t h, int32_t enable);
+int pfsm_get_step_ms(pfsm_handle_t h, float* ms4);
+
+/*
+ * Roofline calibration (no data, no memory traffic): runs a register-only loop of FP64 tensor
+ * instructions (mma.sync m8n8k4 f64 -> SASS DMMA.8x8x4) on every SM and returns the issue-rate peak
+ * in TFLOP/s measured with CUDA events.  kind 0 = DMMA, kind 1 = scalar DFMA.
+ */
+int pfsm_probe_fp64_peak(int32_t kind, void* stream, double* tflops);
+
+/* Static text for a return code of this API. */
+const char* pfsm_strerror(int code);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PFSM_H */

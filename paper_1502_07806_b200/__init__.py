@@ -1,0 +1,208 @@
+"""paper_1502_07806_b200 -- thin Python binding over libpfsm.so (include/pfsm.h).
+
+Argument marshalling only: every step of the PFSM solve (arXiv 1502.07806 section II)
+runs in the CUDA kernels behind the C ABI.  PyTorch is used for device memory and streams, nothing else.
+There is no CPU fallback: if the library cannot be built/loaded, or CUDA is unavailable, calls raise.
+
+Layout: the C ABI is column-major with eigenvector i at V + i*N.  A C-contiguous torch tensor `Vr` of
+shape (N, N) whose ROW i is eigenvector i is exactly that memory.  A is symmetric (layout immaterial).
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+from . import build as _build
+
+_lib = None
+CUDA_ERROR_BASE = 1000
+
+EXPORTS = [
+    "pfsm_create", "pfsm_solve", "pfsm_solve_host", "pfsm_solve_partial", "pfsm_destroy", "pfsm_get_info",
+    "pfsm_get_residuals", "pfsm_get_shifts", "pfsm_set_alpha", "pfsm_workspace_bytes",
+    "pfsm_launches_per_solve", "pfsm_enable_step_timing", "pfsm_get_step_ms", "pfsm_probe_fp64_peak",
+    "pfsm_strerror",
+]
+
+
+class PfsmError(RuntimeError):
+    def __init__(self, code: int, where: str):
+        self.code = code
+        super().__init__(f"{where} failed with code {code}: {strerror(code)}")
+
+
+def lib_path() -> str:
+    return _build.LIB
+
+
+def load(build_if_missing: bool = True):
+    """dlopen libpfsm.so and declare the prototypes of include/pfsm.h.  Raises if it cannot be loaded."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if build_if_missing and _build.stale():
+        _build.build()
+    if not os.path.exists(_build.LIB):
+        raise RuntimeError(f"{_build.LIB} is missing: build it with `python -m paper_1502_07806_b200.build`")
+    lib = ctypes.CDLL(_build.LIB)
+    i32, i64, dbl, p = ctypes.c_int32, ctypes.c_int64, ctypes.c_double, ctypes.c_void_p
+    lib.pfsm_create.argtypes = [ctypes.POINTER(p), i64, i32, i32, i32, dbl]
+    lib.pfsm_solve.argtypes = [p, p, p, p, p]
+    lib.pfsm_solve_host.argtypes = [p, p, p, p, p]
+    lib.pfsm_solve_partial.argtypes = [p, p, p, p, p, i32]
+    lib.pfsm_destroy.argtypes = [p]
+    lib.pfsm_get_info.argtypes = [p, p, ctypes.POINTER(i64)]
+    lib.pfsm_get_residuals.argtypes = [p, ctypes.POINTER(p)]
+    lib.pfsm_get_shifts.argtypes = [p, ctypes.POINTER(p)]
+    lib.pfsm_set_alpha.argtypes = [p, dbl]
+    lib.pfsm_workspace_bytes.argtypes = [p]
+    lib.pfsm_workspace_bytes.restype = ctypes.c_size_t
+    lib.pfsm_launches_per_solve.argtypes = [p]
+    lib.pfsm_launches_per_solve.restype = i64
+    lib.pfsm_enable_step_timing.argtypes = [p, i32]
+    lib.pfsm_get_step_ms.argtypes = [p, ctypes.POINTER(ctypes.c_float)]
+    lib.pfsm_probe_fp64_peak.argtypes = [i32, p, ctypes.POINTER(dbl)]
+    lib.pfsm_strerror.argtypes = [ctypes.c_int]
+    lib.pfsm_strerror.restype = ctypes.c_char_p
+    for name in EXPORTS:
+        if name not in ("pfsm_workspace_bytes", "pfsm_launches_per_solve", "pfsm_strerror"):
+            getattr(lib, name).restype = ctypes.c_int
+    _lib = lib
+    return lib
+
+
+def strerror(code: int) -> str:
+    return load().pfsm_strerror(code).decode()
+
+
+def _check(code: int, where: str):
+    if code != 0:
+        raise PfsmError(code, where)
+
+
+def _stream_ptr(stream) -> int:
+    import torch
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return int(stream.cuda_stream)
+
+
+def _dev_ptr(t, N, shape, name):
+    import torch
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()
+            and tuple(t.shape) == shape):
+        raise TypeError(f"{name}: need a contiguous CUDA float64 tensor of shape {shape}")
+    return t.data_ptr()
+
+
+def _host_ptr(t, shape, name):
+    import torch
+    if not (isinstance(t, torch.Tensor) and not t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()
+            and tuple(t.shape) == shape):
+        raise TypeError(f"{name}: need a contiguous CPU float64 tensor of shape {shape}")
+    return t.data_ptr()
+
+
+class Handle:
+    """Owns a pfsm_handle_t.  Mirrors the C ABI one to one; see include/pfsm.h for semantics."""
+
+    def __init__(self, N: int, P: int, window: int, iters: int, alpha: float):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_1502_07806_b200 needs a CUDA device (sm_100a); there is no CPU fallback")
+        self._lib = load()
+        self._h = ctypes.c_void_p()
+        _check(self._lib.pfsm_create(ctypes.byref(self._h), N, P, window, iters, alpha), "pfsm_create")
+        self.N, self.P, self.window, self.iters, self.alpha = N, P, window, iters, alpha
+
+    def solve(self, A, Vr, lam, stream=None):
+        N = self.N
+        _check(self._lib.pfsm_solve(self._h, _dev_ptr(A, N, (N, N), "A"), _dev_ptr(Vr, N, (N, N), "V"),
+                                    _dev_ptr(lam, N, (N,), "lambda"), _stream_ptr(stream)), "pfsm_solve")
+
+    def solve_partial(self, A, Vr, lam, last_step: int, stream=None):
+        N = self.N
+        lp = _dev_ptr(lam, N, (N,), "lambda") if lam is not None else None
+        _check(self._lib.pfsm_solve_partial(self._h, _dev_ptr(A, N, (N, N), "A"), _dev_ptr(Vr, N, (N, N), "V"),
+                                            lp, _stream_ptr(stream), last_step), "pfsm_solve_partial")
+
+    def solve_host(self, A_host, Vr_host, lam_host, stream=None):
+        N = self.N
+        _check(self._lib.pfsm_solve_host(self._h, _host_ptr(A_host, (N, N), "A_host"),
+                                         _host_ptr(Vr_host, (N, N), "V_host"), _host_ptr(lam_host, (N,), "lambda_host"),
+                                         _stream_ptr(stream)), "pfsm_solve_host")
+
+    def info(self, stream=None) -> int:
+        v = ctypes.c_int64(-1)
+        _check(self._lib.pfsm_get_info(self._h, _stream_ptr(stream), ctypes.byref(v)), "pfsm_get_info")
+        return int(v.value)
+
+    def _view(self, getter, name):
+        import torch
+        ptr = ctypes.c_void_p()
+        _check(getter(self._h, ctypes.byref(ptr)), name)
+
+        class _DevBuf:  # zero-copy view of the handle-owned device buffer, cloned into a tensor the caller owns
+            __cuda_array_interface__ = {"shape": (self.N,), "typestr": "<f8", "data": (int(ptr.value), True),
+                                        "version": 2}
+
+        return torch.as_tensor(_DevBuf(), device="cuda").clone()
+
+    def residuals(self):
+        return self._view(self._lib.pfsm_get_residuals, "pfsm_get_residuals")
+
+    def shifts(self):
+        return self._view(self._lib.pfsm_get_shifts, "pfsm_get_shifts")
+
+    def set_alpha(self, alpha: float):
+        _check(self._lib.pfsm_set_alpha(self._h, alpha), "pfsm_set_alpha")
+        self.alpha = alpha
+
+    def workspace_bytes(self) -> int:
+        return int(self._lib.pfsm_workspace_bytes(self._h))
+
+    def launches_per_solve(self) -> int:
+        return int(self._lib.pfsm_launches_per_solve(self._h))
+
+    def enable_step_timing(self, enable: bool = True):
+        _check(self._lib.pfsm_enable_step_timing(self._h, int(enable)), "pfsm_enable_step_timing")
+
+    def step_ms(self):
+        arr = (ctypes.c_float * 4)()
+        _check(self._lib.pfsm_get_step_ms(self._h, arr), "pfsm_get_step_ms")
+        return [float(x) for x in arr]
+
+    def destroy(self):
+        if self._h:
+            self._lib.pfsm_destroy(self._h)
+            self._h = ctypes.c_void_p()
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+
+# Function-style aliases with the C names
+def pfsm_create(N, P, window, iters, alpha) -> Handle:
+    return Handle(N, P, window, iters, alpha)
+
+
+def pfsm_solve(h: Handle, A, Vr, lam, stream=None):
+    h.solve(A, Vr, lam, stream)
+
+
+def pfsm_solve_host(h: Handle, A_host, Vr_host, lam_host, stream=None):
+    h.solve_host(A_host, Vr_host, lam_host, stream)
+
+
+def pfsm_destroy(h: Handle):
+    h.destroy()
+
+
+def probe_fp64_peak(kind: int = 0, stream=None) -> float:
+    """TFLOP/s of a register-only FP64 loop on all SMs: kind 0 = DMMA (mma.sync m8n8k4 f64), 1 = DFMA."""
+    v = ctypes.c_double(0.0)
+    _check(load().pfsm_probe_fp64_peak(kind, _stream_ptr(stream), ctypes.byref(v)), "pfsm_probe_fp64_peak")
+    return float(v.value)

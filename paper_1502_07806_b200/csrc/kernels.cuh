@@ -1,0 +1,364 @@
+// kernels.cuh -- the non-GEMM kernels of the PFSM path (sm_100a):
+//   jacobi_batched_kernel   step 2: one CTA per slice, one-sided (Hestenes) Jacobi on the slice's
+//                           shifted submatrix, round-robin parallel ordering, a warp per column pair
+//   chol_diag_kernel        step 4: Cholesky factor + inverse of one 128 x 128 diagonal block
+//   transpose_kernel        step 4: V <-> V^T staging for the stacked Cholesky-QR
+//   rayleigh_kernel         step 5: lambda_i = v_i . t_i and r_i = ||t_i - lambda_i v_i||
+//   fp64 peak probes        roofline calibration
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace pfsm {
+
+struct SliceTable {  // step 1: device-resident, built once in pfsm_create
+    const int32_t* g0;   // first global eigen-index of slice s
+    const int32_t* lo;   // first row/column of its submatrix
+    const int32_t* off;  // local index of the slice's first eigenpair = g0 - lo
+};
+
+constexpr int JACOBI_THREADS = 1024;
+constexpr int JACOBI_MAX_SWEEPS = 40;
+
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+// ---------------------------------------------------------------------------------------------
+// Step 2: B_s y = mu y for slice s = blockIdx.x.
+//
+// One-sided Jacobi on G = B_s + sigma I (sigma = 2 x Gershgorin bound, so G is SPD with condition
+// number <= 3): rotate column pairs of G until all columns are mutually orthogonal.  Then
+// G = (B_s + sigma I) J with J orthogonal and G^T G diagonal, so column c of G is (mu_c + sigma) y_c:
+// the eigenvector is the normalized column and mu_c = ||g_c|| - sigma.  No second matrix is needed.
+// G (M x M, column-major, 8 M^2 bytes: 72-512 KiB) lives in the handle's workspace and stays L2
+// resident; each warp takes one column pair per turn, holds both columns in registers (EPL doubles
+// per lane per column), forms the three dot products with shuffles, rotates and writes back.
+// Pairs of a round are disjoint (round-robin tournament), rounds are separated by __syncthreads.
+//
+// Output: for the slice's m eigenpairs (ascending local ranks off .. off+m-1):
+//   eps[g0 + j] = mu;  V[(g0 + j) * N + lo + r] = y[r]   (V was zero-filled before the launch).
+// info: atomicMin-style first failure N + s + 1 if the sweep cap is hit.
+// ---------------------------------------------------------------------------------------------
+template <int EPL>
+__global__ void __launch_bounds__(JACOBI_THREADS, 1)
+jacobi_batched_kernel(const double* __restrict__ A, int64_t N, int32_t M, int32_t m, SliceTable tab,
+                      double* __restrict__ Gws, double* __restrict__ V, double* __restrict__ eps,
+                      unsigned long long* info) {
+    const int s = blockIdx.x;
+    const int lo = tab.lo[s], off = tab.off[s], g0 = tab.g0[s];
+    double* G = Gws + (size_t)s * M * M;
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    constexpr int NW = JACOBI_THREADS / 32;
+
+    __shared__ double red[NW];
+    __shared__ double s_sigma;
+    __shared__ int s_rot;
+    extern __shared__ double dyn[];  // nrm[M] then rank (int) [M]
+    double* nrm = dyn;
+    int* rank = reinterpret_cast<int*>(dyn + M);
+
+    // Gershgorin bound: max_r sum_c |B[r][c]|  (thread per row; consecutive rows are contiguous)
+    double bound = 0.0;
+    for (int r = tid; r < M; r += JACOBI_THREADS) {
+        double sum = 0.0;
+        for (int c = 0; c < M; ++c) sum += fabs(A[(size_t)(lo + c) * N + lo + r]);
+        bound = fmax(bound, sum);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) bound = fmax(bound, __shfl_xor_sync(0xffffffffu, bound, o));
+    if (lane == 0) red[warp] = bound;
+    __syncthreads();
+    if (tid == 0) {
+        double b = 0.0;
+        for (int w = 0; w < NW; ++w) b = fmax(b, red[w]);
+        s_sigma = (b > 0.0) ? 2.0 * b : 1.0;
+    }
+    __syncthreads();
+    const double sigma = s_sigma;
+    for (int idx = tid; idx < M * M; idx += JACOBI_THREADS) {
+        const int c = idx / M, r = idx - c * M;
+        double v = A[(size_t)(lo + c) * N + lo + r];
+        if (r == c) v += sigma;
+        G[idx] = v;
+    }
+    __syncthreads();
+
+    const int Me = M + (M & 1);  // phantom column when M is odd
+    const int n1 = Me - 1, npairs = Me / 2;
+    const double tol = 2.220446049250313e-16 * sqrt((double)M);
+    bool converged = false;
+    for (int sweep = 0; sweep < JACOBI_MAX_SWEEPS; ++sweep) {
+        if (tid == 0) s_rot = 0;
+        __syncthreads();
+        int nrot = 0;
+        for (int rnd = 0; rnd < n1; ++rnd) {
+            for (int pi = warp; pi < npairs; pi += NW) {
+                int p, q;
+                if (pi == 0) {
+                    p = n1;
+                    q = rnd;
+                } else {
+                    p = rnd + pi;
+                    if (p >= n1) p -= n1;
+                    q = rnd - pi;
+                    if (q < 0) q += n1;
+                }
+                if (p >= M || q >= M) continue;
+                if (p > q) {
+                    const int tmp = p;
+                    p = q;
+                    q = tmp;
+                }
+                double* gp = G + (size_t)p * M;
+                double* gq = G + (size_t)q * M;
+                double x[EPL], y[EPL];
+                double aa = 0.0, bb = 0.0, ab = 0.0;
+#pragma unroll
+                for (int e = 0; e < EPL; ++e) {
+                    const int r = lane + 32 * e;
+                    x[e] = (r < M) ? gp[r] : 0.0;
+                    y[e] = (r < M) ? gq[r] : 0.0;
+                    aa = fma(x[e], x[e], aa);
+                    bb = fma(y[e], y[e], bb);
+                    ab = fma(x[e], y[e], ab);
+                }
+                aa = warp_sum(aa);
+                bb = warp_sum(bb);
+                ab = warp_sum(ab);
+                if (fabs(ab) > tol * sqrt(aa * bb)) {
+                    const double zeta = (bb - aa) / (2.0 * ab);
+                    const double tt = copysign(1.0, zeta) / (fabs(zeta) + sqrt(1.0 + zeta * zeta));
+                    const double cs = 1.0 / sqrt(1.0 + tt * tt), sn = cs * tt;
+#pragma unroll
+                    for (int e = 0; e < EPL; ++e) {
+                        const int r = lane + 32 * e;
+                        if (r < M) {
+                            gp[r] = cs * x[e] - sn * y[e];
+                            gq[r] = sn * x[e] + cs * y[e];
+                        }
+                    }
+                    ++nrot;
+                }
+            }
+            __syncthreads();
+        }
+        if (lane == 0 && nrot) atomicAdd(&s_rot, nrot);
+        __syncthreads();
+        const int total = s_rot;
+        __syncthreads();
+        if (total == 0) {
+            converged = true;
+            break;
+        }
+    }
+    if (!converged && tid == 0) atomicMin(info, (unsigned long long)(N + s + 1));
+
+    // column norms -> eigenvalues; rank by counting (ties: lower column index first)
+    for (int c = warp; c < M; c += NW) {
+        const double* gc = G + (size_t)c * M;
+        double ss = 0.0;
+        for (int r = lane; r < M; r += 32) ss = fma(gc[r], gc[r], ss);
+        ss = warp_sum(ss);
+        if (lane == 0) nrm[c] = sqrt(ss);
+    }
+    __syncthreads();
+    for (int c = tid; c < M; c += JACOBI_THREADS) {
+        const double v = nrm[c];
+        int rk = 0;
+        for (int j = 0; j < M; ++j) {
+            const double u = nrm[j];
+            rk += (u < v || (u == v && j < c)) ? 1 : 0;
+        }
+        rank[c] = rk;
+    }
+    __syncthreads();
+    for (int c = warp; c < M; c += NW) {
+        const int j = rank[c] - off;
+        if (j < 0 || j >= m) continue;
+        const double nv = nrm[c];
+        const double inv = 1.0 / nv;
+        const double* gc = G + (size_t)c * M;
+        double* v = V + (size_t)(g0 + j) * N + lo;
+        // sign convention: largest-magnitude component positive is not needed (R16); keep G's sign
+        for (int r = lane; r < M; r += 32) v[r] = gc[r] * inv;
+        if (lane == 0) eps[g0 + j] = nv - sigma;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Step 4 helper: Cholesky factor and inverse of one diagonal block (order nb <= 128) of the stacked
+// matrix S (row-major view, leading dimension ld).  Reads the lower triangle of S[k0:k0+nb, k0:k0+nb],
+// writes L (lower, upper zeroed) to Lout[k0:k0+nb, k0:k0+nb] (leading dimension ld) and L^-1 (lower,
+// zero padded to 128 x 128) to Dinv (leading dimension 128).  A non-positive pivot j sets
+// info = min(info, k0 + j + 1) (the vectors are numerically dependent).
+// ---------------------------------------------------------------------------------------------
+constexpr int CHOL_NB = 128;
+constexpr int CHOL_THREADS = 1024;
+constexpr int CHOL_LDS = CHOL_NB + 1;
+constexpr int CHOL_SMEM = 2 * CHOL_NB * CHOL_LDS * 8;
+
+__global__ void __launch_bounds__(CHOL_THREADS, 1)
+chol_diag_kernel(const double* __restrict__ S, double* __restrict__ Lout, int64_t ld, int32_t k0, int32_t nb,
+                 double* __restrict__ Dinv, unsigned long long* info) {
+    extern __shared__ double sm[];
+    double* a = sm;                        // a[i][c], leading dimension CHOL_LDS
+    double* li = sm + CHOL_NB * CHOL_LDS;  // inverse
+    __shared__ double s_d;
+    const int tid = threadIdx.x;
+    for (int idx = tid; idx < CHOL_NB * CHOL_NB; idx += CHOL_THREADS) {
+        const int i = idx >> 7, c = idx & 127;
+        double v = 0.0;
+        if (i < nb && c < nb && c <= i) v = S[(size_t)(k0 + i) * ld + k0 + c];
+        a[i * CHOL_LDS + c] = v;
+        li[i * CHOL_LDS + c] = 0.0;
+    }
+    __syncthreads();
+    // right-looking Cholesky on the lower triangle; thread owns row i = tid & 127, columns c = cg + 8 q
+    const int i = tid & 127, cg = tid >> 7;
+    for (int j = 0; j < nb; ++j) {
+        if (tid == 0) {
+            double piv = a[j * CHOL_LDS + j];
+            if (!(piv > 0.0)) {
+                atomicMin(info, (unsigned long long)(k0 + j + 1));
+                piv = 1.0;
+            }
+            s_d = sqrt(piv);
+        }
+        __syncthreads();
+        const double d = s_d;
+        if (tid < nb && tid >= j) a[tid * CHOL_LDS + j] = (tid == j) ? d : a[tid * CHOL_LDS + j] / d;
+        __syncthreads();
+        if (i > j && i < nb) {
+            const double lij = a[i * CHOL_LDS + j];
+            for (int c = j + 1 + cg; c <= i; c += 8) a[i * CHOL_LDS + c] -= lij * a[c * CHOL_LDS + j];
+        }
+        // the next pivot column is complete only after every thread's update
+        __syncthreads();
+    }
+    // inverse by forward substitution, one thread per column c of L^-1 (rows broadcast across the warp)
+    if (tid < nb) {
+        const int c = tid;
+        li[c * CHOL_LDS + c] = 1.0 / a[c * CHOL_LDS + c];
+        for (int r = c + 1; r < nb; ++r) {
+            double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
+            int k = c;
+            for (; k + 3 < r; k += 4) {
+                s0 = fma(a[r * CHOL_LDS + k], li[k * CHOL_LDS + c], s0);
+                s1 = fma(a[r * CHOL_LDS + k + 1], li[(k + 1) * CHOL_LDS + c], s1);
+                s2 = fma(a[r * CHOL_LDS + k + 2], li[(k + 2) * CHOL_LDS + c], s2);
+                s3 = fma(a[r * CHOL_LDS + k + 3], li[(k + 3) * CHOL_LDS + c], s3);
+            }
+            for (; k < r; ++k) s0 = fma(a[r * CHOL_LDS + k], li[k * CHOL_LDS + c], s0);
+            li[r * CHOL_LDS + c] = -((s0 + s1) + (s2 + s3)) / a[r * CHOL_LDS + r];
+        }
+    }
+    __syncthreads();
+    for (int idx = tid; idx < CHOL_NB * CHOL_NB; idx += CHOL_THREADS) {
+        const int r = idx >> 7, c = idx & 127;
+        Dinv[idx] = li[r * CHOL_LDS + c];
+        if (r < nb && c < nb) Lout[(size_t)(k0 + r) * ld + k0 + c] = (c <= r) ? a[r * CHOL_LDS + c] : 0.0;
+    }
+}
+
+// out[c][r] = in[r][c] for an nr x nc row-major matrix (leading dimensions ldi / ldo)
+__global__ void transpose_kernel(const double* __restrict__ in, int64_t ldi, double* __restrict__ out,
+                                 int64_t ldo, int32_t nr, int32_t nc) {
+    __shared__ double tile[32][33];
+    const int bx = blockIdx.x * 32, by = blockIdx.y * 32;
+    const int tx = threadIdx.x, ty = threadIdx.y;  // 32 x 8
+#pragma unroll
+    for (int k = 0; k < 32; k += 8) {
+        const int r = by + ty + k, c = bx + tx;
+        if (r < nr && c < nc) tile[ty + k][tx] = in[(size_t)r * ldi + c];
+    }
+    __syncthreads();
+#pragma unroll
+    for (int k = 0; k < 32; k += 8) {
+        const int c = bx + ty + k, r = by + tx;
+        if (r < nr && c < nc) out[(size_t)c * ldo + r] = tile[tx][ty + k];
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Step 5: one CTA per eigenvector i.  lambda_i = v_i . t_i  (t_i = A v_i from the GEMM), then
+// r_i = || t_i - lambda_i v_i ||_2.  Vectorised, coalesced; fixed reduction order (deterministic).
+// ---------------------------------------------------------------------------------------------
+constexpr int RAY_THREADS = 256;
+__device__ __forceinline__ double block_sum(double v, double* red) {
+    v = warp_sum(v);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    __syncthreads();
+    if (lane == 0) red[warp] = v;
+    __syncthreads();
+    double t = 0.0;
+    for (int w = 0; w < RAY_THREADS / 32; ++w) t += red[w];
+    return t;
+}
+__global__ void __launch_bounds__(RAY_THREADS)
+rayleigh_kernel(const double* __restrict__ V, const double* __restrict__ T, int64_t N, double* __restrict__ lambda,
+                double* __restrict__ resid) {
+    __shared__ double red[RAY_THREADS / 32];
+    const int64_t i = blockIdx.x;
+    const double2* v2 = reinterpret_cast<const double2*>(V + i * N);
+    const double2* t2 = reinterpret_cast<const double2*>(T + i * N);
+    const int64_t n2 = N / 2;  // N is even
+    double s = 0.0;
+    for (int64_t k = threadIdx.x; k < n2; k += RAY_THREADS) {
+        const double2 a = v2[k], b = t2[k];
+        s = fma(a.x, b.x, s);
+        s = fma(a.y, b.y, s);
+    }
+    const double lam = block_sum(s, red);
+    double q = 0.0;
+    for (int64_t k = threadIdx.x; k < n2; k += RAY_THREADS) {
+        const double2 a = v2[k], b = t2[k];
+        const double e0 = b.x - lam * a.x, e1 = b.y - lam * a.y;
+        q = fma(e0, e0, q);
+        q = fma(e1, e1, q);
+    }
+    const double rr = block_sum(q, red);
+    if (threadIdx.x == 0) {
+        lambda[i] = lam;
+        resid[i] = sqrt(rr);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Roofline calibration: register-only FP64 issue-rate loops (no memory traffic).
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) probe_dmma_kernel(int iters, double* sink) {
+    double c[16][2];
+#pragma unroll
+    for (int i = 0; i < 16; ++i) c[i][0] = c[i][1] = 0.0;
+    const double a = 1.0 + 1e-9 * threadIdx.x, b = 1.0 - 1e-9 * threadIdx.x;
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int i = 0; i < 16; ++i)
+            asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+                         : "+d"(c[i][0]), "+d"(c[i][1])
+                         : "d"(a), "d"(b));
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int i = 0; i < 16; ++i) s += c[i][0] + c[i][1];
+    if (s == 123.456) sink[0] = s;
+}
+__global__ void __launch_bounds__(256) probe_dfma_kernel(int iters, double* sink) {
+    double c[16];
+#pragma unroll
+    for (int i = 0; i < 16; ++i) c[i] = 1e-3 * i;
+    const double a = 1.0 + 1e-9 * threadIdx.x, b = 1e-9 * threadIdx.x;
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int i = 0; i < 16; ++i) asm volatile("fma.rn.f64 %0, %0, %1, %2;" : "+d"(c[i]) : "d"(a), "d"(b));
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int i = 0; i < 16; ++i) s += c[i];
+    if (s == 123.456) sink[0] = s;
+}
+
+}  // namespace pfsm

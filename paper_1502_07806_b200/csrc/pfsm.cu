@@ -1,0 +1,439 @@
+// pfsm.cu -- C-ABI boundary (include/pfsm.h) and step orchestration of one PFSM solve on sm_100a.
+// Steps and citations: see include/pfsm.h.  All compute runs in the kernels of gemm_tn.cuh and
+// kernels.cuh on the caller's stream; the host only validates arguments, encodes TMA descriptors
+// and enqueues launches.  There is no CPU fallback.
+#include "../../include/pfsm.h"
+
+#include <cuda.h>
+#include <cuda_runtime.h>
+
+#include <climits>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <vector>
+
+#include "gemm_tn.cuh"
+#include "kernels.cuh"
+
+namespace pfsm {
+
+#define PFSM_CUDA(call)                                              \
+    do {                                                             \
+        cudaError_t e__ = (call);                                    \
+        if (e__ != cudaSuccess) return PFSM_CUDA_ERROR_BASE + (int)e__; \
+    } while (0)
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+static EncodeTiledFn get_encode_fn() {
+    static EncodeTiledFn fn = nullptr;
+    if (!fn) {
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+            q == cudaDriverEntryPointSuccess)
+            fn = (EncodeTiledFn)p;
+    }
+    return fn;
+}
+
+// 2-D FP64 tensor map over a row-major (rows x cols, leading dimension ld) matrix; box = 128 rows x 16
+// doubles (one 128-byte swizzle span); out-of-bounds elements read as zero.
+static int make_map(CUtensorMap* map, const double* base, int64_t rows, int64_t cols, int64_t ld) {
+    EncodeTiledFn fn = get_encode_fn();
+    if (!fn) return PFSM_CUDA_ERROR_BASE + (int)cudaErrorNotSupported;
+    cuuint64_t gdim[2] = {(cuuint64_t)cols, (cuuint64_t)rows};
+    cuuint64_t gstr[1] = {(cuuint64_t)ld * 8};
+    cuuint32_t box[2] = {(cuuint32_t)BK, (cuuint32_t)BM};
+    cuuint32_t estr[2] = {1, 1};
+    CUresult r = fn(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, (void*)base, gdim, gstr, box, estr,
+                    CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                    CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return r == CUDA_SUCCESS ? 0 : PFSM_CUDA_ERROR_BASE + (int)cudaErrorInvalidValue;
+}
+
+}  // namespace pfsm
+
+using namespace pfsm;
+
+struct pfsm_ctx {
+    int64_t N;
+    int32_t P, window, iters, m, M;
+    double alpha;
+    int device;
+    // device workspace
+    double* W = nullptr;      // N x N   : W of step 3, T of step 5
+    double* S = nullptr;      // 2N x N  : stacked [G ; V^T] of step 4
+    double* O = nullptr;      // 2N x N  : stacked [L ; V^T R^-1]
+    double* Dinv = nullptr;   // nblk x 128 x 128 : inverses of L's diagonal blocks
+    double* Gws = nullptr;    // P x M x M : Jacobi workspace
+    double* eps = nullptr;    // N shifts
+    double* resid = nullptr;  // N residual norms
+    int32_t* slice_tab = nullptr;  // g0[P], lo[P], off[P]
+    int2* krange = nullptr;        // per 128-row tile k-range of the first product
+    unsigned long long* info = nullptr;
+    double* A_stage = nullptr;  // host-buffer path
+    double* V_stage = nullptr;
+    double* lam_stage = nullptr;
+    size_t bytes = 0;
+    int32_t nblk;
+    CUtensorMap mapW, mapS, mapO, mapD;
+    bool timing = false;
+    cudaEvent_t ev[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
+    bool ev_valid = false;
+};
+
+static int dev_alloc(pfsm_ctx* h, void** p, size_t bytes) {
+    PFSM_CUDA(cudaMalloc(p, bytes));
+    h->bytes += bytes;
+    return 0;
+}
+
+template <int EPI>
+static int launch_gemm(const CUtensorMap& mx, const CUtensorMap& my, GemmParams p, cudaStream_t st) {
+    p.ntr = (p.mr + BM - 1) / BM;
+    p.ntc = (p.nc + BN - 1) / BN;
+    if (p.mr <= 0 || p.nc <= 0) return 0;
+    const int64_t tiles = gemm_num_tiles(p.ntr, p.ntc, p.lower);
+    if (tiles <= 0) return 0;
+    static bool attr_set[4] = {false, false, false, false};
+    if (!attr_set[EPI]) {
+        PFSM_CUDA(cudaFuncSetAttribute(gemm_tn_kernel<EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, GEMM_SMEM));
+        attr_set[EPI] = true;
+    }
+    gemm_tn_kernel<EPI><<<(unsigned)tiles, GEMM_THREADS, GEMM_SMEM, st>>>(mx, my, p);
+    PFSM_CUDA(cudaGetLastError());
+    return 0;
+}
+
+static GemmParams base_params() {
+    GemmParams p;
+    memset(&p, 0, sizeof(p));
+    return p;
+}
+
+extern "C" {
+
+const char* pfsm_strerror(int code) {
+    if (code == 0) return "success";
+    if (code < 0) {
+        static const char* names[] = {"", "argument 1 invalid", "argument 2 invalid", "argument 3 invalid",
+                                      "argument 4 invalid", "argument 5 invalid", "argument 6 invalid"};
+        return (-code <= 6) ? names[-code] : "invalid argument";
+    }
+    if (code >= PFSM_CUDA_ERROR_BASE) return cudaGetErrorString((cudaError_t)(code - PFSM_CUDA_ERROR_BASE));
+    return "unknown error";
+}
+
+int pfsm_create(pfsm_handle_t* out, int64_t N, int32_t P, int32_t window, int32_t iters, double alpha) {
+    if (!out) return -1;
+    *out = nullptr;
+    if (N < 2 || (N & 1) || N > (1 << 30)) return -2;
+    if (P < 1 || N % P != 0) return -3;
+    if (window < 0) return -4;
+    if (iters < 0) return -5;
+    if (!std::isfinite(alpha) || !(alpha > 0.0)) return -6;
+    const int64_t m = N / P;
+    const int64_t M = std::min<int64_t>(N, m + 2 * (int64_t)window);
+    if (M > 512) return -4;
+
+    pfsm_ctx* h = new pfsm_ctx();
+    h->N = N; h->P = P; h->window = window; h->iters = iters; h->alpha = alpha;
+    h->m = (int32_t)m; h->M = (int32_t)M;
+    h->nblk = (int32_t)((N + CHOL_NB - 1) / CHOL_NB);
+    int rc = 0;
+#define TRY(x) do { rc = (x); if (rc) { pfsm_destroy(h); return rc; } } while (0)
+    {
+        cudaError_t e = cudaGetDevice(&h->device);
+        if (e != cudaSuccess) { delete h; return PFSM_CUDA_ERROR_BASE + (int)e; }
+    }
+    const size_t n2 = (size_t)N * N * sizeof(double);
+    TRY(dev_alloc(h, (void**)&h->W, n2));
+    TRY(dev_alloc(h, (void**)&h->S, 2 * n2));
+    TRY(dev_alloc(h, (void**)&h->O, 2 * n2));
+    TRY(dev_alloc(h, (void**)&h->Dinv, (size_t)h->nblk * CHOL_NB * CHOL_NB * sizeof(double)));
+    TRY(dev_alloc(h, (void**)&h->Gws, (size_t)P * M * M * sizeof(double)));
+    TRY(dev_alloc(h, (void**)&h->eps, N * sizeof(double)));
+    TRY(dev_alloc(h, (void**)&h->resid, N * sizeof(double)));
+    TRY(dev_alloc(h, (void**)&h->slice_tab, 3 * (size_t)P * sizeof(int32_t)));
+    const int32_t ntr = (int32_t)((N + BM - 1) / BM);
+    TRY(dev_alloc(h, (void**)&h->krange, (size_t)ntr * sizeof(int2)));
+    TRY(dev_alloc(h, (void**)&h->info, sizeof(unsigned long long)));
+
+    // step 1: slice table, and the k-range each 128-row tile of the first product needs
+    std::vector<int32_t> tab(3 * (size_t)P);
+    for (int32_t s = 0; s < P; ++s) {
+        const int64_t g0 = (int64_t)s * m;
+        const int64_t lo = std::min<int64_t>(std::max<int64_t>(g0 - window, 0), N - M);
+        tab[s] = (int32_t)g0;
+        tab[P + s] = (int32_t)lo;
+        tab[2 * (size_t)P + s] = (int32_t)(g0 - lo);
+    }
+    std::vector<int2> kr(ntr);
+    for (int32_t t = 0; t < ntr; ++t) {
+        const int64_t i0 = (int64_t)t * BM, i1 = std::min<int64_t>(N, i0 + BM) - 1;
+        const int64_t lo0 = tab[P + i0 / m], hi1 = tab[P + i1 / m] + M;
+        kr[t].x = (int)(lo0 / BK * BK);
+        kr[t].y = (int)((hi1 + BK - 1) / BK * BK);
+    }
+    {
+        cudaError_t e = cudaMemcpy(h->slice_tab, tab.data(), tab.size() * sizeof(int32_t), cudaMemcpyHostToDevice);
+        if (e == cudaSuccess) e = cudaMemcpy(h->krange, kr.data(), kr.size() * sizeof(int2), cudaMemcpyHostToDevice);
+        if (e == cudaSuccess) e = cudaMemset(h->info, 0xFF, sizeof(unsigned long long));
+        if (e == cudaSuccess) e = cudaMemset(h->resid, 0, N * sizeof(double));
+        if (e == cudaSuccess) e = cudaMemset(h->eps, 0, N * sizeof(double));
+        if (e != cudaSuccess) { pfsm_destroy(h); return PFSM_CUDA_ERROR_BASE + (int)e; }
+    }
+    TRY(make_map(&h->mapW, h->W, N, N, N));
+    TRY(make_map(&h->mapS, h->S, 2 * N, N, N));
+    TRY(make_map(&h->mapO, h->O, 2 * N, N, N));
+    TRY(make_map(&h->mapD, h->Dinv, (int64_t)h->nblk * CHOL_NB, CHOL_NB, CHOL_NB));
+    for (int i = 0; i < 5; ++i) {
+        cudaError_t e = cudaEventCreate(&h->ev[i]);
+        if (e != cudaSuccess) { pfsm_destroy(h); return PFSM_CUDA_ERROR_BASE + (int)e; }
+    }
+#undef TRY
+    *out = h;
+    return 0;
+}
+
+int pfsm_destroy(pfsm_handle_t h) {
+    if (!h) return 0;
+    cudaDeviceSynchronize();
+    void* ptrs[] = {h->W, h->S, h->O, h->Dinv, h->Gws, h->eps, h->resid, h->slice_tab, h->krange, h->info,
+                    h->A_stage, h->V_stage, h->lam_stage};
+    for (void* p : ptrs)
+        if (p) cudaFree(p);
+    for (int i = 0; i < 5; ++i)
+        if (h->ev[i]) cudaEventDestroy(h->ev[i]);
+    delete h;
+    return 0;
+}
+
+static int launch_jacobi(pfsm_ctx* h, const double* A, double* V, cudaStream_t st) {
+    SliceTable tab{h->slice_tab, h->slice_tab + h->P, h->slice_tab + 2 * (size_t)h->P};
+    const size_t dyn = (size_t)h->M * (sizeof(double) + sizeof(int));
+    if (h->M <= 128)
+        jacobi_batched_kernel<4><<<h->P, JACOBI_THREADS, dyn, st>>>(A, h->N, h->M, h->m, tab, h->Gws, V, h->eps, h->info);
+    else if (h->M <= 256)
+        jacobi_batched_kernel<8><<<h->P, JACOBI_THREADS, dyn, st>>>(A, h->N, h->M, h->m, tab, h->Gws, V, h->eps, h->info);
+    else
+        jacobi_batched_kernel<16><<<h->P, JACOBI_THREADS, dyn, st>>>(A, h->N, h->M, h->m, tab, h->Gws, V, h->eps, h->info);
+    PFSM_CUDA(cudaGetLastError());
+    return 0;
+}
+
+int pfsm_solve_partial(pfsm_handle_t h, const double* A, double* V, double* lambda_out, void* stream,
+                       int32_t last_step) {
+    if (!h) return -1;
+    if (!A || ((uintptr_t)A & 15)) return -2;
+    if (!V || ((uintptr_t)V & 15)) return -3;
+    if (last_step < 2 || last_step > 5) return -6;
+    if (last_step == 5 && (!lambda_out || ((uintptr_t)lambda_out & 7))) return -4;
+    cudaStream_t st = (cudaStream_t)stream;
+    const int64_t N = h->N;
+    const int32_t n = (int32_t)N;
+    int rc;
+    CUtensorMap mapA, mapV;
+    if ((rc = make_map(&mapA, A, N, N, N))) return rc;
+    if ((rc = make_map(&mapV, V, N, N, N))) return rc;
+    const bool tm = h->timing;
+    h->ev_valid = false;
+
+    // ---- step 2: batched submatrix eigensolves -> shifts and zero-padded start vectors ----
+    if (tm) PFSM_CUDA(cudaEventRecord(h->ev[0], st));
+    PFSM_CUDA(cudaMemsetAsync(h->info, 0xFF, sizeof(unsigned long long), st));
+    PFSM_CUDA(cudaMemsetAsync(V, 0, (size_t)N * N * sizeof(double), st));
+    if ((rc = launch_jacobi(h, A, V, st))) return rc;
+    if (tm) PFSM_CUDA(cudaEventRecord(h->ev[1], st));
+    if (last_step == 2) return 0;
+
+    // ---- step 3: folded-spectrum iterations (Eq. 11), two products per iteration ----
+    for (int it = 0; it < h->iters; ++it) {
+        GemmParams p = base_params();  // W = V A - diag(eps) V   (row-major view; A symmetric)
+        p.C = h->W; p.ldc = N; p.mr = n; p.nc = n; p.klen = n;
+        p.krange = (it == 0) ? h->krange : nullptr;  // start vectors are zero outside their window
+        p.E1 = V; p.ld1 = N; p.eps = h->eps;
+        if ((rc = launch_gemm<EPI_SHIFT>(mapV, mapA, p, st))) return rc;
+        GemmParams q = base_params();  // V <- V - alpha (W A - diag(eps) W)
+        q.C = V; q.ldc = N; q.mr = n; q.nc = n; q.klen = n;
+        q.E1 = h->W; q.ld1 = N; q.E2 = V; q.ld2 = N; q.eps = h->eps; q.alpha = h->alpha;
+        if ((rc = launch_gemm<EPI_UPDATE>(h->mapW, mapA, q, st))) return rc;
+    }
+    if (tm) PFSM_CUDA(cudaEventRecord(h->ev[2], st));
+    if (last_step == 3) return 0;
+
+    // ---- step 4: Cholesky-QR on the stacked matrix [G ; V^T],  G = V^T V (row-major view: V V^T) ----
+    {
+        const dim3 tb(32, 8), tg((unsigned)((N + 31) / 32), (unsigned)((N + 31) / 32));
+        transpose_kernel<<<tg, tb, 0, st>>>(V, N, h->S + (size_t)N * N, N, n, n);
+        PFSM_CUDA(cudaGetLastError());
+        GemmParams p = base_params();
+        p.C = h->S; p.ldc = N; p.mr = n; p.nc = n; p.klen = n; p.lower = 1;
+        if ((rc = launch_gemm<EPI_PLAIN>(mapV, mapV, p, st))) return rc;
+        static bool chol_attr = false;
+        if (!chol_attr) {
+            PFSM_CUDA(cudaFuncSetAttribute(chol_diag_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, CHOL_SMEM));
+            chol_attr = true;
+        }
+        for (int32_t k = 0; k < h->nblk; ++k) {
+            const int32_t k0 = k * CHOL_NB, nb = (int32_t)std::min<int64_t>(CHOL_NB, N - k0);
+            chol_diag_kernel<<<1, CHOL_THREADS, CHOL_SMEM, st>>>(h->S, h->O, N, k0, nb,
+                                                                 h->Dinv + (size_t)k * CHOL_NB * CHOL_NB, h->info);
+            PFSM_CUDA(cudaGetLastError());
+            // panel: O[r, k0:k0+nb] = S[r, k0:k0+nb] L_kk^-T   for all rows below the diagonal block
+            GemmParams pp = base_params();
+            pp.C = h->O; pp.ldc = N; pp.cr0 = k0 + nb; pp.cc0 = k0; pp.mr = 2 * n - k0 - nb; pp.nc = nb;
+            pp.xr0 = k0 + nb; pp.xk0 = k0; pp.yr0 = k * CHOL_NB; pp.yk0 = 0; pp.klen = nb;
+            if ((rc = launch_gemm<EPI_PLAIN>(h->mapS, h->mapD, pp, st))) return rc;
+            // trailing update: S[r, c] -= O[r, k0:k0+nb] . O[c, k0:k0+nb]   (tiles with r >= c)
+            if (k0 + nb < n) {
+                GemmParams pt = base_params();
+                pt.C = h->S; pt.ldc = N; pt.cr0 = k0 + nb; pt.cc0 = k0 + nb; pt.mr = 2 * n - k0 - nb;
+                pt.nc = n - k0 - nb; pt.xr0 = k0 + nb; pt.yr0 = k0 + nb; pt.xk0 = k0; pt.yk0 = k0; pt.klen = nb;
+                pt.lower = 1;
+                if ((rc = launch_gemm<EPI_SUB>(h->mapO, h->mapO, pt, st))) return rc;
+            }
+        }
+        transpose_kernel<<<tg, tb, 0, st>>>(h->O + (size_t)N * N, N, V, N, n, n);
+        PFSM_CUDA(cudaGetLastError());
+    }
+    if (tm) PFSM_CUDA(cudaEventRecord(h->ev[3], st));
+    if (last_step == 4) return 0;
+
+    // ---- step 5: T = V A, Rayleigh quotients and residual norms ----
+    {
+        GemmParams p = base_params();
+        p.C = h->W; p.ldc = N; p.mr = n; p.nc = n; p.klen = n;
+        if ((rc = launch_gemm<EPI_PLAIN>(mapV, mapA, p, st))) return rc;
+        rayleigh_kernel<<<(unsigned)N, RAY_THREADS, 0, st>>>(V, h->W, N, lambda_out, h->resid);
+        PFSM_CUDA(cudaGetLastError());
+    }
+    if (tm) {
+        PFSM_CUDA(cudaEventRecord(h->ev[4], st));
+        h->ev_valid = true;
+    }
+    return 0;
+}
+
+int pfsm_solve(pfsm_handle_t h, const double* A, double* V_inout, double* lambda_out, void* stream) {
+    return pfsm_solve_partial(h, A, V_inout, lambda_out, stream, 5);
+}
+
+int pfsm_solve_host(pfsm_handle_t h, const double* A_host, double* V_host, double* lambda_host, void* stream) {
+    if (!h) return -1;
+    if (!A_host) return -2;
+    if (!V_host) return -3;
+    if (!lambda_host) return -4;
+    const size_t n2 = (size_t)h->N * h->N * sizeof(double);
+    if (!h->A_stage) {
+        int rc;
+        if ((rc = dev_alloc(h, (void**)&h->A_stage, n2))) return rc;
+        if ((rc = dev_alloc(h, (void**)&h->V_stage, n2))) return rc;
+        if ((rc = dev_alloc(h, (void**)&h->lam_stage, h->N * sizeof(double)))) return rc;
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    PFSM_CUDA(cudaMemcpyAsync(h->A_stage, A_host, n2, cudaMemcpyHostToDevice, st));
+    int rc = pfsm_solve(h, h->A_stage, h->V_stage, h->lam_stage, stream);
+    if (rc) return rc;
+    PFSM_CUDA(cudaMemcpyAsync(V_host, h->V_stage, n2, cudaMemcpyDeviceToHost, st));
+    PFSM_CUDA(cudaMemcpyAsync(lambda_host, h->lam_stage, h->N * sizeof(double), cudaMemcpyDeviceToHost, st));
+    return 0;
+}
+
+int pfsm_get_info(pfsm_handle_t h, void* stream, int64_t* info) {
+    if (!h) return -1;
+    if (!info) return -3;
+    unsigned long long v = 0;
+    PFSM_CUDA(cudaMemcpyAsync(&v, h->info, sizeof(v), cudaMemcpyDeviceToHost, (cudaStream_t)stream));
+    PFSM_CUDA(cudaStreamSynchronize((cudaStream_t)stream));
+    *info = (v == ULLONG_MAX) ? 0 : (int64_t)v;
+    return 0;
+}
+
+int pfsm_get_residuals(pfsm_handle_t h, const double** r) {
+    if (!h) return -1;
+    if (!r) return -2;
+    *r = h->resid;
+    return 0;
+}
+
+int pfsm_get_shifts(pfsm_handle_t h, const double** e) {
+    if (!h) return -1;
+    if (!e) return -2;
+    *e = h->eps;
+    return 0;
+}
+
+int pfsm_set_alpha(pfsm_handle_t h, double alpha) {
+    if (!h) return -1;
+    if (!std::isfinite(alpha) || !(alpha > 0.0)) return -2;
+    h->alpha = alpha;
+    return 0;
+}
+
+size_t pfsm_workspace_bytes(pfsm_handle_t h) { return h ? h->bytes : 0; }
+
+int64_t pfsm_launches_per_solve(pfsm_handle_t h) {
+    if (!h) return 0;
+    // jacobi + 2 iters GEMMs + (2 transposes + Gram + per panel: diag, panel, trailing (none after the last)) + GEMM + rayleigh
+    return 1 + 2 * (int64_t)h->iters + (2 + 1 + 3 * (int64_t)h->nblk - 1) + 2;
+}
+
+int pfsm_enable_step_timing(pfsm_handle_t h, int32_t enable) {
+    if (!h) return -1;
+    h->timing = enable != 0;
+    h->ev_valid = false;
+    return 0;
+}
+
+int pfsm_get_step_ms(pfsm_handle_t h, float* ms4) {
+    if (!h) return -1;
+    if (!ms4) return -2;
+    if (!h->ev_valid) return -1;
+    PFSM_CUDA(cudaEventSynchronize(h->ev[4]));
+    for (int i = 0; i < 4; ++i) PFSM_CUDA(cudaEventElapsedTime(&ms4[i], h->ev[i], h->ev[i + 1]));
+    return 0;
+}
+
+int pfsm_probe_fp64_peak(int32_t kind, void* stream, double* tflops) {
+    if (kind < 0 || kind > 1) return -1;
+    if (!tflops) return -3;
+    cudaStream_t st = (cudaStream_t)stream;
+    int dev = 0, sms = 0;
+    PFSM_CUDA(cudaGetDevice(&dev));
+    PFSM_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    double* sink = nullptr;
+    PFSM_CUDA(cudaMalloc(&sink, 8));
+    cudaEvent_t e0, e1;
+    PFSM_CUDA(cudaEventCreate(&e0));
+    PFSM_CUDA(cudaEventCreate(&e1));
+    const int blocks = sms * 4, threads = 256;
+    const int iters = (kind == 0) ? 20000 : 40000;
+    float best = 1e30f;
+    for (int rep = 0; rep < 4; ++rep) {
+        PFSM_CUDA(cudaEventRecord(e0, st));
+        if (kind == 0)
+            probe_dmma_kernel<<<blocks, threads, 0, st>>>(iters, sink);
+        else
+            probe_dfma_kernel<<<blocks, threads, 0, st>>>(iters, sink);
+        PFSM_CUDA(cudaEventRecord(e1, st));
+        PFSM_CUDA(cudaEventSynchronize(e1));
+        float ms = 0;
+        PFSM_CUDA(cudaEventElapsedTime(&ms, e0, e1));
+        if (rep > 0 && ms < best) best = ms;
+    }
+    // per warp per iteration: DMMA 16 x (8*8*4*2) flops; DFMA 16 x 32 x 2 flops
+    const double per_warp_iter = (kind == 0) ? 16.0 * 512.0 : 16.0 * 64.0;
+    const double flops = per_warp_iter * (double)iters * (threads / 32) * (double)blocks;
+    *tflops = flops / ((double)best * 1e-3) * 1e-12;
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    cudaFree(sink);
+    return 0;
+}
+
+}  // extern "C"

@@ -1,0 +1,290 @@
+"""GPU parity: the CUDA path (through the C ABI of include/pfsm.h) against the CPU oracle, element by
+element on the same seeded inputs.  Tolerances are north_star's (reading R20):
+    |lambda_gpu - lambda_oracle| <= 1e-10 ||A||_F        per index
+    ||V^T V - I||_max            <= 1e-12 N              (GPU and oracle each)
+    |r_gpu - r_oracle|           <= 1e-9 ||A||_F         per vector
+Eigenvectors are compared up to their sign only where they are unique (reading R16)."""
+import os
+
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import pfsm_inputs as gen
+
+pytestmark = pytest.mark.gpu
+
+pfsm = pytest.importorskip("paper_1502_07806_b200")
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def gpu_solve(A, P, w, iters, alpha, last_step=5):
+    N = A.shape[0]
+    h = pfsm.Handle(N, P, w, iters, alpha)
+    dA = dev(A)
+    dV = torch.full((N, N), float("nan"), dtype=torch.float64, device="cuda")  # input content must be ignored (R13)
+    dl = torch.full((N,), float("nan"), dtype=torch.float64, device="cuda")
+    if last_step == 5:
+        h.solve(dA, dV, dl)
+    else:
+        h.solve_partial(dA, dV, dl, last_step)
+    info = h.info()
+    out = dict(Vr=dV.cpu().numpy(), lam=dl.cpu().numpy(), resid=h.residuals().cpu().numpy(),
+               eps=h.shifts().cpu().numpy(), info=info)
+    h.destroy()
+    return out
+
+
+def align_signs(Vg, Vo):
+    s = np.sign(np.einsum("ij,ij->i", Vg, Vo))
+    s[s == 0] = 1.0
+    return Vg * s[:, None]
+
+
+def check_gates(p_A, g, o):
+    N = p_A.shape[0]
+    nF = float(np.linalg.norm(p_A))
+    assert g["info"] == 0 and o["info"] == 0
+    assert np.abs(g["lam"] - o["lam"]).max() <= 1e-10 * nF
+    assert np.abs(g["Vr"] @ g["Vr"].T - np.eye(N)).max() <= 1e-12 * N
+    assert np.abs(o["Vr"] @ o["Vr"].T - np.eye(N)).max() <= 1e-12 * N
+    assert np.abs(g["resid"] - o["resid"]).max() <= 1e-9 * nF
+    assert abs(g["lam"].sum() - np.trace(p_A)) <= 1e-11 * N * max(1.0, np.abs(np.diag(p_A)).max())  # P7
+
+
+# shapes: several 128-tiles plus ragged tails; odd M; m not dividing the tile; slices straddling tiles
+SMALL_CASES = [
+    # N, P, w, iters, amp, width
+    (256, 4, 16, 3, 1e-3, 16.0),     # BASELINE config 0 shape
+    (304, 4, 10, 2, 2e-3, 12.0),     # ragged: 304 = 2*128 + 48, M = 96
+    (270, 6, 4, 3, 1e-3, 8.0),       # m = 45, M = 53 (odd -> phantom column in the tournament)
+    (400, 5, 24, 1, 1e-3, 16.0),     # M = 128
+    (600, 3, 20, 2, 5e-4, 24.0),     # m = 200, M = 240, slices straddle tiles
+    (130, 1, 0, 2, 1e-2, 8.0),       # P = 1: submatrix = A, PFSM exact (P3)
+    (96, 4, 100, 2, 1e-2, 8.0),      # window >= N: every slice diagonalizes all of A
+    (64, 8, 0, 4, 1e-3, 4.0),        # window 0: M = m
+    (2, 1, 0, 1, 1e-1, 1.0),         # smallest legal problem
+]
+
+
+@pytest.mark.parametrize("N,P,w,iters,amp,width", SMALL_CASES)
+def test_stepwise_parity_small(N, P, w, iters, amp, width):
+    p = gen.small_problem(N, amp, width, seed=1000 + N)
+    nF = p.normF
+    # step 2: shifts and zero-padded start vectors
+    g2 = gpu_solve(p.A, P, w, iters, p.alpha, last_step=2)
+    V2, eps, info2 = oracle.step2(p.A, P, w)
+    assert g2["info"] == 0 and info2 == 0
+    assert np.abs(g2["eps"] - eps).max() <= 1e-13 * max(1.0, nF)
+    assert np.array_equal(g2["Vr"] == 0.0, V2 == 0.0) or np.abs(align_signs(g2["Vr"], V2) - V2).max() < 1e-9
+    M, g0, lo, off = oracle.partition(N, P, w)
+    for s in range(P):   # exactly zero outside the slice's window
+        rows = g2["Vr"][g0[s]:g0[s] + N // P]
+        mask = np.ones(N, bool)
+        mask[lo[s]:lo[s] + M] = False
+        assert np.all(rows[:, mask] == 0.0)
+    assert np.abs(align_signs(g2["Vr"], V2) - V2).max() < 1e-9
+    # step 3 (Eq. 11) from the ORACLE's start vectors' signs
+    g3 = gpu_solve(p.A, P, w, iters, p.alpha, last_step=3)
+    V3 = oracle.step3(p.A, V2, eps, iters, p.alpha)
+    assert np.abs(align_signs(g3["Vr"], V3) - V3).max() < 1e-9
+    # step 4 (Gram-Schmidt as Cholesky-QR) and step 5
+    g = gpu_solve(p.A, P, w, iters, p.alpha)
+    o = oracle.pfsm(p.A, P, w, iters, p.alpha)
+    check_gates(p.A, g, o)
+    assert np.abs(align_signs(g["Vr"], o["Vr"]) - o["Vr"]).max() < 1e-8
+    # uniqueness of thin QR: V_out^T V_in = R upper triangular with positive diagonal (reading R10)
+    R = g["Vr"] @ g3["Vr"].T
+    assert np.abs(np.tril(R, -1)).max() < 1e-10
+    assert np.all(np.diag(R) > 0)
+
+
+def test_iters_zero_is_gram_schmidt_of_start_vectors():
+    p = gen.small_problem(288, 1e-3, 16.0, seed=77)
+    g = gpu_solve(p.A, 4, 12, 0, p.alpha)
+    o = oracle.pfsm(p.A, 4, 12, 0, p.alpha)
+    check_gates(p.A, g, o)
+
+
+def test_diagonal_input_is_a_fixed_point():
+    # P1: B_s diagonal -> eps = d, start vectors = unit vectors, every step leaves them unchanged
+    N = 384
+    d = np.sort(gen.uniform(5, gen.STREAM_TEST, 0, N) * 2 - 1)
+    g = gpu_solve(np.diag(d), 3, 20, 3, 0.5)
+    assert g["info"] == 0
+    assert np.abs(g["lam"] - d).max() < 1e-14
+    assert np.abs(np.abs(g["Vr"]) - np.eye(N)).max() < 1e-14
+    assert g["resid"].max() < 1e-14
+
+
+def test_exact_degeneracy_invariants_only():
+    N = 256
+    d = np.repeat(np.arange(N // 8, dtype=np.float64) * 0.1, 8)
+    g = gpu_solve(np.diag(d), 4, 16, 2, 0.5 / d.max() ** 2)
+    assert g["info"] == 0
+    np.testing.assert_allclose(np.sort(g["lam"]), d, atol=1e-13)
+    assert np.abs(g["Vr"] @ g["Vr"].T - np.eye(N)).max() < 1e-12 * N
+    assert g["resid"].max() < 1e-13
+
+
+def test_block_diagonal_slices_exact():
+    # P2 on the GPU: blocks = slices with separated spectra -> PFSM exact, incl. clamped end windows
+    P, m, w = 4, 64, 16
+    N = P * m
+    A = np.zeros((N, N))
+    expected = []
+    for s in range(P):
+        d = 10.0 * s + np.sort(gen.uniform(77, gen.STREAM_TEST, 100 * s, m))
+        Q = gen.householder_orthogonal(m, 2, 300 + s)
+        Bs = (Q * d) @ Q.T
+        Bs = 0.5 * (Bs + Bs.T)
+        A[s * m:(s + 1) * m, s * m:(s + 1) * m] = Bs
+        expected.append(np.linalg.eigvalsh(Bs))
+    expected = np.concatenate(expected)
+    g = gpu_solve(A, P, w, 2, 0.5 / 31.0 ** 2)
+    nA = np.linalg.norm(A)
+    assert g["info"] == 0
+    np.testing.assert_allclose(g["lam"], expected, atol=1e-13 * nA)
+    assert g["resid"].max() < 1e-13 * nA
+
+
+def test_breakdown_is_flagged_for_dependent_vectors():
+    # P12 / PAPER.md:98: A = Q D Q^T with a dense random Q.  The GPU must either flag it (info != 0)
+    # or return residuals far above the well-conditioned case -- never silently "succeed".
+    N, P, w = 256, 4, 8
+    d = np.sort(gen.uniform(51, gen.STREAM_TEST, 0, N) * 2 - 1)
+    X = gen.normal(51, gen.STREAM_TEST, 10_000, N * N).reshape(N, N)
+    Q, _ = np.linalg.qr(X)
+    A = (Q * d) @ Q.T
+    A = 0.5 * (A + A.T)
+    g = gpu_solve(A, P, w, 3, 0.5)
+    good = gen.small_problem(N, 1e-3, 8.0, seed=51)
+    gg = gpu_solve(good.A, P, w, 3, good.alpha)
+    assert gg["info"] == 0
+    assert g["info"] != 0 or g["resid"].max() > 100 * gg["resid"].max()
+
+
+def test_singular_gram_sets_info():
+    # an all-zero matrix has B_s = 0 for every slice: overlapping windows then yield duplicated unit
+    # vectors?  No: each slice takes distinct local indices of the identity, so vectors stay independent.
+    # Force dependence instead with a rank-deficient coupling: two identical decoupled 2x2 blocks share
+    # eigenvectors only if windows overlap fully -- use window >= N so every slice sees all of A, with an
+    # exactly degenerate spectrum; ranks tie -> stable order -> still independent.  So check the flag
+    # through the Cholesky directly: alpha so large that one iteration annihilates a direction.
+    N = 128
+    d = np.linspace(-1.0, 1.0, N)
+    A = np.diag(d)
+    A[0, 1] = A[1, 0] = 0.3
+    # alpha = 1/(lambda-eps)^2 kills the component along the neighbouring eigenvector exactly; with a tiny
+    # window (M = m, no halo) the start vectors of slice 0 and 1 are unit vectors, not eigenvectors
+    g = gpu_solve(A, 64, 0, 1, 1e6)
+    assert g["info"] != 0 or not np.isfinite(g["lam"]).all() or g["resid"].max() > 1e-3
+
+
+def test_solve_is_deterministic_and_ignores_v_input():
+    p = gen.problem(0)
+    c = p.cfg
+    a = gpu_solve(p.A, c.P, c.window, c.iters, p.alpha)
+    b = gpu_solve(p.A, c.P, c.window, c.iters, p.alpha)
+    assert np.array_equal(a["lam"], b["lam"]) and np.array_equal(a["Vr"], b["Vr"])
+
+
+def test_host_buffer_entry_point_matches_device_entry_point():
+    p = gen.problem(0)
+    c = p.cfg
+    N = c.N
+    h = pfsm.Handle(N, c.P, c.window, c.iters, p.alpha)
+    Ah = torch.from_numpy(p.A).pin_memory()
+    Vh = torch.empty((N, N), dtype=torch.float64).pin_memory()
+    lh = torch.empty((N,), dtype=torch.float64).pin_memory()
+    h.solve_host(Ah, Vh, lh)
+    torch.cuda.synchronize()
+    assert h.info() == 0
+    ref = gpu_solve(p.A, c.P, c.window, c.iters, p.alpha)
+    assert np.array_equal(lh.numpy(), ref["lam"]) and np.array_equal(Vh.numpy(), ref["Vr"])
+    h.destroy()
+
+
+def test_solve_on_a_side_stream():
+    p = gen.problem(0)
+    c = p.cfg
+    N = c.N
+    st = torch.cuda.Stream()
+    h = pfsm.Handle(N, c.P, c.window, c.iters, p.alpha)
+    dA = dev(p.A)
+    dV = torch.empty((N, N), dtype=torch.float64, device="cuda")
+    dl = torch.empty((N,), dtype=torch.float64, device="cuda")
+    torch.cuda.synchronize()
+    with torch.cuda.stream(st):
+        h.solve(dA, dV, dl, stream=st)
+    assert h.info(stream=st) == 0
+    ref = gpu_solve(p.A, c.P, c.window, c.iters, p.alpha)
+    assert np.array_equal(dl.cpu().numpy(), ref["lam"])
+    h.destroy()
+
+
+@pytest.mark.parametrize("k", [0, 1, 2])
+def test_baseline_configs_full_oracle(k):
+    """BASELINE.json configs 0-2 at full size: element-by-element gates against the full oracle run."""
+    p = gen.problem(k)
+    c = p.cfg
+    g = gpu_solve(p.A, c.P, c.window, c.iters, p.alpha)
+    o = oracle.pfsm(p.A, c.P, c.window, c.iters, p.alpha)
+    check_gates(p.A, g, o)
+    assert np.abs(g["eps"] - o["eps"]).max() <= 1e-12 * p.normF
+
+
+@pytest.mark.parametrize("k", [3, 4])
+def test_baseline_configs_large_sampled(k):
+    """BASELINE.json configs 3-4 at full size, in bench.py's launch configuration.  The full oracle needs
+    ~1e13 flop (minutes), so: steps 2-3 are compared with the oracle on sampled whole slices (slices are
+    independent); step 4 through the uniqueness of QR (V_out orthonormal and V_out^T V_3
+    upper triangular with positive diagonal <=> V_out is THE Gram-Schmidt result); step 5 on sampled
+    columns the oracle computes one by one; trace and residual-enclosure hold at any size.
+    PFSM_FULL_ORACLE=1 adds the full element-by-element comparison."""
+    p = gen.problem(k)
+    c = p.cfg
+    N, m = c.N, c.m
+    nF = p.normF
+    g3 = gpu_solve(p.A, c.P, c.window, c.iters, p.alpha, last_step=3)
+    assert g3["info"] == 0
+    M, g0, lo, off = oracle.partition(N, c.P, c.window)
+    for s in sorted({0, 1, c.P // 2, c.P - 1}):
+        B = p.A[lo[s]:lo[s] + M, lo[s]:lo[s] + M]
+        mu, Y, sw = oracle.jacobi_eig(B)
+        assert sw > 0
+        eps_s = mu[off[s]:off[s] + m]
+        assert np.abs(g3["eps"][g0[s]:g0[s] + m] - eps_s).max() <= 1e-12 * nF
+        V0 = np.zeros((N, N))
+        V0[g0[s]:g0[s] + m, lo[s]:lo[s] + M] = Y[:, off[s]:off[s] + m].T
+        eps_full = np.zeros(N)
+        eps_full[g0[s]:g0[s] + m] = eps_s
+        V3 = oracle.step3(p.A, V0, eps_full, c.iters, p.alpha, int(g0[s]), int(g0[s] + m))[g0[s]:g0[s] + m]
+        Vg = g3["Vr"][g0[s]:g0[s] + m]
+        assert np.abs(align_signs(Vg, V3) - V3).max() < 1e-8
+    g = gpu_solve(p.A, c.P, c.window, c.iters, p.alpha)
+    assert g["info"] == 0
+    Vg = torch.from_numpy(g["Vr"]).cuda()
+    V3g = torch.from_numpy(g3["Vr"]).cuda()
+    eye_err = (Vg @ Vg.T - torch.eye(N, dtype=torch.float64, device="cuda")).abs().max().item()
+    assert eye_err <= 1e-12 * N
+    R = Vg @ V3g.T
+    assert torch.tril(R, -1).abs().max().item() < 1e-9
+    assert (torch.diagonal(R) > 0).all()
+    cols = [0, 1, m - 1, m, N // 2, N - 2, N - 1] + [int(x) for x in (gen.uniform(9, gen.STREAM_TEST, k, 9) * N)]
+    for i in cols:
+        lam_o, res_o = oracle.step5(p.A, g["Vr"], i, i + 1)
+        assert abs(lam_o[i] - g["lam"][i]) <= 1e-10 * nF
+        assert abs(res_o[i] - g["resid"][i]) <= 1e-9 * nF
+    assert abs(g["lam"].sum() - np.trace(p.A)) <= 1e-9
+    ex = torch.linalg.eigvalsh(torch.from_numpy(p.A).cuda()).cpu().numpy()   # comparison only (P9 enclosure)
+    idx = np.searchsorted(ex, g["lam"])
+    near = np.minimum(np.abs(ex[np.clip(idx, 0, N - 1)] - g["lam"]), np.abs(ex[np.clip(idx - 1, 0, N - 1)] - g["lam"]))
+    assert np.all(near <= g["resid"] + 1e-10)
+    if os.environ.get("PFSM_FULL_ORACLE") == "1":
+        o = oracle.pfsm(p.A, c.P, c.window, c.iters, p.alpha)
+        check_gates(p.A, g, o)
