@@ -1,0 +1,361 @@
+#!/usr/bin/env python
+"""bench.py -- one PFSM solve per step on synthetic matrices shaped like the paper's workloads.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 4] [--impl ours|reference]
+
+A "step" is one pass of the whole hot path (batched submatrix
+eigensolves, folded-spectrum iterations, Cholesky-QR orthonormalization, Rayleigh quotients) over one
+N x N matrix.  The metric is BASELINE.json's: ms per solve and sustained FP64 TFLOP/s, where the flops are
+the ALGORITHMIC ones of SURVEY.md section 8(d):  F = (4 iters + 7/3) N^3 + 2 N^2 M.
+Prints ONE JSON line (rank 0).  `--impl reference` times the CPU oracle (oracle/) on a bounded sample.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+FP64_NOMINAL_RATIO = 45.0 / 2250.0  # guide's nominal B200 FP64-tensor : bf16-tensor dense peaks
+
+
+def algorithmic_flops(N: int, M: int, iters: int) -> dict:
+    f3 = 2.0 * N * N * M + (2 * iters - 1) * 2.0 * N ** 3 if iters > 0 else 0.0
+    f4 = 7.0 * N ** 3 / 3.0
+    f5 = 2.0 * N ** 3 + 5.0 * N * N
+    return {"step3": f3, "step4": f4, "step5": f5, "total": f3 + f4 + f5}
+
+
+def measured_peaks() -> dict:
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        d = json.load(open(path))
+        d["_source"] = "measured"
+        return d
+    return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0, "_source": "fallback"}
+
+
+class ClockSampler:
+    """Samples nvidia-smi clocks / throttle reasons of one GPU while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index = index
+        self.rows = []
+        self.proc = None
+        self.thread = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                 "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            self.proc = None
+            return
+        self.thread = threading.Thread(target=self._read, daemon=True)
+        self.thread.start()
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.time(), line.strip()))
+
+    def stop(self, t0: float, t1: float) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for t, line in self.rows:
+            if not (t0 - 0.05 <= t <= t1 + 0.05):
+                continue
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
+            except ValueError:
+                continue
+            for name, val in zip(names, f[3:7]):
+                if val.lower().startswith("active"):
+                    reasons.add(name)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples inside the timed region"]}
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": max(mx), "power_w_max": max(pw), "samples": len(sm),
+                "reasons": sorted(reasons)}
+
+
+def oracle_sample(cfg_index: int, ncols: int, reps: int, warmup: int):
+    """Times the oracle, as it stands, on a bounded sample of config `cfg_index`: slice P/2's submatrix
+    eigensolve (O2), then Eq. 11 (O3) and the Rayleigh quotients (O5) for `ncols` of its eigenvectors.
+    Returns (seconds per sample (list), flops per sample, description, threads)."""
+    import numpy as np
+
+    import oracle
+    import pfsm_inputs as gen
+    p = gen.problem(cfg_index)
+    c = p.cfg
+    N, m = c.N, c.m
+    ncols = min(ncols, m)
+    M, g0, lo, off = oracle.partition(N, c.P, c.window)
+    s = c.P // 2
+    times = []
+    for rep in range(warmup + reps):
+        t0 = time.perf_counter()
+        B = p.A[lo[s]:lo[s] + M, lo[s]:lo[s] + M]
+        mu, Y, _ = oracle.jacobi_eig(B)
+        V0 = np.zeros((N, N))
+        eps = np.zeros(N)
+        c0, c1 = int(g0[s]), int(g0[s]) + ncols
+        V0[c0:c1, lo[s]:lo[s] + M] = Y[:, off[s]:off[s] + ncols].T
+        eps[c0:c1] = mu[off[s]:off[s] + ncols]
+        V3 = oracle.step3(p.A, V0, eps, c.iters, p.alpha, c0, c1)
+        rows = V3[c0:c1]
+        V3[c0:c1] = rows / np.linalg.norm(rows, axis=1, keepdims=True)
+        oracle.step5(p.A, V3, c0, c1)
+        dt = time.perf_counter() - t0
+        if rep >= warmup:
+            times.append(dt)
+    # algorithmic flops of the sample (same counting rule as the GPU line; step 2 excluded, step 4 not sampled)
+    flops = ncols * (2.0 * N * M + (2 * c.iters - 1) * 2.0 * N * N) + ncols * 2.0 * N * N
+    desc = (f"config {cfg_index} (N={N}): slice {s}'s {M}x{M} Jacobi eigensolve + {c.iters} folded-spectrum "
+            f"iterations and Rayleigh quotients for {ncols} of its {m} eigenvectors (steps O2,O3,O5; O4 not sampled)")
+    return times, flops, desc, oracle.num_threads()
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    k = args.config
+    import pfsm_inputs as gen
+    c = gen.CONFIGS[k]
+    times, flops, desc, threads = oracle_sample(k, args.ref_cols, args.steps, args.warmup)
+    total = sum(times)
+    value = flops * len(times) / total * 1e-12
+    line = {
+        "impl": "reference",
+        "metric": "PFSM solve sustained FP64 TFLOP/s (algorithmic flops / solve time)",
+        "value": value, "unit": "TFLOP/s", "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": 1e3 * total / len(times), "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": workload_config(c, args.gpus),
+        "cpu_baseline": {"value": value, "unit": "TFLOP/s", "cores": threads, "kind": "oracle", "sample": desc},
+        "e2e": {"value": value, "unit": "TFLOP/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+    return 0
+
+
+def workload_config(c, n_gpus: int) -> dict:
+    return {"workload": f"BASELINE.json configs[{c.index}]: {c.name}, synthetic A = D + E",
+            "N": c.N, "P": c.P, "window": c.window, "M": c.M, "iters": c.iters,
+            "alpha": "0.5/max|d|^2", "replicas": n_gpus, "parallelism": f"replicas x{n_gpus}",
+            "l2_policy": f"inputs larger than L2 (A, V, W are {8 * c.N * c.N / 2**20:.0f} MiB each vs 126 MB L2)"
+            if 8 * c.N * c.N > 126e6 else "L2 flushed between timed iterations (256 MiB write)"}
+
+
+def run_ours(args):
+    import numpy as np
+    import torch
+
+    import paper_1502_07806_b200 as pfsm
+    import pfsm_inputs as gen
+    from paper_1502_07806_b200 import replicas
+
+    world, rank, local_rank = replicas.env_world()
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the PFSM path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    replicas.init("nccl", world, rank, torch.device("cuda", local_rank))
+    n_gpus = world
+
+    k = args.config
+    # replicas only: rank r solves an independent matrix of the same config
+    prob = gen.problem(k, seed_offset=replicas.replica_seed_offset(rank))
+    c = prob.cfg
+    N = c.N
+    flops = algorithmic_flops(N, c.M, c.iters)
+    h = pfsm.Handle(N, c.P, c.window, c.iters, prob.alpha)
+    stream = torch.cuda.current_stream()
+    A_host = torch.from_numpy(prob.A).pin_memory()
+    V_host = torch.empty((N, N), dtype=torch.float64).pin_memory()
+    lam_host = torch.empty((N,), dtype=torch.float64).pin_memory()
+    dA = A_host.cuda()
+    dV = torch.empty((N, N), dtype=torch.float64, device="cuda")
+    dl = torch.empty((N,), dtype=torch.float64, device="cuda")
+    flush = None
+    if 8 * N * N <= 126e6:
+        flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+
+    def barrier():
+        torch.cuda.synchronize()
+        replicas.barrier(world)
+        torch.cuda.synchronize()
+
+    def max_over_ranks(x: float) -> float:
+        return replicas.max_over_ranks(x, world, "cuda")
+
+    # ---- device-resident leg: K solves, CUDA events on the launching stream ----
+    for _ in range(args.warmup):
+        h.solve(dA, dV, dl)
+    barrier()
+    assert replicas.all_ok(h.info() == 0, world, "cuda"), "PFSM reported a numerical breakdown on a bench matrix"
+    h.enable_step_timing(True)
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    time.sleep(0.3)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    step_ms = np.zeros(4)
+    barrier()
+    t_wall0 = time.time()
+    for i in range(args.steps):
+        if flush is not None:
+            flush.fill_(i & 0xFF)
+        ev[i][0].record(stream)
+        h.solve(dA, dV, dl)
+        ev[i][1].record(stream)
+        if flush is not None or True:
+            # per-step device times are read back after each solve (events are already recorded; this sync
+            # sits outside the [start, stop] event pair of the step)
+            ev[i][1].synchronize()
+            step_ms += np.array(h.step_ms())
+    barrier()
+    t_wall1 = time.time()
+    clocks = sampler.stop(t_wall0, t_wall1)
+    h.enable_step_timing(False)
+    solve_ms = [a.elapsed_time(b) for a, b in ev]
+    total_ms = max_over_ranks(float(sum(solve_ms)))
+    ms_per_step = total_ms / args.steps
+    step_ms /= args.steps
+    value = replicas.aggregate_tflops(flops["total"], args.steps, world, total_ms)
+
+    # ---- end-to-end leg: host buffers through pfsm_solve_host, copies inside the timed region ----
+    e2e_steps = max(1, min(args.steps, 3))
+    h.solve_host(A_host, V_host, lam_host)
+    barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(e2e_steps):
+        h.solve_host(A_host, V_host, lam_host)
+    e1.record(stream)
+    barrier()
+    e2e_ms = max_over_ranks(e0.elapsed_time(e1)) / e2e_steps
+    e2e_value = replicas.aggregate_tflops(flops["total"], 1, world, e2e_ms)
+    lam = lam_host.numpy().copy()
+    Vh = V_host.numpy()
+
+    # ---- quality numbers of the result (BASELINE metric: "max residual/orthogonality") ----
+    resid = h.residuals().cpu().numpy()
+    dVt = torch.from_numpy(Vh).cuda()
+    orth = float((dVt @ dVt.T - torch.eye(N, dtype=torch.float64, device="cuda")).abs().max().item())
+    del dVt
+    quality = {"max_residual": float(resid.max()), "orthogonality_max": orth,
+               "trace_error": float(abs(lam.sum() - np.trace(prob.A))), "info": h.info()}
+
+    if rank != 0:
+        replicas.finalize(world)
+        return 0
+
+    # ---- roofline of the dominant kernel (gemm_tn_kernel in step 3), live CUDA-event times ----
+    peaks = measured_peaks()
+    n_launch3 = 2 * c.iters
+    gemm_ms = step_ms[1] / max(1, n_launch3)
+    achieved = flops["step3"] / max(1, n_launch3) / (gemm_ms * 1e-3) * 1e-12 if n_launch3 else 0.0
+    peak = peaks["bf16_tflops_sustained"] * FP64_NOMINAL_RATIO
+    roofline = {
+        "bound": "tensor", "kernel": "gemm_tn_kernel (step 3, FP64 DMMA)", "achieved": achieved, "peak": peak,
+        "unit": "TFLOP/s", "frac": achieved / peak, "traffic": None,
+        "peak_source": f"{peaks['_source']} bf16_tflops_sustained x nominal FP64:bf16 ratio 45/2250 (of {peaks['_source']})",
+        "avg_launch_ms": gemm_ms, "launches_per_step": n_launch3,
+        "flops_per_launch": flops["step3"] / max(1, n_launch3),
+    }
+    extra = {}
+    if args.calibrate:
+        extra["fp64_dmma_issue_peak_tflops"] = pfsm.probe_fp64_peak(0)
+        extra["fp64_dfma_issue_peak_tflops"] = pfsm.probe_fp64_peak(1)
+        a = torch.randn(8192, 8192, dtype=torch.float64, device="cuda")
+        for _ in range(2):
+            a @ a
+        s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        s0.record()
+        for _ in range(3):
+            a @ a
+        s1.record()
+        torch.cuda.synchronize()
+        extra["cublas_dgemm_8192_tflops"] = 3 * 2 * 8192.0 ** 3 / (s0.elapsed_time(s1) * 1e-3) * 1e-12
+        del a
+        roofline["frac_of_cublas_dgemm"] = achieved / extra["cublas_dgemm_8192_tflops"]
+    if args.syevd:
+        # comparison only, never the product: cuSOLVER dense syevd on the same matrix in the same run
+        torch.linalg.eigh(dA[:256, :256].contiguous())
+        s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        s0.record()
+        w_ex, _ = torch.linalg.eigh(dA)
+        s1.record()
+        torch.cuda.synchronize()
+        extra["cusolver_syevd_ms"] = s0.elapsed_time(s1)
+        extra["max_abs_lambda_minus_syevd"] = float(np.abs(np.sort(lam) - w_ex.cpu().numpy()).max())
+
+    cpu_times, cpu_flops, cpu_desc, threads = oracle_sample(k, args.cpu_cols, 1, 0)
+    cpu_value = cpu_flops / cpu_times[0] * 1e-12
+
+    line = {
+        "metric": "PFSM solve sustained FP64 TFLOP/s (algorithmic flops / solve time)",
+        "value": value, "unit": "TFLOP/s", "n_gpus": n_gpus, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic", "config": workload_config(c, n_gpus),
+        "solve_ms": {"median": float(np.median(solve_ms)), "best": float(min(solve_ms))},
+        "step_ms": {"step2_submatrix_eig": step_ms[0], "step3_folded_spectrum": step_ms[1],
+                    "step4_cholesky_qr": step_ms[2], "step5_rayleigh": step_ms[3]},
+        "algorithmic_flops": flops, "quality": quality, "clocks": clocks,
+        "e2e": {"value": e2e_value, "unit": "TFLOP/s", "ms_per_step": e2e_ms,
+                "h2d_bytes_per_step": 8 * N * N, "d2h_bytes_per_step": 8 * N * N + 8 * N},
+        "gpu_launches": int(args.steps * h.launches_per_solve()),
+        "roofline": roofline,
+        "cpu_baseline": {"value": cpu_value, "unit": "TFLOP/s", "cores": threads, "kind": "oracle",
+                         "sample": cpu_desc, "seconds": cpu_times[0]},
+        "workspace_bytes": h.workspace_bytes(),
+    }
+    line.update(extra)
+    print(json.dumps(line))
+    replicas.finalize(world)
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=4, help="BASELINE.json config index (default 4: N=8192)")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--cpu-cols", type=int, default=24, help="eigenvectors in the cpu_baseline sample")
+    ap.add_argument("--ref-cols", type=int, default=8, help="eigenvectors per step of --impl reference")
+    ap.add_argument("--no-syevd", dest="syevd", action="store_false")
+    ap.add_argument("--no-calibrate", dest="calibrate", action="store_false")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -143,7 +143,7 @@ class Handle:
         _check(getter(self._h, ctypes.byref(ptr)), name)
 
         class _DevBuf:  # zero-copy view of the handle-owned device buffer, cloned into a tensor the caller owns
-            __cuda_array_interface__ = {"shape": (self.N,), "typestr": "<f8", "data": (int(ptr.value), True),
+            __cuda_array_interface__ = {"shape": (self.N,), "typestr": "<f8", "data": (int(ptr.value), False),
                                         "version": 2}
 
         return torch.as_tensor(_DevBuf(), device="cuda").clone()

@@ -198,14 +198,16 @@ jacobi_batched_kernel(const double* __restrict__ A, int64_t N, int32_t M, int32_
 constexpr int CHOL_NB = 128;
 constexpr int CHOL_THREADS = 1024;
 constexpr int CHOL_LDS = CHOL_NB + 1;
-constexpr int CHOL_SMEM = 2 * CHOL_NB * CHOL_LDS * 8;
+constexpr int CHOL_SMEM = (CHOL_NB * CHOL_LDS + CHOL_NB) * 8;  // L below, L^-1 (transposed) above the diagonal
 
 __global__ void __launch_bounds__(CHOL_THREADS, 1)
 chol_diag_kernel(const double* __restrict__ S, double* __restrict__ Lout, int64_t ld, int32_t k0, int32_t nb,
                  double* __restrict__ Dinv, unsigned long long* info) {
     extern __shared__ double sm[];
-    double* a = sm;                        // a[i][c], leading dimension CHOL_LDS
-    double* li = sm + CHOL_NB * CHOL_LDS;  // inverse
+    // a[i][c] (leading dimension CHOL_LDS): c <= i holds L; the strictly upper part holds the strictly
+    // lower part of L^-1 transposed (L^-1[r][c] at a[c][r], r > c); L^-1's diagonal sits in idiag[].
+    double* a = sm;
+    double* idiag = sm + CHOL_NB * CHOL_LDS;
     __shared__ double s_d;
     const int tid = threadIdx.x;
     for (int idx = tid; idx < CHOL_NB * CHOL_NB; idx += CHOL_THREADS) {
@@ -213,7 +215,6 @@ chol_diag_kernel(const double* __restrict__ S, double* __restrict__ Lout, int64_
         double v = 0.0;
         if (i < nb && c < nb && c <= i) v = S[(size_t)(k0 + i) * ld + k0 + c];
         a[i * CHOL_LDS + c] = v;
-        li[i * CHOL_LDS + c] = 0.0;
     }
     __syncthreads();
     // right-looking Cholesky on the lower triangle; thread owns row i = tid & 127, columns c = cg + 8 q
@@ -238,27 +239,33 @@ chol_diag_kernel(const double* __restrict__ S, double* __restrict__ Lout, int64_
         // the next pivot column is complete only after every thread's update
         __syncthreads();
     }
-    // inverse by forward substitution, one thread per column c of L^-1 (rows broadcast across the warp)
+    // inverse by forward substitution, one thread per column c of L^-1: x_r = -(sum_{c<=k<r} L[r][k] x_k) / L[r][r].
+    // L[r][k] is a warp-wide broadcast; x_k = L^-1[k][c] lives at a[c][k] (stride CHOL_LDS across threads).
     if (tid < nb) {
         const int c = tid;
-        li[c * CHOL_LDS + c] = 1.0 / a[c * CHOL_LDS + c];
+        const double xc = 1.0 / a[c * CHOL_LDS + c];
+        idiag[c] = xc;
         for (int r = c + 1; r < nb; ++r) {
-            double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
-            int k = c;
+            double s0 = a[r * CHOL_LDS + c] * xc, s1 = 0.0, s2 = 0.0, s3 = 0.0;
+            int k = c + 1;
             for (; k + 3 < r; k += 4) {
-                s0 = fma(a[r * CHOL_LDS + k], li[k * CHOL_LDS + c], s0);
-                s1 = fma(a[r * CHOL_LDS + k + 1], li[(k + 1) * CHOL_LDS + c], s1);
-                s2 = fma(a[r * CHOL_LDS + k + 2], li[(k + 2) * CHOL_LDS + c], s2);
-                s3 = fma(a[r * CHOL_LDS + k + 3], li[(k + 3) * CHOL_LDS + c], s3);
+                s0 = fma(a[r * CHOL_LDS + k], a[c * CHOL_LDS + k], s0);
+                s1 = fma(a[r * CHOL_LDS + k + 1], a[c * CHOL_LDS + k + 1], s1);
+                s2 = fma(a[r * CHOL_LDS + k + 2], a[c * CHOL_LDS + k + 2], s2);
+                s3 = fma(a[r * CHOL_LDS + k + 3], a[c * CHOL_LDS + k + 3], s3);
             }
-            for (; k < r; ++k) s0 = fma(a[r * CHOL_LDS + k], li[k * CHOL_LDS + c], s0);
-            li[r * CHOL_LDS + c] = -((s0 + s1) + (s2 + s3)) / a[r * CHOL_LDS + r];
+            for (; k < r; ++k) s0 = fma(a[r * CHOL_LDS + k], a[c * CHOL_LDS + k], s0);
+            a[c * CHOL_LDS + r] = -((s0 + s1) + (s2 + s3)) / a[r * CHOL_LDS + r];
         }
+    } else if (tid < CHOL_NB) {
+        idiag[tid] = 0.0;
     }
     __syncthreads();
     for (int idx = tid; idx < CHOL_NB * CHOL_NB; idx += CHOL_THREADS) {
         const int r = idx >> 7, c = idx & 127;
-        Dinv[idx] = li[r * CHOL_LDS + c];
+        double inv = 0.0;
+        if (r < nb && c < nb) inv = (c < r) ? a[c * CHOL_LDS + r] : (c == r ? idiag[c] : 0.0);
+        Dinv[idx] = inv;
         if (r < nb && c < nb) Lout[(size_t)(k0 + r) * ld + k0 + c] = (c <= r) ? a[r * CHOL_LDS + c] : 0.0;
     }
 }

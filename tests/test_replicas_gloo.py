@@ -1,0 +1,69 @@
+"""World-size-2 CPU test (gloo) of the N>1 path's host logic: replicas draw distinct matrices, timings are
+reduced with MAX over ranks, the whole-job value aggregates all ranks' flops, failure on any rank is seen
+by all.  (The GPU kernels themselves are single-GPU: replicas only, no data-path collective.)"""
+import os
+import socket
+import sys
+
+import numpy as np
+import torch.multiprocessing as mp
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _free_port():
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    port = s.getsockname()[1]
+    s.close()
+    return port
+
+
+def _worker(rank, world, port, q):
+    sys.path.insert(0, ROOT)
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), WORLD_SIZE=str(world), RANK=str(rank),
+                      LOCAL_RANK=str(rank))
+    import oracle
+    import pfsm_inputs as gen
+    from paper_1502_07806_b200 import replicas
+    assert replicas.env_world() == (world, rank, rank)
+    replicas.init("gloo", world, rank)
+    p = gen.problem(0, seed_offset=replicas.replica_seed_offset(rank))
+    c = p.cfg
+    # stand-in for the GPU solve on this CPU-only box: the oracle solves this rank's replica
+    r = oracle.pfsm(p.A, c.P, c.window, c.iters, p.alpha)
+    fake_ms = 10.0 * (rank + 1)                      # rank 1 is the slow one
+    replicas.barrier(world)
+    tmax = replicas.max_over_ranks(fake_ms, world)
+    ok_all = replicas.all_ok(r["info"] == 0, world)
+    ok_mixed = replicas.all_ok(rank != 1, world)      # rank 1 "fails": every rank must see it
+    val = replicas.aggregate_tflops(1e12, 1, world, tmax)
+    q.put((rank, float(p.A[0, 1]), float(r["lam"].sum()), tmax, ok_all, ok_mixed, val))
+    replicas.finalize(world)
+
+
+def test_two_rank_replicas_gloo():
+    world = 2
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_worker, args=(r, world, port, q)) for r in range(world)]
+    for p in procs:
+        p.start()
+    res = sorted(q.get(timeout=120) for _ in range(world))
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    (r0, a0, s0, t0, ok0, mixed0, v0), (r1, a1, s1, t1, ok1, mixed1, v1) = res
+    assert (r0, r1) == (0, 1)
+    assert a0 != a1 and s0 != s1                      # independent replicas (different seeds)
+    assert t0 == t1 == 20.0                           # MAX over ranks, identical on every rank
+    assert ok0 and ok1 and not mixed0 and not mixed1
+    assert v0 == v1 and abs(v0 - 2 * 1e12 / 20e-3 * 1e-12) < 1e-9   # both ranks' flops over the slowest time
+
+
+def test_single_rank_is_a_no_op():
+    from paper_1502_07806_b200 import replicas
+    assert replicas.max_over_ranks(3.5, 1) == 3.5
+    assert replicas.all_ok(True, 1) and not replicas.all_ok(False, 1)
+    assert np.isclose(replicas.aggregate_tflops(2e12, 3, 1, 1000.0), 6.0)
