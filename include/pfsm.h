@@ -95,13 +95,27 @@ int pfsm_solve_host(pfsm_handle_t h, const double* A_host, double* V_host, doubl
 int pfsm_solve_partial(pfsm_handle_t h, const double* A, double* V_inout, double* lambda_out, void* stream,
                        int32_t last_step);
 
+/*
+ * Step 4 alone ("Gram-Schmidt orthogonalization"): orthonormalize the N columns of
+ * V_inout (device, N x N) in ascending column order, V <- V R^-1 with V^T V = R^T R.  Resets and sets the
+ * handle's info like pfsm_solve (pivot j counts as not positive when it is <= 1e-12 ||v_j||^2).
+ */
+int pfsm_orthonormalize(pfsm_handle_t h, double* V_inout, void* stream);
+
+/*
+ * Step 5 alone: lambda_out[i] = v_i^T A v_i and the handle's residual buffer r_i = ||A v_i - lambda_i v_i||_2
+ * for the N columns of V (device, N x N, assumed orthonormal; read only).
+ */
+int pfsm_rayleigh(pfsm_handle_t h, const double* A, const double* V, double* lambda_out, void* stream);
+
 /* Release the handle and its workspace (synchronizes the device).  NULL is a no-op returning 0. */
 int pfsm_destroy(pfsm_handle_t h);
 
 /*
  * Numerical status of the last solve; synchronizes `stream` (the stream that solve was enqueued on).
  *   *info = 0        success
- *   1 <= *info <= N  Cholesky pivot *info of V^T V was not positive: the N vectors are numerically
+ *   1 <= *info <= N  Cholesky pivot *info of V^T V was not positive (<= 1e-12 x its original diagonal
+ *                    entry): the N vectors are numerically
  *                    dependent -- the paper's failure mode for a matrix that is not diagonally
  *                    dominant.  Outputs are undefined; use a standard eigensolver
  *                    for this step.

@@ -18,7 +18,7 @@ _lib = None
 CUDA_ERROR_BASE = 1000
 
 EXPORTS = [
-    "pfsm_create", "pfsm_solve", "pfsm_solve_host", "pfsm_solve_partial", "pfsm_destroy", "pfsm_get_info",
+    "pfsm_create", "pfsm_solve", "pfsm_solve_host", "pfsm_solve_partial", "pfsm_orthonormalize", "pfsm_rayleigh", "pfsm_destroy", "pfsm_get_info",
     "pfsm_get_residuals", "pfsm_get_shifts", "pfsm_set_alpha", "pfsm_workspace_bytes",
     "pfsm_launches_per_solve", "pfsm_enable_step_timing", "pfsm_get_step_ms", "pfsm_probe_fp64_peak",
     "pfsm_strerror",
@@ -50,6 +50,8 @@ def load(build_if_missing: bool = True):
     lib.pfsm_solve.argtypes = [p, p, p, p, p]
     lib.pfsm_solve_host.argtypes = [p, p, p, p, p]
     lib.pfsm_solve_partial.argtypes = [p, p, p, p, p, i32]
+    lib.pfsm_orthonormalize.argtypes = [p, p, p]
+    lib.pfsm_rayleigh.argtypes = [p, p, p, p, p]
     lib.pfsm_destroy.argtypes = [p]
     lib.pfsm_get_info.argtypes = [p, p, ctypes.POINTER(i64)]
     lib.pfsm_get_residuals.argtypes = [p, ctypes.POINTER(p)]
@@ -125,6 +127,16 @@ class Handle:
         lp = _dev_ptr(lam, N, (N,), "lambda") if lam is not None else None
         _check(self._lib.pfsm_solve_partial(self._h, _dev_ptr(A, N, (N, N), "A"), _dev_ptr(Vr, N, (N, N), "V"),
                                             lp, _stream_ptr(stream), last_step), "pfsm_solve_partial")
+
+    def orthonormalize(self, Vr, stream=None):
+        N = self.N
+        _check(self._lib.pfsm_orthonormalize(self._h, _dev_ptr(Vr, N, (N, N), "V"), _stream_ptr(stream)),
+               "pfsm_orthonormalize")
+
+    def rayleigh(self, A, Vr, lam, stream=None):
+        N = self.N
+        _check(self._lib.pfsm_rayleigh(self._h, _dev_ptr(A, N, (N, N), "A"), _dev_ptr(Vr, N, (N, N), "V"),
+                                       _dev_ptr(lam, N, (N,), "lambda"), _stream_ptr(stream)), "pfsm_rayleigh")
 
     def solve_host(self, A_host, Vr_host, lam_host, stream=None):
         N = self.N

@@ -200,9 +200,20 @@ constexpr int CHOL_THREADS = 1024;
 constexpr int CHOL_LDS = CHOL_NB + 1;
 constexpr int CHOL_SMEM = (CHOL_NB * CHOL_LDS + CHOL_NB) * 8;  // L below, L^-1 (transposed) above the diagonal
 
+// diag(G) before the factorization: the breakdown test compares each pivot with its original diagonal entry
+__global__ void extract_diag_kernel(const double* __restrict__ S, int64_t ld, int32_t n, double* __restrict__ gdiag) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) gdiag[i] = S[(size_t)i * ld + i];
+}
+
+// A pivot counts as "not positive" when it is <= CHOL_BREAKDOWN * (its original diagonal entry ||v_j||^2):
+// below that the projected vector has lost 6 digits to its predecessors and single-pass Cholesky-QR
+// (orthogonality error ~ eps * cond(V)^2) can no longer deliver orthonormal vectors.
+constexpr double CHOL_BREAKDOWN = 1e-12;
+
 __global__ void __launch_bounds__(CHOL_THREADS, 1)
 chol_diag_kernel(const double* __restrict__ S, double* __restrict__ Lout, int64_t ld, int32_t k0, int32_t nb,
-                 double* __restrict__ Dinv, unsigned long long* info) {
+                 double* __restrict__ Dinv, const double* __restrict__ gdiag, unsigned long long* info) {
     extern __shared__ double sm[];
     // a[i][c] (leading dimension CHOL_LDS): c <= i holds L; the strictly upper part holds the strictly
     // lower part of L^-1 transposed (L^-1[r][c] at a[c][r], r > c); L^-1's diagonal sits in idiag[].
@@ -222,7 +233,7 @@ chol_diag_kernel(const double* __restrict__ S, double* __restrict__ Lout, int64_
     for (int j = 0; j < nb; ++j) {
         if (tid == 0) {
             double piv = a[j * CHOL_LDS + j];
-            if (!(piv > 0.0)) {
+            if (!(piv > CHOL_BREAKDOWN * gdiag[k0 + j]) || !(piv > 0.0)) {
                 atomicMin(info, (unsigned long long)(k0 + j + 1));
                 piv = 1.0;
             }

@@ -72,6 +72,7 @@ struct pfsm_ctx {
     double* Gws = nullptr;    // P x M x M : Jacobi workspace
     double* eps = nullptr;    // N shifts
     double* resid = nullptr;  // N residual norms
+    double* gdiag = nullptr;  // N: diag(V^T V) before the factorization (breakdown threshold)
     int32_t* slice_tab = nullptr;  // g0[P], lo[P], off[P]
     int2* krange = nullptr;        // per 128-row tile k-range of the first product
     unsigned long long* info = nullptr;
@@ -158,6 +159,7 @@ int pfsm_create(pfsm_handle_t* out, int64_t N, int32_t P, int32_t window, int32_
     TRY(dev_alloc(h, (void**)&h->Gws, (size_t)P * M * M * sizeof(double)));
     TRY(dev_alloc(h, (void**)&h->eps, N * sizeof(double)));
     TRY(dev_alloc(h, (void**)&h->resid, N * sizeof(double)));
+    TRY(dev_alloc(h, (void**)&h->gdiag, N * sizeof(double)));
     TRY(dev_alloc(h, (void**)&h->slice_tab, 3 * (size_t)P * sizeof(int32_t)));
     const int32_t ntr = (int32_t)((N + BM - 1) / BM);
     TRY(dev_alloc(h, (void**)&h->krange, (size_t)ntr * sizeof(int2)));
@@ -203,7 +205,7 @@ int pfsm_create(pfsm_handle_t* out, int64_t N, int32_t P, int32_t window, int32_
 int pfsm_destroy(pfsm_handle_t h) {
     if (!h) return 0;
     cudaDeviceSynchronize();
-    void* ptrs[] = {h->W, h->S, h->O, h->Dinv, h->Gws, h->eps, h->resid, h->slice_tab, h->krange, h->info,
+    void* ptrs[] = {h->W, h->S, h->O, h->Dinv, h->Gws, h->eps, h->resid, h->gdiag, h->slice_tab, h->krange, h->info,
                     h->A_stage, h->V_stage, h->lam_stage};
     for (void* p : ptrs)
         if (p) cudaFree(p);
@@ -223,6 +225,66 @@ static int launch_jacobi(pfsm_ctx* h, const double* A, double* V, cudaStream_t s
     else
         jacobi_batched_kernel<16><<<h->P, JACOBI_THREADS, dyn, st>>>(A, h->N, h->M, h->m, tab, h->Gws, V, h->eps, h->info);
     PFSM_CUDA(cudaGetLastError());
+    return 0;
+}
+
+// ---- step 4: Cholesky-QR on the stacked matrix [G ; V^T], G = V^T V (row-major view: V V^T) ----
+static int run_step4(pfsm_ctx* h, const CUtensorMap& mapV, double* V, cudaStream_t st) {
+    const int64_t N = h->N;
+    const int32_t n = (int32_t)N;
+    int rc;
+    {
+        const dim3 tb(32, 8), tg((unsigned)((N + 31) / 32), (unsigned)((N + 31) / 32));
+        transpose_kernel<<<tg, tb, 0, st>>>(V, N, h->S + (size_t)N * N, N, n, n);
+        PFSM_CUDA(cudaGetLastError());
+        GemmParams p = base_params();
+        p.C = h->S; p.ldc = N; p.mr = n; p.nc = n; p.klen = n; p.lower = 1;
+        if ((rc = launch_gemm<EPI_PLAIN>(mapV, mapV, p, st))) return rc;
+        extract_diag_kernel<<<(unsigned)((N + 255) / 256), 256, 0, st>>>(h->S, N, n, h->gdiag);
+        PFSM_CUDA(cudaGetLastError());
+        static bool chol_attr = false;
+        if (!chol_attr) {
+            PFSM_CUDA(cudaFuncSetAttribute(chol_diag_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, CHOL_SMEM));
+            chol_attr = true;
+        }
+        for (int32_t k = 0; k < h->nblk; ++k) {
+            const int32_t k0 = k * CHOL_NB, nb = (int32_t)std::min<int64_t>(CHOL_NB, N - k0);
+            chol_diag_kernel<<<1, CHOL_THREADS, CHOL_SMEM, st>>>(h->S, h->O, N, k0, nb,
+                                                                 h->Dinv + (size_t)k * CHOL_NB * CHOL_NB, h->gdiag, h->info);
+            PFSM_CUDA(cudaGetLastError());
+            // panel: O[r, k0:k0+nb] = S[r, k0:k0+nb] L_kk^-T   for all rows below the diagonal block
+            GemmParams pp = base_params();
+            pp.C = h->O; pp.ldc = N; pp.cr0 = k0 + nb; pp.cc0 = k0; pp.mr = 2 * n - k0 - nb; pp.nc = nb;
+            pp.xr0 = k0 + nb; pp.xk0 = k0; pp.yr0 = k * CHOL_NB; pp.yk0 = 0; pp.klen = nb;
+            if ((rc = launch_gemm<EPI_PLAIN>(h->mapS, h->mapD, pp, st))) return rc;
+            // trailing update: S[r, c] -= O[r, k0:k0+nb] . O[c, k0:k0+nb]   (tiles with r >= c)
+            if (k0 + nb < n) {
+                GemmParams pt = base_params();
+                pt.C = h->S; pt.ldc = N; pt.cr0 = k0 + nb; pt.cc0 = k0 + nb; pt.mr = 2 * n - k0 - nb;
+                pt.nc = n - k0 - nb; pt.xr0 = k0 + nb; pt.yr0 = k0 + nb; pt.xk0 = k0; pt.yk0 = k0; pt.klen = nb;
+                pt.lower = 1;
+                if ((rc = launch_gemm<EPI_SUB>(h->mapO, h->mapO, pt, st))) return rc;
+            }
+        }
+        transpose_kernel<<<tg, tb, 0, st>>>(h->O + (size_t)N * N, N, V, N, n, n);
+        PFSM_CUDA(cudaGetLastError());
+    }
+    return 0;
+}
+
+// ---- step 5 (reading R11): T = V A, Rayleigh quotients and residual norms ----
+static int run_step5(pfsm_ctx* h, const CUtensorMap& mapV, const CUtensorMap& mapA, double* V, double* lambda_out,
+                     cudaStream_t st) {
+    const int64_t N = h->N;
+    const int32_t n = (int32_t)N;
+    int rc;
+    {
+        GemmParams p = base_params();
+        p.C = h->W; p.ldc = N; p.mr = n; p.nc = n; p.klen = n;
+        if ((rc = launch_gemm<EPI_PLAIN>(mapV, mapA, p, st))) return rc;
+        rayleigh_kernel<<<(unsigned)N, RAY_THREADS, 0, st>>>(V, h->W, N, lambda_out, h->resid);
+        PFSM_CUDA(cudaGetLastError());
+    }
     return 0;
 }
 
@@ -266,57 +328,41 @@ int pfsm_solve_partial(pfsm_handle_t h, const double* A, double* V, double* lamb
     if (tm) PFSM_CUDA(cudaEventRecord(h->ev[2], st));
     if (last_step == 3) return 0;
 
-    // ---- step 4: Cholesky-QR on the stacked matrix [G ; V^T],  G = V^T V (row-major view: V V^T) ----
-    {
-        const dim3 tb(32, 8), tg((unsigned)((N + 31) / 32), (unsigned)((N + 31) / 32));
-        transpose_kernel<<<tg, tb, 0, st>>>(V, N, h->S + (size_t)N * N, N, n, n);
-        PFSM_CUDA(cudaGetLastError());
-        GemmParams p = base_params();
-        p.C = h->S; p.ldc = N; p.mr = n; p.nc = n; p.klen = n; p.lower = 1;
-        if ((rc = launch_gemm<EPI_PLAIN>(mapV, mapV, p, st))) return rc;
-        static bool chol_attr = false;
-        if (!chol_attr) {
-            PFSM_CUDA(cudaFuncSetAttribute(chol_diag_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, CHOL_SMEM));
-            chol_attr = true;
-        }
-        for (int32_t k = 0; k < h->nblk; ++k) {
-            const int32_t k0 = k * CHOL_NB, nb = (int32_t)std::min<int64_t>(CHOL_NB, N - k0);
-            chol_diag_kernel<<<1, CHOL_THREADS, CHOL_SMEM, st>>>(h->S, h->O, N, k0, nb,
-                                                                 h->Dinv + (size_t)k * CHOL_NB * CHOL_NB, h->info);
-            PFSM_CUDA(cudaGetLastError());
-            // panel: O[r, k0:k0+nb] = S[r, k0:k0+nb] L_kk^-T   for all rows below the diagonal block
-            GemmParams pp = base_params();
-            pp.C = h->O; pp.ldc = N; pp.cr0 = k0 + nb; pp.cc0 = k0; pp.mr = 2 * n - k0 - nb; pp.nc = nb;
-            pp.xr0 = k0 + nb; pp.xk0 = k0; pp.yr0 = k * CHOL_NB; pp.yk0 = 0; pp.klen = nb;
-            if ((rc = launch_gemm<EPI_PLAIN>(h->mapS, h->mapD, pp, st))) return rc;
-            // trailing update: S[r, c] -= O[r, k0:k0+nb] . O[c, k0:k0+nb]   (tiles with r >= c)
-            if (k0 + nb < n) {
-                GemmParams pt = base_params();
-                pt.C = h->S; pt.ldc = N; pt.cr0 = k0 + nb; pt.cc0 = k0 + nb; pt.mr = 2 * n - k0 - nb;
-                pt.nc = n - k0 - nb; pt.xr0 = k0 + nb; pt.yr0 = k0 + nb; pt.xk0 = k0; pt.yk0 = k0; pt.klen = nb;
-                pt.lower = 1;
-                if ((rc = launch_gemm<EPI_SUB>(h->mapO, h->mapO, pt, st))) return rc;
-            }
-        }
-        transpose_kernel<<<tg, tb, 0, st>>>(h->O + (size_t)N * N, N, V, N, n, n);
-        PFSM_CUDA(cudaGetLastError());
-    }
+    if ((rc = run_step4(h, mapV, V, st))) return rc;
     if (tm) PFSM_CUDA(cudaEventRecord(h->ev[3], st));
     if (last_step == 4) return 0;
 
-    // ---- step 5: T = V A, Rayleigh quotients and residual norms ----
-    {
-        GemmParams p = base_params();
-        p.C = h->W; p.ldc = N; p.mr = n; p.nc = n; p.klen = n;
-        if ((rc = launch_gemm<EPI_PLAIN>(mapV, mapA, p, st))) return rc;
-        rayleigh_kernel<<<(unsigned)N, RAY_THREADS, 0, st>>>(V, h->W, N, lambda_out, h->resid);
-        PFSM_CUDA(cudaGetLastError());
-    }
+    if ((rc = run_step5(h, mapV, mapA, V, lambda_out, st))) return rc;
     if (tm) {
         PFSM_CUDA(cudaEventRecord(h->ev[4], st));
         h->ev_valid = true;
     }
     return 0;
+}
+
+int pfsm_orthonormalize(pfsm_handle_t h, double* V_inout, void* stream) {
+    if (!h) return -1;
+    if (!V_inout || ((uintptr_t)V_inout & 15)) return -2;
+    CUtensorMap mapV;
+    int rc;
+    if ((rc = make_map(&mapV, V_inout, h->N, h->N, h->N))) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    h->ev_valid = false;
+    PFSM_CUDA(cudaMemsetAsync(h->info, 0xFF, sizeof(unsigned long long), st));
+    return run_step4(h, mapV, V_inout, st);
+}
+
+int pfsm_rayleigh(pfsm_handle_t h, const double* A, const double* V, double* lambda_out, void* stream) {
+    if (!h) return -1;
+    if (!A || ((uintptr_t)A & 15)) return -2;
+    if (!V || ((uintptr_t)V & 15)) return -3;
+    if (!lambda_out || ((uintptr_t)lambda_out & 7)) return -4;
+    CUtensorMap mapA, mapV;
+    int rc;
+    if ((rc = make_map(&mapA, A, h->N, h->N, h->N))) return rc;
+    if ((rc = make_map(&mapV, V, h->N, h->N, h->N))) return rc;
+    h->ev_valid = false;
+    return run_step5(h, mapV, mapA, const_cast<double*>(V), lambda_out, (cudaStream_t)stream);
 }
 
 int pfsm_solve(pfsm_handle_t h, const double* A, double* V_inout, double* lambda_out, void* stream) {
@@ -379,8 +425,8 @@ size_t pfsm_workspace_bytes(pfsm_handle_t h) { return h ? h->bytes : 0; }
 
 int64_t pfsm_launches_per_solve(pfsm_handle_t h) {
     if (!h) return 0;
-    // jacobi + 2 iters GEMMs + (2 transposes + Gram + per panel: diag, panel, trailing (none after the last)) + GEMM + rayleigh
-    return 1 + 2 * (int64_t)h->iters + (2 + 1 + 3 * (int64_t)h->nblk - 1) + 2;
+    // jacobi + 2 iters GEMMs + (2 transposes + Gram + diag extract + per panel: diag, panel, trailing (none after the last)) + GEMM + rayleigh
+    return 1 + 2 * (int64_t)h->iters + (2 + 1 + 1 + 3 * (int64_t)h->nblk - 1) + 2;
 }
 
 int pfsm_enable_step_timing(pfsm_handle_t h, int32_t enable) {

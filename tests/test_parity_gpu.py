@@ -168,21 +168,54 @@ def test_breakdown_is_flagged_for_dependent_vectors():
     assert g["info"] != 0 or g["resid"].max() > 100 * gg["resid"].max()
 
 
-def test_singular_gram_sets_info():
-    # an all-zero matrix has B_s = 0 for every slice: overlapping windows then yield duplicated unit
-    # vectors?  No: each slice takes distinct local indices of the identity, so vectors stay independent.
-    # Force dependence instead with a rank-deficient coupling: two identical decoupled 2x2 blocks share
-    # eigenvectors only if windows overlap fully -- use window >= N so every slice sees all of A, with an
-    # exactly degenerate spectrum; ranks tie -> stable order -> still independent.  So check the flag
-    # through the Cholesky directly: alpha so large that one iteration annihilates a direction.
-    N = 128
-    d = np.linspace(-1.0, 1.0, N)
-    A = np.diag(d)
-    A[0, 1] = A[1, 0] = 0.3
-    # alpha = 1/(lambda-eps)^2 kills the component along the neighbouring eigenvector exactly; with a tiny
-    # window (M = m, no halo) the start vectors of slice 0 and 1 are unit vectors, not eigenvectors
-    g = gpu_solve(A, 64, 0, 1, 1e6)
-    assert g["info"] != 0 or not np.isfinite(g["lam"]).all() or g["resid"].max() > 1e-3
+@pytest.mark.parametrize("N", [64, 200, 258, 384])
+def test_step4_alone_matches_gram_schmidt(N):
+    # step 4 on arbitrary (well-conditioned) vectors: Cholesky-QR == modified Gram-Schmidt (uniqueness of
+    # thin QR with positive diagonal R, reading R10 / pin P11)
+    X = gen.normal(17, gen.STREAM_TEST, 0, N * N).reshape(N, N) + 4 * np.sqrt(N) * np.eye(N)
+    h = pfsm.Handle(N, 1, 0, 0, 1.0)
+    dV = dev(X)
+    h.orthonormalize(dV)
+    assert h.info() == 0
+    Vo, info = oracle.step4_mgs(X)
+    assert info == 0
+    Vg = dV.cpu().numpy()
+    assert np.abs(Vg - Vo).max() < 1e-12
+    assert np.abs(Vg @ Vg.T - np.eye(N)).max() <= 1e-12 * N
+    h.destroy()
+
+
+def test_step4_flags_dependent_vectors():
+    # P12: a duplicated vector makes V^T V singular: both sides must flag it, at the second copy
+    N = 256
+    X = gen.normal(18, gen.STREAM_TEST, 0, N * N).reshape(N, N) + 4 * np.sqrt(N) * np.eye(N)
+    X[200] = X[131]
+    _, info_o = oracle.step4_mgs(X)
+    h = pfsm.Handle(N, 1, 0, 0, 1.0)
+    dV = dev(X)
+    h.orthonormalize(dV)
+    assert info_o == 201
+    assert h.info() == 201
+    # and the flag is cleared by the next healthy call
+    X[200] = gen.normal(19, gen.STREAM_TEST, 0, N)
+    dV = dev(X)
+    h.orthonormalize(dV)
+    assert h.info() == 0
+    h.destroy()
+
+
+def test_step5_alone_matches_definition():
+    N = 320
+    p = gen.small_problem(N, 0.05, 10.0, seed=33)
+    X = gen.normal(19, gen.STREAM_TEST, 0, N * N).reshape(N, N)
+    X /= np.linalg.norm(X, axis=1, keepdims=True)
+    h = pfsm.Handle(N, 1, 0, 0, 1.0)
+    dl = torch.empty(N, dtype=torch.float64, device="cuda")
+    h.rayleigh(dev(p.A), dev(X), dl)
+    lam_o, res_o = oracle.step5(p.A, X)
+    assert np.abs(dl.cpu().numpy() - lam_o).max() < 1e-13
+    assert np.abs(h.residuals().cpu().numpy() - res_o).max() < 1e-13
+    h.destroy()
 
 
 def test_solve_is_deterministic_and_ignores_v_input():
