@@ -24,6 +24,9 @@ if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
 FP64_NOMINAL_RATIO = 45.0 / 2250.0  # guide's nominal B200 FP64-tensor : bf16-tensor dense peaks
+# dram__bytes_read.sum + dram__bytes_write.sum per full-k gemm_tn_kernel launch, from the committed
+# `ncu --set full` capture profiles/r01_ncu_full_gemm_jacobi.md (config index -> bytes); None = not captured
+NCU_TRAFFIC_PER_GEMM_LAUNCH = {4: 7.54e9 + 0.53e9}
 
 
 def algorithmic_flops(N: int, M: int, iters: int) -> dict:
@@ -281,7 +284,8 @@ def run_ours(args):
     peak = peaks["bf16_tflops_sustained"] * FP64_NOMINAL_RATIO
     roofline = {
         "bound": "tensor", "kernel": "gemm_tn_kernel (step 3, FP64 DMMA)", "achieved": achieved, "peak": peak,
-        "unit": "TFLOP/s", "frac": achieved / peak, "traffic": None,
+        "unit": "TFLOP/s", "frac": achieved / peak, "traffic": NCU_TRAFFIC_PER_GEMM_LAUNCH.get(k),
+        "algorithmic_bytes_per_launch": 32.0 * N * N,
         "peak_source": f"{peaks['_source']} bf16_tflops_sustained x nominal FP64:bf16 ratio 45/2250 (of {peaks['_source']})",
         "avg_launch_ms": gemm_ms, "launches_per_step": n_launch3,
         "flops_per_launch": flops["step3"] / max(1, n_launch3),
