@@ -42,25 +42,47 @@ __device__ __forceinline__ double warp_sum(double v) {
 //   eps[g0 + j] = mu;  V[(g0 + j) * N + lo + r] = y[r]   (V was zero-filled before the launch).
 // info: atomicMin-style first failure N + s + 1 if the sweep cap is hit.
 // ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t cluster_ctarank() {
+    uint32_t r;
+    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+    return r;
+}
+__device__ __forceinline__ uint32_t cluster_nctarank() {
+    uint32_t r;
+    asm volatile("mov.u32 %0, %%cluster_nctarank;" : "=r"(r));
+    return r;
+}
+// barrier over all threads of the cluster's CTAs; release/acquire orders their global-memory accesses
+__device__ __forceinline__ void cluster_sync_all() {
+    asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+
+// A slice is worked on by a thread-block CLUSTER of CS = 1, 2, 4 or 8 CTAs (launch attribute): the column
+// pairs of a tournament round are dealt round-robin to the CS x 32 warps, G stays in L2 (loads bypass L1 with
+// ld.global.cg because another SM may have written the column), and the round barrier is the cluster barrier.
+// The kernel is bound by L2 bandwidth (every round streams G once), so CS SMs per slice give CS x the L2 ports.
 template <int EPL>
 __global__ void __launch_bounds__(JACOBI_THREADS, 1)
 jacobi_batched_kernel(const double* __restrict__ A, int64_t N, int32_t M, int32_t m, SliceTable tab,
                       double* __restrict__ Gws, double* __restrict__ V, double* __restrict__ eps,
-                      unsigned long long* info) {
-    const int s = blockIdx.x;
+                      int* __restrict__ rotcnt, unsigned long long* info) {
+    const int CS = (int)cluster_nctarank(), cr = (int)cluster_ctarank();
+    const int s = blockIdx.x / CS;
     const int lo = tab.lo[s], off = tab.off[s], g0 = tab.g0[s];
     double* G = Gws + (size_t)s * M * M;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     constexpr int NW = JACOBI_THREADS / 32;
+    const int gw = cr * NW + warp, TW = CS * NW;  // warp index / warp count within the cluster
+    int* rot = rotcnt + (size_t)s * JACOBI_MAX_SWEEPS;
 
     __shared__ double red[NW];
     __shared__ double s_sigma;
-    __shared__ int s_rot;
     extern __shared__ double dyn[];  // nrm[M] then rank (int) [M]
     double* nrm = dyn;
     int* rank = reinterpret_cast<int*>(dyn + M);
 
-    // Gershgorin bound: max_r sum_c |B[r][c]|  (thread per row; consecutive rows are contiguous)
+    // Gershgorin bound: max_r sum_c |B[r][c]|  (thread per row; consecutive rows are contiguous).
+    // Every CTA of the cluster computes it (same order -> same sigma).
     double bound = 0.0;
     for (int r = tid; r < M; r += JACOBI_THREADS) {
         double sum = 0.0;
@@ -78,24 +100,22 @@ jacobi_batched_kernel(const double* __restrict__ A, int64_t N, int32_t M, int32_
     }
     __syncthreads();
     const double sigma = s_sigma;
-    for (int idx = tid; idx < M * M; idx += JACOBI_THREADS) {
+    for (int idx = cr * JACOBI_THREADS + tid; idx < M * M; idx += CS * JACOBI_THREADS) {
         const int c = idx / M, r = idx - c * M;
         double v = A[(size_t)(lo + c) * N + lo + r];
         if (r == c) v += sigma;
         G[idx] = v;
     }
-    __syncthreads();
+    cluster_sync_all();
 
     const int Me = M + (M & 1);  // phantom column when M is odd
     const int n1 = Me - 1, npairs = Me / 2;
     const double tol = 2.220446049250313e-16 * sqrt((double)M);
     bool converged = false;
     for (int sweep = 0; sweep < JACOBI_MAX_SWEEPS; ++sweep) {
-        if (tid == 0) s_rot = 0;
-        __syncthreads();
         int nrot = 0;
         for (int rnd = 0; rnd < n1; ++rnd) {
-            for (int pi = warp; pi < npairs; pi += NW) {
+            for (int pi = gw; pi < npairs; pi += TW) {
                 int p, q;
                 if (pi == 0) {
                     p = n1;
@@ -119,8 +139,8 @@ jacobi_batched_kernel(const double* __restrict__ A, int64_t N, int32_t M, int32_
 #pragma unroll
                 for (int e = 0; e < EPL; ++e) {
                     const int r = lane + 32 * e;
-                    x[e] = (r < M) ? gp[r] : 0.0;
-                    y[e] = (r < M) ? gq[r] : 0.0;
+                    x[e] = (r < M) ? __ldcg(gp + r) : 0.0;
+                    y[e] = (r < M) ? __ldcg(gq + r) : 0.0;
                     aa = fma(x[e], x[e], aa);
                     bb = fma(y[e], y[e], bb);
                     ab = fma(x[e], y[e], ab);
@@ -143,24 +163,25 @@ jacobi_batched_kernel(const double* __restrict__ A, int64_t N, int32_t M, int32_
                     ++nrot;
                 }
             }
-            __syncthreads();
+            if (rnd == n1 - 1 && lane == 0 && nrot) atomicAdd(rot + sweep, nrot);
+            cluster_sync_all();
         }
-        if (lane == 0 && nrot) atomicAdd(&s_rot, nrot);
-        __syncthreads();
-        const int total = s_rot;
-        __syncthreads();
+        const int total = __ldcg(rot + sweep);
         if (total == 0) {
             converged = true;
             break;
         }
     }
-    if (!converged && tid == 0) atomicMin(info, (unsigned long long)(N + s + 1));
+    if (!converged && tid == 0 && cr == 0) atomicMin(info, (unsigned long long)(N + s + 1));
 
     // column norms -> eigenvalues; rank by counting (ties: lower column index first)
     for (int c = warp; c < M; c += NW) {
         const double* gc = G + (size_t)c * M;
         double ss = 0.0;
-        for (int r = lane; r < M; r += 32) ss = fma(gc[r], gc[r], ss);
+        for (int r = lane; r < M; r += 32) {
+            const double g = __ldcg(gc + r);
+            ss = fma(g, g, ss);
+        }
         ss = warp_sum(ss);
         if (lane == 0) nrm[c] = sqrt(ss);
     }
@@ -175,7 +196,7 @@ jacobi_batched_kernel(const double* __restrict__ A, int64_t N, int32_t M, int32_
         rank[c] = rk;
     }
     __syncthreads();
-    for (int c = warp; c < M; c += NW) {
+    for (int c = gw; c < M; c += TW) {
         const int j = rank[c] - off;
         if (j < 0 || j >= m) continue;
         const double nv = nrm[c];
@@ -183,7 +204,7 @@ jacobi_batched_kernel(const double* __restrict__ A, int64_t N, int32_t M, int32_
         const double* gc = G + (size_t)c * M;
         double* v = V + (size_t)(g0 + j) * N + lo;
         // sign convention: largest-magnitude component positive is not needed (R16); keep G's sign
-        for (int r = lane; r < M; r += 32) v[r] = gc[r] * inv;
+        for (int r = lane; r < M; r += 32) v[r] = __ldcg(gc + r) * inv;
         if (lane == 0) eps[g0 + j] = nv - sigma;
     }
 }
@@ -198,7 +219,7 @@ jacobi_batched_kernel(const double* __restrict__ A, int64_t N, int32_t M, int32_
 constexpr int CHOL_NB = 128;
 constexpr int CHOL_THREADS = 1024;
 constexpr int CHOL_LDS = CHOL_NB + 1;
-constexpr int CHOL_SMEM = (CHOL_NB * CHOL_LDS + CHOL_NB) * 8;  // L below, L^-1 (transposed) above the diagonal
+constexpr int CHOL_SMEM = (CHOL_NB * CHOL_LDS + CHOL_NB + 7 * 256) * 8;  // L below, L^-1 (transposed) above the diagonal
 
 // diag(G) before the factorization: the breakdown test compares each pivot with its original diagonal entry
 __global__ void extract_diag_kernel(const double* __restrict__ S, int64_t ld, int32_t n, double* __restrict__ gdiag) {
@@ -211,73 +232,132 @@ __global__ void extract_diag_kernel(const double* __restrict__ S, int64_t ld, in
 // (orthogonality error ~ eps * cond(V)^2) can no longer deliver orthonormal vectors.
 constexpr double CHOL_BREAKDOWN = 1e-12;
 
+// Blocked in 16-wide panels so that only 3 block barriers per panel (24 in all) sit on the serial chain:
+//   A1 warp 0 factors the 16 x 16 diagonal block (lane = row, __syncwarp between columns)
+//   A2 one thread per row below solves its 16 entries against that block
+//   A3 all threads apply the rank-16 update to the trailing lower triangle
+// then L^-1 by 16 x 16 blocks: B1 eight warps invert the diagonal blocks, B2 block row I from block rows < I.
+// Rows/columns >= nb are padded with the identity and masked on output.
+__device__ __forceinline__ double chol_linv(const double* a, const double* idiag, int x, int y) {
+    return x > y ? a[y * CHOL_LDS + x] : (x == y ? idiag[x] : 0.0);  // L^-1[x][y], stored transposed above the diagonal
+}
+
 __global__ void __launch_bounds__(CHOL_THREADS, 1)
 chol_diag_kernel(const double* __restrict__ S, double* __restrict__ Lout, int64_t ld, int32_t k0, int32_t nb,
                  double* __restrict__ Dinv, const double* __restrict__ gdiag, unsigned long long* info) {
     extern __shared__ double sm[];
     // a[i][c] (leading dimension CHOL_LDS): c <= i holds L; the strictly upper part holds the strictly
-    // lower part of L^-1 transposed (L^-1[r][c] at a[c][r], r > c); L^-1's diagonal sits in idiag[].
+    // lower part of L^-1 transposed (L^-1[r][c] at a[c][r], r > c); idiag[c] = 1 / L[c][c] = L^-1[c][c].
     double* a = sm;
     double* idiag = sm + CHOL_NB * CHOL_LDS;
-    __shared__ double s_d;
-    const int tid = threadIdx.x;
+    double* T = idiag + CHOL_NB;  // 7 x 256 scratch of phase B2
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     for (int idx = tid; idx < CHOL_NB * CHOL_NB; idx += CHOL_THREADS) {
         const int i = idx >> 7, c = idx & 127;
-        double v = 0.0;
-        if (i < nb && c < nb && c <= i) v = S[(size_t)(k0 + i) * ld + k0 + c];
+        double v = (i == c) ? 1.0 : 0.0;
+        if (i < nb && c < nb) v = (c <= i) ? S[(size_t)(k0 + i) * ld + k0 + c] : 0.0;
         a[i * CHOL_LDS + c] = v;
     }
     __syncthreads();
-    // right-looking Cholesky on the lower triangle; thread owns row i = tid & 127, columns c = cg + 8 q
-    const int i = tid & 127, cg = tid >> 7;
-    for (int j = 0; j < nb; ++j) {
-        if (tid == 0) {
-            double piv = a[j * CHOL_LDS + j];
-            if (!(piv > CHOL_BREAKDOWN * gdiag[k0 + j]) || !(piv > 0.0)) {
-                atomicMin(info, (unsigned long long)(k0 + j + 1));
-                piv = 1.0;
+
+    // ---------------- phase A: L ----------------
+    for (int j0 = 0; j0 < CHOL_NB; j0 += 16) {
+        if (warp == 0) {
+            const int i = j0 + lane;  // lanes 0..15 own rows j0..j0+15
+            for (int j = 0; j < 16; ++j) {
+                const int jj = j0 + j;
+                double piv = a[jj * CHOL_LDS + jj];
+                if (jj < nb && (!(piv > CHOL_BREAKDOWN * gdiag[k0 + jj]) || !(piv > 0.0))) {
+                    if (lane == 0) atomicMin(info, (unsigned long long)(k0 + jj + 1));
+                    piv = 1.0;
+                }
+                const double d = sqrt(piv), rd = 1.0 / d;
+                __syncwarp();
+                if (lane == j) {
+                    a[jj * CHOL_LDS + jj] = d;
+                    idiag[jj] = rd;
+                } else if (lane > j && lane < 16) {
+                    a[i * CHOL_LDS + jj] *= rd;
+                }
+                __syncwarp();
+                if (lane > j && lane < 16) {
+                    const double lij = a[i * CHOL_LDS + jj];
+                    for (int c = jj + 1; c <= i; ++c) a[i * CHOL_LDS + c] -= lij * a[c * CHOL_LDS + jj];
+                }
+                __syncwarp();
             }
-            s_d = sqrt(piv);
         }
         __syncthreads();
-        const double d = s_d;
-        if (tid < nb && tid >= j) a[tid * CHOL_LDS + j] = (tid == j) ? d : a[tid * CHOL_LDS + j] / d;
-        __syncthreads();
-        if (i > j && i < nb) {
-            const double lij = a[i * CHOL_LDS + j];
-            for (int c = j + 1 + cg; c <= i; c += 8) a[i * CHOL_LDS + c] -= lij * a[c * CHOL_LDS + j];
+        if (j0 + 16 >= CHOL_NB) break;
+        if (tid < CHOL_NB && tid >= j0 + 16) {  // A2: row tid of the panel
+            const int i = tid;
+            double x[16];
+#pragma unroll
+            for (int j = 0; j < 16; ++j) {
+                double s = a[i * CHOL_LDS + j0 + j];
+#pragma unroll
+                for (int k = 0; k < j; ++k) s -= x[k] * a[(j0 + j) * CHOL_LDS + j0 + k];
+                x[j] = s * idiag[j0 + j];
+            }
+#pragma unroll
+            for (int j = 0; j < 16; ++j) a[i * CHOL_LDS + j0 + j] = x[j];
         }
-        // the next pivot column is complete only after every thread's update
+        __syncthreads();
+        {  // A3: a[i][c] -= sum_k l[i][k] l[c][k] on the trailing lower triangle
+            const int i = tid & 127, cg = tid >> 7;
+            if (i >= j0 + 16) {
+                double li[16];
+#pragma unroll
+                for (int k = 0; k < 16; ++k) li[k] = a[i * CHOL_LDS + j0 + k];
+                for (int c = j0 + 16 + cg; c <= i; c += 8) {
+                    double s0 = 0.0, s1 = 0.0;
+#pragma unroll
+                    for (int k = 0; k < 16; k += 2) {
+                        s0 = fma(li[k], a[c * CHOL_LDS + j0 + k], s0);
+                        s1 = fma(li[k + 1], a[c * CHOL_LDS + j0 + k + 1], s1);
+                    }
+                    a[i * CHOL_LDS + c] -= s0 + s1;
+                }
+            }
+        }
         __syncthreads();
     }
-    // inverse by forward substitution, one thread per column c of L^-1: x_r = -(sum_{c<=k<r} L[r][k] x_k) / L[r][r].
-    // L[r][k] is a warp-wide broadcast; x_k = L^-1[k][c] lives at a[c][k] (stride CHOL_LDS across threads).
-    if (tid < nb) {
-        const int c = tid;
-        const double xc = 1.0 / a[c * CHOL_LDS + c];
-        idiag[c] = xc;
-        for (int r = c + 1; r < nb; ++r) {
-            double s0 = a[r * CHOL_LDS + c] * xc, s1 = 0.0, s2 = 0.0, s3 = 0.0;
-            int k = c + 1;
-            for (; k + 3 < r; k += 4) {
-                s0 = fma(a[r * CHOL_LDS + k], a[c * CHOL_LDS + k], s0);
-                s1 = fma(a[r * CHOL_LDS + k + 1], a[c * CHOL_LDS + k + 1], s1);
-                s2 = fma(a[r * CHOL_LDS + k + 2], a[c * CHOL_LDS + k + 2], s2);
-                s3 = fma(a[r * CHOL_LDS + k + 3], a[c * CHOL_LDS + k + 3], s3);
-            }
-            for (; k < r; ++k) s0 = fma(a[r * CHOL_LDS + k], a[c * CHOL_LDS + k], s0);
-            a[c * CHOL_LDS + r] = -((s0 + s1) + (s2 + s3)) / a[r * CHOL_LDS + r];
+
+    // ---------------- phase B: L^-1 ----------------
+    if (warp < 8 && lane < 16) {  // B1: diagonal block `warp`, column `lane` by forward substitution
+        const int b0 = warp * 16, c = lane;
+        for (int r = c + 1; r < 16; ++r) {
+            double s = a[(b0 + r) * CHOL_LDS + b0 + c] * idiag[b0 + c];
+            for (int k = c + 1; k < r; ++k) s = fma(a[(b0 + r) * CHOL_LDS + b0 + k], a[(b0 + c) * CHOL_LDS + b0 + k], s);
+            a[(b0 + c) * CHOL_LDS + b0 + r] = -s * idiag[b0 + r];
         }
-    } else if (tid < CHOL_NB) {
-        idiag[tid] = 0.0;
     }
     __syncthreads();
+    for (int I = 1; I < 8; ++I) {  // B2: L^-1[I][J] = -L^-1[I][I] * sum_{J<=K<I} L[I][K] L^-1[K][J], all J < I at once
+        for (int e = tid; e < I * 256; e += CHOL_THREADS) {
+            const int J = e >> 8, rr = (e >> 4) & 15, cc = e & 15;
+            const double* lrow = a + (16 * I + rr) * CHOL_LDS;
+            double s0 = 0.0, s1 = 0.0;
+            for (int k = 16 * J + cc; k < 16 * I; k += 2) {  // L^-1[k][16J+cc] is zero for k < 16J+cc
+                s0 = fma(lrow[k], chol_linv(a, idiag, k, 16 * J + cc), s0);
+                if (k + 1 < 16 * I) s1 = fma(lrow[k + 1], chol_linv(a, idiag, k + 1, 16 * J + cc), s1);
+            }
+            T[e] = s0 + s1;
+        }
+        __syncthreads();
+        for (int e = tid; e < I * 256; e += CHOL_THREADS) {
+            const int J = e >> 8, rr = (e >> 4) & 15, cc = e & 15;
+            double s = 0.0;
+            for (int k = 0; k <= rr; ++k) s = fma(chol_linv(a, idiag, 16 * I + rr, 16 * I + k), T[J * 256 + k * 16 + cc], s);
+            a[(16 * J + cc) * CHOL_LDS + 16 * I + rr] = -s;
+        }
+        __syncthreads();
+    }
     for (int idx = tid; idx < CHOL_NB * CHOL_NB; idx += CHOL_THREADS) {
         const int r = idx >> 7, c = idx & 127;
-        double inv = 0.0;
-        if (r < nb && c < nb) inv = (c < r) ? a[c * CHOL_LDS + r] : (c == r ? idiag[c] : 0.0);
-        Dinv[idx] = inv;
-        if (r < nb && c < nb) Lout[(size_t)(k0 + r) * ld + k0 + c] = (c <= r) ? a[r * CHOL_LDS + c] : 0.0;
+        const bool in = (r < nb && c < nb);
+        Dinv[idx] = in ? chol_linv(a, idiag, r, c) : 0.0;
+        if (in) Lout[(size_t)(k0 + r) * ld + k0 + c] = (c <= r) ? a[r * CHOL_LDS + c] : 0.0;
     }
 }
 

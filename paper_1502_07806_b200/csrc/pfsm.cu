@@ -72,6 +72,7 @@ struct pfsm_ctx {
     double* Gws = nullptr;    // P x M x M : Jacobi workspace
     double* eps = nullptr;    // N shifts
     double* resid = nullptr;  // N residual norms
+    int* rotcnt = nullptr;    // P x JACOBI_MAX_SWEEPS rotation counters of step 2
     double* gdiag = nullptr;  // N: diag(V^T V) before the factorization (breakdown threshold)
     int32_t* slice_tab = nullptr;  // g0[P], lo[P], off[P]
     int2* krange = nullptr;        // per 128-row tile k-range of the first product
@@ -160,6 +161,7 @@ int pfsm_create(pfsm_handle_t* out, int64_t N, int32_t P, int32_t window, int32_
     TRY(dev_alloc(h, (void**)&h->eps, N * sizeof(double)));
     TRY(dev_alloc(h, (void**)&h->resid, N * sizeof(double)));
     TRY(dev_alloc(h, (void**)&h->gdiag, N * sizeof(double)));
+    TRY(dev_alloc(h, (void**)&h->rotcnt, (size_t)P * JACOBI_MAX_SWEEPS * sizeof(int)));
     TRY(dev_alloc(h, (void**)&h->slice_tab, 3 * (size_t)P * sizeof(int32_t)));
     const int32_t ntr = (int32_t)((N + BM - 1) / BM);
     TRY(dev_alloc(h, (void**)&h->krange, (size_t)ntr * sizeof(int2)));
@@ -205,7 +207,7 @@ int pfsm_create(pfsm_handle_t* out, int64_t N, int32_t P, int32_t window, int32_
 int pfsm_destroy(pfsm_handle_t h) {
     if (!h) return 0;
     cudaDeviceSynchronize();
-    void* ptrs[] = {h->W, h->S, h->O, h->Dinv, h->Gws, h->eps, h->resid, h->gdiag, h->slice_tab, h->krange, h->info,
+    void* ptrs[] = {h->W, h->S, h->O, h->Dinv, h->Gws, h->eps, h->resid, h->gdiag, h->rotcnt, h->slice_tab, h->krange, h->info,
                     h->A_stage, h->V_stage, h->lam_stage};
     for (void* p : ptrs)
         if (p) cudaFree(p);
@@ -215,17 +217,43 @@ int pfsm_destroy(pfsm_handle_t h) {
     return 0;
 }
 
-static int launch_jacobi(pfsm_ctx* h, const double* A, double* V, cudaStream_t st) {
+static int jacobi_cluster_size(const pfsm_ctx* h) {
+    // CTAs per slice: as many as fit the chip (148 SMs / P slices) but no more warps than column pairs
+    const int npairs = (h->M + 1) / 2;
+    int cs = 1;
+    while (cs < 8 && (2 * cs) * h->P <= 148 && cs * (JACOBI_THREADS / 32) < npairs) cs *= 2;
+    return cs;
+}
+
+extern "C++" {
+template <int EPL>
+static int launch_jacobi_t(pfsm_ctx* h, const double* A, double* V, cudaStream_t st) {
     SliceTable tab{h->slice_tab, h->slice_tab + h->P, h->slice_tab + 2 * (size_t)h->P};
-    const size_t dyn = (size_t)h->M * (sizeof(double) + sizeof(int));
-    if (h->M <= 128)
-        jacobi_batched_kernel<4><<<h->P, JACOBI_THREADS, dyn, st>>>(A, h->N, h->M, h->m, tab, h->Gws, V, h->eps, h->info);
-    else if (h->M <= 256)
-        jacobi_batched_kernel<8><<<h->P, JACOBI_THREADS, dyn, st>>>(A, h->N, h->M, h->m, tab, h->Gws, V, h->eps, h->info);
-    else
-        jacobi_batched_kernel<16><<<h->P, JACOBI_THREADS, dyn, st>>>(A, h->N, h->M, h->m, tab, h->Gws, V, h->eps, h->info);
-    PFSM_CUDA(cudaGetLastError());
+    const int cs = jacobi_cluster_size(h);
+    cudaLaunchConfig_t cfg;
+    memset(&cfg, 0, sizeof(cfg));
+    cfg.gridDim = dim3((unsigned)(h->P * cs));
+    cfg.blockDim = dim3(JACOBI_THREADS);
+    cfg.dynamicSmemBytes = (size_t)h->M * (sizeof(double) + sizeof(int));
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = (unsigned)cs;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    PFSM_CUDA(cudaLaunchKernelEx(&cfg, jacobi_batched_kernel<EPL>, A, h->N, h->M, h->m, tab, h->Gws, V, h->eps,
+                                 h->rotcnt, h->info));
     return 0;
+}
+}  // extern "C++"
+
+static int launch_jacobi(pfsm_ctx* h, const double* A, double* V, cudaStream_t st) {
+    PFSM_CUDA(cudaMemsetAsync(h->rotcnt, 0, (size_t)h->P * JACOBI_MAX_SWEEPS * sizeof(int), st));
+    if (h->M <= 128) return launch_jacobi_t<4>(h, A, V, st);
+    if (h->M <= 256) return launch_jacobi_t<8>(h, A, V, st);
+    return launch_jacobi_t<16>(h, A, V, st);
 }
 
 // ---- step 4: Cholesky-QR on the stacked matrix [G ; V^T], G = V^T V (row-major view: V V^T) ----
