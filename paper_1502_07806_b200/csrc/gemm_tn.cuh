@@ -144,7 +144,7 @@ inline int64_t gemm_num_tiles(int32_t ntr, int32_t ntc, int lower) {
 template <int EPI>
 __global__ void __launch_bounds__(GEMM_THREADS, 1)
 gemm_tn_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CUtensorMap mapY,
-               const GemmParams p) {
+               const __grid_constant__ CUtensorMap mapC, const GemmParams p) {
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;  // SWIZZLE_128B needs 1024-B alignment
     const uint32_t bar_base = smem_base + GEMM_STAGES * 2 * TILE_BYTES;
@@ -187,6 +187,14 @@ gemm_tn_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__
     if (threadIdx.x == 0) {
         const int32_t npre = nk < GEMM_PREFETCH ? nk : GEMM_PREFETCH;
         for (int32_t j = 0; j < npre; ++j) issue(j);
+    }
+    if ((EPI == EPI_SUB || EPI == EPI_UPDATE) && threadIdx.x == 32) {
+        // the epilogue reads the C tile: pull it from HBM into L2 now, under the main loop (mapC describes C)
+#pragma unroll
+        for (int j = 0; j < BN / BK; ++j)
+            asm volatile("cp.async.bulk.prefetch.tensor.2d.L2.global.tile [%0, {%1, %2}];" ::"l"(&mapC),
+                         "r"(p.cc0 + tc * BN + j * BK), "r"(p.cr0 + tr * BM)
+                         : "memory");
     }
 
     // ===== consumers: warp (wr, wc) of a 2 x 4 grid owns rows [64 wr, +64) x cols [32 wc, +32) =====

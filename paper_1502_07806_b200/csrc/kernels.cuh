@@ -219,7 +219,7 @@ jacobi_batched_kernel(const double* __restrict__ A, int64_t N, int32_t M, int32_
 constexpr int CHOL_NB = 128;
 constexpr int CHOL_THREADS = 1024;
 constexpr int CHOL_LDS = CHOL_NB + 1;
-constexpr int CHOL_SMEM = (CHOL_NB * CHOL_LDS + CHOL_NB + 7 * 256) * 8;  // L below, L^-1 (transposed) above the diagonal
+constexpr int CHOL_SMEM = (CHOL_NB * CHOL_LDS + 2 * CHOL_NB + 7 * 256) * 8;  // L below, L^-1 (transposed) above the diagonal
 
 // diag(G) before the factorization: the breakdown test compares each pivot with its original diagonal entry
 __global__ void extract_diag_kernel(const double* __restrict__ S, int64_t ld, int32_t n, double* __restrict__ gdiag) {
@@ -251,6 +251,7 @@ chol_diag_kernel(const double* __restrict__ S, double* __restrict__ Lout, int64_
     double* a = sm;
     double* idiag = sm + CHOL_NB * CHOL_LDS;
     double* T = idiag + CHOL_NB;  // 7 x 256 scratch of phase B2
+    double* thr = T + 7 * 256;    // breakdown threshold per column (0 for padding columns)
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     for (int idx = tid; idx < CHOL_NB * CHOL_NB; idx += CHOL_THREADS) {
         const int i = idx >> 7, c = idx & 127;
@@ -258,6 +259,7 @@ chol_diag_kernel(const double* __restrict__ S, double* __restrict__ Lout, int64_
         if (i < nb && c < nb) v = (c <= i) ? S[(size_t)(k0 + i) * ld + k0 + c] : 0.0;
         a[i * CHOL_LDS + c] = v;
     }
+    if (tid < CHOL_NB) thr[tid] = (tid < nb) ? CHOL_BREAKDOWN * gdiag[k0 + tid] : 0.0;
     __syncthreads();
 
     // ---------------- phase A: L ----------------
@@ -267,7 +269,7 @@ chol_diag_kernel(const double* __restrict__ S, double* __restrict__ Lout, int64_
             for (int j = 0; j < 16; ++j) {
                 const int jj = j0 + j;
                 double piv = a[jj * CHOL_LDS + jj];
-                if (jj < nb && (!(piv > CHOL_BREAKDOWN * gdiag[k0 + jj]) || !(piv > 0.0))) {
+                if (!(piv > thr[jj]) || !(piv > 0.0)) {
                     if (lane == 0) atomicMin(info, (unsigned long long)(k0 + jj + 1));
                     piv = 1.0;
                 }

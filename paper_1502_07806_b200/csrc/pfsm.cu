@@ -94,8 +94,10 @@ static int dev_alloc(pfsm_ctx* h, void** p, size_t bytes) {
     return 0;
 }
 
+// mc: tensor map of the matrix C lives in (used by the SUB / UPDATE epilogues to prefetch the C tile into L2)
 template <int EPI>
-static int launch_gemm(const CUtensorMap& mx, const CUtensorMap& my, GemmParams p, cudaStream_t st) {
+static int launch_gemm(const CUtensorMap& mx, const CUtensorMap& my, const CUtensorMap& mc, GemmParams p,
+                       cudaStream_t st) {
     p.ntr = (p.mr + BM - 1) / BM;
     p.ntc = (p.nc + BN - 1) / BN;
     if (p.mr <= 0 || p.nc <= 0) return 0;
@@ -106,7 +108,7 @@ static int launch_gemm(const CUtensorMap& mx, const CUtensorMap& my, GemmParams 
         PFSM_CUDA(cudaFuncSetAttribute(gemm_tn_kernel<EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, GEMM_SMEM));
         attr_set[EPI] = true;
     }
-    gemm_tn_kernel<EPI><<<(unsigned)tiles, GEMM_THREADS, GEMM_SMEM, st>>>(mx, my, p);
+    gemm_tn_kernel<EPI><<<(unsigned)tiles, GEMM_THREADS, GEMM_SMEM, st>>>(mx, my, mc, p);
     PFSM_CUDA(cudaGetLastError());
     return 0;
 }
@@ -267,7 +269,7 @@ static int run_step4(pfsm_ctx* h, const CUtensorMap& mapV, double* V, cudaStream
         PFSM_CUDA(cudaGetLastError());
         GemmParams p = base_params();
         p.C = h->S; p.ldc = N; p.mr = n; p.nc = n; p.klen = n; p.lower = 1;
-        if ((rc = launch_gemm<EPI_PLAIN>(mapV, mapV, p, st))) return rc;
+        if ((rc = launch_gemm<EPI_PLAIN>(mapV, mapV, h->mapS, p, st))) return rc;
         extract_diag_kernel<<<(unsigned)((N + 255) / 256), 256, 0, st>>>(h->S, N, n, h->gdiag);
         PFSM_CUDA(cudaGetLastError());
         static bool chol_attr = false;
@@ -275,7 +277,9 @@ static int run_step4(pfsm_ctx* h, const CUtensorMap& mapV, double* V, cudaStream
             PFSM_CUDA(cudaFuncSetAttribute(chol_diag_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, CHOL_SMEM));
             chol_attr = true;
         }
-        for (int32_t k = 0; k < h->nblk; ++k) {
+        // Two-level blocking: 128-wide panels are factored one by one, but the big trailing update is applied
+        // once per PAIR of panels with K = 256, halving the number of times every C tile is read and re-written.
+        auto factor_panel = [&](int32_t k) -> int {
             const int32_t k0 = k * CHOL_NB, nb = (int32_t)std::min<int64_t>(CHOL_NB, N - k0);
             chol_diag_kernel<<<1, CHOL_THREADS, CHOL_SMEM, st>>>(h->S, h->O, N, k0, nb,
                                                                  h->Dinv + (size_t)k * CHOL_NB * CHOL_NB, h->gdiag, h->info);
@@ -284,14 +288,24 @@ static int run_step4(pfsm_ctx* h, const CUtensorMap& mapV, double* V, cudaStream
             GemmParams pp = base_params();
             pp.C = h->O; pp.ldc = N; pp.cr0 = k0 + nb; pp.cc0 = k0; pp.mr = 2 * n - k0 - nb; pp.nc = nb;
             pp.xr0 = k0 + nb; pp.xk0 = k0; pp.yr0 = k * CHOL_NB; pp.yk0 = 0; pp.klen = nb;
-            if ((rc = launch_gemm<EPI_PLAIN>(h->mapS, h->mapD, pp, st))) return rc;
-            // trailing update: S[r, c] -= O[r, k0:k0+nb] . O[c, k0:k0+nb]   (tiles with r >= c)
-            if (k0 + nb < n) {
-                GemmParams pt = base_params();
-                pt.C = h->S; pt.ldc = N; pt.cr0 = k0 + nb; pt.cc0 = k0 + nb; pt.mr = 2 * n - k0 - nb;
-                pt.nc = n - k0 - nb; pt.xr0 = k0 + nb; pt.yr0 = k0 + nb; pt.xk0 = k0; pt.yk0 = k0; pt.klen = nb;
-                pt.lower = 1;
-                if ((rc = launch_gemm<EPI_SUB>(h->mapO, h->mapO, pt, st))) return rc;
+            return launch_gemm<EPI_PLAIN>(h->mapS, h->mapD, h->mapO, pp, st);
+        };
+        // S[r, c0:c0+ncols] -= O[r, kk0:kk0+klen] . O[c, kk0:kk0+klen]  for rows r >= c0 (lower tiles when square)
+        auto update = [&](int32_t c0, int32_t ncols, int32_t kk0, int32_t klen, int lower) -> int {
+            if (ncols <= 0) return 0;
+            GemmParams pt = base_params();
+            pt.C = h->S; pt.ldc = N; pt.cr0 = c0; pt.cc0 = c0; pt.mr = 2 * n - c0; pt.nc = ncols;
+            pt.xr0 = c0; pt.yr0 = c0; pt.xk0 = kk0; pt.yk0 = kk0; pt.klen = klen; pt.lower = lower;
+            return launch_gemm<EPI_SUB>(h->mapO, h->mapO, h->mapS, pt, st);
+        };
+        for (int32_t k = 0; k < h->nblk; k += 2) {
+            const int32_t k0 = k * CHOL_NB;
+            if ((rc = factor_panel(k))) return rc;
+            if (k + 1 < h->nblk) {
+                const int32_t k1 = k0 + CHOL_NB, nb1 = (int32_t)std::min<int64_t>(CHOL_NB, N - k1);
+                if ((rc = update(k1, nb1, k0, CHOL_NB, 0))) return rc;      // second panel's columns only, K = 128
+                if ((rc = factor_panel(k + 1))) return rc;
+                if ((rc = update(k1 + nb1, n - k1 - nb1, k0, CHOL_NB + nb1, 1))) return rc;  // the rest, K = 256
             }
         }
         transpose_kernel<<<tg, tb, 0, st>>>(h->O + (size_t)N * N, N, V, N, n, n);
@@ -309,7 +323,7 @@ static int run_step5(pfsm_ctx* h, const CUtensorMap& mapV, const CUtensorMap& ma
     {
         GemmParams p = base_params();
         p.C = h->W; p.ldc = N; p.mr = n; p.nc = n; p.klen = n;
-        if ((rc = launch_gemm<EPI_PLAIN>(mapV, mapA, p, st))) return rc;
+        if ((rc = launch_gemm<EPI_PLAIN>(mapV, mapA, h->mapW, p, st))) return rc;
         rayleigh_kernel<<<(unsigned)N, RAY_THREADS, 0, st>>>(V, h->W, N, lambda_out, h->resid);
         PFSM_CUDA(cudaGetLastError());
     }
@@ -347,11 +361,11 @@ int pfsm_solve_partial(pfsm_handle_t h, const double* A, double* V, double* lamb
         p.C = h->W; p.ldc = N; p.mr = n; p.nc = n; p.klen = n;
         p.krange = (it == 0) ? h->krange : nullptr;  // start vectors are zero outside their window
         p.E1 = V; p.ld1 = N; p.eps = h->eps;
-        if ((rc = launch_gemm<EPI_SHIFT>(mapV, mapA, p, st))) return rc;
+        if ((rc = launch_gemm<EPI_SHIFT>(mapV, mapA, h->mapW, p, st))) return rc;
         GemmParams q = base_params();  // V <- V - alpha (W A - diag(eps) W)
         q.C = V; q.ldc = N; q.mr = n; q.nc = n; q.klen = n;
         q.E1 = h->W; q.ld1 = N; q.E2 = V; q.ld2 = N; q.eps = h->eps; q.alpha = h->alpha;
-        if ((rc = launch_gemm<EPI_UPDATE>(h->mapW, mapA, q, st))) return rc;
+        if ((rc = launch_gemm<EPI_UPDATE>(h->mapW, mapA, mapV, q, st))) return rc;
     }
     if (tm) PFSM_CUDA(cudaEventRecord(h->ev[2], st));
     if (last_step == 3) return 0;
@@ -454,7 +468,12 @@ size_t pfsm_workspace_bytes(pfsm_handle_t h) { return h ? h->bytes : 0; }
 int64_t pfsm_launches_per_solve(pfsm_handle_t h) {
     if (!h) return 0;
     // jacobi + 2 iters GEMMs + (2 transposes + Gram + diag extract + per panel: diag, panel, trailing (none after the last)) + GEMM + rayleigh
-    return 1 + 2 * (int64_t)h->iters + (2 + 1 + 1 + 3 * (int64_t)h->nblk - 1) + 2;
+    {
+        const int64_t nb = h->nblk, pairs = nb / 2;
+        // per panel: chol_diag + panel GEMM; per pair of panels: inner update + (if columns remain) trailing update
+        const int64_t trailing = (nb % 2 == 0) ? pairs - 1 : pairs;
+        return 1 + 2 * (int64_t)h->iters + (2 + 1 + 1 + 2 * nb + pairs + trailing) + 2;
+    }
 }
 
 int pfsm_enable_step_timing(pfsm_handle_t h, int32_t enable) {
