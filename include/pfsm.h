@@ -108,6 +108,20 @@ int pfsm_orthonormalize(pfsm_handle_t h, double* V_inout, void* stream);
  */
 int pfsm_rayleigh(pfsm_handle_t h, const double* A, const double* V, double* lambda_out, void* stream);
 
+/*
+ * Generalized problem A x = lambda S x (Eq. 13; BASELINE.json configs[4] "generalized form ...
+ * reduced by Cholesky(S)").  S = L L^T, A' = L^-1 A L^-T (symmetrized), PFSM steps 2-5 on A', X = L^-T V.
+ *   A, S       device, N x N, symmetric, read only; S positive definite
+ *   X_out      device, N x N: column i = generalized eigenvector i, X^T S X = I
+ *   lambda_out device, N
+ * The residual buffer then holds the standard-form residuals ||A' v_i - lambda_i v_i||_2.  info in 1..N can
+ * also mean that pivot `info` of Cholesky(S) was not positive.  Allocates 2 N^2 doubles more on first use.
+ * pfsm_generalized_reduce runs the reduction alone and writes A' to Ap_out (device, N x N).
+ */
+int pfsm_solve_generalized(pfsm_handle_t h, const double* A, const double* S, double* X_out, double* lambda_out,
+                           void* stream);
+int pfsm_generalized_reduce(pfsm_handle_t h, const double* A, const double* S, double* Ap_out, void* stream);
+
 /* Release the handle and its workspace (synchronizes the device).  NULL is a no-op returning 0. */
 int pfsm_destroy(pfsm_handle_t h);
 

@@ -18,7 +18,8 @@ _lib = None
 CUDA_ERROR_BASE = 1000
 
 EXPORTS = [
-    "pfsm_create", "pfsm_solve", "pfsm_solve_host", "pfsm_solve_partial", "pfsm_orthonormalize", "pfsm_rayleigh", "pfsm_destroy", "pfsm_get_info",
+    "pfsm_create", "pfsm_solve", "pfsm_solve_host", "pfsm_solve_partial", "pfsm_orthonormalize", "pfsm_rayleigh", "pfsm_solve_generalized",
+    "pfsm_generalized_reduce", "pfsm_destroy", "pfsm_get_info",
     "pfsm_get_residuals", "pfsm_get_shifts", "pfsm_set_alpha", "pfsm_workspace_bytes",
     "pfsm_launches_per_solve", "pfsm_enable_step_timing", "pfsm_get_step_ms", "pfsm_probe_fp64_peak",
     "pfsm_strerror",
@@ -52,6 +53,8 @@ def load(build_if_missing: bool = True):
     lib.pfsm_solve_partial.argtypes = [p, p, p, p, p, i32]
     lib.pfsm_orthonormalize.argtypes = [p, p, p]
     lib.pfsm_rayleigh.argtypes = [p, p, p, p, p]
+    lib.pfsm_solve_generalized.argtypes = [p, p, p, p, p, p]
+    lib.pfsm_generalized_reduce.argtypes = [p, p, p, p, p]
     lib.pfsm_destroy.argtypes = [p]
     lib.pfsm_get_info.argtypes = [p, p, ctypes.POINTER(i64)]
     lib.pfsm_get_residuals.argtypes = [p, ctypes.POINTER(p)]
@@ -137,6 +140,18 @@ class Handle:
         N = self.N
         _check(self._lib.pfsm_rayleigh(self._h, _dev_ptr(A, N, (N, N), "A"), _dev_ptr(Vr, N, (N, N), "V"),
                                        _dev_ptr(lam, N, (N,), "lambda"), _stream_ptr(stream)), "pfsm_rayleigh")
+
+    def solve_generalized(self, A, S, Xr, lam, stream=None):
+        N = self.N
+        _check(self._lib.pfsm_solve_generalized(self._h, _dev_ptr(A, N, (N, N), "A"), _dev_ptr(S, N, (N, N), "S"),
+                                                _dev_ptr(Xr, N, (N, N), "X"), _dev_ptr(lam, N, (N,), "lambda"),
+                                                _stream_ptr(stream)), "pfsm_solve_generalized")
+
+    def generalized_reduce(self, A, S, Ap, stream=None):
+        N = self.N
+        _check(self._lib.pfsm_generalized_reduce(self._h, _dev_ptr(A, N, (N, N), "A"), _dev_ptr(S, N, (N, N), "S"),
+                                                 _dev_ptr(Ap, N, (N, N), "Ap"), _stream_ptr(stream)),
+               "pfsm_generalized_reduce")
 
     def solve_host(self, A_host, Vr_host, lam_host, stream=None):
         N = self.N

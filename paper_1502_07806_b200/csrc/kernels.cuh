@@ -382,6 +382,40 @@ __global__ void transpose_kernel(const double* __restrict__ in, int64_t ldi, dou
     }
 }
 
+// out = (in + in^T) / 2 for an n x n row-major matrix (32 x 32 tiles, both reads coalesced)
+__global__ void symmetrize_kernel(const double* __restrict__ in, int64_t ldi, double* __restrict__ out, int64_t ldo,
+                                  int32_t n) {
+    __shared__ double t1[32][33], t2[32][33];
+    const int bx = blockIdx.x * 32, by = blockIdx.y * 32;
+    const int tx = threadIdx.x, ty = threadIdx.y;  // 32 x 8
+#pragma unroll
+    for (int k = 0; k < 32; k += 8) {
+        const int r = by + ty + k, c = bx + tx;
+        t1[ty + k][tx] = (r < n && c < n) ? in[(size_t)r * ldi + c] : 0.0;
+        const int r2 = bx + ty + k, c2 = by + tx;
+        t2[ty + k][tx] = (r2 < n && c2 < n) ? in[(size_t)r2 * ldi + c2] : 0.0;
+    }
+    __syncthreads();
+#pragma unroll
+    for (int k = 0; k < 32; k += 8) {
+        const int r = by + ty + k, c = bx + tx;
+        if (r < n && c < n) out[(size_t)r * ldo + c] = 0.5 * (t1[ty + k][tx] + t2[tx][ty + k]);
+    }
+}
+
+// out block b = transpose of in block b, for nblocks dense 128 x 128 blocks (grid: 4 x 4 x nblocks, block 32 x 8)
+__global__ void transpose_blocks_kernel(const double* __restrict__ in, double* __restrict__ out) {
+    __shared__ double tile[32][33];
+    const size_t base = (size_t)blockIdx.z * 128 * 128;
+    const int bx = blockIdx.x * 32, by = blockIdx.y * 32;
+    const int tx = threadIdx.x, ty = threadIdx.y;
+#pragma unroll
+    for (int k = 0; k < 32; k += 8) tile[ty + k][tx] = in[base + (size_t)(by + ty + k) * 128 + bx + tx];
+    __syncthreads();
+#pragma unroll
+    for (int k = 0; k < 32; k += 8) out[base + (size_t)(bx + ty + k) * 128 + by + tx] = tile[tx][ty + k];
+}
+
 // ---------------------------------------------------------------------------------------------
 // Step 5: one CTA per eigenvector i.  lambda_i = v_i . t_i  (t_i = A v_i from the GEMM), then
 // r_i = || t_i - lambda_i v_i ||_2.  Vectorised, coalesced; fixed reduction order (deterministic).

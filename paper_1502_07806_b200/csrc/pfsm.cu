@@ -77,6 +77,10 @@ struct pfsm_ctx {
     int32_t* slice_tab = nullptr;  // g0[P], lo[P], off[P]
     int2* krange = nullptr;        // per 128-row tile k-range of the first product
     unsigned long long* info = nullptr;
+    double* Ap = nullptr;       // generalized variant: A' = L^-1 A L^-T
+    double* LT = nullptr;       //   L^T (S = L L^T)
+    double* DinvT = nullptr;    //   transposed inverses of L's diagonal blocks
+    CUtensorMap mapAp, mapLT, mapDT;
     double* A_stage = nullptr;  // host-buffer path
     double* V_stage = nullptr;
     double* lam_stage = nullptr;
@@ -86,6 +90,7 @@ struct pfsm_ctx {
     bool timing = false;
     cudaEvent_t ev[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
     bool ev_valid = false;
+    bool keep_info = false;
 };
 
 static int dev_alloc(pfsm_ctx* h, void** p, size_t bytes) {
@@ -210,7 +215,7 @@ int pfsm_destroy(pfsm_handle_t h) {
     if (!h) return 0;
     cudaDeviceSynchronize();
     void* ptrs[] = {h->W, h->S, h->O, h->Dinv, h->Gws, h->eps, h->resid, h->gdiag, h->rotcnt, h->slice_tab, h->krange, h->info,
-                    h->A_stage, h->V_stage, h->lam_stage};
+                    h->A_stage, h->V_stage, h->lam_stage, h->Ap, h->LT, h->DinvT};
     for (void* p : ptrs)
         if (p) cudaFree(p);
     for (int i = 0; i < 5; ++i)
@@ -258,59 +263,73 @@ static int launch_jacobi(pfsm_ctx* h, const double* A, double* V, cudaStream_t s
     return launch_jacobi_t<16>(h, A, V, st);
 }
 
-// ---- step 4: Cholesky-QR on the stacked matrix [G ; V^T], G = V^T V (row-major view: V V^T) ----
+// ---- Stacked right-looking Cholesky on S = [G ; Z] (2N x N, row-major view): O = [L ; Z L^-T] with G = L L^T.
+// The panel step O[r,k] = S[r,k] L_kk^-T and the trailing update S[r,c] -= O[r,k] O[c,k]^T run over every row
+// below the diagonal block, so the triangular solve of the bottom rows is folded into the factorization's GEMMs.
+// factor = false re-uses L (O's top) and the inverted diagonal blocks of an earlier pass and only transforms
+// the bottom rows [N, 2N).  Two-level blocking: 128-wide panels are factored one by one, but the big trailing
+// update is applied once per PAIR of panels with K = 256, halving how often every C tile is read and re-written.
+static int stacked_cholesky(pfsm_ctx* h, bool factor, cudaStream_t st) {
+    const int64_t N = h->N;
+    const int32_t n = (int32_t)N;
+    int rc;
+    static bool chol_attr = false;
+    if (!chol_attr) {
+        PFSM_CUDA(cudaFuncSetAttribute(chol_diag_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, CHOL_SMEM));
+        chol_attr = true;
+    }
+    auto factor_panel = [&](int32_t k) -> int {
+        const int32_t k0 = k * CHOL_NB, nb = (int32_t)std::min<int64_t>(CHOL_NB, N - k0);
+        if (factor) {
+            chol_diag_kernel<<<1, CHOL_THREADS, CHOL_SMEM, st>>>(h->S, h->O, N, k0, nb,
+                                                                 h->Dinv + (size_t)k * CHOL_NB * CHOL_NB, h->gdiag, h->info);
+            PFSM_CUDA(cudaGetLastError());
+        }
+        // panel: O[r, k0:k0+nb] = S[r, k0:k0+nb] L_kk^-T   for all rows below the diagonal block (or the bottom rows)
+        const int32_t r0 = factor ? k0 + nb : n;
+        GemmParams pp = base_params();
+        pp.C = h->O; pp.ldc = N; pp.cr0 = r0; pp.cc0 = k0; pp.mr = 2 * n - r0; pp.nc = nb;
+        pp.xr0 = r0; pp.xk0 = k0; pp.yr0 = k * CHOL_NB; pp.yk0 = 0; pp.klen = nb;
+        return launch_gemm<EPI_PLAIN>(h->mapS, h->mapD, h->mapO, pp, st);
+    };
+    // S[r, c0:c0+ncols] -= O[r, kk0:kk0+klen] . O[c, kk0:kk0+klen]  for rows r >= c0 (lower tiles when square)
+    auto update = [&](int32_t c0, int32_t ncols, int32_t kk0, int32_t klen, int lower) -> int {
+        if (ncols <= 0) return 0;
+        const int32_t r0 = factor ? c0 : n;
+        GemmParams pt = base_params();
+        pt.C = h->S; pt.ldc = N; pt.cr0 = r0; pt.cc0 = c0; pt.mr = 2 * n - r0; pt.nc = ncols;
+        pt.xr0 = r0; pt.yr0 = c0; pt.xk0 = kk0; pt.yk0 = kk0; pt.klen = klen; pt.lower = factor ? lower : 0;
+        return launch_gemm<EPI_SUB>(h->mapO, h->mapO, h->mapS, pt, st);
+    };
+    for (int32_t k = 0; k < h->nblk; k += 2) {
+        const int32_t k0 = k * CHOL_NB;
+        if ((rc = factor_panel(k))) return rc;
+        if (k + 1 < h->nblk) {
+            const int32_t k1 = k0 + CHOL_NB, nb1 = (int32_t)std::min<int64_t>(CHOL_NB, N - k1);
+            if ((rc = update(k1, nb1, k0, CHOL_NB, 0))) return rc;      // second panel's columns only, K = 128
+            if ((rc = factor_panel(k + 1))) return rc;
+            if ((rc = update(k1 + nb1, n - k1 - nb1, k0, CHOL_NB + nb1, 1))) return rc;  // the rest, K = 256
+        }
+    }
+    return 0;
+}
+
+// ---- step 4: Cholesky-QR.  G = V^T V (row-major view: V V^T), S = [G ; V^T] ----
 static int run_step4(pfsm_ctx* h, const CUtensorMap& mapV, double* V, cudaStream_t st) {
     const int64_t N = h->N;
     const int32_t n = (int32_t)N;
     int rc;
-    {
-        const dim3 tb(32, 8), tg((unsigned)((N + 31) / 32), (unsigned)((N + 31) / 32));
-        transpose_kernel<<<tg, tb, 0, st>>>(V, N, h->S + (size_t)N * N, N, n, n);
-        PFSM_CUDA(cudaGetLastError());
-        GemmParams p = base_params();
-        p.C = h->S; p.ldc = N; p.mr = n; p.nc = n; p.klen = n; p.lower = 1;
-        if ((rc = launch_gemm<EPI_PLAIN>(mapV, mapV, h->mapS, p, st))) return rc;
-        extract_diag_kernel<<<(unsigned)((N + 255) / 256), 256, 0, st>>>(h->S, N, n, h->gdiag);
-        PFSM_CUDA(cudaGetLastError());
-        static bool chol_attr = false;
-        if (!chol_attr) {
-            PFSM_CUDA(cudaFuncSetAttribute(chol_diag_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, CHOL_SMEM));
-            chol_attr = true;
-        }
-        // Two-level blocking: 128-wide panels are factored one by one, but the big trailing update is applied
-        // once per PAIR of panels with K = 256, halving the number of times every C tile is read and re-written.
-        auto factor_panel = [&](int32_t k) -> int {
-            const int32_t k0 = k * CHOL_NB, nb = (int32_t)std::min<int64_t>(CHOL_NB, N - k0);
-            chol_diag_kernel<<<1, CHOL_THREADS, CHOL_SMEM, st>>>(h->S, h->O, N, k0, nb,
-                                                                 h->Dinv + (size_t)k * CHOL_NB * CHOL_NB, h->gdiag, h->info);
-            PFSM_CUDA(cudaGetLastError());
-            // panel: O[r, k0:k0+nb] = S[r, k0:k0+nb] L_kk^-T   for all rows below the diagonal block
-            GemmParams pp = base_params();
-            pp.C = h->O; pp.ldc = N; pp.cr0 = k0 + nb; pp.cc0 = k0; pp.mr = 2 * n - k0 - nb; pp.nc = nb;
-            pp.xr0 = k0 + nb; pp.xk0 = k0; pp.yr0 = k * CHOL_NB; pp.yk0 = 0; pp.klen = nb;
-            return launch_gemm<EPI_PLAIN>(h->mapS, h->mapD, h->mapO, pp, st);
-        };
-        // S[r, c0:c0+ncols] -= O[r, kk0:kk0+klen] . O[c, kk0:kk0+klen]  for rows r >= c0 (lower tiles when square)
-        auto update = [&](int32_t c0, int32_t ncols, int32_t kk0, int32_t klen, int lower) -> int {
-            if (ncols <= 0) return 0;
-            GemmParams pt = base_params();
-            pt.C = h->S; pt.ldc = N; pt.cr0 = c0; pt.cc0 = c0; pt.mr = 2 * n - c0; pt.nc = ncols;
-            pt.xr0 = c0; pt.yr0 = c0; pt.xk0 = kk0; pt.yk0 = kk0; pt.klen = klen; pt.lower = lower;
-            return launch_gemm<EPI_SUB>(h->mapO, h->mapO, h->mapS, pt, st);
-        };
-        for (int32_t k = 0; k < h->nblk; k += 2) {
-            const int32_t k0 = k * CHOL_NB;
-            if ((rc = factor_panel(k))) return rc;
-            if (k + 1 < h->nblk) {
-                const int32_t k1 = k0 + CHOL_NB, nb1 = (int32_t)std::min<int64_t>(CHOL_NB, N - k1);
-                if ((rc = update(k1, nb1, k0, CHOL_NB, 0))) return rc;      // second panel's columns only, K = 128
-                if ((rc = factor_panel(k + 1))) return rc;
-                if ((rc = update(k1 + nb1, n - k1 - nb1, k0, CHOL_NB + nb1, 1))) return rc;  // the rest, K = 256
-            }
-        }
-        transpose_kernel<<<tg, tb, 0, st>>>(h->O + (size_t)N * N, N, V, N, n, n);
-        PFSM_CUDA(cudaGetLastError());
-    }
+    const dim3 tb(32, 8), tg((unsigned)((N + 31) / 32), (unsigned)((N + 31) / 32));
+    transpose_kernel<<<tg, tb, 0, st>>>(V, N, h->S + (size_t)N * N, N, n, n);
+    PFSM_CUDA(cudaGetLastError());
+    GemmParams p = base_params();
+    p.C = h->S; p.ldc = N; p.mr = n; p.nc = n; p.klen = n; p.lower = 1;
+    if ((rc = launch_gemm<EPI_PLAIN>(mapV, mapV, h->mapS, p, st))) return rc;
+    extract_diag_kernel<<<(unsigned)((N + 255) / 256), 256, 0, st>>>(h->S, N, n, h->gdiag);
+    PFSM_CUDA(cudaGetLastError());
+    if ((rc = stacked_cholesky(h, true, st))) return rc;
+    transpose_kernel<<<tg, tb, 0, st>>>(h->O + (size_t)N * N, N, V, N, n, n);
+    PFSM_CUDA(cudaGetLastError());
     return 0;
 }
 
@@ -349,7 +368,7 @@ int pfsm_solve_partial(pfsm_handle_t h, const double* A, double* V, double* lamb
 
     // ---- step 2: batched submatrix eigensolves -> shifts and zero-padded start vectors ----
     if (tm) PFSM_CUDA(cudaEventRecord(h->ev[0], st));
-    PFSM_CUDA(cudaMemsetAsync(h->info, 0xFF, sizeof(unsigned long long), st));
+    if (!h->keep_info) PFSM_CUDA(cudaMemsetAsync(h->info, 0xFF, sizeof(unsigned long long), st));
     PFSM_CUDA(cudaMemsetAsync(V, 0, (size_t)N * N * sizeof(double), st));
     if ((rc = launch_jacobi(h, A, V, st))) return rc;
     if (tm) PFSM_CUDA(cudaEventRecord(h->ev[1], st));
@@ -405,6 +424,102 @@ int pfsm_rayleigh(pfsm_handle_t h, const double* A, const double* V, double* lam
     if ((rc = make_map(&mapV, V, h->N, h->N, h->N))) return rc;
     h->ev_valid = false;
     return run_step5(h, mapV, mapA, const_cast<double*>(V), lambda_out, (cudaStream_t)stream);
+}
+
+// ---- Row G (BASELINE.json configs[4], Eq. 13): A x = lambda S x reduced by Cholesky(S) ----
+static int ensure_generalized(pfsm_ctx* h) {
+    if (h->Ap) return 0;
+    const int64_t N = h->N;
+    const size_t n2 = (size_t)N * N * sizeof(double);
+    int rc;
+    if ((rc = dev_alloc(h, (void**)&h->Ap, n2))) return rc;
+    if ((rc = dev_alloc(h, (void**)&h->LT, n2))) return rc;
+    if ((rc = dev_alloc(h, (void**)&h->DinvT, (size_t)h->nblk * CHOL_NB * CHOL_NB * sizeof(double)))) return rc;
+    if ((rc = make_map(&h->mapAp, h->Ap, N, N, N))) return rc;
+    if ((rc = make_map(&h->mapLT, h->LT, N, N, N))) return rc;
+    if ((rc = make_map(&h->mapDT, h->DinvT, (int64_t)h->nblk * CHOL_NB, CHOL_NB, CHOL_NB))) return rc;
+    return 0;
+}
+
+// S = L L^T;  Ap = L^-1 A L^-T (symmetrized);  keeps L^T and the transposed inverted diagonal blocks for the
+// back-transformation.  Two passes of the stacked Cholesky: [S ; A] -> A L^-T, then [.; (A L^-T)^T] -> L^-1 A L^-T.
+static int run_generalized_reduce(pfsm_ctx* h, const double* A, const double* S_in, double* Ap_out, cudaStream_t st) {
+    const int64_t N = h->N;
+    const int32_t n = (int32_t)N;
+    const size_t n2 = (size_t)N * N * sizeof(double);
+    int rc;
+    const dim3 tb(32, 8), tg((unsigned)((N + 31) / 32), (unsigned)((N + 31) / 32));
+    PFSM_CUDA(cudaMemsetAsync(h->info, 0xFF, sizeof(unsigned long long), st));
+    PFSM_CUDA(cudaMemcpyAsync(h->S, S_in, n2, cudaMemcpyDeviceToDevice, st));
+    PFSM_CUDA(cudaMemcpyAsync(h->S + (size_t)N * N, A, n2, cudaMemcpyDeviceToDevice, st));
+    extract_diag_kernel<<<(unsigned)((N + 255) / 256), 256, 0, st>>>(h->S, N, n, h->gdiag);
+    PFSM_CUDA(cudaGetLastError());
+    if ((rc = stacked_cholesky(h, true, st))) return rc;                       // O = [L ; A L^-T]
+    transpose_kernel<<<tg, tb, 0, st>>>(h->O + (size_t)N * N, N, h->S + (size_t)N * N, N, n, n);  // (A L^-T)^T = L^-1 A
+    PFSM_CUDA(cudaGetLastError());
+    if ((rc = stacked_cholesky(h, false, st))) return rc;                      // O bottom = L^-1 A L^-T
+    symmetrize_kernel<<<tg, tb, 0, st>>>(h->O + (size_t)N * N, N, Ap_out, N, n);
+    PFSM_CUDA(cudaGetLastError());
+    transpose_kernel<<<tg, tb, 0, st>>>(h->O, N, h->LT, N, n, n);
+    PFSM_CUDA(cudaGetLastError());
+    transpose_blocks_kernel<<<dim3(4, 4, (unsigned)h->nblk), tb, 0, st>>>(h->Dinv, h->DinvT);
+    PFSM_CUDA(cudaGetLastError());
+    return 0;
+}
+
+// X = L^-T V, in the row-major view X_rm = V_rm L^-1: block back-substitution from the last panel to the first,
+// X_k = R_k L_kk^-1, then R[:, c] -= X_k L[k, c] for the column blocks c < k.  R = V in place, X collected in W.
+static int run_generalized_back(pfsm_ctx* h, double* V, cudaStream_t st) {
+    const int64_t N = h->N;
+    const int32_t n = (int32_t)N;
+    int rc;
+    CUtensorMap mapV;
+    if ((rc = make_map(&mapV, V, N, N, N))) return rc;
+    for (int32_t k = h->nblk - 1; k >= 0; --k) {
+        const int32_t k0 = k * CHOL_NB, nb = (int32_t)std::min<int64_t>(CHOL_NB, N - k0);
+        GemmParams pp = base_params();
+        pp.C = h->W; pp.ldc = N; pp.cr0 = 0; pp.cc0 = k0; pp.mr = n; pp.nc = nb;
+        pp.xr0 = 0; pp.xk0 = k0; pp.yr0 = k * CHOL_NB; pp.yk0 = 0; pp.klen = nb;
+        if ((rc = launch_gemm<EPI_PLAIN>(mapV, h->mapDT, h->mapW, pp, st))) return rc;
+        if (k0 > 0) {
+            GemmParams pt = base_params();
+            pt.C = V; pt.ldc = N; pt.cr0 = 0; pt.cc0 = 0; pt.mr = n; pt.nc = k0;
+            pt.xr0 = 0; pt.xk0 = k0; pt.yr0 = 0; pt.yk0 = k0; pt.klen = nb;
+            if ((rc = launch_gemm<EPI_SUB>(h->mapW, h->mapLT, mapV, pt, st))) return rc;
+        }
+    }
+    PFSM_CUDA(cudaMemcpyAsync(V, h->W, (size_t)N * N * sizeof(double), cudaMemcpyDeviceToDevice, st));
+    return 0;
+}
+
+int pfsm_generalized_reduce(pfsm_handle_t h, const double* A, const double* S, double* Ap_out, void* stream) {
+    if (!h) return -1;
+    if (!A || ((uintptr_t)A & 15)) return -2;
+    if (!S || ((uintptr_t)S & 15)) return -3;
+    if (!Ap_out || ((uintptr_t)Ap_out & 15)) return -4;
+    int rc;
+    if ((rc = ensure_generalized(h))) return rc;
+    h->ev_valid = false;
+    return run_generalized_reduce(h, A, S, Ap_out, (cudaStream_t)stream);
+}
+
+int pfsm_solve_generalized(pfsm_handle_t h, const double* A, const double* S, double* X_out, double* lambda_out,
+                           void* stream) {
+    if (!h) return -1;
+    if (!A || ((uintptr_t)A & 15)) return -2;
+    if (!S || ((uintptr_t)S & 15)) return -3;
+    if (!X_out || ((uintptr_t)X_out & 15)) return -4;
+    if (!lambda_out || ((uintptr_t)lambda_out & 7)) return -5;
+    int rc;
+    if ((rc = ensure_generalized(h))) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    if ((rc = run_generalized_reduce(h, A, S, h->Ap, st))) return rc;
+    // the reduction's status (S not positive definite) must survive the solve's own reset of info
+    h->keep_info = true;
+    rc = pfsm_solve_partial(h, h->Ap, X_out, lambda_out, stream, 5);
+    h->keep_info = false;
+    if (rc) return rc;
+    return run_generalized_back(h, X_out, st);
 }
 
 int pfsm_solve(pfsm_handle_t h, const double* A, double* V_inout, double* lambda_out, void* stream) {

@@ -321,3 +321,95 @@ def test_baseline_configs_large_sampled(k):
     if os.environ.get("PFSM_FULL_ORACLE") == "1":
         o = oracle.pfsm(p.A, c.P, c.window, c.iters, p.alpha)
         check_gates(p.A, g, o)
+
+
+# ------------------------------------------------------------------ row G: generalized variant A x = lambda S x
+def gpu_generalized(A, S, P, w, iters, alpha):
+    N = A.shape[0]
+    h = pfsm.Handle(N, P, w, iters, alpha)
+    dA, dS = dev(A), dev(S)
+    dAp = torch.empty((N, N), dtype=torch.float64, device="cuda")
+    h.generalized_reduce(dA, dS, dAp)
+    info_r = h.info()
+    dX = torch.empty((N, N), dtype=torch.float64, device="cuda")
+    dl = torch.empty((N,), dtype=torch.float64, device="cuda")
+    h.solve_generalized(dA, dS, dX, dl)
+    out = dict(Ap=dAp.cpu().numpy(), Xr=dX.cpu().numpy(), lam=dl.cpu().numpy(), resid=h.residuals().cpu().numpy(),
+               info=h.info(), info_reduce=info_r)
+    h.destroy()
+    return out
+
+
+@pytest.mark.parametrize("N,P,w,iters", [(192, 4, 12, 2), (300, 5, 10, 3), (384, 3, 40, 2)])
+def test_generalized_small_against_oracle(N, P, w, iters):
+    p = gen.small_problem(N, 2e-3, 12.0, seed=600 + N)
+    S = gen.banded_symmetric(N, np.ones(N), 1e-2, 6.0, 600 + N, gen.STREAM_S)
+    g = gpu_generalized(p.A, S, P, w, iters, p.alpha)
+    L, Ap, info = oracle.generalized_reduce(p.A, S)
+    assert info == 0 and g["info"] == 0 and g["info_reduce"] == 0
+    assert np.abs(g["Ap"] - Ap).max() < 1e-12 * max(1.0, np.abs(Ap).max())
+    assert np.array_equal(g["Ap"], g["Ap"].T)                       # exactly symmetric
+    o = oracle.pfsm(Ap, P, w, iters, p.alpha)
+    Xo = oracle.generalized_back(L, o["Vr"])
+    nF = float(np.linalg.norm(Ap))
+    assert np.abs(g["lam"] - o["lam"]).max() <= 1e-10 * nF
+    assert np.abs(g["resid"] - o["resid"]).max() <= 1e-9 * nF
+    X = g["Xr"]
+    assert np.abs(X @ S @ X.T - np.eye(N)).max() <= 1e-12 * N        # X^T S X = I (pin P13)
+    assert np.abs(align_signs(X, Xo) - Xo).max() < 1e-8
+    # generalized residual = L (A' v - lambda v): bounded by ||L|| r_i
+    R = X @ p.A - (X @ S) * g["lam"][:, None]
+    assert np.all(np.linalg.norm(R, axis=1) <= np.linalg.norm(L, 2) * g["resid"] + 1e-11)
+
+
+def test_generalized_identity_overlap_equals_standard_path():
+    p = gen.problem(0)
+    c = p.cfg
+    g = gpu_generalized(p.A, np.eye(c.N), c.P, c.window, c.iters, p.alpha)
+    ref = gpu_solve(p.A, c.P, c.window, c.iters, p.alpha)
+    assert np.array_equal(g["Ap"], p.A)
+    assert np.array_equal(g["lam"], ref["lam"]) and np.array_equal(g["Xr"], ref["Vr"])
+
+
+def test_generalized_flags_indefinite_overlap():
+    N = 256
+    p = gen.small_problem(N, 1e-3, 8.0, seed=71)
+    S = np.eye(N)
+    S[100, 100] = -1.0
+    g = gpu_generalized(p.A, S, 4, 8, 1, p.alpha)
+    assert g["info_reduce"] == 101 and g["info"] != 0
+
+
+def test_generalized_config4g_properties():
+    """BASELINE.json configs[4] generalized form at full size (N=8192).  The oracle's unblocked reduction needs
+    ~1e12 flop in plain loops, so the reduction is pinned by properties that determine it uniquely: L lower
+    triangular with positive diagonal and L L^T = S (uniqueness of Cholesky), L A' L^T = A; then the standard
+    path on A' is the already-tested one, and X^T S X = I, A X = S X Lambda + L R hold for the result."""
+    p = gen.problem(4, generalized=True)
+    c = p.cfg
+    N = c.N
+    h = pfsm.Handle(N, c.P, c.window, c.iters, p.alpha)
+    dA, dS = dev(p.A), dev(p.S)
+    dAp = torch.empty((N, N), dtype=torch.float64, device="cuda")
+    h.generalized_reduce(dA, dS, dAp)
+    assert h.info() == 0
+    Lt = torch.linalg.cholesky(dS)                       # comparison only: the unique factor
+    back = Lt @ dAp @ Lt.T
+    assert (back - dA).abs().max().item() < 1e-11
+    assert (dAp - dAp.T).abs().max().item() == 0.0
+    dX = torch.empty((N, N), dtype=torch.float64, device="cuda")
+    dl = torch.empty((N,), dtype=torch.float64, device="cuda")
+    h.solve_generalized(dA, dS, dX, dl)
+    assert h.info() == 0
+    eye_err = (dX @ dS @ dX.T - torch.eye(N, dtype=torch.float64, device="cuda")).abs().max().item()
+    assert eye_err <= 1e-12 * N
+    R = dX @ dA - (dX @ dS) * dl[:, None]
+    rn = torch.linalg.norm(R, dim=1)
+    res = h.residuals()
+    assert bool((rn <= 1.01 * res + 1e-10).all())         # ||L|| <= 1.01 for S = I + 1e-4 perturbation
+    # the standard path on A' gives the same eigenvalues
+    dV = torch.empty((N, N), dtype=torch.float64, device="cuda")
+    dl2 = torch.empty((N,), dtype=torch.float64, device="cuda")
+    h.solve(dAp, dV, dl2)
+    assert torch.equal(dl, dl2)
+    h.destroy()
