@@ -463,21 +463,25 @@ rayleigh_kernel(const double* __restrict__ V, const double* __restrict__ T, int6
 // ---------------------------------------------------------------------------------------------
 // Roofline calibration: register-only FP64 issue-rate loops (no memory traffic).
 // ---------------------------------------------------------------------------------------------
+// 4 accumulator pairs per warp, reused in place (with 16 ptxas emits out-of-place DMMAs whose WAW hazards
+// stall the pipe and the loop reads ~20 % low); 8 warps per SMSP hide the DMMA latency.
 __global__ void __launch_bounds__(256) probe_dmma_kernel(int iters, double* sink) {
-    double c[16][2];
+    double c[4][2];
 #pragma unroll
-    for (int i = 0; i < 16; ++i) c[i][0] = c[i][1] = 0.0;
+    for (int i = 0; i < 4; ++i) c[i][0] = c[i][1] = 0.0;
     const double a = 1.0 + 1e-9 * threadIdx.x, b = 1.0 - 1e-9 * threadIdx.x;
     for (int it = 0; it < iters; ++it) {
 #pragma unroll
-        for (int i = 0; i < 16; ++i)
-            asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
-                         : "+d"(c[i][0]), "+d"(c[i][1])
-                         : "d"(a), "d"(b));
+        for (int r = 0; r < 4; ++r)
+#pragma unroll
+            for (int i = 0; i < 4; ++i)
+                asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+                             : "+d"(c[i][0]), "+d"(c[i][1])
+                             : "d"(a), "d"(b));
     }
     double s = 0.0;
 #pragma unroll
-    for (int i = 0; i < 16; ++i) s += c[i][0] + c[i][1];
+    for (int i = 0; i < 4; ++i) s += c[i][0] + c[i][1];
     if (s == 123.456) sink[0] = s;
 }
 __global__ void __launch_bounds__(256) probe_dfma_kernel(int iters, double* sink) {

@@ -10,11 +10,13 @@
 #include <climits>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <vector>
 
 #include "gemm_tn.cuh"
 #include "kernels.cuh"
+#include "jacobi_smem.cuh"
 
 namespace pfsm {
 
@@ -73,6 +75,8 @@ struct pfsm_ctx {
     double* eps = nullptr;    // N shifts
     double* resid = nullptr;  // N residual norms
     int* rotcnt = nullptr;    // P x JACOBI_MAX_SWEEPS rotation counters of step 2
+    double* nrm_g = nullptr;  // P x (M + 16): final column norms of the shared-memory Jacobi
+    int jac_cs = 0, jac_hloc = 0;  // cluster size / seats per CTA of the shared-memory Jacobi (0 = L2 kernel)
     double* gdiag = nullptr;  // N: diag(V^T V) before the factorization (breakdown threshold)
     int32_t* slice_tab = nullptr;  // g0[P], lo[P], off[P]
     int2* krange = nullptr;        // per 128-row tile k-range of the first product
@@ -124,6 +128,8 @@ static GemmParams base_params() {
     return p;
 }
 
+extern "C" { static void choose_jacobi_layout(pfsm_ctx* h); }
+
 extern "C" {
 
 const char* pfsm_strerror(int code) {
@@ -169,6 +175,8 @@ int pfsm_create(pfsm_handle_t* out, int64_t N, int32_t P, int32_t window, int32_
     TRY(dev_alloc(h, (void**)&h->resid, N * sizeof(double)));
     TRY(dev_alloc(h, (void**)&h->gdiag, N * sizeof(double)));
     TRY(dev_alloc(h, (void**)&h->rotcnt, (size_t)P * JACOBI_MAX_SWEEPS * sizeof(int)));
+    TRY(dev_alloc(h, (void**)&h->nrm_g, (size_t)P * (M + 16) * sizeof(double)));
+    choose_jacobi_layout(h);
     TRY(dev_alloc(h, (void**)&h->slice_tab, 3 * (size_t)P * sizeof(int32_t)));
     const int32_t ntr = (int32_t)((N + BM - 1) / BM);
     TRY(dev_alloc(h, (void**)&h->krange, (size_t)ntr * sizeof(int2)));
@@ -214,7 +222,7 @@ int pfsm_create(pfsm_handle_t* out, int64_t N, int32_t P, int32_t window, int32_
 int pfsm_destroy(pfsm_handle_t h) {
     if (!h) return 0;
     cudaDeviceSynchronize();
-    void* ptrs[] = {h->W, h->S, h->O, h->Dinv, h->Gws, h->eps, h->resid, h->gdiag, h->rotcnt, h->slice_tab, h->krange, h->info,
+    void* ptrs[] = {h->W, h->S, h->O, h->Dinv, h->Gws, h->eps, h->resid, h->gdiag, h->rotcnt, h->nrm_g, h->slice_tab, h->krange, h->info,
                     h->A_stage, h->V_stage, h->lam_stage, h->Ap, h->LT, h->DinvT};
     for (void* p : ptrs)
         if (p) cudaFree(p);
@@ -256,8 +264,59 @@ static int launch_jacobi_t(pfsm_ctx* h, const double* A, double* V, cudaStream_t
 }
 }  // extern "C++"
 
+extern "C++" {
+template <int EPL>
+static int launch_jacobi_smem_t(pfsm_ctx* h, const double* A, double* V, cudaStream_t st) {
+    SliceTable tab{h->slice_tab, h->slice_tab + h->P, h->slice_tab + 2 * (size_t)h->P};
+    const size_t smem = jacobi_smem_bytes(h->M, h->jac_hloc);
+    static size_t attr_bytes = 0;  // static smem (~300 B) + dynamic must stay within the 227 KB opt-in limit
+    if (smem > attr_bytes) {
+        PFSM_CUDA(cudaFuncSetAttribute(jacobi_smem_kernel<EPL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        attr_bytes = smem;
+    }
+    cudaLaunchConfig_t cfg;
+    memset(&cfg, 0, sizeof(cfg));
+    cfg.gridDim = dim3((unsigned)(h->P * h->jac_cs));
+    cfg.blockDim = dim3(JACOBI_THREADS);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = (unsigned)h->jac_cs;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    PFSM_CUDA(cudaLaunchKernelEx(&cfg, jacobi_smem_kernel<EPL>, A, h->N, h->M, h->m, (int32_t)h->jac_hloc, tab,
+                                 h->nrm_g, V, h->eps, h->rotcnt, h->info));
+    return 0;
+}
+}  // extern "C++"
+
+// Shared-memory Jacobi layout: the smallest cluster whose CTAs can hold their 2 h_loc + 3 column slots, grown
+// while a CTA would still have more pairs than warps and the chip has SMs to spare.  0 = use the L2 kernel.
+static void choose_jacobi_layout(pfsm_ctx* h) {
+    h->jac_cs = 0;
+    h->jac_hloc = 0;
+    if (getenv("PFSM_JACOBI_L2")) return;  // diagnostic: force the L2-resident kernel (the large-M fallback)
+    const size_t budget = 220 * 1024;
+    auto hloc_of = [&](int cs) { return (h->M + 2 * cs - 1) / (2 * cs); };
+    int cs = 1;
+    for (; cs <= 8; cs *= 2)
+        if (hloc_of(cs) >= 2 && jacobi_smem_bytes(h->M, hloc_of(cs)) <= budget) break;
+    if (cs > 8 || hloc_of(cs) < 2) return;
+    while (cs < 8 && hloc_of(cs) > JACOBI_THREADS / 32 && 2 * cs * h->P <= 148 && hloc_of(2 * cs) >= 2) cs *= 2;
+    h->jac_cs = cs;
+    h->jac_hloc = hloc_of(cs);
+}
+
 static int launch_jacobi(pfsm_ctx* h, const double* A, double* V, cudaStream_t st) {
     PFSM_CUDA(cudaMemsetAsync(h->rotcnt, 0, (size_t)h->P * JACOBI_MAX_SWEEPS * sizeof(int), st));
+    if (h->jac_cs > 0) {
+        if (h->M <= 128) return launch_jacobi_smem_t<4>(h, A, V, st);
+        if (h->M <= 256) return launch_jacobi_smem_t<8>(h, A, V, st);
+        return launch_jacobi_smem_t<16>(h, A, V, st);
+    }
     if (h->M <= 128) return launch_jacobi_t<4>(h, A, V, st);
     if (h->M <= 256) return launch_jacobi_t<8>(h, A, V, st);
     return launch_jacobi_t<16>(h, A, V, st);

@@ -103,6 +103,18 @@ def test_stepwise_parity_small(N, P, w, iters, amp, width):
     assert np.all(np.diag(R) > 0)
 
 
+@pytest.mark.parametrize("N,P,w", [(256, 4, 16), (270, 6, 4), (600, 3, 20)])
+def test_l2_resident_jacobi_fallback_matches_oracle(N, P, w, monkeypatch):
+    # the L2-resident cluster kernel is the fallback for submatrices too large for shared memory; force it
+    monkeypatch.setenv("PFSM_JACOBI_L2", "1")
+    p = gen.small_problem(N, 1e-3, 12.0, seed=1000 + N)
+    g2 = gpu_solve(p.A, P, w, 1, p.alpha, last_step=2)
+    V2, eps, info2 = oracle.step2(p.A, P, w)
+    assert g2["info"] == 0 and info2 == 0
+    assert np.abs(g2["eps"] - eps).max() <= 1e-13 * max(1.0, p.normF)
+    assert np.abs(align_signs(g2["Vr"], V2) - V2).max() < 1e-9
+
+
 def test_iters_zero_is_gram_schmidt_of_start_vectors():
     p = gen.small_problem(288, 1e-3, 16.0, seed=77)
     g = gpu_solve(p.A, 4, 12, 0, p.alpha)
