@@ -270,7 +270,8 @@ def run_ours(args):
     orth = float((dVt @ dVt.T - torch.eye(N, dtype=torch.float64, device="cuda")).abs().max().item())
     del dVt
     quality = {"max_residual": float(resid.max()), "orthogonality_max": orth,
-               "trace_error": float(abs(lam.sum() - np.trace(prob.A))), "info": h.info()}
+               "trace_error": float(abs(lam.sum() - np.trace(prob.A))), "info": h.info(),
+               "step2_jacobi_sweeps": h.step2_sweeps()}
 
     if rank != 0:
         replicas.finalize(world)

@@ -137,6 +137,10 @@ int pfsm_destroy(pfsm_handle_t h);
  */
 int pfsm_get_info(pfsm_handle_t h, void* stream, int64_t* info);
 
+/* Largest number of Jacobi sweeps any slice's submatrix eigensolve (step 2) used in the last solve;
+ * synchronizes `stream`.  The last sweep is the one that found nothing left to rotate. */
+int pfsm_get_step2_sweeps(pfsm_handle_t h, void* stream, int32_t* max_sweeps);
+
 /* Device pointer to the N residual norms r_i = ||A v_i - lambda_i v_i||_2 of the last solve (step 5). */
 int pfsm_get_residuals(pfsm_handle_t h, const double** r_device);
 

@@ -20,7 +20,7 @@ CUDA_ERROR_BASE = 1000
 EXPORTS = [
     "pfsm_create", "pfsm_solve", "pfsm_solve_host", "pfsm_solve_partial", "pfsm_orthonormalize", "pfsm_rayleigh", "pfsm_solve_generalized",
     "pfsm_generalized_reduce", "pfsm_destroy", "pfsm_get_info",
-    "pfsm_get_residuals", "pfsm_get_shifts", "pfsm_set_alpha", "pfsm_workspace_bytes",
+    "pfsm_get_step2_sweeps", "pfsm_get_residuals", "pfsm_get_shifts", "pfsm_set_alpha", "pfsm_workspace_bytes",
     "pfsm_launches_per_solve", "pfsm_enable_step_timing", "pfsm_get_step_ms", "pfsm_probe_fp64_peak",
     "pfsm_strerror",
 ]
@@ -57,6 +57,7 @@ def load(build_if_missing: bool = True):
     lib.pfsm_generalized_reduce.argtypes = [p, p, p, p, p]
     lib.pfsm_destroy.argtypes = [p]
     lib.pfsm_get_info.argtypes = [p, p, ctypes.POINTER(i64)]
+    lib.pfsm_get_step2_sweeps.argtypes = [p, p, ctypes.POINTER(i32)]
     lib.pfsm_get_residuals.argtypes = [p, ctypes.POINTER(p)]
     lib.pfsm_get_shifts.argtypes = [p, ctypes.POINTER(p)]
     lib.pfsm_set_alpha.argtypes = [p, dbl]
@@ -174,6 +175,11 @@ class Handle:
                                         "version": 2}
 
         return torch.as_tensor(_DevBuf(), device="cuda").clone()
+
+    def step2_sweeps(self, stream=None) -> int:
+        v = ctypes.c_int32(0)
+        _check(self._lib.pfsm_get_step2_sweeps(self._h, _stream_ptr(stream), ctypes.byref(v)), "pfsm_get_step2_sweeps")
+        return int(v.value)
 
     def residuals(self):
         return self._view(self._lib.pfsm_get_residuals, "pfsm_get_residuals")

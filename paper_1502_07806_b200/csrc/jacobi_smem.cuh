@@ -68,11 +68,13 @@ jacobi_smem_kernel(const double* __restrict__ A, int64_t N, int32_t M, int32_t m
     const int RT = h_loc + 1;                   // ring size of a standard top ring and of every bottom ring
     const int RT0 = h_loc;                      // ring size of CTA 0's top ring
     int head_t = 0, head_t0 = 0, head_b = 0;    // identical on every CTA of every cluster (pure functions of the round)
+    // heads stay in [0, ring size) and seats in [0, h_loc], so one conditional subtraction replaces the modulo
+    auto wrap = [](int v, int ring) -> int { return v >= ring ? v - ring : v; };
     auto slot_top = [&](int t) -> int {
-        if (cr == 0) return t == 0 ? 0 : T0 + (head_t0 + t - 1) % RT0;
-        return T0 + (head_t + t) % RT;
+        if (cr == 0) return t == 0 ? 0 : T0 + wrap(head_t0 + t - 1, RT0);
+        return T0 + wrap(head_t + t, RT);
     };
-    auto slot_bot = [&](int t) -> int { return B0 + (head_b + t) % RT; };
+    auto slot_bot = [&](int t) -> int { return B0 + wrap(head_b + t, RT); };
 
     // ---- Gershgorin shift (every CTA computes the same sigma) ----
     double bound = 0.0;
@@ -115,7 +117,7 @@ jacobi_smem_kernel(const double* __restrict__ A, int64_t N, int32_t M, int32_t m
     const uint32_t cols_u32 = (uint32_t)__cvta_generic_to_shared(cols);
     const uint32_t ids_u32 = (uint32_t)__cvta_generic_to_shared(ids);
     const int nrounds = Mp - 1;
-    const double tol = 2.220446049250313e-16 * sqrt((double)M);
+    const double tol2 = 2.220446049250313e-16 * 2.220446049250313e-16 * (double)M;  // (sqrt(M) eps)^2
     bool converged = false;
     for (int sweep = 0; sweep < JACOBI_MAX_SWEEPS; ++sweep) {
         int nrot = 0;
@@ -138,11 +140,11 @@ jacobi_smem_kernel(const double* __restrict__ A, int64_t N, int32_t M, int32_t m
                 aa = warp_sum(aa);
                 bb = warp_sum(bb);
                 ab = warp_sum(ab);
-                const bool rotate = fabs(ab) > tol * sqrt(aa * bb);
+                const bool rotate = ab * ab > tol2 * (aa * bb);  // |g_p . g_q| > sqrt(M) eps ||g_p|| ||g_q||
                 if (rotate) {
                     const double zeta = (bb - aa) / (2.0 * ab);
-                    const double tt = copysign(1.0, zeta) / (fabs(zeta) + sqrt(1.0 + zeta * zeta));
-                    const double cs = 1.0 / sqrt(1.0 + tt * tt), sn = cs * tt;
+                    const double tt = copysign(1.0, zeta) / (fabs(zeta) + sqrt(fma(zeta, zeta, 1.0)));
+                    const double cs = rsqrt(fma(tt, tt, 1.0)), sn = cs * tt;
 #pragma unroll
                     for (int e = 0; e < EPL; ++e) {
                         const double xe = x[e], ye = y[e];
@@ -162,9 +164,9 @@ jacobi_smem_kernel(const double* __restrict__ A, int64_t N, int32_t M, int32_t m
                 if (top_leaves) {
                     if (cr < CS - 1) {
                         dst_cta = (uint32_t)(cr + 1);
-                        dst_slot = T0 + (head_t + RT - 1) % RT;
+                        dst_slot = T0 + wrap(head_t + RT - 1, RT);
                     } else {
-                        dst_slot = B0 + (head_b + h_loc) % RT;
+                        dst_slot = B0 + wrap(head_b + h_loc, RT);
                     }
                 }
                 if (top_leaves) {
@@ -188,9 +190,9 @@ jacobi_smem_kernel(const double* __restrict__ A, int64_t N, int32_t M, int32_t m
                     int bslot;
                     if (cr > 0) {
                         bcta = (uint32_t)(cr - 1);
-                        bslot = B0 + (head_b + h_loc) % RT;
+                        bslot = B0 + wrap(head_b + h_loc, RT);
                     } else {
-                        bslot = T0 + (head_t0 + RT0 - 1) % RT0;
+                        bslot = T0 + wrap(head_t0 + RT0 - 1, RT0);
                     }
                     const uint32_t base = mapa_shared(cols_u32 + (uint32_t)((size_t)bslot * M * 8), bcta);
 #pragma unroll
@@ -209,9 +211,9 @@ jacobi_smem_kernel(const double* __restrict__ A, int64_t N, int32_t M, int32_t m
             }
             if (rnd == nrounds - 1 && lane == 0 && nrot) atomicAdd(rot + sweep, nrot);
             if (CS > 1) cluster_sync_all(); else __syncthreads();
-            head_t = (head_t + RT - 1) % RT;
-            head_t0 = (head_t0 + RT0 - 1) % RT0;
-            head_b = (head_b + 1) % RT;
+            head_t = wrap(head_t + RT - 1, RT);
+            head_t0 = wrap(head_t0 + RT0 - 1, RT0);
+            head_b = wrap(head_b + 1, RT);
         }
         const int total = __ldcg(rot + sweep);
         if (total == 0) {

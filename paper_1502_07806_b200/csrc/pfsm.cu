@@ -616,6 +616,23 @@ int pfsm_get_info(pfsm_handle_t h, void* stream, int64_t* info) {
     return 0;
 }
 
+int pfsm_get_step2_sweeps(pfsm_handle_t h, void* stream, int32_t* max_sweeps) {
+    if (!h) return -1;
+    if (!max_sweeps) return -3;
+    std::vector<int> cnt((size_t)h->P * JACOBI_MAX_SWEEPS);
+    PFSM_CUDA(cudaMemcpyAsync(cnt.data(), h->rotcnt, cnt.size() * sizeof(int), cudaMemcpyDeviceToHost,
+                              (cudaStream_t)stream));
+    PFSM_CUDA(cudaStreamSynchronize((cudaStream_t)stream));
+    int mx = 0;
+    for (int s = 0; s < h->P; ++s) {
+        int k = 0;
+        while (k < JACOBI_MAX_SWEEPS && cnt[(size_t)s * JACOBI_MAX_SWEEPS + k] != 0) ++k;
+        mx = std::max(mx, std::min(k + 1, (int)JACOBI_MAX_SWEEPS));
+    }
+    *max_sweeps = mx;
+    return 0;
+}
+
 int pfsm_get_residuals(pfsm_handle_t h, const double** r) {
     if (!h) return -1;
     if (!r) return -2;
