@@ -17,6 +17,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include "gemm_tn.cuh"  // lds128
 #include "kernels.cuh"
 
 namespace pfsm {
@@ -29,14 +30,32 @@ __device__ __forceinline__ uint32_t mapa_shared(uint32_t addr, uint32_t cta) {
 __device__ __forceinline__ void st_cluster_f64(uint32_t addr, double v) {
     asm volatile("st.shared::cluster.f64 [%0], %1;" ::"r"(addr), "d"(v) : "memory");
 }
+__device__ __forceinline__ void st_cluster_v2f64(uint32_t addr, double2 v) {
+    asm volatile("st.shared::cluster.v2.f64 [%0], {%1,%2};" ::"r"(addr), "d"(v.x), "d"(v.y) : "memory");
+}
+// remote shared-memory store whose completion is counted (in bytes) on the destination CTA's mbarrier
+__device__ __forceinline__ void st_async_v2f64(uint32_t raddr, double2 v, uint32_t rmbar) {
+    asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v2.f64 [%0], {%1,%2}, [%3];" ::"r"(raddr),
+                 "d"(v.x), "d"(v.y), "r"(rmbar)
+                 : "memory");
+}
+__device__ __forceinline__ void st_async_s32(uint32_t raddr, int v, uint32_t rmbar) {
+    asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.s32 [%0], %1, [%2];" ::"r"(raddr), "r"(v),
+                 "r"(rmbar)
+                 : "memory");
+}
+__device__ __forceinline__ void sts128(uint32_t addr, double2 v) {
+    asm volatile("st.shared.v2.f64 [%0], {%1,%2};" ::"r"(addr), "d"(v.x), "d"(v.y) : "memory");
+}
 __device__ __forceinline__ void st_cluster_s32(uint32_t addr, int v) {
     asm volatile("st.shared::cluster.s32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
 }
 
 // bytes of dynamic shared memory for (M, h_loc): column slots + ids + norms/ranks scratch
+inline int jacobi_padded_rows(int M) { return (M + 63) / 64 * 64; }  // column slot length: whole double2 per lane
 inline size_t jacobi_smem_bytes(int M, int h_loc) {
     const size_t nslots = 2 * (size_t)h_loc + 3;
-    return nslots * M * sizeof(double) + nslots * sizeof(int) + 16 + (size_t)M * (sizeof(double) + sizeof(int)) + 64;
+    return (nslots + 4) * jacobi_padded_rows(M) * sizeof(double) + nslots * sizeof(int) + 16 + (size_t)M * (sizeof(double) + sizeof(int)) + 64;
 }
 
 template <int EPL>
@@ -50,17 +69,21 @@ jacobi_smem_kernel(const double* __restrict__ A, int64_t N, int32_t M, int32_t m
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     constexpr int NW = JACOBI_THREADS / 32;
     const int h = h_loc * CS, Mp = 2 * h;
+    constexpr int Ms = 32 * EPL, E2 = EPL / 2;  // padded column length (rows M..Ms-1 are zero and stay zero)
     int* rot = rotcnt + (size_t)s * JACOBI_MAX_SWEEPS;
     double* nrm_s = nrm_g + (size_t)s * Mp;  // global scratch: final column norms by column id
 
     extern __shared__ __align__(16) unsigned char smem_jac[];
     const int nslots = 2 * h_loc + 3;
-    double* cols = reinterpret_cast<double*>(smem_jac);                 // cols[slot][M]
-    int* ids = reinterpret_cast<int*>(cols + (size_t)nslots * M);       // column id held by each slot
+    double* cols = reinterpret_cast<double*>(smem_jac);                 // cols[slot][Ms]
+    double* stage = cols + (size_t)nslots * Ms;                          // 2 x 2 columns leaving for a neighbour CTA
+    int* ids = reinterpret_cast<int*>(stage + 4 * Ms);                   // column id held by each slot
     double* nrm = reinterpret_cast<double*>(ids + ((nslots + 3) & ~3)); // nrm[M], then rank[M]
     int* rank = reinterpret_cast<int*>(nrm + M);
     __shared__ double red[NW];
     __shared__ double s_sigma;
+    __shared__ __align__(8) unsigned long long mbar_in[2];  // [0]: top column from the left CTA, [1]: bottom from the right
+    __shared__ int stage_id[4];
 
     // slot map.  slot 0: the fixed column (used by CTA 0 only).  Top ring: slots T0 .. T0+h_loc (CTA 0 uses a
     // ring of h_loc slots for its h_loc-1 moving top seats).  Bottom ring: slots B0 .. B0+h_loc.
@@ -101,10 +124,10 @@ jacobi_smem_kernel(const double* __restrict__ A, int64_t N, int32_t M, int32_t m
         const int tl = is_top ? q : q - h_loc;
         const int cid = (is_top ? 0 : h) + cr * h_loc + tl;
         const int slot = is_top ? slot_top(tl) : slot_bot(tl);
-        double* dst = cols + (size_t)slot * M;
-        for (int r = lane; r < M; r += 32) {
+        double* dst = cols + (size_t)slot * Ms;
+        for (int r = lane; r < Ms; r += 32) {
             double v = 0.0;
-            if (cid < M) {
+            if (cid < M && r < M) {
                 v = A[(size_t)(lo + cid) * N + lo + r];
                 if (r == cid) v += sigma;
             }
@@ -112,8 +135,18 @@ jacobi_smem_kernel(const double* __restrict__ A, int64_t N, int32_t M, int32_t m
         }
         if (lane == 0) ids[slot] = cid;
     }
+    if (tid == 0) {
+        mbar_init((uint32_t)__cvta_generic_to_shared(&mbar_in[0]), 1);
+        mbar_init((uint32_t)__cvta_generic_to_shared(&mbar_in[1]), 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
     if (CS > 1) cluster_sync_all(); else __syncthreads();
 
+    const uint32_t mbar_u32 = (uint32_t)__cvta_generic_to_shared(&mbar_in[0]);
+    const uint32_t stage_u32 = (uint32_t)__cvta_generic_to_shared(stage);
+    const bool has_left = cr > 0, has_right = cr < CS - 1;  // neighbours that exchange a column with this CTA every round
+    const uint32_t col_tx = (uint32_t)(Ms * 8 + 4);       // bytes one incoming column (+ its id) completes on the mbarrier
+    uint32_t phase = 0;
     const uint32_t cols_u32 = (uint32_t)__cvta_generic_to_shared(cols);
     const uint32_t ids_u32 = (uint32_t)__cvta_generic_to_shared(ids);
     const int nrounds = Mp - 1;
@@ -122,34 +155,38 @@ jacobi_smem_kernel(const double* __restrict__ A, int64_t N, int32_t M, int32_t m
     for (int sweep = 0; sweep < JACOBI_MAX_SWEEPS; ++sweep) {
         int nrot = 0;
         for (int rnd = 0; rnd < nrounds; ++rnd) {
+            // staging buffers alternate with the round (a slow sender of round r cannot be overtaken by round r+1's writers)
+            const uint32_t stage_cur = stage_u32 + phase * (uint32_t)(2 * Ms * 8);
             for (int t = warp; t < h_loc; t += NW) {
                 const int sp = slot_top(t), sq = slot_bot(t);
-                double* gp = cols + (size_t)sp * M;
-                double* gq = cols + (size_t)sq * M;
-                double x[EPL], y[EPL];
+                const uint32_t ap = cols_u32 + (uint32_t)(sp * Ms * 8) + 16u * lane;
+                const uint32_t aq = cols_u32 + (uint32_t)(sq * Ms * 8) + 16u * lane;
+                double2 x[E2], y[E2];
                 double aa = 0.0, bb = 0.0, ab = 0.0;
 #pragma unroll
-                for (int e = 0; e < EPL; ++e) {
-                    const int r = lane + 32 * e;
-                    x[e] = (r < M) ? gp[r] : 0.0;
-                    y[e] = (r < M) ? gq[r] : 0.0;
-                    aa = fma(x[e], x[e], aa);
-                    bb = fma(y[e], y[e], bb);
-                    ab = fma(x[e], y[e], ab);
+                for (int e = 0; e < E2; ++e) {  // lane holds rows 2 (lane + 32 e), +1: conflict-free 16-byte accesses
+                    x[e] = lds128(ap + 512u * e);
+                    y[e] = lds128(aq + 512u * e);
+                    aa = fma(x[e].x, x[e].x, aa); aa = fma(x[e].y, x[e].y, aa);
+                    bb = fma(y[e].x, y[e].x, bb); bb = fma(y[e].y, y[e].y, bb);
+                    ab = fma(x[e].x, y[e].x, ab); ab = fma(x[e].y, y[e].y, ab);
                 }
                 aa = warp_sum(aa);
                 bb = warp_sum(bb);
                 ab = warp_sum(ab);
                 const bool rotate = ab * ab > tol2 * (aa * bb);  // |g_p . g_q| > sqrt(M) eps ||g_p|| ||g_q||
                 if (rotate) {
-                    const double zeta = (bb - aa) / (2.0 * ab);
-                    const double tt = copysign(1.0, zeta) / (fabs(zeta) + sqrt(fma(zeta, zeta, 1.0)));
+                    // t = tan(theta) = sign(zeta) / (|zeta| + sqrt(1 + zeta^2)), zeta = (bb - aa) / (2 ab), written
+                    // with one square root and one division: t = 2 ab sign(d) / (|d| + sqrt(d^2 + 4 ab^2)), d = bb - aa
+                    const double d = bb - aa;
+                    const double den = fabs(d) + sqrt(fma(d, d, 4.0 * ab * ab));
+                    const double tt = copysign(2.0 * ab, (d < 0.0) ? -ab : ab) / den;
                     const double cs = rsqrt(fma(tt, tt, 1.0)), sn = cs * tt;
 #pragma unroll
-                    for (int e = 0; e < EPL; ++e) {
-                        const double xe = x[e], ye = y[e];
-                        x[e] = cs * xe - sn * ye;
-                        y[e] = sn * xe + cs * ye;
+                    for (int e = 0; e < E2; ++e) {
+                        const double2 xe = x[e], ye = y[e];
+                        x[e].x = cs * xe.x - sn * ye.x; x[e].y = cs * xe.y - sn * ye.y;
+                        y[e].x = sn * xe.x + cs * ye.x; y[e].y = sn * xe.y + cs * ye.y;
                     }
                     ++nrot;
                 }
@@ -158,59 +195,72 @@ jacobi_smem_kernel(const double* __restrict__ A, int64_t N, int32_t M, int32_t m
                 const bool top_fixed = (cr == 0 && t == 0);
                 const bool top_leaves = (t == h_loc - 1) && !top_fixed;
                 const bool bot_leaves = (t == 0);
-                // destination of a leaving top column: right neighbour's top spare, or (last CTA) own bottom spare
-                uint32_t dst_cta = (uint32_t)cr;
-                int dst_slot = sp;
                 if (top_leaves) {
-                    if (cr < CS - 1) {
-                        dst_cta = (uint32_t)(cr + 1);
-                        dst_slot = T0 + wrap(head_t + RT - 1, RT);
-                    } else {
-                        dst_slot = B0 + wrap(head_b + h_loc, RT);
-                    }
-                }
-                if (top_leaves) {
-                    const uint32_t base = mapa_shared(cols_u32 + (uint32_t)((size_t)dst_slot * M * 8), dst_cta);
+                    if (has_right) {  // to the right neighbour's top spare: staged, sent after the CTA barrier below
 #pragma unroll
-                    for (int e = 0; e < EPL; ++e) {
-                        const int r = lane + 32 * e;
-                        if (r < M) st_cluster_f64(base + 8u * r, x[e]);
+                        for (int e = 0; e < E2; ++e) sts128(stage_cur + 16u * lane + 512u * e, x[e]);
+                        if (lane == 0) stage_id[2 * phase] = ids[sp];
+                    } else {          // last CTA: the column turns the corner into this CTA's bottom spare
+                        const int dslot = B0 + wrap(head_b + h_loc, RT);
+                        const uint32_t base = cols_u32 + (uint32_t)(dslot * Ms * 8) + 16u * lane;
+#pragma unroll
+                        for (int e = 0; e < E2; ++e) sts128(base + 512u * e, x[e]);
+                        if (lane == 0) ids[dslot] = ids[sp];
                     }
-                    if (lane == 0) st_cluster_s32(mapa_shared(ids_u32 + 4u * dst_slot, dst_cta), ids[sp]);
                 } else if (rotate) {
 #pragma unroll
-                    for (int e = 0; e < EPL; ++e) {
-                        const int r = lane + 32 * e;
-                        if (r < M) gp[r] = x[e];
-                    }
+                    for (int e = 0; e < E2; ++e) sts128(ap + 512u * e, x[e]);
                 }
-                // destination of a leaving bottom column: left neighbour's bottom spare, or (CTA 0) own top spare
                 if (bot_leaves) {
-                    uint32_t bcta = (uint32_t)cr;
-                    int bslot;
-                    if (cr > 0) {
-                        bcta = (uint32_t)(cr - 1);
-                        bslot = B0 + wrap(head_b + h_loc, RT);
-                    } else {
-                        bslot = T0 + wrap(head_t0 + RT0 - 1, RT0);
-                    }
-                    const uint32_t base = mapa_shared(cols_u32 + (uint32_t)((size_t)bslot * M * 8), bcta);
+                    if (has_left) {   // to the left neighbour's bottom spare: staged
 #pragma unroll
-                    for (int e = 0; e < EPL; ++e) {
-                        const int r = lane + 32 * e;
-                        if (r < M) st_cluster_f64(base + 8u * r, y[e]);
+                        for (int e = 0; e < E2; ++e) sts128(stage_cur + (uint32_t)(Ms * 8) + 16u * lane + 512u * e, y[e]);
+                        if (lane == 0) stage_id[2 * phase + 1] = ids[sq];
+                    } else {          // CTA 0: the column turns the corner into this CTA's top spare
+                        const int dslot = T0 + wrap(head_t0 + RT0 - 1, RT0);
+                        const uint32_t base = cols_u32 + (uint32_t)(dslot * Ms * 8) + 16u * lane;
+#pragma unroll
+                        for (int e = 0; e < E2; ++e) sts128(base + 512u * e, y[e]);
+                        if (lane == 0) ids[dslot] = ids[sq];
                     }
-                    if (lane == 0) st_cluster_s32(mapa_shared(ids_u32 + 4u * bslot, bcta), ids[sq]);
                 } else if (rotate) {
 #pragma unroll
-                    for (int e = 0; e < EPL; ++e) {
-                        const int r = lane + 32 * e;
-                        if (r < M) gq[r] = y[e];
-                    }
+                    for (int e = 0; e < E2; ++e) sts128(aq + 512u * e, y[e]);
                 }
             }
             if (rnd == nrounds - 1 && lane == 0 && nrot) atomicAdd(rot + sweep, nrot);
-            if (CS > 1) cluster_sync_all(); else __syncthreads();
+            // Every warp of this CTA is done reading and writing its seats; only now may the neighbours' spare
+            // slots be overwritten (they sent us their column of this round after their own barrier, so once it
+            // has arrived they are past all reads of the round too).  The exchange is point to point: st.async
+            // completes its bytes on the receiver's mbarrier, and nobody waits for CTAs it does not talk to.
+            __syncthreads();
+            if (CS > 1) {
+                if (warp == 0 && has_right) {
+                    const int dslot = T0 + wrap(head_t + RT - 1, RT);
+                    const uint32_t rbar = mapa_shared(mbar_u32, (uint32_t)(cr + 1));
+                    const uint32_t base = mapa_shared(cols_u32 + (uint32_t)(dslot * Ms * 8), (uint32_t)(cr + 1)) + 16u * lane;
+#pragma unroll
+                    for (int e = 0; e < E2; ++e) st_async_v2f64(base + 512u * e, lds128(stage_cur + 16u * lane + 512u * e), rbar);
+                    if (lane == 0) st_async_s32(mapa_shared(ids_u32 + 4u * dslot, (uint32_t)(cr + 1)), stage_id[2 * phase], rbar);
+                }
+                if (warp == 1 && has_left) {
+                    const int dslot = B0 + wrap(head_b + h_loc, RT);
+                    const uint32_t rbar = mapa_shared(mbar_u32 + 8u, (uint32_t)(cr - 1));
+                    const uint32_t base = mapa_shared(cols_u32 + (uint32_t)(dslot * Ms * 8), (uint32_t)(cr - 1)) + 16u * lane;
+#pragma unroll
+                    for (int e = 0; e < E2; ++e)
+                        st_async_v2f64(base + 512u * e, lds128(stage_cur + (uint32_t)(Ms * 8) + 16u * lane + 512u * e), rbar);
+                    if (lane == 0) st_async_s32(mapa_shared(ids_u32 + 4u * dslot, (uint32_t)(cr - 1)), stage_id[2 * phase + 1], rbar);
+                }
+                if (tid == 64) {
+                    if (has_left) mbar_expect_tx(mbar_u32, col_tx);
+                    if (has_right) mbar_expect_tx(mbar_u32 + 8u, col_tx);
+                }
+                if (has_left) mbar_wait(mbar_u32, phase);
+                if (has_right) mbar_wait(mbar_u32 + 8u, phase);
+                phase ^= 1u;
+                if (rnd == nrounds - 1) cluster_sync_all();  // once per sweep: every CTA's rotation count is in
+            }
             head_t = wrap(head_t + RT - 1, RT);
             head_t0 = wrap(head_t0 + RT0 - 1, RT0);
             head_b = wrap(head_b + 1, RT);
@@ -227,7 +277,7 @@ jacobi_smem_kernel(const double* __restrict__ A, int64_t N, int32_t M, int32_t m
     for (int q = warp; q < 2 * h_loc; q += NW) {
         const int slot = q < h_loc ? slot_top(q) : slot_bot(q - h_loc);
         const int cid = ids[slot];
-        const double* gc = cols + (size_t)slot * M;
+        const double* gc = cols + (size_t)slot * Ms;
         double ss = 0.0;
         for (int r = lane; r < M; r += 32) ss = fma(gc[r], gc[r], ss);
         ss = warp_sum(ss);
@@ -255,7 +305,7 @@ jacobi_smem_kernel(const double* __restrict__ A, int64_t N, int32_t M, int32_t m
         if (j < 0 || j >= m) continue;
         const double nv = nrm[cid];
         const double inv = 1.0 / nv;
-        const double* gc = cols + (size_t)slot * M;
+        const double* gc = cols + (size_t)slot * Ms;
         double* v = V + (size_t)(g0 + j) * N + lo;
         for (int r = lane; r < M; r += 32) v[r] = gc[r] * inv;
         if (lane == 0) eps[g0 + j] = nv - sigma;

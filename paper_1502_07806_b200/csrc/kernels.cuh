@@ -265,28 +265,35 @@ chol_diag_kernel(const double* __restrict__ S, double* __restrict__ Lout, int64_
     // ---------------- phase A: L ----------------
     for (int j0 = 0; j0 < CHOL_NB; j0 += 16) {
         if (warp == 0) {
-            const int i = j0 + lane;  // lanes 0..15 own rows j0..j0+15
+            // A1: the 16 x 16 diagonal block in registers, lane = row (lanes 16..31 carry zeros), columns exchanged
+            // with shuffles; fully unrolled, no shared-memory round trips on the serial chain.
+            const int i = j0 + (lane & 15);
+            double r[16];
+#pragma unroll
+            for (int c = 0; c < 16; ++c) r[c] = (lane < 16 && c <= lane) ? a[i * CHOL_LDS + j0 + c] : 0.0;
+#pragma unroll
             for (int j = 0; j < 16; ++j) {
-                const int jj = j0 + j;
-                double piv = a[jj * CHOL_LDS + jj];
-                if (!(piv > thr[jj]) || !(piv > 0.0)) {
-                    if (lane == 0) atomicMin(info, (unsigned long long)(k0 + jj + 1));
+                double piv = __shfl_sync(0xffffffffu, r[j], j);
+                if (!(piv > thr[j0 + j]) || !(piv > 0.0)) {
+                    if (lane == 0) atomicMin(info, (unsigned long long)(k0 + j0 + j + 1));
                     piv = 1.0;
                 }
-                const double d = sqrt(piv), rd = 1.0 / d;
-                __syncwarp();
-                if (lane == j) {
-                    a[jj * CHOL_LDS + jj] = d;
-                    idiag[jj] = rd;
-                } else if (lane > j && lane < 16) {
-                    a[i * CHOL_LDS + jj] *= rd;
+                double rd = rsqrt(piv);
+                double d = piv * rd;
+                d = fma(fma(-d, d, piv), 0.5 * rd, d);  // one Newton step: d = sqrt(piv) to the last bit or two
+                rd = fma(fma(-d, rd, 1.0), rd, rd);     // and rd = 1/d
+                r[j] = (lane == j) ? d : r[j] * rd;
+                if (lane == j) idiag[j0 + j] = rd;
+#pragma unroll
+                for (int c = j + 1; c < 16; ++c) {
+                    const double lc = __shfl_sync(0xffffffffu, r[j], c);  // l[c][j]
+                    r[c] = fma(-r[j], lc, r[c]);                          // meaningful for lanes >= c
                 }
-                __syncwarp();
-                if (lane > j && lane < 16) {
-                    const double lij = a[i * CHOL_LDS + jj];
-                    for (int c = jj + 1; c <= i; ++c) a[i * CHOL_LDS + c] -= lij * a[c * CHOL_LDS + jj];
-                }
-                __syncwarp();
+            }
+            if (lane < 16) {
+#pragma unroll
+                for (int c = 0; c < 16; ++c)
+                    if (c <= lane) a[i * CHOL_LDS + j0 + c] = r[c];
             }
         }
         __syncthreads();
@@ -338,19 +345,24 @@ chol_diag_kernel(const double* __restrict__ S, double* __restrict__ Lout, int64_
     for (int I = 1; I < 8; ++I) {  // B2: L^-1[I][J] = -L^-1[I][I] * sum_{J<=K<I} L[I][K] L^-1[K][J], all J < I at once
         for (int e = tid; e < I * 256; e += CHOL_THREADS) {
             const int J = e >> 8, rr = (e >> 4) & 15, cc = e & 15;
-            const double* lrow = a + (16 * I + rr) * CHOL_LDS;
-            double s0 = 0.0, s1 = 0.0;
-            for (int k = 16 * J + cc; k < 16 * I; k += 2) {  // L^-1[k][16J+cc] is zero for k < 16J+cc
-                s0 = fma(lrow[k], chol_linv(a, idiag, k, 16 * J + cc), s0);
-                if (k + 1 < 16 * I) s1 = fma(lrow[k + 1], chol_linv(a, idiag, k + 1, 16 * J + cc), s1);
+            const double* lrow = a + (16 * I + rr) * CHOL_LDS;     // L[16I+rr][.]
+            const double* icol = a + (16 * J + cc) * CHOL_LDS;     // L^-1[.][16J+cc], stored transposed
+            // block K = J: L^-1[16J+k][16J+cc] is idiag for k = cc, the stored entry for k > cc, zero for k < cc
+            double s0 = lrow[16 * J + cc] * idiag[16 * J + cc], s1 = 0.0;
+            for (int k = 16 * J + cc + 1; k < 16 * J + 16; ++k) s0 = fma(lrow[k], icol[k], s0);
+            // blocks J < K < I: plain dot product of a row of L with a stored column of L^-1
+            for (int k = 16 * J + 16; k < 16 * I; k += 2) {
+                s0 = fma(lrow[k], icol[k], s0);
+                s1 = fma(lrow[k + 1], icol[k + 1], s1);
             }
             T[e] = s0 + s1;
         }
         __syncthreads();
         for (int e = tid; e < I * 256; e += CHOL_THREADS) {
             const int J = e >> 8, rr = (e >> 4) & 15, cc = e & 15;
-            double s = 0.0;
-            for (int k = 0; k <= rr; ++k) s = fma(chol_linv(a, idiag, 16 * I + rr, 16 * I + k), T[J * 256 + k * 16 + cc], s);
+            // -L^-1[I][I] * T: row 16I+rr of the diagonal block's inverse (entries k < rr stored transposed, k = rr in idiag)
+            double s = idiag[16 * I + rr] * T[J * 256 + rr * 16 + cc];
+            for (int k = 0; k < rr; ++k) s = fma(a[(16 * I + k) * CHOL_LDS + 16 * I + rr], T[J * 256 + k * 16 + cc], s);
             a[(16 * J + cc) * CHOL_LDS + 16 * I + rr] = -s;
         }
         __syncthreads();

@@ -313,9 +313,16 @@ static void choose_jacobi_layout(pfsm_ctx* h) {
 static int launch_jacobi(pfsm_ctx* h, const double* A, double* V, cudaStream_t st) {
     PFSM_CUDA(cudaMemsetAsync(h->rotcnt, 0, (size_t)h->P * JACOBI_MAX_SWEEPS * sizeof(int), st));
     if (h->jac_cs > 0) {
-        if (h->M <= 128) return launch_jacobi_smem_t<4>(h, A, V, st);
-        if (h->M <= 256) return launch_jacobi_smem_t<8>(h, A, V, st);
-        return launch_jacobi_smem_t<16>(h, A, V, st);
+        switch (jacobi_padded_rows(h->M) / 32) {  // doubles per lane per column
+            case 2: return launch_jacobi_smem_t<2>(h, A, V, st);
+            case 4: return launch_jacobi_smem_t<4>(h, A, V, st);
+            case 6: return launch_jacobi_smem_t<6>(h, A, V, st);
+            case 8: return launch_jacobi_smem_t<8>(h, A, V, st);
+            case 10: return launch_jacobi_smem_t<10>(h, A, V, st);
+            case 12: return launch_jacobi_smem_t<12>(h, A, V, st);
+            case 14: return launch_jacobi_smem_t<14>(h, A, V, st);
+            default: return launch_jacobi_smem_t<16>(h, A, V, st);
+        }
     }
     if (h->M <= 128) return launch_jacobi_t<4>(h, A, V, st);
     if (h->M <= 256) return launch_jacobi_t<8>(h, A, V, st);
