@@ -122,6 +122,18 @@ int pfsm_solve_generalized(pfsm_handle_t h, const double* A, const double* S, do
                            void* stream);
 int pfsm_generalized_reduce(pfsm_handle_t h, const double* A, const double* S, double* Ap_out, void* stream);
 
+/*
+ * SCF-sequence mode ("a sequence of eigenvalue problems where the solution ... is similar but not
+ * identical to the solution from the previous iteration"; A must be diagonally dominant).
+ * V_inout holds, on input, the ORTHONORMAL eigenvectors V_prev of the previous step (e.g. from the last
+ * pfsm_solve_warm, or from a standard eigensolver for the first steps).  The call forms
+ * A' = V_prev^T A V_prev, runs steps 2-5 on A', and returns V = V_prev U (orthonormal) and lambda.  Residuals
+ * are those of (A, V).  Costs three more N^3 products than pfsm_solve; 2 N^2 doubles more workspace on first use.
+ * If get_info != 0 or the residuals are large, A was not close enough to the previous step: fall back to a
+ * standard eigensolver for this step.
+ */
+int pfsm_solve_warm(pfsm_handle_t h, const double* A, double* V_inout, double* lambda_out, void* stream);
+
 /* Release the handle and its workspace (synchronizes the device).  NULL is a no-op returning 0. */
 int pfsm_destroy(pfsm_handle_t h);
 

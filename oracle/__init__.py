@@ -165,3 +165,18 @@ def generalized_back(L, Vr):
     Xr = np.empty((N, N))
     _load().oracle_generalized_back(N, Lr.ctypes.data, Vr.ctypes.data, Xr.ctypes.data)
     return Xr
+
+
+def pfsm_warm(A, Vr_prev, P: int, w: int, iters: int, alpha: float):
+    """SCF-sequence mode: the previous step's orthonormal eigenvectors V_prev (rows of
+    Vr_prev) make A' = V_prev^T A V_prev diagonally dominant; PFSM (O1..O5) runs on A', and the vectors are
+    rotated back, V = V_prev U.  The two changes of basis are plain FP64 matrix products (library primitive)."""
+    A = _f64(A)
+    Vp = _f64(Vr_prev)
+    Ap = Vp @ A @ Vp.T
+    Ap = 0.5 * (Ap + Ap.T)
+    r = pfsm(Ap, P, w, iters, alpha)
+    r["Ur"] = r["Vr"]
+    r["Vr"] = r["Ur"] @ Vp
+    r["Ap"] = Ap
+    return r

@@ -19,7 +19,7 @@ CUDA_ERROR_BASE = 1000
 
 EXPORTS = [
     "pfsm_create", "pfsm_solve", "pfsm_solve_host", "pfsm_solve_partial", "pfsm_orthonormalize", "pfsm_rayleigh", "pfsm_solve_generalized",
-    "pfsm_generalized_reduce", "pfsm_destroy", "pfsm_get_info",
+    "pfsm_generalized_reduce", "pfsm_solve_warm", "pfsm_destroy", "pfsm_get_info",
     "pfsm_get_step2_sweeps", "pfsm_get_residuals", "pfsm_get_shifts", "pfsm_set_alpha", "pfsm_workspace_bytes",
     "pfsm_launches_per_solve", "pfsm_enable_step_timing", "pfsm_get_step_ms", "pfsm_probe_fp64_peak",
     "pfsm_strerror",
@@ -55,6 +55,7 @@ def load(build_if_missing: bool = True):
     lib.pfsm_rayleigh.argtypes = [p, p, p, p, p]
     lib.pfsm_solve_generalized.argtypes = [p, p, p, p, p, p]
     lib.pfsm_generalized_reduce.argtypes = [p, p, p, p, p]
+    lib.pfsm_solve_warm.argtypes = [p, p, p, p, p]
     lib.pfsm_destroy.argtypes = [p]
     lib.pfsm_get_info.argtypes = [p, p, ctypes.POINTER(i64)]
     lib.pfsm_get_step2_sweeps.argtypes = [p, p, ctypes.POINTER(i32)]
@@ -153,6 +154,12 @@ class Handle:
         _check(self._lib.pfsm_generalized_reduce(self._h, _dev_ptr(A, N, (N, N), "A"), _dev_ptr(S, N, (N, N), "S"),
                                                  _dev_ptr(Ap, N, (N, N), "Ap"), _stream_ptr(stream)),
                "pfsm_generalized_reduce")
+
+    def solve_warm(self, A, Vr, lam, stream=None):
+        """SCF-sequence mode: Vr holds the previous step's orthonormal eigenvectors on input."""
+        N = self.N
+        _check(self._lib.pfsm_solve_warm(self._h, _dev_ptr(A, N, (N, N), "A"), _dev_ptr(Vr, N, (N, N), "V"),
+                                         _dev_ptr(lam, N, (N,), "lambda"), _stream_ptr(stream)), "pfsm_solve_warm")
 
     def solve_host(self, A_host, Vr_host, lam_host, stream=None):
         N = self.N

@@ -241,6 +241,47 @@ gemm_tn_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__
 
     // ===== epilogue: thread owns C[row0 + 8 i + g][col0 + 8 j + 2 t + {0,1}] =====
     const int32_t row0 = tr * BM + wr * 64, col0 = tc * BN + wc * 32;
+    if (EPI != EPI_PLAIN && (tr + 1) * BM <= p.mr && (tc + 1) * BN <= p.nc) {
+        // Interior tile: no bounds checks, and the epilogue operands are fetched 16 x 16 bytes at a time before
+        // they are used -- 2 memory round trips per thread instead of 32 dependent load -> store chains.
+        const int64_t base = ((int64_t)p.cr0 + row0 + g) * p.ldc + p.cc0 + col0 + 2 * t;  // ldc == ld1 == ld2 here
+#pragma unroll
+        for (int ib = 0; ib < 8; ib += 4) {
+            double2 u[4][4], w[4][4];
+            double e[4];
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                const int64_t o = base + (int64_t)(8 * (ib + i)) * p.ldc;
+                if (EPI == EPI_SHIFT || EPI == EPI_UPDATE) e[i] = p.eps[(int64_t)p.cr0 + row0 + 8 * (ib + i) + g];
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    if (EPI == EPI_SHIFT || EPI == EPI_UPDATE) u[i][j] = *reinterpret_cast<const double2*>(p.E1 + o + 8 * j);
+                    if (EPI == EPI_UPDATE) w[i][j] = *reinterpret_cast<const double2*>(p.E2 + o + 8 * j);
+                    if (EPI == EPI_SUB) w[i][j] = *reinterpret_cast<const double2*>(p.C + o + 8 * j);
+                }
+            }
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                const int64_t o = base + (int64_t)(8 * (ib + i)) * p.ldc;
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    double v0 = acc[ib + i][j][0], v1 = acc[ib + i][j][1];
+                    if (EPI == EPI_SHIFT) {
+                        v0 -= e[i] * u[i][j].x;
+                        v1 -= e[i] * u[i][j].y;
+                    } else if (EPI == EPI_UPDATE) {
+                        v0 = w[i][j].x - p.alpha * (v0 - e[i] * u[i][j].x);
+                        v1 = w[i][j].y - p.alpha * (v1 - e[i] * u[i][j].y);
+                    } else {
+                        v0 = w[i][j].x - v0;
+                        v1 = w[i][j].y - v1;
+                    }
+                    *reinterpret_cast<double2*>(p.C + o + 8 * j) = make_double2(v0, v1);
+                }
+            }
+        }
+        return;
+    }
 #pragma unroll
     for (int i = 0; i < 8; ++i) {
         const int32_t r = row0 + 8 * i + g;

@@ -588,6 +588,47 @@ int pfsm_solve_generalized(pfsm_handle_t h, const double* A, const double* S, do
     return run_generalized_back(h, X_out, st);
 }
 
+// ---- SCF-sequence mode: A is the subspace matrix of a step whose solution is close to the
+// previous one.  With the previous eigenvectors V_prev (orthonormal), A' = V_prev^T A V_prev is diagonally dominant
+// -- the method's condition for success -- so PFSM runs on A' and the result is rotated back: V = V_prev U. ----
+int pfsm_solve_warm(pfsm_handle_t h, const double* A, double* V_inout, double* lambda_out, void* stream) {
+    if (!h) return -1;
+    if (!A || ((uintptr_t)A & 15)) return -2;
+    if (!V_inout || ((uintptr_t)V_inout & 15)) return -3;
+    if (!lambda_out || ((uintptr_t)lambda_out & 7)) return -4;
+    int rc;
+    if ((rc = ensure_generalized(h))) return rc;  // Ap and LT double as A' and V_prev^T
+    cudaStream_t st = (cudaStream_t)stream;
+    const int64_t N = h->N;
+    const int32_t n = (int32_t)N;
+    CUtensorMap mapA, mapV;
+    if ((rc = make_map(&mapA, A, N, N, N))) return rc;
+    if ((rc = make_map(&mapV, V_inout, N, N, N))) return rc;
+    const dim3 tb(32, 8), tg((unsigned)((N + 31) / 32), (unsigned)((N + 31) / 32));
+    {   // W = V_prev A  (row-major view: row i = (A v_i)^T)
+        GemmParams p = base_params();
+        p.C = h->W; p.ldc = N; p.mr = n; p.nc = n; p.klen = n;
+        if ((rc = launch_gemm<EPI_PLAIN>(mapV, mapA, h->mapW, p, st))) return rc;
+    }
+    {   // A'[i][j] = v_i . (A v_j), into S's top half, then symmetrized into Ap
+        GemmParams p = base_params();
+        p.C = h->S; p.ldc = N; p.mr = n; p.nc = n; p.klen = n;
+        if ((rc = launch_gemm<EPI_PLAIN>(mapV, h->mapW, h->mapS, p, st))) return rc;
+        symmetrize_kernel<<<tg, tb, 0, st>>>(h->S, N, h->Ap, N, n);
+        PFSM_CUDA(cudaGetLastError());
+    }
+    transpose_kernel<<<tg, tb, 0, st>>>(V_inout, N, h->LT, N, n, n);  // V_prev^T, K-contiguous for the rotation back
+    PFSM_CUDA(cudaGetLastError());
+    if ((rc = pfsm_solve_partial(h, h->Ap, V_inout, lambda_out, stream, 5))) return rc;  // U, lambda
+    {   // V = V_prev U: row i of the result = sum_k U[i][k] V_prev[k][:]
+        GemmParams p = base_params();
+        p.C = h->W; p.ldc = N; p.mr = n; p.nc = n; p.klen = n;
+        if ((rc = launch_gemm<EPI_PLAIN>(mapV, h->mapLT, h->mapW, p, st))) return rc;
+    }
+    PFSM_CUDA(cudaMemcpyAsync(V_inout, h->W, (size_t)N * N * sizeof(double), cudaMemcpyDeviceToDevice, st));
+    return 0;
+}
+
 int pfsm_solve(pfsm_handle_t h, const double* A, double* V_inout, double* lambda_out, void* stream) {
     return pfsm_solve_partial(h, A, V_inout, lambda_out, stream, 5);
 }

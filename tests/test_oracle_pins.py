@@ -382,3 +382,50 @@ def test_generalized_reduce_flags_indefinite_overlap():
     S[2, 2] = -1.0
     _, _, info = oracle.generalized_reduce(np.eye(4), S)
     assert info == 3
+
+
+# ---------------------------------------------------------------- SCF-sequence mode
+def test_warm_start_identity_basis_is_plain_pfsm():
+    N, P, w = 48, 4, 5
+    p = gen.small_problem(N, 0.01, 5.0, seed=81)
+    a = oracle.pfsm(p.A, P, w, 2, p.alpha)
+    b = oracle.pfsm_warm(p.A, np.eye(N), P, w, 2, p.alpha)
+    assert np.array_equal(a["lam"], b["lam"]) and np.array_equal(a["Vr"], b["Vr"])
+
+
+def test_warm_start_with_exact_previous_eigenvectors_is_exact():
+    # V_prev = eigenvectors of A itself -> A' is diagonal -> fixed point of every step (P1), for ANY dense A:
+    # this is the paper's point that a good previous solution makes the method applicable.
+    N, P, w = 40, 4, 3
+    d = np.sort(gen.uniform(82, gen.STREAM_TEST, 0, N) * 2 - 1)
+    X = gen.normal(82, gen.STREAM_TEST, 10_000, N * N).reshape(N, N)
+    Q, _ = np.linalg.qr(X)
+    A = (Q * d) @ Q.T
+    A = 0.5 * (A + A.T)
+    lam0, V0 = np.linalg.eigh(A)
+    r = oracle.pfsm_warm(A, V0.T.copy(), P, w, 2, 0.5)
+    assert r["info"] == 0
+    np.testing.assert_allclose(r["lam"], lam0, atol=1e-13)
+    assert np.abs(r["Vr"] @ r["Vr"].T - np.eye(N)).max() < 1e-13
+    assert np.abs(r["Vr"] @ A - r["lam"][:, None] * r["Vr"]).max() < 1e-13
+
+
+def test_warm_start_tracks_a_slowly_changing_matrix():
+    # a sequence A_k = A_0 + k dA with dense small dA: each step starts from the previous step's vectors
+    N, P, w = 64, 4, 8
+    d = np.sort(gen.uniform(83, gen.STREAM_TEST, 0, N) * 2 - 1)
+    X = gen.normal(83, gen.STREAM_TEST, 10_000, N * N).reshape(N, N)
+    Q, _ = np.linalg.qr(X)
+    A0 = (Q * d) @ Q.T
+    dA = gen.normal(83, gen.STREAM_TEST, 50_000, N * N).reshape(N, N) * 2e-4
+    dA = 0.5 * (dA + dA.T)
+    _, V = np.linalg.eigh(0.5 * (A0 + A0.T))
+    Vr = V.T.copy()
+    for k in range(1, 4):
+        Ak = 0.5 * (A0 + A0.T) + k * dA
+        r = oracle.pfsm_warm(Ak, Vr, P, w, 3, 0.5)
+        assert r["info"] == 0
+        ex = np.linalg.eigvalsh(Ak)
+        assert np.abs(np.sort(r["lam"]) - ex).max() < 1e-5
+        assert abs(r["lam"].sum() - np.trace(Ak)) < 1e-12          # P7 for the rotated basis too
+        Vr = r["Vr"]
