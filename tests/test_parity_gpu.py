@@ -425,3 +425,77 @@ def test_generalized_config4g_properties():
     h.solve(dAp, dV, dl2)
     assert torch.equal(dl, dl2)
     h.destroy()
+
+
+# ------------------------------------------------------------------ SCF-sequence mode (pfsm_solve_warm)
+def gpu_warm(A, Vr_prev, P, w, iters, alpha):
+    N = A.shape[0]
+    h = pfsm.Handle(N, P, w, iters, alpha)
+    dA, dV = dev(A), dev(Vr_prev)
+    dl = torch.empty((N,), dtype=torch.float64, device="cuda")
+    h.solve_warm(dA, dV, dl)
+    out = dict(Vr=dV.cpu().numpy(), lam=dl.cpu().numpy(), resid=h.residuals().cpu().numpy(), info=h.info())
+    h.destroy()
+    return out
+
+
+def test_warm_start_sequence_matches_oracle():
+    N, P, w, iters = 384, 4, 24, 3
+    d = np.sort(gen.uniform(83, gen.STREAM_TEST, 0, N) * 2 - 1)
+    X = gen.normal(83, gen.STREAM_TEST, 10_000, N * N).reshape(N, N)
+    Q, _ = np.linalg.qr(X)
+    A0 = (Q * d) @ Q.T
+    A0 = 0.5 * (A0 + A0.T)
+    dA = gen.normal(83, gen.STREAM_TEST, 500_000, N * N).reshape(N, N) * 5e-5
+    dA = 0.5 * (dA + dA.T)
+    _, V = np.linalg.eigh(A0)       # "standard diagonalization for the first SCF steps"
+    Vg = Vo = V.T.copy()
+    for k in range(1, 4):
+        Ak = A0 + k * dA
+        nF = float(np.linalg.norm(Ak))
+        g = gpu_warm(Ak, Vg, P, w, iters, 0.5)
+        o = oracle.pfsm_warm(Ak, Vo, P, w, iters, 0.5)
+        assert g["info"] == 0 and o["info"] == 0
+        assert np.abs(g["lam"] - o["lam"]).max() <= 1e-10 * nF
+        assert np.abs(g["resid"] - o["resid"]).max() <= 1e-9 * nF
+        assert np.abs(g["Vr"] @ g["Vr"].T - np.eye(N)).max() <= 1e-12 * N
+        assert np.abs(align_signs(g["Vr"], o["Vr"]) - o["Vr"]).max() < 1e-8
+        # residuals are those of (A_k, V): the change of basis is orthogonal
+        R = g["Vr"] @ Ak - g["lam"][:, None] * g["Vr"]
+        assert np.abs(np.linalg.norm(R, axis=1) - g["resid"]).max() < 1e-11
+        Vg, Vo = g["Vr"], o["Vr"]
+
+
+def test_warm_start_identity_basis_equals_plain_solve():
+    p = gen.problem(0)
+    c = p.cfg
+    g = gpu_warm(p.A, np.eye(c.N), c.P, c.window, c.iters, p.alpha)
+    ref = gpu_solve(p.A, c.P, c.window, c.iters, p.alpha)
+    assert np.abs(g["lam"] - ref["lam"]).max() < 1e-14 and np.abs(g["Vr"] - ref["Vr"]).max() < 1e-13
+
+
+def test_solve_is_cuda_graph_capturable():
+    # the whole solve enqueues kernels and memsets only (no host sync): capture once, replay many times
+    p = gen.problem(0)
+    c = p.cfg
+    N = c.N
+    h = pfsm.Handle(N, c.P, c.window, c.iters, p.alpha)
+    dA = dev(p.A)
+    dV = torch.empty((N, N), dtype=torch.float64, device="cuda")
+    dl = torch.empty((N,), dtype=torch.float64, device="cuda")
+    st = torch.cuda.Stream()
+    with torch.cuda.stream(st):
+        h.solve(dA, dV, dl, stream=st)      # warm-up: one-time function attributes are set outside the capture
+    st.synchronize()
+    ref_l, ref_V = dl.clone(), dV.clone()
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph, stream=st):
+        h.solve(dA, dV, dl, stream=torch.cuda.current_stream())
+    for _ in range(3):
+        dV.fill_(float("nan"))
+        dl.fill_(float("nan"))
+        graph.replay()
+        torch.cuda.synchronize()
+        assert torch.equal(dl, ref_l) and torch.equal(dV, ref_V)
+    assert h.info() == 0
+    h.destroy()
