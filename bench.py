@@ -351,7 +351,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=4, help="BASELINE.json config index (default 4: N=8192)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--cpu-cols", type=int, default=24, help="eigenvectors in the cpu_baseline sample")
+    ap.add_argument("--cpu-cols", type=int, default=128, help="eigenvectors in the cpu_baseline sample")
     ap.add_argument("--ref-cols", type=int, default=8, help="eigenvectors per step of --impl reference")
     ap.add_argument("--no-syevd", dest="syevd", action="store_false")
     ap.add_argument("--no-calibrate", dest="calibrate", action="store_false")

@@ -134,6 +134,18 @@ int pfsm_generalized_reduce(pfsm_handle_t h, const double* A, const double* S, d
  */
 int pfsm_solve_warm(pfsm_handle_t h, const double* A, double* V_inout, double* lambda_out, void* stream);
 
+/*
+ * The paper's own generalized -> standard conversion (section V, Eq. 14-15): Z = B^-1 A by
+ * the column-parallel iteration  Z_0 = A,  Z_{n+1} = Z_n - D^-1 (B Z_n - A),  D = diag(B)  (Eq. 14 prints
+ * "D^-1 A x"; the matrix iteration is meant), niter times; one fused GEMM per iteration.
+ *   A, B    device, N x N, symmetric; B diagonally dominant (the iteration converges iff rho(I - D^-1 B) < 1)
+ *   Z_out   device, N x N, column-major.  symmetrize != 0 returns (Z + Z^T)/2, the matrix "used in Eq. (3)";
+ *           symmetrize == 0 returns Z itself (not symmetric in general).
+ * Compare pfsm_generalized_reduce, which reduces by Cholesky(B) instead.
+ */
+int pfsm_standard_form_eq14(pfsm_handle_t h, const double* A, const double* B, double* Z_out, int32_t niter,
+                            int32_t symmetrize, void* stream);
+
 /* Release the handle and its workspace (synchronizes the device).  NULL is a no-op returning 0. */
 int pfsm_destroy(pfsm_handle_t h);
 

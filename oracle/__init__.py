@@ -55,6 +55,8 @@ def _load():
         lib.oracle_generalized_reduce.restype = i64
         lib.oracle_generalized_back.argtypes = [i64, p, p, p]
         lib.oracle_generalized_back.restype = None
+        lib.oracle_eq14_iteration.argtypes = [i64, p, p, i64, p]
+        lib.oracle_eq14_iteration.restype = None
         lib.oracle_num_threads.restype = ctypes.c_int
         _lib = lib
     return _lib
@@ -180,3 +182,14 @@ def pfsm_warm(A, Vr_prev, P: int, w: int, iters: int, alpha: float):
     r["Vr"] = r["Ur"] @ Vp
     r["Ap"] = Ap
     return r
+
+
+def eq14_iteration(A, B, niter: int, symmetrize: bool = False):
+    """f2 (Eq. 14-15): Z_0 = A, Z <- Z - D^-1 (B Z - A), niter times.  Returns Z as a numpy
+    matrix (Z[i, j]); symmetrize=True returns (Z + Z^T)/2, the matrix "used in Eq. (3)" (reading R19)."""
+    A, B = _f64(A), _f64(B)
+    N = A.shape[0]
+    Zc = np.empty((N, N))  # column-major Z == C-order Z^T; A, B symmetric so their layout is immaterial
+    _load().oracle_eq14_iteration(N, A.ctypes.data, B.ctypes.data, niter, Zc.ctypes.data)
+    Z = Zc.T.copy()
+    return 0.5 * (Z + Z.T) if symmetrize else Z

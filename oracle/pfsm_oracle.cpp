@@ -18,6 +18,7 @@
  *   O4 oracle_step4_mgs      PAPER.md:94-96 ("Gram-Schmidt orthogonalization")
  *   O5 oracle_step5          north_star step 5 (paper silent, reading R11): Rayleigh quotients
  *   OG oracle_generalized_*  BASELINE.json configs[4] / PAPER.md:171-173 (Eq. 13)
+ *   f2 oracle_eq14_iteration PAPER.md:173-185 (Eq. 14-15: Z = B^-1 A by a column-parallel iteration)
  *
  * Pins (tests/test_oracle_pins.py, -m "not gpu"): P1 diagonal input, P2 slice-aligned block
  * diagonal, P3 P=1 / window >= N vs numpy eigh, P4 known spectrum Q diag(d) Q^T, P5 closed-form
@@ -328,6 +329,31 @@ void oracle_generalized_back(int64_t N, const double* L, const double* V, double
             for (int64_t r = i + 1; r < N; ++r) s -= L[r + i * N] * x[r];
             x[i] = s / L[i + i * N];
         }
+    }
+}
+
+/* ---------------------------------------------------------------------------------------------
+ * f2  The paper's generalized -> standard conversion (Eq. 14-15; reading R19:
+ * Eq. 14 prints "D^-1 A x" where the matrix iteration needs D^-1 A).  D = diag(B);
+ *     Z_0 = A   ("the identity serves as a good initial approximation" of B^-1)
+ *     Z_{n+1} = (I - D^-1 B) Z_n + D^-1 A = Z_n - D^-1 (B Z_n - A),        niter times.
+ * "The individual columns of Z can be computed independently": one column at a time.
+ * Z: N x N column-major output (not symmetric in general).
+ * ------------------------------------------------------------------------------------------- */
+void oracle_eq14_iteration(int64_t N, const double* A, const double* B, int64_t niter, double* Z) {
+#pragma omp parallel for schedule(static)
+    for (int64_t c = 0; c < N; ++c) {
+        std::vector<double> z(N), r(N);
+        for (int64_t i = 0; i < N; ++i) z[i] = A[i + c * N];
+        for (int64_t it = 0; it < niter; ++it) {
+            for (int64_t i = 0; i < N; ++i) {
+                double sum = 0.0;
+                for (int64_t k = 0; k < N; ++k) sum += B[i + k * N] * z[k];
+                r[i] = sum - A[i + c * N];
+            }
+            for (int64_t i = 0; i < N; ++i) z[i] -= r[i] / B[i + i * N];
+        }
+        for (int64_t i = 0; i < N; ++i) Z[i + c * N] = z[i];
     }
 }
 

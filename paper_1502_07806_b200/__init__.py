@@ -19,7 +19,8 @@ CUDA_ERROR_BASE = 1000
 
 EXPORTS = [
     "pfsm_create", "pfsm_solve", "pfsm_solve_host", "pfsm_solve_partial", "pfsm_orthonormalize", "pfsm_rayleigh", "pfsm_solve_generalized",
-    "pfsm_generalized_reduce", "pfsm_solve_warm", "pfsm_destroy", "pfsm_get_info",
+    "pfsm_generalized_reduce", "pfsm_solve_warm", "pfsm_standard_form_eq14",
+    "pfsm_destroy", "pfsm_get_info",
     "pfsm_get_step2_sweeps", "pfsm_get_residuals", "pfsm_get_shifts", "pfsm_set_alpha", "pfsm_workspace_bytes",
     "pfsm_launches_per_solve", "pfsm_enable_step_timing", "pfsm_get_step_ms", "pfsm_probe_fp64_peak",
     "pfsm_strerror",
@@ -56,6 +57,7 @@ def load(build_if_missing: bool = True):
     lib.pfsm_solve_generalized.argtypes = [p, p, p, p, p, p]
     lib.pfsm_generalized_reduce.argtypes = [p, p, p, p, p]
     lib.pfsm_solve_warm.argtypes = [p, p, p, p, p]
+    lib.pfsm_standard_form_eq14.argtypes = [p, p, p, p, i32, i32, p]
     lib.pfsm_destroy.argtypes = [p]
     lib.pfsm_get_info.argtypes = [p, p, ctypes.POINTER(i64)]
     lib.pfsm_get_step2_sweeps.argtypes = [p, p, ctypes.POINTER(i32)]
@@ -160,6 +162,12 @@ class Handle:
         N = self.N
         _check(self._lib.pfsm_solve_warm(self._h, _dev_ptr(A, N, (N, N), "A"), _dev_ptr(Vr, N, (N, N), "V"),
                                          _dev_ptr(lam, N, (N,), "lambda"), _stream_ptr(stream)), "pfsm_solve_warm")
+
+    def standard_form_eq14(self, A, B, Z, niter: int, symmetrize: bool = True, stream=None):
+        N = self.N
+        _check(self._lib.pfsm_standard_form_eq14(self._h, _dev_ptr(A, N, (N, N), "A"), _dev_ptr(B, N, (N, N), "B"),
+                                                 _dev_ptr(Z, N, (N, N), "Z"), niter, int(symmetrize),
+                                                 _stream_ptr(stream)), "pfsm_standard_form_eq14")
 
     def solve_host(self, A_host, Vr_host, lam_host, stream=None):
         N = self.N

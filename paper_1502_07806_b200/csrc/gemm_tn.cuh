@@ -41,6 +41,7 @@ enum Epilogue : int {
     EPI_SHIFT = 1,   // C = acc - eps[i] * E1[i][j]                      (W = A V - V diag(eps))
     EPI_UPDATE = 2,  // C = E2[i][j] - alpha * (acc - eps[i] * E1[i][j])  (V <- V - alpha (A W - W diag(eps)))
     EPI_SUB = 3,     // C = C - acc                                       (trailing update)
+    EPI_JSTEP = 4,   // C = E2[i][j] - (acc - E1[i][j]) * eps[j]           (Eq. 14: Z <- Z - D^-1 (B Z - A), eps = 1/diag(B) per COLUMN)
 };
 
 struct GemmParams {
@@ -61,7 +62,7 @@ struct GemmParams {
     int64_t ld1;
     const double* E2;
     int64_t ld2;
-    const double* eps;  // indexed by absolute C row
+    const double* eps;  // indexed by absolute C row (SHIFT, UPDATE) or absolute C column (JSTEP)
     double alpha;
 };
 
@@ -188,7 +189,7 @@ gemm_tn_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__
         const int32_t npre = nk < GEMM_PREFETCH ? nk : GEMM_PREFETCH;
         for (int32_t j = 0; j < npre; ++j) issue(j);
     }
-    if ((EPI == EPI_SUB || EPI == EPI_UPDATE) && threadIdx.x == 32) {
+    if ((EPI == EPI_SUB || EPI == EPI_UPDATE || EPI == EPI_JSTEP) && threadIdx.x == 32) {
         // the epilogue reads the C tile: pull it from HBM into L2 now, under the main loop (mapC describes C)
 #pragma unroll
         for (int j = 0; j < BN / BK; ++j)
@@ -245,6 +246,11 @@ gemm_tn_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__
         // Interior tile: no bounds checks, and the epilogue operands are fetched 16 x 16 bytes at a time before
         // they are used -- 2 memory round trips per thread instead of 32 dependent load -> store chains.
         const int64_t base = ((int64_t)p.cr0 + row0 + g) * p.ldc + p.cc0 + col0 + 2 * t;  // ldc == ld1 == ld2 here
+        double2 dj[4];
+        if (EPI == EPI_JSTEP) {
+#pragma unroll
+            for (int j = 0; j < 4; ++j) dj[j] = *reinterpret_cast<const double2*>(p.eps + p.cc0 + col0 + 8 * j + 2 * t);
+        }
 #pragma unroll
         for (int ib = 0; ib < 8; ib += 4) {
             double2 u[4][4], w[4][4];
@@ -255,8 +261,9 @@ gemm_tn_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__
                 if (EPI == EPI_SHIFT || EPI == EPI_UPDATE) e[i] = p.eps[(int64_t)p.cr0 + row0 + 8 * (ib + i) + g];
 #pragma unroll
                 for (int j = 0; j < 4; ++j) {
-                    if (EPI == EPI_SHIFT || EPI == EPI_UPDATE) u[i][j] = *reinterpret_cast<const double2*>(p.E1 + o + 8 * j);
-                    if (EPI == EPI_UPDATE) w[i][j] = *reinterpret_cast<const double2*>(p.E2 + o + 8 * j);
+                    if (EPI == EPI_SHIFT || EPI == EPI_UPDATE || EPI == EPI_JSTEP)
+                        u[i][j] = *reinterpret_cast<const double2*>(p.E1 + o + 8 * j);
+                    if (EPI == EPI_UPDATE || EPI == EPI_JSTEP) w[i][j] = *reinterpret_cast<const double2*>(p.E2 + o + 8 * j);
                     if (EPI == EPI_SUB) w[i][j] = *reinterpret_cast<const double2*>(p.C + o + 8 * j);
                 }
             }
@@ -272,6 +279,9 @@ gemm_tn_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__
                     } else if (EPI == EPI_UPDATE) {
                         v0 = w[i][j].x - p.alpha * (v0 - e[i] * u[i][j].x);
                         v1 = w[i][j].y - p.alpha * (v1 - e[i] * u[i][j].y);
+                    } else if (EPI == EPI_JSTEP) {
+                        v0 = w[i][j].x - (v0 - u[i][j].x) * dj[j].x;
+                        v1 = w[i][j].y - (v1 - u[i][j].y) * dj[j].y;
                     } else {
                         v0 = w[i][j].x - v0;
                         v1 = w[i][j].y - v1;
@@ -315,6 +325,11 @@ gemm_tn_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__
                     v1 = y.y - p.alpha * (v1 - e * x.y);
                 } else
                     v0 = e2[0] - p.alpha * (v0 - e * e1[0]);
+            } else if (EPI == EPI_JSTEP) {
+                const double* e1 = p.E1 + ar * p.ld1 + ac;
+                const double* e2 = p.E2 + ar * p.ld2 + ac;
+                v0 = e2[0] - (v0 - e1[0]) * p.eps[ac];
+                if (pair) v1 = e2[1] - (v1 - e1[1]) * p.eps[ac + 1];
             } else if (EPI == EPI_SUB) {
                 if (pair) {
                     const double2 y = *reinterpret_cast<const double2*>(cp);

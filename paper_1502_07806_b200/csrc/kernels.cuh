@@ -227,6 +227,12 @@ __global__ void extract_diag_kernel(const double* __restrict__ S, int64_t ld, in
     if (i < n) gdiag[i] = S[(size_t)i * ld + i];
 }
 
+// dinv[i] = 1 / B[i][i]  (Eq. 14: D = diag(B))
+__global__ void inv_diag_kernel(const double* __restrict__ B, int64_t ld, int32_t n, double* __restrict__ dinv) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) dinv[i] = 1.0 / B[(size_t)i * ld + i];
+}
+
 // A pivot counts as "not positive" when it is <= CHOL_BREAKDOWN * (its original diagonal entry ||v_j||^2):
 // below that the projected vector has lost 6 digits to its predecessors and single-pass Cholesky-QR
 // (orthogonality error ~ eps * cond(V)^2) can no longer deliver orthonormal vectors.

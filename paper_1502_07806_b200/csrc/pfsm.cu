@@ -7,6 +7,7 @@
 #include <cuda.h>
 #include <cuda_runtime.h>
 
+#include <algorithm>
 #include <climits>
 #include <cmath>
 #include <cstdio>
@@ -112,7 +113,7 @@ static int launch_gemm(const CUtensorMap& mx, const CUtensorMap& my, const CUten
     if (p.mr <= 0 || p.nc <= 0) return 0;
     const int64_t tiles = gemm_num_tiles(p.ntr, p.ntc, p.lower);
     if (tiles <= 0) return 0;
-    static bool attr_set[4] = {false, false, false, false};
+    static bool attr_set[5] = {false, false, false, false, false};
     if (!attr_set[EPI]) {
         PFSM_CUDA(cudaFuncSetAttribute(gemm_tn_kernel<EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, GEMM_SMEM));
         attr_set[EPI] = true;
@@ -626,6 +627,51 @@ int pfsm_solve_warm(pfsm_handle_t h, const double* A, double* V_inout, double* l
         if ((rc = launch_gemm<EPI_PLAIN>(mapV, h->mapLT, h->mapW, p, st))) return rc;
     }
     PFSM_CUDA(cudaMemcpyAsync(V_inout, h->W, (size_t)N * N * sizeof(double), cudaMemcpyDeviceToDevice, st));
+    return 0;
+}
+
+// ---- f2: the paper's own generalized -> standard conversion (Eq. 14-15; reading R19):
+//      Z_0 = A (the identity approximates B^-1),  Z_{n+1} = Z_n - D^-1 (B Z_n - A),  D = diag(B).
+// Columns of Z are independent (one block of N/P columns per node in the paper); here all N columns are one
+// GEMM per iteration with the update fused in the epilogue.  Works on Y = Z^T (A, B symmetric):
+//      Y_{n+1}[j][i] = Y_n[j][i] - (sum_k Y_n[j][k] B[i][k] - A[j][i]) / B[i][i].
+int pfsm_standard_form_eq14(pfsm_handle_t h, const double* A, const double* B, double* Z_out, int32_t niter,
+                            int32_t symmetrize, void* stream) {
+    if (!h) return -1;
+    if (!A || ((uintptr_t)A & 15)) return -2;
+    if (!B || ((uintptr_t)B & 15)) return -3;
+    if (!Z_out || ((uintptr_t)Z_out & 15)) return -4;
+    if (niter < 0) return -5;
+    cudaStream_t st = (cudaStream_t)stream;
+    const int64_t N = h->N;
+    const int32_t n = (int32_t)N;
+    const size_t n2 = (size_t)N * N * sizeof(double);
+    int rc;
+    CUtensorMap mapB;
+    if ((rc = make_map(&mapB, B, N, N, N))) return rc;
+    inv_diag_kernel<<<(unsigned)((N + 255) / 256), 256, 0, st>>>(B, N, n, h->gdiag);
+    PFSM_CUDA(cudaGetLastError());
+    double* cur = h->W;       // Y_n
+    double* nxt = h->S;       // Y_{n+1} (top half of S)
+    const CUtensorMap* mcur = &h->mapW;
+    const CUtensorMap* mnxt = &h->mapS;
+    PFSM_CUDA(cudaMemcpyAsync(cur, A, n2, cudaMemcpyDeviceToDevice, st));
+    for (int it = 0; it < niter; ++it) {
+        GemmParams p = base_params();
+        p.C = nxt; p.ldc = N; p.mr = n; p.nc = n; p.klen = n;
+        p.E1 = A; p.ld1 = N; p.E2 = cur; p.ld2 = N; p.eps = h->gdiag;
+        if ((rc = launch_gemm<EPI_JSTEP>(*mcur, mapB, *mnxt, p, st))) return rc;
+        std::swap(cur, nxt);
+        std::swap(mcur, mnxt);
+    }
+    if (symmetrize) {
+        const dim3 tb(32, 8), tg((unsigned)((N + 31) / 32), (unsigned)((N + 31) / 32));
+        symmetrize_kernel<<<tg, tb, 0, st>>>(cur, N, Z_out, N, n);   // (Y + Y^T)/2 = (Z + Z^T)/2
+    } else {
+        // column-major Z is the same memory as row-major Y = Z^T
+        PFSM_CUDA(cudaMemcpyAsync(Z_out, cur, n2, cudaMemcpyDeviceToDevice, st));
+    }
+    PFSM_CUDA(cudaGetLastError());
     return 0;
 }
 

@@ -429,3 +429,38 @@ def test_warm_start_tracks_a_slowly_changing_matrix():
         assert np.abs(np.sort(r["lam"]) - ex).max() < 1e-5
         assert abs(r["lam"].sum() - np.trace(Ak)) < 1e-12          # P7 for the rotated basis too
         Vr = r["Vr"]
+
+
+# ---------------------------------------------------------------- f2: Eq. 14-15
+def test_eq14_identity_overlap_is_a_fixed_point():
+    N = 20
+    p = gen.small_problem(N, 0.1, 4.0, seed=91)
+    for niter in (0, 1, 4):
+        assert np.array_equal(oracle.eq14_iteration(p.A, np.eye(N), niter), p.A)
+
+
+def test_eq14_diagonal_overlap_converges_in_one_step():
+    # B = D diagonal: Z_1 = A - D^-1 (D A - A) = D^-1 A exactly (up to rounding), and stays there
+    N = 16
+    p = gen.small_problem(N, 0.1, 4.0, seed=92)
+    dd = 1.0 + gen.uniform(92, gen.STREAM_TEST, 0, N)
+    want = p.A / dd[:, None]
+    np.testing.assert_allclose(oracle.eq14_iteration(p.A, np.diag(dd), 1), want, atol=1e-15)
+    np.testing.assert_allclose(oracle.eq14_iteration(p.A, np.diag(dd), 3), want, atol=1e-15)
+
+
+def test_eq14_error_contracts_with_the_jacobi_iteration_matrix():
+    # Z_n - B^-1 A = (I - D^-1 B)^n (Z_0 - B^-1 A): closed form of the stationary iteration (Eq. 15 at the
+    # fixed point gives B Z = A).  A sign error, D^-1 on the wrong side, or Z_0 = I all fail this.
+    N = 24
+    p = gen.small_problem(N, 0.1, 4.0, seed=93)
+    B = gen.banded_symmetric(N, np.ones(N), 2e-2, 5.0, 93, gen.STREAM_S)
+    exact = np.linalg.solve(B, p.A)
+    Mj = np.eye(N) - B / np.diag(B)[:, None]
+    for n in (1, 2, 5):
+        want = exact + np.linalg.matrix_power(Mj, n) @ (p.A - exact)
+        np.testing.assert_allclose(oracle.eq14_iteration(p.A, B, n), want, atol=1e-14)
+    Z = oracle.eq14_iteration(p.A, B, 40)
+    assert np.abs(B @ Z - p.A).max() < 1e-14
+    Zs = oracle.eq14_iteration(p.A, B, 40, symmetrize=True)
+    assert np.array_equal(Zs, Zs.T)

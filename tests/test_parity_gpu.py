@@ -499,3 +499,38 @@ def test_solve_is_cuda_graph_capturable():
         assert torch.equal(dl, ref_l) and torch.equal(dV, ref_V)
     assert h.info() == 0
     h.destroy()
+
+
+# ------------------------------------------------------------------ f2: the paper's Eq. 14-15 conversion
+@pytest.mark.parametrize("N,niter", [(256, 1), (300, 3), (384, 6)])
+def test_eq14_iteration_matches_oracle(N, niter):
+    p = gen.small_problem(N, 2e-3, 12.0, seed=900 + N)
+    B = gen.banded_symmetric(N, np.ones(N), 1e-2, 6.0, 900 + N, gen.STREAM_S)
+    h = pfsm.Handle(N, 1, 0, 0, 1.0)
+    dZ = torch.empty((N, N), dtype=torch.float64, device="cuda")
+    h.standard_form_eq14(dev(p.A), dev(B), dZ, niter, symmetrize=False)
+    Zg = dZ.cpu().numpy().T                     # column-major Z -> numpy Z[i, j]
+    Zo = oracle.eq14_iteration(p.A, B, niter)
+    assert np.abs(Zg - Zo).max() < 1e-13 * max(1.0, np.abs(Zo).max())
+    h.standard_form_eq14(dev(p.A), dev(B), dZ, niter, symmetrize=True)
+    Zs = dZ.cpu().numpy()
+    assert np.array_equal(Zs, Zs.T)
+    assert np.abs(Zs - oracle.eq14_iteration(p.A, B, niter, symmetrize=True)).max() < 1e-13
+    h.destroy()
+
+
+def test_eq14_converges_to_the_cholesky_route_on_config4g_shape():
+    # both conversions feed the same standard eigenproblem when S is close to I: B^-1 A (symmetrized) and
+    # L^-1 A L^-T have the same spectrum up to O(||S - I||^2) -- information, checked loosely
+    N = 512
+    p = gen.small_problem(N, 2e-3, 32.0, seed=77)
+    S = gen.banded_symmetric(N, np.ones(N), 1e-4, 128.0, 77, gen.STREAM_S)
+    h = pfsm.Handle(N, 4, 32, 2, p.alpha)
+    dZ = torch.empty((N, N), dtype=torch.float64, device="cuda")
+    h.standard_form_eq14(dev(p.A), dev(S), dZ, 8, symmetrize=False)
+    Z = dZ.cpu().numpy().T
+    assert np.abs(S @ Z - p.A).max() < 1e-14      # Eq. 15: B Z = A at convergence
+    import scipy.linalg
+    ex = scipy.linalg.eigh(p.A, S, eigvals_only=True)
+    assert np.abs(np.sort(np.linalg.eigvals(Z).real) - ex).max() < 1e-10
+    h.destroy()
