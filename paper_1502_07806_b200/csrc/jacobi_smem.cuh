@@ -39,6 +39,11 @@ __device__ __forceinline__ void st_async_v2f64(uint32_t raddr, double2 v, uint32
                  "d"(v.x), "d"(v.y), "r"(rmbar)
                  : "memory");
 }
+__device__ __forceinline__ void st_async_f64(uint32_t raddr, double v, uint32_t rmbar) {
+    asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.f64 [%0], %1, [%2];" ::"r"(raddr), "d"(v),
+                 "r"(rmbar)
+                 : "memory");
+}
 __device__ __forceinline__ void st_async_s32(uint32_t raddr, int v, uint32_t rmbar) {
     asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.s32 [%0], %1, [%2];" ::"r"(raddr), "r"(v),
                  "r"(rmbar)
@@ -72,7 +77,7 @@ __device__ __forceinline__ double fast_rcp_pos(double x) {
 inline int jacobi_padded_rows(int M) { return (M + 63) / 64 * 64; }  // column slot length: whole double2 per lane
 inline size_t jacobi_smem_bytes(int M, int h_loc) {
     const size_t nslots = 2 * (size_t)h_loc + 3;
-    return (nslots + 4) * jacobi_padded_rows(M) * sizeof(double) + nslots * sizeof(int) + 16 + (size_t)M * (sizeof(double) + sizeof(int)) + 64;
+    return (nslots + 4) * jacobi_padded_rows(M) * sizeof(double) + nslots * sizeof(double) + nslots * sizeof(int) + 16 + (size_t)M * (sizeof(double) + sizeof(int)) + 64;
 }
 
 template <int EPL>
@@ -94,13 +99,15 @@ jacobi_smem_kernel(const double* __restrict__ A, int64_t N, int32_t M, int32_t m
     const int nslots = 2 * h_loc + 3;
     double* cols = reinterpret_cast<double*>(smem_jac);                 // cols[slot][Ms]
     double* stage = cols + (size_t)nslots * Ms;                          // 2 x 2 columns leaving for a neighbour CTA
-    int* ids = reinterpret_cast<int*>(stage + 4 * Ms);                   // column id held by each slot
+    double* nrm2 = stage + 4 * Ms;                                       // squared norm of the column in each slot
+    int* ids = reinterpret_cast<int*>(nrm2 + nslots);                    // column id held by each slot
     double* nrm = reinterpret_cast<double*>(ids + ((nslots + 3) & ~3)); // nrm[M], then rank[M]
     int* rank = reinterpret_cast<int*>(nrm + M);
     __shared__ double red[NW];
     __shared__ double s_sigma;
     __shared__ __align__(8) unsigned long long mbar_in[2];  // [0]: top column from the left CTA, [1]: bottom from the right
     __shared__ int stage_id[4];
+    __shared__ double stage_n2[4];
 
     // slot map.  slot 0: the fixed column (used by CTA 0 only).  Top ring: slots T0 .. T0+h_loc (CTA 0 uses a
     // ring of h_loc slots for its h_loc-1 moving top seats).  Bottom ring: slots B0 .. B0+h_loc.
@@ -162,7 +169,8 @@ jacobi_smem_kernel(const double* __restrict__ A, int64_t N, int32_t M, int32_t m
     const uint32_t mbar_u32 = (uint32_t)__cvta_generic_to_shared(&mbar_in[0]);
     const uint32_t stage_u32 = (uint32_t)__cvta_generic_to_shared(stage);
     const bool has_left = cr > 0, has_right = cr < CS - 1;  // neighbours that exchange a column with this CTA every round
-    const uint32_t col_tx = (uint32_t)(Ms * 8 + 4);       // bytes one incoming column (+ its id) completes on the mbarrier
+    const uint32_t col_tx = (uint32_t)(Ms * 8 + 8 + 4);   // bytes one incoming column (+ its squared norm and id) completes
+    const uint32_t nrm2_u32 = (uint32_t)__cvta_generic_to_shared(nrm2);
     uint32_t phase = 0;
     const uint32_t cols_u32 = (uint32_t)__cvta_generic_to_shared(cols);
     const uint32_t ids_u32 = (uint32_t)__cvta_generic_to_shared(ids);
@@ -180,17 +188,33 @@ jacobi_smem_kernel(const double* __restrict__ A, int64_t N, int32_t M, int32_t m
                 const uint32_t aq = cols_u32 + (uint32_t)(sq * Ms * 8) + 16u * lane;
                 double2 x[E2], y[E2];
                 double aa = 0.0, bb = 0.0, ab = 0.0;
+                // Squared column norms travel with the columns and are updated analytically after a rotation
+                // (||x'||^2 = aa - t ab, ||y'||^2 = bb + t ab); they are recomputed from the data in the first round of
+                // every sweep, so rounding drift is bounded by one sweep.  They only steer the rotation angle and the
+                // convergence test; the eigenvalues come from norms recomputed at the end.
+                if (rnd == 0) {
 #pragma unroll
-                for (int e = 0; e < E2; ++e) {  // lane holds rows 2 (lane + 32 e), +1: conflict-free 16-byte accesses
-                    x[e] = lds128(ap + 512u * e);
-                    y[e] = lds128(aq + 512u * e);
-                    aa = fma(x[e].x, x[e].x, aa); aa = fma(x[e].y, x[e].y, aa);
-                    bb = fma(y[e].x, y[e].x, bb); bb = fma(y[e].y, y[e].y, bb);
-                    ab = fma(x[e].x, y[e].x, ab); ab = fma(x[e].y, y[e].y, ab);
+                    for (int e = 0; e < E2; ++e) {  // lane holds rows 2 (lane + 32 e), +1: conflict-free 16-byte accesses
+                        x[e] = lds128(ap + 512u * e);
+                        y[e] = lds128(aq + 512u * e);
+                        aa = fma(x[e].x, x[e].x, aa); aa = fma(x[e].y, x[e].y, aa);
+                        bb = fma(y[e].x, y[e].x, bb); bb = fma(y[e].y, y[e].y, bb);
+                        ab = fma(x[e].x, y[e].x, ab); ab = fma(x[e].y, y[e].y, ab);
+                    }
+                    aa = warp_sum(aa);
+                    bb = warp_sum(bb);
+                    ab = warp_sum(ab);
+                } else {
+#pragma unroll
+                    for (int e = 0; e < E2; ++e) {
+                        x[e] = lds128(ap + 512u * e);
+                        y[e] = lds128(aq + 512u * e);
+                        ab = fma(x[e].x, y[e].x, ab); ab = fma(x[e].y, y[e].y, ab);
+                    }
+                    ab = warp_sum(ab);
+                    aa = nrm2[sp];
+                    bb = nrm2[sq];
                 }
-                aa = warp_sum(aa);
-                bb = warp_sum(bb);
-                ab = warp_sum(ab);
                 const bool rotate = ab * ab > tol2 * (aa * bb);  // |g_p . g_q| > sqrt(M) eps ||g_p|| ||g_q||
                 if (rotate) {
                     // t = tan(theta) = sign(zeta) / (|zeta| + sqrt(1 + zeta^2)), zeta = (bb - aa) / (2 ab), written
@@ -206,6 +230,8 @@ jacobi_smem_kernel(const double* __restrict__ A, int64_t N, int32_t M, int32_t m
                         x[e].x = cs * xe.x - sn * ye.x; x[e].y = cs * xe.y - sn * ye.y;
                         y[e].x = sn * xe.x + cs * ye.x; y[e].y = sn * xe.y + cs * ye.y;
                     }
+                    aa = fma(-tt, ab, aa);
+                    bb = fma(tt, ab, bb);
                     ++nrot;
                 }
                 // where do the two columns sit next round?  top[t] -> top[t+1] (same slot) unless it is the
@@ -217,33 +243,39 @@ jacobi_smem_kernel(const double* __restrict__ A, int64_t N, int32_t M, int32_t m
                     if (has_right) {  // to the right neighbour's top spare: staged, sent after the CTA barrier below
 #pragma unroll
                         for (int e = 0; e < E2; ++e) sts128(stage_cur + 16u * lane + 512u * e, x[e]);
-                        if (lane == 0) stage_id[2 * phase] = ids[sp];
+                        if (lane == 0) { stage_id[2 * phase] = ids[sp]; stage_n2[2 * phase] = aa; }
                     } else {          // last CTA: the column turns the corner into this CTA's bottom spare
                         const int dslot = B0 + wrap(head_b + h_loc, RT);
                         const uint32_t base = cols_u32 + (uint32_t)(dslot * Ms * 8) + 16u * lane;
 #pragma unroll
                         for (int e = 0; e < E2; ++e) sts128(base + 512u * e, x[e]);
-                        if (lane == 0) ids[dslot] = ids[sp];
+                        if (lane == 0) { ids[dslot] = ids[sp]; nrm2[dslot] = aa; }
                     }
-                } else if (rotate) {
+                } else {
+                    if (rotate) {
 #pragma unroll
-                    for (int e = 0; e < E2; ++e) sts128(ap + 512u * e, x[e]);
+                        for (int e = 0; e < E2; ++e) sts128(ap + 512u * e, x[e]);
+                    }
+                    if (lane == 0 && (rotate || rnd == 0)) nrm2[sp] = aa;
                 }
                 if (bot_leaves) {
                     if (has_left) {   // to the left neighbour's bottom spare: staged
 #pragma unroll
                         for (int e = 0; e < E2; ++e) sts128(stage_cur + (uint32_t)(Ms * 8) + 16u * lane + 512u * e, y[e]);
-                        if (lane == 0) stage_id[2 * phase + 1] = ids[sq];
+                        if (lane == 0) { stage_id[2 * phase + 1] = ids[sq]; stage_n2[2 * phase + 1] = bb; }
                     } else {          // CTA 0: the column turns the corner into this CTA's top spare
                         const int dslot = T0 + wrap(head_t0 + RT0 - 1, RT0);
                         const uint32_t base = cols_u32 + (uint32_t)(dslot * Ms * 8) + 16u * lane;
 #pragma unroll
                         for (int e = 0; e < E2; ++e) sts128(base + 512u * e, y[e]);
-                        if (lane == 0) ids[dslot] = ids[sq];
+                        if (lane == 0) { ids[dslot] = ids[sq]; nrm2[dslot] = bb; }
                     }
-                } else if (rotate) {
+                } else {
+                    if (rotate) {
 #pragma unroll
-                    for (int e = 0; e < E2; ++e) sts128(aq + 512u * e, y[e]);
+                        for (int e = 0; e < E2; ++e) sts128(aq + 512u * e, y[e]);
+                    }
+                    if (lane == 0 && (rotate || rnd == 0)) nrm2[sq] = bb;
                 }
             }
             if (rnd == nrounds - 1 && lane == 0 && nrot) atomicAdd(rot + sweep, nrot);
@@ -259,7 +291,10 @@ jacobi_smem_kernel(const double* __restrict__ A, int64_t N, int32_t M, int32_t m
                     const uint32_t base = mapa_shared(cols_u32 + (uint32_t)(dslot * Ms * 8), (uint32_t)(cr + 1)) + 16u * lane;
 #pragma unroll
                     for (int e = 0; e < E2; ++e) st_async_v2f64(base + 512u * e, lds128(stage_cur + 16u * lane + 512u * e), rbar);
-                    if (lane == 0) st_async_s32(mapa_shared(ids_u32 + 4u * dslot, (uint32_t)(cr + 1)), stage_id[2 * phase], rbar);
+                    if (lane == 0) {
+                        st_async_s32(mapa_shared(ids_u32 + 4u * dslot, (uint32_t)(cr + 1)), stage_id[2 * phase], rbar);
+                        st_async_f64(mapa_shared(nrm2_u32 + 8u * dslot, (uint32_t)(cr + 1)), stage_n2[2 * phase], rbar);
+                    }
                 }
                 if (warp == 1 && has_left) {
                     const int dslot = B0 + wrap(head_b + h_loc, RT);
@@ -268,7 +303,10 @@ jacobi_smem_kernel(const double* __restrict__ A, int64_t N, int32_t M, int32_t m
 #pragma unroll
                     for (int e = 0; e < E2; ++e)
                         st_async_v2f64(base + 512u * e, lds128(stage_cur + (uint32_t)(Ms * 8) + 16u * lane + 512u * e), rbar);
-                    if (lane == 0) st_async_s32(mapa_shared(ids_u32 + 4u * dslot, (uint32_t)(cr - 1)), stage_id[2 * phase + 1], rbar);
+                    if (lane == 0) {
+                        st_async_s32(mapa_shared(ids_u32 + 4u * dslot, (uint32_t)(cr - 1)), stage_id[2 * phase + 1], rbar);
+                        st_async_f64(mapa_shared(nrm2_u32 + 8u * dslot, (uint32_t)(cr - 1)), stage_n2[2 * phase + 1], rbar);
+                    }
                 }
                 if (tid == 64) {
                     if (has_left) mbar_expect_tx(mbar_u32, col_tx);
