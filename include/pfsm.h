@@ -146,6 +146,23 @@ int pfsm_solve_warm(pfsm_handle_t h, const double* A, double* V_inout, double* l
 int pfsm_standard_form_eq14(pfsm_handle_t h, const double* A, const double* B, double* Z_out, int32_t niter,
                             int32_t symmetrize, void* stream);
 
+/*
+ * One solve sharded over `world` GPUs (one process and one handle per GPU; the paper's decomposition of slices
+ * over nodes, with its all-gather).  Rank g owns slices [g P/world, (g+1) P/world),
+ * i.e. columns [g N/world, (g+1) N/world) of V.  Requires P % world == 0 and (N/world) % 128 == 0.  A is
+ * replicated.  pfsm_shard_phase runs compute phase 1..4 on the rank's share; between the phases the CALLER
+ * all-gathers (NCCL/torch.distributed; see paper_1502_07806_b200/sharded.py):
+ *   after phase 1 (steps 2-3 on own columns):   the column blocks of V                  (V itself, N x N)
+ *   after phase 2 (own block of V^T V):          the blocks of pfsm_shard_buffer(h, 0)   (N x N)
+ *   after phase 3 (Cholesky + own share of the triangular solve): blocks of pfsm_shard_buffer(h, 1) (N x N)
+ *   after phase 4 (V assembled, step 5 on own columns): the blocks of lambda_out (and of the residuals)
+ * Every buffer is split into `world` equal contiguous blocks of N/world columns (column-major), rank g's first.
+ * A may be NULL in phases 2-3, lambda_out in phases 1-3.  get_info reports as for pfsm_solve.
+ */
+int pfsm_set_shard(pfsm_handle_t h, int32_t rank, int32_t world);
+int pfsm_shard_phase(pfsm_handle_t h, int32_t phase, const double* A, double* V, double* lambda_out, void* stream);
+int pfsm_shard_buffer(pfsm_handle_t h, int32_t which, double** device_ptr);
+
 /* Release the handle and its workspace (synchronizes the device).  NULL is a no-op returning 0. */
 int pfsm_destroy(pfsm_handle_t h);
 

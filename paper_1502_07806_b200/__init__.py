@@ -20,7 +20,7 @@ CUDA_ERROR_BASE = 1000
 EXPORTS = [
     "pfsm_create", "pfsm_solve", "pfsm_solve_host", "pfsm_solve_partial", "pfsm_orthonormalize", "pfsm_rayleigh", "pfsm_solve_generalized",
     "pfsm_generalized_reduce", "pfsm_solve_warm", "pfsm_standard_form_eq14",
-    "pfsm_destroy", "pfsm_get_info",
+    "pfsm_set_shard", "pfsm_shard_phase", "pfsm_shard_buffer", "pfsm_destroy", "pfsm_get_info",
     "pfsm_get_step2_sweeps", "pfsm_get_residuals", "pfsm_get_shifts", "pfsm_set_alpha", "pfsm_workspace_bytes",
     "pfsm_launches_per_solve", "pfsm_enable_step_timing", "pfsm_get_step_ms", "pfsm_probe_fp64_peak",
     "pfsm_strerror",
@@ -58,6 +58,9 @@ def load(build_if_missing: bool = True):
     lib.pfsm_generalized_reduce.argtypes = [p, p, p, p, p]
     lib.pfsm_solve_warm.argtypes = [p, p, p, p, p]
     lib.pfsm_standard_form_eq14.argtypes = [p, p, p, p, i32, i32, p]
+    lib.pfsm_set_shard.argtypes = [p, i32, i32]
+    lib.pfsm_shard_phase.argtypes = [p, i32, p, p, p, p]
+    lib.pfsm_shard_buffer.argtypes = [p, i32, ctypes.POINTER(p)]
     lib.pfsm_destroy.argtypes = [p]
     lib.pfsm_get_info.argtypes = [p, p, ctypes.POINTER(i64)]
     lib.pfsm_get_step2_sweeps.argtypes = [p, p, ctypes.POINTER(i32)]
@@ -168,6 +171,40 @@ class Handle:
         _check(self._lib.pfsm_standard_form_eq14(self._h, _dev_ptr(A, N, (N, N), "A"), _dev_ptr(B, N, (N, N), "B"),
                                                  _dev_ptr(Z, N, (N, N), "Z"), niter, int(symmetrize),
                                                  _stream_ptr(stream)), "pfsm_standard_form_eq14")
+
+    def set_shard(self, rank: int, world: int):
+        _check(self._lib.pfsm_set_shard(self._h, rank, world), "pfsm_set_shard")
+
+    def shard_phase(self, phase: int, A, Vr, lam, stream=None):
+        N = self.N
+        ap = _dev_ptr(A, N, (N, N), "A") if A is not None else None
+        lp = _dev_ptr(lam, N, (N,), "lambda") if lam is not None else None
+        _check(self._lib.pfsm_shard_phase(self._h, phase, ap, _dev_ptr(Vr, N, (N, N), "V"), lp, _stream_ptr(stream)),
+               "pfsm_shard_phase")
+
+    def shard_buffer(self, which: int):
+        """Zero-copy (N, N) tensor view of a handle-owned exchange buffer (0: G, 1: V^T R^-1)."""
+        import torch
+        ptr = ctypes.c_void_p()
+        _check(self._lib.pfsm_shard_buffer(self._h, which, ctypes.byref(ptr)), "pfsm_shard_buffer")
+
+        class _DevBuf:
+            __cuda_array_interface__ = {"shape": (self.N, self.N), "typestr": "<f8", "data": (int(ptr.value), False),
+                                        "version": 2}
+
+        return torch.as_tensor(_DevBuf(), device="cuda")
+
+    def residuals_view(self):
+        """Zero-copy (N,) tensor view of the handle's residual buffer (for the sharded solve's all-gather)."""
+        import torch
+        ptr = ctypes.c_void_p()
+        _check(self._lib.pfsm_get_residuals(self._h, ctypes.byref(ptr)), "pfsm_get_residuals")
+
+        class _DevBuf:
+            __cuda_array_interface__ = {"shape": (self.N,), "typestr": "<f8", "data": (int(ptr.value), False),
+                                        "version": 2}
+
+        return torch.as_tensor(_DevBuf(), device="cuda")
 
     def solve_host(self, A_host, Vr_host, lam_host, stream=None):
         N = self.N

@@ -84,9 +84,9 @@ template <int EPL>
 __global__ void __launch_bounds__(JACOBI_THREADS, 1)
 jacobi_smem_kernel(const double* __restrict__ A, int64_t N, int32_t M, int32_t m, int32_t h_loc, SliceTable tab,
                    double* __restrict__ nrm_g, double* __restrict__ V, double* __restrict__ eps,
-                   int* __restrict__ rotcnt, unsigned long long* info) {
+                   int* __restrict__ rotcnt, unsigned long long* info, int32_t s_off) {
     const int CS = (int)cluster_nctarank(), cr = (int)cluster_ctarank();
-    const int s = blockIdx.x / CS;
+    const int s = s_off + blockIdx.x / CS;  // s_off: first slice of this launch
     const int lo = tab.lo[s], off = tab.off[s], g0 = tab.g0[s];
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     constexpr int NW = JACOBI_THREADS / 32;

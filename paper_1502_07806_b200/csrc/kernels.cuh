@@ -65,9 +65,9 @@ template <int EPL>
 __global__ void __launch_bounds__(JACOBI_THREADS, 1)
 jacobi_batched_kernel(const double* __restrict__ A, int64_t N, int32_t M, int32_t m, SliceTable tab,
                       double* __restrict__ Gws, double* __restrict__ V, double* __restrict__ eps,
-                      int* __restrict__ rotcnt, unsigned long long* info) {
+                      int* __restrict__ rotcnt, unsigned long long* info, int32_t s_off) {
     const int CS = (int)cluster_nctarank(), cr = (int)cluster_ctarank();
-    const int s = blockIdx.x / CS;
+    const int s = s_off + blockIdx.x / CS;  // s_off: first slice of this launch (a rank of the sharded solve owns a range)
     const int lo = tab.lo[s], off = tab.off[s], g0 = tab.g0[s];
     double* G = Gws + (size_t)s * M * M;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -451,9 +451,9 @@ __device__ __forceinline__ double block_sum(double v, double* red) {
 }
 __global__ void __launch_bounds__(RAY_THREADS)
 rayleigh_kernel(const double* __restrict__ V, const double* __restrict__ T, int64_t N, double* __restrict__ lambda,
-                double* __restrict__ resid) {
+                double* __restrict__ resid, int32_t i_off) {
     __shared__ double red[RAY_THREADS / 32];
-    const int64_t i = blockIdx.x;
+    const int64_t i = (int64_t)i_off + blockIdx.x;
     const double2* v2 = reinterpret_cast<const double2*>(V + i * N);
     const double2* t2 = reinterpret_cast<const double2*>(T + i * N);
     const int64_t n2 = N / 2;  // N is even

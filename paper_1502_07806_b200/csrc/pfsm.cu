@@ -96,6 +96,7 @@ struct pfsm_ctx {
     cudaEvent_t ev[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
     bool ev_valid = false;
     bool keep_info = false;
+    int32_t sh_rank = 0, sh_world = 1;  // sharded solve: this handle works on rows [sh_rank, sh_rank+1) * N / sh_world
 };
 
 static int dev_alloc(pfsm_ctx* h, void** p, size_t bytes) {
@@ -243,12 +244,12 @@ static int jacobi_cluster_size(const pfsm_ctx* h) {
 
 extern "C++" {
 template <int EPL>
-static int launch_jacobi_t(pfsm_ctx* h, const double* A, double* V, cudaStream_t st) {
+static int launch_jacobi_t(pfsm_ctx* h, const double* A, double* V, cudaStream_t st, int32_t s0, int32_t ns) {
     SliceTable tab{h->slice_tab, h->slice_tab + h->P, h->slice_tab + 2 * (size_t)h->P};
     const int cs = jacobi_cluster_size(h);
     cudaLaunchConfig_t cfg;
     memset(&cfg, 0, sizeof(cfg));
-    cfg.gridDim = dim3((unsigned)(h->P * cs));
+    cfg.gridDim = dim3((unsigned)(ns * cs));
     cfg.blockDim = dim3(JACOBI_THREADS);
     cfg.dynamicSmemBytes = (size_t)h->M * (sizeof(double) + sizeof(int));
     cfg.stream = st;
@@ -260,14 +261,14 @@ static int launch_jacobi_t(pfsm_ctx* h, const double* A, double* V, cudaStream_t
     cfg.attrs = attr;
     cfg.numAttrs = 1;
     PFSM_CUDA(cudaLaunchKernelEx(&cfg, jacobi_batched_kernel<EPL>, A, h->N, h->M, h->m, tab, h->Gws, V, h->eps,
-                                 h->rotcnt, h->info));
+                                 h->rotcnt, h->info, s0));
     return 0;
 }
 }  // extern "C++"
 
 extern "C++" {
 template <int EPL>
-static int launch_jacobi_smem_t(pfsm_ctx* h, const double* A, double* V, cudaStream_t st) {
+static int launch_jacobi_smem_t(pfsm_ctx* h, const double* A, double* V, cudaStream_t st, int32_t s0, int32_t ns) {
     SliceTable tab{h->slice_tab, h->slice_tab + h->P, h->slice_tab + 2 * (size_t)h->P};
     const size_t smem = jacobi_smem_bytes(h->M, h->jac_hloc);
     static size_t attr_bytes = 0;  // static smem (~300 B) + dynamic must stay within the 227 KB opt-in limit
@@ -277,7 +278,7 @@ static int launch_jacobi_smem_t(pfsm_ctx* h, const double* A, double* V, cudaStr
     }
     cudaLaunchConfig_t cfg;
     memset(&cfg, 0, sizeof(cfg));
-    cfg.gridDim = dim3((unsigned)(h->P * h->jac_cs));
+    cfg.gridDim = dim3((unsigned)(ns * h->jac_cs));
     cfg.blockDim = dim3(JACOBI_THREADS);
     cfg.dynamicSmemBytes = smem;
     cfg.stream = st;
@@ -289,7 +290,7 @@ static int launch_jacobi_smem_t(pfsm_ctx* h, const double* A, double* V, cudaStr
     cfg.attrs = attr;
     cfg.numAttrs = 1;
     PFSM_CUDA(cudaLaunchKernelEx(&cfg, jacobi_smem_kernel<EPL>, A, h->N, h->M, h->m, (int32_t)h->jac_hloc, tab,
-                                 h->nrm_g, V, h->eps, h->rotcnt, h->info));
+                                 h->nrm_g, V, h->eps, h->rotcnt, h->info, s0));
     return 0;
 }
 }  // extern "C++"
@@ -311,23 +312,24 @@ static void choose_jacobi_layout(pfsm_ctx* h) {
     h->jac_hloc = hloc_of(cs);
 }
 
-static int launch_jacobi(pfsm_ctx* h, const double* A, double* V, cudaStream_t st) {
+static int launch_jacobi(pfsm_ctx* h, const double* A, double* V, cudaStream_t st, int32_t s0 = 0, int32_t ns = -1) {
+    if (ns < 0) ns = h->P;
     PFSM_CUDA(cudaMemsetAsync(h->rotcnt, 0, (size_t)h->P * JACOBI_MAX_SWEEPS * sizeof(int), st));
     if (h->jac_cs > 0) {
         switch (jacobi_padded_rows(h->M) / 32) {  // doubles per lane per column
-            case 2: return launch_jacobi_smem_t<2>(h, A, V, st);
-            case 4: return launch_jacobi_smem_t<4>(h, A, V, st);
-            case 6: return launch_jacobi_smem_t<6>(h, A, V, st);
-            case 8: return launch_jacobi_smem_t<8>(h, A, V, st);
-            case 10: return launch_jacobi_smem_t<10>(h, A, V, st);
-            case 12: return launch_jacobi_smem_t<12>(h, A, V, st);
-            case 14: return launch_jacobi_smem_t<14>(h, A, V, st);
-            default: return launch_jacobi_smem_t<16>(h, A, V, st);
+            case 2: return launch_jacobi_smem_t<2>(h, A, V, st, s0, ns);
+            case 4: return launch_jacobi_smem_t<4>(h, A, V, st, s0, ns);
+            case 6: return launch_jacobi_smem_t<6>(h, A, V, st, s0, ns);
+            case 8: return launch_jacobi_smem_t<8>(h, A, V, st, s0, ns);
+            case 10: return launch_jacobi_smem_t<10>(h, A, V, st, s0, ns);
+            case 12: return launch_jacobi_smem_t<12>(h, A, V, st, s0, ns);
+            case 14: return launch_jacobi_smem_t<14>(h, A, V, st, s0, ns);
+            default: return launch_jacobi_smem_t<16>(h, A, V, st, s0, ns);
         }
     }
-    if (h->M <= 128) return launch_jacobi_t<4>(h, A, V, st);
-    if (h->M <= 256) return launch_jacobi_t<8>(h, A, V, st);
-    return launch_jacobi_t<16>(h, A, V, st);
+    if (h->M <= 128) return launch_jacobi_t<4>(h, A, V, st, s0, ns);
+    if (h->M <= 256) return launch_jacobi_t<8>(h, A, V, st, s0, ns);
+    return launch_jacobi_t<16>(h, A, V, st, s0, ns);
 }
 
 // ---- Stacked right-looking Cholesky on S = [G ; Z] (2N x N, row-major view): O = [L ; Z L^-T] with G = L L^T.
@@ -336,15 +338,27 @@ static int launch_jacobi(pfsm_ctx* h, const double* A, double* V, cudaStream_t s
 // factor = false re-uses L (O's top) and the inverted diagonal blocks of an earlier pass and only transforms
 // the bottom rows [N, 2N).  Two-level blocking: 128-wide panels are factored one by one, but the big trailing
 // update is applied once per PAIR of panels with K = 256, halving how often every C tile is read and re-written.
-static int stacked_cholesky(pfsm_ctx* h, bool factor, cudaStream_t st) {
+// b0, b1: only the bottom rows [N + b0, N + b1) are transformed (a rank of the sharded solve owns a row block of Z).
+static int stacked_cholesky(pfsm_ctx* h, bool factor, cudaStream_t st, int32_t b0 = 0, int32_t b1 = -1) {
     const int64_t N = h->N;
     const int32_t n = (int32_t)N;
+    if (b1 < 0) b1 = n;
+    const bool whole = factor && b0 == 0 && b1 == n;  // top and bottom rows form one contiguous row range
     int rc;
     static bool chol_attr = false;
     if (!chol_attr) {
         PFSM_CUDA(cudaFuncSetAttribute(chol_diag_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, CHOL_SMEM));
         chol_attr = true;
     }
+    // panel rows [r0, r0 + nr): O[r, k0:k0+nb] = S[r, k0:k0+nb] L_kk^-T
+    auto panel_rows = [&](int32_t k, int32_t r0, int32_t nr) -> int {
+        if (nr <= 0) return 0;
+        const int32_t k0 = k * CHOL_NB, nb = (int32_t)std::min<int64_t>(CHOL_NB, N - k0);
+        GemmParams pp = base_params();
+        pp.C = h->O; pp.ldc = N; pp.cr0 = r0; pp.cc0 = k0; pp.mr = nr; pp.nc = nb;
+        pp.xr0 = r0; pp.xk0 = k0; pp.yr0 = k * CHOL_NB; pp.yk0 = 0; pp.klen = nb;
+        return launch_gemm<EPI_PLAIN>(h->mapS, h->mapD, h->mapO, pp, st);
+    };
     auto factor_panel = [&](int32_t k) -> int {
         const int32_t k0 = k * CHOL_NB, nb = (int32_t)std::min<int64_t>(CHOL_NB, N - k0);
         if (factor) {
@@ -352,21 +366,23 @@ static int stacked_cholesky(pfsm_ctx* h, bool factor, cudaStream_t st) {
                                                                  h->Dinv + (size_t)k * CHOL_NB * CHOL_NB, h->gdiag, h->info);
             PFSM_CUDA(cudaGetLastError());
         }
-        // panel: O[r, k0:k0+nb] = S[r, k0:k0+nb] L_kk^-T   for all rows below the diagonal block (or the bottom rows)
-        const int32_t r0 = factor ? k0 + nb : n;
-        GemmParams pp = base_params();
-        pp.C = h->O; pp.ldc = N; pp.cr0 = r0; pp.cc0 = k0; pp.mr = 2 * n - r0; pp.nc = nb;
-        pp.xr0 = r0; pp.xk0 = k0; pp.yr0 = k * CHOL_NB; pp.yk0 = 0; pp.klen = nb;
-        return launch_gemm<EPI_PLAIN>(h->mapS, h->mapD, h->mapO, pp, st);
+        if (whole) return panel_rows(k, k0 + nb, 2 * n - k0 - nb);
+        int r = factor ? panel_rows(k, k0 + nb, n - k0 - nb) : 0;   // rows of G below the diagonal block
+        return r ? r : panel_rows(k, n + b0, b1 - b0);              // this call's rows of the bottom part
     };
-    // S[r, c0:c0+ncols] -= O[r, kk0:kk0+klen] . O[c, kk0:kk0+klen]  for rows r >= c0 (lower tiles when square)
-    auto update = [&](int32_t c0, int32_t ncols, int32_t kk0, int32_t klen, int lower) -> int {
-        if (ncols <= 0) return 0;
-        const int32_t r0 = factor ? c0 : n;
+    // rows [r0, r0 + nr): S[r, c0:c0+ncols] -= O[r, kk0:kk0+klen] . O[c, kk0:kk0+klen]
+    auto update_rows = [&](int32_t r0, int32_t nr, int32_t c0, int32_t ncols, int32_t kk0, int32_t klen, int lower) -> int {
+        if (ncols <= 0 || nr <= 0) return 0;
         GemmParams pt = base_params();
-        pt.C = h->S; pt.ldc = N; pt.cr0 = r0; pt.cc0 = c0; pt.mr = 2 * n - r0; pt.nc = ncols;
-        pt.xr0 = r0; pt.yr0 = c0; pt.xk0 = kk0; pt.yk0 = kk0; pt.klen = klen; pt.lower = factor ? lower : 0;
+        pt.C = h->S; pt.ldc = N; pt.cr0 = r0; pt.cc0 = c0; pt.mr = nr; pt.nc = ncols;
+        pt.xr0 = r0; pt.yr0 = c0; pt.xk0 = kk0; pt.yk0 = kk0; pt.klen = klen; pt.lower = lower;
         return launch_gemm<EPI_SUB>(h->mapO, h->mapO, h->mapS, pt, st);
+    };
+    // columns [c0, c0 + ncols) of every active row at or below row c0 (lower tiles only where the region is square)
+    auto update = [&](int32_t c0, int32_t ncols, int32_t kk0, int32_t klen, int lower) -> int {
+        if (whole) return update_rows(c0, 2 * n - c0, c0, ncols, kk0, klen, lower);
+        int r = factor ? update_rows(c0, n - c0, c0, ncols, kk0, klen, lower) : 0;
+        return r ? r : update_rows(n + b0, b1 - b0, c0, ncols, kk0, klen, 0);
     };
     for (int32_t k = 0; k < h->nblk; k += 2) {
         const int32_t k0 = k * CHOL_NB;
@@ -410,7 +426,7 @@ static int run_step5(pfsm_ctx* h, const CUtensorMap& mapV, const CUtensorMap& ma
         GemmParams p = base_params();
         p.C = h->W; p.ldc = N; p.mr = n; p.nc = n; p.klen = n;
         if ((rc = launch_gemm<EPI_PLAIN>(mapV, mapA, h->mapW, p, st))) return rc;
-        rayleigh_kernel<<<(unsigned)N, RAY_THREADS, 0, st>>>(V, h->W, N, lambda_out, h->resid);
+        rayleigh_kernel<<<(unsigned)N, RAY_THREADS, 0, st>>>(V, h->W, N, lambda_out, h->resid, 0);
         PFSM_CUDA(cudaGetLastError());
     }
     return 0;
@@ -672,6 +688,87 @@ int pfsm_standard_form_eq14(pfsm_handle_t h, const double* A, const double* B, d
         PFSM_CUDA(cudaMemcpyAsync(Z_out, cur, n2, cudaMemcpyDeviceToDevice, st));
     }
     PFSM_CUDA(cudaGetLastError());
+    return 0;
+}
+
+// ---- f3: one solve sharded over `world` GPUs (the paper's own decomposition, PAPER.md:88,
+// 185).  Rank g owns the slices [g P/G, (g+1) P/G), i.e. rows [r0, r1) of the row-major V.  Steps 2-3 and 5 need
+// no communication; step 4 needs the vectors of all ranks.  The library provides the four compute phases; the
+// caller (paper_1502_07806_b200/sharded.py) runs an all-gather between them:
+//   phase 1: steps 2-3 on the own rows of V                       -> all-gather V rows
+//   phase 2: own block row of G = V V^T (row-major view)           -> all-gather G rows   (buffer 0)
+//   phase 3: Cholesky of G (replicated, N^3/3) + triangular solve of the own rows of V^T (N^3/G)
+//                                                                  -> all-gather rows of V^T R^-1 (buffer 1)
+//   phase 4: V = (V^T R^-1)^T, step 5 on the own rows              -> all-gather lambda
+int pfsm_set_shard(pfsm_handle_t h, int32_t rank, int32_t world) {
+    if (!h) return -1;
+    if (world < 1 || h->P % world != 0 || (h->N / world) % BM != 0) return -3;
+    if (rank < 0 || rank >= world) return -2;
+    h->sh_rank = rank;
+    h->sh_world = world;
+    return 0;
+}
+
+int pfsm_shard_buffer(pfsm_handle_t h, int32_t which, double** ptr) {
+    if (!h) return -1;
+    if (!ptr) return -3;
+    if (which == 0) *ptr = h->S;                                   // G: N x N (row block = own rows)
+    else if (which == 1) *ptr = h->O + (size_t)h->N * h->N;        // V^T R^-1: N x N (row block = own components)
+    else return -2;
+    return 0;
+}
+
+int pfsm_shard_phase(pfsm_handle_t h, int32_t phase, const double* A, double* V, double* lambda_out, void* stream) {
+    if (!h) return -1;
+    if (phase < 1 || phase > 4) return -2;
+    if ((phase == 1 || phase == 4) && (!A || ((uintptr_t)A & 15))) return -3;
+    if (!V || ((uintptr_t)V & 15)) return -4;
+    if (phase == 4 && !lambda_out) return -5;
+    cudaStream_t st = (cudaStream_t)stream;
+    const int64_t N = h->N;
+    const int32_t n = (int32_t)N;
+    const int32_t rows = n / h->sh_world, r0 = h->sh_rank * rows;
+    const int32_t ns = h->P / h->sh_world, s0 = h->sh_rank * ns;
+    int rc;
+    CUtensorMap mapA, mapV;
+    if ((rc = make_map(&mapV, V, N, N, N))) return rc;
+    if (A && (rc = make_map(&mapA, A, N, N, N))) return rc;
+    const dim3 tb(32, 8), tg((unsigned)((N + 31) / 32), (unsigned)((N + 31) / 32));
+    h->ev_valid = false;
+    if (phase == 1) {
+        PFSM_CUDA(cudaMemsetAsync(h->info, 0xFF, sizeof(unsigned long long), st));
+        PFSM_CUDA(cudaMemsetAsync(V + (size_t)r0 * N, 0, (size_t)rows * N * sizeof(double), st));
+        if ((rc = launch_jacobi(h, A, V, st, s0, ns))) return rc;
+        for (int it = 0; it < h->iters; ++it) {
+            GemmParams p = base_params();
+            p.C = h->W; p.ldc = N; p.cr0 = r0; p.mr = rows; p.nc = n; p.xr0 = r0; p.klen = n;
+            p.krange = (it == 0) ? h->krange + r0 / BM : nullptr;
+            p.E1 = V; p.ld1 = N; p.eps = h->eps;
+            if ((rc = launch_gemm<EPI_SHIFT>(mapV, mapA, h->mapW, p, st))) return rc;
+            GemmParams q = base_params();
+            q.C = V; q.ldc = N; q.cr0 = r0; q.mr = rows; q.nc = n; q.xr0 = r0; q.klen = n;
+            q.E1 = h->W; q.ld1 = N; q.E2 = V; q.ld2 = N; q.eps = h->eps; q.alpha = h->alpha;
+            if ((rc = launch_gemm<EPI_UPDATE>(h->mapW, mapA, mapV, q, st))) return rc;
+        }
+    } else if (phase == 2) {
+        GemmParams p = base_params();  // G[r0:r1, :] = V[r0:r1, :] V^T
+        p.C = h->S; p.ldc = N; p.cr0 = r0; p.mr = rows; p.nc = n; p.xr0 = r0; p.klen = n;
+        if ((rc = launch_gemm<EPI_PLAIN>(mapV, mapV, h->mapS, p, st))) return rc;
+    } else if (phase == 3) {
+        transpose_kernel<<<tg, tb, 0, st>>>(V, N, h->S + (size_t)N * N, N, n, n);
+        PFSM_CUDA(cudaGetLastError());
+        extract_diag_kernel<<<(unsigned)((N + 255) / 256), 256, 0, st>>>(h->S, N, n, h->gdiag);
+        PFSM_CUDA(cudaGetLastError());
+        if ((rc = stacked_cholesky(h, true, st, r0, r0 + rows))) return rc;
+    } else {
+        transpose_kernel<<<tg, tb, 0, st>>>(h->O + (size_t)N * N, N, V, N, n, n);
+        PFSM_CUDA(cudaGetLastError());
+        GemmParams p = base_params();
+        p.C = h->W; p.ldc = N; p.cr0 = r0; p.mr = rows; p.nc = n; p.xr0 = r0; p.klen = n;
+        if ((rc = launch_gemm<EPI_PLAIN>(mapV, mapA, h->mapW, p, st))) return rc;
+        rayleigh_kernel<<<(unsigned)rows, RAY_THREADS, 0, st>>>(V, h->W, N, lambda_out, h->resid, r0);
+        PFSM_CUDA(cudaGetLastError());
+    }
     return 0;
 }
 

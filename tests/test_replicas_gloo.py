@@ -67,3 +67,41 @@ def test_single_rank_is_a_no_op():
     assert replicas.max_over_ranks(3.5, 1) == 3.5
     assert replicas.all_ok(True, 1) and not replicas.all_ok(False, 1)
     assert np.isclose(replicas.aggregate_tflops(2e12, 3, 1, 1000.0), 6.0)
+
+
+def _gather_worker(rank, world, port, q):
+    sys.path.insert(0, ROOT)
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), WORLD_SIZE=str(world), RANK=str(rank))
+    import torch
+    import torch.distributed as dist
+    from paper_1502_07806_b200 import sharded
+    dist.init_process_group("gloo", world_size=world, rank=rank)
+    N = 8
+    t = torch.full((N, N), float("nan"), dtype=torch.float64)
+    rows = N // world
+    t[rank * rows:(rank + 1) * rows] = float(rank + 1)      # only the own row block is valid
+    sharded._all_gather_rows(t, world, rank)
+    v = torch.full((N,), float("nan"), dtype=torch.float64)
+    v[rank * rows:(rank + 1) * rows] = float(10 * (rank + 1))
+    sharded._all_gather_rows(v, world, rank)
+    q.put((rank, t.tolist(), v.tolist()))
+    dist.destroy_process_group()
+
+
+def test_sharded_all_gather_of_row_blocks_gloo():
+    """Host logic of the sharded solve (f3): the in-place all-gather of equal row blocks, world size 2, CPU."""
+    world = 2
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_gather_worker, args=(r, world, port, q)) for r in range(world)]
+    for p in procs:
+        p.start()
+    res = sorted(q.get(timeout=120) for _ in range(world))
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    want_t = [[1.0] * 8] * 4 + [[2.0] * 8] * 4
+    want_v = [10.0] * 4 + [20.0] * 4
+    for rank, t, v in res:
+        assert t == want_t and v == want_v

@@ -1,0 +1,85 @@
+"""f3: one solve sharded over 2 ranks.  The box has one GPU, so the two ranks are two processes time-sharing it and
+the all-gathers go through the gloo backend (host staging); no kernel of one rank waits on the other.  The result
+must equal the single-rank solve."""
+import os
+import socket
+import sys
+
+import numpy as np
+import pytest
+import torch.multiprocessing as mp
+
+pytestmark = pytest.mark.gpu
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _free_port():
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    port = s.getsockname()[1]
+    s.close()
+    return port
+
+
+def _worker(rank, world, port, N, P, w, iters, out_dir):
+    sys.path.insert(0, ROOT)
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), WORLD_SIZE=str(world), RANK=str(rank))
+    import torch
+    import torch.distributed as dist
+
+    import paper_1502_07806_b200 as pfsm
+    import pfsm_inputs as gen
+    from paper_1502_07806_b200 import sharded
+    dist.init_process_group("gloo", world_size=world, rank=rank)
+    torch.cuda.set_device(0)
+    p = gen.small_problem(N, 1e-3, 16.0, seed=4242)
+    h = pfsm.Handle(N, P, w, iters, p.alpha)
+    h.set_shard(rank, world)
+    dA = torch.from_numpy(p.A).cuda()
+    dV = torch.full((N, N), float("nan"), dtype=torch.float64, device="cuda")
+    dl = torch.full((N,), float("nan"), dtype=torch.float64, device="cuda")
+    sharded.solve_sharded(h, dA, dV, dl)
+    torch.cuda.synchronize()
+    np.savez(os.path.join(out_dir, f"rank{rank}.npz"), lam=dl.cpu().numpy(), V=dV.cpu().numpy(),
+             res=h.residuals().cpu().numpy(), info=h.info())
+    h.destroy()
+    dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("N,P,w,iters", [(512, 4, 16, 2), (768, 6, 24, 3)])
+def test_two_rank_sharded_solve_equals_single_rank(tmp_path, N, P, w, iters):
+    import torch
+
+    import oracle
+    import paper_1502_07806_b200 as pfsm
+    import pfsm_inputs as gen
+    world = 2
+    ctx = mp.get_context("spawn")
+    port = _free_port()
+    procs = [ctx.Process(target=_worker, args=(r, world, port, N, P, w, iters, str(tmp_path))) for r in range(world)]
+    for pr in procs:
+        pr.start()
+    for pr in procs:
+        pr.join(timeout=300)
+        assert pr.exitcode == 0
+    p = gen.small_problem(N, 1e-3, 16.0, seed=4242)
+    h = pfsm.Handle(N, P, w, iters, p.alpha)
+    dA = torch.from_numpy(p.A).cuda()
+    dV = torch.empty((N, N), dtype=torch.float64, device="cuda")
+    dl = torch.empty((N,), dtype=torch.float64, device="cuda")
+    h.solve(dA, dV, dl)
+    ref_l, ref_V, ref_r = dl.cpu().numpy(), dV.cpu().numpy(), h.residuals().cpu().numpy()
+    assert h.info() == 0
+    h.destroy()
+    o = oracle.pfsm(p.A, P, w, iters, p.alpha)
+    nF = p.normF
+    for r in range(world):
+        d = np.load(os.path.join(str(tmp_path), f"rank{r}.npz"))
+        assert int(d["info"]) == 0
+        # every rank ends with the complete result, equal to the single-rank solve to rounding
+        assert np.abs(d["lam"] - ref_l).max() < 1e-13
+        assert np.abs(d["V"] - ref_V).max() < 1e-12
+        assert np.abs(d["res"] - ref_r).max() < 1e-13
+        # and within the parity gates of the oracle
+        assert np.abs(d["lam"] - o["lam"]).max() <= 1e-10 * nF
+        assert np.abs(d["V"] @ d["V"].T - np.eye(N)).max() <= 1e-12 * N
