@@ -166,10 +166,11 @@ def run_reference(args):
     return 0
 
 
-def workload_config(c, n_gpus: int) -> dict:
+def workload_config(c, n_gpus: int, sharded: bool = False) -> dict:
     return {"workload": f"BASELINE.json configs[{c.index}]: {c.name}, synthetic A = D + E",
             "N": c.N, "P": c.P, "window": c.window, "M": c.M, "iters": c.iters,
-            "alpha": "0.5/max|d|^2", "replicas": n_gpus, "parallelism": f"replicas x{n_gpus}",
+            "alpha": "0.5/max|d|^2", "replicas": n_gpus, "parallelism": (f"one solve sharded over {n_gpus} ranks (all-gathers between the 4 phases)" if sharded
+                            else f"replicas x{n_gpus}"),
             "l2_policy": f"inputs larger than L2 (A, V, W are {8 * c.N * c.N / 2**20:.0f} MiB each vs 126 MB L2)"
             if 8 * c.N * c.N > 126e6 else "L2 flushed between timed iterations (256 MiB write)"}
 
@@ -191,11 +192,23 @@ def run_ours(args):
 
     k = args.config
     # replicas only: rank r solves an independent matrix of the same config
-    prob = gen.problem(k, seed_offset=replicas.replica_seed_offset(rank))
+    sharded_mode = bool(args.sharded) and world > 1
+    # default: replicas (rank r solves an independent matrix); --sharded: ONE solve split over the ranks (f3)
+    prob = gen.problem(k, seed_offset=0 if sharded_mode else replicas.replica_seed_offset(rank))
     c = prob.cfg
     N = c.N
     flops = algorithmic_flops(N, c.M, c.iters)
     h = pfsm.Handle(N, c.P, c.window, c.iters, prob.alpha)
+    if sharded_mode:
+        from paper_1502_07806_b200 import sharded
+        h.set_shard(rank, world)
+
+    def solve_once():
+        if sharded_mode:
+            sharded.solve_sharded(h, dA, dV, dl)
+        else:
+            h.solve(dA, dV, dl)
+
     stream = torch.cuda.current_stream()
     A_host = torch.from_numpy(prob.A).pin_memory()
     V_host = torch.empty((N, N), dtype=torch.float64).pin_memory()
@@ -217,7 +230,7 @@ def run_ours(args):
 
     # ---- device-resident leg: K solves, CUDA events on the launching stream ----
     for _ in range(args.warmup):
-        h.solve(dA, dV, dl)
+        solve_once()
     barrier()
     assert replicas.all_ok(h.info() == 0, world, "cuda"), "PFSM reported a numerical breakdown on a bench matrix"
     h.enable_step_timing(True)
@@ -232,13 +245,14 @@ def run_ours(args):
         if flush is not None:
             flush.fill_(i & 0xFF)
         ev[i][0].record(stream)
-        h.solve(dA, dV, dl)
+        solve_once()
         ev[i][1].record(stream)
         if flush is not None or True:
             # per-step device times are read back after each solve (events are already recorded; this sync
             # sits outside the [start, stop] event pair of the step)
             ev[i][1].synchronize()
-            step_ms += np.array(h.step_ms())
+            if not sharded_mode:
+                step_ms += np.array(h.step_ms())
     barrier()
     t_wall1 = time.time()
     clocks = sampler.stop(t_wall0, t_wall1)
@@ -247,7 +261,7 @@ def run_ours(args):
     total_ms = max_over_ranks(float(sum(solve_ms)))
     ms_per_step = total_ms / args.steps
     step_ms /= args.steps
-    value = replicas.aggregate_tflops(flops["total"], args.steps, world, total_ms)
+    value = replicas.aggregate_tflops(flops["total"], args.steps, 1 if sharded_mode else world, total_ms)
 
     # ---- end-to-end leg: host buffers through pfsm_solve_host, copies inside the timed region ----
     e2e_steps = max(1, min(args.steps, 3))
@@ -260,7 +274,7 @@ def run_ours(args):
     e1.record(stream)
     barrier()
     e2e_ms = max_over_ranks(e0.elapsed_time(e1)) / e2e_steps
-    e2e_value = replicas.aggregate_tflops(flops["total"], 1, world, e2e_ms)
+    e2e_value = replicas.aggregate_tflops(flops["total"], 1, 1 if sharded_mode else world, e2e_ms)
     lam = lam_host.numpy().copy()
     Vh = V_host.numpy()
 
@@ -324,8 +338,9 @@ def run_ours(args):
     line = {
         "metric": "PFSM solve sustained FP64 TFLOP/s (algorithmic flops / solve time)",
         "value": value, "unit": "TFLOP/s", "n_gpus": n_gpus, "steps": args.steps, "warmup": args.warmup,
-        "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": "f64", "data": "synthetic", "config": workload_config(c, n_gpus),
+        "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "strong" if sharded_mode else "weak",
+        "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic", "config": workload_config(c, n_gpus, sharded_mode),
         "solve_ms": {"median": float(np.median(solve_ms)), "best": float(min(solve_ms))},
         "step_ms": {"step2_submatrix_eig": step_ms[0], "step3_folded_spectrum": step_ms[1],
                     "step4_cholesky_qr": step_ms[2], "step5_rayleigh": step_ms[3]},
@@ -353,6 +368,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--cpu-cols", type=int, default=128, help="eigenvectors in the cpu_baseline sample")
     ap.add_argument("--ref-cols", type=int, default=8, help="eigenvectors per step of --impl reference")
+    ap.add_argument("--sharded", action="store_true",
+                    help="N>1: split ONE solve over the ranks (strong scaling) instead of independent replicas")
     ap.add_argument("--no-syevd", dest="syevd", action="store_false")
     ap.add_argument("--no-calibrate", dest="calibrate", action="store_false")
     args = ap.parse_args()
