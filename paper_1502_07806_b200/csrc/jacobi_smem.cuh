@@ -9,10 +9,11 @@
 //      top[1] -> top[2] -> ... -> top[h-1] -> bot[h-1] -> bot[h-2] -> ... -> bot[0] -> top[1].
 // CTA k of the cluster owns seats t in [k h_loc, (k+1) h_loc).  Its top and bottom seats are ring buffers of
 // h_loc + 1 column slots each, so "moving one seat" is a head-pointer increment; only the two columns that
-// cross a CTA boundary are copied: the warp that rotated them stores the result straight into the spare slot
-// of the neighbour's ring through distributed shared memory (mapa + st.shared::cluster), and the round ends
-// with one cluster barrier (release/acquire).  Per round a CTA streams its 2 h_loc columns through the SM's
-// own 128 B/clk shared-memory port instead of the chip-wide L2.
+// cross a CTA boundary are copied: they are staged, and after the CTA barrier of the round two warps send them
+// into the spare slots of the neighbours' rings through distributed shared memory with st.async, which completes
+// its bytes on the receiver's mbarrier -- a point-to-point exchange; a cluster barrier is needed only once per
+// sweep (convergence count).  Per round a CTA streams its 2 h_loc columns through the SM's own 128 B/clk
+// shared-memory port instead of the chip-wide L2.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>

@@ -534,3 +534,31 @@ def test_eq14_converges_to_the_cholesky_route_on_config4g_shape():
     ex = scipy.linalg.eigh(p.A, S, eigvals_only=True)
     assert np.abs(np.sort(np.linalg.eigvals(Z).real) - ex).max() < 1e-10
     h.destroy()
+
+
+# ------------------------------------------------------------------ seeded sweep over ragged shapes
+def _fuzz_cases(count=24):
+    u = gen.uniform(20260101, gen.STREAM_TEST, 0, 4 * count)
+    cases = []
+    for k in range(count):
+        N = 2 * int(2 + u[4 * k] * 330)                      # even, 4 .. 662
+        divs = [d for d in range(1, N + 1) if N % d == 0 and N // d >= 1]
+        P = divs[int(u[4 * k + 1] * len(divs)) % len(divs)]
+        m = N // P
+        w = int(u[4 * k + 2] * 40)
+        if min(N, m + 2 * w) > 512:                          # library limit on the submatrix order
+            w = max(0, (512 - m) // 2)
+        if m > 512:
+            continue
+        iters = int(u[4 * k + 3] * 4)
+        cases.append((N, P, w, iters))
+    return cases
+
+
+@pytest.mark.parametrize("N,P,w,iters", _fuzz_cases())
+def test_seeded_shape_sweep_against_oracle(N, P, w, iters):
+    p = gen.small_problem(N, 1e-3, max(2.0, N / 16.0), seed=31000 + N + P)
+    g = gpu_solve(p.A, P, w, iters, p.alpha)
+    o = oracle.pfsm(p.A, P, w, iters, p.alpha)
+    check_gates(p.A, g, o)
+    assert np.abs(g["eps"] - o["eps"]).max() <= 1e-12 * max(1.0, p.normF)
