@@ -96,6 +96,9 @@ struct pfsm_ctx {
     cudaEvent_t ev[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
     bool ev_valid = false;
     bool keep_info = false;
+    cudaStream_t side = nullptr;       // high-priority stream of the Cholesky look-ahead
+    cudaEvent_t ev_chain = nullptr, ev_rest = nullptr, ev_fork = nullptr;
+    bool lookahead = true;
     int32_t sh_rank = 0, sh_world = 1;  // sharded solve: this handle works on rows [sh_rank, sh_rank+1) * N / sh_world
 };
 
@@ -216,6 +219,16 @@ int pfsm_create(pfsm_handle_t* out, int64_t N, int32_t P, int32_t window, int32_
         cudaError_t e = cudaEventCreate(&h->ev[i]);
         if (e != cudaSuccess) { pfsm_destroy(h); return PFSM_CUDA_ERROR_BASE + (int)e; }
     }
+    {
+        int lo_prio = 0, hi_prio = 0;
+        cudaError_t e = cudaDeviceGetStreamPriorityRange(&lo_prio, &hi_prio);
+        if (e == cudaSuccess) e = cudaStreamCreateWithPriority(&h->side, cudaStreamNonBlocking, hi_prio);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&h->ev_chain, cudaEventDisableTiming);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&h->ev_rest, cudaEventDisableTiming);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&h->ev_fork, cudaEventDisableTiming);
+        if (e != cudaSuccess) { pfsm_destroy(h); return PFSM_CUDA_ERROR_BASE + (int)e; }
+        h->lookahead = getenv("PFSM_NO_LOOKAHEAD") == nullptr;
+    }
 #undef TRY
     *out = h;
     return 0;
@@ -230,6 +243,10 @@ int pfsm_destroy(pfsm_handle_t h) {
         if (p) cudaFree(p);
     for (int i = 0; i < 5; ++i)
         if (h->ev[i]) cudaEventDestroy(h->ev[i]);
+    if (h->ev_chain) cudaEventDestroy(h->ev_chain);
+    if (h->ev_rest) cudaEventDestroy(h->ev_rest);
+    if (h->ev_fork) cudaEventDestroy(h->ev_fork);
+    if (h->side) cudaStreamDestroy(h->side);
     delete h;
     return 0;
 }
@@ -350,6 +367,7 @@ static int stacked_cholesky(pfsm_ctx* h, bool factor, cudaStream_t st, int32_t b
         PFSM_CUDA(cudaFuncSetAttribute(chol_diag_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, CHOL_SMEM));
         chol_attr = true;
     }
+    cudaStream_t cs = st;  // stream the helpers below launch on (switched by the look-ahead schedule)
     // panel rows [r0, r0 + nr): O[r, k0:k0+nb] = S[r, k0:k0+nb] L_kk^-T
     auto panel_rows = [&](int32_t k, int32_t r0, int32_t nr) -> int {
         if (nr <= 0) return 0;
@@ -357,12 +375,12 @@ static int stacked_cholesky(pfsm_ctx* h, bool factor, cudaStream_t st, int32_t b
         GemmParams pp = base_params();
         pp.C = h->O; pp.ldc = N; pp.cr0 = r0; pp.cc0 = k0; pp.mr = nr; pp.nc = nb;
         pp.xr0 = r0; pp.xk0 = k0; pp.yr0 = k * CHOL_NB; pp.yk0 = 0; pp.klen = nb;
-        return launch_gemm<EPI_PLAIN>(h->mapS, h->mapD, h->mapO, pp, st);
+        return launch_gemm<EPI_PLAIN>(h->mapS, h->mapD, h->mapO, pp, cs);
     };
     auto factor_panel = [&](int32_t k) -> int {
         const int32_t k0 = k * CHOL_NB, nb = (int32_t)std::min<int64_t>(CHOL_NB, N - k0);
         if (factor) {
-            chol_diag_kernel<<<1, CHOL_THREADS, CHOL_SMEM, st>>>(h->S, h->O, N, k0, nb,
+            chol_diag_kernel<<<1, CHOL_THREADS, CHOL_SMEM, cs>>>(h->S, h->O, N, k0, nb,
                                                                  h->Dinv + (size_t)k * CHOL_NB * CHOL_NB, h->gdiag, h->info);
             PFSM_CUDA(cudaGetLastError());
         }
@@ -376,7 +394,7 @@ static int stacked_cholesky(pfsm_ctx* h, bool factor, cudaStream_t st, int32_t b
         GemmParams pt = base_params();
         pt.C = h->S; pt.ldc = N; pt.cr0 = r0; pt.cc0 = c0; pt.mr = nr; pt.nc = ncols;
         pt.xr0 = r0; pt.yr0 = c0; pt.xk0 = kk0; pt.yk0 = kk0; pt.klen = klen; pt.lower = lower;
-        return launch_gemm<EPI_SUB>(h->mapO, h->mapO, h->mapS, pt, st);
+        return launch_gemm<EPI_SUB>(h->mapO, h->mapO, h->mapS, pt, cs);
     };
     // columns [c0, c0 + ncols) of every active row at or below row c0 (lower tiles only where the region is square)
     auto update = [&](int32_t c0, int32_t ncols, int32_t kk0, int32_t klen, int lower) -> int {
@@ -384,15 +402,54 @@ static int stacked_cholesky(pfsm_ctx* h, bool factor, cudaStream_t st, int32_t b
         int r = factor ? update_rows(c0, n - c0, c0, ncols, kk0, klen, lower) : 0;
         return r ? r : update_rows(n + b0, b1 - b0, c0, ncols, kk0, klen, 0);
     };
-    for (int32_t k = 0; k < h->nblk; k += 2) {
-        const int32_t k0 = k * CHOL_NB;
-        if ((rc = factor_panel(k))) return rc;
-        if (k + 1 < h->nblk) {
-            const int32_t k1 = k0 + CHOL_NB, nb1 = (int32_t)std::min<int64_t>(CHOL_NB, N - k1);
-            if ((rc = update(k1, nb1, k0, CHOL_NB, 0))) return rc;      // second panel's columns only, K = 128
-            if ((rc = factor_panel(k + 1))) return rc;
-            if ((rc = update(k1 + nb1, n - k1 - nb1, k0, CHOL_NB + nb1, 1))) return rc;  // the rest, K = 256
+    const int32_t npairs = (h->nblk + 1) / 2;
+    auto pair_c0 = [&](int32_t p) { return std::min<int32_t>(n, 2 * p * CHOL_NB); };  // first column of pair p
+    // the serial chain of pair p: factor its first panel, bring the second panel's columns up to date, factor it
+    auto chain = [&](int32_t p) -> int {
+        const int32_t k = 2 * p, k0 = k * CHOL_NB;
+        int r = factor_panel(k);
+        if (r || k + 1 >= h->nblk) return r;
+        const int32_t k1 = k0 + CHOL_NB, nb1 = (int32_t)std::min<int64_t>(CHOL_NB, N - k1);
+        if ((r = update(k1, nb1, k0, CHOL_NB, 0))) return r;  // second panel's columns only, K = 128
+        return factor_panel(k + 1);
+    };
+    // columns [c0, c1) of the trailing matrix updated with pair p's panels (K = 256)
+    auto trailing = [&](int32_t p, int32_t c0, int32_t c1) -> int {
+        const int32_t k0 = 2 * p * CHOL_NB, kend = pair_c0(p + 1);
+        return update(c0, c1 - c0, k0, kend - k0, 1);
+    };
+    if (whole && h->lookahead && npairs >= 3) {
+        // Look-ahead: while the main stream applies pair p's update to the bulk of the trailing matrix, a
+        // high-priority side stream updates just the next pair's 256 columns and runs that pair's serial chain
+        // (diagonal-block kernels and under-filled panel GEMMs), so the chain hides behind the bulk update.
+        PFSM_CUDA(cudaEventRecord(h->ev_fork, st));
+        PFSM_CUDA(cudaStreamWaitEvent(h->side, h->ev_fork, 0));
+        cs = h->side;
+        if ((rc = chain(0))) return rc;
+        PFSM_CUDA(cudaEventRecord(h->ev_chain, h->side));
+        for (int32_t p = 0; p < npairs; ++p) {
+            const int32_t cn0 = pair_c0(p + 1), cn1 = pair_c0(p + 2);
+            PFSM_CUDA(cudaStreamWaitEvent(st, h->ev_chain, 0));      // main needs pair p's panels
+            if (cn0 < n) {
+                cs = h->side;                                        // side: next pair's columns, then its chain
+                if (p > 0) PFSM_CUDA(cudaStreamWaitEvent(h->side, h->ev_rest, 0));  // ... on top of update p-1
+                if ((rc = trailing(p, cn0, cn1))) return rc;
+                if ((rc = chain(p + 1))) return rc;
+                PFSM_CUDA(cudaEventRecord(h->ev_chain, h->side));
+            }
+            if (cn1 < n) {
+                cs = st;                                             // main: the bulk of pair p's update
+                if ((rc = trailing(p, cn1, n))) return rc;
+                PFSM_CUDA(cudaEventRecord(h->ev_rest, st));
+            }
         }
+        PFSM_CUDA(cudaStreamWaitEvent(st, h->ev_chain, 0));          // join
+        return 0;
+    }
+    for (int32_t p = 0; p < npairs; ++p) {
+        if ((rc = chain(p))) return rc;
+        const int32_t cn0 = pair_c0(p + 1);
+        if (cn0 < n && (rc = trailing(p, cn0, n))) return rc;
     }
     return 0;
 }
