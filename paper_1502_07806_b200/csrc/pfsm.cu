@@ -288,11 +288,8 @@ template <int EPL>
 static int launch_jacobi_smem_t(pfsm_ctx* h, const double* A, double* V, cudaStream_t st, int32_t s0, int32_t ns) {
     SliceTable tab{h->slice_tab, h->slice_tab + h->P, h->slice_tab + 2 * (size_t)h->P};
     const size_t smem = jacobi_smem_bytes(h->M, h->jac_hloc);
-    static size_t attr_bytes = 0;  // static smem (~300 B) + dynamic must stay within the 227 KB opt-in limit
-    if (smem > attr_bytes) {
-        PFSM_CUDA(cudaFuncSetAttribute(jacobi_smem_kernel<EPL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        attr_bytes = smem;
-    }
+    // static smem (~300 B) + dynamic must stay within the 227 KB opt-in limit; set per launch (handles differ)
+    PFSM_CUDA(cudaFuncSetAttribute(jacobi_smem_kernel<EPL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     cudaLaunchConfig_t cfg;
     memset(&cfg, 0, sizeof(cfg));
     cfg.gridDim = dim3((unsigned)(ns * h->jac_cs));
@@ -312,19 +309,72 @@ static int launch_jacobi_smem_t(pfsm_ctx* h, const double* A, double* V, cudaStr
 }
 }  // extern "C++"
 
-// Shared-memory Jacobi layout: the smallest cluster whose CTAs can hold their 2 h_loc + 3 column slots, grown
-// while a CTA would still have more pairs than warps and the chip has SMs to spare.  0 = use the L2 kernel.
+extern "C++" {
+// how many clusters of `cs` CTAs of the shared-memory Jacobi kernel the device can hold at once
+template <int EPL>
+static int jacobi_max_clusters_t(int cs, size_t smem) {
+    if (cudaFuncSetAttribute(jacobi_smem_kernel<EPL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) {
+        cudaGetLastError();
+        return 0;
+    }
+    cudaLaunchConfig_t cfg;
+    memset(&cfg, 0, sizeof(cfg));
+    cfg.gridDim = dim3((unsigned)cs);
+    cfg.blockDim = dim3(JACOBI_THREADS);
+    cfg.dynamicSmemBytes = smem;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = (unsigned)cs;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    int n = 0;
+    if (cudaOccupancyMaxActiveClusters(&n, jacobi_smem_kernel<EPL>, &cfg) != cudaSuccess) {
+        cudaGetLastError();
+        return 0;
+    }
+    return n;
+}
+}  // extern "C++"
+
+static int jacobi_max_clusters(int M, int cs, size_t smem) {
+    switch (jacobi_padded_rows(M) / 32) {
+        case 2: return jacobi_max_clusters_t<2>(cs, smem);
+        case 4: return jacobi_max_clusters_t<4>(cs, smem);
+        case 6: return jacobi_max_clusters_t<6>(cs, smem);
+        case 8: return jacobi_max_clusters_t<8>(cs, smem);
+        case 10: return jacobi_max_clusters_t<10>(cs, smem);
+        case 12: return jacobi_max_clusters_t<12>(cs, smem);
+        case 14: return jacobi_max_clusters_t<14>(cs, smem);
+        default: return jacobi_max_clusters_t<16>(cs, smem);
+    }
+}
+
+// Shared-memory Jacobi layout.  The kernel is bound by the dependent chain of a round (load, reduce, rotate,
+// exchange: ~1.2 us whatever the number of pairs a CTA holds), so more CTAs per slice help only while all P
+// clusters are co-resident: the largest cluster size in {1,2,4,8} that fits the column slots in shared memory,
+// leaves a CTA at least 6 pairs, and keeps the launch in ONE wave (cudaOccupancyMaxActiveClusters); if no size
+// gives one wave, the smallest that fits.  0 = use the L2-resident kernel.
 static void choose_jacobi_layout(pfsm_ctx* h) {
     h->jac_cs = 0;
     h->jac_hloc = 0;
     if (getenv("PFSM_JACOBI_L2")) return;  // diagnostic: force the L2-resident kernel (the large-M fallback)
     const size_t budget = 220 * 1024;
     auto hloc_of = [&](int cs) { return (h->M + 2 * cs - 1) / (2 * cs); };
-    int cs = 1;
-    for (; cs <= 8; cs *= 2)
-        if (hloc_of(cs) >= 2 && jacobi_smem_bytes(h->M, hloc_of(cs)) <= budget) break;
-    if (cs > 8 || hloc_of(cs) < 2) return;
-    while (cs < 8 && hloc_of(cs) > JACOBI_THREADS / 32 && 2 * cs * h->P <= 148 && hloc_of(2 * cs) >= 2) cs *= 2;
+    auto fits = [&](int cs) { return hloc_of(cs) >= 2 && jacobi_smem_bytes(h->M, hloc_of(cs)) <= budget; };
+    int cs_min = 1;
+    while (cs_min <= 8 && !fits(cs_min)) cs_min *= 2;
+    if (cs_min > 8) return;
+    int cs = cs_min;
+    for (int c = cs_min; c <= 8; c *= 2) {
+        if (!fits(c) || (c > cs_min && hloc_of(c) < 6)) break;
+        if (jacobi_max_clusters(h->M, c, jacobi_smem_bytes(h->M, hloc_of(c))) >= h->P) cs = c;
+    }
+    if (const char* e = getenv("PFSM_JACOBI_CS")) {  // diagnostic override of the cluster size
+        const int want = atoi(e);
+        if ((want == 1 || want == 2 || want == 4 || want == 8) && fits(want)) cs = want;
+    }
     h->jac_cs = cs;
     h->jac_hloc = hloc_of(cs);
 }
