@@ -67,16 +67,6 @@ __device__ __forceinline__ double fast_rsqrt_pos(double x) {
     y = y * fma(-hx * y, y, 1.5);
     return y;
 }
-// one Newton step (~48 bits): enough for the rotation ANGLE, whose error only delays convergence; the cosine
-// itself is computed with fast_rsqrt_pos so that every rotation stays orthogonal to rounding
-__device__ __forceinline__ double fast_rsqrt_pos_1(double x) {
-    double y = (double)rsqrtf((float)x);
-    return y * fma(-0.5 * x * y, y, 1.5);
-}
-__device__ __forceinline__ double fast_rcp_pos_1(double x) {
-    double r = (double)__frcp_rn((float)x);
-    return r * fma(-x, r, 2.0);
-}
 __device__ __forceinline__ double fast_rcp_pos(double x) {
     double r = (double)__frcp_rn((float)x);
     r = r * fma(-x, r, 2.0);
@@ -234,8 +224,8 @@ jacobi_smem_kernel(const double* __restrict__ A, int64_t N, int32_t M, int32_t m
                     // with one square root and one division: t = 2 ab sign(d) / (|d| + sqrt(d^2 + 4 ab^2)), d = bb - aa
                     const double d = bb - aa;
                     const double z = fma(d, d, 4.0 * ab * ab);
-                    const double den = fabs(d) + z * fast_rsqrt_pos_1(z);
-                    const double tt = copysign(2.0 * ab, (d < 0.0) ? -ab : ab) * fast_rcp_pos_1(den);
+                    const double den = fabs(d) + z * fast_rsqrt_pos(z);
+                    const double tt = copysign(2.0 * ab, (d < 0.0) ? -ab : ab) * fast_rcp_pos(den);
                     const double cs = fast_rsqrt_pos(fma(tt, tt, 1.0)), sn = cs * tt;
 #pragma unroll
                     for (int e = 0; e < E2; ++e) {
