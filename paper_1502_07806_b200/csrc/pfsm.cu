@@ -958,9 +958,15 @@ int64_t pfsm_launches_per_solve(pfsm_handle_t h) {
     if (!h) return 0;
     // jacobi + 2 iters GEMMs + (2 transposes + Gram + diag extract + per panel: diag, panel, trailing (none after the last)) + GEMM + rayleigh
     {
-        const int64_t nb = h->nblk, pairs = nb / 2;
-        // per panel: chol_diag + panel GEMM; per pair of panels: inner update + (if columns remain) trailing update
-        const int64_t trailing = (nb % 2 == 0) ? pairs - 1 : pairs;
+        const int64_t nb = h->nblk, pairs = nb / 2, npairs = (nb + 1) / 2;
+        // per panel: chol_diag + panel GEMM; per pair of panels: inner update; trailing updates: one per pair with
+        // columns left, split in two (next pair's columns / the rest) when the look-ahead schedule is active
+        int64_t trailing = 0;
+        for (int64_t p = 0; p < npairs; ++p) {
+            const int64_t cn0 = std::min<int64_t>(h->N, 2 * (p + 1) * CHOL_NB), cn1 = std::min<int64_t>(h->N, 2 * (p + 2) * CHOL_NB);
+            if (cn0 >= h->N) continue;
+            trailing += (h->lookahead && npairs >= 3 && cn1 < h->N) ? 2 : 1;
+        }
         return 1 + 2 * (int64_t)h->iters + (2 + 1 + 1 + 2 * nb + pairs + trailing) + 2;
     }
 }
