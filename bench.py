@@ -25,8 +25,8 @@ if ROOT not in sys.path:
 
 FP64_NOMINAL_RATIO = 45.0 / 2250.0  # guide's nominal B200 FP64-tensor : bf16-tensor dense peaks
 # dram__bytes_read.sum + dram__bytes_write.sum per full-k gemm_tn_kernel launch, from the committed
-# `ncu --set full` capture profiles/r01_ncu_full_gemm_jacobi.md (config index -> bytes); None = not captured
-NCU_TRAFFIC_PER_GEMM_LAUNCH = {4: 7.54e9 + 0.53e9}
+# `ncu --set full` capture profiles/r01c_ncu_full_gemm_final.md (config index -> bytes); None = not captured
+NCU_TRAFFIC_PER_GEMM_LAUNCH = {4: 8.14e9 + 0.53e9}
 
 
 def algorithmic_flops(N: int, M: int, iters: int) -> dict:

@@ -220,13 +220,18 @@ jacobi_smem_kernel(const double* __restrict__ A, int64_t N, int32_t M, int32_t m
                 }
                 const bool rotate = ab * ab > tol2 * (aa * bb);  // |g_p . g_q| > sqrt(M) eps ||g_p|| ||g_q||
                 if (rotate) {
-                    // t = tan(theta) = sign(zeta) / (|zeta| + sqrt(1 + zeta^2)), zeta = (bb - aa) / (2 ab), written
-                    // with one square root and one division: t = 2 ab sign(d) / (|d| + sqrt(d^2 + 4 ab^2)), d = bb - aa
+                    // The rotation that makes the two columns orthogonal has tan(2 theta) = 2 ab / (bb - aa).  With
+                    // d = bb - aa, r = 1/sqrt(d^2 + 4 ab^2):  cos(2 theta) = |d| r,  cos^2(theta) = x = (1 + |d| r)/2,
+                    // cs = sqrt(x) = x rsqrt(x),  sn = sign(d) ab r / cs = sign(d) ab r rsqrt(x),  t = sn / cs = sn rsqrt(x)
+                    // -- the smaller-angle root, same as t = sign(zeta)/(|zeta| + sqrt(1 + zeta^2)), zeta = d/(2 ab), with
+                    // two dependent reciprocal square roots and no division on the chain.
                     const double d = bb - aa;
-                    const double z = fma(d, d, 4.0 * ab * ab);
-                    const double den = fabs(d) + z * fast_rsqrt_pos(z);
-                    const double tt = copysign(2.0 * ab, (d < 0.0) ? -ab : ab) * fast_rcp_pos(den);
-                    const double cs = fast_rsqrt_pos(fma(tt, tt, 1.0)), sn = cs * tt;
+                    const double r = fast_rsqrt_pos(fma(d, d, 4.0 * ab * ab));
+                    const double xx = fma(0.5 * fabs(d), r, 0.5);
+                    const double rs = fast_rsqrt_pos(xx);
+                    const double cs = xx * rs;
+                    const double sn = ((d < 0.0) ? -ab : ab) * r * rs;
+                    const double tt = sn * rs;
 #pragma unroll
                     for (int e = 0; e < E2; ++e) {
                         const double2 xe = x[e], ye = y[e];
