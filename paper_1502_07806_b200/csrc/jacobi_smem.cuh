@@ -28,12 +28,6 @@ __device__ __forceinline__ uint32_t mapa_shared(uint32_t addr, uint32_t cta) {
     asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(addr), "r"(cta));
     return r;
 }
-__device__ __forceinline__ void st_cluster_f64(uint32_t addr, double v) {
-    asm volatile("st.shared::cluster.f64 [%0], %1;" ::"r"(addr), "d"(v) : "memory");
-}
-__device__ __forceinline__ void st_cluster_v2f64(uint32_t addr, double2 v) {
-    asm volatile("st.shared::cluster.v2.f64 [%0], {%1,%2};" ::"r"(addr), "d"(v.x), "d"(v.y) : "memory");
-}
 // remote shared-memory store whose completion is counted (in bytes) on the destination CTA's mbarrier
 __device__ __forceinline__ void st_async_v2f64(uint32_t raddr, double2 v, uint32_t rmbar) {
     asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v2.f64 [%0], {%1,%2}, [%3];" ::"r"(raddr),
@@ -53,11 +47,8 @@ __device__ __forceinline__ void st_async_s32(uint32_t raddr, int v, uint32_t rmb
 __device__ __forceinline__ void sts128(uint32_t addr, double2 v) {
     asm volatile("st.shared.v2.f64 [%0], {%1,%2};" ::"r"(addr), "d"(v.x), "d"(v.y) : "memory");
 }
-__device__ __forceinline__ void st_cluster_s32(uint32_t addr, int v) {
-    asm volatile("st.shared::cluster.s32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
-}
 
-// Inline FP64 reciprocal square root / reciprocal for well-scaled positive arguments (column norms and their
+// Inline FP64 reciprocal square root for well-scaled positive arguments (column norms and their
 // combinations: no zeros, infinities or subnormals): FP32 seed + two Newton steps (24 -> 48 -> 96 bits), about 8
 // instructions each instead of the library's call with its special-case handling.
 __device__ __forceinline__ double fast_rsqrt_pos(double x) {
@@ -66,12 +57,6 @@ __device__ __forceinline__ double fast_rsqrt_pos(double x) {
     y = y * fma(-hx * y, y, 1.5);
     y = y * fma(-hx * y, y, 1.5);
     return y;
-}
-__device__ __forceinline__ double fast_rcp_pos(double x) {
-    double r = (double)__frcp_rn((float)x);
-    r = r * fma(-x, r, 2.0);
-    r = r * fma(-x, r, 2.0);
-    return r;
 }
 
 // bytes of dynamic shared memory for (M, h_loc): column slots + ids + norms/ranks scratch

@@ -897,10 +897,16 @@ int pfsm_solve_host(pfsm_handle_t h, const double* A_host, double* V_host, doubl
     }
     cudaStream_t st = (cudaStream_t)stream;
     PFSM_CUDA(cudaMemcpyAsync(h->A_stage, A_host, n2, cudaMemcpyHostToDevice, st));
-    int rc = pfsm_solve(h, h->A_stage, h->V_stage, h->lam_stage, stream);
+    int rc = pfsm_solve_partial(h, h->A_stage, h->V_stage, h->lam_stage, stream, 4);  // steps 2-4: V is final
     if (rc) return rc;
-    PFSM_CUDA(cudaMemcpyAsync(V_host, h->V_stage, n2, cudaMemcpyDeviceToHost, st));
+    // V goes back to the host on the side stream while step 5 (which only reads V) computes lambda
+    PFSM_CUDA(cudaEventRecord(h->ev_fork, st));
+    PFSM_CUDA(cudaStreamWaitEvent(h->side, h->ev_fork, 0));
+    PFSM_CUDA(cudaMemcpyAsync(V_host, h->V_stage, n2, cudaMemcpyDeviceToHost, h->side));
+    PFSM_CUDA(cudaEventRecord(h->ev_chain, h->side));
+    if ((rc = pfsm_rayleigh(h, h->A_stage, h->V_stage, h->lam_stage, stream))) return rc;
     PFSM_CUDA(cudaMemcpyAsync(lambda_host, h->lam_stage, h->N * sizeof(double), cudaMemcpyDeviceToHost, st));
+    PFSM_CUDA(cudaStreamWaitEvent(st, h->ev_chain, 0));  // join: the caller's stream covers both copies
     return 0;
 }
 
