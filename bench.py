@@ -302,6 +302,8 @@ def run_ours(args):
         "unit": "TFLOP/s", "frac": achieved / peak, "traffic": NCU_TRAFFIC_PER_GEMM_LAUNCH.get(k),
         "algorithmic_bytes_per_launch": 32.0 * N * N,
         "peak_source": f"{peaks['_source']} bf16_tflops_sustained x nominal FP64:bf16 ratio 45/2250 (of {peaks['_source']})",
+        "fp64_pipe_peak_tflops": 148 * 64 * 2 * 1.965e-3,  # 148 SMs x 64 FP64 FMA/clk x 2 flop x 1.965 GHz
+        "frac_of_fp64_pipe": achieved / (148 * 64 * 2 * 1.965e-3),
         "avg_launch_ms": gemm_ms, "launches_per_step": n_launch3,
         "flops_per_launch": flops["step3"] / max(1, n_launch3),
     }
