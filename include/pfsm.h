@@ -194,7 +194,7 @@ int pfsm_set_alpha(pfsm_handle_t h, double alpha);
 /* Bytes of device workspace the handle currently owns. */
 size_t pfsm_workspace_bytes(pfsm_handle_t h);
 
-/* Number of kernels (and memsets/copies excluded) one pfsm_solve of this handle launches. */
+/* Number of kernel launches (memsets and copies not counted) one pfsm_solve of this handle makes. */
 int64_t pfsm_launches_per_solve(pfsm_handle_t h);
 
 /*
