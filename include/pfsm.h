@@ -80,9 +80,11 @@ int pfsm_solve(pfsm_handle_t h, const double* A, double* V_inout, double* lambda
 
 /*
  * Same solve with HOST buffers: copies A host->device, runs pfsm_solve, copies V and lambda back,
- * all asynchronously on `stream` (pinned host memory recommended), using device staging buffers owned
- * by the handle (2 N^2 doubles more, allocated on first use).  The caller synchronizes the stream
- * before reading V_host / lambda_host.
+ * all asynchronously (pinned host memory recommended), using device staging buffers owned by the handle
+ * (2 N^2 doubles more, allocated on first use).  The copies overlap the compute: the P diagonal blocks that
+ * step 2 needs go first, the full matrix follows on an internal stream under the step-2 kernel, and V returns
+ * while step 5 runs; everything is joined back into `stream`, which the caller synchronizes before reading
+ * V_host / lambda_host.
  */
 int pfsm_solve_host(pfsm_handle_t h, const double* A_host, double* V_host, double* lambda_host, void* stream);
 

@@ -70,10 +70,14 @@ template <int EPL>
 __global__ void __launch_bounds__(JACOBI_THREADS, 1)
 jacobi_smem_kernel(const double* __restrict__ A, int64_t N, int32_t M, int32_t m, int32_t h_loc, SliceTable tab,
                    double* __restrict__ nrm_g, double* __restrict__ V, double* __restrict__ eps,
-                   int* __restrict__ rotcnt, unsigned long long* info, int32_t s_off) {
+                   int* __restrict__ rotcnt, unsigned long long* info, int32_t s_off, int32_t compact) {
     const int CS = (int)cluster_nctarank(), cr = (int)cluster_ctarank();
     const int s = s_off + blockIdx.x / CS;  // s_off: first slice of this launch
     const int lo = tab.lo[s], off = tab.off[s], g0 = tab.g0[s];
+    // the slice's submatrix B_s: a principal block of A (leading dimension N), or -- compact != 0 -- block s of a
+    // packed P x M x M copy of the diagonal blocks (pfsm_solve_host uploads those first)
+    const double* Ab = compact ? A + (size_t)s * M * M : A + (size_t)lo * N + lo;
+    const int64_t ldb = compact ? (int64_t)M : N;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     constexpr int NW = JACOBI_THREADS / 32;
     const int h = h_loc * CS, Mp = 2 * h;
@@ -113,7 +117,7 @@ jacobi_smem_kernel(const double* __restrict__ A, int64_t N, int32_t M, int32_t m
     double bound = 0.0;
     for (int r = tid; r < M; r += JACOBI_THREADS) {
         double sum = 0.0;
-        for (int c = 0; c < M; ++c) sum += fabs(A[(size_t)(lo + c) * N + lo + r]);
+        for (int c = 0; c < M; ++c) sum += fabs(Ab[(size_t)c * ldb + r]);
         bound = fmax(bound, sum);
     }
 #pragma unroll
@@ -138,7 +142,7 @@ jacobi_smem_kernel(const double* __restrict__ A, int64_t N, int32_t M, int32_t m
         for (int r = lane; r < Ms; r += 32) {
             double v = 0.0;
             if (cid < M && r < M) {
-                v = A[(size_t)(lo + cid) * N + lo + r];
+                v = Ab[(size_t)cid * ldb + r];
                 if (r == cid) v += sigma;
             }
             dst[r] = v;

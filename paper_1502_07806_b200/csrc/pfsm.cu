@@ -285,7 +285,8 @@ static int launch_jacobi_t(pfsm_ctx* h, const double* A, double* V, cudaStream_t
 
 extern "C++" {
 template <int EPL>
-static int launch_jacobi_smem_t(pfsm_ctx* h, const double* A, double* V, cudaStream_t st, int32_t s0, int32_t ns) {
+static int launch_jacobi_smem_t(pfsm_ctx* h, const double* A, double* V, cudaStream_t st, int32_t s0, int32_t ns,
+                                int32_t compact) {
     SliceTable tab{h->slice_tab, h->slice_tab + h->P, h->slice_tab + 2 * (size_t)h->P};
     const size_t smem = jacobi_smem_bytes(h->M, h->jac_hloc);
     // static smem (~300 B) + dynamic must stay within the 227 KB opt-in limit; set per launch (handles differ)
@@ -304,7 +305,7 @@ static int launch_jacobi_smem_t(pfsm_ctx* h, const double* A, double* V, cudaStr
     cfg.attrs = attr;
     cfg.numAttrs = 1;
     PFSM_CUDA(cudaLaunchKernelEx(&cfg, jacobi_smem_kernel<EPL>, A, h->N, h->M, h->m, (int32_t)h->jac_hloc, tab,
-                                 h->nrm_g, V, h->eps, h->rotcnt, h->info, s0));
+                                 h->nrm_g, V, h->eps, h->rotcnt, h->info, s0, compact));
     return 0;
 }
 }  // extern "C++"
@@ -379,19 +380,20 @@ static void choose_jacobi_layout(pfsm_ctx* h) {
     h->jac_hloc = hloc_of(cs);
 }
 
-static int launch_jacobi(pfsm_ctx* h, const double* A, double* V, cudaStream_t st, int32_t s0 = 0, int32_t ns = -1) {
+static int launch_jacobi(pfsm_ctx* h, const double* A, double* V, cudaStream_t st, int32_t s0 = 0, int32_t ns = -1,
+                         int32_t compact = 0) {
     if (ns < 0) ns = h->P;
     PFSM_CUDA(cudaMemsetAsync(h->rotcnt, 0, (size_t)h->P * JACOBI_MAX_SWEEPS * sizeof(int), st));
     if (h->jac_cs > 0) {
         switch (jacobi_padded_rows(h->M) / 32) {  // doubles per lane per column
-            case 2: return launch_jacobi_smem_t<2>(h, A, V, st, s0, ns);
-            case 4: return launch_jacobi_smem_t<4>(h, A, V, st, s0, ns);
-            case 6: return launch_jacobi_smem_t<6>(h, A, V, st, s0, ns);
-            case 8: return launch_jacobi_smem_t<8>(h, A, V, st, s0, ns);
-            case 10: return launch_jacobi_smem_t<10>(h, A, V, st, s0, ns);
-            case 12: return launch_jacobi_smem_t<12>(h, A, V, st, s0, ns);
-            case 14: return launch_jacobi_smem_t<14>(h, A, V, st, s0, ns);
-            default: return launch_jacobi_smem_t<16>(h, A, V, st, s0, ns);
+            case 2: return launch_jacobi_smem_t<2>(h, A, V, st, s0, ns, compact);
+            case 4: return launch_jacobi_smem_t<4>(h, A, V, st, s0, ns, compact);
+            case 6: return launch_jacobi_smem_t<6>(h, A, V, st, s0, ns, compact);
+            case 8: return launch_jacobi_smem_t<8>(h, A, V, st, s0, ns, compact);
+            case 10: return launch_jacobi_smem_t<10>(h, A, V, st, s0, ns, compact);
+            case 12: return launch_jacobi_smem_t<12>(h, A, V, st, s0, ns, compact);
+            case 14: return launch_jacobi_smem_t<14>(h, A, V, st, s0, ns, compact);
+            default: return launch_jacobi_smem_t<16>(h, A, V, st, s0, ns, compact);
         }
     }
     if (h->M <= 128) return launch_jacobi_t<4>(h, A, V, st, s0, ns);
@@ -539,8 +541,10 @@ static int run_step5(pfsm_ctx* h, const CUtensorMap& mapV, const CUtensorMap& ma
     return 0;
 }
 
-int pfsm_solve_partial(pfsm_handle_t h, const double* A, double* V, double* lambda_out, void* stream,
-                       int32_t last_step) {
+// band != nullptr: packed copy of the P diagonal blocks for step 2 (A itself may still be in flight on the side
+// stream; `a_ready` is waited for before step 3 reads it)
+static int solve_impl(pfsm_handle_t h, const double* A, double* V, double* lambda_out, void* stream, int32_t last_step,
+                      const double* band, cudaEvent_t a_ready) {
     if (!h) return -1;
     if (!A || ((uintptr_t)A & 15)) return -2;
     if (!V || ((uintptr_t)V & 15)) return -3;
@@ -560,7 +564,8 @@ int pfsm_solve_partial(pfsm_handle_t h, const double* A, double* V, double* lamb
     if (tm) PFSM_CUDA(cudaEventRecord(h->ev[0], st));
     if (!h->keep_info) PFSM_CUDA(cudaMemsetAsync(h->info, 0xFF, sizeof(unsigned long long), st));
     PFSM_CUDA(cudaMemsetAsync(V, 0, (size_t)N * N * sizeof(double), st));
-    if ((rc = launch_jacobi(h, A, V, st))) return rc;
+    if ((rc = launch_jacobi(h, band ? band : A, V, st, 0, -1, band ? 1 : 0))) return rc;
+    if (band) PFSM_CUDA(cudaStreamWaitEvent(st, a_ready, 0));
     if (tm) PFSM_CUDA(cudaEventRecord(h->ev[1], st));
     if (last_step == 2) return 0;
 
@@ -589,6 +594,11 @@ int pfsm_solve_partial(pfsm_handle_t h, const double* A, double* V, double* lamb
         h->ev_valid = true;
     }
     return 0;
+}
+
+int pfsm_solve_partial(pfsm_handle_t h, const double* A, double* V, double* lambda_out, void* stream,
+                       int32_t last_step) {
+    return solve_impl(h, A, V, lambda_out, stream, last_step, nullptr, nullptr);
 }
 
 int pfsm_orthonormalize(pfsm_handle_t h, double* V_inout, void* stream) {
@@ -896,8 +906,26 @@ int pfsm_solve_host(pfsm_handle_t h, const double* A_host, double* V_host, doubl
         if ((rc = dev_alloc(h, (void**)&h->lam_stage, h->N * sizeof(double)))) return rc;
     }
     cudaStream_t st = (cudaStream_t)stream;
-    PFSM_CUDA(cudaMemcpyAsync(h->A_stage, A_host, n2, cudaMemcpyHostToDevice, st));
-    int rc = pfsm_solve_partial(h, h->A_stage, h->V_stage, h->lam_stage, stream, 4);  // steps 2-4: V is final
+    int rc;
+    if (h->jac_cs > 0) {
+        // Step 2 only needs the P diagonal blocks: upload those first (packed, into the L2-Jacobi workspace that the
+        // shared-memory kernel leaves free) and let the full matrix follow on the side stream under the Jacobi kernel.
+        const size_t M = (size_t)h->M;
+        for (int32_t sl = 0; sl < h->P; ++sl) {
+            const int64_t g0 = (int64_t)sl * h->m;
+            const int64_t lo = std::min<int64_t>(std::max<int64_t>(g0 - h->window, 0), h->N - (int64_t)M);
+            PFSM_CUDA(cudaMemcpy2DAsync(h->Gws + (size_t)sl * M * M, M * sizeof(double), A_host + (size_t)lo * h->N + lo,
+                                        (size_t)h->N * sizeof(double), M * sizeof(double), M, cudaMemcpyHostToDevice, st));
+        }
+        PFSM_CUDA(cudaEventRecord(h->ev_fork, st));
+        PFSM_CUDA(cudaStreamWaitEvent(h->side, h->ev_fork, 0));
+        PFSM_CUDA(cudaMemcpyAsync(h->A_stage, A_host, n2, cudaMemcpyHostToDevice, h->side));
+        PFSM_CUDA(cudaEventRecord(h->ev_rest, h->side));
+        rc = solve_impl(h, h->A_stage, h->V_stage, h->lam_stage, stream, 4, h->Gws, h->ev_rest);  // steps 2-4: V is final
+    } else {
+        PFSM_CUDA(cudaMemcpyAsync(h->A_stage, A_host, n2, cudaMemcpyHostToDevice, st));
+        rc = pfsm_solve_partial(h, h->A_stage, h->V_stage, h->lam_stage, stream, 4);
+    }
     if (rc) return rc;
     // V goes back to the host on the side stream while step 5 (which only reads V) computes lambda
     PFSM_CUDA(cudaEventRecord(h->ev_fork, st));
