@@ -190,6 +190,14 @@ int pfsm_get_residuals(pfsm_handle_t h, const double** r_device);
 /* Device pointer to the N shifts eps_i (submatrix eigenvalues) of the last solve (step 2). */
 int pfsm_get_shifts(pfsm_handle_t h, const double** eps_device);
 
+/*
+ * Number of Cholesky-QR passes of step 4: 1 (default) or 2.  One pass leaves ||V^T V - I||_max ~ eps cond(V)^2, which
+ * meets the 1e-12 N gate up to cond(V) ~ 1e3 (BASELINE config 4: cond ~ 500, 5e-13 measured); a second pass
+ * (CholeskyQR2) brings it to ~eps for cond(V) up to ~1e7 at the cost of step 4 twice.  The exact-arithmetic result,
+ * the Gram-Schmidt basis in ascending column order, is the same.
+ */
+int pfsm_set_cholqr_passes(pfsm_handle_t h, int32_t passes);
+
 /* Change alpha (it scales with 1/||A||^2, so it changes when the spectrum's extent does). */
 int pfsm_set_alpha(pfsm_handle_t h, double alpha);
 

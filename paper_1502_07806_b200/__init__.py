@@ -21,7 +21,7 @@ EXPORTS = [
     "pfsm_create", "pfsm_solve", "pfsm_solve_host", "pfsm_solve_partial", "pfsm_orthonormalize", "pfsm_rayleigh", "pfsm_solve_generalized",
     "pfsm_generalized_reduce", "pfsm_solve_warm", "pfsm_standard_form_eq14",
     "pfsm_set_shard", "pfsm_shard_phase", "pfsm_shard_buffer", "pfsm_destroy", "pfsm_get_info",
-    "pfsm_get_step2_sweeps", "pfsm_get_residuals", "pfsm_get_shifts", "pfsm_set_alpha", "pfsm_workspace_bytes",
+    "pfsm_get_step2_sweeps", "pfsm_get_residuals", "pfsm_get_shifts", "pfsm_set_alpha", "pfsm_set_cholqr_passes", "pfsm_workspace_bytes",
     "pfsm_launches_per_solve", "pfsm_enable_step_timing", "pfsm_get_step_ms", "pfsm_probe_fp64_peak",
     "pfsm_strerror",
 ]
@@ -67,6 +67,7 @@ def load(build_if_missing: bool = True):
     lib.pfsm_get_residuals.argtypes = [p, ctypes.POINTER(p)]
     lib.pfsm_get_shifts.argtypes = [p, ctypes.POINTER(p)]
     lib.pfsm_set_alpha.argtypes = [p, dbl]
+    lib.pfsm_set_cholqr_passes.argtypes = [p, i32]
     lib.pfsm_workspace_bytes.argtypes = [p]
     lib.pfsm_workspace_bytes.restype = ctypes.c_size_t
     lib.pfsm_launches_per_solve.argtypes = [p]
@@ -242,6 +243,9 @@ class Handle:
     def set_alpha(self, alpha: float):
         _check(self._lib.pfsm_set_alpha(self._h, alpha), "pfsm_set_alpha")
         self.alpha = alpha
+
+    def set_cholqr_passes(self, passes: int):
+        _check(self._lib.pfsm_set_cholqr_passes(self._h, passes), "pfsm_set_cholqr_passes")
 
     def workspace_bytes(self) -> int:
         return int(self._lib.pfsm_workspace_bytes(self._h))

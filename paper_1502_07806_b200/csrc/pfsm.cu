@@ -99,6 +99,7 @@ struct pfsm_ctx {
     cudaStream_t side = nullptr;       // high-priority stream of the Cholesky look-ahead
     cudaEvent_t ev_chain = nullptr, ev_rest = nullptr, ev_fork = nullptr;
     bool lookahead = true;
+    int32_t cholqr_passes = 1;         // 2 = CholeskyQR2 (re-orthonormalize once; reading R10)
     int32_t sh_rank = 0, sh_world = 1;  // sharded solve: this handle works on rows [sh_rank, sh_rank+1) * N / sh_world
 };
 
@@ -507,7 +508,7 @@ static int stacked_cholesky(pfsm_ctx* h, bool factor, cudaStream_t st, int32_t b
 }
 
 // ---- step 4: Cholesky-QR.  G = V^T V (row-major view: V V^T), S = [G ; V^T] ----
-static int run_step4(pfsm_ctx* h, const CUtensorMap& mapV, double* V, cudaStream_t st) {
+static int run_step4_once(pfsm_ctx* h, const CUtensorMap& mapV, double* V, cudaStream_t st) {
     const int64_t N = h->N;
     const int32_t n = (int32_t)N;
     int rc;
@@ -522,6 +523,16 @@ static int run_step4(pfsm_ctx* h, const CUtensorMap& mapV, double* V, cudaStream
     if ((rc = stacked_cholesky(h, true, st))) return rc;
     transpose_kernel<<<tg, tb, 0, st>>>(h->O + (size_t)N * N, N, V, N, n, n);
     PFSM_CUDA(cudaGetLastError());
+    return 0;
+}
+
+// One pass leaves ||V^T V - I|| ~ eps cond(V)^2; a second pass on the result (CholeskyQR2) brings it to ~eps and does
+// not change the exact-arithmetic result (V R1^-1 R2^-1 with R2 -> I), so it stays the Gram-Schmidt basis.
+static int run_step4(pfsm_ctx* h, const CUtensorMap& mapV, double* V, cudaStream_t st) {
+    for (int32_t pass = 0; pass < h->cholqr_passes; ++pass) {
+        int rc = run_step4_once(h, mapV, V, st);
+        if (rc) return rc;
+    }
     return 0;
 }
 
@@ -979,6 +990,13 @@ int pfsm_get_shifts(pfsm_handle_t h, const double** e) {
     return 0;
 }
 
+int pfsm_set_cholqr_passes(pfsm_handle_t h, int32_t passes) {
+    if (!h) return -1;
+    if (passes < 1 || passes > 2) return -2;
+    h->cholqr_passes = passes;
+    return 0;
+}
+
 int pfsm_set_alpha(pfsm_handle_t h, double alpha) {
     if (!h) return -1;
     if (!std::isfinite(alpha) || !(alpha > 0.0)) return -2;
@@ -1001,7 +1019,7 @@ int64_t pfsm_launches_per_solve(pfsm_handle_t h) {
             if (cn0 >= h->N) continue;
             trailing += (h->lookahead && npairs >= 3 && cn1 < h->N) ? 2 : 1;
         }
-        return 1 + 2 * (int64_t)h->iters + (2 + 1 + 1 + 2 * nb + pairs + trailing) + 2;
+        return 1 + 2 * (int64_t)h->iters + h->cholqr_passes * (2 + 1 + 1 + 2 * nb + pairs + trailing) + 2;
     }
 }
 

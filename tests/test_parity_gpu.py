@@ -562,3 +562,27 @@ def test_seeded_shape_sweep_against_oracle(N, P, w, iters):
     o = oracle.pfsm(p.A, P, w, iters, p.alpha)
     check_gates(p.A, g, o)
     assert np.abs(g["eps"] - o["eps"]).max() <= 1e-12 * max(1.0, p.normF)
+
+
+def test_second_cholqr_pass_restores_orthogonality_of_ill_conditioned_vectors():
+    # vectors with cond ~ 1e5: one Cholesky-QR pass leaves ~eps cond^2 ~ 1e-6 of non-orthogonality, two passes ~eps;
+    # both are the Gram-Schmidt basis (same exact-arithmetic result, reading R10)
+    N = 256
+    Q1, _ = np.linalg.qr(gen.normal(41, gen.STREAM_TEST, 0, N * N).reshape(N, N))
+    Q2, _ = np.linalg.qr(gen.normal(42, gen.STREAM_TEST, 0, N * N).reshape(N, N))
+    X = (Q1 * np.logspace(0, -5, N)) @ Q2.T
+    Vo, info = oracle.step4_mgs(X)
+    assert info == 0
+    h = pfsm.Handle(N, 1, 0, 0, 1.0)
+    errs = {}
+    for passes in (1, 2):
+        h.set_cholqr_passes(passes)
+        dV = dev(X)
+        h.orthonormalize(dV)
+        assert h.info() == 0
+        Vg = dV.cpu().numpy()
+        errs[passes] = np.abs(Vg @ Vg.T - np.eye(N)).max()
+        if passes == 2:
+            assert np.abs(Vg - Vo).max() < 1e-9       # MGS itself loses eps cond ~ 1e-11 here
+    assert errs[2] < 1e-13 and errs[2] < 1e-3 * errs[1]
+    h.destroy()
