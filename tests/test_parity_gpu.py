@@ -586,3 +586,17 @@ def test_second_cholqr_pass_restores_orthogonality_of_ill_conditioned_vectors():
             assert np.abs(Vg - Vo).max() < 1e-9       # MGS itself loses eps cond ~ 1e-11 here
     assert errs[2] < 1e-13 and errs[2] < 1e-3 * errs[1]
     h.destroy()
+
+
+@pytest.mark.parametrize("N,P,w", [(800, 2, 0), (1024, 2, 0), (1024, 4, 128)])
+def test_large_submatrices_up_to_the_library_limit(N, P, w):
+    # M = 400 (shared-memory kernel, cluster of 8), M = 512 (the limit: L2-resident fallback kernel, 16 doubles/lane)
+    p = gen.small_problem(N, 1e-3, 24.0, seed=5000 + N + w)
+    g2 = gpu_solve(p.A, P, w, 1, p.alpha, last_step=2)
+    V2, eps, info2 = oracle.step2(p.A, P, w)
+    assert g2["info"] == 0 and info2 == 0
+    assert np.abs(g2["eps"] - eps).max() <= 1e-12 * max(1.0, p.normF)
+    assert np.abs(align_signs(g2["Vr"], V2) - V2).max() < 1e-8
+    g = gpu_solve(p.A, P, w, 1, p.alpha)
+    o = oracle.pfsm(p.A, P, w, 1, p.alpha)
+    check_gates(p.A, g, o)
