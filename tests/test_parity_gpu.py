@@ -474,10 +474,16 @@ def test_warm_start_identity_basis_equals_plain_solve():
     assert np.abs(g["lam"] - ref["lam"]).max() < 1e-14 and np.abs(g["Vr"] - ref["Vr"]).max() < 1e-13
 
 
-def test_solve_is_cuda_graph_capturable():
-    # the whole solve enqueues kernels and memsets only (no host sync): capture once, replay many times
-    p = gen.problem(0)
-    c = p.cfg
+@pytest.mark.parametrize("big", [False, True])
+def test_solve_is_cuda_graph_capturable(big):
+    # the whole solve enqueues kernels and memsets only (no host sync): capture once, replay many times.
+    # big: N = 896 has 4 panel pairs, so step 4 runs its two-stream look-ahead schedule inside the capture.
+    if big:
+        p = gen.small_problem(896, 1e-3, 16.0, seed=606)
+        c = gen.Config(-1, "graph", 896, 7, 16, 2, 1e-3, 16.0)
+    else:
+        p = gen.problem(0)
+        c = p.cfg
     N = c.N
     h = pfsm.Handle(N, c.P, c.window, c.iters, p.alpha)
     dA = dev(p.A)
