@@ -606,3 +606,25 @@ def test_large_submatrices_up_to_the_library_limit(N, P, w):
     g = gpu_solve(p.A, P, w, 1, p.alpha)
     o = oracle.pfsm(p.A, P, w, 1, p.alpha)
     check_gates(p.A, g, o)
+
+
+@pytest.mark.parametrize("k,reps", [(0, 60), (1, 12)])
+def test_repeated_solves_are_bitwise_identical(k, reps):
+    # race detector: the cluster exchange of step 2, the two-stream schedule of step 4 and every reduction have a
+    # fixed order, so a solve is bitwise reproducible; any data race shows up as a differing bit sooner or later
+    p = gen.problem(k)
+    c = p.cfg
+    N = c.N
+    h = pfsm.Handle(N, c.P, c.window, c.iters, p.alpha)
+    dA = dev(p.A)
+    dV = torch.empty((N, N), dtype=torch.float64, device="cuda")
+    dl = torch.empty((N,), dtype=torch.float64, device="cuda")
+    h.solve(dA, dV, dl)
+    ref_l, ref_V, ref_e = dl.clone(), dV.clone(), h.shifts()
+    for _ in range(reps):
+        dV.fill_(float("nan"))
+        dl.fill_(float("nan"))
+        h.solve(dA, dV, dl)
+        assert torch.equal(dl, ref_l) and torch.equal(dV, ref_V) and torch.equal(h.shifts(), ref_e)
+    assert h.info() == 0
+    h.destroy()
