@@ -9,10 +9,10 @@
 //      top[1] -> top[2] -> ... -> top[h-1] -> bot[h-1] -> bot[h-2] -> ... -> bot[0] -> top[1].
 // CTA k of the cluster owns seats t in [k h_loc, (k+1) h_loc).  Its top and bottom seats are ring buffers of
 // h_loc + 1 column slots each, so "moving one seat" is a head-pointer increment; only the two columns that
-// cross a CTA boundary are copied: they are staged, and after the CTA barrier of the round two warps send them
-// into the spare slots of the neighbours' rings through distributed shared memory with st.async, which completes
-// its bytes on the receiver's mbarrier -- a point-to-point exchange; a cluster barrier is needed only once per
-// sweep (convergence count).  Per round a CTA streams its 2 h_loc columns through the SM's own 128 B/clk
+// cross a CTA boundary are copied: the warp that rotated one sends it, straight from its registers, into the spare
+// slot of the neighbour's ring through distributed shared memory with st.async, which completes its bytes on the
+// receiver's mbarrier -- a point-to-point exchange that overlaps the CTA's other pairs; a cluster barrier is needed
+// only once per sweep (convergence count).  Per round a CTA streams its 2 h_loc columns through the SM's own 128 B/clk
 // shared-memory port instead of the chip-wide L2.
 #pragma once
 #include <cuda_runtime.h>
@@ -63,7 +63,7 @@ __device__ __forceinline__ double fast_rsqrt_pos(double x) {
 inline int jacobi_padded_rows(int M) { return (M + 63) / 64 * 64; }  // column slot length: whole double2 per lane
 inline size_t jacobi_smem_bytes(int M, int h_loc) {
     const size_t nslots = 2 * (size_t)h_loc + 3;
-    return (nslots + 4) * jacobi_padded_rows(M) * sizeof(double) + nslots * sizeof(double) + nslots * sizeof(int) + 16 + (size_t)M * (sizeof(double) + sizeof(int)) + 64;
+    return nslots * jacobi_padded_rows(M) * sizeof(double) + nslots * sizeof(double) + nslots * sizeof(int) + 16 + (size_t)M * (sizeof(double) + sizeof(int)) + 64;
 }
 
 template <int EPL>
@@ -88,16 +88,16 @@ jacobi_smem_kernel(const double* __restrict__ A, int64_t N, int32_t M, int32_t m
     extern __shared__ __align__(16) unsigned char smem_jac[];
     const int nslots = 2 * h_loc + 3;
     double* cols = reinterpret_cast<double*>(smem_jac);                 // cols[slot][Ms]
-    double* stage = cols + (size_t)nslots * Ms;                          // 2 x 2 columns leaving for a neighbour CTA
-    double* nrm2 = stage + 4 * Ms;                                       // squared norm of the column in each slot
+    double* nrm2 = cols + (size_t)nslots * Ms;                                       // squared norm of the column in each slot
     int* ids = reinterpret_cast<int*>(nrm2 + nslots);                    // column id held by each slot
     double* nrm = reinterpret_cast<double*>(ids + ((nslots + 3) & ~3)); // nrm[M], then rank[M]
     int* rank = reinterpret_cast<int*>(nrm + M);
     __shared__ double red[NW];
     __shared__ double s_sigma;
-    __shared__ __align__(8) unsigned long long mbar_in[2];  // [0]: top column from the left CTA, [1]: bottom from the right
-    __shared__ int stage_id[4];
-    __shared__ double stage_n2[4];
+    // incoming-column barriers: [2 dir + par], dir 0 = top column from the left CTA, 1 = bottom column from the right;
+    // rounds alternate between the two barriers of a direction (par = round & 1), so a fast neighbour's next column can
+    // never be counted into the phase this CTA is still waiting for
+    __shared__ __align__(8) unsigned long long mbar_in[4];
 
     // slot map.  slot 0: the fixed column (used by CTA 0 only).  Top ring: slots T0 .. T0+h_loc (CTA 0 uses a
     // ring of h_loc slots for its h_loc-1 moving top seats).  Bottom ring: slots B0 .. B0+h_loc.
@@ -150,18 +150,16 @@ jacobi_smem_kernel(const double* __restrict__ A, int64_t N, int32_t M, int32_t m
         if (lane == 0) ids[slot] = cid;
     }
     if (tid == 0) {
-        mbar_init((uint32_t)__cvta_generic_to_shared(&mbar_in[0]), 1);
-        mbar_init((uint32_t)__cvta_generic_to_shared(&mbar_in[1]), 1);
+        for (int b = 0; b < 4; ++b) mbar_init((uint32_t)__cvta_generic_to_shared(&mbar_in[b]), 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (CS > 1) cluster_sync_all(); else __syncthreads();
 
     const uint32_t mbar_u32 = (uint32_t)__cvta_generic_to_shared(&mbar_in[0]);
-    const uint32_t stage_u32 = (uint32_t)__cvta_generic_to_shared(stage);
     const bool has_left = cr > 0, has_right = cr < CS - 1;  // neighbours that exchange a column with this CTA every round
     const uint32_t col_tx = (uint32_t)(Ms * 8 + 8 + 4);   // bytes one incoming column (+ its squared norm and id) completes
     const uint32_t nrm2_u32 = (uint32_t)__cvta_generic_to_shared(nrm2);
-    uint32_t phase = 0;
+    uint32_t rcount = 0;  // rounds done so far (all sweeps): barrier parity = rcount & 1, its phase bit = (rcount >> 1) & 1
     const uint32_t cols_u32 = (uint32_t)__cvta_generic_to_shared(cols);
     const uint32_t ids_u32 = (uint32_t)__cvta_generic_to_shared(ids);
     const int nrounds = Mp - 1;
@@ -170,8 +168,7 @@ jacobi_smem_kernel(const double* __restrict__ A, int64_t N, int32_t M, int32_t m
     for (int sweep = 0; sweep < JACOBI_MAX_SWEEPS; ++sweep) {
         int nrot = 0;
         for (int rnd = 0; rnd < nrounds; ++rnd) {
-            // staging buffers alternate with the round (a slow sender of round r cannot be overtaken by round r+1's writers)
-            const uint32_t stage_cur = stage_u32 + phase * (uint32_t)(2 * Ms * 8);
+            const uint32_t par = rcount & 1u;
             for (int t = warp; t < h_loc; t += NW) {
                 const int sp = slot_top(t), sq = slot_bot(t);
                 const uint32_t ap = cols_u32 + (uint32_t)(sp * Ms * 8) + 16u * lane;
@@ -207,6 +204,16 @@ jacobi_smem_kernel(const double* __restrict__ A, int64_t N, int32_t M, int32_t m
                     aa = nrm2[sp];
                     bb = nrm2[sq];
                 }
+                // Boundary seats: read what travels with the column now, then meet the other boundary warp.  A column
+                // sent to a neighbour lets that neighbour run ahead and overwrite, with ITS next column, the slot the
+                // other boundary seat is reading from this round -- so neither boundary warp sends before both loaded.
+                const bool boundary = (CS > 1) && (t == 0 || t == h_loc - 1);
+                int idp = 0, idq = 0;
+                if (t == 0 || t == h_loc - 1) {
+                    idp = ids[sp];
+                    idq = ids[sq];
+                }
+                if (boundary) asm volatile("bar.sync 1, 64;" ::: "memory");
                 const bool rotate = ab * ab > tol2 * (aa * bb);  // |g_p . g_q| > sqrt(M) eps ||g_p|| ||g_q||
                 if (rotate) {
                     // The rotation that makes the two columns orthogonal has tan(2 theta) = 2 ab / (bb - aa).  With
@@ -237,16 +244,23 @@ jacobi_smem_kernel(const double* __restrict__ A, int64_t N, int32_t M, int32_t m
                 const bool top_leaves = (t == h_loc - 1) && !top_fixed;
                 const bool bot_leaves = (t == 0);
                 if (top_leaves) {
-                    if (has_right) {  // to the right neighbour's top spare: staged, sent after the CTA barrier below
+                    if (has_right) {  // straight from registers into the right neighbour's top spare
+                        const int dslot = T0 + wrap(head_t + RT - 1, RT);
+                        const uint32_t rcta = (uint32_t)(cr + 1);
+                        const uint32_t rbar = mapa_shared(mbar_u32 + 8u * par, rcta);
+                        const uint32_t base = mapa_shared(cols_u32 + (uint32_t)(dslot * Ms * 8), rcta) + 16u * lane;
 #pragma unroll
-                        for (int e = 0; e < E2; ++e) sts128(stage_cur + 16u * lane + 512u * e, x[e]);
-                        if (lane == 0) { stage_id[2 * phase] = ids[sp]; stage_n2[2 * phase] = aa; }
+                        for (int e = 0; e < E2; ++e) st_async_v2f64(base + 512u * e, x[e], rbar);
+                        if (lane == 0) {
+                            st_async_s32(mapa_shared(ids_u32 + 4u * dslot, rcta), idp, rbar);
+                            st_async_f64(mapa_shared(nrm2_u32 + 8u * dslot, rcta), aa, rbar);
+                        }
                     } else {          // last CTA: the column turns the corner into this CTA's bottom spare
                         const int dslot = B0 + wrap(head_b + h_loc, RT);
                         const uint32_t base = cols_u32 + (uint32_t)(dslot * Ms * 8) + 16u * lane;
 #pragma unroll
                         for (int e = 0; e < E2; ++e) sts128(base + 512u * e, x[e]);
-                        if (lane == 0) { ids[dslot] = ids[sp]; nrm2[dslot] = aa; }
+                        if (lane == 0) { ids[dslot] = idp; nrm2[dslot] = aa; }
                     }
                 } else {
                     if (rotate) {
@@ -256,16 +270,23 @@ jacobi_smem_kernel(const double* __restrict__ A, int64_t N, int32_t M, int32_t m
                     if (lane == 0 && (rotate || rnd == 0)) nrm2[sp] = aa;
                 }
                 if (bot_leaves) {
-                    if (has_left) {   // to the left neighbour's bottom spare: staged
+                    if (has_left) {   // straight from registers into the left neighbour's bottom spare
+                        const int dslot = B0 + wrap(head_b + h_loc, RT);
+                        const uint32_t rcta = (uint32_t)(cr - 1);
+                        const uint32_t rbar = mapa_shared(mbar_u32 + 16u + 8u * par, rcta);
+                        const uint32_t base = mapa_shared(cols_u32 + (uint32_t)(dslot * Ms * 8), rcta) + 16u * lane;
 #pragma unroll
-                        for (int e = 0; e < E2; ++e) sts128(stage_cur + (uint32_t)(Ms * 8) + 16u * lane + 512u * e, y[e]);
-                        if (lane == 0) { stage_id[2 * phase + 1] = ids[sq]; stage_n2[2 * phase + 1] = bb; }
+                        for (int e = 0; e < E2; ++e) st_async_v2f64(base + 512u * e, y[e], rbar);
+                        if (lane == 0) {
+                            st_async_s32(mapa_shared(ids_u32 + 4u * dslot, rcta), idq, rbar);
+                            st_async_f64(mapa_shared(nrm2_u32 + 8u * dslot, rcta), bb, rbar);
+                        }
                     } else {          // CTA 0: the column turns the corner into this CTA's top spare
                         const int dslot = T0 + wrap(head_t0 + RT0 - 1, RT0);
                         const uint32_t base = cols_u32 + (uint32_t)(dslot * Ms * 8) + 16u * lane;
 #pragma unroll
                         for (int e = 0; e < E2; ++e) sts128(base + 512u * e, y[e]);
-                        if (lane == 0) { ids[dslot] = ids[sq]; nrm2[dslot] = bb; }
+                        if (lane == 0) { ids[dslot] = idq; nrm2[dslot] = bb; }
                     }
                 } else {
                     if (rotate) {
@@ -276,44 +297,22 @@ jacobi_smem_kernel(const double* __restrict__ A, int64_t N, int32_t M, int32_t m
                 }
             }
             if (rnd == nrounds - 1 && lane == 0 && nrot) atomicAdd(rot + sweep, nrot);
-            // Every warp of this CTA is done reading and writing its seats; only now may the neighbours' spare
-            // slots be overwritten (they sent us their column of this round after their own barrier, so once it
-            // has arrived they are past all reads of the round too).  The exchange is point to point: st.async
-            // completes its bytes on the receiver's mbarrier, and nobody waits for CTAs it does not talk to.
+            // The boundary columns are already on their way (sent as soon as they were rotated, so the DSMEM latency
+            // hides under the other pairs).  The CTA barrier orders this round's local writes before next round's
+            // reads; then wait for the two incoming columns of this round.  Point to point: nobody waits for CTAs
+            // it does not exchange with.
             __syncthreads();
             if (CS > 1) {
-                if (warp == 0 && has_right) {
-                    const int dslot = T0 + wrap(head_t + RT - 1, RT);
-                    const uint32_t rbar = mapa_shared(mbar_u32, (uint32_t)(cr + 1));
-                    const uint32_t base = mapa_shared(cols_u32 + (uint32_t)(dslot * Ms * 8), (uint32_t)(cr + 1)) + 16u * lane;
-#pragma unroll
-                    for (int e = 0; e < E2; ++e) st_async_v2f64(base + 512u * e, lds128(stage_cur + 16u * lane + 512u * e), rbar);
-                    if (lane == 0) {
-                        st_async_s32(mapa_shared(ids_u32 + 4u * dslot, (uint32_t)(cr + 1)), stage_id[2 * phase], rbar);
-                        st_async_f64(mapa_shared(nrm2_u32 + 8u * dslot, (uint32_t)(cr + 1)), stage_n2[2 * phase], rbar);
-                    }
-                }
-                if (warp == 1 && has_left) {
-                    const int dslot = B0 + wrap(head_b + h_loc, RT);
-                    const uint32_t rbar = mapa_shared(mbar_u32 + 8u, (uint32_t)(cr - 1));
-                    const uint32_t base = mapa_shared(cols_u32 + (uint32_t)(dslot * Ms * 8), (uint32_t)(cr - 1)) + 16u * lane;
-#pragma unroll
-                    for (int e = 0; e < E2; ++e)
-                        st_async_v2f64(base + 512u * e, lds128(stage_cur + (uint32_t)(Ms * 8) + 16u * lane + 512u * e), rbar);
-                    if (lane == 0) {
-                        st_async_s32(mapa_shared(ids_u32 + 4u * dslot, (uint32_t)(cr - 1)), stage_id[2 * phase + 1], rbar);
-                        st_async_f64(mapa_shared(nrm2_u32 + 8u * dslot, (uint32_t)(cr - 1)), stage_n2[2 * phase + 1], rbar);
-                    }
-                }
+                const uint32_t ph = (rcount >> 1) & 1u;
                 if (tid == 64) {
-                    if (has_left) mbar_expect_tx(mbar_u32, col_tx);
-                    if (has_right) mbar_expect_tx(mbar_u32 + 8u, col_tx);
+                    if (has_left) mbar_expect_tx(mbar_u32 + 8u * par, col_tx);
+                    if (has_right) mbar_expect_tx(mbar_u32 + 16u + 8u * par, col_tx);
                 }
-                if (has_left) mbar_wait(mbar_u32, phase);
-                if (has_right) mbar_wait(mbar_u32 + 8u, phase);
-                phase ^= 1u;
+                if (has_left) mbar_wait(mbar_u32 + 8u * par, ph);
+                if (has_right) mbar_wait(mbar_u32 + 16u + 8u * par, ph);
                 if (rnd == nrounds - 1) cluster_sync_all();  // once per sweep: every CTA's rotation count is in
             }
+            ++rcount;
             head_t = wrap(head_t + RT - 1, RT);
             head_t0 = wrap(head_t0 + RT0 - 1, RT0);
             head_b = wrap(head_b + 1, RT);

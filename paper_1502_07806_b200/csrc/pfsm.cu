@@ -363,7 +363,13 @@ static void choose_jacobi_layout(pfsm_ctx* h) {
     h->jac_hloc = 0;
     if (getenv("PFSM_JACOBI_L2")) return;  // diagnostic: force the L2-resident kernel (the large-M fallback)
     const size_t budget = 220 * 1024;
-    auto hloc_of = [&](int cs) { return (h->M + 2 * cs - 1) / (2 * cs); };
+    // seats per CTA; one more (phantom) pair when seat 0 and seat h_loc-1 would fall to the same warp, because the
+    // two boundary seats of a CTA synchronise with each other inside a round (jacobi_smem.cuh)
+    auto hloc_of = [&](int cs) {
+        int hl = (h->M + 2 * cs - 1) / (2 * cs);
+        if (hl > 1 && (hl - 1) % (JACOBI_THREADS / 32) == 0) ++hl;
+        return hl;
+    };
     auto fits = [&](int cs) { return hloc_of(cs) >= 2 && jacobi_smem_bytes(h->M, hloc_of(cs)) <= budget; };
     int cs_min = 1;
     while (cs_min <= 8 && !fits(cs_min)) cs_min *= 2;
