@@ -464,3 +464,34 @@ def test_eq14_error_contracts_with_the_jacobi_iteration_matrix():
     assert np.abs(B @ Z - p.A).max() < 1e-14
     Zs = oracle.eq14_iteration(p.A, B, 40, symmetrize=True)
     assert np.array_equal(Zs, Zs.T)
+
+
+# ---------------------------------------------------------------- seeded sweep of shapes: invariants that hold for ANY PFSM run
+def _oracle_sweep_cases(count=14):
+    u = gen.uniform(424242, gen.STREAM_TEST, 0, 4 * count)
+    out = []
+    for k in range(count):
+        N = 2 * int(3 + u[4 * k] * 45)                       # 6 .. 94
+        divs = [d for d in range(1, N + 1) if N % d == 0]
+        P = divs[int(u[4 * k + 1] * len(divs)) % len(divs)]
+        out.append((N, P, int(u[4 * k + 2] * 12), int(u[4 * k + 3] * 5)))
+    return out
+
+
+@pytest.mark.parametrize("N,P,w,iters", _oracle_sweep_cases())
+def test_oracle_invariants_on_a_seeded_sweep(N, P, w, iters):
+    p = gen.small_problem(N, 2e-3, max(2.0, N / 8.0), seed=7000 + N + P)
+    r = oracle.pfsm(p.A, P, w, iters, p.alpha)
+    assert r["info"] == 0
+    V = r["Vr"]
+    assert np.abs(V @ V.T - np.eye(N)).max() < 1e-12 * N                       # P8
+    assert abs(r["lam"].sum() - np.trace(p.A)) < 1e-12 * N                    # P7
+    ex = np.linalg.eigvalsh(p.A)
+    assert np.all(np.abs(r["lam"][:, None] - ex[None, :]).min(axis=1) <= r["resid"] + 1e-13)   # P9
+    np.testing.assert_allclose(r["lam"], np.einsum("ij,ij->i", V @ p.A, V), atol=1e-13)         # step 5 definition
+    # slice structure: the shifts of slice s are m consecutive eigenvalues of its own submatrix (R7)
+    M, g0, lo, off = oracle.partition(N, P, w)
+    m = N // P
+    for s in range(P):
+        mu = np.linalg.eigvalsh(p.A[lo[s]:lo[s] + M, lo[s]:lo[s] + M])
+        np.testing.assert_allclose(r["eps"][g0[s]:g0[s] + m], mu[off[s]:off[s] + m], atol=1e-13)
