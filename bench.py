@@ -105,7 +105,7 @@ class ClockSampler:
 
 def oracle_sample(cfg_index: int, ncols: int, reps: int, warmup: int):
     """Times the oracle, as it stands, on a bounded sample of config `cfg_index`: slice P/2's submatrix
-    eigensolve (O2), then Eq. 11 (O3) and the Rayleigh quotients (O5) for `ncols` of its eigenvectors.
+    eigensolve (O2), then Eq. 11 (O3), Gram-Schmidt (O4) and the Rayleigh quotients (O5) for `ncols` of its eigenvectors.
     Returns (seconds per sample (list), flops per sample, description, threads)."""
     import numpy as np
 
@@ -128,16 +128,18 @@ def oracle_sample(cfg_index: int, ncols: int, reps: int, warmup: int):
         V0[c0:c1, lo[s]:lo[s] + M] = Y[:, off[s]:off[s] + ncols].T
         eps[c0:c1] = mu[off[s]:off[s] + ncols]
         V3 = oracle.step3(p.A, V0, eps, c.iters, p.alpha, c0, c1)
-        rows = V3[c0:c1]
-        V3[c0:c1] = rows / np.linalg.norm(rows, axis=1, keepdims=True)
+        Q, info = oracle.step4_mgs(V3[c0:c1])          # Gram-Schmidt among the sampled vectors (O4 on a subset)
+        assert info == 0
+        V3[c0:c1] = Q
         oracle.step5(p.A, V3, c0, c1)
         dt = time.perf_counter() - t0
         if rep >= warmup:
             times.append(dt)
-    # algorithmic flops of the sample (same counting rule as the GPU line; step 2 excluded, step 4 not sampled)
-    flops = ncols * (2.0 * N * M + (2 * c.iters - 1) * 2.0 * N * N) + ncols * 2.0 * N * N
-    desc = (f"config {cfg_index} (N={N}): slice {s}'s {M}x{M} Jacobi eigensolve + {c.iters} folded-spectrum "
-            f"iterations and Rayleigh quotients for {ncols} of its {m} eigenvectors (steps O2,O3,O5; O4 not sampled)")
+    # algorithmic flops of the sample (same counting rule as the GPU line; step 2 excluded; step 4 = Gram-Schmidt of
+    # ncols vectors of length N)
+    flops = ncols * (2.0 * N * M + (2 * c.iters - 1) * 2.0 * N * N) + 2.0 * N * ncols * ncols + ncols * 2.0 * N * N
+    desc = (f"config {cfg_index} (N={N}): slice {s}'s {M}x{M} Jacobi eigensolve, {c.iters} folded-spectrum iterations, "
+            f"Gram-Schmidt and Rayleigh quotients for {ncols} of its {m} eigenvectors (steps O2-O5 on a subset)")
     return times, flops, desc, oracle.num_threads()
 
 
