@@ -13,6 +13,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include "gemm_tn.cuh"  // dmma884
+
 namespace pfsm {
 
 struct SliceTable {  // step 1: device-resident, built once in pfsm_create
@@ -223,7 +225,7 @@ jacobi_batched_kernel(const double* __restrict__ A, int64_t N, int32_t M, int32_
 constexpr int CHOL_NB = 128;
 constexpr int CHOL_THREADS = 1024;
 constexpr int CHOL_LDS = CHOL_NB + 1;
-constexpr int CHOL_SMEM = (CHOL_NB * CHOL_LDS + 2 * CHOL_NB + 7 * 256) * 8;  // L below, L^-1 (transposed) above the diagonal
+constexpr int CHOL_SMEM = (CHOL_NB * CHOL_LDS + 3 * CHOL_NB + 64 * 64) * 8;  // L below, L^-1 (transposed) above the diagonal
 
 // diag(G) before the factorization: the breakdown test compares each pivot with its original diagonal entry
 __global__ void extract_diag_kernel(const double* __restrict__ S, int64_t ld, int32_t n, double* __restrict__ gdiag) {
@@ -246,12 +248,9 @@ constexpr double CHOL_BREAKDOWN = 1e-12;
 //   A1 warp 0 factors the 16 x 16 diagonal block (lane = row, __syncwarp between columns)
 //   A2 one thread per row below solves its 16 entries against that block
 //   A3 all threads apply the rank-16 update to the trailing lower triangle
-// then L^-1 by 16 x 16 blocks: B1 eight warps invert the diagonal blocks, B2 block row I from block rows < I.
+// then L^-1: B1 eight warps invert the 16 x 16 diagonal blocks, B2 recursive doubling (b = 16, 32, 64) joins adjacent
+// inverted blocks.  The rank-16 updates of A3 and the products of B2 run on the FP64 tensor pipe (DMMA).
 // Rows/columns >= nb are padded with the identity and masked on output.
-__device__ __forceinline__ double chol_linv(const double* a, const double* idiag, int x, int y) {
-    return x > y ? a[y * CHOL_LDS + x] : (x == y ? idiag[x] : 0.0);  // L^-1[x][y], stored transposed above the diagonal
-}
-
 __global__ void __launch_bounds__(CHOL_THREADS, 1)
 chol_diag_kernel(const double* __restrict__ S, double* __restrict__ Lout, int64_t ld, int32_t k0, int32_t nb,
                  double* __restrict__ Dinv, const double* __restrict__ gdiag, unsigned long long* info) {
@@ -260,8 +259,9 @@ chol_diag_kernel(const double* __restrict__ S, double* __restrict__ Lout, int64_
     // lower part of L^-1 transposed (L^-1[r][c] at a[c][r], r > c); idiag[c] = 1 / L[c][c] = L^-1[c][c].
     double* a = sm;
     double* idiag = sm + CHOL_NB * CHOL_LDS;
-    double* T = idiag + CHOL_NB;  // 7 x 256 scratch of phase B2
-    double* thr = T + 7 * 256;    // breakdown threshold per column (0 for padding columns)
+    double* T = idiag + CHOL_NB;  // 64 x 64 scratch of phase B2
+    double* thr = T + 64 * 64;    // breakdown threshold per column (0 for padding columns)
+    double* ldiag = thr + CHOL_NB;  // L's diagonal while `a`'s diagonal holds L^-1's
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     for (int idx = tid; idx < CHOL_NB * CHOL_NB; idx += CHOL_THREADS) {
         const int i = idx >> 7, c = idx & 127;
@@ -322,21 +322,34 @@ chol_diag_kernel(const double* __restrict__ S, double* __restrict__ Lout, int64_
             for (int j = 0; j < 16; ++j) a[i * CHOL_LDS + j0 + j] = x[j];
         }
         __syncthreads();
-        {  // A3: a[i][c] -= sum_k l[i][k] l[c][k] on the trailing lower triangle
-            const int i = tid & 127, cg = tid >> 7;
-            if (i >= j0 + 16) {
-                double li[16];
+        {  // A3: a[i][c] -= sum_k l[i][k] l[c][k] on the trailing lower triangle, on the FP64 tensor pipe: one
+           // 16 x 16 block per warp (at most 28 lower blocks), K = 16 = four DMMA k-steps.  The part of a diagonal
+           // block above the diagonal gets updated too; nothing reads it before phase B overwrites it.
+            const int nbk = (CHOL_NB - j0 - 16) / 16;
+            if (warp < nbk * (nbk + 1) / 2) {
+                int bi = 0;
+                while ((bi + 1) * (bi + 2) / 2 <= warp) ++bi;
+                const int bj = warp - bi * (bi + 1) / 2;
+                const int i0 = j0 + 16 + 16 * bi, c0 = j0 + 16 + 16 * bj;
+                const int g = lane >> 2, t = lane & 3;
+                double acc[2][2][2] = {{{0.0, 0.0}, {0.0, 0.0}}, {{0.0, 0.0}, {0.0, 0.0}}};
 #pragma unroll
-                for (int k = 0; k < 16; ++k) li[k] = a[i * CHOL_LDS + j0 + k];
-                for (int c = j0 + 16 + cg; c <= i; c += 8) {
-                    double s0 = 0.0, s1 = 0.0;
-#pragma unroll
-                    for (int k = 0; k < 16; k += 2) {
-                        s0 = fma(li[k], a[c * CHOL_LDS + j0 + k], s0);
-                        s1 = fma(li[k + 1], a[c * CHOL_LDS + j0 + k + 1], s1);
-                    }
-                    a[i * CHOL_LDS + c] -= s0 + s1;
+                for (int k = 0; k < 16; k += 4) {
+                    const double x0 = a[(i0 + g) * CHOL_LDS + j0 + k + t], x1 = a[(i0 + 8 + g) * CHOL_LDS + j0 + k + t];
+                    const double y0 = a[(c0 + g) * CHOL_LDS + j0 + k + t], y1 = a[(c0 + 8 + g) * CHOL_LDS + j0 + k + t];
+                    dmma884(acc[0][0][0], acc[0][0][1], x0, y0);
+                    dmma884(acc[0][1][0], acc[0][1][1], x0, y1);
+                    dmma884(acc[1][0][0], acc[1][0][1], x1, y0);
+                    dmma884(acc[1][1][0], acc[1][1][1], x1, y1);
                 }
+#pragma unroll
+                for (int ri = 0; ri < 2; ++ri)
+#pragma unroll
+                    for (int ci = 0; ci < 2; ++ci) {
+                        double* cp = a + (i0 + 8 * ri + g) * CHOL_LDS + c0 + 8 * ci + 2 * t;
+                        cp[0] -= acc[ri][ci][0];
+                        cp[1] -= acc[ri][ci][1];
+                    }
             }
         }
         __syncthreads();
@@ -352,36 +365,83 @@ chol_diag_kernel(const double* __restrict__ S, double* __restrict__ Lout, int64_
         }
     }
     __syncthreads();
-    for (int I = 1; I < 8; ++I) {  // B2: L^-1[I][J] = -L^-1[I][I] * sum_{J<=K<I} L[I][K] L^-1[K][J], all J < I at once
-        for (int e = tid; e < I * 256; e += CHOL_THREADS) {
-            const int J = e >> 8, rr = (e >> 4) & 15, cc = e & 15;
-            const double* lrow = a + (16 * I + rr) * CHOL_LDS;     // L[16I+rr][.]
-            const double* icol = a + (16 * J + cc) * CHOL_LDS;     // L^-1[.][16J+cc], stored transposed
-            // block K = J: L^-1[16J+k][16J+cc] is idiag for k = cc, the stored entry for k > cc, zero for k < cc
-            double s0 = lrow[16 * J + cc] * idiag[16 * J + cc], s1 = 0.0;
-            for (int k = 16 * J + cc + 1; k < 16 * J + 16; ++k) s0 = fma(lrow[k], icol[k], s0);
-            // blocks J < K < I: plain dot product of a row of L with a stored column of L^-1
-            for (int k = 16 * J + 16; k < 16 * I; k += 2) {
-                s0 = fma(lrow[k], icol[k], s0);
-                s1 = fma(lrow[k + 1], icol[k + 1], s1);
-            }
-            T[e] = s0 + s1;
-        }
-        __syncthreads();
-        for (int e = tid; e < I * 256; e += CHOL_THREADS) {
-            const int J = e >> 8, rr = (e >> 4) & 15, cc = e & 15;
-            // -L^-1[I][I] * T: row 16I+rr of the diagonal block's inverse (entries k < rr stored transposed, k = rr in idiag)
-            double s = idiag[16 * I + rr] * T[J * 256 + rr * 16 + cc];
-            for (int k = 0; k < rr; ++k) s = fma(a[(16 * I + k) * CHOL_LDS + 16 * I + rr], T[J * 256 + k * 16 + cc], s);
-            a[(16 * J + cc) * CHOL_LDS + 16 * I + rr] = -s;
-        }
-        __syncthreads();
+    // From here on the diagonal of `a` holds L^-1's diagonal (L's goes to ldiag), so L^-1[x][y] for x >= y is
+    // uniformly a[y][x] (transposed storage).
+    if (tid < CHOL_NB) {
+        ldiag[tid] = a[tid * CHOL_LDS + tid];
+        a[tid * CHOL_LDS + tid] = idiag[tid];
     }
+    __syncthreads();
+    // B2: recursive doubling on the FP64 tensor pipe.  With the inverses A^-1, B^-1 of two adjacent b x b diagonal
+    // blocks known,  [A 0; C B]^-1 = [A^-1 0; -B^-1 C A^-1  B^-1];  b = 16, 32, 64: three levels, each two products,
+    // one 16 x 16 output block per warp (4, 8, 16 warps), fragments gathered straight from the (transposed) storage.
+    {
+        const int g = lane >> 2, t = lane & 3;
+        for (int b = 16, lb = 4; b < CHOL_NB; b *= 2, ++lb) {
+            const int n16 = b >> 4, bpp = n16 * n16, total = (CHOL_NB / (2 * b)) * bpp;
+            const int pr = warp / bpp, rem = warp - pr * bpp, bi = rem / n16, bj = rem - bi * n16;
+            const int o = pr * 2 * b, i0 = 16 * bi, j0 = 16 * bj;
+            double* Tp = T + (pr << (2 * lb));  // T of this pair, b x b row-major
+            if (warp < total) {  // T = C A^-1:  T[i][j] = sum_{k >= j} C[i][k] A^-1[k][j]
+                double acc[2][2][2] = {{{0.0, 0.0}, {0.0, 0.0}}, {{0.0, 0.0}, {0.0, 0.0}}};
+                for (int kb = bj; kb < n16; ++kb) {
+#pragma unroll
+                    for (int k4 = 0; k4 < 16; k4 += 4) {
+                        const int k = 16 * kb + k4 + t;
+                        const double x0 = a[(o + b + i0 + g) * CHOL_LDS + o + k], x1 = a[(o + b + i0 + 8 + g) * CHOL_LDS + o + k];
+                        double y0 = a[(o + j0 + g) * CHOL_LDS + o + k], y1 = a[(o + j0 + 8 + g) * CHOL_LDS + o + k];
+                        if (k < j0 + g) y0 = 0.0;      // A^-1[k][j] = 0 for k < j (the storage holds L there)
+                        if (k < j0 + 8 + g) y1 = 0.0;
+                        dmma884(acc[0][0][0], acc[0][0][1], x0, y0);
+                        dmma884(acc[0][1][0], acc[0][1][1], x0, y1);
+                        dmma884(acc[1][0][0], acc[1][0][1], x1, y0);
+                        dmma884(acc[1][1][0], acc[1][1][1], x1, y1);
+                    }
+                }
+#pragma unroll
+                for (int ri = 0; ri < 2; ++ri)
+#pragma unroll
+                    for (int ci = 0; ci < 2; ++ci) {
+                        double* tp = Tp + ((i0 + 8 * ri + g) << lb) + j0 + 8 * ci + 2 * t;
+                        tp[0] = acc[ri][ci][0];
+                        tp[1] = acc[ri][ci][1];
+                    }
+            }
+            __syncthreads();
+            if (warp < total) {  // out^T[j][i] = -sum_{k <= i} T[k][j] B^-1[i][k], stored at a[o+j][o+b+i]
+                double acc[2][2][2] = {{{0.0, 0.0}, {0.0, 0.0}}, {{0.0, 0.0}, {0.0, 0.0}}};
+                for (int kb = 0; kb <= bi; ++kb) {
+#pragma unroll
+                    for (int k4 = 0; k4 < 16; k4 += 4) {
+                        const int k = 16 * kb + k4 + t;
+                        const double x0 = Tp[(k << lb) + j0 + g], x1 = Tp[(k << lb) + j0 + 8 + g];
+                        double y0 = a[(o + b + k) * CHOL_LDS + o + b + i0 + g], y1 = a[(o + b + k) * CHOL_LDS + o + b + i0 + 8 + g];
+                        if (k > i0 + g) y0 = 0.0;      // B^-1[i][k] = 0 for k > i
+                        if (k > i0 + 8 + g) y1 = 0.0;
+                        dmma884(acc[0][0][0], acc[0][0][1], x0, y0);
+                        dmma884(acc[0][1][0], acc[0][1][1], x0, y1);
+                        dmma884(acc[1][0][0], acc[1][0][1], x1, y0);
+                        dmma884(acc[1][1][0], acc[1][1][1], x1, y1);
+                    }
+                }
+#pragma unroll
+                for (int ri = 0; ri < 2; ++ri)      // tile rows = j, tile columns = i
+#pragma unroll
+                    for (int ci = 0; ci < 2; ++ci) {
+                        double* op = a + (o + j0 + 8 * ri + g) * CHOL_LDS + o + b + i0 + 8 * ci + 2 * t;
+                        op[0] = -acc[ri][ci][0];
+                        op[1] = -acc[ri][ci][1];
+                    }
+            }
+            __syncthreads();
+        }
+    }
+#pragma unroll 4
     for (int idx = tid; idx < CHOL_NB * CHOL_NB; idx += CHOL_THREADS) {
         const int r = idx >> 7, c = idx & 127;
         const bool in = (r < nb && c < nb);
-        Dinv[idx] = in ? chol_linv(a, idiag, r, c) : 0.0;
-        if (in) Lout[(size_t)(k0 + r) * ld + k0 + c] = (c <= r) ? a[r * CHOL_LDS + c] : 0.0;
+        Dinv[idx] = (in && c <= r) ? a[c * CHOL_LDS + r] : 0.0;
+        if (in) Lout[(size_t)(k0 + r) * ld + k0 + c] = (c < r) ? a[r * CHOL_LDS + c] : (c == r ? ldiag[r] : 0.0);
     }
 }
 
