@@ -263,11 +263,18 @@ chol_diag_kernel(const double* __restrict__ S, double* __restrict__ Lout, int64_
     double* thr = T + 64 * 64;    // breakdown threshold per column (0 for padding columns)
     double* ldiag = thr + CHOL_NB;  // L's diagonal while `a`'s diagonal holds L^-1's
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    for (int idx = tid; idx < CHOL_NB * CHOL_NB; idx += CHOL_THREADS) {
-        const int i = idx >> 7, c = idx & 127;
-        double v = (i == c) ? 1.0 : 0.0;
-        if (i < nb && c < nb) v = (c <= i) ? S[(size_t)(k0 + i) * ld + k0 + c] : 0.0;
-        a[i * CHOL_LDS + c] = v;
+    {   // all 16 loads of a thread are issued before the first use (clamped addresses, masked afterwards)
+        double v[CHOL_NB * CHOL_NB / CHOL_THREADS];
+#pragma unroll
+        for (int q = 0; q < CHOL_NB * CHOL_NB / CHOL_THREADS; ++q) {
+            const int idx = tid + q * CHOL_THREADS, i = idx >> 7, c = idx & 127;
+            v[q] = S[(size_t)(k0 + min(i, nb - 1)) * ld + k0 + min(c, nb - 1)];
+        }
+#pragma unroll
+        for (int q = 0; q < CHOL_NB * CHOL_NB / CHOL_THREADS; ++q) {
+            const int idx = tid + q * CHOL_THREADS, i = idx >> 7, c = idx & 127;
+            a[i * CHOL_LDS + c] = (i < nb && c < nb) ? (c <= i ? v[q] : 0.0) : (i == c ? 1.0 : 0.0);
+        }
     }
     if (tid < CHOL_NB) thr[tid] = (tid < nb) ? CHOL_BREAKDOWN * gdiag[k0 + tid] : 0.0;
     __syncthreads();
