@@ -529,6 +529,7 @@ rayleigh_kernel(const double* __restrict__ V, const double* __restrict__ T, int6
     const double2* t2 = reinterpret_cast<const double2*>(T + i * N);
     const int64_t n2 = N / 2;  // N is even
     double s = 0.0;
+#pragma unroll 4
     for (int64_t k = threadIdx.x; k < n2; k += RAY_THREADS) {
         const double2 a = v2[k], b = t2[k];
         s = fma(a.x, b.x, s);
@@ -536,6 +537,7 @@ rayleigh_kernel(const double* __restrict__ V, const double* __restrict__ T, int6
     }
     const double lam = block_sum(s, red);
     double q = 0.0;
+#pragma unroll 4
     for (int64_t k = threadIdx.x; k < n2; k += RAY_THREADS) {
         const double2 a = v2[k], b = t2[k];
         const double e0 = b.x - lam * a.x, e1 = b.y - lam * a.y;

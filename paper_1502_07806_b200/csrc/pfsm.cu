@@ -542,6 +542,19 @@ static int run_step4(pfsm_ctx* h, const CUtensorMap& mapV, double* V, cudaStream
     return 0;
 }
 
+// The kernel reads rows v_i and t_i twice (lambda_i first, then the residual).  With 8 blocks per SM the rows in flight
+// (148 x 8 x 16 N bytes = 155 MB at N = 8192) outgrow the 126 MB L2 and the second read goes to HBM (ncu: 2.0 GB read for
+// 1.07 GB of operands); a dynamic shared-memory reservation caps residency at 3 blocks per SM so the rows stay in L2.
+static int launch_rayleigh(pfsm_ctx* h, const double* V, double* lambda_out, int32_t r0, int32_t rows, cudaStream_t st) {
+    static const size_t RAY_CAP_SMEM = 72 * 1024;
+    const size_t in_flight = (size_t)148 * 8 * 16 * (size_t)h->N;
+    const size_t smem = in_flight > ((size_t)48 << 20) ? RAY_CAP_SMEM : 0;
+    if (smem) PFSM_CUDA(cudaFuncSetAttribute(rayleigh_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    rayleigh_kernel<<<(unsigned)rows, RAY_THREADS, smem, st>>>(V, h->W, h->N, lambda_out, h->resid, r0);
+    PFSM_CUDA(cudaGetLastError());
+    return 0;
+}
+
 // ---- step 5 (reading R11): T = V A, Rayleigh quotients and residual norms ----
 static int run_step5(pfsm_ctx* h, const CUtensorMap& mapV, const CUtensorMap& mapA, double* V, double* lambda_out,
                      cudaStream_t st) {
@@ -552,8 +565,7 @@ static int run_step5(pfsm_ctx* h, const CUtensorMap& mapV, const CUtensorMap& ma
         GemmParams p = base_params();
         p.C = h->W; p.ldc = N; p.mr = n; p.nc = n; p.klen = n;
         if ((rc = launch_gemm<EPI_PLAIN>(mapV, mapA, h->mapW, p, st))) return rc;
-        rayleigh_kernel<<<(unsigned)N, RAY_THREADS, 0, st>>>(V, h->W, N, lambda_out, h->resid, 0);
-        PFSM_CUDA(cudaGetLastError());
+        if ((rc = launch_rayleigh(h, V, lambda_out, 0, n, st))) return rc;
     }
     return 0;
 }
@@ -900,8 +912,7 @@ int pfsm_shard_phase(pfsm_handle_t h, int32_t phase, const double* A, double* V,
         GemmParams p = base_params();
         p.C = h->W; p.ldc = N; p.cr0 = r0; p.mr = rows; p.nc = n; p.xr0 = r0; p.klen = n;
         if ((rc = launch_gemm<EPI_PLAIN>(mapV, mapA, h->mapW, p, st))) return rc;
-        rayleigh_kernel<<<(unsigned)rows, RAY_THREADS, 0, st>>>(V, h->W, N, lambda_out, h->resid, r0);
-        PFSM_CUDA(cudaGetLastError());
+        if ((rc = launch_rayleigh(h, V, lambda_out, r0, rows, st))) return rc;
     }
     return 0;
 }
