@@ -64,6 +64,12 @@ struct GemmParams {
     int64_t ld2;
     const double* eps;  // indexed by absolute C row (SHIFT, UPDATE) or absolute C column (JSTEP)
     double alpha;
+    // Chained launches (programmatic dependent launch, see launch_gemm): this kernel's operand X and its epilogue
+    // operands are the previous kernel's output.  A tile of row block tr starts once wait_cnt[tr] == wait_target
+    // (all tiles of that row block of the previous kernel have stored), and bumps signal_cnt[tr] after its own stores.
+    const int32_t* wait_cnt;
+    int32_t wait_target;
+    int32_t* signal_cnt;
 };
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -151,6 +157,9 @@ gemm_tn_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__
     const uint32_t bar_base = smem_base + GEMM_STAGES * 2 * TILE_BYTES;
     // full[s] at bar_base + 8 s, empty[s] at bar_base + 8 (STAGES + s)
 
+    // lets a kernel launched with programmatic stream serialization become resident while this grid's last wave runs
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+
     int32_t tr, tc;
     if (!tile_coords(p, (int32_t)blockIdx.x, tr, tc)) return;
 
@@ -169,6 +178,18 @@ gemm_tn_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        if (p.wait_cnt) {
+            // The producer grid is resident or finished (it triggered the dependent launch from every CTA), so this
+            // spin cannot starve it.  acquire + bar.sync order every thread's later loads, the proxy fence the TMA reads.
+            const int32_t* c = p.wait_cnt + tr;
+            int32_t seen;
+            for (;;) {
+                asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(seen) : "l"(c) : "memory");
+                if (seen >= p.wait_target) break;
+                __nanosleep(256);
+            }
+            asm volatile("fence.proxy.async.global;" ::: "memory");
+        }
     }
     __syncthreads();
 
@@ -240,6 +261,15 @@ gemm_tn_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__
         if (lane == 0) mbar_arrive(bar_base + 8 * (GEMM_STAGES + s));
     }
 
+    // chained launches: publish this tile (every thread's stores, for generic and TMA readers) and count it
+    auto signal_done = [&]() {
+        if (!p.signal_cnt) return;
+        __threadfence();
+        asm volatile("fence.proxy.async.global;" ::: "memory");
+        __syncthreads();
+        if (threadIdx.x == 0) asm volatile("red.release.gpu.global.add.s32 [%0], 1;" ::"l"(p.signal_cnt + tr) : "memory");
+    };
+
     // ===== epilogue: thread owns C[row0 + 8 i + g][col0 + 8 j + 2 t + {0,1}] =====
     const int32_t row0 = tr * BM + wr * 64, col0 = tc * BN + wc * 32;
     if (EPI != EPI_PLAIN && (tr + 1) * BM <= p.mr && (tc + 1) * BN <= p.nc) {
@@ -262,8 +292,8 @@ gemm_tn_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__
 #pragma unroll
                 for (int j = 0; j < 4; ++j) {
                     if (EPI == EPI_SHIFT || EPI == EPI_UPDATE || EPI == EPI_JSTEP)
-                        u[i][j] = *reinterpret_cast<const double2*>(p.E1 + o + 8 * j);
-                    if (EPI == EPI_UPDATE || EPI == EPI_JSTEP) w[i][j] = *reinterpret_cast<const double2*>(p.E2 + o + 8 * j);
+                        u[i][j] = __ldcg(reinterpret_cast<const double2*>(p.E1 + o + 8 * j));
+                    if (EPI == EPI_UPDATE || EPI == EPI_JSTEP) w[i][j] = __ldcg(reinterpret_cast<const double2*>(p.E2 + o + 8 * j));
                     if (EPI == EPI_SUB) w[i][j] = *reinterpret_cast<const double2*>(p.C + o + 8 * j);
                 }
             }
@@ -290,6 +320,7 @@ gemm_tn_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__
                 }
             }
         }
+        signal_done();
         return;
     }
 #pragma unroll
@@ -310,21 +341,21 @@ gemm_tn_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__
             if (EPI == EPI_SHIFT) {
                 const double* e1 = p.E1 + ar * p.ld1 + ac;
                 if (pair) {
-                    const double2 x = *reinterpret_cast<const double2*>(e1);
+                    const double2 x = __ldcg(reinterpret_cast<const double2*>(e1));
                     v0 -= e * x.x;
                     v1 -= e * x.y;
                 } else
-                    v0 -= e * e1[0];
+                    v0 -= e * __ldcg(e1);
             } else if (EPI == EPI_UPDATE) {
                 const double* e1 = p.E1 + ar * p.ld1 + ac;
                 const double* e2 = p.E2 + ar * p.ld2 + ac;
                 if (pair) {
-                    const double2 x = *reinterpret_cast<const double2*>(e1);
-                    const double2 y = *reinterpret_cast<const double2*>(e2);
+                    const double2 x = __ldcg(reinterpret_cast<const double2*>(e1));
+                    const double2 y = __ldcg(reinterpret_cast<const double2*>(e2));
                     v0 = y.x - p.alpha * (v0 - e * x.x);
                     v1 = y.y - p.alpha * (v1 - e * x.y);
                 } else
-                    v0 = e2[0] - p.alpha * (v0 - e * e1[0]);
+                    v0 = __ldcg(e2) - p.alpha * (v0 - e * __ldcg(e1));
             } else if (EPI == EPI_JSTEP) {
                 const double* e1 = p.E1 + ar * p.ld1 + ac;
                 const double* e2 = p.E2 + ar * p.ld2 + ac;
@@ -344,6 +375,7 @@ gemm_tn_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__
                 cp[0] = v0;
         }
     }
+    signal_done();
 }
 
 }  // namespace pfsm

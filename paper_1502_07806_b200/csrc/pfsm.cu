@@ -99,6 +99,8 @@ struct pfsm_ctx {
     cudaStream_t side = nullptr;       // high-priority stream of the Cholesky look-ahead
     cudaEvent_t ev_chain = nullptr, ev_rest = nullptr, ev_fork = nullptr;
     bool lookahead = true;
+    bool chain = true;                 // step 3: consecutive GEMMs overlap their last waves (row-block counters + PDL)
+    int32_t* chain_cnt = nullptr;      // [2 * iters][ceil(N / BM)] tiles stored per row block of each step-3 GEMM
     int32_t cholqr_passes = 1;         // 2 = CholeskyQR2 (re-orthonormalize once; reading R10)
     int32_t sh_rank = 0, sh_world = 1;  // sharded solve: this handle works on rows [sh_rank, sh_rank+1) * N / sh_world
 };
@@ -111,8 +113,10 @@ static int dev_alloc(pfsm_ctx* h, void** p, size_t bytes) {
 
 // mc: tensor map of the matrix C lives in (used by the SUB / UPDATE epilogues to prefetch the C tile into L2)
 template <int EPI>
+// pdl: launch with programmatic stream serialization -- the grid may become resident while the previous gemm_tn_kernel
+// in the stream drains its last wave; p.wait_cnt must then carry the real dependency (GemmParams).
 static int launch_gemm(const CUtensorMap& mx, const CUtensorMap& my, const CUtensorMap& mc, GemmParams p,
-                       cudaStream_t st) {
+                       cudaStream_t st, bool pdl = false) {
     p.ntr = (p.mr + BM - 1) / BM;
     p.ntc = (p.nc + BN - 1) / BN;
     if (p.mr <= 0 || p.nc <= 0) return 0;
@@ -122,6 +126,21 @@ static int launch_gemm(const CUtensorMap& mx, const CUtensorMap& my, const CUten
     if (!attr_set[EPI]) {
         PFSM_CUDA(cudaFuncSetAttribute(gemm_tn_kernel<EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, GEMM_SMEM));
         attr_set[EPI] = true;
+    }
+    if (pdl) {
+        cudaLaunchConfig_t cfg;
+        memset(&cfg, 0, sizeof(cfg));
+        cfg.gridDim = dim3((unsigned)tiles);
+        cfg.blockDim = dim3(GEMM_THREADS);
+        cfg.dynamicSmemBytes = GEMM_SMEM;
+        cfg.stream = st;
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        at[0].val.programmaticStreamSerializationAllowed = 1;
+        cfg.attrs = at;
+        cfg.numAttrs = 1;
+        PFSM_CUDA(cudaLaunchKernelEx(&cfg, gemm_tn_kernel<EPI>, mx, my, mc, p));
+        return 0;
     }
     gemm_tn_kernel<EPI><<<(unsigned)tiles, GEMM_THREADS, GEMM_SMEM, st>>>(mx, my, mc, p);
     PFSM_CUDA(cudaGetLastError());
@@ -187,6 +206,7 @@ int pfsm_create(pfsm_handle_t* out, int64_t N, int32_t P, int32_t window, int32_
     const int32_t ntr = (int32_t)((N + BM - 1) / BM);
     TRY(dev_alloc(h, (void**)&h->krange, (size_t)ntr * sizeof(int2)));
     TRY(dev_alloc(h, (void**)&h->info, sizeof(unsigned long long)));
+    TRY(dev_alloc(h, (void**)&h->chain_cnt, (size_t)2 * (iters > 0 ? iters : 1) * ntr * sizeof(int32_t)));
 
     // step 1: slice table, and the k-range each 128-row tile of the first product needs
     std::vector<int32_t> tab(3 * (size_t)P);
@@ -229,6 +249,7 @@ int pfsm_create(pfsm_handle_t* out, int64_t N, int32_t P, int32_t window, int32_
         if (e == cudaSuccess) e = cudaEventCreateWithFlags(&h->ev_fork, cudaEventDisableTiming);
         if (e != cudaSuccess) { pfsm_destroy(h); return PFSM_CUDA_ERROR_BASE + (int)e; }
         h->lookahead = getenv("PFSM_NO_LOOKAHEAD") == nullptr;
+        h->chain = getenv("PFSM_NO_CHAIN") == nullptr;
     }
 #undef TRY
     *out = h;
@@ -238,7 +259,7 @@ int pfsm_create(pfsm_handle_t* out, int64_t N, int32_t P, int32_t window, int32_
 int pfsm_destroy(pfsm_handle_t h) {
     if (!h) return 0;
     cudaDeviceSynchronize();
-    void* ptrs[] = {h->W, h->S, h->O, h->Dinv, h->Gws, h->eps, h->resid, h->gdiag, h->rotcnt, h->nrm_g, h->slice_tab, h->krange, h->info,
+    void* ptrs[] = {h->W, h->S, h->O, h->Dinv, h->Gws, h->eps, h->resid, h->gdiag, h->rotcnt, h->nrm_g, h->slice_tab, h->krange, h->info, h->chain_cnt,
                     h->A_stage, h->V_stage, h->lam_stage, h->Ap, h->LT, h->DinvT};
     for (void* p : ptrs)
         if (p) cudaFree(p);
@@ -599,16 +620,30 @@ static int solve_impl(pfsm_handle_t h, const double* A, double* V, double* lambd
     if (last_step == 2) return 0;
 
     // ---- step 3: folded-spectrum iterations (Eq. 11), two products per iteration ----
+    // Each product needs whole rows of the previous one's output, so the GEMMs are serial -- but only row block by row
+    // block: with 4096 tiles on 148 SMs the last wave of each is 100 tiles, and the next GEMM's first tiles (whose row
+    // blocks were finished waves ago) fill the idle SMs.  Hazards: tile (i, j) of GEMM g+1 overwrites what only tiles
+    // (i, .) of GEMM g read, and it starts after all of those have signalled.
+    const int32_t nrb = (n + BM - 1) / BM, ncb = (n + BN - 1) / BN;
+    const bool chain = h->chain && h->iters > 0;
+    if (chain) PFSM_CUDA(cudaMemsetAsync(h->chain_cnt, 0, (size_t)2 * h->iters * nrb * sizeof(int32_t), st));
     for (int it = 0; it < h->iters; ++it) {
         GemmParams p = base_params();  // W = V A - diag(eps) V   (row-major view; A symmetric)
         p.C = h->W; p.ldc = N; p.mr = n; p.nc = n; p.klen = n;
         p.krange = (it == 0) ? h->krange : nullptr;  // start vectors are zero outside their window
         p.E1 = V; p.ld1 = N; p.eps = h->eps;
-        if ((rc = launch_gemm<EPI_SHIFT>(mapV, mapA, h->mapW, p, st))) return rc;
         GemmParams q = base_params();  // V <- V - alpha (W A - diag(eps) W)
         q.C = V; q.ldc = N; q.mr = n; q.nc = n; q.klen = n;
         q.E1 = h->W; q.ld1 = N; q.E2 = V; q.ld2 = N; q.eps = h->eps; q.alpha = h->alpha;
-        if ((rc = launch_gemm<EPI_UPDATE>(h->mapW, mapA, mapV, q, st))) return rc;
+        if (chain) {
+            int32_t* c0 = h->chain_cnt + (size_t)(2 * it) * nrb;
+            p.signal_cnt = c0;
+            q.signal_cnt = c0 + nrb;
+            q.wait_cnt = c0; q.wait_target = ncb;
+            if (it > 0) { p.wait_cnt = c0 - nrb; p.wait_target = ncb; }
+        }
+        if ((rc = launch_gemm<EPI_SHIFT>(mapV, mapA, h->mapW, p, st, chain && it > 0))) return rc;
+        if ((rc = launch_gemm<EPI_UPDATE>(h->mapW, mapA, mapV, q, st, chain))) return rc;
     }
     if (tm) PFSM_CUDA(cudaEventRecord(h->ev[2], st));
     if (last_step == 3) return 0;
