@@ -149,7 +149,7 @@ def run_reference(args):
         return 0
     k = args.config
     import pfsm_inputs as gen
-    c = gen.CONFIGS[k]
+    c = gen.config(k)
     times, flops, desc, threads = oracle_sample(k, args.ref_cols, args.steps, args.warmup)
     total = sum(times)
     value = flops * len(times) / total * 1e-12
@@ -169,7 +169,8 @@ def run_reference(args):
 
 
 def workload_config(c, n_gpus: int, sharded: bool = False) -> dict:
-    return {"workload": f"BASELINE.json configs[{c.index}]: {c.name}, synthetic A = D + E",
+    origin = f"BASELINE.json configs[{c.index}]" if c.index < len(gen.CONFIGS) else "extra (SURVEY 8(f) f4)"
+    return {"workload": f"{origin}: {c.name}, synthetic A = D + E",
             "N": c.N, "P": c.P, "window": c.window, "M": c.M, "iters": c.iters,
             "alpha": "0.5/max|d|^2", "replicas": n_gpus, "parallelism": (f"one solve sharded over {n_gpus} ranks (all-gathers between the 4 phases)" if sharded
                             else f"replicas x{n_gpus}"),
@@ -369,7 +370,7 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=4, help="BASELINE.json config index (default 4: N=8192)")
+    ap.add_argument("--config", type=int, default=4, help="BASELINE.json config index (default 4: N=8192); 5 = Cu256-shaped N=1664 extra case")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--cpu-cols", type=int, default=128, help="eigenvectors in the cpu_baseline sample")
     ap.add_argument("--ref-cols", type=int, default=8, help="eigenvectors per step of --impl reference")

@@ -73,13 +73,26 @@ def num_threads() -> int:
     return int(_load().oracle_num_threads())
 
 
-def partition(N: int, P: int, w: int):
-    """O1 (PAPER.md:88).  Returns (M, g0, lo, off) as int64 arrays of length P."""
-    g0, lo, off = (np.zeros(P, dtype=np.int64) for _ in range(3))
+def _partition_full(N: int, P: int, w: int):
+    if P < 1:
+        raise ValueError("invalid partition (P < 1)")
+    g0 = np.zeros(P + 1, dtype=np.int64)
+    lo, off = (np.zeros(P, dtype=np.int64) for _ in range(2))
     M = _load().oracle_partition(N, P, w, g0.ctypes.data, lo.ctypes.data, off.ctypes.data)
     if M < 0:
-        raise ValueError("invalid partition (N % P != 0 or bad sizes)")
+        raise ValueError("invalid partition (need 1 <= P <= N, w >= 0)")
     return int(M), g0, lo, off
+
+
+def partition(N: int, P: int, w: int):
+    """O1 (PAPER.md:88).  Returns (M, g0, lo, off) as int64 arrays of length P."""
+    M, g0, lo, off = _partition_full(N, P, w)
+    return M, g0[:P].copy(), lo, off
+
+
+def slice_counts(N: int, P: int) -> np.ndarray:
+    """Eigenpairs per slice, m_s = g0[s+1] - g0[s] (all N/P when P divides N; reading R14 otherwise)."""
+    return np.diff(_partition_full(N, P, 0)[1])
 
 
 def jacobi_eig(B):

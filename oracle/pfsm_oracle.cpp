@@ -41,18 +41,21 @@ extern "C" {
 
 /* ---------------------------------------------------------------------------------------------
  * O1  Partition (readings R6, R7, R14).
- * m = N/P; M = min(N, m + 2w).  Slice s: g0 = s*m, lo = clamp(g0 - w, 0, N - M), off = g0 - lo.
- * Returns M, or -1 if N % P != 0.
+ * Slice s holds the eigen-indices g0[s] .. g0[s+1]-1 with g0[s] = floor(s N / P) (m = N/P of them when P divides N,
+ * the paper's case; otherwise floor(N/P) or ceil(N/P) -- R14).  Every submatrix has the same order
+ * M = min(N, ceil(N/P) + 2w); lo = clamp(g0 - w, 0, N - M), off = g0 - lo.
+ * g0 has P + 1 entries (g0[P] = N).  Returns M, or -1 for bad sizes (P > N leaves a slice empty).
  * ------------------------------------------------------------------------------------------- */
 int64_t oracle_partition(int64_t N, int64_t P, int64_t w, int64_t* g0, int64_t* lo, int64_t* off) {
-    if (N < 1 || P < 1 || w < 0 || N % P != 0) return -1;
-    const int64_t m = N / P;
-    const int64_t M = std::min<int64_t>(N, m + 2 * w);
+    if (N < 1 || P < 1 || w < 0 || P > N) return -1;
+    const int64_t mmax = (N + P - 1) / P;
+    const int64_t M = std::min<int64_t>(N, mmax + 2 * w);
     for (int64_t s = 0; s < P; ++s) {
-        g0[s] = s * m;
+        g0[s] = (s * N) / P;
         lo[s] = std::min<int64_t>(std::max<int64_t>(g0[s] - w, 0), N - M);
         off[s] = g0[s] - lo[s];
     }
+    g0[P] = N;
     return M;
 }
 
@@ -122,16 +125,16 @@ int oracle_jacobi_eig(int64_t n, double* B, double* mu, double* Y) {
 
 /* ---------------------------------------------------------------------------------------------
  * O2  Step 2.  For each slice s: B_s = A[lo:lo+M, lo:lo+M]; B_s Y = Y diag(mu);
- * for j < m: eps[g0+j] = mu[off+j]; V[:, g0+j] = 0 except rows lo..lo+M-1 <- Y[:, off+j]
+ * for j < m_s = g0[s+1] - g0[s]: eps[g0+j] = mu[off+j]; V[:, g0+j] = 0 except rows lo..lo+M-1 <- Y[:, off+j]
  * ("the elements of x_i that do not have a corresponding component in the submatrix solution
  * are set to zero").  Slices are independent (one per node in the paper).
  * Returns 0, or N + s + 1 if slice s's Jacobi did not converge.
  * ------------------------------------------------------------------------------------------- */
 int64_t oracle_step2(int64_t N, int64_t P, int64_t w, const double* A, double* V, double* eps) {
-    std::vector<int64_t> g0(P), lo(P), off(P);
+    if (P < 1) return -1;
+    std::vector<int64_t> g0(P + 1), lo(P), off(P);
     const int64_t M = oracle_partition(N, P, w, g0.data(), lo.data(), off.data());
     if (M < 0) return -1;
-    const int64_t m = N / P;
     int64_t info = 0;
 #pragma omp parallel for schedule(dynamic, 1)
     for (int64_t s = 0; s < P; ++s) {
@@ -143,6 +146,7 @@ int64_t oracle_step2(int64_t N, int64_t P, int64_t w, const double* A, double* V
 #pragma omp critical
             if (info == 0 || N + s + 1 < info) info = N + s + 1;
         }
+        const int64_t m = g0[s + 1] - g0[s];
         for (int64_t j = 0; j < m; ++j) {
             const int64_t i = g0[s] + j;
             eps[i] = mu[off[s] + j];

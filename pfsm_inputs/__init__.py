@@ -109,10 +109,22 @@ CONFIGS = [
     Config(4, "metal, dense spectrum (Al4000 shape)", 8192, 64, 64, 5, 2e-3, 128.0),
 ]
 
+# Beyond BASELINE.json: the size of the paper's Table I workload (256-atom copper cell with 256
+# unoccupied orbitals, N = 1664) with the submatrix width the paper recommends, gamma = M / N = 0.25
+# (PAPER.md:100-108): m = 128, window 144, M = 416.
+EXTRA_CONFIGS = [
+    Config(5, "transition metal with unoccupied states (Cu256 shape, Table I), gamma = 0.25", 1664, 13, 144, 3, 2e-3, 64.0),
+]
+
+
+def config(k: int) -> Config:
+    """BASELINE.json config k (0-4) or an extra one (5)."""
+    return CONFIGS[k] if k < len(CONFIGS) else EXTRA_CONFIGS[k - len(CONFIGS)]
+
 
 def spectrum(k: int) -> np.ndarray:
     """The intended eigenvalues d (sorted ascending) of config k -- SURVEY.md §8(d) table."""
-    c = CONFIGS[k]
+    c = config(k)
     s, N = c.seed, c.N
     if k == 0:
         d = -1.0 + 2.0 * uniform(s, STREAM_D, 0, N)
@@ -133,6 +145,11 @@ def spectrum(k: int) -> np.ndarray:
     elif k == 4:
         u = uniform(s, STREAM_D, 0, N)
         d = -1.0 + 4.0 * u ** (2.0 / 3.0)  # density ~ sqrt(E + 1) on [-1, 3]
+    elif k == 5:
+        dband = -0.40 + 0.30 * uniform(s, STREAM_D, 0, 1280)       # narrow, dense d band: 5 states per atom
+        u = uniform(s, STREAM_D, 1280, 384)
+        spband = -0.80 + 2.0 * u ** (2.0 / 3.0)                     # free-electron-like s/p band, density ~ sqrt(E)
+        d = np.concatenate([dband, spband])
     else:
         raise IndexError(k)
     d = np.sort(d)
@@ -160,7 +177,7 @@ def alpha_rule(d: np.ndarray) -> float:
 def problem(k: int, generalized: bool = False, seed_offset: int = 0) -> Problem:
     """Matrix + parameters of config k.  seed_offset draws an independent matrix of the same
     shape (used for multi-GPU replicas: rank r solves problem(k, seed_offset=r))."""
-    c = CONFIGS[k]
+    c = config(k)
     d = spectrum(k)
     seed = c.seed + 1000 * seed_offset
     A = banded_symmetric(c.N, d, c.amp, c.width, seed, STREAM_E)

@@ -44,8 +44,33 @@ def test_partition_baseline_configs():
 def test_partition_wide_window_and_bad_args():
     M, g0, lo, off = oracle.partition(16, 4, 100)
     assert M == 16 and lo.tolist() == [0, 0, 0, 0] and off.tolist() == [0, 4, 8, 12]
-    with pytest.raises(ValueError):
-        oracle.partition(10, 3, 1)
+    for bad in [(10, 0, 1), (10, 11, 1), (10, 3, -1), (0, 1, 0)]:
+        with pytest.raises(ValueError):
+            oracle.partition(*bad)
+
+
+def test_partition_uneven_hand_case():
+    # R14: N = 10, P = 3, w = 1.  g0 = floor(s N / P) = 0, 3, 6: slices of 3, 3 and 4 eigenpairs; every
+    # submatrix has order ceil(10/3) + 2 = 6; lo = clamp(g0 - 1, 0, 4), off = g0 - lo.
+    M, g0, lo, off = oracle.partition(10, 3, 1)
+    assert M == 6
+    assert g0.tolist() == [0, 3, 6] and oracle.slice_counts(10, 3).tolist() == [3, 3, 4]
+    assert lo.tolist() == [0, 2, 4] and off.tolist() == [0, 1, 2]
+
+
+@pytest.mark.parametrize("N,P,w", [(10, 3, 1), (250, 7, 9), (97, 5, 0), (1664, 12, 100), (64, 64, 2), (50, 49, 3), (31, 4, 40)])
+def test_partition_invariants_any_sizes(N, P, w):
+    M, g0, lo, off = oracle.partition(N, P, w)
+    cnt = oracle.slice_counts(N, P)
+    assert cnt.sum() == N and cnt.min() >= N // P and cnt.max() <= -(-N // P)      # slices tile 0..N-1, sizes differ by <= 1
+    assert np.array_equal(g0, np.concatenate([[0], np.cumsum(cnt)[:-1]]))
+    assert M == min(N, cnt.max() + 2 * w)
+    assert np.all(lo >= 0) and np.all(lo + M <= N)                                 # window inside the matrix
+    assert np.all(off == g0 - lo) and np.all(off >= 0) and np.all(off + cnt <= M)  # the slice's rows are inside its window
+    inner = (g0 - w >= 0) & (g0 - w + M <= N)
+    assert np.all(off[inner] == w)                                                 # unclamped windows are centred (halo w below)
+    if N % P == 0:
+        assert np.all(cnt == N // P)
 
 
 # ---------------------------------------------------------------- P6: 2x2 / 3x3 hand cases
@@ -91,7 +116,7 @@ def test_jacobi_known_spectrum(N):
 
 
 # ---------------------------------------------------------------- P1: diagonal A is a fixed point of every step
-@pytest.mark.parametrize("P,w,iters", [(4, 3, 2), (1, 0, 1), (8, 0, 3), (2, 100, 4)])
+@pytest.mark.parametrize("P,w,iters", [(4, 3, 2), (1, 0, 1), (8, 0, 3), (2, 100, 4), (5, 2, 2), (7, 0, 1), (31, 1, 2)])
 def test_diagonal_input_exact(P, w, iters):
     N = 32
     d = np.sort(gen.uniform(5, gen.STREAM_TEST, 0, N) * 2 - 1)
@@ -144,8 +169,38 @@ def test_block_diagonal_slices_exact(w):
         assert np.abs(rows[:, mask]).max() < 1e-15
 
 
+@pytest.mark.parametrize("w", [0, 3])
+def test_block_diagonal_uneven_slices_exact(w):
+    # Same pin with P not dividing N (R14): N = 22, P = 4 -> slices of 5, 6, 5, 6 eigenpairs at g0 = 0, 5, 11, 16.
+    # Blocks = slices, spectra separated, so slice s must return exactly block s's eigenpairs; a wrong slice size,
+    # start or window offset mixes neighbouring blocks and fails.
+    N, P = 22, 4
+    cnt = oracle.slice_counts(N, P)
+    assert cnt.tolist() == [5, 6, 5, 6]
+    g0 = np.concatenate([[0], np.cumsum(cnt)])
+    A = np.zeros((N, N))
+    expected = []
+    for s in range(P):
+        d = 10.0 * s + np.sort(gen.uniform(78, gen.STREAM_TEST, 100 * s, int(cnt[s])))
+        Bs, _ = known_spectrum_matrix(int(cnt[s]), d, seed=400 + s, nreflect=2)
+        A[g0[s]:g0[s + 1], g0[s]:g0[s + 1]] = Bs
+        expected.append(np.linalg.eigvalsh(Bs))
+    expected = np.concatenate(expected)
+    r = oracle.pfsm(A, P, w, 2, 0.5 / 31.0 ** 2)
+    assert r["info"] == 0
+    nA = np.linalg.norm(A)
+    np.testing.assert_allclose(r["lam"], expected, atol=1e-14 * nA)
+    np.testing.assert_allclose(r["eps"], expected, atol=1e-14 * nA)
+    assert r["resid"].max() < 1e-14 * nA
+    V = r["Vr"]
+    for s in range(P):
+        mask = np.ones(N, bool)
+        mask[g0[s]:g0[s + 1]] = False
+        assert np.abs(V[g0[s]:g0[s + 1]][:, mask]).max() < 1e-15
+
+
 # ---------------------------------------------------------------- P3: P=1 or m+2w >= N reduces to a full eigensolve
-@pytest.mark.parametrize("P,w", [(1, 0), (4, 40)])
+@pytest.mark.parametrize("P,w", [(1, 0), (4, 40), (3, 40), (7, 20)])
 def test_full_window_reduces_to_eigh(P, w):
     N = 40
     p = gen.small_problem(N, 0.05, 6.0, seed=9)
@@ -159,17 +214,17 @@ def test_full_window_reduces_to_eigh(P, w):
 
 
 # ---------------------------------------------------------------- step 2 start vectors
-def test_step2_zero_padding_and_shifts():
-    N, P, w = 48, 4, 5
+@pytest.mark.parametrize("N,P,w", [(48, 4, 5), (50, 4, 5), (47 + 1, 7, 3)])
+def test_step2_zero_padding_and_shifts(N, P, w):
     p = gen.small_problem(N, 0.02, 4.0, seed=21)
     M, g0, lo, off = oracle.partition(N, P, w)
     Vr, eps, info = oracle.step2(p.A, P, w)
     assert info == 0
-    m = N // P
+    cnt = oracle.slice_counts(N, P)
     for s in range(P):
         B = p.A[lo[s]:lo[s] + M, lo[s]:lo[s] + M]
         mu, Y = np.linalg.eigh(B)
-        for j in range(m):
+        for j in range(cnt[s]):
             i = g0[s] + j
             assert abs(eps[i] - mu[off[s] + j]) < 1e-14
             v = Vr[i]
@@ -474,6 +529,8 @@ def _oracle_sweep_cases(count=14):
         N = 2 * int(3 + u[4 * k] * 45)                       # 6 .. 94
         divs = [d for d in range(1, N + 1) if N % d == 0]
         P = divs[int(u[4 * k + 1] * len(divs)) % len(divs)]
+        if k % 3 == 2:
+            P = 1 + int(u[4 * k + 1] * min(N, 12))               # any P: uneven slices (R14)
         out.append((N, P, int(u[4 * k + 2] * 12), int(u[4 * k + 3] * 5)))
     return out
 
@@ -491,7 +548,7 @@ def test_oracle_invariants_on_a_seeded_sweep(N, P, w, iters):
     np.testing.assert_allclose(r["lam"], np.einsum("ij,ij->i", V @ p.A, V), atol=1e-13)         # step 5 definition
     # slice structure: the shifts of slice s are m consecutive eigenvalues of its own submatrix (R7)
     M, g0, lo, off = oracle.partition(N, P, w)
-    m = N // P
+    cnt = oracle.slice_counts(N, P)
     for s in range(P):
         mu = np.linalg.eigvalsh(p.A[lo[s]:lo[s] + M, lo[s]:lo[s] + M])
-        np.testing.assert_allclose(r["eps"][g0[s]:g0[s] + m], mu[off[s]:off[s] + m], atol=1e-13)
+        np.testing.assert_allclose(r["eps"][g0[s]:g0[s] + cnt[s]], mu[off[s]:off[s] + cnt[s]], atol=1e-13)

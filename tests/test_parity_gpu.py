@@ -272,9 +272,10 @@ def test_solve_on_a_side_stream():
     h.destroy()
 
 
-@pytest.mark.parametrize("k", [0, 1, 2])
+@pytest.mark.parametrize("k", [0, 1, 2, 5])
 def test_baseline_configs_full_oracle(k):
-    """BASELINE.json configs 0-2 at full size: element-by-element gates against the full oracle run."""
+    """BASELINE.json configs 0-2 at full size, and the Cu256-shaped extra case (N = 1664, window at the paper's
+    gamma = 0.25: M = 416, clamped windows on 4 of 13 slices): element-by-element gates against the full oracle run."""
     p = gen.problem(k)
     c = p.cfg
     g = gpu_solve(p.A, c.P, c.window, c.iters, p.alpha)
