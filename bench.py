@@ -169,7 +169,7 @@ def run_reference(args):
 
 
 def workload_config(c, n_gpus: int, sharded: bool = False) -> dict:
-    origin = f"BASELINE.json configs[{c.index}]" if c.index < len(gen.CONFIGS) else "extra (SURVEY 8(f) f4)"
+    origin = f"BASELINE.json configs[{c.index}]" if c.index <= 4 else "extra (SURVEY 8(f) f4)"
     return {"workload": f"{origin}: {c.name}, synthetic A = D + E",
             "N": c.N, "P": c.P, "window": c.window, "M": c.M, "iters": c.iters,
             "alpha": "0.5/max|d|^2", "replicas": n_gpus, "parallelism": (f"one solve sharded over {n_gpus} ranks (all-gathers between the 4 phases)" if sharded

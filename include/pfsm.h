@@ -57,9 +57,10 @@ typedef struct pfsm_ctx* pfsm_handle_t; /* opaque */
  * (about 5 N^2 doubles + P M^2 doubles) on the current device.           [step 1, PAPER.md:88]
  *   out     host pointer receiving the handle
  *   N       matrix order; N >= 2, even (TMA row pitch must be a multiple of 16 bytes)
- *   P       number of spectral slices; P >= 1 and N % P == 0 (the paper writes m = N/P)
+ *   P       number of spectral slices; 1 <= P <= N.  Slice s holds eigen-indices floor(s N / P) .. floor((s+1) N / P) - 1:
+ *           N/P of them when P divides N (the paper writes m = N/P), else floor(N/P) or ceil(N/P) (reading R14)
  *   window  halo rows/columns added on each side of a slice's diagonal block; >= 0.
- *           M = min(N, N/P + 2*window) must be <= 512 in this version.
+ *           M = min(N, ceil(N/P) + 2*window), the order of every submatrix, must be <= 512 in this version.
  *   iters   folded-spectrum iterations of Eq. 11; >= 0
  *   alpha   step length of Eq. 11; finite and > 0.  The library does not estimate spectra:
  *           alpha = 0.5 / max|lambda|^2 keeps every damping factor 1 - alpha (lambda - eps)^2 in [-1, 1].
@@ -151,7 +152,7 @@ int pfsm_standard_form_eq14(pfsm_handle_t h, const double* A, const double* B, d
 /*
  * One solve sharded over `world` GPUs (one process and one handle per GPU; the paper's decomposition of slices
  * over nodes, with its all-gather).  Rank g owns slices [g P/world, (g+1) P/world),
- * i.e. columns [g N/world, (g+1) N/world) of V.  Requires P % world == 0 and (N/world) % 128 == 0.  A is
+ * i.e. columns [g N/world, (g+1) N/world) of V.  Requires N % P == 0, P % world == 0 and (N/world) % 128 == 0.  A is
  * replicated.  pfsm_shard_phase runs compute phase 1..4 on the rank's share; between the phases the CALLER
  * all-gathers (NCCL/torch.distributed; see paper_1502_07806_b200/sharded.py):
  *   after phase 1 (steps 2-3 on own columns):   the column blocks of V                  (V itself, N x N)

@@ -66,20 +66,26 @@ inline size_t jacobi_smem_bytes(int M, int h_loc) {
     return nslots * jacobi_padded_rows(M) * sizeof(double) + nslots * sizeof(double) + nslots * sizeof(int) + 16 + (size_t)M * (sizeof(double) + sizeof(int)) + 64;
 }
 
+// Threads per CTA.  A warp keeps both columns of its pair in registers (2 EPL doubles per lane): with 1024 threads the
+// register file allows 64 per thread, which holds EPL <= 8 (M <= 256); wider columns get 512 threads (128 registers)
+// and a warp takes two pairs per round instead of spilling the columns to local memory (measured at 13 slices, per
+// round: M = 416 6.6 -> 3.1 us, M = 384 3.7 -> 2.9 us; at EPL = 10 the 64-byte spill of the 1024-thread build is faster).
+__host__ __device__ constexpr int jacobi_smem_threads(int epl) { return epl <= 10 ? 1024 : 512; }
+
 template <int EPL>
-__global__ void __launch_bounds__(JACOBI_THREADS, 1)
-jacobi_smem_kernel(const double* __restrict__ A, int64_t N, int32_t M, int32_t m, int32_t h_loc, SliceTable tab,
+__global__ void __launch_bounds__(jacobi_smem_threads(EPL), 1)
+jacobi_smem_kernel(const double* __restrict__ A, int64_t N, int32_t M, int32_t h_loc, SliceTable tab,
                    double* __restrict__ nrm_g, double* __restrict__ V, double* __restrict__ eps,
                    int* __restrict__ rotcnt, unsigned long long* info, int32_t s_off, int32_t compact) {
     const int CS = (int)cluster_nctarank(), cr = (int)cluster_ctarank();
     const int s = s_off + blockIdx.x / CS;  // s_off: first slice of this launch
-    const int lo = tab.lo[s], off = tab.off[s], g0 = tab.g0[s];
+    const int lo = tab.lo[s], off = tab.off[s], g0 = tab.g0[s], m = tab.cnt[s];
     // the slice's submatrix B_s: a principal block of A (leading dimension N), or -- compact != 0 -- block s of a
     // packed P x M x M copy of the diagonal blocks (pfsm_solve_host uploads those first)
     const double* Ab = compact ? A + (size_t)s * M * M : A + (size_t)lo * N + lo;
     const int64_t ldb = compact ? (int64_t)M : N;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    constexpr int NW = JACOBI_THREADS / 32;
+    constexpr int NT = jacobi_smem_threads(EPL), NW = NT / 32;
     const int h = h_loc * CS, Mp = 2 * h;
     constexpr int Ms = 32 * EPL, E2 = EPL / 2;  // padded column length (rows M..Ms-1 are zero and stay zero)
     int* rot = rotcnt + (size_t)s * JACOBI_MAX_SWEEPS;
@@ -115,7 +121,7 @@ jacobi_smem_kernel(const double* __restrict__ A, int64_t N, int32_t M, int32_t m
 
     // ---- Gershgorin shift (every CTA computes the same sigma) ----
     double bound = 0.0;
-    for (int r = tid; r < M; r += JACOBI_THREADS) {
+    for (int r = tid; r < M; r += NT) {
         double sum = 0.0;
         for (int c = 0; c < M; ++c) sum += fabs(Ab[(size_t)c * ldb + r]);
         bound = fmax(bound, sum);
@@ -337,9 +343,9 @@ jacobi_smem_kernel(const double* __restrict__ A, int64_t N, int32_t M, int32_t m
     }
     __threadfence();
     if (CS > 1) cluster_sync_all(); else __syncthreads();
-    for (int c = tid; c < M; c += JACOBI_THREADS) nrm[c] = __ldcg(nrm_s + c);
+    for (int c = tid; c < M; c += NT) nrm[c] = __ldcg(nrm_s + c);
     __syncthreads();
-    for (int c = tid; c < M; c += JACOBI_THREADS) {
+    for (int c = tid; c < M; c += NT) {
         const double v = nrm[c];
         int rk = 0;
         for (int j = 0; j < M; ++j) {

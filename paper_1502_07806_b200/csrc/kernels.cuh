@@ -21,6 +21,7 @@ struct SliceTable {  // step 1: device-resident, built once in pfs
     const int32_t* g0;   // first global eigen-index of slice s
     const int32_t* lo;   // first row/column of its submatrix
     const int32_t* off;  // local index of the slice's first eigenpair = g0 - lo
+    const int32_t* cnt;  // eigenpairs in slice s (N/P, or floor/ceil of it when P does not divide N; reading R14)
 };
 
 constexpr int JACOBI_THREADS = 1024;
@@ -67,17 +68,20 @@ __device__ __forceinline__ void cluster_sync_all() {
 // pairs of a tournament round are dealt round-robin to the CS x 32 warps, G stays in L2 (loads bypass L1 with
 // ld.global.cg because another SM may have written the column), and the round barrier is the cluster barrier.
 // The kernel is bound by L2 bandwidth (every round streams G once), so CS SMs per slice give CS x the L2 ports.
+// threads per CTA of the L2-resident kernel: 2 EPL doubles per lane must fit the register file (see jacobi_smem_threads)
+__host__ __device__ constexpr int jacobi_l2_threads(int epl) { return epl <= 8 ? JACOBI_THREADS : 512; }
+
 template <int EPL>
-__global__ void __launch_bounds__(JACOBI_THREADS, 1)
-jacobi_batched_kernel(const double* __restrict__ A, int64_t N, int32_t M, int32_t m, SliceTable tab,
+__global__ void __launch_bounds__(jacobi_l2_threads(EPL), 1)
+jacobi_batched_kernel(const double* __restrict__ A, int64_t N, int32_t M, SliceTable tab,
                       double* __restrict__ Gws, double* __restrict__ V, double* __restrict__ eps,
                       int* __restrict__ rotcnt, unsigned long long* info, int32_t s_off) {
     const int CS = (int)cluster_nctarank(), cr = (int)cluster_ctarank();
     const int s = s_off + blockIdx.x / CS;  // s_off: first slice of this launch (a rank of the sharded solve owns a range)
-    const int lo = tab.lo[s], off = tab.off[s], g0 = tab.g0[s];
+    const int lo = tab.lo[s], off = tab.off[s], g0 = tab.g0[s], m = tab.cnt[s];
     double* G = Gws + (size_t)s * M * M;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    constexpr int NW = JACOBI_THREADS / 32;
+    constexpr int NT = jacobi_l2_threads(EPL), NW = NT / 32;
     const int gw = cr * NW + warp, TW = CS * NW;  // warp index / warp count within the cluster
     int* rot = rotcnt + (size_t)s * JACOBI_MAX_SWEEPS;
 
@@ -90,7 +94,7 @@ jacobi_batched_kernel(const double* __restrict__ A, int64_t N, int32_t M, int32_
     // Gershgorin bound: max_r sum_c |B[r][c]|  (thread per row; consecutive rows are contiguous).
     // Every CTA of the cluster computes it (same order -> same sigma).
     double bound = 0.0;
-    for (int r = tid; r < M; r += JACOBI_THREADS) {
+    for (int r = tid; r < M; r += NT) {
         double sum = 0.0;
         for (int c = 0; c < M; ++c) sum += fabs(A[(size_t)(lo + c) * N + lo + r]);
         bound = fmax(bound, sum);
@@ -106,7 +110,7 @@ jacobi_batched_kernel(const double* __restrict__ A, int64_t N, int32_t M, int32_
     }
     __syncthreads();
     const double sigma = s_sigma;
-    for (int idx = cr * JACOBI_THREADS + tid; idx < M * M; idx += CS * JACOBI_THREADS) {
+    for (int idx = cr * NT + tid; idx < M * M; idx += CS * NT) {
         const int c = idx / M, r = idx - c * M;
         double v = A[(size_t)(lo + c) * N + lo + r];
         if (r == c) v += sigma;
@@ -192,7 +196,7 @@ jacobi_batched_kernel(const double* __restrict__ A, int64_t N, int32_t M, int32_
         if (lane == 0) nrm[c] = sqrt(ss);
     }
     __syncthreads();
-    for (int c = tid; c < M; c += JACOBI_THREADS) {
+    for (int c = tid; c < M; c += NT) {
         const double v = nrm[c];
         int rk = 0;
         for (int j = 0; j < M; ++j) {

@@ -79,7 +79,8 @@ struct pfsm_ctx {
     double* nrm_g = nullptr;  // P x (M + 16): final column norms of the shared-memory Jacobi
     int jac_cs = 0, jac_hloc = 0;  // cluster size / seats per CTA of the shared-memory Jacobi (0 = L2 kernel)
     double* gdiag = nullptr;  // N: diag(V^T V) before the factorization (breakdown threshold)
-    int32_t* slice_tab = nullptr;  // g0[P], lo[P], off[P]
+    int32_t* slice_tab = nullptr;  // g0[P], lo[P], off[P], cnt[P]
+    std::vector<int32_t> tab_host;  // the same table on the host
     int2* krange = nullptr;        // per 128-row tile k-range of the first product
     unsigned long long* info = nullptr;
     double* Ap = nullptr;       // generalized variant: A' = L^-1 A L^-T
@@ -172,11 +173,11 @@ int pfsm_create(pfsm_handle_t* out, int64_t N, int32_t P, int32_t window, int32_
     if (!out) return -1;
     *out = nullptr;
     if (N < 2 || (N & 1) || N > (1 << 30)) return -2;
-    if (P < 1 || N % P != 0) return -3;
+    if (P < 1 || P > N) return -3;
     if (window < 0) return -4;
     if (iters < 0) return -5;
     if (!std::isfinite(alpha) || !(alpha > 0.0)) return -6;
-    const int64_t m = N / P;
+    const int64_t m = (N + P - 1) / P;  // largest slice; all slices have N / P eigenpairs when P divides N (R14)
     const int64_t M = std::min<int64_t>(N, m + 2 * (int64_t)window);
     if (M > 512) return -4;
 
@@ -202,27 +203,34 @@ int pfsm_create(pfsm_handle_t* out, int64_t N, int32_t P, int32_t window, int32_
     TRY(dev_alloc(h, (void**)&h->rotcnt, (size_t)P * JACOBI_MAX_SWEEPS * sizeof(int)));
     TRY(dev_alloc(h, (void**)&h->nrm_g, (size_t)P * (M + 16) * sizeof(double)));
     choose_jacobi_layout(h);
-    TRY(dev_alloc(h, (void**)&h->slice_tab, 3 * (size_t)P * sizeof(int32_t)));
+    TRY(dev_alloc(h, (void**)&h->slice_tab, 4 * (size_t)P * sizeof(int32_t)));
     const int32_t ntr = (int32_t)((N + BM - 1) / BM);
     TRY(dev_alloc(h, (void**)&h->krange, (size_t)ntr * sizeof(int2)));
     TRY(dev_alloc(h, (void**)&h->info, sizeof(unsigned long long)));
     TRY(dev_alloc(h, (void**)&h->chain_cnt, (size_t)2 * (iters > 0 ? iters : 1) * ntr * sizeof(int32_t)));
 
     // step 1: slice table, and the k-range each 128-row tile of the first product needs
-    std::vector<int32_t> tab(3 * (size_t)P);
+    std::vector<int32_t>& tab = h->tab_host;
+    tab.resize(4 * (size_t)P);
     for (int32_t s = 0; s < P; ++s) {
-        const int64_t g0 = (int64_t)s * m;
+        const int64_t g0 = ((int64_t)s * N) / P, g1 = ((int64_t)(s + 1) * N) / P;
         const int64_t lo = std::min<int64_t>(std::max<int64_t>(g0 - window, 0), N - M);
         tab[s] = (int32_t)g0;
         tab[P + s] = (int32_t)lo;
         tab[2 * (size_t)P + s] = (int32_t)(g0 - lo);
+        tab[3 * (size_t)P + s] = (int32_t)(g1 - g0);
     }
     std::vector<int2> kr(ntr);
-    for (int32_t t = 0; t < ntr; ++t) {
-        const int64_t i0 = (int64_t)t * BM, i1 = std::min<int64_t>(N, i0 + BM) - 1;
-        const int64_t lo0 = tab[P + i0 / m], hi1 = tab[P + i1 / m] + M;
-        kr[t].x = (int)(lo0 / BK * BK);
-        kr[t].y = (int)((hi1 + BK - 1) / BK * BK);
+    {
+        int32_t s0 = 0, s1 = 0;  // slices of the first and last row of the tile (lo is non-decreasing in s)
+        for (int32_t t = 0; t < ntr; ++t) {
+            const int64_t i0 = (int64_t)t * BM, i1 = std::min<int64_t>(N, i0 + BM) - 1;
+            while (s0 + 1 < P && tab[s0 + 1] <= i0) ++s0;
+            while (s1 + 1 < P && tab[s1 + 1] <= i1) ++s1;
+            const int64_t lo0 = tab[P + s0], hi1 = tab[P + s1] + M;
+            kr[t].x = (int)(lo0 / BK * BK);
+            kr[t].y = (int)((hi1 + BK - 1) / BK * BK);
+        }
     }
     {
         cudaError_t e = cudaMemcpy(h->slice_tab, tab.data(), tab.size() * sizeof(int32_t), cudaMemcpyHostToDevice);
@@ -277,19 +285,20 @@ static int jacobi_cluster_size(const pfsm_ctx* h) {
     // CTAs per slice: as many as fit the chip (148 SMs / P slices) but no more warps than column pairs
     const int npairs = (h->M + 1) / 2;
     int cs = 1;
-    while (cs < 8 && (2 * cs) * h->P <= 148 && cs * (JACOBI_THREADS / 32) < npairs) cs *= 2;
+    const int nw = jacobi_l2_threads(h->M > 256 ? 16 : (h->M > 128 ? 8 : 4)) / 32;  // warps per CTA
+    while (cs < 8 && (2 * cs) * h->P <= 148 && cs * nw < npairs) cs *= 2;
     return cs;
 }
 
 extern "C++" {
 template <int EPL>
 static int launch_jacobi_t(pfsm_ctx* h, const double* A, double* V, cudaStream_t st, int32_t s0, int32_t ns) {
-    SliceTable tab{h->slice_tab, h->slice_tab + h->P, h->slice_tab + 2 * (size_t)h->P};
+    SliceTable tab{h->slice_tab, h->slice_tab + h->P, h->slice_tab + 2 * (size_t)h->P, h->slice_tab + 3 * (size_t)h->P};
     const int cs = jacobi_cluster_size(h);
     cudaLaunchConfig_t cfg;
     memset(&cfg, 0, sizeof(cfg));
     cfg.gridDim = dim3((unsigned)(ns * cs));
-    cfg.blockDim = dim3(JACOBI_THREADS);
+    cfg.blockDim = dim3(jacobi_l2_threads(EPL));
     cfg.dynamicSmemBytes = (size_t)h->M * (sizeof(double) + sizeof(int));
     cfg.stream = st;
     cudaLaunchAttribute attr[1];
@@ -299,7 +308,7 @@ static int launch_jacobi_t(pfsm_ctx* h, const double* A, double* V, cudaStream_t
     attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
-    PFSM_CUDA(cudaLaunchKernelEx(&cfg, jacobi_batched_kernel<EPL>, A, h->N, h->M, h->m, tab, h->Gws, V, h->eps,
+    PFSM_CUDA(cudaLaunchKernelEx(&cfg, jacobi_batched_kernel<EPL>, A, h->N, h->M, tab, h->Gws, V, h->eps,
                                  h->rotcnt, h->info, s0));
     return 0;
 }
@@ -309,14 +318,14 @@ extern "C++" {
 template <int EPL>
 static int launch_jacobi_smem_t(pfsm_ctx* h, const double* A, double* V, cudaStream_t st, int32_t s0, int32_t ns,
                                 int32_t compact) {
-    SliceTable tab{h->slice_tab, h->slice_tab + h->P, h->slice_tab + 2 * (size_t)h->P};
+    SliceTable tab{h->slice_tab, h->slice_tab + h->P, h->slice_tab + 2 * (size_t)h->P, h->slice_tab + 3 * (size_t)h->P};
     const size_t smem = jacobi_smem_bytes(h->M, h->jac_hloc);
     // static smem (~300 B) + dynamic must stay within the 227 KB opt-in limit; set per launch (handles differ)
     PFSM_CUDA(cudaFuncSetAttribute(jacobi_smem_kernel<EPL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     cudaLaunchConfig_t cfg;
     memset(&cfg, 0, sizeof(cfg));
     cfg.gridDim = dim3((unsigned)(ns * h->jac_cs));
-    cfg.blockDim = dim3(JACOBI_THREADS);
+    cfg.blockDim = dim3(jacobi_smem_threads(EPL));
     cfg.dynamicSmemBytes = smem;
     cfg.stream = st;
     cudaLaunchAttribute attr[1];
@@ -326,7 +335,7 @@ static int launch_jacobi_smem_t(pfsm_ctx* h, const double* A, double* V, cudaStr
     attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
-    PFSM_CUDA(cudaLaunchKernelEx(&cfg, jacobi_smem_kernel<EPL>, A, h->N, h->M, h->m, (int32_t)h->jac_hloc, tab,
+    PFSM_CUDA(cudaLaunchKernelEx(&cfg, jacobi_smem_kernel<EPL>, A, h->N, h->M, (int32_t)h->jac_hloc, tab,
                                  h->nrm_g, V, h->eps, h->rotcnt, h->info, s0, compact));
     return 0;
 }
@@ -343,7 +352,7 @@ static int jacobi_max_clusters_t(int cs, size_t smem) {
     cudaLaunchConfig_t cfg;
     memset(&cfg, 0, sizeof(cfg));
     cfg.gridDim = dim3((unsigned)cs);
-    cfg.blockDim = dim3(JACOBI_THREADS);
+    cfg.blockDim = dim3(jacobi_smem_threads(EPL));
     cfg.dynamicSmemBytes = smem;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeClusterDimension;
@@ -388,7 +397,8 @@ static void choose_jacobi_layout(pfsm_ctx* h) {
     // two boundary seats of a CTA synchronise with each other inside a round (jacobi_smem.cuh)
     auto hloc_of = [&](int cs) {
         int hl = (h->M + 2 * cs - 1) / (2 * cs);
-        if (hl > 1 && (hl - 1) % (JACOBI_THREADS / 32) == 0) ++hl;
+        const int nw = jacobi_smem_threads(jacobi_padded_rows(h->M) / 32) / 32;  // warps per CTA
+        if (hl > 1 && (hl - 1) % nw == 0) ++hl;
         return hl;
     };
     auto fits = [&](int cs) { return hloc_of(cs) >= 2 && jacobi_smem_bytes(h->M, hloc_of(cs)) <= budget; };
@@ -883,7 +893,7 @@ int pfsm_standard_form_eq14(pfsm_handle_t h, const double* A, const double* B, d
 //   phase 4: V = (V^T R^-1)^T, step 5 on the own rows              -> all-gather lambda
 int pfsm_set_shard(pfsm_handle_t h, int32_t rank, int32_t world) {
     if (!h) return -1;
-    if (world < 1 || h->P % world != 0 || (h->N / world) % BM != 0) return -3;
+    if (world < 1 || h->N % h->P != 0 || h->P % world != 0 || (h->N / world) % BM != 0) return -3;
     if (rank < 0 || rank >= world) return -2;
     h->sh_rank = rank;
     h->sh_world = world;
@@ -975,8 +985,7 @@ int pfsm_solve_host(pfsm_handle_t h, const double* A_host, double* V_host, doubl
         // shared-memory kernel leaves free) and let the full matrix follow on the side stream under the Jacobi kernel.
         const size_t M = (size_t)h->M;
         for (int32_t sl = 0; sl < h->P; ++sl) {
-            const int64_t g0 = (int64_t)sl * h->m;
-            const int64_t lo = std::min<int64_t>(std::max<int64_t>(g0 - h->window, 0), h->N - (int64_t)M);
+            const int64_t lo = h->tab_host[(size_t)h->P + sl];
             PFSM_CUDA(cudaMemcpy2DAsync(h->Gws + (size_t)sl * M * M, M * sizeof(double), A_host + (size_t)lo * h->N + lo,
                                         (size_t)h->N * sizeof(double), M * sizeof(double), M, cudaMemcpyHostToDevice, st));
         }

@@ -68,6 +68,10 @@ SMALL_CASES = [
     (96, 4, 100, 2, 1e-2, 8.0),      # window >= N: every slice diagonalizes all of A
     (64, 8, 0, 4, 1e-3, 4.0),        # window 0: M = m
     (2, 1, 0, 1, 1e-1, 1.0),         # smallest legal problem
+    (250, 4, 10, 2, 1e-3, 12.0),     # P does not divide N (R14): slices of 62, 63, 62, 63
+    (500, 7, 20, 3, 1e-3, 16.0),     # slices of 71 / 72, M = 112, tiles straddle uneven slice boundaries
+    (64, 64, 3, 1, 1e-3, 4.0),       # one eigenpair per slice
+    (66, 64, 2, 2, 1e-3, 4.0),       # slices of 1 and 2
 ]
 
 
@@ -82,8 +86,9 @@ def test_stepwise_parity_small(N, P, w, iters, amp, width):
     assert np.abs(g2["eps"] - eps).max() <= 1e-13 * max(1.0, nF)
     assert np.array_equal(g2["Vr"] == 0.0, V2 == 0.0) or np.abs(align_signs(g2["Vr"], V2) - V2).max() < 1e-9
     M, g0, lo, off = oracle.partition(N, P, w)
+    cnt = oracle.slice_counts(N, P)
     for s in range(P):   # exactly zero outside the slice's window
-        rows = g2["Vr"][g0[s]:g0[s] + N // P]
+        rows = g2["Vr"][g0[s]:g0[s] + cnt[s]]
         mask = np.ones(N, bool)
         mask[lo[s]:lo[s] + M] = False
         assert np.all(rows[:, mask] == 0.0)
@@ -551,7 +556,9 @@ def _fuzz_cases(count=24):
         N = 2 * int(2 + u[4 * k] * 330)                      # even, 4 .. 662
         divs = [d for d in range(1, N + 1) if N % d == 0 and N // d >= 1]
         P = divs[int(u[4 * k + 1] * len(divs)) % len(divs)]
-        m = N // P
+        if k % 3 == 2:
+            P = 1 + int(u[4 * k + 1] * min(N, 40))           # any P: slices of unequal size (R14)
+        m = -(-N // P)
         w = int(u[4 * k + 2] * 40)
         if min(N, m + 2 * w) > 512:                          # library limit on the submatrix order
             w = max(0, (512 - m) // 2)
