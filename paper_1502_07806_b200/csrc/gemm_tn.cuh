@@ -54,7 +54,7 @@ struct GemmParams {
     int32_t xr0, yr0, xk0, yk0, klen;
     // optional per-row-tile k-range {begin, end} (multiples of BK), overrides [0, klen)
     const int2* krange;
-    // lower != 0: only tiles (tr, tc) with tr >= tc are computed
+    // lower != 0: only tiles (tr, tc) with tr >= tc are computed (1: column by column; 2: row by row, ntr == ntc)
     int32_t lower;
     int32_t ntr, ntc;
     // epilogue operands, same coordinates as C
@@ -129,6 +129,17 @@ __device__ __forceinline__ bool tile_coords(const GemmParams& p, int32_t idx, in
         tc = rem / gsz;
         return tr < p.ntr && tc < p.ntc;
     }
+    if (p.lower == 2) {
+        // square region, row by row: row tr holds columns 0..tr, prefix(tr) = tr (tr + 1) / 2.  Early tiles only touch
+        // early row blocks, which is what a chained launch (wait_cnt) needs.
+        int32_t r = (int32_t)((sqrt(8.0 * (double)idx + 1.0) - 1.0) * 0.5);
+        r = max(0, min(r, p.ntr - 1));
+        while (r > 0 && (int64_t)r * (r + 1) / 2 > idx) --r;
+        while ((int64_t)(r + 1) * (r + 2) / 2 <= idx) ++r;
+        tr = r;
+        tc = (int32_t)(idx - (int64_t)r * (r + 1) / 2);
+        return tr < p.ntr;
+    }
     // column tc holds rows tc..ntr-1: count ntr - tc; prefix(tc) = tc*ntr - tc(tc-1)/2
     const double n = (double)p.ntr + 0.5;
     int32_t c = (int32_t)(n - sqrt(n * n - 2.0 * (double)idx));
@@ -143,6 +154,7 @@ __device__ __forceinline__ bool tile_coords(const GemmParams& p, int32_t idx, in
 
 inline int64_t gemm_num_tiles(int32_t ntr, int32_t ntc, int lower) {
     if (!lower) return (int64_t)ntr * ntc;
+    if (lower == 2) return (int64_t)ntr * (ntr + 1) / 2;
     int64_t t = 0;
     for (int c = 0; c < ntc; ++c) t += (ntr - c > 0 ? ntr - c : 0);
     return t;
@@ -181,12 +193,15 @@ gemm_tn_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__
         if (p.wait_cnt) {
             // The producer grid is resident or finished (it triggered the dependent launch from every CTA), so this
             // spin cannot starve it.  acquire + bar.sync order every thread's later loads, the proxy fence the TMA reads.
-            const int32_t* c = p.wait_cnt + tr;
-            int32_t seen;
-            for (;;) {
-                asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(seen) : "l"(c) : "memory");
-                if (seen >= p.wait_target) break;
-                __nanosleep(256);
+            // a lower-triangular product X X^T also reads row block tc of the previous output (tc <= tr)
+            for (int32_t rb = p.lower ? tc : tr; rb <= tr; rb += max(1, tr - tc)) {
+                const int32_t* c = p.wait_cnt + rb;
+                int32_t seen;
+                for (;;) {
+                    asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(seen) : "l"(c) : "memory");
+                    if (seen >= p.wait_target) break;
+                    __nanosleep(256);
+                }
             }
             asm volatile("fence.proxy.async.global;" ::: "memory");
         }

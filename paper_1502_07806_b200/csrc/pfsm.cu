@@ -545,16 +545,25 @@ static int stacked_cholesky(pfsm_ctx* h, bool factor, cudaStream_t st, int32_t b
 }
 
 // ---- step 4: Cholesky-QR.  G = V^T V (row-major view: V V^T), S = [G ; V^T] ----
-static int run_step4_once(pfsm_ctx* h, const CUtensorMap& mapV, double* V, cudaStream_t st) {
+// wait_cnt != nullptr: V is the output of a step-3 GEMM that may still be in its last wave; the Gram product is chained
+// to it (row-block counters, see the step-3 loop) and starts on the SMs that wave leaves idle.
+static int run_step4_once(pfsm_ctx* h, const CUtensorMap& mapV, double* V, cudaStream_t st,
+                          const int32_t* wait_cnt = nullptr, int32_t wait_target = 0) {
     const int64_t N = h->N;
     const int32_t n = (int32_t)N;
     int rc;
     const dim3 tb(32, 8), tg((unsigned)((N + 31) / 32), (unsigned)((N + 31) / 32));
+    GemmParams p = base_params();
+    p.C = h->S; p.ldc = N; p.mr = n; p.nc = n; p.klen = n; p.lower = 2;
+    p.wait_cnt = wait_cnt; p.wait_target = wait_target;
+    if (wait_cnt) {
+        if ((rc = launch_gemm<EPI_PLAIN>(mapV, mapV, h->mapS, p, st, true))) return rc;
+    }
     transpose_kernel<<<tg, tb, 0, st>>>(V, N, h->S + (size_t)N * N, N, n, n);
     PFSM_CUDA(cudaGetLastError());
-    GemmParams p = base_params();
-    p.C = h->S; p.ldc = N; p.mr = n; p.nc = n; p.klen = n; p.lower = 1;
-    if ((rc = launch_gemm<EPI_PLAIN>(mapV, mapV, h->mapS, p, st))) return rc;
+    if (!wait_cnt) {
+        if ((rc = launch_gemm<EPI_PLAIN>(mapV, mapV, h->mapS, p, st))) return rc;
+    }
     extract_diag_kernel<<<(unsigned)((N + 255) / 256), 256, 0, st>>>(h->S, N, n, h->gdiag);
     PFSM_CUDA(cudaGetLastError());
     if ((rc = stacked_cholesky(h, true, st))) return rc;
@@ -565,9 +574,10 @@ static int run_step4_once(pfsm_ctx* h, const CUtensorMap& mapV, double* V, cudaS
 
 // One pass leaves ||V^T V - I|| ~ eps cond(V)^2; a second pass on the result (CholeskyQR2) brings it to ~eps and does
 // not change the exact-arithmetic result (V R1^-1 R2^-1 with R2 -> I), so it stays the Gram-Schmidt basis.
-static int run_step4(pfsm_ctx* h, const CUtensorMap& mapV, double* V, cudaStream_t st) {
+static int run_step4(pfsm_ctx* h, const CUtensorMap& mapV, double* V, cudaStream_t st,
+                     const int32_t* wait_cnt = nullptr, int32_t wait_target = 0) {
     for (int32_t pass = 0; pass < h->cholqr_passes; ++pass) {
-        int rc = run_step4_once(h, mapV, V, st);
+        int rc = pass == 0 ? run_step4_once(h, mapV, V, st, wait_cnt, wait_target) : run_step4_once(h, mapV, V, st);
         if (rc) return rc;
     }
     return 0;
@@ -658,7 +668,10 @@ static int solve_impl(pfsm_handle_t h, const double* A, double* V, double* lambd
     if (tm) PFSM_CUDA(cudaEventRecord(h->ev[2], st));
     if (last_step == 3) return 0;
 
-    if ((rc = run_step4(h, mapV, V, st))) return rc;
+    // The Gram product of step 4 is one more link of the chain: it reads row blocks of the last update.  Not with step
+    // timing on: the event between the two kernels would sit inside the overlap and blur both step times.
+    const int32_t* last_cnt = (chain && !tm) ? h->chain_cnt + (size_t)(2 * h->iters - 1) * nrb : nullptr;
+    if ((rc = run_step4(h, mapV, V, st, last_cnt, ncb))) return rc;
     if (tm) PFSM_CUDA(cudaEventRecord(h->ev[3], st));
     if (last_step == 4) return 0;
 
