@@ -277,6 +277,21 @@ def test_solve_on_a_side_stream():
     h.destroy()
 
 
+@pytest.mark.parametrize("N,P,w,iters", [(2048, 16, 32, 3), (600, 3, 20, 2), (1000, 7, 30, 4)])
+def test_chained_launches_change_no_bit(N, P, w, iters, monkeypatch):
+    """The step-3 GEMMs (and step 4's Gram product) overlap their last waves through programmatic dependent launch and
+    per-row-block counters.  That is scheduling only: the result must equal the plain stream-ordered
+    launches bit for bit, solve after solve (a tile that started before its operand rows were complete would differ)."""
+    p = gen.small_problem(N, 1e-3, 24.0, seed=52000 + N)
+    chained = [gpu_solve(p.A, P, w, iters, p.alpha) for _ in range(3)]
+    monkeypatch.setenv("PFSM_NO_CHAIN", "1")
+    plain = gpu_solve(p.A, P, w, iters, p.alpha)
+    for g in chained:
+        assert g["info"] == 0
+        assert np.array_equal(g["Vr"], plain["Vr"]) and np.array_equal(g["lam"], plain["lam"])
+        assert np.array_equal(g["resid"], plain["resid"])
+
+
 @pytest.mark.parametrize("k", [0, 1, 2, 5])
 def test_baseline_configs_full_oracle(k):
     """BASELINE.json configs 0-2 at full size, and the Cu256-shaped extra case (N = 1664, window at the paper's
