@@ -181,6 +181,20 @@ int pfsm_destroy(pfsm_handle_t h);
  */
 int pfsm_get_info(pfsm_handle_t h, void* stream, int64_t* info);
 
+/*
+ * The paper's validity guard in one call (PFSM needs a diagonally dominant matrix, "standard
+ * diagonalization" is used while that does not hold): after a full solve (pfsm_solve, _host, _warm, _generalized)
+ * reduces the residual norms on the device and synchronizes `stream`.
+ *   resid_tol            largest acceptable r_i = ||A v_i - lambda_i v_i||_2 (absolute; scale it with ||A||); >= 0
+ *   *use_standard_solver host, out: 1 if pfsm_get_info would be non-zero or max_i r_i > resid_tol (NaN counts as
+ *                        too large) -- the caller should diagonalize this step with a standard solver -- else 0
+ *   *max_resid_out       host, out, optional (may be NULL): max_i r_i
+ *   *info_out            host, out, optional: the same value pfsm_get_info returns
+ * Errors: -1 handle, -3 resid_tol negative or NaN, -4 NULL verdict pointer, 1000+cudaError.
+ */
+int pfsm_check_validity(pfsm_handle_t h, void* stream, double resid_tol, int32_t* use_standard_solver,
+                        double* max_resid_out, int64_t* info_out);
+
 /* Largest number of Jacobi sweeps any slice's submatrix eigensolve (step 2) used in the last solve;
  * synchronizes `stream`.  The last sweep is the one that found nothing left to rotate. */
 int pfsm_get_step2_sweeps(pfsm_handle_t h, void* stream, int32_t* max_sweeps);

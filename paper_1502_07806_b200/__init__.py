@@ -20,7 +20,7 @@ CUDA_ERROR_BASE = 1000
 EXPORTS = [
     "pfsm_create", "pfsm_solve", "pfsm_solve_host", "pfsm_solve_partial", "pfsm_orthonormalize", "pfsm_rayleigh", "pfsm_solve_generalized",
     "pfsm_generalized_reduce", "pfsm_solve_warm", "pfsm_standard_form_eq14",
-    "pfsm_set_shard", "pfsm_shard_phase", "pfsm_shard_buffer", "pfsm_destroy", "pfsm_get_info",
+    "pfsm_set_shard", "pfsm_shard_phase", "pfsm_shard_buffer", "pfsm_destroy", "pfsm_get_info", "pfsm_check_validity",
     "pfsm_get_step2_sweeps", "pfsm_get_residuals", "pfsm_get_shifts", "pfsm_set_alpha", "pfsm_set_cholqr_passes", "pfsm_workspace_bytes",
     "pfsm_launches_per_solve", "pfsm_enable_step_timing", "pfsm_get_step_ms", "pfsm_probe_fp64_peak",
     "pfsm_strerror",
@@ -64,6 +64,7 @@ def load(build_if_missing: bool = True):
     lib.pfsm_destroy.argtypes = [p]
     lib.pfsm_get_info.argtypes = [p, p, ctypes.POINTER(i64)]
     lib.pfsm_get_step2_sweeps.argtypes = [p, p, ctypes.POINTER(i32)]
+    lib.pfsm_check_validity.argtypes = [p, p, dbl, ctypes.POINTER(i32), ctypes.POINTER(dbl), ctypes.POINTER(i64)]
     lib.pfsm_get_residuals.argtypes = [p, ctypes.POINTER(p)]
     lib.pfsm_get_shifts.argtypes = [p, ctypes.POINTER(p)]
     lib.pfsm_set_alpha.argtypes = [p, dbl]
@@ -217,6 +218,13 @@ class Handle:
         v = ctypes.c_int64(-1)
         _check(self._lib.pfsm_get_info(self._h, _stream_ptr(stream), ctypes.byref(v)), "pfsm_get_info")
         return int(v.value)
+
+    def check_validity(self, resid_tol: float, stream=None):
+        """PAPER.md:98-100 guard.  Returns (use_standard_solver: bool, max_resid: float, info: int)."""
+        verdict, mx, info = ctypes.c_int32(-1), ctypes.c_double(0.0), ctypes.c_int64(-1)
+        _check(self._lib.pfsm_check_validity(self._h, _stream_ptr(stream), resid_tol, ctypes.byref(verdict),
+                                             ctypes.byref(mx), ctypes.byref(info)), "pfsm_check_validity")
+        return bool(verdict.value), float(mx.value), int(info.value)
 
     def _view(self, getter, name):
         import torch

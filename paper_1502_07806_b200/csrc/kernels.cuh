@@ -555,6 +555,25 @@ rayleigh_kernel(const double* __restrict__ V, const double* __restrict__ T, int6
     }
 }
 
+// max_i r[i] (NaN counts as +inf) -> out[0]; one CTA, fixed order.  The validity guard of PAPER.md:98-100.
+__global__ void __launch_bounds__(1024) max_residual_kernel(const double* __restrict__ r, int64_t N, double* __restrict__ out) {
+    __shared__ double red[32];
+    double m = 0.0;
+    for (int64_t i = threadIdx.x; i < N; i += 1024) {
+        const double v = r[i];
+        m = fmax(m, (v == v) ? v : __longlong_as_double(0x7ff0000000000000LL));
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, o));
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = m;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double t = 0.0;
+        for (int w = 0; w < 32; ++w) t = fmax(t, red[w]);
+        out[0] = t;
+    }
+}
+
 // ---------------------------------------------------------------------------------------------
 // Roofline calibration: register-only FP64 issue-rate loops (no memory traffic).
 // ---------------------------------------------------------------------------------------------

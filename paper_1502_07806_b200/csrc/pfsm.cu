@@ -1033,6 +1033,27 @@ int pfsm_get_info(pfsm_handle_t h, void* stream, int64_t* info) {
     return 0;
 }
 
+int pfsm_check_validity(pfsm_handle_t h, void* stream, double resid_tol, int32_t* use_standard_solver,
+                        double* max_resid_out, int64_t* info_out) {
+    if (!h) return -1;
+    if (!(resid_tol >= 0.0)) return -3;
+    if (!use_standard_solver) return -4;
+    cudaStream_t st = (cudaStream_t)stream;
+    // gdiag (step 4's scratch) is free after a solve: slot 0 receives the maximum
+    max_residual_kernel<<<1, 1024, 0, st>>>(h->resid, h->N, h->gdiag);
+    PFSM_CUDA(cudaGetLastError());
+    double mx = 0.0;
+    unsigned long long v = 0;
+    PFSM_CUDA(cudaMemcpyAsync(&mx, h->gdiag, sizeof(double), cudaMemcpyDeviceToHost, st));
+    PFSM_CUDA(cudaMemcpyAsync(&v, h->info, sizeof(v), cudaMemcpyDeviceToHost, st));
+    PFSM_CUDA(cudaStreamSynchronize(st));
+    const int64_t info = (v == ~0ULL) ? 0 : (int64_t)v;
+    *use_standard_solver = (info != 0 || !(mx <= resid_tol)) ? 1 : 0;
+    if (max_resid_out) *max_resid_out = mx;
+    if (info_out) *info_out = info;
+    return 0;
+}
+
 int pfsm_get_step2_sweeps(pfsm_handle_t h, void* stream, int32_t* max_sweeps) {
     if (!h) return -1;
     if (!max_sweeps) return -3;

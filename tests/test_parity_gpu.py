@@ -277,6 +277,34 @@ def test_solve_on_a_side_stream():
     h.destroy()
 
 
+def test_validity_guard_follows_the_paper_failure_mode():
+    """PFSM is valid for diagonally dominant matrices; otherwise standard diagonalization is used.
+    The guard must pass a dominant matrix, and flag A = Q D Q^T with a dense random Q (no dominance: the submatrix
+    eigenvectors say nothing about A's), where the oracle shows the same large residuals."""
+    N, P, w, iters = 256, 4, 16, 3
+    p = gen.small_problem(N, 1e-3, 16.0, seed=77)
+    nF = p.normF
+    h = pfsm.Handle(N, P, w, iters, p.alpha)
+    dV = torch.empty((N, N), dtype=torch.float64, device="cuda")
+    dl = torch.empty((N,), dtype=torch.float64, device="cuda")
+    h.solve(dev(p.A), dV, dl)
+    use_std, mx, info = h.check_validity(1e-2 * nF)
+    r = h.residuals().cpu().numpy()
+    assert not use_std and info == 0 and mx == r.max()
+    assert h.check_validity(0.5 * r.max())[0]                      # same solve, tighter tolerance: flagged
+    Q = gen.householder_orthogonal(N, N // 2, seed=5)
+    A2 = Q @ np.diag(p.d) @ Q.T
+    A2 = 0.5 * (A2 + A2.T)
+    h.solve(dev(A2), dV, dl)
+    use_std, mx2, info2 = h.check_validity(1e-2 * nF)
+    o = oracle.pfsm(A2, P, w, iters, p.alpha)
+    assert o["info"] != 0 or o["resid"].max() > 1e-2 * nF           # the oracle shows the failure too
+    assert use_std and (info2 != 0 or mx2 > 1e-2 * nF)
+    with pytest.raises(pfsm.PfsmError):
+        h.check_validity(float("nan"))
+    h.destroy()
+
+
 @pytest.mark.parametrize("N,P,w,iters", [(2048, 16, 32, 3), (600, 3, 20, 2), (1000, 7, 30, 4)])
 def test_chained_launches_change_no_bit(N, P, w, iters, monkeypatch):
     """The step-3 GEMMs (and step 4's Gram product) overlap their last waves through programmatic dependent launch and
