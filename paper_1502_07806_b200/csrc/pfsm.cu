@@ -128,7 +128,8 @@ static int launch_gemm(const CUtensorMap& mx, const CUtensorMap& my, const CUten
         PFSM_CUDA(cudaFuncSetAttribute(gemm_tn_kernel<EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, GEMM_SMEM));
         attr_set[EPI] = true;
     }
-    if (pdl) {
+    static bool pdl_ok = true;  // cleared if the driver refuses the attribute: plain stream order is always correct
+    if (pdl && pdl_ok) {
         cudaLaunchConfig_t cfg;
         memset(&cfg, 0, sizeof(cfg));
         cfg.gridDim = dim3((unsigned)tiles);
@@ -140,8 +141,11 @@ static int launch_gemm(const CUtensorMap& mx, const CUtensorMap& my, const CUten
         at[0].val.programmaticStreamSerializationAllowed = 1;
         cfg.attrs = at;
         cfg.numAttrs = 1;
-        PFSM_CUDA(cudaLaunchKernelEx(&cfg, gemm_tn_kernel<EPI>, mx, my, mc, p));
-        return 0;
+        const cudaError_t e = cudaLaunchKernelEx(&cfg, gemm_tn_kernel<EPI>, mx, my, mc, p);
+        if (e == cudaSuccess) return 0;
+        if (e != cudaErrorNotSupported && e != cudaErrorInvalidValue) return PFSM_CUDA_ERROR_BASE + (int)e;
+        cudaGetLastError();
+        pdl_ok = false;
     }
     gemm_tn_kernel<EPI><<<(unsigned)tiles, GEMM_THREADS, GEMM_SMEM, st>>>(mx, my, mc, p);
     PFSM_CUDA(cudaGetLastError());
