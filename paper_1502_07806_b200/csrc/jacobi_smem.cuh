@@ -72,8 +72,11 @@ inline size_t jacobi_smem_bytes(int M, int h_loc) {
 // round: M = 416 6.6 -> 3.1 us, M = 384 3.7 -> 2.9 us; at EPL = 10 the 64-byte spill of the 1024-thread build is faster).
 __host__ __device__ constexpr int jacobi_smem_threads(int epl) { return epl <= 10 ? 1024 : 512; }
 
-template <int EPL>
-__global__ void __launch_bounds__(jacobi_smem_threads(EPL), 1)
+// HALF (EPL <= 8 only): 512 threads and 64 registers, so two CTAs -- of two different slices -- share an SM and one
+// fills the other's barrier and exchange waits.  Chosen when the slices need more than one wave anyway
+// (choose_jacobi_layout; config 4: 64 clusters of 8 half CTAs 12.5 ms vs 64 clusters of 4 full CTAs 13.4 ms).
+template <int EPL, bool HALF = false>
+__global__ void __launch_bounds__(HALF ? 512 : jacobi_smem_threads(EPL), HALF ? 2 : 1)
 jacobi_smem_kernel(const double* __restrict__ A, int64_t N, int32_t M, int32_t h_loc, SliceTable tab,
                    double* __restrict__ nrm_g, double* __restrict__ V, double* __restrict__ eps,
                    int* __restrict__ rotcnt, unsigned long long* info, int32_t s_off, int32_t compact) {
@@ -85,7 +88,7 @@ jacobi_smem_kernel(const double* __restrict__ A, int64_t N, int32_t M, int32_t h
     const double* Ab = compact ? A + (size_t)s * M * M : A + (size_t)lo * N + lo;
     const int64_t ldb = compact ? (int64_t)M : N;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    constexpr int NT = jacobi_smem_threads(EPL), NW = NT / 32;
+    constexpr int NT = HALF ? 512 : jacobi_smem_threads(EPL), NW = NT / 32;
     const int h = h_loc * CS, Mp = 2 * h;
     constexpr int Ms = 32 * EPL, E2 = EPL / 2;  // padded column length (rows M..Ms-1 are zero and stay zero)
     int* rot = rotcnt + (size_t)s * JACOBI_MAX_SWEEPS;

@@ -103,6 +103,7 @@ struct pfsm_ctx {
     bool chain = true;                 // step 3: consecutive GEMMs overlap their last waves (row-block counters + PDL)
     int32_t* chain_cnt = nullptr;      // [2 * iters][ceil(N / BM)] tiles stored per row block of each step-3 GEMM
     int32_t cholqr_passes = 1;         // 2 = CholeskyQR2 (re-orthonormalize once; reading R10)
+    bool jac_half = false;             // shared-memory Jacobi with 512-thread CTAs, two per SM (jacobi_smem.cuh)
     int32_t sh_rank = 0, sh_world = 1;  // sharded solve: this handle works on rows [sh_rank, sh_rank+1) * N / sh_world
 };
 
@@ -319,17 +320,17 @@ static int launch_jacobi_t(pfsm_ctx* h, const double* A, double* V, cudaStream_t
 }  // extern "C++"
 
 extern "C++" {
-template <int EPL>
+template <int EPL, bool HALF = false>
 static int launch_jacobi_smem_t(pfsm_ctx* h, const double* A, double* V, cudaStream_t st, int32_t s0, int32_t ns,
                                 int32_t compact) {
     SliceTable tab{h->slice_tab, h->slice_tab + h->P, h->slice_tab + 2 * (size_t)h->P, h->slice_tab + 3 * (size_t)h->P};
     const size_t smem = jacobi_smem_bytes(h->M, h->jac_hloc);
     // static smem (~300 B) + dynamic must stay within the 227 KB opt-in limit; set per launch (handles differ)
-    PFSM_CUDA(cudaFuncSetAttribute(jacobi_smem_kernel<EPL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    PFSM_CUDA(cudaFuncSetAttribute(jacobi_smem_kernel<EPL, HALF>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     cudaLaunchConfig_t cfg;
     memset(&cfg, 0, sizeof(cfg));
     cfg.gridDim = dim3((unsigned)(ns * h->jac_cs));
-    cfg.blockDim = dim3(jacobi_smem_threads(EPL));
+    cfg.blockDim = dim3(HALF ? 512 : jacobi_smem_threads(EPL));
     cfg.dynamicSmemBytes = smem;
     cfg.stream = st;
     cudaLaunchAttribute attr[1];
@@ -339,7 +340,7 @@ static int launch_jacobi_smem_t(pfsm_ctx* h, const double* A, double* V, cudaStr
     attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
-    PFSM_CUDA(cudaLaunchKernelEx(&cfg, jacobi_smem_kernel<EPL>, A, h->N, h->M, (int32_t)h->jac_hloc, tab,
+    PFSM_CUDA(cudaLaunchKernelEx(&cfg, jacobi_smem_kernel<EPL, HALF>, A, h->N, h->M, (int32_t)h->jac_hloc, tab,
                                  h->nrm_g, V, h->eps, h->rotcnt, h->info, s0, compact));
     return 0;
 }
@@ -347,16 +348,16 @@ static int launch_jacobi_smem_t(pfsm_ctx* h, const double* A, double* V, cudaStr
 
 extern "C++" {
 // how many clusters of `cs` CTAs of the shared-memory Jacobi kernel the device can hold at once
-template <int EPL>
+template <int EPL, bool HALF = false>
 static int jacobi_max_clusters_t(int cs, size_t smem) {
-    if (cudaFuncSetAttribute(jacobi_smem_kernel<EPL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) {
+    if (cudaFuncSetAttribute(jacobi_smem_kernel<EPL, HALF>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) {
         cudaGetLastError();
         return 0;
     }
     cudaLaunchConfig_t cfg;
     memset(&cfg, 0, sizeof(cfg));
     cfg.gridDim = dim3((unsigned)cs);
-    cfg.blockDim = dim3(jacobi_smem_threads(EPL));
+    cfg.blockDim = dim3(HALF ? 512 : jacobi_smem_threads(EPL));
     cfg.dynamicSmemBytes = smem;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeClusterDimension;
@@ -366,7 +367,7 @@ static int jacobi_max_clusters_t(int cs, size_t smem) {
     cfg.attrs = attr;
     cfg.numAttrs = 1;
     int n = 0;
-    if (cudaOccupancyMaxActiveClusters(&n, jacobi_smem_kernel<EPL>, &cfg) != cudaSuccess) {
+    if (cudaOccupancyMaxActiveClusters(&n, jacobi_smem_kernel<EPL, HALF>, &cfg) != cudaSuccess) {
         cudaGetLastError();
         return 0;
     }
@@ -374,7 +375,16 @@ static int jacobi_max_clusters_t(int cs, size_t smem) {
 }
 }  // extern "C++"
 
-static int jacobi_max_clusters(int M, int cs, size_t smem) {
+static int jacobi_max_clusters(int M, int cs, size_t smem, bool half = false) {
+    if (half) {
+        switch (jacobi_padded_rows(M) / 32) {
+            case 2: return jacobi_max_clusters_t<2, true>(cs, smem);
+            case 4: return jacobi_max_clusters_t<4, true>(cs, smem);
+            case 6: return jacobi_max_clusters_t<6, true>(cs, smem);
+            case 8: return jacobi_max_clusters_t<8, true>(cs, smem);
+            default: return 0;
+        }
+    }
     switch (jacobi_padded_rows(M) / 32) {
         case 2: return jacobi_max_clusters_t<2>(cs, smem);
         case 4: return jacobi_max_clusters_t<4>(cs, smem);
@@ -399,33 +409,58 @@ static void choose_jacobi_layout(pfsm_ctx* h) {
     const size_t budget = 220 * 1024;
     // seats per CTA; one more (phantom) pair when seat 0 and seat h_loc-1 would fall to the same warp, because the
     // two boundary seats of a CTA synchronise with each other inside a round (jacobi_smem.cuh)
-    auto hloc_of = [&](int cs) {
+    const int epl = jacobi_padded_rows(h->M) / 32;
+    auto hloc_of = [&](int cs, bool half = false) {
         int hl = (h->M + 2 * cs - 1) / (2 * cs);
-        const int nw = jacobi_smem_threads(jacobi_padded_rows(h->M) / 32) / 32;  // warps per CTA
+        const int nw = (half ? 512 : jacobi_smem_threads(epl)) / 32;  // warps per CTA
         if (hl > 1 && (hl - 1) % nw == 0) ++hl;
         return hl;
     };
-    auto fits = [&](int cs) { return hloc_of(cs) >= 2 && jacobi_smem_bytes(h->M, hloc_of(cs)) <= budget; };
+    auto fits = [&](int cs, bool half = false) {
+        return hloc_of(cs, half) >= 2 && jacobi_smem_bytes(h->M, hloc_of(cs, half)) <= budget;
+    };
     int cs_min = 1;
     while (cs_min <= 8 && !fits(cs_min)) cs_min *= 2;
     if (cs_min > 8) return;
     int cs = cs_min;
+    bool one_wave = false;
     for (int c = cs_min; c <= 8; c *= 2) {
         if (!fits(c) || (c > cs_min && hloc_of(c) < 6)) break;
-        if (jacobi_max_clusters(h->M, c, jacobi_smem_bytes(h->M, hloc_of(c))) >= h->P) cs = c;
+        if (jacobi_max_clusters(h->M, c, jacobi_smem_bytes(h->M, hloc_of(c))) >= h->P) { cs = c; one_wave = true; }
+    }
+    // More than one wave of full CTAs: clusters of 8 half CTAs (512 threads, one pair per warp, two CTAs of different
+    // slices per SM) hold as many slices per wave and overlap each other's barrier and exchange waits.
+    bool half = false;
+    if (!one_wave && epl <= 8 && fits(8, true) && hloc_of(8, true) >= 6 && hloc_of(8, true) <= 16) {
+        const int full_per_wave = jacobi_max_clusters(h->M, cs, jacobi_smem_bytes(h->M, hloc_of(cs)));
+        const int half_per_wave = jacobi_max_clusters(h->M, 8, jacobi_smem_bytes(h->M, hloc_of(8, true)), true);
+        auto waves = [&](int per) { return per > 0 ? (h->P + per - 1) / per : 1 << 20; };
+        if (waves(half_per_wave) <= waves(full_per_wave) && !getenv("PFSM_JACOBI_FULL")) {  // env: diagnostic, full CTAs only
+            half = true;
+            cs = 8;
+        }
     }
     if (const char* e = getenv("PFSM_JACOBI_CS")) {  // diagnostic override of the cluster size
         const int want = atoi(e);
-        if ((want == 1 || want == 2 || want == 4 || want == 8) && fits(want)) cs = want;
+        if ((want == 1 || want == 2 || want == 4 || want == 8) && fits(want, half)) cs = want;
     }
+    h->jac_half = half;
     h->jac_cs = cs;
-    h->jac_hloc = hloc_of(cs);
+    h->jac_hloc = hloc_of(cs, half);
 }
 
 static int launch_jacobi(pfsm_ctx* h, const double* A, double* V, cudaStream_t st, int32_t s0 = 0, int32_t ns = -1,
                          int32_t compact = 0) {
     if (ns < 0) ns = h->P;
     PFSM_CUDA(cudaMemsetAsync(h->rotcnt, 0, (size_t)h->P * JACOBI_MAX_SWEEPS * sizeof(int), st));
+    if (h->jac_cs > 0 && h->jac_half) {
+        switch (jacobi_padded_rows(h->M) / 32) {
+            case 2: return launch_jacobi_smem_t<2, true>(h, A, V, st, s0, ns, compact);
+            case 4: return launch_jacobi_smem_t<4, true>(h, A, V, st, s0, ns, compact);
+            case 6: return launch_jacobi_smem_t<6, true>(h, A, V, st, s0, ns, compact);
+            default: return launch_jacobi_smem_t<8, true>(h, A, V, st, s0, ns, compact);
+        }
+    }
     if (h->jac_cs > 0) {
         switch (jacobi_padded_rows(h->M) / 32) {  // doubles per lane per column
             case 2: return launch_jacobi_smem_t<2>(h, A, V, st, s0, ns, compact);
