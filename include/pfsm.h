@@ -60,7 +60,9 @@ typedef struct pfsm_ctx* pfsm_handle_t; /* opaque */
  *   P       number of spectral slices; 1 <= P <= N.  Slice s holds eigen-indices floor(s N / P) .. floor((s+1) N / P) - 1:
  *           N/P of them when P divides N (the paper writes m = N/P), else floor(N/P) or ceil(N/P) (reading R14)
  *   window  halo rows/columns added on each side of a slice's diagonal block; >= 0.
- *           M = min(N, ceil(N/P) + 2*window), the order of every submatrix, must be <= 512 in this version.
+ *           M = min(N, ceil(N/P) + 2*window), the order of every submatrix, must be <= 4096 in this version
+ *           (M <= ~480: shared-memory resident Jacobi; M <= 512: L2-resident; 512 < M <= 4096: the wide-window
+ *           kernel, one persistent grid over all slices -- the paper's gamma = 0.2-0.3 regime).
  *   iters   folded-spectrum iterations of Eq. 11; >= 0
  *   alpha   step length of Eq. 11; finite and > 0.  The library does not estimate spectra:
  *           alpha = 0.5 / max|lambda|^2 keeps every damping factor 1 - alpha (lambda - eps)^2 in [-1, 1].

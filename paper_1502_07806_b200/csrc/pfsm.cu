@@ -18,6 +18,7 @@
 #include "gemm_tn.cuh"
 #include "kernels.cuh"
 #include "jacobi_smem.cuh"
+#include "jacobi_wide.cuh"
 
 namespace pfsm {
 
@@ -76,7 +77,9 @@ struct pfsm_ctx {
     double* eps = nullptr;    // N shifts
     double* resid = nullptr;  // N residual norms
     int* rotcnt = nullptr;    // P x JACOBI_MAX_SWEEPS rotation counters of step 2
+    unsigned int* jw_bar = nullptr;  // grid-barrier counter of the wide-window Jacobi (M > 512)
     double* nrm_g = nullptr;  // P x (M + 16): final column norms of the shared-memory Jacobi
+    bool jac_wide = false;             // forced use of the wide-window Jacobi (jacobi_wide.cuh) below M = 513
     int jac_cs = 0, jac_hloc = 0;  // cluster size / seats per CTA of the shared-memory Jacobi (0 = L2 kernel)
     double* gdiag = nullptr;  // N: diag(V^T V) before the factorization (breakdown threshold)
     int32_t* slice_tab = nullptr;  // g0[P], lo[P], off[P], cnt[P]
@@ -184,7 +187,7 @@ int pfsm_create(pfsm_handle_t* out, int64_t N, int32_t P, int32_t window, int32_
     if (!std::isfinite(alpha) || !(alpha > 0.0)) return -6;
     const int64_t m = (N + P - 1) / P;  // largest slice; all slices have N / P eigenpairs when P divides N (R14)
     const int64_t M = std::min<int64_t>(N, m + 2 * (int64_t)window);
-    if (M > 512) return -4;
+    if (M > JW_MAX_M) return -4;
 
     pfsm_ctx* h = new pfsm_ctx();
     h->N = N; h->P = P; h->window = window; h->iters = iters; h->alpha = alpha;
@@ -207,6 +210,7 @@ int pfsm_create(pfsm_handle_t* out, int64_t N, int32_t P, int32_t window, int32_
     TRY(dev_alloc(h, (void**)&h->gdiag, N * sizeof(double)));
     TRY(dev_alloc(h, (void**)&h->rotcnt, (size_t)P * JACOBI_MAX_SWEEPS * sizeof(int)));
     TRY(dev_alloc(h, (void**)&h->nrm_g, (size_t)P * (M + 16) * sizeof(double)));
+    TRY(dev_alloc(h, (void**)&h->jw_bar, sizeof(unsigned int)));
     choose_jacobi_layout(h);
     TRY(dev_alloc(h, (void**)&h->slice_tab, 4 * (size_t)P * sizeof(int32_t)));
     const int32_t ntr = (int32_t)((N + BM - 1) / BM);
@@ -272,7 +276,7 @@ int pfsm_create(pfsm_handle_t* out, int64_t N, int32_t P, int32_t window, int32_
 int pfsm_destroy(pfsm_handle_t h) {
     if (!h) return 0;
     cudaDeviceSynchronize();
-    void* ptrs[] = {h->W, h->S, h->O, h->Dinv, h->Gws, h->eps, h->resid, h->gdiag, h->rotcnt, h->nrm_g, h->slice_tab, h->krange, h->info, h->chain_cnt,
+    void* ptrs[] = {h->W, h->S, h->O, h->Dinv, h->Gws, h->eps, h->resid, h->gdiag, h->rotcnt, h->nrm_g, h->jw_bar, h->slice_tab, h->krange, h->info, h->chain_cnt,
                     h->A_stage, h->V_stage, h->lam_stage, h->Ap, h->LT, h->DinvT};
     for (void* p : ptrs)
         if (p) cudaFree(p);
@@ -405,6 +409,8 @@ static int jacobi_max_clusters(int M, int cs, size_t smem, bool half = false) {
 static void choose_jacobi_layout(pfsm_ctx* h) {
     h->jac_cs = 0;
     h->jac_hloc = 0;
+    h->jac_wide = getenv("PFSM_JACOBI_WIDE") != nullptr;  // diagnostic: the wide-window kernel at any M
+    if (h->M > 512 || h->jac_wide) return;
     if (getenv("PFSM_JACOBI_L2")) return;  // diagnostic: force the L2-resident kernel (the large-M fallback)
     const size_t budget = 220 * 1024;
     // seats per CTA; one more (phantom) pair when seat 0 and seat h_loc-1 would fall to the same warp, because the
@@ -449,10 +455,50 @@ static void choose_jacobi_layout(pfsm_ctx* h) {
     h->jac_hloc = hloc_of(cs, half);
 }
 
+// Wide windows (512 < M <= 4096): one persistent cooperative grid over all slices (jacobi_wide.cuh)
+extern "C++" {
+template <int EPT>
+static int launch_jacobi_wide_t(pfsm_ctx* h, const double* A, double* V, cudaStream_t st, int32_t s0, int32_t ns) {
+    SliceTable tab{h->slice_tab, h->slice_tab + h->P, h->slice_tab + 2 * (size_t)h->P, h->slice_tab + 3 * (size_t)h->P};
+    const size_t smem = (size_t)ns * sizeof(int);
+    int per_sm = 0, sms = 0;
+    PFSM_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, jacobi_wide_kernel<EPT>, JW_THREADS, smem));
+    PFSM_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, h->device));
+    if (per_sm < 1) return PFSM_CUDA_ERROR_BASE + (int)cudaErrorLaunchOutOfResources;
+    const int64_t units = (int64_t)ns * ((h->M + 1) / 2);
+    const int64_t want = (units + JW_GPC - 1) / JW_GPC;
+    const int grid = (int)std::max<int64_t>(1, std::min<int64_t>((int64_t)per_sm * sms, want));
+    PFSM_CUDA(cudaMemsetAsync(h->jw_bar, 0, sizeof(unsigned int), st));
+    cudaLaunchConfig_t cfg;
+    memset(&cfg, 0, sizeof(cfg));
+    cfg.gridDim = dim3((unsigned)grid);
+    cfg.blockDim = dim3(JW_THREADS);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeCooperative;  // all CTAs co-resident: the grid barrier cannot deadlock
+    attr[0].val.cooperative = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    PFSM_CUDA(cudaLaunchKernelEx(&cfg, jacobi_wide_kernel<EPT>, A, h->N, h->M, tab, h->Gws, h->nrm_g, V, h->eps,
+                                 h->rotcnt, h->info, s0, ns, h->jw_bar));
+    return 0;
+}
+}  // extern "C++"
+
 static int launch_jacobi(pfsm_ctx* h, const double* A, double* V, cudaStream_t st, int32_t s0 = 0, int32_t ns = -1,
                          int32_t compact = 0) {
     if (ns < 0) ns = h->P;
     PFSM_CUDA(cudaMemsetAsync(h->rotcnt, 0, (size_t)h->P * JACOBI_MAX_SWEEPS * sizeof(int), st));
+    if (h->M > 512 || h->jac_wide) {
+        const int ept = (h->M + JW_GROUP - 1) / JW_GROUP;
+        if (ept <= 2) return launch_jacobi_wide_t<2>(h, A, V, st, s0, ns);
+        if (ept <= 4) return launch_jacobi_wide_t<4>(h, A, V, st, s0, ns);
+        if (ept <= 6) return launch_jacobi_wide_t<6>(h, A, V, st, s0, ns);
+        if (ept <= 8) return launch_jacobi_wide_t<8>(h, A, V, st, s0, ns);
+        if (ept <= 12) return launch_jacobi_wide_t<12>(h, A, V, st, s0, ns);
+        return launch_jacobi_wide_t<16>(h, A, V, st, s0, ns);
+    }
     if (h->jac_cs > 0 && h->jac_half) {
         switch (jacobi_padded_rows(h->M) / 32) {
             case 2: return launch_jacobi_smem_t<2, true>(h, A, V, st, s0, ns, compact);
