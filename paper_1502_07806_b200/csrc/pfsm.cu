@@ -19,6 +19,7 @@
 #include "kernels.cuh"
 #include "jacobi_smem.cuh"
 #include "jacobi_wide.cuh"
+#include "tridiag_eig.cuh"
 
 namespace pfsm {
 
@@ -79,7 +80,9 @@ struct pfsm_ctx {
     int* rotcnt = nullptr;    // P x JACOBI_MAX_SWEEPS rotation counters of step 2
     unsigned int* jw_bar = nullptr;  // grid-barrier counter of the wide-window Jacobi (M > 512)
     double* nrm_g = nullptr;  // P x (M + 16): final column norms of the shared-memory Jacobi
-    bool jac_wide = false;             // forced use of the wide-window Jacobi (jacobi_wide.cuh) below M = 513
+    bool jac_wide = false;             // wide-window Jacobi (jacobi_wide.cuh): PFSM_JACOBI_WIDE=1, at any M
+    bool tridiag = false;              // tridiagonalization route (tridiag_eig.cuh): default for M > 512, PFSM_TRIDIAG=1 at any M
+    TriWs tri{};                       // its workspace
     int jac_cs = 0, jac_hloc = 0;  // cluster size / seats per CTA of the shared-memory Jacobi (0 = L2 kernel)
     double* gdiag = nullptr;  // N: diag(V^T V) before the factorization (breakdown threshold)
     int32_t* slice_tab = nullptr;  // g0[P], lo[P], off[P], cnt[P]
@@ -212,6 +215,18 @@ int pfsm_create(pfsm_handle_t* out, int64_t N, int32_t P, int32_t window, int32_
     TRY(dev_alloc(h, (void**)&h->nrm_g, (size_t)P * (M + 16) * sizeof(double)));
     TRY(dev_alloc(h, (void**)&h->jw_bar, sizeof(unsigned int)));
     choose_jacobi_layout(h);
+    if (h->tridiag) {
+        const size_t pm = (size_t)P * M * sizeof(double), mn = (size_t)M * N;
+        TRY(dev_alloc(h, (void**)&h->tri.d, pm));
+        TRY(dev_alloc(h, (void**)&h->tri.e, pm));
+        TRY(dev_alloc(h, (void**)&h->tri.tau, pm));
+        TRY(dev_alloc(h, (void**)&h->tri.pbuf, 2 * pm));
+        TRY(dev_alloc(h, (void**)&h->tri.vbuf, 2 * pm));
+        TRY(dev_alloc(h, (void**)&h->tri.lam, N * sizeof(double)));
+        TRY(dev_alloc(h, (void**)&h->tri.zscale, N * sizeof(double)));
+        for (int i = 0; i < 5; ++i) TRY(dev_alloc(h, (void**)&h->tri.f[i], mn * sizeof(double)));
+        TRY(dev_alloc(h, (void**)&h->tri.piv, mn));
+    }
     TRY(dev_alloc(h, (void**)&h->slice_tab, 4 * (size_t)P * sizeof(int32_t)));
     const int32_t ntr = (int32_t)((N + BM - 1) / BM);
     TRY(dev_alloc(h, (void**)&h->krange, (size_t)ntr * sizeof(int2)));
@@ -277,7 +292,9 @@ int pfsm_destroy(pfsm_handle_t h) {
     if (!h) return 0;
     cudaDeviceSynchronize();
     void* ptrs[] = {h->W, h->S, h->O, h->Dinv, h->Gws, h->eps, h->resid, h->gdiag, h->rotcnt, h->nrm_g, h->jw_bar, h->slice_tab, h->krange, h->info, h->chain_cnt,
-                    h->A_stage, h->V_stage, h->lam_stage, h->Ap, h->LT, h->DinvT};
+                    h->A_stage, h->V_stage, h->lam_stage, h->Ap, h->LT, h->DinvT,
+                    h->tri.d, h->tri.e, h->tri.tau, h->tri.pbuf, h->tri.vbuf, h->tri.lam, h->tri.zscale,
+                    h->tri.f[0], h->tri.f[1], h->tri.f[2], h->tri.f[3], h->tri.f[4], h->tri.piv};
     for (void* p : ptrs)
         if (p) cudaFree(p);
     for (int i = 0; i < 5; ++i)
@@ -409,8 +426,9 @@ static int jacobi_max_clusters(int M, int cs, size_t smem, bool half = false) {
 static void choose_jacobi_layout(pfsm_ctx* h) {
     h->jac_cs = 0;
     h->jac_hloc = 0;
-    h->jac_wide = getenv("PFSM_JACOBI_WIDE") != nullptr;  // diagnostic: the wide-window kernel at any M
-    if (h->M > 512 || h->jac_wide) return;
+    h->jac_wide = getenv("PFSM_JACOBI_WIDE") != nullptr;  // diagnostic: the wide-window Jacobi kernel at any M
+    h->tridiag = !h->jac_wide && (h->M > 512 || getenv("PFSM_TRIDIAG") != nullptr);  // default for wide windows
+    if (h->M > 512 || h->jac_wide || h->tridiag) return;
     if (getenv("PFSM_JACOBI_L2")) return;  // diagnostic: force the L2-resident kernel (the large-M fallback)
     const size_t budget = 220 * 1024;
     // seats per CTA; one more (phantom) pair when seat 0 and seat h_loc-1 would fall to the same warp, because the
@@ -486,10 +504,58 @@ static int launch_jacobi_wide_t(pfsm_ctx* h, const double* A, double* V, cudaStr
 }
 }  // extern "C++"
 
+// Wide windows, default route: Householder tridiagonalization + bisection + inverse iteration + back-transformation
+static int launch_tridiag(pfsm_ctx* h, const double* A, double* V, cudaStream_t st, int32_t s0, int32_t ns) {
+    SliceTable tab{h->slice_tab, h->slice_tab + h->P, h->slice_tab + 2 * (size_t)h->P, h->slice_tab + 3 * (size_t)h->P};
+    const int M = h->M;
+    int sms = 0;
+    PFSM_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, h->device));
+    {
+        const size_t smem = 3 * (size_t)M * sizeof(double);
+        PFSM_CUDA(cudaFuncSetAttribute(sytrd_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        int per_sm = 0;
+        PFSM_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, sytrd_kernel, TRD_THREADS, smem));
+        if (per_sm < 1) return PFSM_CUDA_ERROR_BASE + (int)cudaErrorLaunchOutOfResources;
+        const int cap = per_sm * sms;
+        int C = std::max(1, std::min(cap / ns, (M + 15) / 16));  // CTAs per slice; a CTA keeps >= 16 rows while rows last
+        const int grid = std::min(cap, ns * C);
+        PFSM_CUDA(cudaMemsetAsync(h->jw_bar, 0, sizeof(unsigned int), st));
+        cudaLaunchConfig_t cfg;
+        memset(&cfg, 0, sizeof(cfg));
+        cfg.gridDim = dim3((unsigned)grid);
+        cfg.blockDim = dim3(TRD_THREADS);
+        cfg.dynamicSmemBytes = smem;
+        cfg.stream = st;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeCooperative;  // all CTAs co-resident: the grid barrier cannot deadlock
+        attr[0].val.cooperative = 1;
+        cfg.attrs = attr;
+        cfg.numAttrs = 1;
+        PFSM_CUDA(cudaLaunchKernelEx(&cfg, sytrd_kernel, A, h->N, (int32_t)M, tab, h->Gws, h->tri, h->P, s0, ns, (int32_t)C,
+                                     h->jw_bar));
+    }
+    const size_t smem2 = 2 * (size_t)M * sizeof(double);
+    PFSM_CUDA(cudaFuncSetAttribute(tri_bisect_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem2));
+    PFSM_CUDA(cudaFuncSetAttribute(tri_invit_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem2));
+    const dim3 g2((unsigned)((h->m + TRI_THREADS - 1) / TRI_THREADS), (unsigned)ns);
+    tri_bisect_kernel<<<g2, TRI_THREADS, smem2, st>>>((int32_t)M, tab, h->tri, s0);
+    PFSM_CUDA(cudaGetLastError());
+    tri_invit_kernel<<<g2, TRI_THREADS, smem2, st>>>(h->N, (int32_t)M, tab, h->tri, s0);
+    PFSM_CUDA(cudaGetLastError());
+    const int nvec = (int)std::max<size_t>(1, std::min<size_t>(BT_WARPS, (size_t)200 * 1024 / ((size_t)M * sizeof(double))));
+    const size_t smem3 = (size_t)nvec * M * sizeof(double);
+    PFSM_CUDA(cudaFuncSetAttribute(tri_backtransform_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem3));
+    const dim3 g3((unsigned)((h->m + nvec - 1) / nvec), (unsigned)ns);
+    tri_backtransform_kernel<<<g3, 32 * nvec, smem3, st>>>(h->N, (int32_t)M, tab, h->Gws, h->tri, V, h->eps, s0);
+    PFSM_CUDA(cudaGetLastError());
+    return 0;
+}
+
 static int launch_jacobi(pfsm_ctx* h, const double* A, double* V, cudaStream_t st, int32_t s0 = 0, int32_t ns = -1,
                          int32_t compact = 0) {
     if (ns < 0) ns = h->P;
     PFSM_CUDA(cudaMemsetAsync(h->rotcnt, 0, (size_t)h->P * JACOBI_MAX_SWEEPS * sizeof(int), st));
+    if (h->tridiag) return launch_tridiag(h, A, V, st, s0, ns);
     if (h->M > 512 || h->jac_wide) {
         const int ept = (h->M + JW_GROUP - 1) / JW_GROUP;
         if (ept <= 2) return launch_jacobi_wide_t<2>(h, A, V, st, s0, ns);

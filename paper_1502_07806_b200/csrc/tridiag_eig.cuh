@@ -1,0 +1,427 @@
+// tridiag_eig.cuh -- step 2 for wide windows (512 < M <= 4096; the paper's gamma = M/N = 0.2-0.3 regime,
+// "M <= 3000") as a batched dense symmetric eigensolver in four kernels.  Only the slice's m of
+// the M eigenpairs of B_s are wanted (local ascending ranks off .. off+m-1), which this route exploits:
+//
+//   sytrd_kernel            B_s = Q T Q^T, Householder tridiagonalization of all slices at once by ONE persistent
+//                           cooperative grid (C CTAs per slice, grid barrier per column).  The rank-2 update of column
+//                           k-1 is applied inside the pass that forms the matrix-vector product of column k, so the
+//                           trailing matrix is read and written once per column: 16 (M-k)^2 bytes -> (16/3) M^3 bytes
+//                           per slice.  HBM / L2 bandwidth bound.
+//   tri_bisect_kernel       eigenvalue of rank off+t of T by bisection on the Sturm count, one thread per eigenvalue
+//   tri_invit_kernel        its eigenvector by inverse iteration: LU of T - lambda I with partial pivoting, three
+//                           solves from a counter-based random start, one thread per eigenvector, factors stored
+//                           [row][vector] so that a warp's accesses coalesce
+//   tri_backtransform_kernel  y = H_0 H_1 ... H_{M-3} z, one warp per eigenvector (the vector stays in shared
+//                           memory, the reflectors stream through L1/L2), written zero-padded into V
+//
+// Eigenvalues closer than 10 eps |lambda| get shifts pushed apart as LAPACK's dstein does; there is no
+// re-orthogonalization inside clusters: step 4 orthonormalizes all N vectors anyway, and vectors of a
+// tight cluster that come out numerically dependent are flagged there (info = index of the dependent vector).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "jacobi_wide.cuh"  // jw_grid_barrier
+#include "kernels.cuh"
+
+namespace pfsm {
+
+constexpr int TRD_THREADS = 512;
+constexpr int TRI_THREADS = 128;  // bisection / inverse iteration: threads (= eigenpairs) per CTA
+constexpr int BT_WARPS = 8;       // back-transformation: eigenvectors per CTA (fewer when 8 M-vectors exceed shared memory)
+
+struct TriWs {                  // workspace of the tridiagonal route (device pointers)
+    double* d;                  // P x M   diagonal of T
+    double* e;                  // P x M   sub-diagonal of T (e[k] couples k and k+1)
+    double* tau;                // P x M   Householder scalars
+    double* pbuf;               // 2 x P x M   matrix-vector products, double-buffered by column parity
+    double* vbuf;               // 2 x P x M   current Householder vector, double-buffered
+    double* lam;                // N       eigenvalues (unperturbed)
+    double* zscale;             // N       1 / ||z|| of the inverse-iteration vector
+    double* f[5];               // 5 x (M x N): U diagonal reciprocal, U super-diagonals 1 and 2, L multipliers, z
+    unsigned char* piv;         // M x N   row interchange flags
+};
+
+__device__ __forceinline__ double block_sum_512(double v, double* red) {  // fixed order -> every CTA gets the same bits
+    v = warp_sum(v);
+    __syncthreads();
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = v;
+    __syncthreads();
+    double s = 0.0;
+#pragma unroll
+    for (int w = 0; w < TRD_THREADS / 32; ++w) s += red[w];
+    return s;
+}
+
+// ---------------------------------------------------------------------------------------------
+// Householder tridiagonalization (the unblocked LAPACK dsytd2 recurrence, lower variant, on full symmetric storage).
+// Virtual CTA (sl, c), c < C, owns rows i with i % C == c of slice s_off + sl.  Column k:
+//   prologue (every CTA of the slice, redundantly and bitwise identically):
+//     w_{k-1} = p_{k-1} - (tau_{k-1}/2)(p_{k-1} . v_{k-1}) v_{k-1}            (p from pbuf, v from vbuf)
+//     column k of the updated matrix: cc = B[k, k:] - (v_{k-1} w_{k-1}[k] + w_{k-1} v_{k-1}[k]);  d[k] = cc[k]
+//     Householder vector of cc[k+1:]: beta = -sign(alpha) ||x||, tau = (beta - alpha)/beta, v = x/(alpha - beta), v[k+1] = 1
+//   pass (owned rows i > k): B[i, k+1:] -= v_{k-1}[i] w_{k-1} + w_{k-1}[i] v_{k-1};  p_k[i] = tau_k B[i, k+1:] . v_k
+//   grid barrier.
+// Reflector k is kept in row k of the slice's matrix (columns k+1 .., leading 1 stored) once that row is dead.
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(TRD_THREADS, 1)
+sytrd_kernel(const double* __restrict__ A, int64_t N, int32_t M, SliceTable tab, double* __restrict__ Gws, TriWs ws,
+             int32_t P, int32_t s_off, int32_t ns, int32_t C, unsigned int* __restrict__ bar) {
+    extern __shared__ double sm[];
+    double* vp = sm;          // v_{k-1}
+    double* wp = sm + M;      // w_{k-1}
+    double* vn = sm + 2 * M;  // v_k
+    __shared__ double red[TRD_THREADS / 32];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    constexpr int NW = TRD_THREADS / 32;
+    unsigned int phase = 0;
+    const int nv = ns * C;
+
+    // copy B_s (row lo + i of A, columns lo ..) into the workspace
+    for (int vb = blockIdx.x; vb < nv; vb += gridDim.x) {
+        const int sl = vb / C, c = vb - sl * C, s = s_off + sl;
+        const int lo = tab.lo[s];
+        double* G = Gws + (size_t)s * M * M;
+        for (int i = c + C * warp; i < M; i += C * NW) {
+            const double* a = A + (size_t)(lo + i) * N + lo;
+            for (int j = lane; j < M; j += 32) G[(size_t)i * M + j] = a[j];
+        }
+    }
+    jw_grid_barrier(bar, phase);
+
+    for (int k = 0; k <= M - 2; ++k) {
+        for (int vb = blockIdx.x; vb < nv; vb += gridDim.x) {
+            const int sl = vb / C, c = vb - sl * C, s = s_off + sl;
+            double* G = Gws + (size_t)s * M * M;
+            const size_t so = (size_t)s * M;
+            __syncthreads();  // shared vectors of the previous virtual CTA are no longer read
+            // ---- prologue
+            double tau_p = 0.0;
+            if (k > 0) {
+                tau_p = __ldcg(ws.tau + so + k - 1);
+                const double* pv_ = ws.pbuf + (size_t)((k - 1) & 1) * P * M + so;
+                const double* vv_ = ws.vbuf + (size_t)((k - 1) & 1) * P * M + so;
+                double acc = 0.0;
+                for (int i = k + tid; i < M; i += TRD_THREADS) {
+                    const double v = __ldcg(vv_ + i), p = __ldcg(pv_ + i);
+                    vp[i] = v;
+                    wp[i] = p;
+                    acc = fma(p, v, acc);
+                }
+                const double pv = block_sum_512(acc, red);
+                const double hf = 0.5 * tau_p * pv;
+                for (int i = k + tid; i < M; i += TRD_THREADS) wp[i] = fma(-hf, vp[i], wp[i]);
+                __syncthreads();
+                if (c == 0)  // row k-1 is dead: keep reflector k-1 there (columns k .., leading 1 included)
+                    for (int i = k + tid; i < M; i += TRD_THREADS) G[(size_t)(k - 1) * M + i] = vp[i];
+            }
+            double acc = 0.0, alpha = 0.0, dk = 0.0;
+            {
+                const double wk = (k > 0) ? wp[k] : 0.0, vk = (k > 0) ? vp[k] : 0.0;
+                for (int i = k + tid; i < M; i += TRD_THREADS) {
+                    double b = __ldcg(G + (size_t)k * M + i);
+                    if (k > 0) b -= (__dmul_rn(vp[i], wk) + __dmul_rn(wp[i], vk));
+                    vn[i] = b;
+                    if (i >= k + 2) acc = fma(b, b, acc);
+                }
+            }
+            const double xn2 = block_sum_512(acc, red);  // (its barriers also publish vn)
+            dk = vn[k];
+            alpha = vn[k + 1];
+            double tau = 0.0, beta = alpha, scal = 0.0;
+            if (xn2 > 0.0) {
+                beta = -copysign(sqrt(fma(alpha, alpha, xn2)), alpha);
+                tau = (beta - alpha) / beta;
+                scal = 1.0 / (alpha - beta);
+            }
+            __syncthreads();
+            for (int i = k + 1 + tid; i < M; i += TRD_THREADS) vn[i] = (i == k + 1) ? 1.0 : vn[i] * scal;
+            __syncthreads();
+            if (c == 0) {
+                double* vb_ = ws.vbuf + (size_t)(k & 1) * P * M + so;
+                for (int i = k + 1 + tid; i < M; i += TRD_THREADS) vb_[i] = vn[i];
+                if (tid == 0) {
+                    ws.d[so + k] = dk;
+                    ws.e[so + k] = beta;
+                    ws.tau[so + k] = tau;
+                }
+            }
+            // ---- pass over the owned rows below k
+            double* pb = ws.pbuf + (size_t)(k & 1) * P * M + so;
+            int i0 = k + 1;
+            i0 += ((c - i0) % C + C) % C;  // first owned row >= k+1
+            for (int i = i0 + C * warp; i < M; i += C * NW) {
+                double* row = G + (size_t)i * M;
+                const double vi = (k > 0) ? vp[i] : 0.0, wi = (k > 0) ? wp[i] : 0.0;
+                double a0 = 0.0, a1 = 0.0;
+                int j = k + 1 + lane;
+                for (; j + 32 < M; j += 64) {
+                    double b0 = __ldcg(row + j), b1 = __ldcg(row + j + 32);
+                    if (k > 0) {
+                        b0 -= (__dmul_rn(vi, wp[j]) + __dmul_rn(wi, vp[j]));
+                        b1 -= (__dmul_rn(vi, wp[j + 32]) + __dmul_rn(wi, vp[j + 32]));
+                        row[j] = b0;
+                        row[j + 32] = b1;
+                    }
+                    a0 = fma(b0, vn[j], a0);
+                    a1 = fma(b1, vn[j + 32], a1);
+                }
+                if (j < M) {
+                    double b0 = __ldcg(row + j);
+                    if (k > 0) {
+                        b0 -= (__dmul_rn(vi, wp[j]) + __dmul_rn(wi, vp[j]));
+                        row[j] = b0;
+                    }
+                    a0 = fma(b0, vn[j], a0);
+                }
+                a0 = warp_sum(a0 + a1);
+                if (lane == 0) pb[i] = tau * a0;
+            }
+        }
+        jw_grid_barrier(bar, phase);
+    }
+    // last diagonal entry (its pending update was applied by the pass of column M-2)
+    for (int vb = blockIdx.x; vb < nv; vb += gridDim.x) {
+        const int sl = vb / C, c = vb - sl * C, s = s_off + sl;
+        if (c == 0 && tid == 0) {
+            ws.d[(size_t)s * M + M - 1] = __ldcg(Gws + (size_t)s * M * M + (size_t)(M - 1) * M + M - 1);
+            ws.e[(size_t)s * M + M - 1] = 0.0;
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Eigenvalue of local rank off + t of T_s by bisection.  count(x) = number of eigenvalues < x = number of negative
+// pivots of the LDL^T recurrence q_i = d_i - x - e_{i-1}^2 / q_{i-1}  (Sturm sequence; |q| < pivmin -> -pivmin).
+// grid.x = ceil(mmax / TRI_THREADS), grid.y = ns.  Dynamic shared memory: d[M], e2[M].
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(TRI_THREADS)
+tri_bisect_kernel(int32_t M, SliceTable tab, TriWs ws, int32_t s_off) {
+    extern __shared__ double sm[];
+    double* d = sm;
+    double* e2 = sm + M;
+    __shared__ double rlo[TRI_THREADS / 32], rhi[TRI_THREADS / 32], rem[TRI_THREADS / 32];
+    const int s = s_off + blockIdx.y, tid = threadIdx.x;
+    const size_t so = (size_t)s * M;
+    double glo = 1e300, ghi = -1e300, emax = 0.0;
+    for (int i = tid; i < M; i += TRI_THREADS) {
+        const double di = ws.d[so + i], ei = (i < M - 1) ? ws.e[so + i] : 0.0, em = (i > 0) ? ws.e[so + i - 1] : 0.0;
+        d[i] = di;
+        e2[i] = ei * ei;
+        const double r = fabs(ei) + fabs(em);
+        glo = fmin(glo, di - r);
+        ghi = fmax(ghi, di + r);
+        emax = fmax(emax, ei * ei);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        glo = fmin(glo, __shfl_xor_sync(0xffffffffu, glo, o));
+        ghi = fmax(ghi, __shfl_xor_sync(0xffffffffu, ghi, o));
+        emax = fmax(emax, __shfl_xor_sync(0xffffffffu, emax, o));
+    }
+    if ((tid & 31) == 0) {
+        rlo[tid >> 5] = glo;
+        rhi[tid >> 5] = ghi;
+        rem[tid >> 5] = emax;
+    }
+    __syncthreads();
+    for (int w = 0; w < TRI_THREADS / 32; ++w) {
+        glo = fmin(glo, rlo[w]);
+        ghi = fmax(ghi, rhi[w]);
+        emax = fmax(emax, rem[w]);
+    }
+    const int t = blockIdx.x * TRI_THREADS + tid;
+    if (t >= tab.cnt[s]) return;
+    const int rank = tab.off[s] + t;
+    const double pivmin = 2.2250738585072014e-308 * fmax(1.0, emax);
+    const double span = fmax(fabs(glo), fabs(ghi));
+    double lo = glo - 2.0 * 2.220446049250313e-16 * span * M - 2.0 * pivmin;
+    double hi = ghi + 2.0 * 2.220446049250313e-16 * span * M + 2.0 * pivmin;
+    for (int it = 0; it < 200; ++it) {
+        const double mid = 0.5 * (lo + hi);
+        if (mid <= lo || mid >= hi) break;
+        if (hi - lo <= 2.220446049250313e-16 * (fmax(fabs(lo), fabs(hi)) + 0.125 * span) + 2.0 * pivmin) break;
+        double q = d[0] - mid;
+        if (fabs(q) < pivmin) q = -pivmin;
+        int cnt = q < 0.0 ? 1 : 0;
+        for (int i = 1; i < M; ++i) {
+            q = d[i] - mid - e2[i - 1] / q;
+            if (fabs(q) < pivmin) q = -pivmin;
+            cnt += q < 0.0 ? 1 : 0;
+        }
+        if (cnt > rank) hi = mid;
+        else lo = mid;
+    }
+    ws.lam[tab.g0[s] + t] = 0.5 * (lo + hi);
+}
+
+// counter-based uniform in (-1, 1): splitmix64 finalizer of (vector, row)
+__device__ __forceinline__ double tri_start_value(uint32_t vec, uint32_t row) {
+    uint64_t z = ((uint64_t)vec << 32 | row) * 0x9E3779B97F4A7C15ull + 0xD1B54A32D192ED03ull;
+    z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull;
+    z = (z ^ (z >> 27)) * 0x94D049BB133111EBull;
+    z ^= z >> 31;
+    return ((double)(z >> 11) + 0.5) * (2.0 / 9007199254740992.0) - 1.0;
+}
+
+// ---------------------------------------------------------------------------------------------
+// Eigenvector of T_s for eigenvalue lam[g0 + t]: inverse iteration (the LAPACK dstein scheme without its cluster
+// re-orthogonalization).  T - x I = P L U with partial pivoting (the dgttrf recurrence), pivots below eps ||T|| are
+// replaced by eps ||T||; three solves from a random start, the vector rescaled to unit 2-norm between solves.
+// Factors and vector live in global memory as [row i][vector g], g = g0 + t: a warp touches 32 consecutive doubles.
+// Output: z in ws.f[4] (not normalized), ws.zscale[g] = 1 / ||z||_2.
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(TRI_THREADS)
+tri_invit_kernel(int64_t N, int32_t M, SliceTable tab, TriWs ws, int32_t s_off) {
+    extern __shared__ double sm[];
+    double* d = sm;
+    double* e = sm + M;
+    __shared__ double rmx[TRI_THREADS / 32];
+    const int s = s_off + blockIdx.y, tid = threadIdx.x;
+    const size_t so = (size_t)s * M;
+    double tmax = 0.0;
+    for (int i = tid; i < M; i += TRI_THREADS) {
+        const double di = ws.d[so + i], ei = (i < M - 1) ? ws.e[so + i] : 0.0;
+        d[i] = di;
+        e[i] = ei;
+        tmax = fmax(tmax, fabs(di) + 2.0 * fabs(ei));
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) tmax = fmax(tmax, __shfl_xor_sync(0xffffffffu, tmax, o));
+    if ((tid & 31) == 0) rmx[tid >> 5] = tmax;
+    __syncthreads();
+    for (int w = 0; w < TRI_THREADS / 32; ++w) tmax = fmax(tmax, rmx[w]);
+    const int t = blockIdx.x * TRI_THREADS + tid;
+    const int m = tab.cnt[s];
+    if (t >= m) return;
+    const int g0 = tab.g0[s];
+    const size_t g = (size_t)g0 + t;
+    const double EPS = 2.220446049250313e-16;
+    // shifts of eigenvalues closer than 10 eps |lambda| are pushed apart (dstein); the chain is followed from the
+    // slice's first eigenvalue so that every thread derives the same perturbed sequence
+    double x = ws.lam[g0];
+    for (int j = 1; j <= t; ++j) {
+        const double xj = ws.lam[g0 + j];
+        const double pertol = 10.0 * fabs(EPS * xj);
+        x = (xj - x < pertol) ? x + pertol : xj;
+    }
+    const double pivtol = fmax(EPS * tmax, 1e-300);
+    double* uinv = ws.f[0] + g;  // 1 / U[i][i]
+    double* u1 = ws.f[1] + g;    // U[i][i+1]
+    double* u2 = ws.f[2] + g;    // U[i][i+2]
+    double* lm = ws.f[3] + g;    // multiplier of elimination step i
+    double* z = ws.f[4] + g;
+    unsigned char* pv = ws.piv + g;
+    const size_t st = (size_t)N;
+    {
+        double cur_d = d[0] - x, cur_du = (M > 1) ? e[0] : 0.0;
+        for (int i = 0; i < M - 1; ++i) {
+            const double sub = e[i], nxt_d = d[i + 1] - x, nxt_du = (i + 1 < M - 1) ? e[i + 1] : 0.0;
+            if (fabs(cur_d) >= fabs(sub)) {
+                double piv = cur_d;
+                if (fabs(piv) < pivtol) piv = (piv < 0.0) ? -pivtol : pivtol;
+                const double inv = 1.0 / piv;
+                const double f = sub * inv;
+                uinv[i * st] = inv;
+                u1[i * st] = cur_du;
+                u2[i * st] = 0.0;
+                lm[i * st] = f;
+                pv[i * st] = 0;
+                cur_d = fma(-f, cur_du, nxt_d);
+                cur_du = nxt_du;
+            } else {
+                const double inv = 1.0 / sub;
+                const double f = cur_d * inv;
+                uinv[i * st] = inv;
+                u1[i * st] = nxt_d;
+                u2[i * st] = nxt_du;
+                lm[i * st] = f;
+                pv[i * st] = 1;
+                cur_d = fma(-f, nxt_d, cur_du);
+                cur_du = -f * nxt_du;
+            }
+        }
+        double piv = cur_d;
+        if (fabs(piv) < pivtol) piv = (piv < 0.0) ? -pivtol : pivtol;
+        uinv[(size_t)(M - 1) * st] = 1.0 / piv;
+    }
+    double scale = 1.0;
+    for (int iter = 0; iter < 3; ++iter) {
+        // forward: L^-1 P^T b   (b = scale * previous z, or the random start)
+        double bi = (iter == 0) ? tri_start_value((uint32_t)g, 0u) : z[0] * scale;
+        for (int i = 0; i < M - 1; ++i) {
+            const double bn = (iter == 0) ? tri_start_value((uint32_t)g, (uint32_t)(i + 1)) : z[(size_t)(i + 1) * st] * scale;
+            const double f = lm[i * st];
+            if (pv[i * st]) {
+                z[i * st] = bn;
+                bi = fma(-f, bn, bi);
+            } else {
+                z[i * st] = bi;
+                bi = fma(-f, bi, bn);
+            }
+        }
+        // backward: U^-1
+        double x1 = bi * uinv[(size_t)(M - 1) * st], x2 = 0.0;
+        z[(size_t)(M - 1) * st] = x1;
+        double ss = x1 * x1;
+        for (int i = M - 2; i >= 0; --i) {
+            const double xi = (z[i * st] - u1[i * st] * x1 - u2[i * st] * x2) * uinv[i * st];
+            z[i * st] = xi;
+            ss = fma(xi, xi, ss);
+            x2 = x1;
+            x1 = xi;
+        }
+        scale = rsqrt(ss);
+        // guard against overflow of the sum of squares (growth ~ 1/(eps ||T||) per solve from a unit vector)
+        if (!(ss < 1e300)) {
+            double mx = 0.0;
+            for (int i = 0; i < M; ++i) mx = fmax(mx, fabs(z[i * st]));
+            double s2 = 0.0;
+            for (int i = 0; i < M; ++i) {
+                const double q = z[i * st] / mx;
+                s2 = fma(q, q, s2);
+            }
+            scale = 1.0 / (mx * sqrt(s2));
+        }
+    }
+    ws.zscale[g] = scale;
+}
+
+// ---------------------------------------------------------------------------------------------
+// y = Q z = H_0 H_1 ... H_{M-3} z,  H_k = I - tau_k v_k v_k^T, v_k in row k of the slice's matrix (columns k+1 ..).
+// One warp per eigenvector: z sits in shared memory, the reflectors are read through L1 (all warps of a CTA walk
+// the same reflectors), no block-level synchronization.  Writes V[g0 + j][lo .. lo + M) and eps[g0 + j].
+// grid.x = ceil(mmax / nvec), grid.y = ns; blockDim = 32 nvec; dynamic shared memory nvec * M doubles.
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(32 * BT_WARPS)
+tri_backtransform_kernel(int64_t N, int32_t M, SliceTable tab, const double* __restrict__ Gws, TriWs ws,
+                         double* __restrict__ V, double* __restrict__ eps, int32_t s_off) {
+    extern __shared__ double sm[];
+    const int s = s_off + blockIdx.y, lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nvec = blockDim.x >> 5;
+    const int t = blockIdx.x * nvec + warp;
+    if (t >= tab.cnt[s]) return;
+    const int g0 = tab.g0[s], lo = tab.lo[s];
+    const size_t g = (size_t)g0 + t;
+    double* x = sm + (size_t)warp * M;
+    const double sc = ws.zscale[g];
+    const double* z = ws.f[4] + g;
+    for (int i = lane; i < M; i += 32) x[i] = z[(size_t)i * N] * sc;
+    __syncwarp();
+    const double* G = Gws + (size_t)s * M * M;
+    const double* tau = ws.tau + (size_t)s * M;
+    for (int k = M - 3; k >= 0; --k) {
+        const double tk = __ldg(tau + k);
+        if (tk == 0.0) continue;
+        const double* v = G + (size_t)k * M;
+        double acc = 0.0;
+        for (int i = k + 1 + lane; i < M; i += 32) acc = fma(__ldg(v + i), x[i], acc);
+        acc = warp_sum(acc) * tk;
+        for (int i = k + 1 + lane; i < M; i += 32) x[i] = fma(-acc, __ldg(v + i), x[i]);
+        __syncwarp();
+    }
+    double* out = V + g * (size_t)N + lo;
+    for (int i = lane; i < M; i += 32) out[i] = x[i];
+    if (lane == 0) eps[g] = ws.lam[g];
+}
+
+}  // namespace pfsm

@@ -120,24 +120,31 @@ def test_l2_resident_jacobi_fallback_matches_oracle(N, P, w, monkeypatch):
     assert np.abs(align_signs(g2["Vr"], V2) - V2).max() < 1e-9
 
 
-@pytest.mark.parametrize("N,P,w", [(256, 4, 16), (270, 6, 4), (600, 3, 20), (66, 64, 2)])
-def test_wide_window_jacobi_forced_at_small_shapes_matches_oracle(N, P, w, monkeypatch):
-    # the persistent-grid kernel of the wide-window regime (M > 512), forced at shapes the oracle finishes quickly:
-    # several slices per CTA, odd M (phantom column), one-eigenpair slices
-    monkeypatch.setenv("PFSM_JACOBI_WIDE", "1")
+WIDE_ROUTES = ["PFSM_TRIDIAG", "PFSM_JACOBI_WIDE"]   # tridiagonalization (default for M > 512) / persistent-grid Jacobi
+
+
+@pytest.mark.parametrize("route", WIDE_ROUTES)
+@pytest.mark.parametrize("N,P,w", [(256, 4, 16), (270, 6, 4), (600, 3, 20), (66, 64, 2), (96, 4, 100), (300, 200, 30)])
+def test_wide_window_routes_forced_at_small_shapes_match_oracle(N, P, w, route, monkeypatch):
+    # the two step-2 routes of the wide-window regime (M > 512), forced at shapes the oracle finishes quickly:
+    # several slices per CTA, odd M, one-eigenpair slices, window >= N, more slices than co-resident CTAs
+    monkeypatch.setenv(route, "1")
     p = gen.small_problem(N, 1e-3, 12.0, seed=1000 + N)
     g2 = gpu_solve(p.A, P, w, 1, p.alpha, last_step=2)
     V2, eps, info2 = oracle.step2(p.A, P, w)
     assert g2["info"] == 0 and info2 == 0
     assert np.abs(g2["eps"] - eps).max() <= 1e-13 * max(1.0, p.normF)
     assert np.abs(align_signs(g2["Vr"], V2) - V2).max() < 1e-9
-    again = gpu_solve(p.A, P, w, 1, p.alpha, last_step=2)      # fixed rotation and reduction order: same bits
+    again = gpu_solve(p.A, P, w, 1, p.alpha, last_step=2)      # fixed operation and reduction order: same bits
     assert np.array_equal(again["Vr"], g2["Vr"]) and np.array_equal(again["eps"], g2["eps"])
 
 
+@pytest.mark.parametrize("route", WIDE_ROUTES)
 @pytest.mark.parametrize("N,P,w,iters", [(1200, 2, 0, 1), (1280, 4, 200, 2), (1102, 2, 1, 1)])
-def test_wide_windows_beyond_512_match_oracle(N, P, w, iters):
+def test_wide_windows_beyond_512_match_oracle(N, P, w, iters, route, monkeypatch):
     # M = 600, 720 (gamma = 0.56) and 553 (odd); full solve against the oracle
+    if route == "PFSM_JACOBI_WIDE":
+        monkeypatch.setenv(route, "1")
     p = gen.small_problem(N, 1e-3, 24.0, seed=5000 + N + w)
     g2 = gpu_solve(p.A, P, w, iters, p.alpha, last_step=2)
     V2, eps, info2 = oracle.step2(p.A, P, w)
