@@ -542,12 +542,20 @@ static int launch_tridiag(pfsm_ctx* h, const double* A, double* V, cudaStream_t 
     PFSM_CUDA(cudaGetLastError());
     tri_invit_kernel<<<g2, TRI_THREADS, smem2, st>>>(h->N, (int32_t)M, tab, h->tri, s0);
     PFSM_CUDA(cudaGetLastError());
-    const int nvec = (int)std::max<size_t>(1, std::min<size_t>(BT_WARPS, (size_t)200 * 1024 / ((size_t)M * sizeof(double))));
-    const size_t smem3 = (size_t)nvec * M * sizeof(double);
-    PFSM_CUDA(cudaFuncSetAttribute(tri_backtransform_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem3));
-    const dim3 g3((unsigned)((h->m + nvec - 1) / nvec), (unsigned)ns);
-    tri_backtransform_kernel<<<g3, 32 * nvec, smem3, st>>>(h->N, (int32_t)M, tab, h->Gws, h->tri, V, h->eps, s0);
-    PFSM_CUDA(cudaGetLastError());
+    {
+        const int ept = (M + BT_THREADS - 1) / BT_THREADS;
+        const int nvec = ept <= 8 ? 8 : 4;
+        const dim3 g3((unsigned)((h->m + nvec - 1) / nvec), (unsigned)ns);
+#define PFSM_BT(E, NVEC) tri_backtransform_kernel<E, NVEC><<<g3, BT_THREADS, 0, st>>>(h->N, (int32_t)M, tab, h->Gws, h->tri, V, h->eps, s0)
+        if (ept <= 2) PFSM_BT(2, 8);
+        else if (ept <= 4) PFSM_BT(4, 8);
+        else if (ept <= 6) PFSM_BT(6, 8);
+        else if (ept <= 8) PFSM_BT(8, 8);
+        else if (ept <= 12) PFSM_BT(12, 4);
+        else PFSM_BT(16, 4);
+#undef PFSM_BT
+        PFSM_CUDA(cudaGetLastError());
+    }
     return 0;
 }
 

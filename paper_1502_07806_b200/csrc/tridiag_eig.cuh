@@ -11,8 +11,8 @@
 //   tri_invit_kernel        its eigenvector by inverse iteration: LU of T - lambda I with partial pivoting, three
 //                           solves from a counter-based random start, one thread per eigenvector, factors stored
 //                           [row][vector] so that a warp's accesses coalesce
-//   tri_backtransform_kernel  y = H_0 H_1 ... H_{M-3} z, one warp per eigenvector (the vector stays in shared
-//                           memory, the reflectors stream through L1/L2), written zero-padded into V
+//   tri_backtransform_kernel  y = H_0 H_1 ... H_{M-3} z, eight (four) eigenvectors per CTA held in registers, each
+//                           reflector read once per CTA, written zero-padded into V
 //
 // Eigenvalues closer than 10 eps |lambda| get shifts pushed apart as LAPACK's dstein does; there is no
 // re-orthogonalization inside clusters: step 4 orthonormalizes all N vectors anyway, and vectors of a
@@ -28,7 +28,6 @@ namespace pfsm {
 
 constexpr int TRD_THREADS = 512;
 constexpr int TRI_THREADS = 128;  // bisection / inverse iteration: threads (= eigenpairs) per CTA
-constexpr int BT_WARPS = 8;       // back-transformation: eigenvectors per CTA (fewer when 8 M-vectors exceed shared memory)
 
 struct TriWs {                  // workspace of the tridiagonal route (device pointers)
     double* d;                  // P x M   diagonal of T
@@ -64,7 +63,7 @@ __device__ __forceinline__ double block_sum_512(double v, double* red) {  // fix
 //   grid barrier.
 // Reflector k is kept in row k of the slice's matrix (columns k+1 .., leading 1 stored) once that row is dead.
 // ---------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(TRD_THREADS, 1)
+__global__ void __launch_bounds__(TRD_THREADS, 2)
 sytrd_kernel(const double* __restrict__ A, int64_t N, int32_t M, SliceTable tab, double* __restrict__ Gws, TriWs ws,
              int32_t P, int32_t s_off, int32_t ns, int32_t C, unsigned int* __restrict__ bar) {
     extern __shared__ double sm[];
@@ -153,20 +152,26 @@ sytrd_kernel(const double* __restrict__ A, int64_t N, int32_t M, SliceTable tab,
             for (int i = i0 + C * warp; i < M; i += C * NW) {
                 double* row = G + (size_t)i * M;
                 const double vi = (k > 0) ? vp[i] : 0.0, wi = (k > 0) ? wp[i] : 0.0;
-                double a0 = 0.0, a1 = 0.0;
+                double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
                 int j = k + 1 + lane;
-                for (; j + 32 < M; j += 64) {
-                    double b0 = __ldcg(row + j), b1 = __ldcg(row + j + 32);
+                for (; j + 96 < M; j += 128) {  // four independent loads per lane in flight
+                    double b0 = __ldcg(row + j), b1 = __ldcg(row + j + 32), b2 = __ldcg(row + j + 64), b3 = __ldcg(row + j + 96);
                     if (k > 0) {
                         b0 -= (__dmul_rn(vi, wp[j]) + __dmul_rn(wi, vp[j]));
                         b1 -= (__dmul_rn(vi, wp[j + 32]) + __dmul_rn(wi, vp[j + 32]));
+                        b2 -= (__dmul_rn(vi, wp[j + 64]) + __dmul_rn(wi, vp[j + 64]));
+                        b3 -= (__dmul_rn(vi, wp[j + 96]) + __dmul_rn(wi, vp[j + 96]));
                         row[j] = b0;
                         row[j + 32] = b1;
+                        row[j + 64] = b2;
+                        row[j + 96] = b3;
                     }
                     a0 = fma(b0, vn[j], a0);
                     a1 = fma(b1, vn[j + 32], a1);
+                    a2 = fma(b2, vn[j + 64], a2);
+                    a3 = fma(b3, vn[j + 96], a3);
                 }
-                if (j < M) {
+                for (; j < M; j += 32) {
                     double b0 = __ldcg(row + j);
                     if (k > 0) {
                         b0 -= (__dmul_rn(vi, wp[j]) + __dmul_rn(wi, vp[j]));
@@ -174,7 +179,7 @@ sytrd_kernel(const double* __restrict__ A, int64_t N, int32_t M, SliceTable tab,
                     }
                     a0 = fma(b0, vn[j], a0);
                 }
-                a0 = warp_sum(a0 + a1);
+                a0 = warp_sum((a0 + a1) + (a2 + a3));
                 if (lane == 0) pb[i] = tau * a0;
             }
         }
@@ -389,39 +394,89 @@ tri_invit_kernel(int64_t N, int32_t M, SliceTable tab, TriWs ws, int32_t s_off) 
 
 // ---------------------------------------------------------------------------------------------
 // y = Q z = H_0 H_1 ... H_{M-3} z,  H_k = I - tau_k v_k v_k^T, v_k in row k of the slice's matrix (columns k+1 ..).
-// One warp per eigenvector: z sits in shared memory, the reflectors are read through L1 (all warps of a CTA walk
-// the same reflectors), no block-level synchronization.  Writes V[g0 + j][lo .. lo + M) and eps[g0 + j].
-// grid.x = ceil(mmax / nvec), grid.y = ns; blockDim = 32 nvec; dynamic shared memory nvec * M doubles.
+// A CTA of 256 threads takes NV eigenvectors and keeps them in REGISTERS: thread t holds rows t + 256 e (e < EPT,
+// M <= 256 EPT) of all NV vectors.  Per reflector: v_k is read once per CTA (coalesced, prefetched one reflector
+// ahead; rows <= k read as 0 so no predicates are needed), NV dot products are reduced by shuffles and one block
+// barrier (partials double-buffered by reflector parity), then the NV axpys.  FP64 FMA issue bound; the reflectors
+// (4 M^2 bytes per slice) come from L2.  Writes V[g0 + j][lo .. lo + M) and eps[g0 + j].
+// grid.x = ceil(mmax / NV), grid.y = ns.
 // ---------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(32 * BT_WARPS)
+constexpr int BT_THREADS = 256;
+
+template <int EPT, int NV>
+__global__ void __launch_bounds__(BT_THREADS, 1)
 tri_backtransform_kernel(int64_t N, int32_t M, SliceTable tab, const double* __restrict__ Gws, TriWs ws,
                          double* __restrict__ V, double* __restrict__ eps, int32_t s_off) {
-    extern __shared__ double sm[];
-    const int s = s_off + blockIdx.y, lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nvec = blockDim.x >> 5;
-    const int t = blockIdx.x * nvec + warp;
-    if (t >= tab.cnt[s]) return;
+    __shared__ double part[2][BT_THREADS / 32][NV];
+    const int s = s_off + blockIdx.y, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int t0 = blockIdx.x * NV, cnt = tab.cnt[s];
+    if (t0 >= cnt) return;
     const int g0 = tab.g0[s], lo = tab.lo[s];
-    const size_t g = (size_t)g0 + t;
-    double* x = sm + (size_t)warp * M;
-    const double sc = ws.zscale[g];
-    const double* z = ws.f[4] + g;
-    for (int i = lane; i < M; i += 32) x[i] = z[(size_t)i * N] * sc;
-    __syncwarp();
+    const size_t g = (size_t)g0 + t0;
+    double x[NV][EPT];
+#pragma unroll
+    for (int n = 0; n < NV; ++n) {
+        const bool live = t0 + n < cnt;
+        const double sc = live ? ws.zscale[g + n] : 0.0;
+#pragma unroll
+        for (int e = 0; e < EPT; ++e) {
+            const int i = tid + BT_THREADS * e;
+            x[n][e] = (live && i < M) ? ws.f[4][(size_t)i * N + g + n] * sc : 0.0;
+        }
+    }
     const double* G = Gws + (size_t)s * M * M;
     const double* tau = ws.tau + (size_t)s * M;
-    for (int k = M - 3; k >= 0; --k) {
-        const double tk = __ldg(tau + k);
-        if (tk == 0.0) continue;
-        const double* v = G + (size_t)k * M;
-        double acc = 0.0;
-        for (int i = k + 1 + lane; i < M; i += 32) acc = fma(__ldg(v + i), x[i], acc);
-        acc = warp_sum(acc) * tk;
-        for (int i = k + 1 + lane; i < M; i += 32) x[i] = fma(-acc, __ldg(v + i), x[i]);
-        __syncwarp();
+    double vc[EPT], vx[EPT];
+    int k = M - 3;
+#pragma unroll
+    for (int e = 0; e < EPT; ++e) {
+        const int i = tid + BT_THREADS * e;
+        vc[e] = (k >= 0 && i > k && i < M) ? __ldg(G + (size_t)k * M + i) : 0.0;
     }
-    double* out = V + g * (size_t)N + lo;
-    for (int i = lane; i < M; i += 32) out[i] = x[i];
-    if (lane == 0) eps[g] = ws.lam[g];
+    for (; k >= 0; --k) {
+        const double tk = __ldg(tau + k);
+#pragma unroll
+        for (int e = 0; e < EPT; ++e) {  // next reflector (k - 1) while this one is applied
+            const int i = tid + BT_THREADS * e;
+            vx[e] = (k >= 1 && i >= k && i < M) ? __ldg(G + (size_t)(k - 1) * M + i) : 0.0;
+        }
+        double acc[NV];
+#pragma unroll
+        for (int n = 0; n < NV; ++n) {
+            double a = 0.0;
+#pragma unroll
+            for (int e = 0; e < EPT; ++e) a = fma(vc[e], x[n][e], a);
+            acc[n] = warp_sum(a);
+        }
+        double(*pb)[NV] = part[k & 1];
+        if (lane == 0) {
+#pragma unroll
+            for (int n = 0; n < NV; ++n) pb[warp][n] = acc[n];
+        }
+        __syncthreads();
+#pragma unroll
+        for (int n = 0; n < NV; ++n) {
+            double tsum = 0.0;
+#pragma unroll
+            for (int w = 0; w < BT_THREADS / 32; ++w) tsum += pb[w][n];
+            tsum *= tk;
+#pragma unroll
+            for (int e = 0; e < EPT; ++e) x[n][e] = fma(-tsum, vc[e], x[n][e]);
+        }
+#pragma unroll
+        for (int e = 0; e < EPT; ++e) vc[e] = vx[e];
+    }
+#pragma unroll
+    for (int n = 0; n < NV; ++n) {
+        if (t0 + n >= cnt) continue;
+        double* out = V + (g + n) * (size_t)N + lo;
+#pragma unroll
+        for (int e = 0; e < EPT; ++e) {
+            const int i = tid + BT_THREADS * e;
+            if (i < M) out[i] = x[n][e];
+        }
+        if (tid == 0) eps[g + n] = ws.lam[g + n];
+    }
 }
 
 }  // namespace pfsm
