@@ -343,9 +343,13 @@ def run_ours(args):
 
     # the sample is repeated until ~12 s of CPU work have been timed (at most 8 times), so a fast host still gives
     # a stable figure; the value is flops over the total time of the repeats
-    cpu_times, cpu_flops, cpu_desc, threads = oracle_sample(k, args.cpu_cols, 1, 0, min_seconds=args.cpu_seconds)
-    cpu_value = cpu_flops * len(cpu_times) / sum(cpu_times) * 1e-12
-    cpu_desc += f", repeated {len(cpu_times)}x"
+    if args.cpu_cols > 0:
+        cpu_times, cpu_flops, cpu_desc, threads = oracle_sample(k, args.cpu_cols, 1, 0, min_seconds=args.cpu_seconds)
+        cpu_value = cpu_flops * len(cpu_times) / sum(cpu_times) * 1e-12
+        cpu_desc += f", repeated {len(cpu_times)}x"
+    else:  # --cpu-cols 0: skipped (the 2048 x 2048 CPU Jacobi of config 6 alone takes minutes)
+        import oracle
+        cpu_times, cpu_value, cpu_desc, threads = [0.0], None, "skipped (--cpu-cols 0)", oracle.num_threads()
 
     line = {
         "metric": "PFSM solve sustained FP64 TFLOP/s (algorithmic flops / solve time)",
@@ -358,7 +362,8 @@ def run_ours(args):
                     "step4_cholesky_qr": step_ms[2], "step5_rayleigh": step_ms[3]},
         "algorithmic_flops": flops, "quality": quality, "clocks": clocks,
         "e2e": {"value": e2e_value, "unit": "TFLOP/s", "ms_per_step": e2e_ms,
-                "h2d_bytes_per_step": 8 * N * N + 8 * c.P * c.M * c.M,  # A, plus the P diagonal blocks sent ahead for step 2
+                # A, plus the P diagonal blocks sent ahead for the shared-memory Jacobi of step 2 (M <= 480)
+                "h2d_bytes_per_step": 8 * N * N + (8 * c.P * c.M * c.M if c.M <= 480 else 0),
                 "d2h_bytes_per_step": 8 * N * N + 8 * N},
         "gpu_launches": int(args.steps * h.launches_per_solve()),
         "roofline": roofline,
@@ -377,9 +382,9 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=4, help="BASELINE.json config index (default 4: N=8192); 5 = Cu256-shaped N=1664 extra case")
+    ap.add_argument("--config", type=int, default=4, help="BASELINE.json config index (default 4: N=8192); extra cases: 5 = Cu256-shaped N=1664, 6 = config 4 shape at gamma = 0.25 (M = 2048)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--cpu-cols", type=int, default=128, help="eigenvectors in the cpu_baseline sample")
+    ap.add_argument("--cpu-cols", type=int, default=128, help="eigenvectors in the cpu_baseline sample (0 = skip the CPU leg)")
     ap.add_argument("--cpu-seconds", type=float, default=12.0, help="repeat the cpu_baseline sample until this much CPU time is timed (max 8 repeats)")
     ap.add_argument("--ref-cols", type=int, default=8, help="eigenvectors per step of --impl reference")
     ap.add_argument("--sharded", action="store_true",

@@ -83,6 +83,7 @@ struct pfsm_ctx {
     bool jac_wide = false;             // wide-window Jacobi (jacobi_wide.cuh): PFSM_JACOBI_WIDE=1, at any M
     bool tridiag = false;              // tridiagonalization route (tridiag_eig.cuh): default for M > 512, PFSM_TRIDIAG=1 at any M
     TriWs tri{};                       // its workspace
+    bool sytrd_full = false, sytrd_half = false;  // PFSM_SYTRD_FULL=1 / PFSM_SYTRD_HALF=1: force one of the two tridiagonalization kernels
     int jac_cs = 0, jac_hloc = 0;  // cluster size / seats per CTA of the shared-memory Jacobi (0 = L2 kernel)
     double* gdiag = nullptr;  // N: diag(V^T V) before the factorization (breakdown threshold)
     int32_t* slice_tab = nullptr;  // g0[P], lo[P], off[P], cnt[P]
@@ -222,6 +223,11 @@ int pfsm_create(pfsm_handle_t* out, int64_t N, int32_t P, int32_t window, int32_
         TRY(dev_alloc(h, (void**)&h->tri.tau, pm));
         TRY(dev_alloc(h, (void**)&h->tri.pbuf, 2 * pm));
         TRY(dev_alloc(h, (void**)&h->tri.vbuf, 2 * pm));
+        TRY(dev_alloc(h, (void**)&h->tri.rowbuf, pm * ((M + 31) / 32)));
+        TRY(dev_alloc(h, (void**)&h->tri.colbuf, pm * ((M + 31) / 32)));
+        TRY(dev_alloc(h, (void**)&h->tri.colk, 2 * pm));
+        h->sytrd_full = getenv("PFSM_SYTRD_FULL") != nullptr;  // diagnostic: force full-storage tridiagonalization
+        h->sytrd_half = getenv("PFSM_SYTRD_HALF") != nullptr;  // diagnostic: force lower-triangle tridiagonalization
         TRY(dev_alloc(h, (void**)&h->tri.lam, N * sizeof(double)));
         TRY(dev_alloc(h, (void**)&h->tri.zscale, N * sizeof(double)));
         for (int i = 0; i < 5; ++i) TRY(dev_alloc(h, (void**)&h->tri.f[i], mn * sizeof(double)));
@@ -293,7 +299,7 @@ int pfsm_destroy(pfsm_handle_t h) {
     cudaDeviceSynchronize();
     void* ptrs[] = {h->W, h->S, h->O, h->Dinv, h->Gws, h->eps, h->resid, h->gdiag, h->rotcnt, h->nrm_g, h->jw_bar, h->slice_tab, h->krange, h->info, h->chain_cnt,
                     h->A_stage, h->V_stage, h->lam_stage, h->Ap, h->LT, h->DinvT,
-                    h->tri.d, h->tri.e, h->tri.tau, h->tri.pbuf, h->tri.vbuf, h->tri.lam, h->tri.zscale,
+                    h->tri.d, h->tri.e, h->tri.tau, h->tri.pbuf, h->tri.vbuf, h->tri.rowbuf, h->tri.colbuf, h->tri.colk, h->tri.lam, h->tri.zscale,
                     h->tri.f[0], h->tri.f[1], h->tri.f[2], h->tri.f[3], h->tri.f[4], h->tri.piv};
     for (void* p : ptrs)
         if (p) cudaFree(p);
@@ -512,9 +518,16 @@ static int launch_tridiag(pfsm_ctx* h, const double* A, double* V, cudaStream_t 
     PFSM_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, h->device));
     {
         const size_t smem = 3 * (size_t)M * sizeof(double);
-        PFSM_CUDA(cudaFuncSetAttribute(sytrd_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        // Lower-triangle storage halves the HBM traffic but pays a second grid barrier and a partial-sum pass per
+        // column: it wins once the batch of submatrices no longer fits L2 (M = 2048 x 16: 147 -> 104 ms; M = 1024 x 4,
+        // L2 resident: 11 -> 17 ms, so full storage is kept there)
+        int l2 = 0;
+        PFSM_CUDA(cudaDeviceGetAttribute(&l2, cudaDevAttrL2CacheSize, h->device));
+        const bool half = !h->sytrd_full && (h->sytrd_half || (size_t)ns * M * M * sizeof(double) > (size_t)l2);
+        auto kern = half ? sytrd_half_kernel : sytrd_kernel;
+        PFSM_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         int per_sm = 0;
-        PFSM_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, sytrd_kernel, TRD_THREADS, smem));
+        PFSM_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, TRD_THREADS, smem));
         if (per_sm < 1) return PFSM_CUDA_ERROR_BASE + (int)cudaErrorLaunchOutOfResources;
         const int cap = per_sm * sms;
         int C = std::max(1, std::min(cap / ns, (M + 15) / 16));  // CTAs per slice; a CTA keeps >= 16 rows while rows last
@@ -531,7 +544,7 @@ static int launch_tridiag(pfsm_ctx* h, const double* A, double* V, cudaStream_t 
         attr[0].val.cooperative = 1;
         cfg.attrs = attr;
         cfg.numAttrs = 1;
-        PFSM_CUDA(cudaLaunchKernelEx(&cfg, sytrd_kernel, A, h->N, (int32_t)M, tab, h->Gws, h->tri, h->P, s0, ns, (int32_t)C,
+        PFSM_CUDA(cudaLaunchKernelEx(&cfg, kern, A, h->N, (int32_t)M, tab, h->Gws, h->tri, h->P, s0, ns, (int32_t)C,
                                      h->jw_bar));
     }
     const size_t smem2 = 2 * (size_t)M * sizeof(double);
@@ -1273,7 +1286,8 @@ int64_t pfsm_launches_per_solve(pfsm_handle_t h) {
             if (cn0 >= h->N) continue;
             trailing += (h->lookahead && npairs >= 3 && cn1 < h->N) ? 2 : 1;
         }
-        return 1 + 2 * (int64_t)h->iters + h->cholqr_passes * (2 + 1 + 1 + 2 * nb + pairs + trailing) + 2;
+        const int64_t step2 = h->tridiag ? 4 : 1;  // tridiagonal route: sytrd, bisection, inverse iteration, back-transformation
+        return step2 + 2 * (int64_t)h->iters + h->cholqr_passes * (2 + 1 + 1 + 2 * nb + pairs + trailing) + 2;
     }
 }
 

@@ -35,6 +35,9 @@ struct TriWs {                  // workspace of the tridiagonal route (device po
     double* tau;                // P x M   Householder scalars
     double* pbuf;               // 2 x P x M   matrix-vector products, double-buffered by column parity
     double* vbuf;               // 2 x P x M   current Householder vector, double-buffered
+    double* rowbuf;             // P x ceil(M/32) x M   row-part partial sums of the half-storage product
+    double* colbuf;             // P x ceil(M/32) x M   column-part partial sums
+    double* colk;               // 2 x P x M   column k+1 of the trailing matrix, written by the pass of column k
     double* lam;                // N       eigenvalues (unperturbed)
     double* zscale;             // N       1 / ||z|| of the inverse-iteration vector
     double* f[5];               // 5 x (M x N): U diagonal reciprocal, U super-diagonals 1 and 2, L multipliers, z
@@ -186,6 +189,191 @@ sytrd_kernel(const double* __restrict__ A, int64_t N, int32_t M, SliceTable tab,
         jw_grid_barrier(bar, phase);
     }
     // last diagonal entry (its pending update was applied by the pass of column M-2)
+    for (int vb = blockIdx.x; vb < nv; vb += gridDim.x) {
+        const int sl = vb / C, c = vb - sl * C, s = s_off + sl;
+        if (c == 0 && tid == 0) {
+            ws.d[(size_t)s * M + M - 1] = __ldcg(Gws + (size_t)s * M * M + (size_t)(M - 1) * M + M - 1);
+            ws.e[(size_t)s * M + M - 1] = 0.0;
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// The same recurrence on the LOWER TRIANGLE only (entries j <= i): half the memory traffic, 8 (M-k)^2 bytes per column.
+// The product p = B v needs, for row i, the row part sum_{j<=i} B[i][j] v[j] and the column part sum_{r>i} B[r][i] v[r].
+// The active triangle is cut into 32 x 32 tiles (row block Rb, column strip S <= Rb), dealt cyclically to the warps of
+// the slice's CTAs.  A warp walks the 32 rows of its tile with lane = column: the column part accumulates in a register,
+// the row part is a shuffle reduction per row.  Tiles write their partial sums to rowbuf[S][i] and colbuf[Rb][j] (each
+// entry written by exactly one warp), a grid barrier follows, then p[i] = tau (sum_S rowbuf[S][i] + sum_Rb colbuf[Rb][i])
+// is summed in fixed order by the CTA that owns a contiguous range of rows, and a second grid barrier publishes p.
+// No atomics: bitwise reproducible.  Column k itself (B[i][k], i > k) is read with stride M in the prologue.
+// Reflector k goes to the (unused) upper part of row k: columns k+1 .., leading 1 stored.
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(TRD_THREADS, 1)
+sytrd_half_kernel(const double* __restrict__ A, int64_t N, int32_t M, SliceTable tab, double* __restrict__ Gws, TriWs ws,
+                  int32_t P, int32_t s_off, int32_t ns, int32_t C, unsigned int* __restrict__ bar) {
+    extern __shared__ double sm[];
+    double* vp = sm;          // v_{k-1}
+    double* wp = sm + M;      // w_{k-1}
+    double* vn = sm + 2 * M;  // v_k
+    __shared__ double red[TRD_THREADS / 32];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    constexpr int NW = TRD_THREADS / 32;
+    unsigned int phase = 0;
+    const int nv = ns * C;
+    const int nb = (M + 31) / 32;
+    const size_t bufs = (size_t)nb * M;  // rowbuf / colbuf doubles per slice
+
+    for (int vb = blockIdx.x; vb < nv; vb += gridDim.x) {
+        const int sl = vb / C, c = vb - sl * C, s = s_off + sl;
+        const int lo = tab.lo[s];
+        double* G = Gws + (size_t)s * M * M;
+        for (int i = c + C * warp; i < M; i += C * NW) {
+            const double* a = A + (size_t)(lo + i) * N + lo;
+            for (int j = lane; j <= i; j += 32) G[(size_t)i * M + j] = a[j];
+        }
+    }
+    jw_grid_barrier(bar, phase);
+
+    for (int k = 0; k <= M - 2; ++k) {
+        const int b0 = (k + 1) / 32, nbk = nb - b0, ntiles = nbk * (nbk + 1) / 2;
+        for (int vb = blockIdx.x; vb < nv; vb += gridDim.x) {
+            const int sl = vb / C, c = vb - sl * C, s = s_off + sl;
+            double* G = Gws + (size_t)s * M * M;
+            const size_t so = (size_t)s * M;
+            __syncthreads();
+            // ---- prologue (as in sytrd_kernel; column k is read down the column)
+            if (k > 0) {
+                const double tau_p = __ldcg(ws.tau + so + k - 1);
+                const double* pv_ = ws.pbuf + (size_t)((k - 1) & 1) * P * M + so;
+                const double* vv_ = ws.vbuf + (size_t)((k - 1) & 1) * P * M + so;
+                double acc = 0.0;
+                for (int i = k + tid; i < M; i += TRD_THREADS) {
+                    const double v = __ldcg(vv_ + i), p = __ldcg(pv_ + i);
+                    vp[i] = v;
+                    wp[i] = p;
+                    acc = fma(p, v, acc);
+                }
+                const double pv = block_sum_512(acc, red);
+                const double hf = 0.5 * tau_p * pv;
+                for (int i = k + tid; i < M; i += TRD_THREADS) wp[i] = fma(-hf, vp[i], wp[i]);
+                __syncthreads();
+            }
+            double acc = 0.0;
+            {
+                const double wk = (k > 0) ? wp[k] : 0.0, vk = (k > 0) ? vp[k] : 0.0;
+                for (int i = k + tid; i < M; i += TRD_THREADS) {
+                    // column k: written contiguously by the previous pass (k = 0: down the column of the copy)
+                    double b = (k > 0) ? __ldcg(ws.colk + (size_t)((k - 1) & 1) * P * M + so + i) : __ldcg(G + (size_t)i * M);
+                    if (k > 0) b -= (__dmul_rn(vp[i], wk) + __dmul_rn(wp[i], vk));
+                    vn[i] = b;
+                    if (i >= k + 2) acc = fma(b, b, acc);
+                }
+            }
+            const double xn2 = block_sum_512(acc, red);
+            const double dk = vn[k], alpha = vn[k + 1];
+            double tau = 0.0, beta = alpha, scal = 0.0;
+            if (xn2 > 0.0) {
+                beta = -copysign(sqrt(fma(alpha, alpha, xn2)), alpha);
+                tau = (beta - alpha) / beta;
+                scal = 1.0 / (alpha - beta);
+            }
+            __syncthreads();
+            for (int i = k + 1 + tid; i < M; i += TRD_THREADS) vn[i] = (i == k + 1) ? 1.0 : vn[i] * scal;
+            __syncthreads();
+            if (c == 0) {
+                double* vb_ = ws.vbuf + (size_t)(k & 1) * P * M + so;
+                for (int i = k + 1 + tid; i < M; i += TRD_THREADS) {
+                    vb_[i] = vn[i];
+                    G[(size_t)k * M + i] = vn[i];  // reflector k: upper part of row k, never touched by the recurrence
+                }
+                if (tid == 0) {
+                    ws.d[so + k] = dk;
+                    ws.e[so + k] = beta;
+                    ws.tau[so + k] = tau;
+                }
+            }
+            // ---- pass over the tiles of the active lower triangle
+            double* rowbuf = ws.rowbuf + (size_t)s * bufs;
+            double* colbuf = ws.colbuf + (size_t)s * bufs;
+            double* nextcol = ws.colk + (size_t)(k & 1) * P * M + so;
+            for (int t = c * NW + warp; t < ntiles; t += C * NW) {
+                int rb = (int)((sqrt(8.0 * (double)t + 1.0) - 1.0) * 0.5);
+                while ((rb + 1) * (rb + 2) / 2 <= t) ++rb;
+                while (rb * (rb + 1) / 2 > t) --rb;
+                const int S = b0 + (t - rb * (rb + 1) / 2), Rb = b0 + rb;
+                const int j = 32 * S + lane, ib = 32 * Rb;
+                const bool jok = j >= k + 1 && j < M;
+                const double wj = (jok && k > 0) ? wp[j] : 0.0, vj = (jok && k > 0) ? vp[j] : 0.0, vnj = jok ? vn[j] : 0.0;
+                double colacc = 0.0;
+                double b[32];
+#pragma unroll
+                for (int r = 0; r < 32; ++r) {  // the whole tile column of this lane in flight at once
+                    const int i = ib + r;
+                    b[r] = (jok && i < M && j <= i) ? __ldcg(G + (size_t)i * M + j) : 0.0;
+                }
+#pragma unroll
+                for (int r = 0; r < 32; ++r) {
+                    const int i = ib + r;
+                    const bool ok = jok && i < M && j <= i;  // (i >= k+1 follows from j >= k+1)
+                    double bb = b[r];
+                    if (k > 0 && ok) {
+                        bb -= (__dmul_rn(vp[i], wj) + __dmul_rn(wp[i], vj));
+                        G[(size_t)i * M + j] = bb;
+                    }
+                    if (ok && j == k + 1) nextcol[i] = bb;  // column k+1 for the next prologue (update k still pending)
+                    if (ok && j < i) colacc = fma(bb, vn[i], colacc);
+                    b[r] = bb * vnj;
+                }
+                // row sums: transposed butterfly, 31 shuffles; lane l ends with the sum of row ib + l over the 32 columns
+#pragma unroll
+                for (int h = 16; h >= 1; h >>= 1) {
+                    const bool up = (lane & h) != 0;
+#pragma unroll
+                    for (int r = 0; r < h; ++r) {
+                        const double send = up ? b[r] : b[r + h], keep = up ? b[r + h] : b[r];
+                        b[r] = keep + __shfl_xor_sync(0xffffffffu, send, h);
+                    }
+                }
+                const double myrow = b[0];
+                const int i = ib + lane;
+                if (i >= k + 1 && i < M) rowbuf[(size_t)S * M + i] = myrow;
+                if (j < M) colbuf[(size_t)Rb * M + j] = colacc;
+            }
+        }
+        jw_grid_barrier(bar, phase);
+        // ---- p = tau (row parts + column parts), contiguous row ranges per CTA, thread per row, fixed order
+        for (int vb = blockIdx.x; vb < nv; vb += gridDim.x) {
+            const int sl = vb / C, c = vb - sl * C, s = s_off + sl;
+            const size_t so = (size_t)s * M;
+            const double tau = __ldcg(ws.tau + so + k);
+            const double* rowbuf = ws.rowbuf + (size_t)s * bufs;
+            const double* colbuf = ws.colbuf + (size_t)s * bufs;
+            double* pb = ws.pbuf + (size_t)(k & 1) * P * M + so;
+            const int L = M - k - 1, per = (L + C - 1) / C;
+            const int i0 = k + 1 + c * per, i1 = min(M, i0 + per);
+            for (int i = i0 + tid; i < i1; i += TRD_THREADS) {
+                double a = 0.0;
+                const int bi = i / 32;
+                // terms in fixed order: strips b0 .. bi of rowbuf, then row blocks bi .. nb-1 of colbuf (8 loads in flight)
+                const int n1 = bi - b0 + 1, nt = n1 + nb - bi;
+                for (int q0 = 0; q0 < nt; q0 += 8) {
+                    double x[8];
+#pragma unroll
+                    for (int u = 0; u < 8; ++u) {
+                        const int q = q0 + u;
+                        x[u] = (q >= nt) ? 0.0
+                               : (q < n1) ? __ldcg(rowbuf + (size_t)(b0 + q) * M + i)
+                                          : __ldcg(colbuf + (size_t)(bi + q - n1) * M + i);
+                    }
+#pragma unroll
+                    for (int u = 0; u < 8; ++u) a += x[u];
+                }
+                pb[i] = tau * a;
+            }
+        }
+        jw_grid_barrier(bar, phase);
+    }
     for (int vb = blockIdx.x; vb < nv; vb += gridDim.x) {
         const int sl = vb / C, c = vb - sl * C, s = s_off + sl;
         if (c == 0 && tid == 0) {

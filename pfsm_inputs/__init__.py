@@ -114,11 +114,14 @@ CONFIGS = [
 # (PAPER.md:100-108): m = 128, window 144, M = 416.
 EXTRA_CONFIGS = [
     Config(5, "transition metal with unoccupied states (Cu256 shape, Table I), gamma = 0.25", 1664, 13, 144, 3, 2e-3, 64.0),
+    # config 4's workload (Al4000 shape, Table III) at the paper's recommended width gamma = M / N = 0.25
+    # ("M <= 3000"): m = 512, window 768, M = 2048 -- the wide-window route of step 2
+    Config(6, "metal, dense spectrum (Al4000 shape), gamma = 0.25", 8192, 16, 768, 3, 2e-3, 128.0),
 ]
 
 
 def config(k: int) -> Config:
-    """BASELINE.json config k (0-4) or an extra one (5)."""
+    """BASELINE.json config k (0-4) or an extra one (5, 6)."""
     return CONFIGS[k] if k < len(CONFIGS) else EXTRA_CONFIGS[k - len(CONFIGS)]
 
 
@@ -142,7 +145,7 @@ def spectrum(k: int) -> np.ndarray:
         u = uniform(s, STREAM_D, 432, 8640)
         unocc = (0.125 + 7.875 * u) ** (2.0 / 3.0)  # density ~ sqrt(E) on [0.25, 4]
         d = np.concatenate([occ, unocc])
-    elif k == 4:
+    elif k == 4 or k == 6:
         u = uniform(s, STREAM_D, 0, N)
         d = -1.0 + 4.0 * u ** (2.0 / 3.0)  # density ~ sqrt(E + 1) on [-1, 3]
     elif k == 5:

@@ -120,7 +120,9 @@ def test_l2_resident_jacobi_fallback_matches_oracle(N, P, w, monkeypatch):
     assert np.abs(align_signs(g2["Vr"], V2) - V2).max() < 1e-9
 
 
-WIDE_ROUTES = ["PFSM_TRIDIAG", "PFSM_JACOBI_WIDE"]   # tridiagonalization (default for M > 512) / persistent-grid Jacobi
+# step-2 routes of the wide-window regime: tridiagonalization (default for M > 512) with full symmetric storage (batch
+# fits L2) or lower-triangle storage (batch larger than L2), and the persistent-grid Jacobi
+WIDE_ROUTES = [("PFSM_TRIDIAG",), ("PFSM_TRIDIAG", "PFSM_SYTRD_HALF"), ("PFSM_JACOBI_WIDE",)]
 
 
 @pytest.mark.parametrize("route", WIDE_ROUTES)
@@ -128,7 +130,8 @@ WIDE_ROUTES = ["PFSM_TRIDIAG", "PFSM_JACOBI_WIDE"]   # tridiagonalization (defau
 def test_wide_window_routes_forced_at_small_shapes_match_oracle(N, P, w, route, monkeypatch):
     # the two step-2 routes of the wide-window regime (M > 512), forced at shapes the oracle finishes quickly:
     # several slices per CTA, odd M, one-eigenpair slices, window >= N, more slices than co-resident CTAs
-    monkeypatch.setenv(route, "1")
+    for name in route:
+        monkeypatch.setenv(name, "1")
     p = gen.small_problem(N, 1e-3, 12.0, seed=1000 + N)
     g2 = gpu_solve(p.A, P, w, 1, p.alpha, last_step=2)
     V2, eps, info2 = oracle.step2(p.A, P, w)
@@ -143,8 +146,9 @@ def test_wide_window_routes_forced_at_small_shapes_match_oracle(N, P, w, route, 
 @pytest.mark.parametrize("N,P,w,iters", [(1200, 2, 0, 1), (1280, 4, 200, 2), (1102, 2, 1, 1)])
 def test_wide_windows_beyond_512_match_oracle(N, P, w, iters, route, monkeypatch):
     # M = 600, 720 (gamma = 0.56) and 553 (odd); full solve against the oracle
-    if route == "PFSM_JACOBI_WIDE":
-        monkeypatch.setenv(route, "1")
+    for name in route:
+        if name != "PFSM_TRIDIAG":                      # the tridiagonal route is the default beyond M = 512
+            monkeypatch.setenv(name, "1")
     p = gen.small_problem(N, 1e-3, 24.0, seed=5000 + N + w)
     g2 = gpu_solve(p.A, P, w, iters, p.alpha, last_step=2)
     V2, eps, info2 = oracle.step2(p.A, P, w)
@@ -154,6 +158,31 @@ def test_wide_windows_beyond_512_match_oracle(N, P, w, iters, route, monkeypatch
     g = gpu_solve(p.A, P, w, iters, p.alpha)
     o = oracle.pfsm(p.A, P, w, iters, p.alpha)
     check_gates(p.A, g, o)
+
+
+@pytest.mark.parametrize("route", WIDE_ROUTES)
+def test_wide_window_routes_on_doubly_degenerate_spectrum(route, monkeypatch):
+    # A = blockdiag(B, B): every eigenvalue is exactly double.  The eigenvectors of a pair are not unique, so only
+    # rotation-invariant quantities are compared (reading R16); the tridiagonal route has no re-orthogonalization
+    # inside clusters (reading R25) and must still hand step 4 independent vectors (info = 0)
+    for name in route:
+        monkeypatch.setenv(name, "1")
+    n = 96
+    B = gen.small_problem(n, 5e-2, 8.0, seed=4242).A
+    A = np.zeros((2 * n, 2 * n))
+    A[:n, :n] = B
+    A[n:, n:] = B
+    ex = np.linalg.eigvalsh(A)
+    alpha = 0.5 / np.abs(ex).max() ** 2
+    for P, w in [(1, 0), (2, 2 * n)]:                   # M = N: every slice sees the whole (degenerate) spectrum
+        g2 = gpu_solve(A, P, w, 2, alpha, last_step=2)
+        assert g2["info"] == 0
+        assert np.abs(g2["eps"] - ex).max() < 1e-13 * np.linalg.norm(A)
+        g = gpu_solve(A, P, w, 2, alpha)
+        assert g["info"] == 0
+        assert np.abs(g["lam"] - ex).max() < 1e-12 * np.linalg.norm(A)
+        assert np.abs(g["Vr"] @ g["Vr"].T - np.eye(2 * n)).max() <= 1e-12 * 2 * n
+        assert g["resid"].max() < 1e-11 * np.linalg.norm(A)
 
 
 def test_iters_zero_is_gram_schmidt_of_start_vectors():
