@@ -433,7 +433,13 @@ static void choose_jacobi_layout(pfsm_ctx* h) {
     h->jac_cs = 0;
     h->jac_hloc = 0;
     h->jac_wide = getenv("PFSM_JACOBI_WIDE") != nullptr;  // diagnostic: the wide-window Jacobi kernel at any M
-    h->tridiag = !h->jac_wide && (h->M > 512 || getenv("PFSM_TRIDIAG") != nullptr);  // default for wide windows
+    // Route of step 2.  Tridiagonalization + bisection + inverse iteration + back-transformation costs ~M latency-bound
+    // columns; the Jacobi kernels cost sweeps x (M - 1) rounds.  Measured (step 2, Jacobi -> tridiagonal): M = 96 x 4
+    // slices 0.60 -> 1.14 ms, M = 192 x 16 2.66 -> 2.59, M = 224 x 24 4.57 -> 3.30, M = 254 x 72 13.5 -> 5.8, M = 256 x 64
+    // 12.5 -> 5.3, M = 416 x 13 15.2 -> 6.1 ms.  So: Jacobi up to M = 200, the tridiagonal route above.
+    // PFSM_JACOBI=1 / PFSM_TRIDIAG=1 force one family (M > 512 has no shared-memory / L2 Jacobi: PFSM_JACOBI_WIDE).
+    const bool want_jacobi = getenv("PFSM_JACOBI") != nullptr && h->M <= 512;
+    h->tridiag = !h->jac_wide && !want_jacobi && (h->M > 200 || getenv("PFSM_TRIDIAG") != nullptr);
     if (h->M > 512 || h->jac_wide || h->tridiag) return;
     if (getenv("PFSM_JACOBI_L2")) return;  // diagnostic: force the L2-resident kernel (the large-M fallback)
     const size_t budget = 220 * 1024;
@@ -524,15 +530,40 @@ static int launch_tridiag(pfsm_ctx* h, const double* A, double* V, cudaStream_t 
         int l2 = 0;
         PFSM_CUDA(cudaDeviceGetAttribute(&l2, cudaDevAttrL2CacheSize, h->device));
         const bool half = !h->sytrd_full && (h->sytrd_half || (size_t)ns * M * M * sizeof(double) > (size_t)l2);
-        auto kern = half ? sytrd_half_kernel : sytrd_kernel;
+        // Small submatrices (a column is latency bound): the CTAs of a slice form a cluster and use its barrier
+        bool cluster = !half && M <= 768 && !getenv("PFSM_SYTRD_GRID");
+        int ccl = 1;  // cluster size: the largest of 8, 4, 2 that keeps all ns clusters co-resident (one wave)
+        if (cluster) {
+            PFSM_CUDA(cudaFuncSetAttribute(sytrd_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            cluster = false;
+            for (int c2 = 8; c2 >= 2 && !cluster; c2 /= 2) {
+                if (c2 * 16 > M + 15) continue;
+                cudaLaunchConfig_t q;
+                memset(&q, 0, sizeof(q));
+                q.gridDim = dim3((unsigned)(ns * c2));
+                q.blockDim = dim3(TRD_THREADS);
+                q.dynamicSmemBytes = smem;
+                cudaLaunchAttribute qa[1];
+                qa[0].id = cudaLaunchAttributeClusterDimension;
+                qa[0].val.clusterDim.x = (unsigned)c2;
+                qa[0].val.clusterDim.y = 1;
+                qa[0].val.clusterDim.z = 1;
+                q.attrs = qa;
+                q.numAttrs = 1;
+                int nmax = 0;
+                if (cudaOccupancyMaxActiveClusters(&nmax, sytrd_kernel<true>, &q) != cudaSuccess) { (void)cudaGetLastError(); break; }
+                if (nmax >= ns) { cluster = true; ccl = c2; }
+            }
+        }
+        auto kern = half ? sytrd_half_kernel : (cluster ? sytrd_kernel<true> : sytrd_kernel<false>);
         PFSM_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         int per_sm = 0;
         PFSM_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, TRD_THREADS, smem));
         if (per_sm < 1) return PFSM_CUDA_ERROR_BASE + (int)cudaErrorLaunchOutOfResources;
         const int cap = per_sm * sms;
         int C = std::max(1, std::min(cap / ns, (M + 15) / 16));  // CTAs per slice; a CTA keeps >= 16 rows while rows last
-        const int grid = std::min(cap, ns * C);
-        PFSM_CUDA(cudaMemsetAsync(h->jw_bar, 0, sizeof(unsigned int), st));
+        if (cluster) C = ccl;
+        const int grid = cluster ? ns * C : std::min(cap, ns * C);
         cudaLaunchConfig_t cfg;
         memset(&cfg, 0, sizeof(cfg));
         cfg.gridDim = dim3((unsigned)grid);
@@ -540,8 +571,16 @@ static int launch_tridiag(pfsm_ctx* h, const double* A, double* V, cudaStream_t 
         cfg.dynamicSmemBytes = smem;
         cfg.stream = st;
         cudaLaunchAttribute attr[1];
-        attr[0].id = cudaLaunchAttributeCooperative;  // all CTAs co-resident: the grid barrier cannot deadlock
-        attr[0].val.cooperative = 1;
+        if (cluster) {
+            attr[0].id = cudaLaunchAttributeClusterDimension;
+            attr[0].val.clusterDim.x = (unsigned)C;
+            attr[0].val.clusterDim.y = 1;
+            attr[0].val.clusterDim.z = 1;
+        } else {
+            PFSM_CUDA(cudaMemsetAsync(h->jw_bar, 0, sizeof(unsigned int), st));
+            attr[0].id = cudaLaunchAttributeCooperative;  // all CTAs co-resident: the grid barrier cannot deadlock
+            attr[0].val.cooperative = 1;
+        }
         cfg.attrs = attr;
         cfg.numAttrs = 1;
         PFSM_CUDA(cudaLaunchKernelEx(&cfg, kern, A, h->N, (int32_t)M, tab, h->Gws, h->tri, h->P, s0, ns, (int32_t)C,
@@ -560,7 +599,8 @@ static int launch_tridiag(pfsm_ctx* h, const double* A, double* V, cudaStream_t 
         const int nvec = ept <= 8 ? 8 : 4;
         const dim3 g3((unsigned)((h->m + nvec - 1) / nvec), (unsigned)ns);
 #define PFSM_BT(E, NVEC) tri_backtransform_kernel<E, NVEC><<<g3, BT_THREADS, 0, st>>>(h->N, (int32_t)M, tab, h->Gws, h->tri, V, h->eps, s0)
-        if (ept <= 2) PFSM_BT(2, 8);
+        if (ept <= 1) PFSM_BT(1, 8);
+        else if (ept <= 2) PFSM_BT(2, 8);
         else if (ept <= 4) PFSM_BT(4, 8);
         else if (ept <= 6) PFSM_BT(6, 8);
         else if (ept <= 8) PFSM_BT(8, 8);

@@ -66,6 +66,10 @@ __device__ __forceinline__ double block_sum_512(double v, double* red) {  // fix
 //   grid barrier.
 // Reflector k is kept in row k of the slice's matrix (columns k+1 .., leading 1 stored) once that row is dead.
 // ---------------------------------------------------------------------------------------------
+// CLUSTER: the C CTAs of a slice form one thread-block cluster (grid = ns * C, no cooperative launch) and synchronize
+// with the hardware cluster barrier instead of the grid-wide counter -- slices are independent, and for the small
+// submatrices of the BASELINE configs a column is latency bound (M = 256, P = 64: 13.7 -> ~5 us per column).
+template <bool CLUSTER>
 __global__ void __launch_bounds__(TRD_THREADS, 2)
 sytrd_kernel(const double* __restrict__ A, int64_t N, int32_t M, SliceTable tab, double* __restrict__ Gws, TriWs ws,
              int32_t P, int32_t s_off, int32_t ns, int32_t C, unsigned int* __restrict__ bar) {
@@ -89,7 +93,7 @@ sytrd_kernel(const double* __restrict__ A, int64_t N, int32_t M, SliceTable tab,
             for (int j = lane; j < M; j += 32) G[(size_t)i * M + j] = a[j];
         }
     }
-    jw_grid_barrier(bar, phase);
+    if (CLUSTER) cluster_sync_all(); else jw_grid_barrier(bar, phase);
 
     for (int k = 0; k <= M - 2; ++k) {
         for (int vb = blockIdx.x; vb < nv; vb += gridDim.x) {
@@ -97,7 +101,13 @@ sytrd_kernel(const double* __restrict__ A, int64_t N, int32_t M, SliceTable tab,
             double* G = Gws + (size_t)s * M * M;
             const size_t so = (size_t)s * M;
             __syncthreads();  // shared vectors of the previous virtual CTA are no longer read
-            // ---- prologue
+            // ---- prologue (row k is requested first so that its latency overlaps the p / v loads)
+            double bk[8];  // M <= 4096 = 8 x 512
+#pragma unroll
+            for (int e = 0; e < 8; ++e) {
+                const int i = k + tid + TRD_THREADS * e;
+                bk[e] = (i < M) ? __ldcg(G + (size_t)k * M + i) : 0.0;
+            }
             double tau_p = 0.0;
             if (k > 0) {
                 tau_p = __ldcg(ws.tau + so + k - 1);
@@ -120,11 +130,15 @@ sytrd_kernel(const double* __restrict__ A, int64_t N, int32_t M, SliceTable tab,
             double acc = 0.0, alpha = 0.0, dk = 0.0;
             {
                 const double wk = (k > 0) ? wp[k] : 0.0, vk = (k > 0) ? vp[k] : 0.0;
-                for (int i = k + tid; i < M; i += TRD_THREADS) {
-                    double b = __ldcg(G + (size_t)k * M + i);
-                    if (k > 0) b -= (__dmul_rn(vp[i], wk) + __dmul_rn(wp[i], vk));
-                    vn[i] = b;
-                    if (i >= k + 2) acc = fma(b, b, acc);
+#pragma unroll
+                for (int e = 0; e < 8; ++e) {
+                    const int i = k + tid + TRD_THREADS * e;
+                    if (i < M) {
+                        double b = bk[e];
+                        if (k > 0) b -= (__dmul_rn(vp[i], wk) + __dmul_rn(wp[i], vk));
+                        vn[i] = b;
+                        if (i >= k + 2) acc = fma(b, b, acc);
+                    }
                 }
             }
             const double xn2 = block_sum_512(acc, red);  // (its barriers also publish vn)
@@ -186,7 +200,7 @@ sytrd_kernel(const double* __restrict__ A, int64_t N, int32_t M, SliceTable tab,
                 if (lane == 0) pb[i] = tau * a0;
             }
         }
-        jw_grid_barrier(bar, phase);
+        if (CLUSTER) cluster_sync_all(); else jw_grid_barrier(bar, phase);
     }
     // last diagonal entry (its pending update was applied by the pass of column M-2)
     for (int vb = blockIdx.x; vb < nv; vb += gridDim.x) {
@@ -384,8 +398,8 @@ sytrd_half_kernel(const double* __restrict__ A, int64_t N, int32_t M, SliceTable
 }
 
 // ---------------------------------------------------------------------------------------------
-// Eigenvalue of local rank off + t of T_s by bisection.  count(x) = number of eigenvalues < x = number of negative
-// pivots of the LDL^T recurrence q_i = d_i - x - e_{i-1}^2 / q_{i-1}  (Sturm sequence; |q| < pivmin -> -pivmin).
+// Eigenvalue of local rank off + t of T_s by bisection.  count(x) = number of eigenvalues < x = number of sign changes
+// of the Sturm sequence p_i = (d_i - x) p_{i-1} - e_{i-1}^2 p_{i-2}, p_{-1} = 1 (= negative pivots of LDL^T).
 // grid.x = ceil(mmax / TRI_THREADS), grid.y = ns.  Dynamic shared memory: d[M], e2[M].
 // ---------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(TRI_THREADS)
@@ -434,13 +448,28 @@ tri_bisect_kernel(int32_t M, SliceTable tab, TriWs ws, int32_t s_off) {
         const double mid = 0.5 * (lo + hi);
         if (mid <= lo || mid >= hi) break;
         if (hi - lo <= 2.220446049250313e-16 * (fmax(fabs(lo), fabs(hi)) + 0.125 * span) + 2.0 * pivmin) break;
-        double q = d[0] - mid;
-        if (fabs(q) < pivmin) q = -pivmin;
-        int cnt = q < 0.0 ? 1 : 0;
+        // Sturm sequence in product form p_i = (d_i - x) p_{i-1} - e_{i-1}^2 p_{i-2} (two dependent FMAs per row instead
+        // of a division); a sign change between consecutive members = one eigenvalue below x; an exact zero takes the
+        // sign opposite to its predecessor; both members are rescaled every four rows against over/underflow
+        double p0 = 1.0, p1 = d[0] - mid;
+        if (p1 == 0.0) p1 = -pivmin;
+        int cnt = p1 < 0.0 ? 1 : 0;
         for (int i = 1; i < M; ++i) {
-            q = d[i] - mid - e2[i - 1] / q;
-            if (fabs(q) < pivmin) q = -pivmin;
-            cnt += q < 0.0 ? 1 : 0;
+            double p2 = fma(d[i] - mid, p1, -e2[i - 1] * p0);
+            if (p2 == 0.0) p2 = -copysign(fmax(fabs(p1), 1e-280) * 1e-20, p1);
+            cnt += ((p2 < 0.0) != (p1 < 0.0)) ? 1 : 0;
+            p0 = p1;
+            p1 = p2;
+            if ((i & 3) == 0) {
+                const double a = fmax(fabs(p0), fabs(p1));
+                if (a > 1e120) {
+                    p0 *= 1e-120;
+                    p1 *= 1e-120;
+                } else if (a < 1e-120) {
+                    p0 *= 1e120;
+                    p1 *= 1e120;
+                }
+            }
         }
         if (cnt > rank) hi = mid;
         else lo = mid;
@@ -614,19 +643,32 @@ tri_backtransform_kernel(int64_t N, int32_t M, SliceTable tab, const double* __r
     }
     const double* G = Gws + (size_t)s * M * M;
     const double* tau = ws.tau + (size_t)s * M;
-    double vc[EPT], vx[EPT];
+    // reflectors k, k-1, .., k-D+1 in flight: at small M one reflector's arithmetic is shorter than an L2 round trip
+    constexpr int D = EPT <= 2 ? 4 : (EPT <= 4 ? 3 : 2);
+    double vq[D][EPT];
     int k = M - 3;
 #pragma unroll
-    for (int e = 0; e < EPT; ++e) {
-        const int i = tid + BT_THREADS * e;
-        vc[e] = (k >= 0 && i > k && i < M) ? __ldg(G + (size_t)k * M + i) : 0.0;
+    for (int q = 0; q < D; ++q) {
+#pragma unroll
+        for (int e = 0; e < EPT; ++e) {
+            const int i = tid + BT_THREADS * e, kk = k - q;
+            vq[q][e] = (kk >= 0 && i > kk && i < M) ? __ldg(G + (size_t)kk * M + i) : 0.0;
+        }
     }
     for (; k >= 0; --k) {
         const double tk = __ldg(tau + k);
+        double vc[EPT];
 #pragma unroll
-        for (int e = 0; e < EPT; ++e) {  // next reflector (k - 1) while this one is applied
-            const int i = tid + BT_THREADS * e;
-            vx[e] = (k >= 1 && i >= k && i < M) ? __ldg(G + (size_t)(k - 1) * M + i) : 0.0;
+        for (int e = 0; e < EPT; ++e) vc[e] = vq[0][e];
+#pragma unroll
+        for (int q = 0; q + 1 < D; ++q) {
+#pragma unroll
+            for (int e = 0; e < EPT; ++e) vq[q][e] = vq[q + 1][e];
+        }
+#pragma unroll
+        for (int e = 0; e < EPT; ++e) {  // reflector k - D
+            const int i = tid + BT_THREADS * e, kk = k - D;
+            vq[D - 1][e] = (kk >= 0 && i > kk && i < M) ? __ldg(G + (size_t)kk * M + i) : 0.0;
         }
         double acc[NV];
 #pragma unroll
@@ -651,8 +693,6 @@ tri_backtransform_kernel(int64_t N, int32_t M, SliceTable tab, const double* __r
 #pragma unroll
             for (int e = 0; e < EPT; ++e) x[n][e] = fma(-tsum, vc[e], x[n][e]);
         }
-#pragma unroll
-        for (int e = 0; e < EPT; ++e) vc[e] = vx[e];
     }
 #pragma unroll
     for (int n = 0; n < NV; ++n) {

@@ -111,6 +111,7 @@ def test_stepwise_parity_small(N, P, w, iters, amp, width):
 @pytest.mark.parametrize("N,P,w", [(256, 4, 16), (270, 6, 4), (600, 3, 20)])
 def test_l2_resident_jacobi_fallback_matches_oracle(N, P, w, monkeypatch):
     # the L2-resident cluster kernel is the fallback for submatrices too large for shared memory; force it
+    monkeypatch.setenv("PFSM_JACOBI", "1")      # (above M = 200 the tridiagonal route is the default)
     monkeypatch.setenv("PFSM_JACOBI_L2", "1")
     p = gen.small_problem(N, 1e-3, 12.0, seed=1000 + N)
     g2 = gpu_solve(p.A, P, w, 1, p.alpha, last_step=2)
@@ -385,10 +386,15 @@ def test_chained_launches_change_no_bit(N, P, w, iters, monkeypatch):
         assert np.array_equal(g["resid"], plain["resid"])
 
 
-@pytest.mark.parametrize("k", [0, 1, 2, 5])
-def test_baseline_configs_full_oracle(k):
+@pytest.mark.parametrize("k,family", [(0, "default"), (1, "default"), (2, "default"), (5, "default"),
+                                      (1, "tridiag"), (2, "jacobi"), (5, "jacobi")])
+def test_baseline_configs_full_oracle(k, family, monkeypatch):
     """BASELINE.json configs 0-2 at full size, and the Cu256-shaped extra case (N = 1664, window at the paper's
-    gamma = 0.25: M = 416, clamped windows on 4 of 13 slices): element-by-element gates against the full oracle run."""
+    gamma = 0.25: M = 416, clamped windows on 4 of 13 slices): element-by-element gates against the full oracle run.
+    default = the route the library picks (Jacobi for configs 0-1, tridiagonalization for 2 and 5); the other family
+    is forced as well."""
+    if family != "default":
+        monkeypatch.setenv("PFSM_JACOBI" if family == "jacobi" else "PFSM_TRIDIAG", "1")
     p = gen.problem(k)
     c = p.cfg
     g = gpu_solve(p.A, c.P, c.window, c.iters, p.alpha)
@@ -397,14 +403,80 @@ def test_baseline_configs_full_oracle(k):
     assert np.abs(g["eps"] - o["eps"]).max() <= 1e-12 * p.normF
 
 
-@pytest.mark.parametrize("k", [3, 4])
-def test_baseline_configs_large_sampled(k):
+def _check_steps_4_5_at_full_size(p, g3, g, k):
+    """Step 4 through the uniqueness of QR, step 5 on sampled columns the oracle computes one by one, trace and
+    residual enclosure -- properties that hold at any size."""
+    c = p.cfg
+    N, m = c.N, c.m
+    nF = p.normF
+    assert g["info"] == 0
+    Vg = torch.from_numpy(g["Vr"]).cuda()
+    V3g = torch.from_numpy(g3["Vr"]).cuda()
+    eye_err = (Vg @ Vg.T - torch.eye(N, dtype=torch.float64, device="cuda")).abs().max().item()
+    assert eye_err <= 1e-12 * N
+    R = Vg @ V3g.T
+    assert torch.tril(R, -1).abs().max().item() < 1e-9
+    assert (torch.diagonal(R) > 0).all()
+    cols = [0, 1, m - 1, m, N // 2, N - 2, N - 1] + [int(x) for x in (gen.uniform(9, gen.STREAM_TEST, k, 9) * N)]
+    for i in cols:
+        lam_o, res_o = oracle.step5(p.A, g["Vr"], i, i + 1)
+        assert abs(lam_o[i] - g["lam"][i]) <= 1e-10 * nF
+        assert abs(res_o[i] - g["resid"][i]) <= 1e-9 * nF
+    assert abs(g["lam"].sum() - np.trace(p.A)) <= 1e-9
+    ex = torch.linalg.eigvalsh(torch.from_numpy(p.A).cuda()).cpu().numpy()   # comparison only (P9 enclosure)
+    idx = np.searchsorted(ex, g["lam"])
+    near = np.minimum(np.abs(ex[np.clip(idx, 0, N - 1)] - g["lam"]), np.abs(ex[np.clip(idx - 1, 0, N - 1)] - g["lam"]))
+    assert np.all(near <= g["resid"] + 1e-10)
+
+
+def test_wide_window_config6_at_full_size():
+    """Config 4's matrix at the paper's gamma = 0.25 (N = 8192, P = 16, M = 2048: the tridiagonalization route of
+    step 2, lower-triangle storage).  The oracle's Jacobi needs minutes per 2048 x 2048 slice, so step 2 is checked
+    against what it must deliver by definition -- the eigenpairs of rank off .. off+m-1 of B_s:
+    eigenvalues against LAPACK on sampled slices, residuals ||B y - mu y||, zero padding -- and steps 4-5 as for
+    configs 3-4."""
+    p = gen.problem(6)
+    c = p.cfg
+    N, m = c.N, c.m
+    g3 = gpu_solve(p.A, c.P, c.window, c.iters, p.alpha, last_step=2)
+    assert g3["info"] == 0
+    M, g0, lo, off = oracle.partition(N, c.P, c.window)
+    assert M == 2048
+    for s in (0, c.P // 2, c.P - 1):
+        B = p.A[lo[s]:lo[s] + M, lo[s]:lo[s] + M]
+        mu = np.linalg.eigvalsh(B)[off[s]:off[s] + m]
+        eps_s = g3["eps"][g0[s]:g0[s] + m]
+        assert np.abs(eps_s - mu).max() <= 1e-12 * p.normF
+        rows = g3["Vr"][g0[s]:g0[s] + m]
+        mask = np.ones(N, bool)
+        mask[lo[s]:lo[s] + M] = False
+        assert np.all(rows[:, mask] == 0.0)
+        Y = rows[:, lo[s]:lo[s] + M]
+        assert np.abs(Y @ B - eps_s[:, None] * Y).max() <= 1e-12 * np.linalg.norm(B)
+        assert np.abs(np.einsum("ij,ij->i", Y, Y) - 1.0).max() < 1e-13
+        assert np.abs(Y @ Y.T - np.eye(m)).max() < 1e-7     # eps ||B|| / gap; step 4 orthonormalizes (reading R25)
+        if os.environ.get("PFSM_FULL_ORACLE") == "1" and s == c.P // 2:   # the oracle's own Jacobi: ~7 min on 16 cores
+            mu_o, Y_o, sw = oracle.jacobi_eig(B)
+            assert sw > 0
+            assert np.abs(eps_s - mu_o[off[s]:off[s] + m]).max() <= 1e-12 * p.normF
+            Yo = Y_o[:, off[s]:off[s] + m].T
+            assert np.abs(align_signs(Y, Yo) - Yo).max() < 1e-7
+    g3 = gpu_solve(p.A, c.P, c.window, c.iters, p.alpha, last_step=3)
+    g = gpu_solve(p.A, c.P, c.window, c.iters, p.alpha)
+    _check_steps_4_5_at_full_size(p, g3, g, 6)
+
+
+@pytest.mark.parametrize("k,family", [(3, "default"), (4, "default"), (4, "jacobi")])
+def test_baseline_configs_large_sampled(k, family, monkeypatch):
     """BASELINE.json configs 3-4 at full size, in bench.py's launch configuration.  The full oracle needs
     ~1e13 flop (minutes), so: steps 2-3 are compared with the oracle on sampled whole slices (slices are
     independent); step 4 through the uniqueness of QR (V_out orthonormal and V_out^T V_3
     upper triangular with positive diagonal <=> V_out is THE Gram-Schmidt result); step 5 on sampled
     columns the oracle computes one by one; trace and residual-enclosure hold at any size.
-    PFSM_FULL_ORACLE=1 adds the full element-by-element comparison."""
+    PFSM_FULL_ORACLE=1 adds the full element-by-element comparison.  default = the tridiagonal route of step 2;
+    jacobi = the shared-memory Jacobi (clusters of 8 half CTAs)."""
+    if family == "jacobi":
+        monkeypatch.setenv("PFSM_JACOBI", "1")
     p = gen.problem(k)
     c = p.cfg
     N, m = c.N, c.m
@@ -426,24 +498,7 @@ def test_baseline_configs_large_sampled(k):
         Vg = g3["Vr"][g0[s]:g0[s] + m]
         assert np.abs(align_signs(Vg, V3) - V3).max() < 1e-8
     g = gpu_solve(p.A, c.P, c.window, c.iters, p.alpha)
-    assert g["info"] == 0
-    Vg = torch.from_numpy(g["Vr"]).cuda()
-    V3g = torch.from_numpy(g3["Vr"]).cuda()
-    eye_err = (Vg @ Vg.T - torch.eye(N, dtype=torch.float64, device="cuda")).abs().max().item()
-    assert eye_err <= 1e-12 * N
-    R = Vg @ V3g.T
-    assert torch.tril(R, -1).abs().max().item() < 1e-9
-    assert (torch.diagonal(R) > 0).all()
-    cols = [0, 1, m - 1, m, N // 2, N - 2, N - 1] + [int(x) for x in (gen.uniform(9, gen.STREAM_TEST, k, 9) * N)]
-    for i in cols:
-        lam_o, res_o = oracle.step5(p.A, g["Vr"], i, i + 1)
-        assert abs(lam_o[i] - g["lam"][i]) <= 1e-10 * nF
-        assert abs(res_o[i] - g["resid"][i]) <= 1e-9 * nF
-    assert abs(g["lam"].sum() - np.trace(p.A)) <= 1e-9
-    ex = torch.linalg.eigvalsh(torch.from_numpy(p.A).cuda()).cpu().numpy()   # comparison only (P9 enclosure)
-    idx = np.searchsorted(ex, g["lam"])
-    near = np.minimum(np.abs(ex[np.clip(idx, 0, N - 1)] - g["lam"]), np.abs(ex[np.clip(idx - 1, 0, N - 1)] - g["lam"]))
-    assert np.all(near <= g["resid"] + 1e-10)
+    _check_steps_4_5_at_full_size(p, g3, g, k)
     if os.environ.get("PFSM_FULL_ORACLE") == "1":
         o = oracle.pfsm(p.A, c.P, c.window, c.iters, p.alpha)
         check_gates(p.A, g, o)
@@ -710,9 +765,13 @@ def test_second_cholqr_pass_restores_orthogonality_of_ill_conditioned_vectors():
     h.destroy()
 
 
+@pytest.mark.parametrize("family", ["default", "jacobi"])
 @pytest.mark.parametrize("N,P,w", [(800, 2, 0), (1024, 2, 0), (1024, 4, 128)])
-def test_large_submatrices_up_to_the_library_limit(N, P, w):
-    # M = 400 (shared-memory kernel, cluster of 8), M = 512 (the limit: L2-resident fallback kernel, 16 doubles/lane)
+def test_large_submatrices_up_to_the_jacobi_limit(N, P, w, family, monkeypatch):
+    # M = 400 and M = 512.  default: the tridiagonal route (cluster-barrier tridiagonalization); jacobi: the
+    # shared-memory kernel with a cluster of 8 (M = 400) and the L2-resident fallback with 16 doubles/lane (M = 512)
+    if family == "jacobi":
+        monkeypatch.setenv("PFSM_JACOBI", "1")
     p = gen.small_problem(N, 1e-3, 24.0, seed=5000 + N + w)
     g2 = gpu_solve(p.A, P, w, 1, p.alpha, last_step=2)
     V2, eps, info2 = oracle.step2(p.A, P, w)
@@ -724,7 +783,7 @@ def test_large_submatrices_up_to_the_library_limit(N, P, w):
     check_gates(p.A, g, o)
 
 
-@pytest.mark.parametrize("k,reps", [(0, 60), (1, 12)])
+@pytest.mark.parametrize("k,reps", [(0, 60), (1, 12), (2, 8)])
 def test_repeated_solves_are_bitwise_identical(k, reps):
     # race detector: the cluster exchange of step 2, the two-stream schedule of step 4 and every reduction have a
     # fixed order, so a solve is bitwise reproducible; any data race shows up as a differing bit sooner or later
