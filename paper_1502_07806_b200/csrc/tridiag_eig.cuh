@@ -620,7 +620,7 @@ tri_invit_kernel(int64_t N, int32_t M, SliceTable tab, TriWs ws, int32_t s_off) 
 // ---------------------------------------------------------------------------------------------
 constexpr int BT_THREADS = 256;
 
-template <int EPT, int NV>
+template <int EPT, int NV>  // NV = 8 or 4; BT_THREADS = 256 (8 warps) is assumed by the cross-warp sum
 __global__ void __launch_bounds__(BT_THREADS, 1)
 tri_backtransform_kernel(int64_t N, int32_t M, SliceTable tab, const double* __restrict__ Gws, TriWs ws,
                          double* __restrict__ V, double* __restrict__ eps, int32_t s_off) {
@@ -676,20 +676,41 @@ tri_backtransform_kernel(int64_t N, int32_t M, SliceTable tab, const double* __r
             double a = 0.0;
 #pragma unroll
             for (int e = 0; e < EPT; ++e) a = fma(vc[e], x[n][e], a);
-            acc[n] = warp_sum(a);
+            acc[n] = a;
         }
-        double(*pb)[NV] = part[k & 1];
-        if (lane == 0) {
+        // NV warp sums at once: halving butterfly (NV - 1 shuffles) leaves lane l with the 32/NV-lane partial of value
+        // n = l / (32 / NV), the remaining xor steps complete it; the shuffle / shared-memory queue, not FP64, bounds
+        // this kernel, so the plain version (5 NV shuffles, 8 NV shared loads per thread) was 3 x slower
 #pragma unroll
-            for (int n = 0; n < NV; ++n) pb[warp][n] = acc[n];
+        for (int h = 16, cn = NV / 2; cn >= 1; h >>= 1, cn >>= 1) {
+            const bool up = (lane & h) != 0;
+#pragma unroll
+            for (int r = 0; r < cn; ++r) {
+                const double send = up ? acc[r] : acc[r + cn], keep = up ? acc[r + cn] : acc[r];
+                acc[r] = keep + __shfl_xor_sync(0xffffffffu, send, h);
+            }
         }
+#pragma unroll
+        for (int h = 16 / NV; h >= 1; h >>= 1) acc[0] += __shfl_xor_sync(0xffffffffu, acc[0], h);
+        double(*pb)[NV] = part[k & 1];
+        if ((lane & (32 / NV - 1)) == 0) pb[warp][lane / (32 / NV)] = acc[0];
         __syncthreads();
+        // totals over the 8 warps: lane l adds the partials of value l % NV (fixed tree), then the NV totals are broadcast
+        double t;
+        if (NV == 8) {
+            t = pb[lane >> 3][lane & 7] + pb[(lane >> 3) + 4][lane & 7];
+            t += __shfl_xor_sync(0xffffffffu, t, 8);
+            t += __shfl_xor_sync(0xffffffffu, t, 16);
+        } else {
+            t = pb[lane >> 2][lane & 3];
+            t += __shfl_xor_sync(0xffffffffu, t, 4);
+            t += __shfl_xor_sync(0xffffffffu, t, 8);
+            t += __shfl_xor_sync(0xffffffffu, t, 16);
+        }
+        t *= tk;
 #pragma unroll
         for (int n = 0; n < NV; ++n) {
-            double tsum = 0.0;
-#pragma unroll
-            for (int w = 0; w < BT_THREADS / 32; ++w) tsum += pb[w][n];
-            tsum *= tk;
+            const double tsum = __shfl_sync(0xffffffffu, t, n);
 #pragma unroll
             for (int e = 0; e < EPT; ++e) x[n][e] = fma(-tsum, vc[e], x[n][e]);
         }
