@@ -435,11 +435,11 @@ static void choose_jacobi_layout(pfsm_ctx* h) {
     h->jac_wide = getenv("PFSM_JACOBI_WIDE") != nullptr;  // diagnostic: the wide-window Jacobi kernel at any M
     // Route of step 2.  Tridiagonalization + bisection + inverse iteration + back-transformation costs ~M latency-bound
     // columns; the Jacobi kernels cost sweeps x (M - 1) rounds.  Measured (step 2, Jacobi -> tridiagonal): M = 96 x 4
-    // slices 0.60 -> 1.14 ms, M = 192 x 16 2.66 -> 2.59, M = 224 x 24 4.57 -> 3.30, M = 254 x 72 13.5 -> 5.8, M = 256 x 64
-    // 12.5 -> 5.3, M = 416 x 13 15.2 -> 6.1 ms.  So: Jacobi up to M = 200, the tridiagonal route above.
+    // slices 0.60 -> 1.00 ms, M = 192 x 16 2.66 -> 2.15, M = 224 x 24 4.57 -> 2.69, M = 254 x 72 13.5 -> 4.9, M = 256 x 64
+    // 12.5 -> 4.0, M = 416 x 13 15.2 -> 5.4 ms.  So: Jacobi up to M = 160, the tridiagonal route above.
     // PFSM_JACOBI=1 / PFSM_TRIDIAG=1 force one family (M > 512 has no shared-memory / L2 Jacobi: PFSM_JACOBI_WIDE).
     const bool want_jacobi = getenv("PFSM_JACOBI") != nullptr && h->M <= 512;
-    h->tridiag = !h->jac_wide && !want_jacobi && (h->M > 200 || getenv("PFSM_TRIDIAG") != nullptr);
+    h->tridiag = !h->jac_wide && !want_jacobi && (h->M > 160 || getenv("PFSM_TRIDIAG") != nullptr);
     if (h->M > 512 || h->jac_wide || h->tridiag) return;
     if (getenv("PFSM_JACOBI_L2")) return;  // diagnostic: force the L2-resident kernel (the large-M fallback)
     const size_t budget = 220 * 1024;
@@ -517,7 +517,7 @@ static int launch_jacobi_wide_t(pfsm_ctx* h, const double* A, double* V, cudaStr
 }  // extern "C++"
 
 // Wide windows, default route: Householder tridiagonalization + bisection + inverse iteration + back-transformation
-static int launch_tridiag(pfsm_ctx* h, const double* A, double* V, cudaStream_t st, int32_t s0, int32_t ns) {
+static int launch_tridiag(pfsm_ctx* h, const double* A, double* V, cudaStream_t st, int32_t s0, int32_t ns, int32_t precopied) {
     SliceTable tab{h->slice_tab, h->slice_tab + h->P, h->slice_tab + 2 * (size_t)h->P, h->slice_tab + 3 * (size_t)h->P};
     const int M = h->M;
     int sms = 0;
@@ -584,13 +584,14 @@ static int launch_tridiag(pfsm_ctx* h, const double* A, double* V, cudaStream_t 
         cfg.attrs = attr;
         cfg.numAttrs = 1;
         PFSM_CUDA(cudaLaunchKernelEx(&cfg, kern, A, h->N, (int32_t)M, tab, h->Gws, h->tri, h->P, s0, ns, (int32_t)C,
-                                     h->jw_bar));
+                                     h->jw_bar, precopied));
     }
     const size_t smem2 = 2 * (size_t)M * sizeof(double);
     PFSM_CUDA(cudaFuncSetAttribute(tri_bisect_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem2));
     PFSM_CUDA(cudaFuncSetAttribute(tri_invit_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem2));
     const dim3 g2((unsigned)((h->m + TRI_THREADS - 1) / TRI_THREADS), (unsigned)ns);
-    tri_bisect_kernel<<<g2, TRI_THREADS, smem2, st>>>((int32_t)M, tab, h->tri, s0);
+    const dim3 g2b((unsigned)((h->m + TRI_THREADS / 32 - 1) / (TRI_THREADS / 32)), (unsigned)ns);
+    tri_bisect_kernel<<<g2b, TRI_THREADS, smem2, st>>>((int32_t)M, tab, h->tri, s0);
     PFSM_CUDA(cudaGetLastError());
     tri_invit_kernel<<<g2, TRI_THREADS, smem2, st>>>(h->N, (int32_t)M, tab, h->tri, s0);
     PFSM_CUDA(cudaGetLastError());
@@ -616,7 +617,7 @@ static int launch_jacobi(pfsm_ctx* h, const double* A, double* V, cudaStream_t s
                          int32_t compact = 0) {
     if (ns < 0) ns = h->P;
     PFSM_CUDA(cudaMemsetAsync(h->rotcnt, 0, (size_t)h->P * JACOBI_MAX_SWEEPS * sizeof(int), st));
-    if (h->tridiag) return launch_tridiag(h, A, V, st, s0, ns);
+    if (h->tridiag) return launch_tridiag(h, A, V, st, s0, ns, compact);
     if (h->M > 512 || h->jac_wide) {
         const int ept = (h->M + JW_GROUP - 1) / JW_GROUP;
         if (ept <= 2) return launch_jacobi_wide_t<2>(h, A, V, st, s0, ns);
@@ -1205,9 +1206,10 @@ int pfsm_solve_host(pfsm_handle_t h, const double* A_host, double* V_host, doubl
     }
     cudaStream_t st = (cudaStream_t)stream;
     int rc;
-    if (h->jac_cs > 0) {
-        // Step 2 only needs the P diagonal blocks: upload those first (packed, into the L2-Jacobi workspace that the
-        // shared-memory kernel leaves free) and let the full matrix follow on the side stream under the Jacobi kernel.
+    if (h->jac_cs > 0 || (h->tridiag && 2 * (size_t)h->P * h->M * h->M <= (size_t)h->N * h->N)) {
+        // Step 2 only needs the P diagonal blocks: upload those first (packed, into the workspace the shared-memory
+        // Jacobi leaves free and the tridiagonal route works in) and let the full matrix follow on the side stream
+        // under the step-2 kernels.  (Not when the blocks are as large as A itself: wide windows.)
         const size_t M = (size_t)h->M;
         for (int32_t sl = 0; sl < h->P; ++sl) {
             const int64_t lo = h->tab_host[(size_t)h->P + sl];

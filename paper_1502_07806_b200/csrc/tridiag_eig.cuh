@@ -7,7 +7,7 @@
 //                           k-1 is applied inside the pass that forms the matrix-vector product of column k, so the
 //                           trailing matrix is read and written once per column: 16 (M-k)^2 bytes -> (16/3) M^3 bytes
 //                           per slice.  HBM / L2 bandwidth bound.
-//   tri_bisect_kernel       eigenvalue of rank off+t of T by bisection on the Sturm count, one thread per eigenvalue
+//   tri_bisect_kernel       eigenvalue of rank off+t of T by 33-way multi-section on the Sturm count, one warp per eigenvalue
 //   tri_invit_kernel        its eigenvector by inverse iteration: LU of T - lambda I with partial pivoting, three
 //                           solves from a counter-based random start, one thread per eigenvector, factors stored
 //                           [row][vector] so that a warp's accesses coalesce
@@ -72,7 +72,7 @@ __device__ __forceinline__ double block_sum_512(double v, double* red) {  // fix
 template <bool CLUSTER>
 __global__ void __launch_bounds__(TRD_THREADS, 2)
 sytrd_kernel(const double* __restrict__ A, int64_t N, int32_t M, SliceTable tab, double* __restrict__ Gws, TriWs ws,
-             int32_t P, int32_t s_off, int32_t ns, int32_t C, unsigned int* __restrict__ bar) {
+             int32_t P, int32_t s_off, int32_t ns, int32_t C, unsigned int* __restrict__ bar, int32_t precopied) {
     extern __shared__ double sm[];
     double* vp = sm;          // v_{k-1}
     double* wp = sm + M;      // w_{k-1}
@@ -83,8 +83,8 @@ sytrd_kernel(const double* __restrict__ A, int64_t N, int32_t M, SliceTable tab,
     unsigned int phase = 0;
     const int nv = ns * C;
 
-    // copy B_s (row lo + i of A, columns lo ..) into the workspace
-    for (int vb = blockIdx.x; vb < nv; vb += gridDim.x) {
+    // copy B_s (row lo + i of A, columns lo ..) into the workspace, unless pfsm_solve_host uploaded the blocks there
+    for (int vb = blockIdx.x; vb < nv && !precopied; vb += gridDim.x) {
         const int sl = vb / C, c = vb - sl * C, s = s_off + sl;
         const int lo = tab.lo[s];
         double* G = Gws + (size_t)s * M * M;
@@ -225,7 +225,7 @@ sytrd_kernel(const double* __restrict__ A, int64_t N, int32_t M, SliceTable tab,
 // ---------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(TRD_THREADS, 1)
 sytrd_half_kernel(const double* __restrict__ A, int64_t N, int32_t M, SliceTable tab, double* __restrict__ Gws, TriWs ws,
-                  int32_t P, int32_t s_off, int32_t ns, int32_t C, unsigned int* __restrict__ bar) {
+                  int32_t P, int32_t s_off, int32_t ns, int32_t C, unsigned int* __restrict__ bar, int32_t precopied) {
     extern __shared__ double sm[];
     double* vp = sm;          // v_{k-1}
     double* wp = sm + M;      // w_{k-1}
@@ -238,7 +238,7 @@ sytrd_half_kernel(const double* __restrict__ A, int64_t N, int32_t M, SliceTable
     const int nb = (M + 31) / 32;
     const size_t bufs = (size_t)nb * M;  // rowbuf / colbuf doubles per slice
 
-    for (int vb = blockIdx.x; vb < nv; vb += gridDim.x) {
+    for (int vb = blockIdx.x; vb < nv && !precopied; vb += gridDim.x) {
         const int sl = vb / C, c = vb - sl * C, s = s_off + sl;
         const int lo = tab.lo[s];
         double* G = Gws + (size_t)s * M * M;
@@ -400,7 +400,7 @@ sytrd_half_kernel(const double* __restrict__ A, int64_t N, int32_t M, SliceTable
 // ---------------------------------------------------------------------------------------------
 // Eigenvalue of local rank off + t of T_s by bisection.  count(x) = number of eigenvalues < x = number of sign changes
 // of the Sturm sequence p_i = (d_i - x) p_{i-1} - e_{i-1}^2 p_{i-2}, p_{-1} = 1 (= negative pivots of LDL^T).
-// grid.x = ceil(mmax / TRI_THREADS), grid.y = ns.  Dynamic shared memory: d[M], e2[M].
+// grid.x = ceil(mmax / (TRI_THREADS / 32)) (a warp per eigenvalue), grid.y = ns.  Dynamic shared memory: d[M], e2[M].
 // ---------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(TRI_THREADS)
 tri_bisect_kernel(int32_t M, SliceTable tab, TriWs ws, int32_t s_off) {
@@ -437,17 +437,20 @@ tri_bisect_kernel(int32_t M, SliceTable tab, TriWs ws, int32_t s_off) {
         ghi = fmax(ghi, rhi[w]);
         emax = fmax(emax, rem[w]);
     }
-    const int t = blockIdx.x * TRI_THREADS + tid;
+    // One WARP per eigenvalue: 32 probes x_l = lo + (l + 1)(hi - lo)/33 per round (multi-section), so an interval shrinks
+    // 33-fold per serial Sturm chain instead of 2-fold: ~11 rounds instead of ~55.
+    const int lane = tid & 31;
+    const int t = blockIdx.x * (TRI_THREADS / 32) + (tid >> 5);
     if (t >= tab.cnt[s]) return;
     const int rank = tab.off[s] + t;
     const double pivmin = 2.2250738585072014e-308 * fmax(1.0, emax);
     const double span = fmax(fabs(glo), fabs(ghi));
     double lo = glo - 2.0 * 2.220446049250313e-16 * span * M - 2.0 * pivmin;
     double hi = ghi + 2.0 * 2.220446049250313e-16 * span * M + 2.0 * pivmin;
-    for (int it = 0; it < 200; ++it) {
-        const double mid = 0.5 * (lo + hi);
-        if (mid <= lo || mid >= hi) break;
+    for (int it = 0; it < 64; ++it) {
         if (hi - lo <= 2.220446049250313e-16 * (fmax(fabs(lo), fabs(hi)) + 0.125 * span) + 2.0 * pivmin) break;
+        const double hstep = (hi - lo) * (1.0 / 33.0);
+        const double mid = fma((double)(lane + 1), hstep, lo);
         // Sturm sequence in product form p_i = (d_i - x) p_{i-1} - e_{i-1}^2 p_{i-2} (two dependent FMAs per row instead
         // of a division); a sign change between consecutive members = one eigenvalue below x; an exact zero takes the
         // sign opposite to its predecessor; both members are rescaled every four rows against over/underflow
@@ -471,10 +474,17 @@ tri_bisect_kernel(int32_t M, SliceTable tab, TriWs ws, int32_t s_off) {
                 }
             }
         }
-        if (cnt > rank) hi = mid;
-        else lo = mid;
+        // first probe with more than `rank` eigenvalues below it bounds the eigenvalue from above, its left neighbour
+        // (or the old lo) from below
+        const unsigned above = __ballot_sync(0xffffffffu, cnt > rank);
+        const int f = above ? __ffs(above) - 1 : 32;
+        const double nhi = __shfl_sync(0xffffffffu, mid, f & 31), nlo = __shfl_sync(0xffffffffu, mid, (f + 31) & 31);
+        const double olo = lo, ohi = hi;
+        hi = (f < 32) ? nhi : ohi;
+        lo = (f > 0) ? nlo : olo;
+        if (!(hi > lo) || (lo == olo && hi == ohi)) break;  // no representable progress
     }
-    ws.lam[tab.g0[s] + t] = 0.5 * (lo + hi);
+    if (lane == 0) ws.lam[tab.g0[s] + t] = 0.5 * (lo + hi);
 }
 
 // counter-based uniform in (-1, 1): splitmix64 finalizer of (vector, row)

@@ -111,7 +111,7 @@ def test_stepwise_parity_small(N, P, w, iters, amp, width):
 @pytest.mark.parametrize("N,P,w", [(256, 4, 16), (270, 6, 4), (600, 3, 20)])
 def test_l2_resident_jacobi_fallback_matches_oracle(N, P, w, monkeypatch):
     # the L2-resident cluster kernel is the fallback for submatrices too large for shared memory; force it
-    monkeypatch.setenv("PFSM_JACOBI", "1")      # (above M = 200 the tridiagonal route is the default)
+    monkeypatch.setenv("PFSM_JACOBI", "1")      # (above M = 160 the tridiagonal route is the default)
     monkeypatch.setenv("PFSM_JACOBI_L2", "1")
     p = gen.small_problem(N, 1e-3, 12.0, seed=1000 + N)
     g2 = gpu_solve(p.A, P, w, 1, p.alpha, last_step=2)
@@ -309,18 +309,24 @@ def test_solve_is_deterministic_and_ignores_v_input():
     assert np.array_equal(a["lam"], b["lam"]) and np.array_equal(a["Vr"], b["Vr"])
 
 
-def test_host_buffer_entry_point_matches_device_entry_point():
-    p = gen.problem(0)
-    c = p.cfg
-    N = c.N
-    h = pfsm.Handle(N, c.P, c.window, c.iters, p.alpha)
+@pytest.mark.parametrize("case", ["config0", "config1", "wide"])
+def test_host_buffer_entry_point_matches_device_entry_point(case):
+    # config 0: shared-memory Jacobi, config 1: tridiagonal route -- both with the diagonal blocks uploaded ahead of A;
+    # wide: M = 700 (blocks as large as A: plain upload)
+    if case == "wide":
+        p = gen.small_problem(1000, 1e-3, 24.0, seed=808)
+        N, P, w, iters = 1000, 2, 100, 2
+    else:
+        p = gen.problem(int(case[-1]))
+        N, P, w, iters = p.cfg.N, p.cfg.P, p.cfg.window, p.cfg.iters
+    h = pfsm.Handle(N, P, w, iters, p.alpha)
     Ah = torch.from_numpy(p.A).pin_memory()
     Vh = torch.empty((N, N), dtype=torch.float64).pin_memory()
     lh = torch.empty((N,), dtype=torch.float64).pin_memory()
     h.solve_host(Ah, Vh, lh)
     torch.cuda.synchronize()
     assert h.info() == 0
-    ref = gpu_solve(p.A, c.P, c.window, c.iters, p.alpha)
+    ref = gpu_solve(p.A, P, w, iters, p.alpha)
     assert np.array_equal(lh.numpy(), ref["lam"]) and np.array_equal(Vh.numpy(), ref["Vr"])
     h.destroy()
 
@@ -387,11 +393,11 @@ def test_chained_launches_change_no_bit(N, P, w, iters, monkeypatch):
 
 
 @pytest.mark.parametrize("k,family", [(0, "default"), (1, "default"), (2, "default"), (5, "default"),
-                                      (1, "tridiag"), (2, "jacobi"), (5, "jacobi")])
+                                      (0, "tridiag"), (1, "jacobi"), (2, "jacobi"), (5, "jacobi")])
 def test_baseline_configs_full_oracle(k, family, monkeypatch):
     """BASELINE.json configs 0-2 at full size, and the Cu256-shaped extra case (N = 1664, window at the paper's
     gamma = 0.25: M = 416, clamped windows on 4 of 13 slices): element-by-element gates against the full oracle run.
-    default = the route the library picks (Jacobi for configs 0-1, tridiagonalization for 2 and 5); the other family
+    default = the route the library picks (Jacobi for config 0, tridiagonalization for 1, 2 and 5); the other family
     is forced as well."""
     if family != "default":
         monkeypatch.setenv("PFSM_JACOBI" if family == "jacobi" else "PFSM_TRIDIAG", "1")
