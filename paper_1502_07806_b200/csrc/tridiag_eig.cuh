@@ -580,28 +580,62 @@ tri_invit_kernel(int64_t N, int32_t M, SliceTable tab, TriWs ws, int32_t s_off) 
     double scale = 1.0;
     for (int iter = 0; iter < 3; ++iter) {
         // forward: L^-1 P^T b   (b = scale * previous z, or the random start)
+        // (operands of IB rows are requested together: the recurrences are short, the global-memory latency is not)
+        constexpr int IB = 8;
         double bi = (iter == 0) ? tri_start_value((uint32_t)g, 0u) : z[0] * scale;
-        for (int i = 0; i < M - 1; ++i) {
-            const double bn = (iter == 0) ? tri_start_value((uint32_t)g, (uint32_t)(i + 1)) : z[(size_t)(i + 1) * st] * scale;
-            const double f = lm[i * st];
-            if (pv[i * st]) {
-                z[i * st] = bn;
-                bi = fma(-f, bn, bi);
-            } else {
-                z[i * st] = bi;
-                bi = fma(-f, bi, bn);
+        for (int i0 = 0; i0 < M - 1; i0 += IB) {
+            double bnv[IB], fv[IB];
+            unsigned char pvv[IB];
+#pragma unroll
+            for (int u = 0; u < IB; ++u) {
+                const int i = i0 + u;
+                if (i < M - 1) {
+                    bnv[u] = (iter == 0) ? tri_start_value((uint32_t)g, (uint32_t)(i + 1)) : z[(size_t)(i + 1) * st] * scale;
+                    fv[u] = lm[i * st];
+                    pvv[u] = pv[i * st];
+                }
+            }
+#pragma unroll
+            for (int u = 0; u < IB; ++u) {
+                const int i = i0 + u;
+                if (i < M - 1) {
+                    if (pvv[u]) {
+                        z[i * st] = bnv[u];
+                        bi = fma(-fv[u], bnv[u], bi);
+                    } else {
+                        z[i * st] = bi;
+                        bi = fma(-fv[u], bi, bnv[u]);
+                    }
+                }
             }
         }
         // backward: U^-1
         double x1 = bi * uinv[(size_t)(M - 1) * st], x2 = 0.0;
         z[(size_t)(M - 1) * st] = x1;
         double ss = x1 * x1;
-        for (int i = M - 2; i >= 0; --i) {
-            const double xi = (z[i * st] - u1[i * st] * x1 - u2[i * st] * x2) * uinv[i * st];
-            z[i * st] = xi;
-            ss = fma(xi, xi, ss);
-            x2 = x1;
-            x1 = xi;
+        for (int i0 = M - 2; i0 >= 0; i0 -= IB) {
+            double zv[IB], a1[IB], a2[IB], iv[IB];
+#pragma unroll
+            for (int u = 0; u < IB; ++u) {
+                const int i = i0 - u;
+                if (i >= 0) {
+                    zv[u] = z[i * st];
+                    a1[u] = u1[i * st];
+                    a2[u] = u2[i * st];
+                    iv[u] = uinv[i * st];
+                }
+            }
+#pragma unroll
+            for (int u = 0; u < IB; ++u) {
+                const int i = i0 - u;
+                if (i >= 0) {
+                    const double xi = (zv[u] - a1[u] * x1 - a2[u] * x2) * iv[u];
+                    z[i * st] = xi;
+                    ss = fma(xi, xi, ss);
+                    x2 = x1;
+                    x1 = xi;
+                }
+            }
         }
         scale = rsqrt(ss);
         // guard against overflow of the sum of squares (growth ~ 1/(eps ||T||) per solve from a unit vector)
