@@ -61,8 +61,10 @@ typedef struct pfsm_ctx* pfsm_handle_t; /* opaque */
  *           N/P of them when P divides N (the paper writes m = N/P), else floor(N/P) or ceil(N/P) (reading R14)
  *   window  halo rows/columns added on each side of a slice's diagonal block; >= 0.
  *           M = min(N, ceil(N/P) + 2*window), the order of every submatrix, must be <= 4096 in this version
- *           (M <= ~480: shared-memory resident Jacobi; M <= 512: L2-resident; 512 < M <= 4096: the wide-window
- *           kernel, one persistent grid over all slices -- the paper's gamma = 0.2-0.3 regime).
+ *           (M <= 160: shared-memory resident cluster Jacobi; 160 < M <= 4096: Householder tridiagonalization +
+ *           multi-section + inverse iteration + back-transformation of the slice's own eigenpairs -- this covers the
+ *           paper's wide windows, gamma = M/N = 0.2-0.3.  Both deliver the eigenpairs to O(eps ||B||);
+ *           the vectors of a tight eigenvalue cluster are accurate to eps ||B|| / gap and are orthonormalized by step 4.)
  *   iters   folded-spectrum iterations of Eq. 11; >= 0
  *   alpha   step length of Eq. 11; finite and > 0.  The library does not estimate spectra:
  *           alpha = 0.5 / max|lambda|^2 keeps every damping factor 1 - alpha (lambda - eps)^2 in [-1, 1].
@@ -198,7 +200,8 @@ int pfsm_check_validity(pfsm_handle_t h, void* stream, double resid_tol, int32_t
                         double* max_resid_out, int64_t* info_out);
 
 /* Largest number of Jacobi sweeps any slice's submatrix eigensolve (step 2) used in the last solve;
- * synchronizes `stream`.  The last sweep is the one that found nothing left to rotate. */
+ * synchronizes `stream`.  The last sweep is the one that found nothing left to rotate.  Reads 1 when step 2 took
+ * the tridiagonal route (M > 160), which has no sweeps. */
 int pfsm_get_step2_sweeps(pfsm_handle_t h, void* stream, int32_t* max_sweeps);
 
 /* Device pointer to the N residual norms r_i = ||A v_i - lambda_i v_i||_2 of the last solve (step 5). */
