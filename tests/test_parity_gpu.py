@@ -186,6 +186,49 @@ def test_wide_window_routes_on_doubly_degenerate_spectrum(route, monkeypatch):
         assert g["resid"].max() < 1e-11 * np.linalg.norm(A)
 
 
+@pytest.mark.parametrize("mult", [3, 13])
+def test_tridiagonal_route_on_exact_multiplets(mult):
+    # A = Q diag(d) Q^T with every eigenvalue repeated `mult` times (13 = the multiplet size of BASELINE config 2,
+    # here exactly degenerate up to rounding): inverse iteration has no re-orthogonalization inside clusters (reading
+    # R25), so the vectors of a multiplet come out as independent random combinations and step 4 must make them
+    # orthonormal.  Only rotation-invariant quantities are compared (reading R16).  P = 2 with full windows: M = N > 160.
+    nm = 20
+    N = nm * mult
+    if N % 2:
+        N += mult
+        nm += 1
+    d = np.repeat(np.linspace(-1.0, 1.0, nm), mult)
+    Q = gen.householder_orthogonal(N, 6, seed=99)
+    A = (Q * d) @ Q.T
+    A = 0.5 * (A + A.T)
+    nF = np.linalg.norm(A)
+    g2 = gpu_solve(A, 2, N, 2, 0.5, last_step=2)
+    assert g2["info"] == 0
+    assert np.abs(g2["eps"] - d).max() < 1e-13 * nF
+    g = gpu_solve(A, 2, N, 2, 0.5)
+    assert g["info"] == 0
+    assert np.abs(g["lam"] - d).max() < 1e-12 * nF
+    assert np.abs(g["Vr"] @ g["Vr"].T - np.eye(N)).max() <= 1e-12 * N
+    assert g["resid"].max() < 1e-11 * nF
+
+
+@pytest.mark.parametrize("N", [3000, 4096])
+def test_submatrix_order_up_to_the_library_limit(N):
+    # P = 1: the submatrix is A itself, M = N = 3000 ("M <= 3000") and 4096 (the library limit: 16 rows
+    # per thread in the back-transformation, 8 prologue rows per thread in the tridiagonalization).  The oracle's Jacobi
+    # would need hours, so step 2 is checked against its definition: eigenvalues vs LAPACK, residuals, orthonormality
+    p = gen.small_problem(N, 1e-3, 48.0, seed=6000 + N)
+    g2 = gpu_solve(p.A, 1, 0, 1, p.alpha, last_step=2)
+    assert g2["info"] == 0
+    dA = torch.from_numpy(p.A).cuda()
+    mu = torch.linalg.eigvalsh(dA).cpu().numpy()
+    assert np.abs(g2["eps"] - mu).max() <= 1e-12 * p.normF
+    Y = torch.from_numpy(g2["Vr"]).cuda()
+    R = Y @ dA - torch.from_numpy(g2["eps"]).cuda()[:, None] * Y
+    assert R.abs().max().item() <= 1e-12 * p.normF
+    assert (Y @ Y.T - torch.eye(N, dtype=torch.float64, device="cuda")).abs().max().item() < 1e-7   # eps ||A|| / gap (R25)
+
+
 def test_iters_zero_is_gram_schmidt_of_start_vectors():
     p = gen.small_problem(288, 1e-3, 16.0, seed=77)
     g = gpu_solve(p.A, 4, 12, 0, p.alpha)
