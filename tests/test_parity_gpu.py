@@ -22,6 +22,25 @@ def dev(a):
     return torch.from_numpy(np.ascontiguousarray(a)).cuda()
 
 
+_ORACLE_MEMO = {}
+
+
+def oracle_step2_memo(A, P, w):
+    key = ("step2", A.shape[0], P, w, float(A.sum()), float(np.abs(A).sum()))
+    if key not in _ORACLE_MEMO:
+        _ORACLE_MEMO[key] = oracle.step2(A, P, w)
+    return _ORACLE_MEMO[key]
+
+
+def oracle_pfsm_memo(A, P, w, iters, alpha):
+    """oracle.pfsm, computed once per input: tests parametrized over the step-2 route compare every route with the
+    same oracle run (the oracle has one route)."""
+    key = (A.shape[0], P, w, iters, float(alpha), float(A.sum()), float(np.abs(A).sum()))
+    if key not in _ORACLE_MEMO:
+        _ORACLE_MEMO[key] = oracle.pfsm(A, P, w, iters, alpha)
+    return _ORACLE_MEMO[key]
+
+
 def gpu_solve(A, P, w, iters, alpha, last_step=5):
     N = A.shape[0]
     h = pfsm.Handle(N, P, w, iters, alpha)
@@ -135,7 +154,7 @@ def test_wide_window_routes_forced_at_small_shapes_match_oracle(N, P, w, route, 
         monkeypatch.setenv(name, "1")
     p = gen.small_problem(N, 1e-3, 12.0, seed=1000 + N)
     g2 = gpu_solve(p.A, P, w, 1, p.alpha, last_step=2)
-    V2, eps, info2 = oracle.step2(p.A, P, w)
+    V2, eps, info2 = oracle_step2_memo(p.A, P, w)
     assert g2["info"] == 0 and info2 == 0
     assert np.abs(g2["eps"] - eps).max() <= 1e-13 * max(1.0, p.normF)
     assert np.abs(align_signs(g2["Vr"], V2) - V2).max() < 1e-9
@@ -152,12 +171,12 @@ def test_wide_windows_beyond_512_match_oracle(N, P, w, iters, route, monkeypatch
             monkeypatch.setenv(name, "1")
     p = gen.small_problem(N, 1e-3, 24.0, seed=5000 + N + w)
     g2 = gpu_solve(p.A, P, w, iters, p.alpha, last_step=2)
-    V2, eps, info2 = oracle.step2(p.A, P, w)
+    V2, eps, info2 = oracle_step2_memo(p.A, P, w)
     assert g2["info"] == 0 and info2 == 0
     assert np.abs(g2["eps"] - eps).max() <= 1e-12 * max(1.0, p.normF)
     assert np.abs(align_signs(g2["Vr"], V2) - V2).max() < 1e-8
     g = gpu_solve(p.A, P, w, iters, p.alpha)
-    o = oracle.pfsm(p.A, P, w, iters, p.alpha)
+    o = oracle_pfsm_memo(p.A, P, w, iters, p.alpha)
     check_gates(p.A, g, o)
 
 
@@ -447,7 +466,7 @@ def test_baseline_configs_full_oracle(k, family, monkeypatch):
     p = gen.problem(k)
     c = p.cfg
     g = gpu_solve(p.A, c.P, c.window, c.iters, p.alpha)
-    o = oracle.pfsm(p.A, c.P, c.window, c.iters, p.alpha)
+    o = oracle_pfsm_memo(p.A, c.P, c.window, c.iters, p.alpha)
     check_gates(p.A, g, o)
     assert np.abs(g["eps"] - o["eps"]).max() <= 1e-12 * p.normF
 
@@ -823,12 +842,12 @@ def test_large_submatrices_up_to_the_jacobi_limit(N, P, w, family, monkeypatch):
         monkeypatch.setenv("PFSM_JACOBI", "1")
     p = gen.small_problem(N, 1e-3, 24.0, seed=5000 + N + w)
     g2 = gpu_solve(p.A, P, w, 1, p.alpha, last_step=2)
-    V2, eps, info2 = oracle.step2(p.A, P, w)
+    V2, eps, info2 = oracle_step2_memo(p.A, P, w)
     assert g2["info"] == 0 and info2 == 0
     assert np.abs(g2["eps"] - eps).max() <= 1e-12 * max(1.0, p.normF)
     assert np.abs(align_signs(g2["Vr"], V2) - V2).max() < 1e-8
     g = gpu_solve(p.A, P, w, 1, p.alpha)
-    o = oracle.pfsm(p.A, P, w, 1, p.alpha)
+    o = oracle_pfsm_memo(p.A, P, w, 1, p.alpha)
     check_gates(p.A, g, o)
 
 
