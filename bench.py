@@ -383,8 +383,10 @@ def run_ours(args):
                     "step4_cholesky_qr": step_ms[2], "step5_rayleigh": step_ms[3]},
         "algorithmic_flops": flops, "quality": quality, "clocks": clocks,
         "e2e": {"value": e2e_value, "unit": "TFLOP/s", "ms_per_step": e2e_ms,
-                # A, plus the P diagonal blocks sent ahead for step 2 (not when they are as large as A: wide windows)
-                "h2d_bytes_per_step": 8 * N * N + (8 * c.P * c.M * c.M if (c.M <= 160 or 2 * c.P * c.M * c.M <= N * N) else 0),
+                # the lower block triangle of A (256-row blocks; A = A^T, mirrored on the device), plus the P diagonal
+                # blocks sent ahead for step 2 (not when they are as large as A: wide windows)
+                "h2d_bytes_per_step": 8 * sum(min(256, N - r0) * min(N, r0 + 256) for r0 in range(0, N, 256))
+                + (8 * c.P * c.M * c.M if (c.M <= 160 or 2 * c.P * c.M * c.M <= N * N) else 0),
                 "d2h_bytes_per_step": 8 * N * N + 8 * N},
         "gpu_launches": int(args.steps * h.launches_per_solve()),
         "roofline": roofline,

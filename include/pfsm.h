@@ -89,7 +89,9 @@ int pfsm_solve(pfsm_handle_t h, const double* A, double* V_inout, double* lambda
  * (2 N^2 doubles more, allocated on first use).  The copies overlap the compute: the P diagonal blocks that
  * step 2 needs go first, the full matrix follows on an internal stream under the step-2 kernel, and V returns
  * while step 5 runs; everything is joined back into `stream`, which the caller synchronizes before reading
- * V_host / lambda_host.
+ * V_host / lambda_host.  A is symmetric, so only its lower block triangle (256-row blocks, each up to the end of its
+ * diagonal block) and the P diagonal submatrices are read from A_host and sent over PCIe; the rest is mirrored on the device.  (pfsm_solve, with a
+ * device matrix, reads both triangles: reading R15.)
  */
 int pfsm_solve_host(pfsm_handle_t h, const double* A_host, double* V_host, double* lambda_host, void* stream);
 

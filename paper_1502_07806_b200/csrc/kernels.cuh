@@ -475,6 +475,27 @@ __global__ void transpose_kernel(const double* __restrict__ in, int64_t ldi, dou
     }
 }
 
+// Fills the block-upper part of a symmetric matrix from its block-lower part: for 32 x 32 tiles whose column lies in
+// a later RB-row block than their row, out tile (r, c) = transpose of tile (c, r).  pfsm_solve_host uploads only the
+// lower block triangle of A (half the PCIe bytes) and mirrors it here.  RB must be a multiple of 32.
+__global__ void mirror_lower_kernel(double* __restrict__ A, int64_t ld, int32_t n, int32_t RB) {
+    __shared__ double tile[32][33];
+    const int bx = blockIdx.x * 32, by = blockIdx.y * 32;  // destination tile: rows by.., columns bx..
+    if (bx / RB <= by / RB) return;
+    const int tx = threadIdx.x, ty = threadIdx.y;  // 32 x 8
+#pragma unroll
+    for (int k = 0; k < 32; k += 8) {
+        const int r = bx + ty + k, c = by + tx;  // source tile: rows bx.., columns by..
+        if (r < n && c < n) tile[ty + k][tx] = A[(size_t)r * ld + c];
+    }
+    __syncthreads();
+#pragma unroll
+    for (int k = 0; k < 32; k += 8) {
+        const int r = by + ty + k, c = bx + tx;
+        if (r < n && c < n) A[(size_t)r * ld + c] = tile[tx][ty + k];
+    }
+}
+
 // out = (in + in^T) / 2 for an n x n row-major matrix (32 x 32 tiles, both reads coalesced)
 __global__ void symmetrize_kernel(const double* __restrict__ in, int64_t ldi, double* __restrict__ out, int64_t ldo,
                                   int32_t n) {

@@ -1192,6 +1192,22 @@ int pfsm_solve(pfsm_handle_t h, const double* A, double* V_inout, double* lambda
     return pfsm_solve_partial(h, A, V_inout, lambda_out, stream, 5);
 }
 
+// A = A^T: only the lower block triangle (256-row blocks, each with its columns up to the end of its diagonal block)
+// crosses PCIe, 52 % of 8 N^2 bytes at N = 8192; the upper part is mirrored on the device (0.2 ms).
+static int upload_symmetric(pfsm_ctx* h, const double* A_host, cudaStream_t s) {
+    const int64_t N = h->N, RB = 256;
+    for (int64_t r0 = 0; r0 < N; r0 += RB) {
+        const int64_t rows = std::min<int64_t>(RB, N - r0), width = std::min<int64_t>(N, r0 + RB);
+        PFSM_CUDA(cudaMemcpy2DAsync(h->A_stage + (size_t)r0 * N, (size_t)N * sizeof(double), A_host + (size_t)r0 * N,
+                                    (size_t)N * sizeof(double), (size_t)width * sizeof(double), (size_t)rows,
+                                    cudaMemcpyHostToDevice, s));
+    }
+    const dim3 tb(32, 8), tg((unsigned)((N + 31) / 32), (unsigned)((N + 31) / 32));
+    mirror_lower_kernel<<<tg, tb, 0, s>>>(h->A_stage, N, (int32_t)N, (int32_t)RB);
+    PFSM_CUDA(cudaGetLastError());
+    return 0;
+}
+
 int pfsm_solve_host(pfsm_handle_t h, const double* A_host, double* V_host, double* lambda_host, void* stream) {
     if (!h) return -1;
     if (!A_host) return -2;
@@ -1218,11 +1234,11 @@ int pfsm_solve_host(pfsm_handle_t h, const double* A_host, double* V_host, doubl
         }
         PFSM_CUDA(cudaEventRecord(h->ev_fork, st));
         PFSM_CUDA(cudaStreamWaitEvent(h->side, h->ev_fork, 0));
-        PFSM_CUDA(cudaMemcpyAsync(h->A_stage, A_host, n2, cudaMemcpyHostToDevice, h->side));
+        if ((rc = upload_symmetric(h, A_host, h->side))) return rc;
         PFSM_CUDA(cudaEventRecord(h->ev_rest, h->side));
         rc = solve_impl(h, h->A_stage, h->V_stage, h->lam_stage, stream, 4, h->Gws, h->ev_rest);  // steps 2-4: V is final
     } else {
-        PFSM_CUDA(cudaMemcpyAsync(h->A_stage, A_host, n2, cudaMemcpyHostToDevice, st));
+        if ((rc = upload_symmetric(h, A_host, st))) return rc;
         rc = pfsm_solve_partial(h, h->A_stage, h->V_stage, h->lam_stage, stream, 4);
     }
     if (rc) return rc;

@@ -390,6 +390,17 @@ def test_host_buffer_entry_point_matches_device_entry_point(case):
     assert h.info() == 0
     ref = gpu_solve(p.A, P, w, iters, p.alpha)
     assert np.array_equal(lh.numpy(), ref["lam"]) and np.array_equal(Vh.numpy(), ref["Vr"])
+    # A = A^T: only the lower block triangle (256-row blocks) and the P diagonal submatrices (entries with
+    # |row - col| < M) are read from the host buffer and cross PCIe
+    M = min(N, -(-N // P) + 2 * w)
+    rr, cc = np.meshgrid(np.arange(N), np.arange(N), indexing="ij")
+    unread = (cc >= (rr // 256 + 1) * 256) & (cc - rr >= M)
+    Ah.numpy()[unread] = float("nan")
+    Vh.zero_()
+    lh.zero_()
+    h.solve_host(Ah, Vh, lh)
+    torch.cuda.synchronize()
+    assert np.array_equal(lh.numpy(), ref["lam"]) and np.array_equal(Vh.numpy(), ref["Vr"])
     h.destroy()
 
 
