@@ -1,12 +1,15 @@
-// tridiag_eig.cuh -- step 2 for wide windows (512 < M <= 4096; the paper's gamma = M/N = 0.2-0.3 regime,
-// "M <= 3000") as a batched dense symmetric eigensolver in four kernels.  Only the slice's m of
-// the M eigenpairs of B_s are wanted (local ascending ranks off .. off+m-1), which this route exploits:
+// tridiag_eig.cuh -- step 2 as a batched dense symmetric eigensolver in four kernels: the product path for
+// submatrix orders 160 < M <= 4096, i.e. BASELINE configs 1-4 (M = 192-256) and the paper's wide windows (gamma = M/N = 0.2-0.3,
+// "M <= 3000").  Only the slice's m of the M eigenpairs of B_s are wanted (local ascending ranks
+// off .. off+m-1), which this route exploits:
 //
-//   sytrd_kernel            B_s = Q T Q^T, Householder tridiagonalization of all slices at once by ONE persistent
-//                           cooperative grid (C CTAs per slice, grid barrier per column).  The rank-2 update of column
-//                           k-1 is applied inside the pass that forms the matrix-vector product of column k, so the
-//                           trailing matrix is read and written once per column: 16 (M-k)^2 bytes -> (16/3) M^3 bytes
-//                           per slice.  HBM / L2 bandwidth bound.
+//   sytrd_kernel<CLUSTER>   B_s = Q T Q^T, Householder tridiagonalization of all slices at once on full symmetric storage.  The
+//                           rank-2 update of column k-1 is applied inside the pass that forms the matrix-vector product of
+//                           column k, so the trailing matrix is read and written once per column (16 (M-k)^2 bytes).
+//                           CLUSTER (M <= 768): one thread-block cluster per slice, cluster barrier per column -- latency bound;
+//                           otherwise ONE persistent cooperative grid, C CTAs per slice, grid barrier per column.
+//   sytrd_half_kernel       the same on the lower triangle only (half the bytes, two grid barriers per column): used when the
+//                           batch 8 P M^2 exceeds L2, where the tridiagonalization is HBM bound
 //   tri_bisect_kernel       eigenvalue of rank off+t of T by 33-way multi-section on the Sturm count, one warp per eigenvalue
 //   tri_invit_kernel        its eigenvector by inverse iteration: LU of T - lambda I with partial pivoting, three
 //                           solves from a counter-based random start, one thread per eigenvector, factors stored
@@ -17,6 +20,7 @@
 // Eigenvalues closer than 10 eps |lambda| get shifts pushed apart as LAPACK's dstein does; there is no
 // re-orthogonalization inside clusters: step 4 orthonormalizes all N vectors anyway, and vectors of a
 // tight cluster that come out numerically dependent are flagged there (info = index of the dependent vector).
+// Every reduction has a fixed order: results are bitwise reproducible.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
