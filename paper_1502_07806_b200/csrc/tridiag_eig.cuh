@@ -370,16 +370,19 @@ sytrd_half_kernel(const double* __restrict__ A, int64_t N, int32_t M, SliceTable
             double* pb = ws.pbuf + (size_t)(k & 1) * P * M + so;
             const int L = M - k - 1, per = (L + C - 1) / C;
             const int i0 = k + 1 + c * per, i1 = min(M, i0 + per);
-            for (int i = i0 + tid; i < i1; i += TRD_THREADS) {
-                double a = 0.0;
+            // two threads per row (even / odd terms), 8 loads in flight each; terms in fixed order: strips b0 .. bi of
+            // rowbuf, then row blocks bi .. nb-1 of colbuf; the two partial sums are added by a shuffle (commutative: same bits)
+            for (int base = 0; base < per; base += TRD_THREADS / 2) {
+                const int i = i0 + base + (tid >> 1), sub = tid & 1;
+                const bool valid = i < i1;
                 const int bi = i / 32;
-                // terms in fixed order: strips b0 .. bi of rowbuf, then row blocks bi .. nb-1 of colbuf (8 loads in flight)
-                const int n1 = bi - b0 + 1, nt = n1 + nb - bi;
-                for (int q0 = 0; q0 < nt; q0 += 8) {
+                const int n1 = bi - b0 + 1, nt = valid ? n1 + nb - bi : 0;
+                double a = 0.0;
+                for (int q0 = sub; q0 < nt; q0 += 16) {
                     double x[8];
 #pragma unroll
                     for (int u = 0; u < 8; ++u) {
-                        const int q = q0 + u;
+                        const int q = q0 + 2 * u;
                         x[u] = (q >= nt) ? 0.0
                                : (q < n1) ? __ldcg(rowbuf + (size_t)(b0 + q) * M + i)
                                           : __ldcg(colbuf + (size_t)(bi + q - n1) * M + i);
@@ -387,7 +390,8 @@ sytrd_half_kernel(const double* __restrict__ A, int64_t N, int32_t M, SliceTable
 #pragma unroll
                     for (int u = 0; u < 8; ++u) a += x[u];
                 }
-                pb[i] = tau * a;
+                a += __shfl_xor_sync(0xffffffffu, a, 1);
+                if (valid && sub == 0) pb[i] = tau * a;
             }
         }
         jw_grid_barrier(bar, phase);
