@@ -722,11 +722,19 @@ def test_warm_start_identity_basis_equals_plain_solve():
     assert np.abs(g["lam"] - ref["lam"]).max() < 1e-14 and np.abs(g["Vr"] - ref["Vr"]).max() < 1e-13
 
 
-@pytest.mark.parametrize("big", [False, True])
+@pytest.mark.parametrize("big", [False, True, "tridiag", "tridiag_grid"])
 def test_solve_is_cuda_graph_capturable(big):
     # the whole solve enqueues kernels and memsets only (no host sync): capture once, replay many times.
     # big: N = 896 has 4 panel pairs, so step 4 runs its two-stream look-ahead schedule inside the capture.
-    if big:
+    # tridiag: M = 256, step 2's tridiagonal route with one cluster per slice; tridiag_grid: M = 900, its persistent
+    # cooperative grid (a cooperative launch inside the capture)
+    if big == "tridiag":
+        p = gen.small_problem(896, 1e-3, 16.0, seed=606)
+        c = gen.Config(-1, "graph", 896, 4, 16, 2, 1e-3, 16.0)
+    elif big == "tridiag_grid":
+        p = gen.small_problem(1800, 1e-3, 16.0, seed=607)
+        c = gen.Config(-1, "graph", 1800, 2, 0, 1, 1e-3, 16.0)
+    elif big:
         p = gen.small_problem(896, 1e-3, 16.0, seed=606)
         c = gen.Config(-1, "graph", 896, 7, 16, 2, 1e-3, 16.0)
     else:
