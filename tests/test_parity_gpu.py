@@ -687,8 +687,9 @@ def gpu_warm(A, Vr_prev, P, w, iters, alpha):
     return out
 
 
-def test_warm_start_sequence_matches_oracle():
-    N, P, w, iters = 384, 4, 24, 3
+@pytest.mark.parametrize("P", [4, 2])    # M = 144 (Jacobi in step 2) and M = 240 (the tridiagonal route)
+def test_warm_start_sequence_matches_oracle(P):
+    N, w, iters = 384, 24, 3
     d = np.sort(gen.uniform(83, gen.STREAM_TEST, 0, N) * 2 - 1)
     X = gen.normal(83, gen.STREAM_TEST, 10_000, N * N).reshape(N, N)
     Q, _ = np.linalg.qr(X)
