@@ -464,27 +464,33 @@ tri_bisect_kernel(int32_t M, SliceTable tab, TriWs ws, int32_t s_off) {
         // sign opposite to its predecessor; both members are rescaled every four rows against over/underflow
         double p0 = 1.0, p1 = d[0] - mid;
         if (p1 == 0.0) p1 = -pivmin;
-        int cnt = p1 < 0.0 ? 1 : 0;
-        for (int i = 1; i < M; ++i) {
+        unsigned int cnt = p1 < 0.0 ? 1u : 0u;
+        auto step = [&](int i) {
             double p2 = fma(d[i] - mid, p1, -e2[i - 1] * p0);
             if (p2 == 0.0) p2 = -copysign(fmax(fabs(p1), 1e-280) * 1e-20, p1);
-            cnt += ((p2 < 0.0) != (p1 < 0.0)) ? 1 : 0;
+            cnt += ((unsigned int)(__double2hiint(p2) ^ __double2hiint(p1))) >> 31;  // sign change
             p0 = p1;
             p1 = p2;
-            if ((i & 3) == 0) {
-                const double a = fmax(fabs(p0), fabs(p1));
-                if (a > 1e120) {
-                    p0 *= 1e-120;
-                    p1 *= 1e-120;
-                } else if (a < 1e-120) {
-                    p0 *= 1e120;
-                    p1 *= 1e120;
-                }
+        };
+        int i = 1;
+        for (; i + 3 < M; i += 4) {
+            step(i);
+            step(i + 1);
+            step(i + 2);
+            step(i + 3);
+            const double a = fmax(fabs(p0), fabs(p1));
+            if (a > 1e120) {
+                p0 *= 1e-120;
+                p1 *= 1e-120;
+            } else if (a < 1e-120) {
+                p0 *= 1e120;
+                p1 *= 1e120;
             }
         }
+        for (; i < M; ++i) step(i);
         // first probe with more than `rank` eigenvalues below it bounds the eigenvalue from above, its left neighbour
         // (or the old lo) from below
-        const unsigned above = __ballot_sync(0xffffffffu, cnt > rank);
+        const unsigned above = __ballot_sync(0xffffffffu, (int)cnt > rank);
         const int f = above ? __ffs(above) - 1 : 32;
         const double nhi = __shfl_sync(0xffffffffu, mid, f & 31), nlo = __shfl_sync(0xffffffffu, mid, (f + 31) & 31);
         const double olo = lo, ohi = hi;
