@@ -1,13 +1,14 @@
 // kernels.cuh -- the non-GEMM kernels of the PFSM path (sm_100a):
-//   jacobi_batched_kernel   step 2, fallback for submatrices too large for shared memory: a cluster of CTAs per
-//                           slice, one-sided (Hestenes) Jacobi on the slice's shifted submatrix kept in L2,
-//                           round-robin parallel ordering, a warp per column pair (the shared-memory resident
-//                           kernel every BASELINE config uses is jacobi_smem.cuh)
+//   jacobi_batched_kernel   step 2, second route (PFSM_JACOBI=1) for submatrices too large for shared memory: a cluster
+//                           of CTAs per slice, one-sided (Hestenes) Jacobi on the slice's shifted submatrix kept in L2,
+//                           round-robin parallel ordering, a warp per column pair.  (The product path of step 2 is
+//                           jacobi_smem.cuh up to M = 160 and tridiag_eig.cuh above.)
 //   chol_diag_kernel        step 4: Cholesky factor + inverse of one 128 x 128 diagonal block
 //   extract_diag_kernel     step 4: diag(V^T V) for the breakdown threshold
 //   transpose_kernel        step 4: V <-> V^T staging for the stacked Cholesky-QR
 //   rayleigh_kernel         step 5: lambda_i = v_i . t_i and r_i = ||t_i - lambda_i v_i||
 //   symmetrize_kernel, transpose_blocks_kernel, inv_diag_kernel   row G / Eq. 14 helpers
+//   mirror_lower_kernel     pfsm_solve_host: upper block triangle of A from the uploaded lower one
 //   fp64 peak probes        roofline calibration
 #pragma once
 #include <cuda_runtime.h>
