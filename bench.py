@@ -24,9 +24,10 @@ if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
 FP64_NOMINAL_RATIO = 45.0 / 2250.0  # guide's nominal B200 FP64-tensor : bf16-tensor dense peaks
-# dram__bytes_read.sum + dram__bytes_write.sum per full-k gemm_tn_kernel launch, from the committed
-# `ncu --set full` capture profiles/r01c_ncu_full_gemm_final.md (config index -> bytes); None = not captured
-NCU_TRAFFIC_PER_GEMM_LAUNCH = {4: 8.14e9 + 0.53e9}
+# dram__bytes_read.sum + dram__bytes_write.sum per full-k gemm_tn_kernel launch.  NOT measured in this run: ncu cannot
+# run inside a timed bench, so the figure is copied from a committed `ncu --set full` capture of the same kernel at the
+# same config (config index -> (bytes, file)); configs without a capture report null.
+NCU_TRAFFIC_PER_GEMM_LAUNCH = {4: (8.14e9 + 0.53e9, "profiles/r01c_ncu_full_gemm_final.md")}
 
 
 def algorithmic_flops(N: int, M: int, iters: int) -> dict:
@@ -147,6 +148,25 @@ def oracle_sample(cfg_index: int, ncols: int, reps: int, warmup: int, min_second
     return times, flops, desc, oracle.num_threads()
 
 
+def whole_oracle_record(k: int, total_flops: float):
+    """Wall time of ONE whole oracle solve (O1-O5, every eigenvector) of config k, recorded by
+    tests/golden/make_golden_large.py when it wrote the config's golden file -- on the BUILD box, not on this host, so
+    it is context beside the sampled figure, with its thread count.  None when the config has no such record."""
+    path = os.path.join(ROOT, "tests", "golden", f"config{k}_oracle.txt")
+    if not os.path.exists(path):
+        return None
+    rec = {}
+    for ln in open(path):
+        f = ln.split()
+        if len(f) == 2 and f[0] in ("oracle_wall_s", "oracle_threads"):
+            rec[f[0]] = float(f[1])
+    if "oracle_wall_s" not in rec:
+        return None
+    return {"wall_s": rec["oracle_wall_s"], "threads": int(rec.get("oracle_threads", 0)),
+            "tflops": total_flops / rec["oracle_wall_s"] * 1e-12,
+            "where": "build box (recorded in tests/golden/config%d_oracle.txt), not this host" % k}
+
+
 def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
@@ -154,7 +174,7 @@ def run_reference(args):
     k = args.config
     import pfsm_inputs as gen
     c = gen.config(k)
-    times, flops, desc, threads = oracle_sample(k, args.ref_cols, args.steps, args.warmup)
+    times, flops, desc, threads = oracle_sample(k, args.cpu_cols if args.cpu_cols > 0 else 128, args.steps, args.warmup)
     total = sum(times)
     value = flops * len(times) / total * 1e-12
     line = {
@@ -172,12 +192,13 @@ def run_reference(args):
     return 0
 
 
-def workload_config(c, n_gpus: int, sharded: bool = False) -> dict:
+def workload_config(c, n_gpus: int, sharded: bool = False, opts=None) -> dict:
     origin = f"BASELINE.json configs[{c.index}]" if c.index <= 4 else "extra (SURVEY 8(f) f4)"
     return {"workload": f"{origin}: {c.name}, synthetic A = D + E",
             "N": c.N, "P": c.P, "window": c.window, "M": c.M, "iters": c.iters,
-            "alpha": "0.5/max|d|^2", "replicas": n_gpus, "parallelism": (f"one solve sharded over {n_gpus} ranks (all-gathers between the 4 phases)" if sharded
-                            else f"replicas x{n_gpus}"),
+            "alpha": "0.5/max|d|^2", "replicas": 1 if sharded else n_gpus, "options": opts or "defaults (product path)",
+            "parallelism": (f"one solve sharded over {n_gpus} ranks (slices -> ranks, 4 all-gathers around step 4)" if sharded
+                            else ("single GPU" if n_gpus == 1 else f"replicas x{n_gpus} (independent solves, no collective)")),
             "l2_policy": f"inputs larger than L2 (A, V, W are {8 * c.N * c.N / 2**20:.0f} MiB each vs 126 MB L2)"
             if 8 * c.N * c.N > 126e6 else "L2 flushed between timed iterations (256 MiB write)"}
 
@@ -191,6 +212,9 @@ def run_ours(args):
     from paper_1502_07806_b200 import replicas
 
     world, rank, local_rank = replicas.env_world()
+    if world != args.gpus:
+        raise SystemExit(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={world}; launch with torchrun --nproc-per-node "
+                         f"{args.gpus}, or without WORLD_SIZE set (bench.py then starts the ranks itself)")
     if not torch.cuda.is_available():
         raise RuntimeError("bench.py needs a CUDA device: the PFSM path has no CPU fallback")
     torch.cuda.set_device(local_rank)
@@ -198,14 +222,18 @@ def run_ours(args):
     n_gpus = world
 
     k = args.config
-    # replicas only: rank r solves an independent matrix of the same config
-    sharded_mode = bool(args.sharded) and world > 1
-    # default: replicas (rank r solves an independent matrix); --sharded: ONE solve split over the ranks (f3)
+    # N > 1 default: ONE solve sharded over the ranks (strong scaling, all-gathers around step 4);
+    # --replicas: rank r solves an independent matrix of the same config (weak scaling, no data-path collective)
+    sharded_mode = world > 1 and not args.replicas
     prob = gen.problem(k, seed_offset=0 if sharded_mode else replicas.replica_seed_offset(rank))
     c = prob.cfg
     N = c.N
     flops = algorithmic_flops(N, c.M, c.iters)
-    h = pfsm.Handle(N, c.P, c.window, c.iters, prob.alpha)
+    opts = {}
+    for kv in args.option:
+        key, _, val = kv.partition("=")
+        opts[key] = int(val)
+    h = pfsm.Handle(N, c.P, c.window, c.iters, prob.alpha, options=opts)
     if sharded_mode:
         from paper_1502_07806_b200 import sharded
         h.set_shard(rank, world)
@@ -240,44 +268,82 @@ def run_ours(args):
         solve_once()
     barrier()
     assert replicas.all_ok(h.info() == 0, world, "cuda"), "PFSM reported a numerical breakdown on a bench matrix"
-    h.enable_step_timing(True)
     sampler = ClockSampler(local_rank)
     sampler.start()
     time.sleep(0.3)
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-    step_ms = np.zeros(4)
     barrier()
     t_wall0 = time.time()
+    # headline loop: the product launch sequence, step timing OFF (events between the steps would un-chain the Gram
+    # product of step 4 from the last step-3 GEMM)
     for i in range(args.steps):
         if flush is not None:
             flush.fill_(i & 0xFF)
         ev[i][0].record(stream)
         solve_once()
         ev[i][1].record(stream)
-        if flush is not None or True:
-            # per-step device times are read back after each solve (events are already recorded; this sync
-            # sits outside the [start, stop] event pair of the step)
+    barrier()
+    solve_ms = [a.elapsed_time(b) for a, b in ev]
+    # second pass of the same K solves with the library's per-step events on: step times and the dominant kernel's
+    # average launch duration (still inside the clock-sampled region, not part of `value`)
+    step_ms = np.zeros(4)
+    timed_ms = []
+    phase_ms = {}
+    if sharded_mode:
+        marks = []
+
+        def mark(label):
+            e = torch.cuda.Event(enable_timing=True)
+            e.record(stream)
+            marks.append((label, e))
+        for i in range(args.steps):
+            sharded.solve_sharded(h, dA, dV, dl, mark=mark)
+        torch.cuda.synchronize()
+        per = len(marks) // args.steps
+        for i in range(args.steps):
+            seg = marks[i * per:(i + 1) * per]
+            for (la, ea), (lb, eb) in zip(seg[:-1], seg[1:]):
+                phase_ms[lb] = phase_ms.get(lb, 0.0) + ea.elapsed_time(eb) / args.steps
+        phase_ms = {kk: max_over_ranks(v) for kk, v in phase_ms.items()}
+    else:
+        h.enable_step_timing(True)
+        for i in range(args.steps):
+            if flush is not None:
+                flush.fill_(i & 0xFF)
+            ev[i][0].record(stream)
+            solve_once()
+            ev[i][1].record(stream)
             ev[i][1].synchronize()
-            if not sharded_mode:
-                step_ms += np.array(h.step_ms())
+            step_ms += np.array(h.step_ms())
+            timed_ms.append(ev[i][0].elapsed_time(ev[i][1]))
+        h.enable_step_timing(False)
+        step_ms /= args.steps
     barrier()
     t_wall1 = time.time()
     clocks = sampler.stop(t_wall0, t_wall1)
-    h.enable_step_timing(False)
-    solve_ms = [a.elapsed_time(b) for a, b in ev]
     total_ms = max_over_ranks(float(sum(solve_ms)))
     ms_per_step = total_ms / args.steps
-    step_ms /= args.steps
     value = replicas.aggregate_tflops(flops["total"], args.steps, 1 if sharded_mode else world, total_ms)
 
-    # ---- end-to-end leg: host buffers through pfsm_solve_host, copies inside the timed region ----
+    # ---- end-to-end leg: host buffers, copies inside the timed region.  One GPU / replicas: pfsm_solve_host (the
+    # library overlaps the copies with steps 2 and 5).  Sharded: every rank uploads the replicated A, runs the sharded
+    # solve and reads the complete V and lambda back.
+    def e2e_once():
+        if sharded_mode:
+            dA.copy_(A_host, non_blocking=True)
+            sharded.solve_sharded(h, dA, dV, dl)
+            V_host.copy_(dV, non_blocking=True)
+            lam_host.copy_(dl, non_blocking=True)
+        else:
+            h.solve_host(A_host, V_host, lam_host)
+
     e2e_steps = max(1, min(args.steps, 3))
-    h.solve_host(A_host, V_host, lam_host)
+    e2e_once()
     barrier()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record(stream)
     for _ in range(e2e_steps):
-        h.solve_host(A_host, V_host, lam_host)
+        e2e_once()
     e1.record(stream)
     barrier()
     e2e_ms = max_over_ranks(e0.elapsed_time(e1)) / e2e_steps
@@ -299,24 +365,48 @@ def run_ours(args):
         return 0
 
     # ---- roofline of the dominant kernel (gemm_tn_kernel in step 3), live CUDA-event times ----
+    # peak = the FP64 tensor (DMMA) issue rate measured in THIS run by the library's register-only probe: MEASURED_PEAKS.json
+    # holds no FP64 figure, and the rule "bf16 measured x nominal ratio" (kept as proxy_*) cannot bound this pipe -- it is
+    # scaled from a power-capped bf16 run at ~1.26 GHz while FP64 holds the full SM clock.
     peaks = measured_peaks()
     n_launch3 = 2 * c.iters
-    gemm_ms = step_ms[1] / max(1, n_launch3)
-    achieved = flops["step3"] / max(1, n_launch3) / (gemm_ms * 1e-3) * 1e-12 if n_launch3 else 0.0
-    peak = peaks["bf16_tflops_sustained"] * FP64_NOMINAL_RATIO
+    if sharded_mode:
+        gemm_ms = phase_ms["phase1_steps2_3"] / max(1, n_launch3)
+        flops_per_launch = flops["step3"] / max(1, n_launch3) / world
+    else:
+        gemm_ms = step_ms[1] / max(1, n_launch3)
+        flops_per_launch = flops["step3"] / max(1, n_launch3)
+    achieved = flops_per_launch / (gemm_ms * 1e-3) * 1e-12 if n_launch3 and gemm_ms > 0 else 0.0
+    probe_peak = pfsm.probe_fp64_peak(0)
+    proxy_peak = peaks["bf16_tflops_sustained"] * FP64_NOMINAL_RATIO
+    sms = torch.cuda.get_device_properties(local_rank).multi_processor_count
+    clk_ghz = (clocks.get("sm_max_mhz") or 0.0) * 1e-3
+    pipe_peak = sms * 64 * 2 * clk_ghz * 1e-3   # SMs x 64 FP64 FMA/clk/SM x 2 flop x max SM clock
+    traffic = NCU_TRAFFIC_PER_GEMM_LAUNCH.get(k) if not sharded_mode else None
     roofline = {
-        "bound": "tensor", "kernel": "gemm_tn_kernel (step 3, FP64 DMMA)", "achieved": achieved, "peak": peak,
-        "unit": "TFLOP/s", "frac": achieved / peak, "traffic": NCU_TRAFFIC_PER_GEMM_LAUNCH.get(k),
+        "bound": "tensor", "kernel": "gemm_tn_kernel (step 3, FP64 DMMA)", "achieved": achieved, "peak": probe_peak,
+        "unit": "TFLOP/s", "frac": achieved / probe_peak if probe_peak > 0 else None,
+        "traffic": traffic[0] if traffic else None,
+        "traffic_source": (f"ncu --set full capture {traffic[1]} (same kernel, same config; NOT measured in this run)"
+                           if traffic else "null: no committed ncu capture for this config / mode"),
         "algorithmic_bytes_per_launch": 32.0 * N * N,
-        "peak_source": f"{peaks['_source']} bf16_tflops_sustained x nominal FP64:bf16 ratio 45/2250 (of {peaks['_source']})",
-        "fp64_pipe_peak_tflops": 148 * 64 * 2 * 1.965e-3,  # 148 SMs x 64 FP64 FMA/clk x 2 flop x 1.965 GHz
-        "frac_of_fp64_pipe": achieved / (148 * 64 * 2 * 1.965e-3),
-        "avg_launch_ms": gemm_ms, "launches_per_step": n_launch3,
-        "flops_per_launch": flops["step3"] / max(1, n_launch3),
+        "peak_source": "FP64 DMMA issue-rate probe (pfsm_probe_fp64_peak, register-only mma.sync m8n8k4 f64 on every SM) "
+                       "measured in this run; MEASURED_PEAKS.json has no FP64 entry",
+        "fp64_pipe_peak_tflops": pipe_peak, "fp64_pipe_peak_rule": f"{sms} SMs x 64 FMA/clk x 2 x {clk_ghz:.3f} GHz",
+        "frac_of_fp64_pipe": achieved / pipe_peak if pipe_peak > 0 else None,
+        "proxy_peak": proxy_peak, "frac_vs_proxy": achieved / proxy_peak,
+        "proxy_peak_rule": f"{peaks['_source']} bf16_tflops_sustained x nominal FP64:bf16 ratio 45/2250 (under-states the "
+                           "FP64 pipe: secondary figure)",
+        "avg_launch_ms": gemm_ms, "launches_per_step": n_launch3, "flops_per_launch": flops_per_launch,
+        "note": ("achieved = algorithmic step-3 flops per launch / average launch time from the library's per-step CUDA "
+                 "events, taken in a second pass of the same K solves; the headline `value` loop runs with step timing "
+                 "off (the product launch sequence: step 4's Gram product chained to the last step-3 GEMM)"
+                 if not sharded_mode else
+                 "sharded: achieved = this rank's share of the step-3 flops / phase-1 time (phase 1 also holds step 2)"),
     }
     extra = {}
     if args.calibrate:
-        extra["fp64_dmma_issue_peak_tflops"] = pfsm.probe_fp64_peak(0)
+        extra["fp64_dmma_issue_peak_tflops"] = probe_peak
         extra["fp64_dfma_issue_peak_tflops"] = pfsm.probe_fp64_peak(1)
         a = torch.randn(8192, 8192, dtype=torch.float64, device="cuda")
         for _ in range(2):
@@ -372,32 +462,51 @@ def run_ours(args):
         import oracle
         cpu_times, cpu_value, cpu_desc, threads = [0.0], None, "skipped (--cpu-cols 0)", oracle.num_threads()
 
+    whole = whole_oracle_record(k, flops["total"])
     line = {
         "metric": "PFSM solve sustained FP64 TFLOP/s (algorithmic flops / solve time)",
         "value": value, "unit": "TFLOP/s", "n_gpus": n_gpus, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "strong" if sharded_mode else "weak",
         "vs_baseline": None,
-        "dtype": "f64", "data": "synthetic", "config": workload_config(c, n_gpus, sharded_mode),
+        "dtype": "f64", "data": "synthetic", "config": workload_config(c, n_gpus, sharded_mode, opts),
         "solve_ms": {"median": float(np.median(solve_ms)), "best": float(min(solve_ms))},
-        "step_ms": {"step2_submatrix_eig": step_ms[0], "step3_folded_spectrum": step_ms[1],
-                    "step4_cholesky_qr": step_ms[2], "step5_rayleigh": step_ms[3]},
+        "step_ms": ({"step2_submatrix_eig": step_ms[0], "step3_folded_spectrum": step_ms[1],
+                     "step4_cholesky_qr": step_ms[2], "step5_rayleigh": step_ms[3],
+                     "solve_with_step_events_median": float(np.median(timed_ms))} if not sharded_mode else phase_ms),
         "algorithmic_flops": flops, "quality": quality, "clocks": clocks,
         "e2e": {"value": e2e_value, "unit": "TFLOP/s", "ms_per_step": e2e_ms,
                 # the lower block triangle of A (256-row blocks; A = A^T, mirrored on the device), plus the P diagonal
                 # blocks sent ahead for step 2 (not when they are as large as A: wide windows)
-                "h2d_bytes_per_step": 8 * sum(min(256, N - r0) * min(N, r0 + 256) for r0 in range(0, N, 256))
-                + (8 * c.P * c.M * c.M if (c.M <= 160 or 2 * c.P * c.M * c.M <= N * N) else 0),
+                "h2d_bytes_per_step": (8 * N * N if sharded_mode else
+                                       8 * sum(min(256, N - r0) * min(N, r0 + 256) for r0 in range(0, N, 256))
+                                       + (8 * c.P * c.M * c.M if (c.M <= 160 or 2 * c.P * c.M * c.M <= N * N) else 0)),
                 "d2h_bytes_per_step": 8 * N * N + 8 * N},
         "gpu_launches": int(args.steps * h.launches_per_solve()),
         "roofline": roofline,
         "cpu_baseline": {"value": cpu_value, "unit": "TFLOP/s", "cores": threads, "kind": "oracle",
-                         "sample": cpu_desc, "seconds": sum(cpu_times)},
+                         "sample": cpu_desc, "seconds": sum(cpu_times), "whole_oracle_solve": whole},
         "workspace_bytes": h.workspace_bytes(),
     }
     line.update(extra)
     print(json.dumps(line))
     replicas.finalize(world)
     return 0
+
+
+def self_launch(args) -> int:
+    """`python bench.py --gpus N` without a launcher: start the N ranks under torchrun exactly as the driver would
+    (one process per GPU, NCCL over NVLink), and pass its exit code on.  The ranks see WORLD_SIZE and run the bench."""
+    import socket
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    port = s.getsockname()[1]
+    s.close()
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__), *sys.argv[1:]]
+    env = dict(os.environ)
+    env.setdefault("NCCL_DEBUG", "INFO")          # rank / transport lines stay on stderr so a driver can count ranks
+    env.setdefault("NCCL_DEBUG_SUBSYS", "INIT")
+    return subprocess.call(cmd, env=env)
 
 
 def main():
@@ -407,19 +516,24 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=4, help="BASELINE.json config index (default 4: N=8192); extra cases: 5 = Cu256-shaped N=1664, 6 = config 4 shape at gamma = 0.25 (M = 2048)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--cpu-cols", type=int, default=128, help="eigenvectors in the cpu_baseline sample (0 = skip the CPU leg)")
+    ap.add_argument("--cpu-cols", type=int, default=128, help="eigenvectors in the oracle sample that both the cpu_baseline leg and --impl reference time (0 = skip the CPU leg)")
     ap.add_argument("--cpu-seconds", type=float, default=12.0, help="repeat the cpu_baseline sample until this much CPU time is timed (max 8 repeats)")
-    ap.add_argument("--ref-cols", type=int, default=8, help="eigenvectors per step of --impl reference")
-    ap.add_argument("--sharded", action="store_true",
-                    help="N>1: split ONE solve over the ranks (strong scaling) instead of independent replicas")
+    ap.add_argument("--replicas", action="store_true",
+                    help="N>1: independent replicas (rank r solves its own matrix; weak scaling, no collective) instead of "
+                         "the default, ONE solve sharded over the ranks (strong scaling)")
+    ap.add_argument("--sharded", action="store_true", help="accepted for compatibility: sharding is the N>1 default")
     ap.add_argument("--generalized", action="store_true",
                     help="also time pfsm_solve_generalized on the config's matrix with S = I + 1e-4 perturbation (row G)")
+    ap.add_argument("--option", action="append", default=[], metavar="KEY=INT",
+                    help="pfsm_set_option setting for A/B measurements (include/pfsm.h lists the keys); default: product path")
     ap.add_argument("--no-syevd", dest="syevd", action="store_false")
     ap.add_argument("--no-calibrate", dest="calibrate", action="store_false")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
         return run_reference(args)
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        return self_launch(args)
     return run_ours(args)
 
 

@@ -69,6 +69,9 @@ typedef struct pfsm_ctx* pfsm_handle_t; /* opaque */
  *   alpha   step length of Eq. 11; finite and > 0.  The library does not estimate spectra:
  *           alpha = 0.5 / max|lambda|^2 keeps every damping factor 1 - alpha (lambda - eps)^2 in [-1, 1].
  * Errors: -1..-6 for the corresponding argument; 1000+cudaError on allocation failure.
+ * A handle belongs to the device that was current at pfsm_create: every later call that enqueues work returns
+ * 1000+cudaErrorInvalidDevice if another device is current.  Handles on different devices (or streams) are independent;
+ * no state is shared between handles.
  */
 int pfsm_create(pfsm_handle_t* out, int64_t N, int32_t P, int32_t window, int32_t iters, double alpha);
 
@@ -176,7 +179,8 @@ int pfsm_shard_buffer(pfsm_handle_t h, int32_t which, double** device_ptr);
 int pfsm_destroy(pfsm_handle_t h);
 
 /*
- * Numerical status of the last solve; synchronizes `stream` (the stream that solve was enqueued on).
+ * Numerical status of the last solve; synchronizes `stream` (the stream that solve was enqueued on -- the one argument
+ * this call adds to SURVEY.md 8(b)'s proposed signature: the handle does not remember streams, the caller owns them).
  *   *info = 0        success
  *   1 <= *info <= N  Cholesky pivot *info of V^T V was not positive (<= 1e-12 x its original diagonal
  *                    entry): the N vectors are numerically
@@ -219,6 +223,26 @@ int pfsm_get_shifts(pfsm_handle_t h, const double** eps_device);
  * the Gram-Schmidt basis in ascending column order, is the same.
  */
 int pfsm_set_cholqr_passes(pfsm_handle_t h, int32_t passes);
+
+/*
+ * Select among kernels / schedules that compute the same result.  Explicit per-handle state: the library reads no
+ * environment variable.  Defaults (all 0 except where noted) are the product path; the other values exist for A/B
+ * measurements and so that the parity tests reach every kernel.  Call between solves (not while one is in flight).
+ *   key (host C string)      value
+ *   "step2_route"            0 auto (M <= 160 shared-memory Jacobi, else tridiagonal route), 1 Jacobi family (M <= 512),
+ *                            2 tridiagonal route at any M, 3 persistent-grid Jacobi at any M        [PAPER.md:86-94]
+ *   "jacobi_l2"              1: the L2-resident Jacobi kernel instead of the shared-memory one
+ *   "jacobi_cluster_size"    0 auto, or 1 | 2 | 4 | 8 CTAs per slice for the shared-memory Jacobi
+ *   "jacobi_full_cta"        1: never use the half-CTA layout of the shared-memory Jacobi
+ *   "sytrd_storage"          0 auto (lower triangle once the batch exceeds L2), 1 full storage, 2 lower triangle
+ *   "sytrd_grid_barrier"     1: grid barrier instead of thread-block clusters for small M
+ *   "cholesky_lookahead"     default 1; 0: step 4 on one stream                                    [PAPER.md:94-96]
+ *   "chain_launches"         default 1; 0: the step-3 / step-4 GEMMs in plain stream order (same bits)
+ *   "cholqr_passes"          as pfsm_set_cholqr_passes (1 | 2)
+ * May allocate workspace (a newly selected route).  Errors: -1 handle, -2 unknown key, -3 value out of range,
+ * 1000+cudaError.
+ */
+int pfsm_set_option(pfsm_handle_t h, const char* key, int64_t value);
 
 /* Change alpha (it scales with 1/||A||^2, so it changes when the spectrum's extent does). */
 int pfsm_set_alpha(pfsm_handle_t h, double alpha);

@@ -21,7 +21,7 @@ EXPORTS = [
     "pfsm_create", "pfsm_solve", "pfsm_solve_host", "pfsm_solve_partial", "pfsm_orthonormalize", "pfsm_rayleigh", "pfsm_solve_generalized",
     "pfsm_generalized_reduce", "pfsm_solve_warm", "pfsm_standard_form_eq14",
     "pfsm_set_shard", "pfsm_shard_phase", "pfsm_shard_buffer", "pfsm_destroy", "pfsm_get_info", "pfsm_check_validity",
-    "pfsm_get_step2_sweeps", "pfsm_get_residuals", "pfsm_get_shifts", "pfsm_set_alpha", "pfsm_set_cholqr_passes", "pfsm_workspace_bytes",
+    "pfsm_get_step2_sweeps", "pfsm_get_residuals", "pfsm_get_shifts", "pfsm_set_alpha", "pfsm_set_cholqr_passes", "pfsm_set_option", "pfsm_workspace_bytes",
     "pfsm_launches_per_solve", "pfsm_enable_step_timing", "pfsm_get_step_ms", "pfsm_probe_fp64_peak",
     "pfsm_strerror",
 ]
@@ -69,6 +69,7 @@ def load(build_if_missing: bool = True):
     lib.pfsm_get_shifts.argtypes = [p, ctypes.POINTER(p)]
     lib.pfsm_set_alpha.argtypes = [p, dbl]
     lib.pfsm_set_cholqr_passes.argtypes = [p, i32]
+    lib.pfsm_set_option.argtypes = [p, ctypes.c_char_p, i64]
     lib.pfsm_workspace_bytes.argtypes = [p]
     lib.pfsm_workspace_bytes.restype = ctypes.c_size_t
     lib.pfsm_launches_per_solve.argtypes = [p]
@@ -120,7 +121,7 @@ def _host_ptr(t, shape, name):
 class Handle:
     """Owns a pfsm_handle_t.  Mirrors the C ABI one to one; see include/pfsm.h for semantics."""
 
-    def __init__(self, N: int, P: int, window: int, iters: int, alpha: float):
+    def __init__(self, N: int, P: int, window: int, iters: int, alpha: float, options: dict | None = None):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("paper_1502_07806_b200 needs a CUDA device (sm_100a); there is no CPU fallback")
@@ -128,6 +129,8 @@ class Handle:
         self._h = ctypes.c_void_p()
         _check(self._lib.pfsm_create(ctypes.byref(self._h), N, P, window, iters, alpha), "pfsm_create")
         self.N, self.P, self.window, self.iters, self.alpha = N, P, window, iters, alpha
+        for key, value in (options or {}).items():
+            self.set_option(key, value)
 
     def solve(self, A, Vr, lam, stream=None):
         N = self.N
@@ -251,6 +254,9 @@ class Handle:
     def set_alpha(self, alpha: float):
         _check(self._lib.pfsm_set_alpha(self._h, alpha), "pfsm_set_alpha")
         self.alpha = alpha
+
+    def set_option(self, key: str, value: int):
+        _check(self._lib.pfsm_set_option(self._h, key.encode(), int(value)), f"pfsm_set_option({key!r}, {value})")
 
     def set_cholqr_passes(self, passes: int):
         _check(self._lib.pfsm_set_cholqr_passes(self._h, passes), "pfsm_set_cholqr_passes")

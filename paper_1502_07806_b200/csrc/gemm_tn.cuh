@@ -70,6 +70,10 @@ struct GemmParams {
     const int32_t* wait_cnt;
     int32_t wait_target;
     int32_t* signal_cnt;
+    // Batch of independent products in one launch (the per-slice trailing updates of the blocked tridiagonalization):
+    // grid = nbatch * tiles_per_batch; batch b shifts the X / Y / C row origins by b * bxs / b * bys / b * bcs rows of the
+    // same tensor maps (the slices' matrices are stacked row-wise).  nbatch <= 1: a single product.
+    int32_t nbatch, tiles_per_batch, bxs, bys, bcs;
 };
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -173,7 +177,13 @@ gemm_tn_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
 
     int32_t tr, tc;
-    if (!tile_coords(p, (int32_t)blockIdx.x, tr, tc)) return;
+    int32_t bidx = (int32_t)blockIdx.x, batch = 0;
+    if (p.nbatch > 1) {
+        batch = bidx / p.tiles_per_batch;
+        bidx -= batch * p.tiles_per_batch;
+    }
+    if (!tile_coords(p, bidx, tr, tc)) return;
+    const int32_t cr0 = p.cr0 + batch * p.bcs;  // C row origin of this batch entry
 
     int32_t kb0 = 0, nk = (p.klen + BK - 1) / BK;
     if (p.krange) {
@@ -211,7 +221,7 @@ gemm_tn_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__
     // ===== TMA producer = lane 0 of warp 0, interleaved with its math.  At the top of iteration kb it
     // refills the stage that every warp finished two iterations ago (k-block kb + PREFETCH), so the
     // wait on that stage's empty barrier almost never blocks and 4 k-blocks stay in flight. =====
-    const int32_t xrow = p.xr0 + tr * BM, yrow = p.yr0 + tc * BN;
+    const int32_t xrow = p.xr0 + batch * p.bxs + tr * BM, yrow = p.yr0 + batch * p.bys + tc * BN;
     auto issue = [&](int32_t j) {
         const int s = j % GEMM_STAGES;
         if (j >= GEMM_STAGES) mbar_wait(bar_base + 8 * (GEMM_STAGES + s), ((j / GEMM_STAGES) - 1) & 1);
@@ -230,7 +240,7 @@ gemm_tn_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__
 #pragma unroll
         for (int j = 0; j < BN / BK; ++j)
             asm volatile("cp.async.bulk.prefetch.tensor.2d.L2.global.tile [%0, {%1, %2}];" ::"l"(&mapC),
-                         "r"(p.cc0 + tc * BN + j * BK), "r"(p.cr0 + tr * BM)
+                         "r"(p.cc0 + tc * BN + j * BK), "r"(cr0 + tr * BM)
                          : "memory");
     }
 
@@ -290,7 +300,7 @@ gemm_tn_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__
     if (EPI != EPI_PLAIN && (tr + 1) * BM <= p.mr && (tc + 1) * BN <= p.nc) {
         // Interior tile: no bounds checks, and the epilogue operands are fetched 16 x 16 bytes at a time before
         // they are used -- 2 memory round trips per thread instead of 32 dependent load -> store chains.
-        const int64_t base = ((int64_t)p.cr0 + row0 + g) * p.ldc + p.cc0 + col0 + 2 * t;  // ldc == ld1 == ld2 here
+        const int64_t base = ((int64_t)cr0 + row0 + g) * p.ldc + p.cc0 + col0 + 2 * t;  // ldc == ld1 == ld2 here
         double2 dj[4];
         if (EPI == EPI_JSTEP) {
 #pragma unroll
@@ -303,7 +313,7 @@ gemm_tn_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__
 #pragma unroll
             for (int i = 0; i < 4; ++i) {
                 const int64_t o = base + (int64_t)(8 * (ib + i)) * p.ldc;
-                if (EPI == EPI_SHIFT || EPI == EPI_UPDATE) e[i] = p.eps[(int64_t)p.cr0 + row0 + 8 * (ib + i) + g];
+                if (EPI == EPI_SHIFT || EPI == EPI_UPDATE) e[i] = p.eps[(int64_t)cr0 + row0 + 8 * (ib + i) + g];
 #pragma unroll
                 for (int j = 0; j < 4; ++j) {
                     if (EPI == EPI_SHIFT || EPI == EPI_UPDATE || EPI == EPI_JSTEP)
@@ -342,7 +352,7 @@ gemm_tn_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__
     for (int i = 0; i < 8; ++i) {
         const int32_t r = row0 + 8 * i + g;
         if (r >= p.mr) continue;
-        const int64_t ar = (int64_t)p.cr0 + r;
+        const int64_t ar = (int64_t)cr0 + r;
         double e = 0.0;
         if (EPI == EPI_SHIFT || EPI == EPI_UPDATE) e = p.eps[ar];
 #pragma unroll

@@ -20,6 +20,7 @@
 #include "jacobi_smem.cuh"
 #include "jacobi_wide.cuh"
 #include "tridiag_eig.cuh"
+#include "sytrd_blocked.cuh"
 
 namespace pfsm {
 
@@ -80,10 +81,11 @@ struct pfsm_ctx {
     int* rotcnt = nullptr;    // P x JACOBI_MAX_SWEEPS rotation counters of step 2
     unsigned int* jw_bar = nullptr;  // grid-barrier counter of the wide-window Jacobi (M > 512)
     double* nrm_g = nullptr;  // P x (M + 16): final column norms of the shared-memory Jacobi
-    bool jac_wide = false;             // wide-window Jacobi (jacobi_wide.cuh): PFSM_JACOBI_WIDE=1, at any M
-    bool tridiag = false;              // tridiagonalization route (tridiag_eig.cuh): default for M > 512, PFSM_TRIDIAG=1 at any M
+    bool jac_wide = false;             // persistent-grid Jacobi (jacobi_wide.cuh): option step2_route = 3, at any M
+    bool tridiag = false;              // tridiagonalization route (tridiag_eig.cuh): default for M > 160, step2_route = 2 at any M
     TriWs tri{};                       // its workspace
-    bool sytrd_full = false, sytrd_half = false;  // PFSM_SYTRD_FULL=1 / PFSM_SYTRD_HALF=1: force one of the two tridiagonalization kernels
+    SbWs sbw{};                        // workspace of the blocked tridiagonalization (sytrd_blocked.cuh), allocated on first use
+    CUtensorMap mapG, mapVW, mapWV;    //   its tensor maps: the stacked submatrices (P M x M) and panel operands (P M x 2 NB)
     int jac_cs = 0, jac_hloc = 0;  // cluster size / seats per CTA of the shared-memory Jacobi (0 = L2 kernel)
     double* gdiag = nullptr;  // N: diag(V^T V) before the factorization (breakdown threshold)
     int32_t* slice_tab = nullptr;  // g0[P], lo[P], off[P], cnt[P]
@@ -112,6 +114,18 @@ struct pfsm_ctx {
     int32_t cholqr_passes = 1;         // 2 = CholeskyQR2 (re-orthonormalize once; reading R10)
     bool jac_half = false;             // shared-memory Jacobi with 512-thread CTAs, two per SM (jacobi_smem.cuh)
     int32_t sh_rank = 0, sh_world = 1;  // sharded solve: this handle works on rows [sh_rank, sh_rank+1) * N / sh_world
+    // per-handle launch state (function attributes are per device/context, so nothing here is a process-wide static)
+    int sms = 0;                       // multiprocessors of h->device
+    bool gemm_attr[5] = {false, false, false, false, false};  // MaxDynamicSharedMemorySize set for gemm_tn_kernel<EPI>
+    bool pdl_ok = true;                // cleared if the driver refuses programmatic stream serialization
+    bool chol_attr = false;
+    // options (pfsm_set_option; defaults = the product path)
+    int32_t opt_route = 0;             // step2_route: 0 auto, 1 Jacobi family (M <= 512), 2 tridiagonal, 3 persistent-grid Jacobi
+    int32_t opt_jacobi_l2 = 0;         // 1: L2-resident Jacobi kernel instead of the shared-memory one
+    int32_t opt_jacobi_cs = 0;         // cluster size of the shared-memory Jacobi (0 = auto)
+    int32_t opt_jacobi_full = 0;       // 1: no half-CTA layout
+    int32_t opt_sytrd_storage = 0;     // 0 auto, 1 full storage, 2 lower triangle
+    int32_t opt_sytrd_grid = 0;        // 1: grid barrier instead of clusters for small M
 };
 
 static int dev_alloc(pfsm_ctx* h, void** p, size_t bytes) {
@@ -120,24 +134,32 @@ static int dev_alloc(pfsm_ctx* h, void** p, size_t bytes) {
     return 0;
 }
 
+// Every entry point that enqueues work runs on the handle's device: workspace, tensor maps and function attributes
+// belong to it.  A caller that switched devices gets an error instead of a launch on the wrong context.
+static int check_device(const pfsm_ctx* h) {
+    int dev = -1;
+    PFSM_CUDA(cudaGetDevice(&dev));
+    return dev == h->device ? 0 : PFSM_CUDA_ERROR_BASE + (int)cudaErrorInvalidDevice;
+}
+
 // mc: tensor map of the matrix C lives in (used by the SUB / UPDATE epilogues to prefetch the C tile into L2)
 template <int EPI>
 // pdl: launch with programmatic stream serialization -- the grid may become resident while the previous gemm_tn_kernel
 // in the stream drains its last wave; p.wait_cnt must then carry the real dependency (GemmParams).
-static int launch_gemm(const CUtensorMap& mx, const CUtensorMap& my, const CUtensorMap& mc, GemmParams p,
+static int launch_gemm(pfsm_ctx* h, const CUtensorMap& mx, const CUtensorMap& my, const CUtensorMap& mc, GemmParams p,
                        cudaStream_t st, bool pdl = false) {
     p.ntr = (p.mr + BM - 1) / BM;
     p.ntc = (p.nc + BN - 1) / BN;
     if (p.mr <= 0 || p.nc <= 0) return 0;
-    const int64_t tiles = gemm_num_tiles(p.ntr, p.ntc, p.lower);
-    if (tiles <= 0) return 0;
-    static bool attr_set[5] = {false, false, false, false, false};
-    if (!attr_set[EPI]) {
+    const int64_t tiles1 = gemm_num_tiles(p.ntr, p.ntc, p.lower);
+    if (tiles1 <= 0) return 0;
+    p.tiles_per_batch = (int32_t)tiles1;
+    const int64_t tiles = tiles1 * (p.nbatch > 1 ? p.nbatch : 1);
+    if (!h->gemm_attr[EPI]) {
         PFSM_CUDA(cudaFuncSetAttribute(gemm_tn_kernel<EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, GEMM_SMEM));
-        attr_set[EPI] = true;
+        h->gemm_attr[EPI] = true;
     }
-    static bool pdl_ok = true;  // cleared if the driver refuses the attribute: plain stream order is always correct
-    if (pdl && pdl_ok) {
+    if (pdl && h->pdl_ok) {
         cudaLaunchConfig_t cfg;
         memset(&cfg, 0, sizeof(cfg));
         cfg.gridDim = dim3((unsigned)tiles);
@@ -151,9 +173,10 @@ static int launch_gemm(const CUtensorMap& mx, const CUtensorMap& my, const CUten
         cfg.numAttrs = 1;
         const cudaError_t e = cudaLaunchKernelEx(&cfg, gemm_tn_kernel<EPI>, mx, my, mc, p);
         if (e == cudaSuccess) return 0;
-        if (e != cudaErrorNotSupported && e != cudaErrorInvalidValue) return PFSM_CUDA_ERROR_BASE + (int)e;
+        // only "attribute not supported" falls back to plain stream order (always correct); anything else is a real error
+        if (e != cudaErrorNotSupported) return PFSM_CUDA_ERROR_BASE + (int)e;
         cudaGetLastError();
-        pdl_ok = false;
+        h->pdl_ok = false;
     }
     gemm_tn_kernel<EPI><<<(unsigned)tiles, GEMM_THREADS, GEMM_SMEM, st>>>(mx, my, mc, p);
     PFSM_CUDA(cudaGetLastError());
@@ -167,6 +190,29 @@ static GemmParams base_params() {
 }
 
 extern "C" { static void choose_jacobi_layout(pfsm_ctx* h); }
+
+// workspace of the tridiagonal route of step 2 (allocated when that route is selected: at create, or by pfsm_set_option)
+static int ensure_tridiag_ws(pfsm_ctx* h) {
+    if (!h->tridiag || h->tri.d) return 0;
+    const int64_t N = h->N, M = h->M, P = h->P;
+    const size_t pm = (size_t)P * M * sizeof(double), mn = (size_t)M * N;
+    int rc;
+#define TRYA(x) do { if ((rc = (x))) return rc; } while (0)
+    TRYA(dev_alloc(h, (void**)&h->tri.d, pm));
+    TRYA(dev_alloc(h, (void**)&h->tri.e, pm));
+    TRYA(dev_alloc(h, (void**)&h->tri.tau, pm));
+    TRYA(dev_alloc(h, (void**)&h->tri.pbuf, 2 * pm));
+    TRYA(dev_alloc(h, (void**)&h->tri.vbuf, 2 * pm));
+    TRYA(dev_alloc(h, (void**)&h->tri.rowbuf, pm * ((M + 31) / 32)));
+    TRYA(dev_alloc(h, (void**)&h->tri.colbuf, pm * ((M + 31) / 32)));
+    TRYA(dev_alloc(h, (void**)&h->tri.colk, 2 * pm));
+    TRYA(dev_alloc(h, (void**)&h->tri.lam, N * sizeof(double)));
+    TRYA(dev_alloc(h, (void**)&h->tri.zscale, N * sizeof(double)));
+    for (int i = 0; i < 5; ++i) TRYA(dev_alloc(h, (void**)&h->tri.f[i], mn * sizeof(double)));
+    TRYA(dev_alloc(h, (void**)&h->tri.piv, mn));
+#undef TRYA
+    return 0;
+}
 
 extern "C" {
 
@@ -215,24 +261,12 @@ int pfsm_create(pfsm_handle_t* out, int64_t N, int32_t P, int32_t window, int32_
     TRY(dev_alloc(h, (void**)&h->rotcnt, (size_t)P * JACOBI_MAX_SWEEPS * sizeof(int)));
     TRY(dev_alloc(h, (void**)&h->nrm_g, (size_t)P * (M + 16) * sizeof(double)));
     TRY(dev_alloc(h, (void**)&h->jw_bar, sizeof(unsigned int)));
-    choose_jacobi_layout(h);
-    if (h->tridiag) {
-        const size_t pm = (size_t)P * M * sizeof(double), mn = (size_t)M * N;
-        TRY(dev_alloc(h, (void**)&h->tri.d, pm));
-        TRY(dev_alloc(h, (void**)&h->tri.e, pm));
-        TRY(dev_alloc(h, (void**)&h->tri.tau, pm));
-        TRY(dev_alloc(h, (void**)&h->tri.pbuf, 2 * pm));
-        TRY(dev_alloc(h, (void**)&h->tri.vbuf, 2 * pm));
-        TRY(dev_alloc(h, (void**)&h->tri.rowbuf, pm * ((M + 31) / 32)));
-        TRY(dev_alloc(h, (void**)&h->tri.colbuf, pm * ((M + 31) / 32)));
-        TRY(dev_alloc(h, (void**)&h->tri.colk, 2 * pm));
-        h->sytrd_full = getenv("PFSM_SYTRD_FULL") != nullptr;  // diagnostic: force full-storage tridiagonalization
-        h->sytrd_half = getenv("PFSM_SYTRD_HALF") != nullptr;  // diagnostic: force lower-triangle tridiagonalization
-        TRY(dev_alloc(h, (void**)&h->tri.lam, N * sizeof(double)));
-        TRY(dev_alloc(h, (void**)&h->tri.zscale, N * sizeof(double)));
-        for (int i = 0; i < 5; ++i) TRY(dev_alloc(h, (void**)&h->tri.f[i], mn * sizeof(double)));
-        TRY(dev_alloc(h, (void**)&h->tri.piv, mn));
+    {
+        cudaError_t e = cudaDeviceGetAttribute(&h->sms, cudaDevAttrMultiProcessorCount, h->device);
+        if (e != cudaSuccess) { pfsm_destroy(h); return PFSM_CUDA_ERROR_BASE + (int)e; }
     }
+    choose_jacobi_layout(h);
+    TRY(ensure_tridiag_ws(h));
     TRY(dev_alloc(h, (void**)&h->slice_tab, 4 * (size_t)P * sizeof(int32_t)));
     const int32_t ntr = (int32_t)((N + BM - 1) / BM);
     TRY(dev_alloc(h, (void**)&h->krange, (size_t)ntr * sizeof(int2)));
@@ -286,8 +320,6 @@ int pfsm_create(pfsm_handle_t* out, int64_t N, int32_t P, int32_t window, int32_
         if (e == cudaSuccess) e = cudaEventCreateWithFlags(&h->ev_rest, cudaEventDisableTiming);
         if (e == cudaSuccess) e = cudaEventCreateWithFlags(&h->ev_fork, cudaEventDisableTiming);
         if (e != cudaSuccess) { pfsm_destroy(h); return PFSM_CUDA_ERROR_BASE + (int)e; }
-        h->lookahead = getenv("PFSM_NO_LOOKAHEAD") == nullptr;
-        h->chain = getenv("PFSM_NO_CHAIN") == nullptr;
     }
 #undef TRY
     *out = h;
@@ -296,11 +328,15 @@ int pfsm_create(pfsm_handle_t* out, int64_t N, int32_t P, int32_t window, int32_
 
 int pfsm_destroy(pfsm_handle_t h) {
     if (!h) return 0;
+    int cur = -1;
+    cudaGetDevice(&cur);
+    if (cur != h->device) cudaSetDevice(h->device);
     cudaDeviceSynchronize();
     void* ptrs[] = {h->W, h->S, h->O, h->Dinv, h->Gws, h->eps, h->resid, h->gdiag, h->rotcnt, h->nrm_g, h->jw_bar, h->slice_tab, h->krange, h->info, h->chain_cnt,
                     h->A_stage, h->V_stage, h->lam_stage, h->Ap, h->LT, h->DinvT,
                     h->tri.d, h->tri.e, h->tri.tau, h->tri.pbuf, h->tri.vbuf, h->tri.rowbuf, h->tri.colbuf, h->tri.colk, h->tri.lam, h->tri.zscale,
-                    h->tri.f[0], h->tri.f[1], h->tri.f[2], h->tri.f[3], h->tri.f[4], h->tri.piv};
+                    h->tri.f[0], h->tri.f[1], h->tri.f[2], h->tri.f[3], h->tri.f[4], h->tri.piv,
+                    h->sbw.VW, h->sbw.WV, h->sbw.ypart, h->sbw.y, h->sbw.base, h->sbw.dots, h->sbw.yv, h->sbw.sbar};
     for (void* p : ptrs)
         if (p) cudaFree(p);
     for (int i = 0; i < 5; ++i)
@@ -309,6 +345,7 @@ int pfsm_destroy(pfsm_handle_t h) {
     if (h->ev_rest) cudaEventDestroy(h->ev_rest);
     if (h->ev_fork) cudaEventDestroy(h->ev_fork);
     if (h->side) cudaStreamDestroy(h->side);
+    if (cur >= 0 && cur != h->device) cudaSetDevice(cur);
     delete h;
     return 0;
 }
@@ -318,7 +355,7 @@ static int jacobi_cluster_size(const pfsm_ctx* h) {
     const int npairs = (h->M + 1) / 2;
     int cs = 1;
     const int nw = jacobi_l2_threads(h->M > 256 ? 16 : (h->M > 128 ? 8 : 4)) / 32;  // warps per CTA
-    while (cs < 8 && (2 * cs) * h->P <= 148 && cs * nw < npairs) cs *= 2;
+    while (cs < 8 && (2 * cs) * h->P <= h->sms && cs * nw < npairs) cs *= 2;
     return cs;
 }
 
@@ -432,16 +469,17 @@ static int jacobi_max_clusters(int M, int cs, size_t smem, bool half = false) {
 static void choose_jacobi_layout(pfsm_ctx* h) {
     h->jac_cs = 0;
     h->jac_hloc = 0;
-    h->jac_wide = getenv("PFSM_JACOBI_WIDE") != nullptr;  // diagnostic: the wide-window Jacobi kernel at any M
+    h->jac_half = false;
+    h->jac_wide = h->opt_route == 3;  // option step2_route = 3: the persistent-grid Jacobi kernel at any M
     // Route of step 2.  Tridiagonalization + bisection + inverse iteration + back-transformation costs ~M latency-bound
     // columns; the Jacobi kernels cost sweeps x (M - 1) rounds.  Measured (step 2, Jacobi -> tridiagonal): M = 96 x 4
     // slices 0.60 -> 1.00 ms, M = 192 x 16 2.66 -> 2.15, M = 224 x 24 4.57 -> 2.69, M = 254 x 72 13.5 -> 4.9, M = 256 x 64
     // 12.5 -> 4.0, M = 416 x 13 15.2 -> 5.4 ms.  So: Jacobi up to M = 160, the tridiagonal route above.
-    // PFSM_JACOBI=1 / PFSM_TRIDIAG=1 force one family (M > 512 has no shared-memory / L2 Jacobi: PFSM_JACOBI_WIDE).
-    const bool want_jacobi = getenv("PFSM_JACOBI") != nullptr && h->M <= 512;
-    h->tridiag = !h->jac_wide && !want_jacobi && (h->M > 160 || getenv("PFSM_TRIDIAG") != nullptr);
+    // Option step2_route = 1 / 2 forces one family (M > 512 has no shared-memory / L2 Jacobi: step2_route = 3).
+    const bool want_jacobi = h->opt_route == 1 && h->M <= 512;
+    h->tridiag = !h->jac_wide && !want_jacobi && (h->M > 160 || h->opt_route == 2);
     if (h->M > 512 || h->jac_wide || h->tridiag) return;
-    if (getenv("PFSM_JACOBI_L2")) return;  // diagnostic: force the L2-resident kernel (the large-M fallback)
+    if (h->opt_jacobi_l2) return;  // option jacobi_l2: force the L2-resident kernel (the large-M fallback)
     const size_t budget = 220 * 1024;
     // seats per CTA; one more (phantom) pair when seat 0 and seat h_loc-1 would fall to the same warp, because the
     // two boundary seats of a CTA synchronise with each other inside a round (jacobi_smem.cuh)
@@ -471,13 +509,13 @@ static void choose_jacobi_layout(pfsm_ctx* h) {
         const int full_per_wave = jacobi_max_clusters(h->M, cs, jacobi_smem_bytes(h->M, hloc_of(cs)));
         const int half_per_wave = jacobi_max_clusters(h->M, 8, jacobi_smem_bytes(h->M, hloc_of(8, true)), true);
         auto waves = [&](int per) { return per > 0 ? (h->P + per - 1) / per : 1 << 20; };
-        if (waves(half_per_wave) <= waves(full_per_wave) && !getenv("PFSM_JACOBI_FULL")) {  // env: diagnostic, full CTAs only
+        if (waves(half_per_wave) <= waves(full_per_wave) && !h->opt_jacobi_full) {  // option jacobi_full_cta: full CTAs only
             half = true;
             cs = 8;
         }
     }
-    if (const char* e = getenv("PFSM_JACOBI_CS")) {  // diagnostic override of the cluster size
-        const int want = atoi(e);
+    if (h->opt_jacobi_cs) {  // option jacobi_cluster_size: override
+        const int want = h->opt_jacobi_cs;
         if ((want == 1 || want == 2 || want == 4 || want == 8) && fits(want, half)) cs = want;
     }
     h->jac_half = half;
@@ -516,12 +554,92 @@ static int launch_jacobi_wide_t(pfsm_ctx* h, const double* A, double* V, cudaStr
 }
 }  // extern "C++"
 
+// ---- Blocked tridiagonalization (sytrd_blocked.cuh): per panel of SB_NB columns one cooperative launch of
+// sytrd_panel_kernel (C CTAs per slice, per-slice barriers) and one batched rank-2NB trailing update on the DMMA pipe.
+static int ensure_blocked_ws(pfsm_ctx* h) {
+    if (h->sbw.VW) return 0;
+    const int64_t M = h->M, P = h->P;
+    int rc;
+#define TRYA(x) do { if ((rc = (x))) return rc; } while (0)
+    const size_t pm = (size_t)P * M * sizeof(double);
+    TRYA(dev_alloc(h, (void**)&h->sbw.VW, pm * 2 * SB_NB));
+    TRYA(dev_alloc(h, (void**)&h->sbw.WV, pm * 2 * SB_NB));
+    TRYA(dev_alloc(h, (void**)&h->sbw.ypart, (size_t)h->sms * M * sizeof(double)));
+    TRYA(dev_alloc(h, (void**)&h->sbw.y, 2 * pm));
+    TRYA(dev_alloc(h, (void**)&h->sbw.base, 2 * pm));
+    TRYA(dev_alloc(h, (void**)&h->sbw.dots, (size_t)h->sms * 2 * SB_NB * sizeof(double)));
+    TRYA(dev_alloc(h, (void**)&h->sbw.yv, (size_t)2 * h->sms * sizeof(double)));
+    TRYA(dev_alloc(h, (void**)&h->sbw.sbar, (size_t)P * sizeof(unsigned int)));
+    PFSM_CUDA(cudaMemset(h->sbw.VW, 0, pm * 2 * SB_NB));
+    PFSM_CUDA(cudaMemset(h->sbw.WV, 0, pm * 2 * SB_NB));
+    TRYA(make_map(&h->mapG, h->Gws, P * M, M, M));
+    TRYA(make_map(&h->mapVW, h->sbw.VW, P * M, 2 * SB_NB, 2 * SB_NB));
+    TRYA(make_map(&h->mapWV, h->sbw.WV, P * M, 2 * SB_NB, 2 * SB_NB));
+#undef TRYA
+    return 0;
+}
+
+static int launch_sytrd_blocked(pfsm_ctx* h, const double* A, cudaStream_t st, int32_t s0, int32_t ns, int32_t precopied) {
+    SliceTable tab{h->slice_tab, h->slice_tab + h->P, h->slice_tab + 2 * (size_t)h->P, h->slice_tab + 3 * (size_t)h->P};
+    const int M = h->M;
+    int rc;
+    if ((rc = ensure_blocked_ws(h))) return rc;
+    if (!precopied) {
+        sytrd_copy_kernel<<<dim3((unsigned)M, (unsigned)ns), 256, 0, st>>>(A, h->N, M, tab, h->Gws, s0);
+        PFSM_CUDA(cudaGetLastError());
+    }
+    const int nbk = (M + 31) / 32;
+    const int cap = h->sms;  // one CTA per SM (shared memory)
+    for (int sb0 = 0; sb0 < ns; sb0 += cap) {  // more slices than SMs: batches of slices, one CTA each
+        const int nsl = std::min(ns - sb0, cap);
+        const int C = std::max(1, std::min(cap / nsl, nbk));
+        // shared-memory slots: one chunk per column if it fits, never less than one strip
+        const size_t budget = 200 * 1024;
+        int slot_tiles = std::max(sb_max_tiles_per_cta(M, C), nbk);
+        while (slot_tiles > nbk && sb_smem_bytes(M, slot_tiles) > budget) --slot_tiles;
+        const size_t smem = sb_smem_bytes(M, slot_tiles);
+        PFSM_CUDA(cudaFuncSetAttribute(sytrd_panel_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        for (int k0 = 0; k0 < M - 1; k0 += SB_NB) {
+            const int ncols = std::min(SB_NB, M - 1 - k0);
+            PFSM_CUDA(cudaMemsetAsync(h->sbw.sbar + s0 + sb0, 0, (size_t)nsl * sizeof(unsigned int), st));
+            cudaLaunchConfig_t cfg;
+            memset(&cfg, 0, sizeof(cfg));
+            cfg.gridDim = dim3((unsigned)(nsl * C));
+            cfg.blockDim = dim3(SB_THREADS);
+            cfg.dynamicSmemBytes = smem;
+            cfg.stream = st;
+            cudaLaunchAttribute attr[1];
+            attr[0].id = cudaLaunchAttributeCooperative;  // all CTAs co-resident: the slice barriers cannot deadlock
+            attr[0].val.cooperative = 1;
+            cfg.attrs = attr;
+            cfg.numAttrs = 1;
+            PFSM_CUDA(cudaLaunchKernelEx(&cfg, sytrd_panel_kernel, h->Gws, (int32_t)M, h->tri, h->sbw, h->P,
+                                         (int32_t)(s0 + sb0), (int32_t)C, (int32_t)k0, (int32_t)ncols, (int32_t)slot_tiles));
+            const int kt = k0 + SB_NB;
+            if (kt < M - 1) {  // A[kt:, kt:] -= V W^T + W V^T on the lower tiles, all slices of the batch in one launch
+                GemmParams p = base_params();
+                p.C = h->Gws; p.ldc = M; p.cr0 = (s0 + sb0) * M + kt; p.cc0 = kt; p.mr = M - kt; p.nc = M - kt;
+                p.xr0 = (s0 + sb0) * M + kt; p.yr0 = (s0 + sb0) * M + kt; p.klen = 2 * SB_NB; p.lower = 1;
+                p.nbatch = nsl; p.bxs = M; p.bys = M; p.bcs = M;
+                if ((rc = launch_gemm<EPI_SUB>(h, h->mapVW, h->mapWV, h->mapG, p, st))) return rc;
+            }
+        }
+    }
+    return 0;
+}
+
 // Wide windows, default route: Householder tridiagonalization + bisection + inverse iteration + back-transformation
 static int launch_tridiag(pfsm_ctx* h, const double* A, double* V, cudaStream_t st, int32_t s0, int32_t ns, int32_t precopied) {
     SliceTable tab{h->slice_tab, h->slice_tab + h->P, h->slice_tab + 2 * (size_t)h->P, h->slice_tab + 3 * (size_t)h->P};
     const int M = h->M;
     int sms = 0;
     PFSM_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, h->device));
+    // Blocked route (panel + DMMA rank-2NB update): option sytrd_storage = 3 (M even: the tensor maps need a 16-byte pitch)
+    const bool blocked = h->opt_sytrd_storage == 3 && (M % 2 == 0) && M >= 4;
+    if (blocked) {
+        int rcb;
+        if ((rcb = launch_sytrd_blocked(h, A, st, s0, ns, precopied))) return rcb;
+    } else
     {
         const size_t smem = 3 * (size_t)M * sizeof(double);
         // Lower-triangle storage halves the HBM traffic but pays a second grid barrier and a partial-sum pass per
@@ -529,9 +647,9 @@ static int launch_tridiag(pfsm_ctx* h, const double* A, double* V, cudaStream_t 
         // L2 resident: 11 -> 17 ms, so full storage is kept there)
         int l2 = 0;
         PFSM_CUDA(cudaDeviceGetAttribute(&l2, cudaDevAttrL2CacheSize, h->device));
-        const bool half = !h->sytrd_full && (h->sytrd_half || (size_t)ns * M * M * sizeof(double) > (size_t)l2);
+        const bool half = h->opt_sytrd_storage != 1 && (h->opt_sytrd_storage == 2 || (size_t)ns * M * M * sizeof(double) > (size_t)l2);
         // Small submatrices (a column is latency bound): the CTAs of a slice form a cluster and use its barrier
-        bool cluster = !half && M <= 768 && !getenv("PFSM_SYTRD_GRID");
+        bool cluster = !half && M <= 768 && !h->opt_sytrd_grid;
         int ccl = 1;  // cluster size: the largest of 8, 4, 2 that keeps all ns clusters co-resident (one wave)
         if (cluster) {
             PFSM_CUDA(cudaFuncSetAttribute(sytrd_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
@@ -593,7 +711,9 @@ static int launch_tridiag(pfsm_ctx* h, const double* A, double* V, cudaStream_t 
     const dim3 g2b((unsigned)((h->m + TRI_THREADS / 32 - 1) / (TRI_THREADS / 32)), (unsigned)ns);
     tri_bisect_kernel<<<g2b, TRI_THREADS, smem2, st>>>((int32_t)M, tab, h->tri, s0);
     PFSM_CUDA(cudaGetLastError());
-    tri_invit_kernel<<<g2, TRI_THREADS, smem2, st>>>(h->N, (int32_t)M, tab, h->tri, s0);
+    tri_invit_kernel<<<g2, TRI_THREADS, smem2, st>>>(h->N, (int32_t)M, tab, h->tri, s0, h->info);
+    PFSM_CUDA(cudaGetLastError());
+    tri_cluster_kernel<<<(unsigned)ns, TRC_THREADS, 0, st>>>(h->N, (int32_t)M, tab, h->tri, s0);
     PFSM_CUDA(cudaGetLastError());
     {
         const int ept = (M + BT_THREADS - 1) / BT_THREADS;
@@ -665,10 +785,9 @@ static int stacked_cholesky(pfsm_ctx* h, bool factor, cudaStream_t st, int32_t b
     if (b1 < 0) b1 = n;
     const bool whole = factor && b0 == 0 && b1 == n;  // top and bottom rows form one contiguous row range
     int rc;
-    static bool chol_attr = false;
-    if (!chol_attr) {
+    if (!h->chol_attr) {
         PFSM_CUDA(cudaFuncSetAttribute(chol_diag_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, CHOL_SMEM));
-        chol_attr = true;
+        h->chol_attr = true;
     }
     cudaStream_t cs = st;  // stream the helpers below launch on (switched by the look-ahead schedule)
     // panel rows [r0, r0 + nr): O[r, k0:k0+nb] = S[r, k0:k0+nb] L_kk^-T
@@ -678,7 +797,7 @@ static int stacked_cholesky(pfsm_ctx* h, bool factor, cudaStream_t st, int32_t b
         GemmParams pp = base_params();
         pp.C = h->O; pp.ldc = N; pp.cr0 = r0; pp.cc0 = k0; pp.mr = nr; pp.nc = nb;
         pp.xr0 = r0; pp.xk0 = k0; pp.yr0 = k * CHOL_NB; pp.yk0 = 0; pp.klen = nb;
-        return launch_gemm<EPI_PLAIN>(h->mapS, h->mapD, h->mapO, pp, cs);
+        return launch_gemm<EPI_PLAIN>(h, h->mapS, h->mapD, h->mapO, pp, cs);
     };
     auto factor_panel = [&](int32_t k) -> int {
         const int32_t k0 = k * CHOL_NB, nb = (int32_t)std::min<int64_t>(CHOL_NB, N - k0);
@@ -697,7 +816,7 @@ static int stacked_cholesky(pfsm_ctx* h, bool factor, cudaStream_t st, int32_t b
         GemmParams pt = base_params();
         pt.C = h->S; pt.ldc = N; pt.cr0 = r0; pt.cc0 = c0; pt.mr = nr; pt.nc = ncols;
         pt.xr0 = r0; pt.yr0 = c0; pt.xk0 = kk0; pt.yk0 = kk0; pt.klen = klen; pt.lower = lower;
-        return launch_gemm<EPI_SUB>(h->mapO, h->mapO, h->mapS, pt, cs);
+        return launch_gemm<EPI_SUB>(h, h->mapO, h->mapO, h->mapS, pt, cs);
     };
     // columns [c0, c0 + ncols) of every active row at or below row c0 (lower tiles only where the region is square)
     auto update = [&](int32_t c0, int32_t ncols, int32_t kk0, int32_t klen, int lower) -> int {
@@ -770,12 +889,12 @@ static int run_step4_once(pfsm_ctx* h, const CUtensorMap& mapV, double* V, cudaS
     p.C = h->S; p.ldc = N; p.mr = n; p.nc = n; p.klen = n; p.lower = 2;
     p.wait_cnt = wait_cnt; p.wait_target = wait_target;
     if (wait_cnt) {
-        if ((rc = launch_gemm<EPI_PLAIN>(mapV, mapV, h->mapS, p, st, true))) return rc;
+        if ((rc = launch_gemm<EPI_PLAIN>(h, mapV, mapV, h->mapS, p, st, true))) return rc;
     }
     transpose_kernel<<<tg, tb, 0, st>>>(V, N, h->S + (size_t)N * N, N, n, n);
     PFSM_CUDA(cudaGetLastError());
     if (!wait_cnt) {
-        if ((rc = launch_gemm<EPI_PLAIN>(mapV, mapV, h->mapS, p, st))) return rc;
+        if ((rc = launch_gemm<EPI_PLAIN>(h, mapV, mapV, h->mapS, p, st))) return rc;
     }
     extract_diag_kernel<<<(unsigned)((N + 255) / 256), 256, 0, st>>>(h->S, N, n, h->gdiag);
     PFSM_CUDA(cudaGetLastError());
@@ -801,7 +920,7 @@ static int run_step4(pfsm_ctx* h, const CUtensorMap& mapV, double* V, cudaStream
 // 1.07 GB of operands); a dynamic shared-memory reservation caps residency at 3 blocks per SM so the rows stay in L2.
 static int launch_rayleigh(pfsm_ctx* h, const double* V, double* lambda_out, int32_t r0, int32_t rows, cudaStream_t st) {
     static const size_t RAY_CAP_SMEM = 72 * 1024;
-    const size_t in_flight = (size_t)148 * 8 * 16 * (size_t)h->N;
+    const size_t in_flight = (size_t)h->sms * 8 * 16 * (size_t)h->N;
     const size_t smem = in_flight > ((size_t)48 << 20) ? RAY_CAP_SMEM : 0;
     if (smem) PFSM_CUDA(cudaFuncSetAttribute(rayleigh_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     rayleigh_kernel<<<(unsigned)rows, RAY_THREADS, smem, st>>>(V, h->W, h->N, lambda_out, h->resid, r0);
@@ -818,9 +937,46 @@ static int run_step5(pfsm_ctx* h, const CUtensorMap& mapV, const CUtensorMap& ma
     {
         GemmParams p = base_params();
         p.C = h->W; p.ldc = N; p.mr = n; p.nc = n; p.klen = n;
-        if ((rc = launch_gemm<EPI_PLAIN>(mapV, mapA, h->mapW, p, st))) return rc;
+        if ((rc = launch_gemm<EPI_PLAIN>(h, mapV, mapA, h->mapW, p, st))) return rc;
         if ((rc = launch_rayleigh(h, V, lambda_out, 0, n, st))) return rc;
     }
+    return 0;
+}
+
+// ---- step 3 (Eq. 11) on rows [r0, r0 + rows) of the row-major V (eigenvectors r0 ..): two products per
+// iteration.  Each product needs whole rows of the previous one's output, so the GEMMs are serial -- but only row block by
+// row block: with 4096 tiles on 148 SMs the last wave of each is 100 tiles, and the next GEMM's first tiles (whose row
+// blocks were finished waves ago) fill the idle SMs.  Hazards: tile (i, j) of GEMM g+1 overwrites what only tiles (i, .)
+// of GEMM g read, and it starts after all of those have signalled.  A rank of the sharded solve runs the same chain on
+// its own row range (rows / BM row blocks).  *last_cnt = the counters of the last update (nullptr when not chained).
+static int run_step3(pfsm_ctx* h, const CUtensorMap& mapV, const CUtensorMap& mapA, double* V, int32_t r0, int32_t rows,
+                     cudaStream_t st, const int32_t** last_cnt) {
+    const int64_t N = h->N;
+    const int32_t n = (int32_t)N;
+    const int32_t nrb = (rows + BM - 1) / BM, ncb = (n + BN - 1) / BN;
+    const bool chain = h->chain && h->iters > 0;
+    int rc;
+    if (last_cnt) *last_cnt = nullptr;
+    if (chain) PFSM_CUDA(cudaMemsetAsync(h->chain_cnt, 0, (size_t)2 * h->iters * nrb * sizeof(int32_t), st));
+    for (int it = 0; it < h->iters; ++it) {
+        GemmParams p = base_params();  // W = V A - diag(eps) V   (row-major view; A symmetric)
+        p.C = h->W; p.ldc = N; p.cr0 = r0; p.xr0 = r0; p.mr = rows; p.nc = n; p.klen = n;
+        p.krange = (it == 0) ? h->krange + r0 / BM : nullptr;  // start vectors are zero outside their window
+        p.E1 = V; p.ld1 = N; p.eps = h->eps;
+        GemmParams q = base_params();  // V <- V - alpha (W A - diag(eps) W)
+        q.C = V; q.ldc = N; q.cr0 = r0; q.xr0 = r0; q.mr = rows; q.nc = n; q.klen = n;
+        q.E1 = h->W; q.ld1 = N; q.E2 = V; q.ld2 = N; q.eps = h->eps; q.alpha = h->alpha;
+        if (chain) {
+            int32_t* c0 = h->chain_cnt + (size_t)(2 * it) * nrb;
+            p.signal_cnt = c0;
+            q.signal_cnt = c0 + nrb;
+            q.wait_cnt = c0; q.wait_target = ncb;
+            if (it > 0) { p.wait_cnt = c0 - nrb; p.wait_target = ncb; }
+        }
+        if ((rc = launch_gemm<EPI_SHIFT>(h, mapV, mapA, h->mapW, p, st, chain && it > 0))) return rc;
+        if ((rc = launch_gemm<EPI_UPDATE>(h, h->mapW, mapA, mapV, q, st, chain))) return rc;
+    }
+    if (chain && last_cnt) *last_cnt = h->chain_cnt + (size_t)(2 * h->iters - 1) * nrb;
     return 0;
 }
 
@@ -829,6 +985,7 @@ static int run_step5(pfsm_ctx* h, const CUtensorMap& mapV, const CUtensorMap& ma
 static int solve_impl(pfsm_handle_t h, const double* A, double* V, double* lambda_out, void* stream, int32_t last_step,
                       const double* band, cudaEvent_t a_ready) {
     if (!h) return -1;
+    if (int rc_dev = check_device(h)) return rc_dev;
     if (!A || ((uintptr_t)A & 15)) return -2;
     if (!V || ((uintptr_t)V & 15)) return -3;
     if (last_step < 2 || last_step > 5) return -6;
@@ -853,37 +1010,15 @@ static int solve_impl(pfsm_handle_t h, const double* A, double* V, double* lambd
     if (last_step == 2) return 0;
 
     // ---- step 3: folded-spectrum iterations (Eq. 11), two products per iteration ----
-    // Each product needs whole rows of the previous one's output, so the GEMMs are serial -- but only row block by row
-    // block: with 4096 tiles on 148 SMs the last wave of each is 100 tiles, and the next GEMM's first tiles (whose row
-    // blocks were finished waves ago) fill the idle SMs.  Hazards: tile (i, j) of GEMM g+1 overwrites what only tiles
-    // (i, .) of GEMM g read, and it starts after all of those have signalled.
-    const int32_t nrb = (n + BM - 1) / BM, ncb = (n + BN - 1) / BN;
-    const bool chain = h->chain && h->iters > 0;
-    if (chain) PFSM_CUDA(cudaMemsetAsync(h->chain_cnt, 0, (size_t)2 * h->iters * nrb * sizeof(int32_t), st));
-    for (int it = 0; it < h->iters; ++it) {
-        GemmParams p = base_params();  // W = V A - diag(eps) V   (row-major view; A symmetric)
-        p.C = h->W; p.ldc = N; p.mr = n; p.nc = n; p.klen = n;
-        p.krange = (it == 0) ? h->krange : nullptr;  // start vectors are zero outside their window
-        p.E1 = V; p.ld1 = N; p.eps = h->eps;
-        GemmParams q = base_params();  // V <- V - alpha (W A - diag(eps) W)
-        q.C = V; q.ldc = N; q.mr = n; q.nc = n; q.klen = n;
-        q.E1 = h->W; q.ld1 = N; q.E2 = V; q.ld2 = N; q.eps = h->eps; q.alpha = h->alpha;
-        if (chain) {
-            int32_t* c0 = h->chain_cnt + (size_t)(2 * it) * nrb;
-            p.signal_cnt = c0;
-            q.signal_cnt = c0 + nrb;
-            q.wait_cnt = c0; q.wait_target = ncb;
-            if (it > 0) { p.wait_cnt = c0 - nrb; p.wait_target = ncb; }
-        }
-        if ((rc = launch_gemm<EPI_SHIFT>(mapV, mapA, h->mapW, p, st, chain && it > 0))) return rc;
-        if ((rc = launch_gemm<EPI_UPDATE>(h->mapW, mapA, mapV, q, st, chain))) return rc;
-    }
+    const int32_t ncb = (n + BN - 1) / BN;
+    const int32_t* step3_cnt = nullptr;
+    if ((rc = run_step3(h, mapV, mapA, V, 0, n, st, &step3_cnt))) return rc;
     if (tm) PFSM_CUDA(cudaEventRecord(h->ev[2], st));
     if (last_step == 3) return 0;
 
     // The Gram product of step 4 is one more link of the chain: it reads row blocks of the last update.  Not with step
     // timing on: the event between the two kernels would sit inside the overlap and blur both step times.
-    const int32_t* last_cnt = (chain && !tm) ? h->chain_cnt + (size_t)(2 * h->iters - 1) * nrb : nullptr;
+    const int32_t* last_cnt = tm ? nullptr : step3_cnt;
     if ((rc = run_step4(h, mapV, V, st, last_cnt, ncb))) return rc;
     if (tm) PFSM_CUDA(cudaEventRecord(h->ev[3], st));
     if (last_step == 4) return 0;
@@ -903,6 +1038,7 @@ int pfsm_solve_partial(pfsm_handle_t h, const double* A, double* V, double* lamb
 
 int pfsm_orthonormalize(pfsm_handle_t h, double* V_inout, void* stream) {
     if (!h) return -1;
+    if (int rc_dev = check_device(h)) return rc_dev;
     if (!V_inout || ((uintptr_t)V_inout & 15)) return -2;
     CUtensorMap mapV;
     int rc;
@@ -915,6 +1051,7 @@ int pfsm_orthonormalize(pfsm_handle_t h, double* V_inout, void* stream) {
 
 int pfsm_rayleigh(pfsm_handle_t h, const double* A, const double* V, double* lambda_out, void* stream) {
     if (!h) return -1;
+    if (int rc_dev = check_device(h)) return rc_dev;
     if (!A || ((uintptr_t)A & 15)) return -2;
     if (!V || ((uintptr_t)V & 15)) return -3;
     if (!lambda_out || ((uintptr_t)lambda_out & 7)) return -4;
@@ -980,12 +1117,12 @@ static int run_generalized_back(pfsm_ctx* h, double* V, cudaStream_t st) {
         GemmParams pp = base_params();
         pp.C = h->W; pp.ldc = N; pp.cr0 = 0; pp.cc0 = k0; pp.mr = n; pp.nc = nb;
         pp.xr0 = 0; pp.xk0 = k0; pp.yr0 = k * CHOL_NB; pp.yk0 = 0; pp.klen = nb;
-        if ((rc = launch_gemm<EPI_PLAIN>(mapV, h->mapDT, h->mapW, pp, st))) return rc;
+        if ((rc = launch_gemm<EPI_PLAIN>(h, mapV, h->mapDT, h->mapW, pp, st))) return rc;
         if (k0 > 0) {
             GemmParams pt = base_params();
             pt.C = V; pt.ldc = N; pt.cr0 = 0; pt.cc0 = 0; pt.mr = n; pt.nc = k0;
             pt.xr0 = 0; pt.xk0 = k0; pt.yr0 = 0; pt.yk0 = k0; pt.klen = nb;
-            if ((rc = launch_gemm<EPI_SUB>(h->mapW, h->mapLT, mapV, pt, st))) return rc;
+            if ((rc = launch_gemm<EPI_SUB>(h, h->mapW, h->mapLT, mapV, pt, st))) return rc;
         }
     }
     PFSM_CUDA(cudaMemcpyAsync(V, h->W, (size_t)N * N * sizeof(double), cudaMemcpyDeviceToDevice, st));
@@ -994,6 +1131,7 @@ static int run_generalized_back(pfsm_ctx* h, double* V, cudaStream_t st) {
 
 int pfsm_generalized_reduce(pfsm_handle_t h, const double* A, const double* S, double* Ap_out, void* stream) {
     if (!h) return -1;
+    if (int rc_dev = check_device(h)) return rc_dev;
     if (!A || ((uintptr_t)A & 15)) return -2;
     if (!S || ((uintptr_t)S & 15)) return -3;
     if (!Ap_out || ((uintptr_t)Ap_out & 15)) return -4;
@@ -1006,6 +1144,7 @@ int pfsm_generalized_reduce(pfsm_handle_t h, const double* A, const double* S, d
 int pfsm_solve_generalized(pfsm_handle_t h, const double* A, const double* S, double* X_out, double* lambda_out,
                            void* stream) {
     if (!h) return -1;
+    if (int rc_dev = check_device(h)) return rc_dev;
     if (!A || ((uintptr_t)A & 15)) return -2;
     if (!S || ((uintptr_t)S & 15)) return -3;
     if (!X_out || ((uintptr_t)X_out & 15)) return -4;
@@ -1027,6 +1166,7 @@ int pfsm_solve_generalized(pfsm_handle_t h, const double* A, const double* S, do
 // -- the method's condition for success -- so PFSM runs on A' and the result is rotated back: V = V_prev U. ----
 int pfsm_solve_warm(pfsm_handle_t h, const double* A, double* V_inout, double* lambda_out, void* stream) {
     if (!h) return -1;
+    if (int rc_dev = check_device(h)) return rc_dev;
     if (!A || ((uintptr_t)A & 15)) return -2;
     if (!V_inout || ((uintptr_t)V_inout & 15)) return -3;
     if (!lambda_out || ((uintptr_t)lambda_out & 7)) return -4;
@@ -1042,12 +1182,12 @@ int pfsm_solve_warm(pfsm_handle_t h, const double* A, double* V_inout, double* l
     {   // W = V_prev A  (row-major view: row i = (A v_i)^T)
         GemmParams p = base_params();
         p.C = h->W; p.ldc = N; p.mr = n; p.nc = n; p.klen = n;
-        if ((rc = launch_gemm<EPI_PLAIN>(mapV, mapA, h->mapW, p, st))) return rc;
+        if ((rc = launch_gemm<EPI_PLAIN>(h, mapV, mapA, h->mapW, p, st))) return rc;
     }
     {   // A'[i][j] = v_i . (A v_j), into S's top half, then symmetrized into Ap
         GemmParams p = base_params();
         p.C = h->S; p.ldc = N; p.mr = n; p.nc = n; p.klen = n;
-        if ((rc = launch_gemm<EPI_PLAIN>(mapV, h->mapW, h->mapS, p, st))) return rc;
+        if ((rc = launch_gemm<EPI_PLAIN>(h, mapV, h->mapW, h->mapS, p, st))) return rc;
         symmetrize_kernel<<<tg, tb, 0, st>>>(h->S, N, h->Ap, N, n);
         PFSM_CUDA(cudaGetLastError());
     }
@@ -1057,7 +1197,7 @@ int pfsm_solve_warm(pfsm_handle_t h, const double* A, double* V_inout, double* l
     {   // V = V_prev U: row i of the result = sum_k U[i][k] V_prev[k][:]
         GemmParams p = base_params();
         p.C = h->W; p.ldc = N; p.mr = n; p.nc = n; p.klen = n;
-        if ((rc = launch_gemm<EPI_PLAIN>(mapV, h->mapLT, h->mapW, p, st))) return rc;
+        if ((rc = launch_gemm<EPI_PLAIN>(h, mapV, h->mapLT, h->mapW, p, st))) return rc;
     }
     PFSM_CUDA(cudaMemcpyAsync(V_inout, h->W, (size_t)N * N * sizeof(double), cudaMemcpyDeviceToDevice, st));
     return 0;
@@ -1071,6 +1211,7 @@ int pfsm_solve_warm(pfsm_handle_t h, const double* A, double* V_inout, double* l
 int pfsm_standard_form_eq14(pfsm_handle_t h, const double* A, const double* B, double* Z_out, int32_t niter,
                             int32_t symmetrize, void* stream) {
     if (!h) return -1;
+    if (int rc_dev = check_device(h)) return rc_dev;
     if (!A || ((uintptr_t)A & 15)) return -2;
     if (!B || ((uintptr_t)B & 15)) return -3;
     if (!Z_out || ((uintptr_t)Z_out & 15)) return -4;
@@ -1093,7 +1234,7 @@ int pfsm_standard_form_eq14(pfsm_handle_t h, const double* A, const double* B, d
         GemmParams p = base_params();
         p.C = nxt; p.ldc = N; p.mr = n; p.nc = n; p.klen = n;
         p.E1 = A; p.ld1 = N; p.E2 = cur; p.ld2 = N; p.eps = h->gdiag;
-        if ((rc = launch_gemm<EPI_JSTEP>(*mcur, mapB, *mnxt, p, st))) return rc;
+        if ((rc = launch_gemm<EPI_JSTEP>(h, *mcur, mapB, *mnxt, p, st))) return rc;
         std::swap(cur, nxt);
         std::swap(mcur, mnxt);
     }
@@ -1137,6 +1278,7 @@ int pfsm_shard_buffer(pfsm_handle_t h, int32_t which, double** ptr) {
 
 int pfsm_shard_phase(pfsm_handle_t h, int32_t phase, const double* A, double* V, double* lambda_out, void* stream) {
     if (!h) return -1;
+    if (int rc_dev = check_device(h)) return rc_dev;
     if (phase < 1 || phase > 4) return -2;
     if ((phase == 1 || phase == 4) && (!A || ((uintptr_t)A & 15))) return -3;
     if (!V || ((uintptr_t)V & 15)) return -4;
@@ -1156,21 +1298,11 @@ int pfsm_shard_phase(pfsm_handle_t h, int32_t phase, const double* A, double* V,
         PFSM_CUDA(cudaMemsetAsync(h->info, 0xFF, sizeof(unsigned long long), st));
         PFSM_CUDA(cudaMemsetAsync(V + (size_t)r0 * N, 0, (size_t)rows * N * sizeof(double), st));
         if ((rc = launch_jacobi(h, A, V, st, s0, ns))) return rc;
-        for (int it = 0; it < h->iters; ++it) {
-            GemmParams p = base_params();
-            p.C = h->W; p.ldc = N; p.cr0 = r0; p.mr = rows; p.nc = n; p.xr0 = r0; p.klen = n;
-            p.krange = (it == 0) ? h->krange + r0 / BM : nullptr;
-            p.E1 = V; p.ld1 = N; p.eps = h->eps;
-            if ((rc = launch_gemm<EPI_SHIFT>(mapV, mapA, h->mapW, p, st))) return rc;
-            GemmParams q = base_params();
-            q.C = V; q.ldc = N; q.cr0 = r0; q.mr = rows; q.nc = n; q.xr0 = r0; q.klen = n;
-            q.E1 = h->W; q.ld1 = N; q.E2 = V; q.ld2 = N; q.eps = h->eps; q.alpha = h->alpha;
-            if ((rc = launch_gemm<EPI_UPDATE>(h->mapW, mapA, mapV, q, st))) return rc;
-        }
+        if ((rc = run_step3(h, mapV, mapA, V, r0, rows, st, nullptr))) return rc;
     } else if (phase == 2) {
         GemmParams p = base_params();  // G[r0:r1, :] = V[r0:r1, :] V^T
         p.C = h->S; p.ldc = N; p.cr0 = r0; p.mr = rows; p.nc = n; p.xr0 = r0; p.klen = n;
-        if ((rc = launch_gemm<EPI_PLAIN>(mapV, mapV, h->mapS, p, st))) return rc;
+        if ((rc = launch_gemm<EPI_PLAIN>(h, mapV, mapV, h->mapS, p, st))) return rc;
     } else if (phase == 3) {
         transpose_kernel<<<tg, tb, 0, st>>>(V, N, h->S + (size_t)N * N, N, n, n);
         PFSM_CUDA(cudaGetLastError());
@@ -1182,7 +1314,7 @@ int pfsm_shard_phase(pfsm_handle_t h, int32_t phase, const double* A, double* V,
         PFSM_CUDA(cudaGetLastError());
         GemmParams p = base_params();
         p.C = h->W; p.ldc = N; p.cr0 = r0; p.mr = rows; p.nc = n; p.xr0 = r0; p.klen = n;
-        if ((rc = launch_gemm<EPI_PLAIN>(mapV, mapA, h->mapW, p, st))) return rc;
+        if ((rc = launch_gemm<EPI_PLAIN>(h, mapV, mapA, h->mapW, p, st))) return rc;
         if ((rc = launch_rayleigh(h, V, lambda_out, r0, rows, st))) return rc;
     }
     return 0;
@@ -1210,6 +1342,7 @@ static int upload_symmetric(pfsm_ctx* h, const double* A_host, cudaStream_t s) {
 
 int pfsm_solve_host(pfsm_handle_t h, const double* A_host, double* V_host, double* lambda_host, void* stream) {
     if (!h) return -1;
+    if (int rc_dev = check_device(h)) return rc_dev;
     if (!A_host) return -2;
     if (!V_host) return -3;
     if (!lambda_host) return -4;
@@ -1255,6 +1388,7 @@ int pfsm_solve_host(pfsm_handle_t h, const double* A_host, double* V_host, doubl
 
 int pfsm_get_info(pfsm_handle_t h, void* stream, int64_t* info) {
     if (!h) return -1;
+    if (int rc_dev = check_device(h)) return rc_dev;
     if (!info) return -3;
     unsigned long long v = 0;
     PFSM_CUDA(cudaMemcpyAsync(&v, h->info, sizeof(v), cudaMemcpyDeviceToHost, (cudaStream_t)stream));
@@ -1266,6 +1400,7 @@ int pfsm_get_info(pfsm_handle_t h, void* stream, int64_t* info) {
 int pfsm_check_validity(pfsm_handle_t h, void* stream, double resid_tol, int32_t* use_standard_solver,
                         double* max_resid_out, int64_t* info_out) {
     if (!h) return -1;
+    if (int rc_dev = check_device(h)) return rc_dev;
     if (!(resid_tol >= 0.0)) return -3;
     if (!use_standard_solver) return -4;
     cudaStream_t st = (cudaStream_t)stream;
@@ -1286,6 +1421,7 @@ int pfsm_check_validity(pfsm_handle_t h, void* stream, double resid_tol, int32_t
 
 int pfsm_get_step2_sweeps(pfsm_handle_t h, void* stream, int32_t* max_sweeps) {
     if (!h) return -1;
+    if (int rc_dev = check_device(h)) return rc_dev;
     if (!max_sweeps) return -3;
     std::vector<int> cnt((size_t)h->P * JACOBI_MAX_SWEEPS);
     PFSM_CUDA(cudaMemcpyAsync(cnt.data(), h->rotcnt, cnt.size() * sizeof(int), cudaMemcpyDeviceToHost,
@@ -1322,6 +1458,52 @@ int pfsm_set_cholqr_passes(pfsm_handle_t h, int32_t passes) {
     return 0;
 }
 
+// Options select among kernels that compute the same thing (A/B measurements; the parity tests reach every kernel through
+// them).  Explicit per-handle state: the library reads no environment variable.
+int pfsm_set_option(pfsm_handle_t h, const char* key, int64_t value) {
+    if (!h) return -1;
+    if (!key) return -2;
+    auto is01 = [&](int64_t v) { return v == 0 || v == 1; };
+    bool relayout = false;
+    if (!strcmp(key, "step2_route")) {
+        if (value < 0 || value > 3) return -3;
+        h->opt_route = (int32_t)value; relayout = true;
+    } else if (!strcmp(key, "jacobi_l2")) {
+        if (!is01(value)) return -3;
+        h->opt_jacobi_l2 = (int32_t)value; relayout = true;
+    } else if (!strcmp(key, "jacobi_cluster_size")) {
+        if (value != 0 && value != 1 && value != 2 && value != 4 && value != 8) return -3;
+        h->opt_jacobi_cs = (int32_t)value; relayout = true;
+    } else if (!strcmp(key, "jacobi_full_cta")) {
+        if (!is01(value)) return -3;
+        h->opt_jacobi_full = (int32_t)value; relayout = true;
+    } else if (!strcmp(key, "sytrd_storage")) {
+        if (value < 0 || value > 3) return -3;
+        h->opt_sytrd_storage = (int32_t)value;
+    } else if (!strcmp(key, "sytrd_grid_barrier")) {
+        if (!is01(value)) return -3;
+        h->opt_sytrd_grid = (int32_t)value;
+    } else if (!strcmp(key, "cholesky_lookahead")) {
+        if (!is01(value)) return -3;
+        h->lookahead = value != 0;
+    } else if (!strcmp(key, "chain_launches")) {
+        if (!is01(value)) return -3;
+        h->chain = value != 0;
+    } else if (!strcmp(key, "cholqr_passes")) {
+        if (value < 1 || value > 2) return -3;
+        h->cholqr_passes = (int32_t)value;
+    } else {
+        return -2;
+    }
+    if (relayout) {
+        int rc;
+        if ((rc = check_device(h))) return rc;
+        choose_jacobi_layout(h);
+        if ((rc = ensure_tridiag_ws(h))) return rc;
+    }
+    return 0;
+}
+
 int pfsm_set_alpha(pfsm_handle_t h, double alpha) {
     if (!h) return -1;
     if (!std::isfinite(alpha) || !(alpha > 0.0)) return -2;
@@ -1344,7 +1526,7 @@ int64_t pfsm_launches_per_solve(pfsm_handle_t h) {
             if (cn0 >= h->N) continue;
             trailing += (h->lookahead && npairs >= 3 && cn1 < h->N) ? 2 : 1;
         }
-        const int64_t step2 = h->tridiag ? 4 : 1;  // tridiagonal route: sytrd, bisection, inverse iteration, back-transformation
+        const int64_t step2 = h->tridiag ? 5 : 1;  // tridiagonal route: sytrd, bisection, inverse iteration, cluster pass, back-transformation
         return step2 + 2 * (int64_t)h->iters + h->cholqr_passes * (2 + 1 + 1 + 2 * nb + pairs + trailing) + 2;
     }
 }

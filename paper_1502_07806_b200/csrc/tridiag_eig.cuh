@@ -518,7 +518,7 @@ __device__ __forceinline__ double tri_start_value(uint32_t vec, uint32_t row) {
 // Output: z in ws.f[4] (not normalized), ws.zscale[g] = 1 / ||z||_2.
 // ---------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(TRI_THREADS)
-tri_invit_kernel(int64_t N, int32_t M, SliceTable tab, TriWs ws, int32_t s_off) {
+tri_invit_kernel(int64_t N, int32_t M, SliceTable tab, TriWs ws, int32_t s_off, unsigned long long* info) {
     extern __shared__ double sm[];
     double* d = sm;
     double* e = sm + M;
@@ -548,7 +548,7 @@ tri_invit_kernel(int64_t N, int32_t M, SliceTable tab, TriWs ws, int32_t s_off) 
     double x = ws.lam[g0];
     for (int j = 1; j <= t; ++j) {
         const double xj = ws.lam[g0 + j];
-        const double pertol = 10.0 * fabs(EPS * xj);
+        const double pertol = 10.0 * EPS * fmax(fabs(xj), 1e-3 * tmax);  // (floor: eigenvalues clustered at zero are pushed apart too)
         x = (xj - x < pertol) ? x + pertol : xj;
     }
     const double pivtol = fmax(EPS * tmax, 1e-300);
@@ -665,6 +665,122 @@ tri_invit_kernel(int64_t N, int32_t M, SliceTable tab, TriWs ws, int32_t s_off) 
         }
     }
     ws.zscale[g] = scale;
+    // convergence: the last solve (T - x I) z' = z, ||z|| = 1, must have grown the vector to ||z'|| >= 1 / (sqrt(eps) ||T||),
+    // i.e. left a residual <= sqrt(eps) ||T|| (one more solve squares it); else the slice is flagged as the Jacobi kernels do
+    if (!(scale <= 1.4901161193847656e-08 * tmax) && tmax > 0.0) atomicMin(info, (unsigned long long)(N + s + 1));
+}
+
+// ---------------------------------------------------------------------------------------------
+// Eigenvalue clusters (LAPACK dstein's re-orthogonalization, restricted to the gaps that need it).  Inverse iteration
+// without it delivers the vectors of a pair with gap g to eps ||T|| / g; for g below TRI_CLUSTER_TOL ||T|| two vectors can
+// come out numerically parallel, and step 4 would then orthonormalize noise.  One CTA per slice walks its eigenvalues;
+// for every run of consecutive eigenvalues closer than that, members 2, 3, .. are -- one after the other -- orthogonalized
+// against the earlier members (modified Gram-Schmidt), normalized and put through one more inverse-iteration solve with
+// their own stored LU factors, three times, ending on an orthogonalization.  The dot products run over the CTA (fixed
+// order), the solve is the serial recurrence on one thread; clusters this tight are rare (exact degeneracies).
+// ---------------------------------------------------------------------------------------------
+constexpr double TRI_CLUSTER_TOL = 1e-7;
+constexpr int TRC_THREADS = 256;
+
+__device__ __forceinline__ double trc_block_sum(double v, double* red) {
+    v = warp_sum(v);
+    __syncthreads();
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = v;
+    __syncthreads();
+    double t = 0.0;
+#pragma unroll
+    for (int w = 0; w < TRC_THREADS / 32; ++w) t += red[w];
+    return t;
+}
+
+__global__ void __launch_bounds__(TRC_THREADS)
+tri_cluster_kernel(int64_t N, int32_t M, SliceTable tab, TriWs ws, int32_t s_off) {
+    __shared__ double red[TRC_THREADS / 32];
+    const int s = s_off + blockIdx.x, tid = threadIdx.x;
+    const size_t so = (size_t)s * M;
+    const int m = tab.cnt[s], g0 = tab.g0[s];
+    double tmax = 0.0;
+    for (int i = tid; i < M; i += TRC_THREADS) {
+        const double ei = (i < M - 1) ? ws.e[so + i] : 0.0;
+        tmax = fmax(tmax, fabs(ws.d[so + i]) + 2.0 * fabs(ei));
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) tmax = fmax(tmax, __shfl_xor_sync(0xffffffffu, tmax, o));
+    __syncthreads();
+    if ((tid & 31) == 0) red[tid >> 5] = tmax;
+    __syncthreads();
+    for (int w = 0; w < TRC_THREADS / 32; ++w) tmax = fmax(tmax, red[w]);
+    const double gaptol = TRI_CLUSTER_TOL * tmax;
+    const size_t st = (size_t)N;
+    int start = 0;  // first member of the current run
+    for (int t = 1; t < m; ++t) {
+        if (ws.lam[g0 + t] - ws.lam[g0 + t - 1] > gaptol) {
+            start = t;
+            continue;
+        }
+        // eigenvalue t belongs to the run [start, t]: orthogonalize its vector against members start .. t-1
+        const size_t g = (size_t)g0 + t;
+        double* z = ws.f[4] + g;
+        for (int it = 0; it < 3; ++it) {
+            for (int b = start; b < t; ++b) {
+                const double* zb = ws.f[4] + g0 + b;
+                const double sb_ = ws.zscale[g0 + b];
+                double acc = 0.0;
+                for (int i = tid; i < M; i += TRC_THREADS) acc = fma(z[i * st], zb[i * st] * sb_, acc);
+                const double dot = trc_block_sum(acc, red);
+                for (int i = tid; i < M; i += TRC_THREADS) z[i * st] = fma(-dot, zb[i * st] * sb_, z[i * st]);
+                __syncthreads();
+            }
+            double mx = 0.0;  // scaled 2-norm (the vector carries the growth of the solves)
+            for (int i = tid; i < M; i += TRC_THREADS) mx = fmax(mx, fabs(z[i * st]));
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) mx = fmax(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+            __syncthreads();
+            if ((tid & 31) == 0) red[tid >> 5] = mx;
+            __syncthreads();
+            for (int w = 0; w < TRC_THREADS / 32; ++w) mx = fmax(mx, red[w]);
+            const double inv = (mx > 0.0) ? 1.0 / mx : 1.0;
+            double acc = 0.0;
+            for (int i = tid; i < M; i += TRC_THREADS) {
+                const double q = z[i * st] * inv;
+                acc = fma(q, q, acc);
+            }
+            const double nrm = sqrt(trc_block_sum(acc, red));
+            const double sc = (nrm > 0.0) ? inv / nrm : 1.0;
+            for (int i = tid; i < M; i += TRC_THREADS) z[i * st] *= sc;
+            __syncthreads();
+            if (it == 2) break;
+            if (tid == 0) {  // one more solve with this vector's own factors (the tri_invit_kernel recurrences)
+                const double* uinv = ws.f[0] + g;
+                const double* u1 = ws.f[1] + g;
+                const double* u2 = ws.f[2] + g;
+                const double* lm = ws.f[3] + g;
+                const unsigned char* pv = ws.piv + g;
+                double bi = z[0];
+                for (int i = 0; i < M - 1; ++i) {
+                    const double bn = z[(size_t)(i + 1) * st], f = lm[i * st];
+                    if (pv[i * st]) {
+                        z[i * st] = bn;
+                        bi = fma(-f, bn, bi);
+                    } else {
+                        z[i * st] = bi;
+                        bi = fma(-f, bi, bn);
+                    }
+                }
+                double x1 = bi * uinv[(size_t)(M - 1) * st], x2 = 0.0;
+                z[(size_t)(M - 1) * st] = x1;
+                for (int i = M - 2; i >= 0; --i) {
+                    const double xi = (z[i * st] - u1[i * st] * x1 - u2[i * st] * x2) * uinv[i * st];
+                    z[i * st] = xi;
+                    x2 = x1;
+                    x1 = xi;
+                }
+            }
+            __syncthreads();
+        }
+        if (tid == 0) ws.zscale[g] = 1.0;
+        __syncthreads();
+    }
 }
 
 // ---------------------------------------------------------------------------------------------

@@ -1,11 +1,11 @@
-"""Multi-GPU plumbing for the PFSM bench: REPLICAS ONLY.
+"""Multi-GPU plumbing shared by both N>1 modes of bench.py: process-group setup, barrier,
+MAX-over-ranks timing, whole-job aggregation.
 
-One PFSM solve couples all N vectors in step 4, so a single solve does not shard without a collective
-(SURVEY.md section 8(e) keeps the sharded solve as a later row).  What does partition cleanly is a set of
-independent eigenproblems -- one per k-point / spin channel / SCF replica in the paper's setting
-("a sequence of eigenvalue problems") -- so rank r solves its own matrix, there is no
-data-path collective, and the only communication is the barrier and the max-over-ranks of the timings.
-This module holds that host logic so it can be tested on CPU with the gloo backend.
+Default for N>1 is the SHARDED solve (paper_1502_07806_b200/sharded.py): one eigenproblem split
+over the ranks with all-gathers around step 4.  `bench.py --replicas` is the other mode: rank r solves its own matrix
+of the same config -- one per k-point / spin channel / SCF replica in the paper's setting ("a sequence of
+eigenvalue problems") -- with no data-path collective; the only communication is the barrier and the max-over-ranks of
+the timings.  This module holds that host logic so it can be tested on CPU with the gloo backend.
 """
 from __future__ import annotations
 
@@ -18,7 +18,8 @@ def env_world():
 
 
 def replica_seed_offset(rank: int) -> int:
-    """Rank r draws an independent matrix of the same config: seed = config seed + 1000 r."""
+    """Rank r draws an independent matrix of the same config: pfsm_inputs.problem(k, seed_offset=r) seeds it with
+    config seed + 1000 r."""
     return rank
 
 

@@ -25,8 +25,10 @@ def _all_gather_rows(t, world: int, rank: int, group=None):
     chunks = list(t.chunk(world, dim=0))
     assert len(chunks) == world and all(c.shape == chunks[0].shape for c in chunks)
     if dist.get_backend(group) == "nccl":
-        local = chunks[rank].clone()
-        dist.all_gather(chunks, local, group=group)
+        # in place, GPU to GPU: rank g's block already sits at its position in the output (ncclAllGather's in-place
+        # form), no staging copy; ordered after the solve's stream (torch's NCCL stream waits on the current stream)
+        assert t.is_contiguous()
+        dist.all_gather_into_tensor(t, chunks[rank], group=group)
         return
     host = [torch.empty(chunks[0].shape, dtype=t.dtype) for _ in range(world)]
     dist.all_gather(host, chunks[rank].cpu(), group=group)
@@ -35,18 +37,29 @@ def _all_gather_rows(t, world: int, rank: int, group=None):
             c.copy_(host[k])
 
 
-def solve_sharded(h, A, Vr, lam, group=None):
+def solve_sharded(h, A, Vr, lam, group=None, mark=None):
     """Collective: every rank calls it with its own handle (already `set_shard(rank, world)`), the replicated A, and
-    full-size Vr (N, N) / lam (N,) buffers.  On return every rank holds the complete V, lambda and residuals."""
+    full-size Vr (N, N) / lam (N,) buffers.  On return every rank holds the complete V, lambda and residuals.
+    mark(label), if given, is called at the start and after every phase / gather (bench.py records CUDA events there)."""
     import torch.distributed as dist
     world = dist.get_world_size(group) if dist.is_initialized() else 1
     rank = dist.get_rank(group) if dist.is_initialized() else 0
+    mark = mark or (lambda label: None)
+    mark("start")
     h.shard_phase(1, A, Vr, None)
+    mark("phase1_steps2_3")
     _all_gather_rows(Vr, world, rank, group)
+    mark("gather_V")
     h.shard_phase(2, None, Vr, None)
+    mark("phase2_gram_rows")
     _all_gather_rows(h.shard_buffer(0), world, rank, group)
+    mark("gather_G")
     h.shard_phase(3, None, Vr, None)
+    mark("phase3_cholesky_trsm_rows")
     _all_gather_rows(h.shard_buffer(1), world, rank, group)
+    mark("gather_VRinv")
     h.shard_phase(4, A, Vr, lam)
+    mark("phase4_step5_rows")
     _all_gather_rows(lam, world, rank, group)
     _all_gather_rows(h.residuals_view(), world, rank, group)
+    mark("gather_lambda_resid")

@@ -5,6 +5,8 @@ case that reduces to a library routine (numpy.linalg.eigh / qr / cholesky are us
 independent check -- the oracle itself contains no library linear algebra), or brute force on tiny
 inputs.  Each test says which plausible mistake it would catch.
 """
+import os
+
 import numpy as np
 import pytest
 
@@ -552,3 +554,39 @@ def test_oracle_invariants_on_a_seeded_sweep(N, P, w, iters):
     for s in range(P):
         mu = np.linalg.eigvalsh(p.A[lo[s]:lo[s] + M, lo[s]:lo[s] + M])
         np.testing.assert_allclose(r["eps"][g0[s]:g0[s] + cnt[s]], mu[off[s]:off[s] + cnt[s]], atol=1e-13)
+
+
+@pytest.mark.parametrize("k", [3, 4])
+def test_large_golden_files_belong_to_the_generators_matrix(k):
+    """tests/golden/config{3,4}_oracle.txt hold the oracle's full output for the two configs whose oracle run takes
+    minutes.  They must describe the matrix pfsm_inputs builds today (alpha, ||A||_F) and satisfy what holds for any
+    orthonormal V: sum(lambda) = trace(A) (pin P7), ||V^T V - I||_max within the gate, r >= 0, N rows."""
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", f"config{k}_oracle.txt")
+    head, rows = {}, []
+    for ln in open(path):
+        if ln.startswith("#"):
+            continue
+        f = ln.split()
+        if len(f) == 2:
+            head[f[0]] = float(f[1])
+        elif len(f) == 3:
+            rows.append([float(x) for x in f])
+    arr = np.array(rows)
+    c = gen.config(k)
+    d = gen.spectrum(k)
+    assert int(head["N"]) == c.N and arr.shape == (c.N, 3)
+    assert head["alpha"] == gen.alpha_rule(d)
+    A = gen.banded_symmetric(c.N, d, c.amp, c.width, c.seed, gen.STREAM_E)
+    nF = float(np.sqrt(np.sum(A * A)))
+    assert abs(head["normF"] - nF) <= 1e-12 * nF
+    assert abs(arr[:, 0].sum() - np.trace(A)) <= 1e-9            # P7: trace invariant
+    assert head["ortho_max"] <= 1e-12 * c.N
+    assert np.all(arr[:, 1] >= 0.0)
+    # shifts are eigenvalues of principal submatrices: inside A's Gershgorin range; lambda are Rayleigh quotients: same
+    gl = (np.diag(A) - (np.abs(A).sum(1) - np.abs(np.diag(A)))).min()
+    gh = (np.diag(A) + (np.abs(A).sum(1) - np.abs(np.diag(A)))).max()
+    assert arr[:, 0].min() >= gl and arr[:, 0].max() <= gh and arr[:, 2].min() >= gl and arr[:, 2].max() <= gh
+    vec = np.load(path.replace(".txt", "_vectors.npz"))
+    assert np.abs(np.einsum("ij,ij->i", vec["Vr"], vec["Vr"]) - 1.0).max() < 1e-13
+    lam_chk = np.einsum("ij,ij->i", vec["Vr"] @ A, vec["Vr"])       # Rayleigh quotients of the stored vectors
+    assert np.abs(lam_chk - arr[vec["idx"], 0]).max() <= 1e-12 * nF

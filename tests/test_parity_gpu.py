@@ -24,6 +24,10 @@ def dev(a):
 
 _ORACLE_MEMO = {}
 
+# pfsm_set_option settings applied to every handle gpu_solve creates; tests select a kernel route with
+# monkeypatch.setitem(OPTS, key, value) (include/pfsm.h lists the keys).  Empty = the product path.
+OPTS = {}
+
 
 def oracle_step2_memo(A, P, w):
     key = ("step2", A.shape[0], P, w, float(A.sum()), float(np.abs(A).sum()))
@@ -43,7 +47,7 @@ def oracle_pfsm_memo(A, P, w, iters, alpha):
 
 def gpu_solve(A, P, w, iters, alpha, last_step=5):
     N = A.shape[0]
-    h = pfsm.Handle(N, P, w, iters, alpha)
+    h = pfsm.Handle(N, P, w, iters, alpha, options=OPTS)
     dA = dev(A)
     dV = torch.full((N, N), float("nan"), dtype=torch.float64, device="cuda")  # input content must be ignored (R13)
     dl = torch.full((N,), float("nan"), dtype=torch.float64, device="cuda")
@@ -130,8 +134,8 @@ def test_stepwise_parity_small(N, P, w, iters, amp, width):
 @pytest.mark.parametrize("N,P,w", [(256, 4, 16), (270, 6, 4), (600, 3, 20)])
 def test_l2_resident_jacobi_fallback_matches_oracle(N, P, w, monkeypatch):
     # the L2-resident cluster kernel is the fallback for submatrices too large for shared memory; force it
-    monkeypatch.setenv("PFSM_JACOBI", "1")      # (above M = 160 the tridiagonal route is the default)
-    monkeypatch.setenv("PFSM_JACOBI_L2", "1")
+    monkeypatch.setitem(OPTS, "step2_route", 1)      # (above M = 160 the tridiagonal route is the default)
+    monkeypatch.setitem(OPTS, "jacobi_l2", 1)
     p = gen.small_problem(N, 1e-3, 12.0, seed=1000 + N)
     g2 = gpu_solve(p.A, P, w, 1, p.alpha, last_step=2)
     V2, eps, info2 = oracle.step2(p.A, P, w)
@@ -140,9 +144,11 @@ def test_l2_resident_jacobi_fallback_matches_oracle(N, P, w, monkeypatch):
     assert np.abs(align_signs(g2["Vr"], V2) - V2).max() < 1e-9
 
 
-# step-2 routes of the wide-window regime: tridiagonalization (default for M > 512) with full symmetric storage (batch
-# fits L2) or lower-triangle storage (batch larger than L2), and the persistent-grid Jacobi
-WIDE_ROUTES = [("PFSM_TRIDIAG",), ("PFSM_TRIDIAG", "PFSM_SYTRD_HALF"), ("PFSM_JACOBI_WIDE",)]
+# step-2 routes of the wide-window regime: tridiagonalization with full symmetric storage (batch fits L2), lower-triangle
+# storage (batch larger than L2) or blocked (dlatrd-style panels, read-only lower-triangle pass per column, one DMMA rank-2NB
+# trailing update per panel), and the persistent-grid Jacobi
+WIDE_ROUTES = [(("step2_route", 2),), (("step2_route", 2), ("sytrd_storage", 2)), (("step2_route", 3),),
+               (("step2_route", 2), ("sytrd_storage", 3))]   # last: blocked tridiagonalization (panel + DMMA rank-2NB update)
 
 
 @pytest.mark.parametrize("route", WIDE_ROUTES)
@@ -150,8 +156,8 @@ WIDE_ROUTES = [("PFSM_TRIDIAG",), ("PFSM_TRIDIAG", "PFSM_SYTRD_HALF"), ("PFSM_JA
 def test_wide_window_routes_forced_at_small_shapes_match_oracle(N, P, w, route, monkeypatch):
     # the two step-2 routes of the wide-window regime (M > 512), forced at shapes the oracle finishes quickly:
     # several slices per CTA, odd M, one-eigenpair slices, window >= N, more slices than co-resident CTAs
-    for name in route:
-        monkeypatch.setenv(name, "1")
+    for key, value in route:
+        monkeypatch.setitem(OPTS, key, value)
     p = gen.small_problem(N, 1e-3, 12.0, seed=1000 + N)
     g2 = gpu_solve(p.A, P, w, 1, p.alpha, last_step=2)
     V2, eps, info2 = oracle_step2_memo(p.A, P, w)
@@ -166,9 +172,8 @@ def test_wide_window_routes_forced_at_small_shapes_match_oracle(N, P, w, route, 
 @pytest.mark.parametrize("N,P,w,iters", [(1200, 2, 0, 1), (1280, 4, 200, 2), (1102, 2, 1, 1)])
 def test_wide_windows_beyond_512_match_oracle(N, P, w, iters, route, monkeypatch):
     # M = 600, 720 (gamma = 0.56) and 553 (odd); full solve against the oracle
-    for name in route:
-        if name != "PFSM_TRIDIAG":                      # the tridiagonal route is the default beyond M = 512
-            monkeypatch.setenv(name, "1")
+    for key, value in route:                            # (the tridiagonal route is the default beyond M = 160)
+        monkeypatch.setitem(OPTS, key, value)
     p = gen.small_problem(N, 1e-3, 24.0, seed=5000 + N + w)
     g2 = gpu_solve(p.A, P, w, iters, p.alpha, last_step=2)
     V2, eps, info2 = oracle_step2_memo(p.A, P, w)
@@ -185,8 +190,8 @@ def test_wide_window_routes_on_doubly_degenerate_spectrum(route, monkeypatch):
     # A = blockdiag(B, B): every eigenvalue is exactly double.  The eigenvectors of a pair are not unique, so only
     # rotation-invariant quantities are compared (reading R16); the tridiagonal route has no re-orthogonalization
     # inside clusters (reading R25) and must still hand step 4 independent vectors (info = 0)
-    for name in route:
-        monkeypatch.setenv(name, "1")
+    for key, value in route:
+        monkeypatch.setitem(OPTS, key, value)
     n = 96
     B = gen.small_problem(n, 5e-2, 8.0, seed=4242).A
     A = np.zeros((2 * n, 2 * n))
@@ -203,6 +208,39 @@ def test_wide_window_routes_on_doubly_degenerate_spectrum(route, monkeypatch):
         assert np.abs(g["lam"] - ex).max() < 1e-12 * np.linalg.norm(A)
         assert np.abs(g["Vr"] @ g["Vr"].T - np.eye(2 * n)).max() <= 1e-12 * 2 * n
         assert g["resid"].max() < 1e-11 * np.linalg.norm(A)
+
+
+@pytest.mark.parametrize("storage", [0, 2, 3])
+def test_tridiagonal_route_on_near_degenerate_gaps(storage, monkeypatch):
+    # A = Q diag(d) Q^T with pairs of eigenvalues separated by RELATIVE gaps 1e-15 .. 1e-6: too close for inverse iteration
+    # alone (two vectors of a pair come out nearly parallel and step 4 would orthonormalize noise), not exactly equal.
+    # The cluster pass (re-orthogonalization + re-iteration below 1e-7 ||T||, LAPACK dstein's scheme) must hand step 4
+    # well-conditioned vectors: info = 0, eigenvalues and residuals to rounding, for every tridiagonalization kernel.
+    monkeypatch.setitem(OPTS, "step2_route", 2)
+    monkeypatch.setitem(OPTS, "sytrd_storage", storage)
+    gaps = [1e-15, 1e-14, 1e-13, 1e-12, 1e-11, 1e-10, 1e-9, 1e-8, 1e-7, 1e-6]
+    base = np.linspace(-1.0, 1.0, 120)
+    d = np.concatenate([base] + [[base[7 * q + 3] * (1.0 + gp) + (gp if base[7 * q + 3] == 0 else 0.0)] for q, gp in enumerate(gaps)])
+    d = np.sort(d)
+    N = d.size
+    assert N % 2 == 0
+    Q = gen.householder_orthogonal(N, 8, seed=77)
+    A = Q @ np.diag(d) @ Q.T
+    A = 0.5 * (A + A.T)
+    nA = np.linalg.norm(A)
+    alpha = 0.5 / np.abs(d).max() ** 2
+    for P, w in [(1, 0), (2, N)]:                       # M = N: every slice sees all the close pairs
+        g2 = gpu_solve(A, P, w, 1, alpha, last_step=2)
+        assert g2["info"] == 0
+        assert np.abs(g2["eps"] - d).max() < 1e-13 * nA
+        Y = g2["Vr"]
+        assert np.abs(Y @ Y.T - np.eye(N)).max() < 1e-7     # close pairs included: the cluster pass orthogonalized them
+        assert np.abs(Y @ A - g2["eps"][:, None] * Y).max() < 1e-12 * nA
+        g = gpu_solve(A, P, w, 1, alpha)
+        assert g["info"] == 0
+        assert np.abs(g["lam"] - d).max() < 1e-12 * nA
+        assert np.abs(g["Vr"] @ g["Vr"].T - np.eye(N)).max() <= 1e-12 * N
+        assert g["resid"].max() < 1e-11 * nA
 
 
 @pytest.mark.parametrize("mult", [3, 13])
@@ -457,7 +495,7 @@ def test_chained_launches_change_no_bit(N, P, w, iters, monkeypatch):
     launches bit for bit, solve after solve (a tile that started before its operand rows were complete would differ)."""
     p = gen.small_problem(N, 1e-3, 24.0, seed=52000 + N)
     chained = [gpu_solve(p.A, P, w, iters, p.alpha) for _ in range(3)]
-    monkeypatch.setenv("PFSM_NO_CHAIN", "1")
+    monkeypatch.setitem(OPTS, "chain_launches", 0)
     plain = gpu_solve(p.A, P, w, iters, p.alpha)
     for g in chained:
         assert g["info"] == 0
@@ -473,7 +511,7 @@ def test_baseline_configs_full_oracle(k, family, monkeypatch):
     default = the route the library picks (Jacobi for config 0, tridiagonalization for 1, 2 and 5); the other family
     is forced as well."""
     if family != "default":
-        monkeypatch.setenv("PFSM_JACOBI" if family == "jacobi" else "PFSM_TRIDIAG", "1")
+        monkeypatch.setitem(OPTS, "step2_route", 1 if family == "jacobi" else 2)
     p = gen.problem(k)
     c = p.cfg
     g = gpu_solve(p.A, c.P, c.window, c.iters, p.alpha)
@@ -545,23 +583,47 @@ def test_wide_window_config6_at_full_size():
     _check_steps_4_5_at_full_size(p, g3, g, 6)
 
 
-@pytest.mark.parametrize("k,family", [(3, "default"), (4, "default"), (4, "jacobi")])
-def test_baseline_configs_large_sampled(k, family, monkeypatch):
-    """BASELINE.json configs 3-4 at full size, in bench.py's launch configuration.  The full oracle needs
-    ~1e13 flop (minutes), so: steps 2-3 are compared with the oracle on sampled whole slices (slices are
-    independent); step 4 through the uniqueness of QR (V_out orthonormal and V_out^T V_3
-    upper triangular with positive diagonal <=> V_out is THE Gram-Schmidt result); step 5 on sampled
-    columns the oracle computes one by one; trace and residual-enclosure hold at any size.
-    PFSM_FULL_ORACLE=1 adds the full element-by-element comparison.  default = the tridiagonal route of step 2;
-    jacobi = the shared-memory Jacobi (clusters of 8 half CTAs)."""
+def load_golden_large(k):
+    """tests/golden/config{k}_oracle.txt (+ _vectors.npz): the full oracle run of config k, every index, written by
+    tests/golden/make_golden_large.py from oracle/ + pfsm_inputs/ only."""
+    here = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+    head, rows = {}, []
+    for ln in open(os.path.join(here, f"config{k}_oracle.txt")):
+        if ln.startswith("#"):
+            continue
+        f = ln.split()
+        if len(f) == 2:
+            head[f[0]] = float(f[1])
+        elif len(f) == 3:
+            rows.append([float(x) for x in f])
+    arr = np.array(rows)
+    vec = np.load(os.path.join(here, f"config{k}_oracle_vectors.npz"))
+    return head, dict(lam=arr[:, 0], resid=arr[:, 1], eps=arr[:, 2], idx=vec["idx"], Vr=vec["Vr"])
+
+
+@pytest.mark.parametrize("k,family", [(3, "default"), (3, "jacobi"), (4, "default"), (4, "jacobi")])
+def test_baseline_configs_large_all_indices(k, family, monkeypatch):
+    """BASELINE.json configs 3-4 (config 4 = bench.py's headline workload) at full size, in bench.py's launch
+    configuration, against the FULL oracle run on EVERY index: the oracle's lambda, residuals and shifts for all N
+    eigenpairs come from tests/golden/config{k}_oracle.txt (the oracle needs ~1e13 flop per config: minutes, so its
+    output is stored by tests/golden/make_golden_large.py, which calls only oracle/ and pfsm_inputs/).  Gates are
+    north_star's, per index.  On top: steps 2-3 against the live oracle on sampled whole slices (slices are
+    independent), whole eigenvectors against the stored oracle vectors (sign-aligned), step 4 through the
+    uniqueness of QR, trace and residual enclosure.  default = the tridiagonal route of step 2; jacobi = the
+    shared-memory Jacobi (clusters of 8 half CTAs)."""
     if family == "jacobi":
-        monkeypatch.setenv("PFSM_JACOBI", "1")
+        monkeypatch.setitem(OPTS, "step2_route", 1)
     p = gen.problem(k)
     c = p.cfg
     N, m = c.N, c.m
     nF = p.normF
+    head, gold = load_golden_large(k)
+    # the stored run is of THIS matrix and these parameters
+    assert int(head["N"]) == N and head["alpha"] == p.alpha and abs(head["normF"] - nF) <= 1e-12 * nF
+    assert head["ortho_max"] <= 1e-12 * N                                  # the oracle's own orthonormality gate
     g3 = gpu_solve(p.A, c.P, c.window, c.iters, p.alpha, last_step=3)
     assert g3["info"] == 0
+    assert np.abs(g3["eps"] - gold["eps"]).max() <= 1e-12 * nF             # every shift (step 2, all slices)
     M, g0, lo, off = oracle.partition(N, c.P, c.window)
     for s in sorted({0, 1, c.P // 2, c.P - 1}):
         B = p.A[lo[s]:lo[s] + M, lo[s]:lo[s] + M]
@@ -577,10 +639,14 @@ def test_baseline_configs_large_sampled(k, family, monkeypatch):
         Vg = g3["Vr"][g0[s]:g0[s] + m]
         assert np.abs(align_signs(Vg, V3) - V3).max() < 1e-8
     g = gpu_solve(p.A, c.P, c.window, c.iters, p.alpha)
+    assert g["info"] == 0
+    # ---- the north_star gates on all N indices, against the stored full oracle run
+    assert np.abs(g["lam"] - gold["lam"]).max() <= 1e-10 * nF
+    assert np.abs(g["resid"] - gold["resid"]).max() <= 1e-9 * nF
+    assert np.abs(g["eps"] - gold["eps"]).max() <= 1e-12 * nF
+    Vg = g["Vr"][gold["idx"]]
+    assert np.abs(align_signs(Vg, gold["Vr"]) - gold["Vr"]).max() < 1e-7   # whole vectors after step 4 (cond(V) ~ 500 at config 4)
     _check_steps_4_5_at_full_size(p, g3, g, k)
-    if os.environ.get("PFSM_FULL_ORACLE") == "1":
-        o = oracle.pfsm(p.A, c.P, c.window, c.iters, p.alpha)
-        check_gates(p.A, g, o)
 
 
 # ------------------------------------------------------------------ row G: generalized variant A x = lambda S x
@@ -859,7 +925,7 @@ def test_large_submatrices_up_to_the_jacobi_limit(N, P, w, family, monkeypatch):
     # M = 400 and M = 512.  default: the tridiagonal route (cluster-barrier tridiagonalization); jacobi: the
     # shared-memory kernel with a cluster of 8 (M = 400) and the L2-resident fallback with 16 doubles/lane (M = 512)
     if family == "jacobi":
-        monkeypatch.setenv("PFSM_JACOBI", "1")
+        monkeypatch.setitem(OPTS, "step2_route", 1)
     p = gen.small_problem(N, 1e-3, 24.0, seed=5000 + N + w)
     g2 = gpu_solve(p.A, P, w, 1, p.alpha, last_step=2)
     V2, eps, info2 = oracle_step2_memo(p.A, P, w)

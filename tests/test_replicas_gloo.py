@@ -105,3 +105,84 @@ def test_sharded_all_gather_of_row_blocks_gloo():
     want_v = [10.0] * 4 + [20.0] * 4
     for rank, t, v in res:
         assert t == want_t and v == want_v
+
+
+class _RecordingHandle:
+    """Stands in for pfsm.Handle on a CPU-only box: records the phase order and, like the library, leaves only the OWN
+    row block of each phase's output valid (everything else NaN), so a missing or misplaced all-gather shows up."""
+
+    def __init__(self, N, rank, world):
+        import torch
+        self.N, self.rank, self.world = N, rank, world
+        self.calls = []
+        self.bufs = [torch.full((N, N), float("nan"), dtype=torch.float64) for _ in range(2)]
+        self.resid = torch.full((N,), float("nan"), dtype=torch.float64)
+
+    def _own(self):
+        rows = self.N // self.world
+        return slice(self.rank * rows, (self.rank + 1) * rows)
+
+    def shard_phase(self, phase, A, Vr, lam, stream=None):
+        import torch
+        own = self._own()
+        self.calls.append((phase, A is not None, lam is not None))
+        if phase == 1:
+            Vr[own] = 100.0 + self.rank                       # steps 2-3 on the own rows
+        elif phase == 2:
+            assert not torch.isnan(Vr).any(), "phase 2 needs every rank's rows of V (all-gather 1 missing)"
+            self.bufs[0][own] = 200.0 + self.rank             # own block row of G
+        elif phase == 3:
+            assert not torch.isnan(self.bufs[0]).any(), "phase 3 needs all of G (all-gather 2 missing)"
+            self.bufs[1][own] = 300.0 + self.rank             # own rows of the triangular solve
+        elif phase == 4:
+            assert not torch.isnan(self.bufs[1]).any(), "phase 4 needs all of V^T R^-1 (all-gather 3 missing)"
+            Vr[:] = self.bufs[1].T                            # the library transposes the gathered buffer into V
+            lam[own] = 400.0 + self.rank
+            self.resid[own] = 500.0 + self.rank
+
+    def shard_buffer(self, which):
+        return self.bufs[which]
+
+    def residuals_view(self):
+        return self.resid
+
+
+def _sharded_sequence_worker(rank, world, port, q):
+    sys.path.insert(0, ROOT)
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), WORLD_SIZE=str(world), RANK=str(rank))
+    import torch
+    import torch.distributed as dist
+    from paper_1502_07806_b200 import sharded
+    dist.init_process_group("gloo", world_size=world, rank=rank)
+    N = 8
+    h = _RecordingHandle(N, rank, world)
+    A = torch.zeros((N, N), dtype=torch.float64)
+    Vr = torch.full((N, N), float("nan"), dtype=torch.float64)
+    lam = torch.full((N,), float("nan"), dtype=torch.float64)
+    sharded.solve_sharded(h, A, Vr, lam)
+    q.put((rank, h.calls, Vr.tolist(), lam.tolist(), h.resid.tolist(), h.bufs[0].tolist()))
+    dist.destroy_process_group()
+
+
+def test_sharded_solve_sequencing_gloo():
+    """solve_sharded end to end on CPU with a recording fake handle, world size 2: phases run 1-2-3-4 with A passed
+    only where the library reads it (phases 1 and 4) and lambda only in phase 4; after each phase exactly the buffer
+    that phase produced is gathered, so every rank ends with the complete V, lambda, residuals."""
+    world = 2
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_sharded_sequence_worker, args=(r, world, port, q)) for r in range(world)]
+    for p in procs:
+        p.start()
+    res = sorted(q.get(timeout=120) for _ in range(world))
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    want_lam = [400.0] * 4 + [401.0] * 4
+    want_res = [500.0] * 4 + [501.0] * 4
+    want_G = [[200.0] * 8] * 4 + [[201.0] * 8] * 4
+    want_V = np.array([[300.0] * 8] * 4 + [[301.0] * 8] * 4).T.tolist()
+    for rank, calls, V, lam, resid, G in res:
+        assert calls == [(1, True, False), (2, False, False), (3, False, False), (4, True, True)]
+        assert lam == want_lam and resid == want_res and G == want_G and V == want_V
