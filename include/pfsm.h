@@ -234,7 +234,9 @@ int pfsm_set_cholqr_passes(pfsm_handle_t h, int32_t passes);
  *   "jacobi_l2"              1: the L2-resident Jacobi kernel instead of the shared-memory one
  *   "jacobi_cluster_size"    0 auto, or 1 | 2 | 4 | 8 CTAs per slice for the shared-memory Jacobi
  *   "jacobi_full_cta"        1: never use the half-CTA layout of the shared-memory Jacobi
- *   "sytrd_storage"          0 auto (lower triangle once the batch exceeds L2), 1 full storage, 2 lower triangle
+ *   "sytrd_storage"          0 auto (full storage while the batch of submatrices fits L2, lower triangle beyond, blocked
+ *                            -- panels of 32 columns + one DMMA rank-64 trailing update each -- beyond 1.5 x L2),
+ *                            1 full storage, 2 lower triangle, 3 blocked (M even)
  *   "sytrd_grid_barrier"     1: grid barrier instead of thread-block clusters for small M
  *   "cholesky_lookahead"     default 1; 0: step 4 on one stream                                    [PAPER.md:94-96]
  *   "chain_launches"         default 1; 0: the step-3 / step-4 GEMMs in plain stream order (same bits)

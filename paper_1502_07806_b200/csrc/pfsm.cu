@@ -634,8 +634,15 @@ static int launch_tridiag(pfsm_ctx* h, const double* A, double* V, cudaStream_t 
     const int M = h->M;
     int sms = 0;
     PFSM_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, h->device));
-    // Blocked route (panel + DMMA rank-2NB update): option sytrd_storage = 3 (M even: the tensor maps need a 16-byte pitch)
-    const bool blocked = h->opt_sytrd_storage == 3 && (M % 2 == 0) && M >= 4;
+    // Blocked route (panel + DMMA rank-2NB update; M even: the tensor maps need a 16-byte pitch).  Its read-only pass per
+    // column halves the HBM traffic of the lower-triangle kernel but costs two slice barriers and more O(M) work per column,
+    // so it wins once the batch is well beyond L2 (step 2, full / lower / blocked: 1536 x 8 = 151 MB 45 / 42 / 42 ms,
+    // 2048 x 8 = 268 MB 96 / 80 / 69, 2048 x 16 = 537 MB 163 / 120 / 83; 2048 x 4 = 134 MB 60 / 61 / 75).
+    int l2b = 0;
+    PFSM_CUDA(cudaDeviceGetAttribute(&l2b, cudaDevAttrL2CacheSize, h->device));
+    const bool blocked_ok = (M % 2 == 0) && M >= 4;
+    const bool blocked = blocked_ok && (h->opt_sytrd_storage == 3 ||
+                                        (h->opt_sytrd_storage == 0 && (size_t)ns * M * M * sizeof(double) > (size_t)l2b + (size_t)l2b / 2));
     if (blocked) {
         int rcb;
         if ((rcb = launch_sytrd_blocked(h, A, st, s0, ns, precopied))) return rcb;

@@ -252,6 +252,10 @@ sytrd_panel_kernel(double* __restrict__ Gws, int32_t M, TriWs ws, SbWs sb, int32
         // ---------------- phase 1d: symv over this CTA's share of A0's lower triangle ----------------
         // the T tiles of the active triangle (row-major order) are cut into C equal contiguous runs
         for (int i = tid; i < Mp; i += SB_THREADS) ycta[i] = 0.0;
+        if (tid < 256 && k + 1 < M) {  // phase 2 reads A0[i][k+1] of the own rows (a strided column): HBM -> L2 under the pass
+            const int i = 32 * (rb_first + (tid >> 5) * C) + (tid & 31);
+            if (i > k && i < M) asm volatile("prefetch.global.L2 [%0];" ::"l"(G + (size_t)i * M + k + 1));
+        }
         const int nbr = nbk - b0;
         const int T = nbr * (nbr + 1) / 2;
         const int g_lo = (int)((int64_t)c * T / C), g_hi = (int)((int64_t)(c + 1) * T / C);
@@ -270,6 +274,17 @@ sytrd_panel_kernel(double* __restrict__ Gws, int32_t M, TriWs ws, SbWs sb, int32
                     const double* gp = G + (size_t)ib * M + jc;
 #pragma unroll
                     for (int r = 0; r < 32; ++r) b[r] = __ldg(gp + (size_t)r * M);
+                    if (g + SB_NW < sub1) {
+                        // the warp's next tile: HBM -> L2 now, under this tile's loads and arithmetic (lane = row, 256 bytes)
+                        int Rn, Sn;
+                        sb_tile_rc(g + SB_NW, Rn, Sn);
+                        const int in = 32 * (b0 + Rn) + lane;
+                        if (in < M) {
+                            const double* pn = G + (size_t)in * M + 32 * (b0 + Sn);
+                            asm volatile("prefetch.global.L2 [%0];" ::"l"(pn));
+                            asm volatile("prefetch.global.L2 [%0];" ::"l"(pn + 16));
+                        }
+                    }
 #pragma unroll
                     for (int r = 0; r < 32; ++r) {
                         colacc = fma(b[r], vn[ib + r], colacc);
