@@ -237,7 +237,8 @@ int pfsm_set_cholqr_passes(pfsm_handle_t h, int32_t passes);
  *   "sytrd_storage"          0 auto (full storage while the batch of submatrices fits L2, lower triangle beyond, blocked
  *                            -- panels of 32 columns + one DMMA rank-64 trailing update each -- beyond 1.5 x L2),
  *                            1 full storage, 2 lower triangle, 3 blocked (M even)
- *   "sytrd_grid_barrier"     1: grid barrier instead of thread-block clusters for small M
+ *   "sytrd_grid_barrier"     small M (<= 768): 0 = submatrix resident in the cluster's distributed shared memory when it
+ *                            fits (default), 2 = L2-resident submatrix with cluster barriers, 1 = with the grid barrier
  *   "cholesky_lookahead"     default 1; 0: step 4 on one stream                                    [PAPER.md:94-96]
  *   "chain_launches"         default 1; 0: the step-3 / step-4 GEMMs in plain stream order (same bits)
  *   "cholqr_passes"          as pfsm_set_cholqr_passes (1 | 2)

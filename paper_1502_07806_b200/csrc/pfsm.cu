@@ -472,12 +472,14 @@ static void choose_jacobi_layout(pfsm_ctx* h) {
     h->jac_half = false;
     h->jac_wide = h->opt_route == 3;  // option step2_route = 3: the persistent-grid Jacobi kernel at any M
     // Route of step 2.  Tridiagonalization + bisection + inverse iteration + back-transformation costs ~M latency-bound
-    // columns; the Jacobi kernels cost sweeps x (M - 1) rounds.  Measured (step 2, Jacobi -> tridiagonal): M = 96 x 4
-    // slices 0.60 -> 1.00 ms, M = 192 x 16 2.66 -> 2.15, M = 224 x 24 4.57 -> 2.69, M = 254 x 72 13.5 -> 4.9, M = 256 x 64
-    // 12.5 -> 4.0, M = 416 x 13 15.2 -> 5.4 ms.  So: Jacobi up to M = 160, the tridiagonal route above.
+    // columns; the Jacobi kernels cost sweeps x (M - 1) rounds.  With the submatrix resident in the cluster's distributed
+    // shared memory (sytrd_dsmem_kernel) the tridiagonal route wins at every size measured (step 2, Jacobi -> tridiagonal):
+    // M = 32 x 8 slices 0.20 -> 0.17 ms, 64 x 64 0.55 -> 0.34, 96 x 4 0.61 -> 0.46, 128 x 32 1.29 -> 0.68, 160 x 4 1.39 -> 0.77,
+    // 192 x 16 2.66 -> 1.10, 224 x 24 4.57 -> 1.46, 256 x 64 12.5 -> 3.4, 416 x 13 15.2 -> 2.65 ms.  So: the tridiagonal route
+    // from M = 16 on; the shared-memory Jacobi only for tiny submatrices.
     // Option step2_route = 1 / 2 forces one family (M > 512 has no shared-memory / L2 Jacobi: step2_route = 3).
     const bool want_jacobi = h->opt_route == 1 && h->M <= 512;
-    h->tridiag = !h->jac_wide && !want_jacobi && (h->M > 160 || h->opt_route == 2);
+    h->tridiag = !h->jac_wide && !want_jacobi && (h->M >= 16 || h->opt_route == 2);
     if (h->M > 512 || h->jac_wide || h->tridiag) return;
     if (h->opt_jacobi_l2) return;  // option jacobi_l2: force the L2-resident kernel (the large-M fallback)
     const size_t budget = 220 * 1024;
@@ -656,7 +658,8 @@ static int launch_tridiag(pfsm_ctx* h, const double* A, double* V, cudaStream_t 
         PFSM_CUDA(cudaDeviceGetAttribute(&l2, cudaDevAttrL2CacheSize, h->device));
         const bool half = h->opt_sytrd_storage != 1 && (h->opt_sytrd_storage == 2 || (size_t)ns * M * M * sizeof(double) > (size_t)l2);
         // Small submatrices (a column is latency bound): the CTAs of a slice form a cluster and use its barrier
-        bool cluster = !half && M <= 768 && !h->opt_sytrd_grid;
+        const bool small = !half && M <= 768 && h->opt_sytrd_grid != 1;
+        bool cluster = small;
         int ccl = 1;  // cluster size: the largest of 8, 4, 2 that keeps all ns clusters co-resident (one wave)
         if (cluster) {
             PFSM_CUDA(cudaFuncSetAttribute(sytrd_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
@@ -680,6 +683,60 @@ static int launch_tridiag(pfsm_ctx* h, const double* A, double* V, cudaStream_t 
                 if (nmax >= ns) { cluster = true; ccl = c2; }
             }
         }
+        // Small submatrices: resident in the distributed shared memory of the slice's cluster (sytrd_dsmem_kernel) when some
+        // cluster size fits 8 M^2 / C bytes per CTA; the size with the fewest waves wins (a column is latency bound whatever
+        // C is), ties go to the larger cluster.  Option sytrd_grid_barrier = 2 keeps the L2-resident cluster kernel.
+        int dsC = 0;
+        if (small && h->opt_sytrd_grid != 2) {
+            int best_waves = INT_MAX;
+            for (int c2 = 8; c2 >= 1; c2 /= 2) {
+                if (c2 > 1 && c2 * 16 > M + 15) continue;
+                const size_t sm = sytrd_dsmem_bytes(M, c2);
+                if (sm > (size_t)220 * 1024) continue;
+                if (cudaFuncSetAttribute(sytrd_dsmem_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm) != cudaSuccess) {
+                    (void)cudaGetLastError();
+                    continue;
+                }
+                cudaLaunchConfig_t q;
+                memset(&q, 0, sizeof(q));
+                q.gridDim = dim3((unsigned)(ns * c2));
+                q.blockDim = dim3(TRD_THREADS);
+                q.dynamicSmemBytes = sm;
+                cudaLaunchAttribute qa[1];
+                qa[0].id = cudaLaunchAttributeClusterDimension;
+                qa[0].val.clusterDim.x = (unsigned)c2;
+                qa[0].val.clusterDim.y = 1;
+                qa[0].val.clusterDim.z = 1;
+                q.attrs = qa;
+                q.numAttrs = 1;
+                int nmax = 0;
+                if (cudaOccupancyMaxActiveClusters(&nmax, sytrd_dsmem_kernel, &q) != cudaSuccess || nmax < 1) { (void)cudaGetLastError(); continue; }
+                const int waves = (ns + nmax - 1) / nmax;
+                if (waves < best_waves) { best_waves = waves; dsC = c2; }
+            }
+            // measured (step 2, DSMEM / L2-resident): 16 x 192 1.10 / 1.50 ms, 24 x 224 1.46 / 1.99, 13 x 416 2.65 / 3.93,
+            // 64 x 256 (2 waves) 3.43 / 3.54, 72 x 254 (3 waves) 4.52 / 4.33: beyond two waves the L2-resident kernel, whose
+            // clusters are all co-resident, is the faster one
+            if (best_waves > 2) dsC = 0;
+        }
+        if (dsC > 0) {
+            const size_t sm = sytrd_dsmem_bytes(M, dsC);
+            PFSM_CUDA(cudaFuncSetAttribute(sytrd_dsmem_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
+            cudaLaunchConfig_t cfg;
+            memset(&cfg, 0, sizeof(cfg));
+            cfg.gridDim = dim3((unsigned)(ns * dsC));
+            cfg.blockDim = dim3(TRD_THREADS);
+            cfg.dynamicSmemBytes = sm;
+            cfg.stream = st;
+            cudaLaunchAttribute attr[1];
+            attr[0].id = cudaLaunchAttributeClusterDimension;
+            attr[0].val.clusterDim.x = (unsigned)dsC;
+            attr[0].val.clusterDim.y = 1;
+            attr[0].val.clusterDim.z = 1;
+            cfg.attrs = attr;
+            cfg.numAttrs = 1;
+            PFSM_CUDA(cudaLaunchKernelEx(&cfg, sytrd_dsmem_kernel, A, h->N, (int32_t)M, tab, h->Gws, h->tri, h->P, s0, (int32_t)dsC, precopied));
+        } else {
         auto kern = half ? sytrd_half_kernel : (cluster ? sytrd_kernel<true> : sytrd_kernel<false>);
         PFSM_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         int per_sm = 0;
@@ -711,6 +768,7 @@ static int launch_tridiag(pfsm_ctx* h, const double* A, double* V, cudaStream_t 
         PFSM_CUDA(cudaLaunchKernelEx(&cfg, kern, A, h->N, (int32_t)M, tab, h->Gws, h->tri, h->P, s0, ns, (int32_t)C,
                                      h->jw_bar, precopied));
     }
+        }
     const size_t smem2 = 2 * (size_t)M * sizeof(double);
     PFSM_CUDA(cudaFuncSetAttribute(tri_bisect_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem2));
     PFSM_CUDA(cudaFuncSetAttribute(tri_invit_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem2));
@@ -1488,7 +1546,7 @@ int pfsm_set_option(pfsm_handle_t h, const char* key, int64_t value) {
         if (value < 0 || value > 3) return -3;
         h->opt_sytrd_storage = (int32_t)value;
     } else if (!strcmp(key, "sytrd_grid_barrier")) {
-        if (!is01(value)) return -3;
+        if (value < 0 || value > 2) return -3;
         h->opt_sytrd_grid = (int32_t)value;
     } else if (!strcmp(key, "cholesky_lookahead")) {
         if (!is01(value)) return -3;

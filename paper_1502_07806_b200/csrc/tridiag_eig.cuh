@@ -217,6 +217,170 @@ sytrd_kernel(const double* __restrict__ A, int64_t N, int32_t M, SliceTable tab,
 }
 
 // ---------------------------------------------------------------------------------------------
+// The same recurrence with the submatrix RESIDENT IN THE DISTRIBUTED SHARED MEMORY of the slice's cluster (small M: the
+// BASELINE configs, M = 192-256, and the Table-I-shaped case, M = 416).  CTA c of the C-CTA cluster keeps rows i = c (mod C)
+// of B_s in its shared memory for the whole reduction (8 M^2 / C bytes), so the pass over the owned rows is shared-memory
+// traffic only; what crosses CTAs is small and goes through DSMEM: every CTA reads row k from its owner's shared memory
+// (column k of the symmetric matrix), and the owner of row i stores p_k[i] into every CTA's copy of p.  One hardware cluster
+// barrier per column orders those stores; no global-memory round trip is left on the per-column chain (the L2-resident
+// version: ~8 us per column of dependent L2 loads, stores and barriers).  Reflectors, tau, d, e still go to global memory
+// (CTA 0), where the later kernels expect them.  Bitwise identical to sytrd_kernel: same operations in the same order.
+// Dynamic shared memory: Gs[rpc][M], vA[M], vB[M], wp[M], pn[2][M].
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t trd_mapa(uint32_t addr, uint32_t cta) {
+    uint32_t r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(addr), "r"(cta));
+    return r;
+}
+__device__ __forceinline__ double trd_ld_cluster(uint32_t raddr) {
+    double v;
+    asm volatile("ld.shared::cluster.f64 %0, [%1];" : "=d"(v) : "r"(raddr) : "memory");
+    return v;
+}
+__device__ __forceinline__ void trd_st_cluster(uint32_t raddr, double v) {
+    asm volatile("st.shared::cluster.f64 [%0], %1;" ::"r"(raddr), "d"(v) : "memory");
+}
+
+inline size_t sytrd_dsmem_bytes(int M, int C) { return ((size_t)((M + C - 1) / C) * M + 5 * (size_t)M) * sizeof(double); }
+
+__global__ void __launch_bounds__(TRD_THREADS, 1)
+sytrd_dsmem_kernel(const double* __restrict__ A, int64_t N, int32_t M, SliceTable tab, double* __restrict__ Gws, TriWs ws,
+                   int32_t P, int32_t s_off, int32_t C, int32_t precopied) {
+    extern __shared__ double sm[];
+    const int rpc = (M + C - 1) / C;  // rows per CTA
+    double* Gs = sm;                   // own rows: local row li = i / C
+    double* vbuf0 = Gs + (size_t)rpc * M;
+    double* vbuf1 = vbuf0 + M;
+    double* wp = vbuf1 + M;            // w_{k-1}
+    double* pn = wp + M;               // p of the column, [2][M] by column parity; every CTA holds the full vector
+    __shared__ double red[TRD_THREADS / 32];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    constexpr int NW = TRD_THREADS / 32;
+    const int c = (int)cluster_ctarank();
+    const int s = s_off + blockIdx.x / C;
+    const int lo = tab.lo[s];
+    const size_t so = (size_t)s * M;
+    double* G = Gws + (size_t)s * M * M;  // global copy: receives the reflectors
+    const uint32_t Gs_u32 = (uint32_t)__cvta_generic_to_shared(Gs), pn_u32 = (uint32_t)__cvta_generic_to_shared(pn);
+
+    for (int li = warp; li < rpc; li += NW) {  // own rows of B_s (from A, or from the packed blocks pfsm_solve_host uploaded)
+        const int i = li * C + c;
+        if (i >= M) break;
+        const double* a = precopied ? G + (size_t)i * M : A + (size_t)(lo + i) * N + lo;
+        for (int j = lane; j < M; j += 32) Gs[(size_t)li * M + j] = a[j];
+    }
+    for (int i = tid; i < M; i += TRD_THREADS) vbuf0[i] = vbuf1[i] = 0.0;
+    cluster_sync_all();
+
+    double tau_p = 0.0;
+    for (int k = 0; k <= M - 2; ++k) {
+        double* vn = (k & 1) ? vbuf1 : vbuf0;        // v_k
+        const double* vp = (k & 1) ? vbuf0 : vbuf1;  // v_{k-1}
+        // ---- prologue: row k (= column k of the symmetric matrix) from its owner's shared memory
+        double bk[2];  // M <= 1024 = 2 x 512
+        {
+            const uint32_t rrow = trd_mapa(Gs_u32 + (uint32_t)(((size_t)(k / C) * M) * 8), (uint32_t)(k % C));
+#pragma unroll
+            for (int e = 0; e < 2; ++e) {
+                const int i = k + tid + TRD_THREADS * e;
+                bk[e] = (i < M) ? trd_ld_cluster(rrow + 8u * (uint32_t)i) : 0.0;
+            }
+        }
+        if (k > 0) {
+            const double* pv_ = pn + (size_t)((k - 1) & 1) * M;
+            double acc = 0.0;
+            for (int i = k + tid; i < M; i += TRD_THREADS) {
+                const double v = vp[i], p = pv_[i];
+                wp[i] = p;
+                acc = fma(p, v, acc);
+            }
+            const double pv = block_sum_512(acc, red);
+            const double hf = 0.5 * tau_p * pv;
+            for (int i = k + tid; i < M; i += TRD_THREADS) wp[i] = fma(-hf, vp[i], wp[i]);
+            __syncthreads();
+            if (c == 0)  // row k-1 is dead: keep reflector k-1 there (columns k .., leading 1 included)
+                for (int i = k + tid; i < M; i += TRD_THREADS) G[(size_t)(k - 1) * M + i] = vp[i];
+        }
+        double acc = 0.0;
+        {
+            const double wk = (k > 0) ? wp[k] : 0.0, vk = (k > 0) ? vp[k] : 0.0;
+#pragma unroll
+            for (int e = 0; e < 2; ++e) {
+                const int i = k + tid + TRD_THREADS * e;
+                if (i < M) {
+                    double b = bk[e];
+                    if (k > 0) b -= (__dmul_rn(vp[i], wk) + __dmul_rn(wp[i], vk));
+                    vn[i] = b;
+                    if (i >= k + 2) acc = fma(b, b, acc);
+                }
+            }
+        }
+        const double xn2 = block_sum_512(acc, red);  // (its barriers also publish vn)
+        const double dk = vn[k], alpha = vn[k + 1];
+        double tau = 0.0, beta = alpha, scal = 0.0;
+        if (xn2 > 0.0) {
+            beta = -copysign(sqrt(fma(alpha, alpha, xn2)), alpha);
+            tau = (beta - alpha) / beta;
+            scal = 1.0 / (alpha - beta);
+        }
+        __syncthreads();
+        for (int i = k + 1 + tid; i < M; i += TRD_THREADS) vn[i] = (i == k + 1) ? 1.0 : vn[i] * scal;
+        __syncthreads();
+        if (c == 0 && tid == 0) {
+            ws.d[so + k] = dk;
+            ws.e[so + k] = beta;
+            ws.tau[so + k] = tau;
+        }
+        // ---- pass over the owned rows below k (shared memory only); p_k[i] goes to every CTA of the cluster
+        const uint32_t pdst = pn_u32 + (uint32_t)((size_t)(k & 1) * M * 8);
+        int li0 = (k + 1) / C;
+        if (li0 * C + c < k + 1) ++li0;  // first owned row >= k+1
+        for (int li = li0 + warp; li < rpc; li += NW) {
+            const int i = li * C + c;
+            if (i >= M) break;
+            double* row = Gs + (size_t)li * M;
+            const double vi = (k > 0) ? vp[i] : 0.0, wi = (k > 0) ? wp[i] : 0.0;
+            double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
+            int j = k + 1 + lane;
+            for (; j + 96 < M; j += 128) {
+                double b0 = row[j], b1 = row[j + 32], b2 = row[j + 64], b3 = row[j + 96];
+                if (k > 0) {
+                    b0 -= (__dmul_rn(vi, wp[j]) + __dmul_rn(wi, vp[j]));
+                    b1 -= (__dmul_rn(vi, wp[j + 32]) + __dmul_rn(wi, vp[j + 32]));
+                    b2 -= (__dmul_rn(vi, wp[j + 64]) + __dmul_rn(wi, vp[j + 64]));
+                    b3 -= (__dmul_rn(vi, wp[j + 96]) + __dmul_rn(wi, vp[j + 96]));
+                    row[j] = b0;
+                    row[j + 32] = b1;
+                    row[j + 64] = b2;
+                    row[j + 96] = b3;
+                }
+                a0 = fma(b0, vn[j], a0);
+                a1 = fma(b1, vn[j + 32], a1);
+                a2 = fma(b2, vn[j + 64], a2);
+                a3 = fma(b3, vn[j + 96], a3);
+            }
+            for (; j < M; j += 32) {
+                double b0 = row[j];
+                if (k > 0) {
+                    b0 -= (__dmul_rn(vi, wp[j]) + __dmul_rn(wi, vp[j]));
+                    row[j] = b0;
+                }
+                a0 = fma(b0, vn[j], a0);
+            }
+            a0 = warp_sum((a0 + a1) + (a2 + a3));
+            if (lane < C) trd_st_cluster(trd_mapa(pdst + 8u * (uint32_t)i, (uint32_t)lane), tau * a0);
+        }
+        tau_p = tau;
+        cluster_sync_all();
+    }
+    // last diagonal entry (its pending update was applied by the pass of column M-2)
+    if (tid == 0 && (M - 1) % C == c) {
+        ws.d[so + M - 1] = Gs[(size_t)((M - 1) / C) * M + M - 1];
+        ws.e[so + M - 1] = 0.0;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
 // The same recurrence on the LOWER TRIANGLE only (entries j <= i): half the memory traffic, 8 (M-k)^2 bytes per column.
 // The product p = B v needs, for row i, the row part sum_{j<=i} B[i][j] v[j] and the column part sum_{r>i} B[r][i] v[r].
 // The active triangle is cut into 32 x 32 tiles (row block Rb, column strip S <= Rb), dealt cyclically to the warps of

@@ -94,12 +94,15 @@ SMALL_CASES = [
     (250, 4, 10, 2, 1e-3, 12.0),     # P does not divide N (R14): slices of 62, 63, 62, 63
     (500, 7, 20, 3, 1e-3, 16.0),     # slices of 71 / 72, M = 112, tiles straddle uneven slice boundaries
     (64, 64, 3, 1, 1e-3, 4.0),       # one eigenpair per slice
+    (48, 48, 0, 2, 1e-3, 4.0),       # M = 1: every submatrix is one diagonal entry
     (66, 64, 2, 2, 1e-3, 4.0),       # slices of 1 and 2
 ]
 
 
+@pytest.mark.parametrize("route", [0, 1])   # 0 = the library's choice (tridiagonal route from M = 16 on), 1 = the Jacobi kernels
 @pytest.mark.parametrize("N,P,w,iters,amp,width", SMALL_CASES)
-def test_stepwise_parity_small(N, P, w, iters, amp, width):
+def test_stepwise_parity_small(N, P, w, iters, amp, width, route, monkeypatch):
+    monkeypatch.setitem(OPTS, "step2_route", route)
     p = gen.small_problem(N, amp, width, seed=1000 + N)
     nF = p.normF
     # step 2: shifts and zero-padded start vectors
@@ -504,12 +507,12 @@ def test_chained_launches_change_no_bit(N, P, w, iters, monkeypatch):
 
 
 @pytest.mark.parametrize("k,family", [(0, "default"), (1, "default"), (2, "default"), (5, "default"),
-                                      (0, "tridiag"), (1, "jacobi"), (2, "jacobi"), (5, "jacobi")])
+                                      (0, "jacobi"), (1, "jacobi"), (2, "jacobi"), (5, "jacobi")])
 def test_baseline_configs_full_oracle(k, family, monkeypatch):
     """BASELINE.json configs 0-2 at full size, and the Cu256-shaped extra case (N = 1664, window at the paper's
     gamma = 0.25: M = 416, clamped windows on 4 of 13 slices): element-by-element gates against the full oracle run.
-    default = the route the library picks (Jacobi for config 0, tridiagonalization for 1, 2 and 5); the other family
-    is forced as well."""
+    default = the route the library picks (tridiagonalization, submatrices resident in the clusters' distributed shared
+    memory); the Jacobi family is forced as well."""
     if family != "default":
         monkeypatch.setitem(OPTS, "step2_route", 1 if family == "jacobi" else 2)
     p = gen.problem(k)
