@@ -27,7 +27,7 @@
  *   - All matrices are FP64, column-major with leading dimension N.  Eigenvector i is the
  *     contiguous column V + i*N.  A is full storage: both triangles valid and exactly mirrored.
  *   - "device" pointers are CUDA device memory on the device current at pfsm_create; "host"
- *     pointers are ordinary (ideally pinned) host memory.  All must be 16-byte aligned.
+ *     pointers are ordinary (ideally pinned) host memory.  Device matrices must be 16-byte aligned (8 for odd N).
  *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  pfsm_solve
  *     only enqueues work and returns without synchronizing the host.
  *   - Return value: 0 = success; -k = the k-th argument is invalid (LAPACK convention);
@@ -56,15 +56,20 @@ typedef struct pfsm_ctx* pfsm_handle_t; /* opaque */
  * Create a solver for fixed (N, P, window, iters, alpha) and allocate its device workspace
  * (about 5 N^2 doubles + P M^2 doubles) on the current device.           [step 1, PAPER.md:88]
  *   out     host pointer receiving the handle
- *   N       matrix order; N >= 2, even (TMA row pitch must be a multiple of 16 bytes)
+ *   N       matrix order; N >= 2.  Odd N is accepted: tensor maps need a 16-byte row pitch, so internal matrices use the
+ *           leading dimension N + 1 and the caller's matrices (leading dimension N, 8-byte alignment suffices) are staged
+ *           through padded copies (two extra N^2 device buffers, two extra 2-D copies per call); even N runs in place.
+ *           pfsm_set_shard needs an even N.
  *   P       number of spectral slices; 1 <= P <= N.  Slice s holds eigen-indices floor(s N / P) .. floor((s+1) N / P) - 1:
  *           N/P of them when P divides N (the paper writes m = N/P), else floor(N/P) or ceil(N/P) (reading R14)
  *   window  halo rows/columns added on each side of a slice's diagonal block; >= 0.
- *           M = min(N, ceil(N/P) + 2*window), the order of every submatrix, must be <= 4096 in this version
- *           (M <= 160: shared-memory resident cluster Jacobi; 160 < M <= 4096: Householder tridiagonalization +
- *           multi-section + inverse iteration + back-transformation of the slice's own eigenpairs -- this covers the
- *           paper's wide windows, gamma = M/N = 0.2-0.3.  Both deliver the eigenpairs to O(eps ||B||);
- *           the vectors of a tight eigenvalue cluster are accurate to eps ||B|| / gap and are orthonormalized by step 4.)
+ *           M = min(N, ceil(N/P) + 2*window), the order of every submatrix, must be <= 4096 in this version (else -4; the
+ *           paper ran "M <= 3000").  Step 2 is a Householder tridiagonalization + multi-section + inverse
+ *           iteration (with re-orthogonalization inside tight eigenvalue clusters) + back-transformation of the slice's own
+ *           eigenpairs: the submatrix resident in its cluster's distributed shared memory for small M (the BASELINE
+ *           configs), L2- or HBM-resident up to the paper's wide windows, gamma = M/N = 0.2-0.3, where
+ *           it is blocked with DMMA trailing updates.  A shared-memory cluster Jacobi serves M < 16 and is selectable by
+ *           pfsm_set_option.  All routes deliver the eigenpairs to O(eps ||B||).
  *   iters   folded-spectrum iterations of Eq. 11; >= 0
  *   alpha   step length of Eq. 11; finite and > 0.  The library does not estimate spectra:
  *           alpha = 0.5 / max|lambda|^2 keeps every damping factor 1 - alpha (lambda - eps)^2 in [-1, 1].

@@ -547,14 +547,16 @@ __device__ __forceinline__ double block_sum(double v, double* red) {
     return t;
 }
 __global__ void __launch_bounds__(RAY_THREADS)
-rayleigh_kernel(const double* __restrict__ V, const double* __restrict__ T, int64_t N, double* __restrict__ lambda,
+rayleigh_kernel(const double* __restrict__ V, const double* __restrict__ T, int64_t ld, int64_t N, double* __restrict__ lambda,
                 double* __restrict__ resid, int32_t i_off) {
     __shared__ double red[RAY_THREADS / 32];
     const int64_t i = (int64_t)i_off + blockIdx.x;
-    const double2* v2 = reinterpret_cast<const double2*>(V + i * N);
-    const double2* t2 = reinterpret_cast<const double2*>(T + i * N);
-    const int64_t n2 = N / 2;  // N is even
-    double s = 0.0;
+    const double2* v2 = reinterpret_cast<const double2*>(V + i * ld);  // ld is even: rows are 16-byte aligned
+    const double2* t2 = reinterpret_cast<const double2*>(T + i * ld);
+    const int64_t n2 = N / 2;
+    const bool tail = (N & 1) && threadIdx.x == 0;  // odd N: the last component, by thread 0
+    const double vt = tail ? V[i * ld + N - 1] : 0.0, tt = tail ? T[i * ld + N - 1] : 0.0;
+    double s = vt * tt;
 #pragma unroll 4
     for (int64_t k = threadIdx.x; k < n2; k += RAY_THREADS) {
         const double2 a = v2[k], b = t2[k];
@@ -562,7 +564,8 @@ rayleigh_kernel(const double* __restrict__ V, const double* __restrict__ T, int6
         s = fma(a.y, b.y, s);
     }
     const double lam = block_sum(s, red);
-    double q = 0.0;
+    const double et = tt - lam * vt;
+    double q = et * et;
 #pragma unroll 4
     for (int64_t k = threadIdx.x; k < n2; k += RAY_THREADS) {
         const double2 a = v2[k], b = t2[k];

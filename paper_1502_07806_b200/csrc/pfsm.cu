@@ -67,6 +67,11 @@ using namespace pfsm;
 
 struct pfsm_ctx {
     int64_t N;
+    int64_t ld;               // leading dimension of every internal N x N matrix: N rounded up to even (TMA needs a 16-byte row pitch)
+    double* padA = nullptr;   // odd N: the caller's matrices (ld = N) are staged through these (ld = N + 1)
+    double* padB = nullptr;
+    double* padV = nullptr;
+    double* Ub = nullptr;     // pfsm_solve_warm: eigenvectors of the rotated problem
     int32_t P, window, iters, m, M;
     double alpha;
     int device;
@@ -142,6 +147,25 @@ static int check_device(const pfsm_ctx* h) {
     return dev == h->device ? 0 : PFSM_CUDA_ERROR_BASE + (int)cudaErrorInvalidDevice;
 }
 
+// Odd N: a caller matrix (N x N, leading dimension N) cannot be described by a tensor map (its row pitch is not a multiple
+// of 16 bytes), so it is staged through an internal copy with leading dimension ld = N + 1.  Even N: used in place.
+static int copy_mat(double* dst, int64_t dld, const double* src, int64_t sld, int64_t N, cudaStream_t st) {
+    PFSM_CUDA(cudaMemcpy2DAsync(dst, (size_t)dld * sizeof(double), src, (size_t)sld * sizeof(double), (size_t)N * sizeof(double),
+                                (size_t)N, cudaMemcpyDeviceToDevice, st));
+    return 0;
+}
+// *use = src itself (even N) or the padded copy in *pad (allocated on first use; filled when `fill`)
+static int stage_in(pfsm_ctx* h, const double* src, double** pad, double** use, cudaStream_t st, bool fill = true) {
+    if (h->ld == h->N) { *use = const_cast<double*>(src); return 0; }
+    int rc;
+    if (!*pad && (rc = dev_alloc(h, (void**)pad, (size_t)h->N * h->ld * sizeof(double)))) return rc;
+    *use = *pad;
+    return fill ? copy_mat(*pad, h->ld, src, h->N, h->N, st) : 0;
+}
+static int stage_out(pfsm_ctx* h, const double* use, double* dst, cudaStream_t st) {
+    return (use == dst) ? 0 : copy_mat(dst, h->N, use, h->ld, h->N, st);
+}
+
 // mc: tensor map of the matrix C lives in (used by the SUB / UPDATE epilogues to prefetch the C tile into L2)
 template <int EPI>
 // pdl: launch with programmatic stream serialization -- the grid may become resident while the previous gemm_tn_kernel
@@ -195,7 +219,7 @@ extern "C" { static void choose_jacobi_layout(pfsm_ctx* h); }
 static int ensure_tridiag_ws(pfsm_ctx* h) {
     if (!h->tridiag || h->tri.d) return 0;
     const int64_t N = h->N, M = h->M, P = h->P;
-    const size_t pm = (size_t)P * M * sizeof(double), mn = (size_t)M * N;
+    const size_t pm = (size_t)P * M * sizeof(double), mn = (size_t)M * h->ld;
     int rc;
 #define TRYA(x) do { if ((rc = (x))) return rc; } while (0)
     TRYA(dev_alloc(h, (void**)&h->tri.d, pm));
@@ -230,7 +254,7 @@ const char* pfsm_strerror(int code) {
 int pfsm_create(pfsm_handle_t* out, int64_t N, int32_t P, int32_t window, int32_t iters, double alpha) {
     if (!out) return -1;
     *out = nullptr;
-    if (N < 2 || (N & 1) || N > (1 << 30)) return -2;
+    if (N < 2 || N > (1 << 30)) return -2;
     if (P < 1 || P > N) return -3;
     if (window < 0) return -4;
     if (iters < 0) return -5;
@@ -240,7 +264,7 @@ int pfsm_create(pfsm_handle_t* out, int64_t N, int32_t P, int32_t window, int32_
     if (M > JW_MAX_M) return -4;
 
     pfsm_ctx* h = new pfsm_ctx();
-    h->N = N; h->P = P; h->window = window; h->iters = iters; h->alpha = alpha;
+    h->N = N; h->ld = N + (N & 1); h->P = P; h->window = window; h->iters = iters; h->alpha = alpha;
     h->m = (int32_t)m; h->M = (int32_t)M;
     h->nblk = (int32_t)((N + CHOL_NB - 1) / CHOL_NB);
     int rc = 0;
@@ -249,7 +273,8 @@ int pfsm_create(pfsm_handle_t* out, int64_t N, int32_t P, int32_t window, int32_
         cudaError_t e = cudaGetDevice(&h->device);
         if (e != cudaSuccess) { delete h; return PFSM_CUDA_ERROR_BASE + (int)e; }
     }
-    const size_t n2 = (size_t)N * N * sizeof(double);
+    const int64_t L = h->ld;
+    const size_t n2 = (size_t)N * L * sizeof(double);
     TRY(dev_alloc(h, (void**)&h->W, n2));
     TRY(dev_alloc(h, (void**)&h->S, 2 * n2));
     TRY(dev_alloc(h, (void**)&h->O, 2 * n2));
@@ -304,9 +329,9 @@ int pfsm_create(pfsm_handle_t* out, int64_t N, int32_t P, int32_t window, int32_
         if (e == cudaSuccess) e = cudaMemset(h->eps, 0, N * sizeof(double));
         if (e != cudaSuccess) { pfsm_destroy(h); return PFSM_CUDA_ERROR_BASE + (int)e; }
     }
-    TRY(make_map(&h->mapW, h->W, N, N, N));
-    TRY(make_map(&h->mapS, h->S, 2 * N, N, N));
-    TRY(make_map(&h->mapO, h->O, 2 * N, N, N));
+    TRY(make_map(&h->mapW, h->W, N, N, L));
+    TRY(make_map(&h->mapS, h->S, 2 * N, N, L));
+    TRY(make_map(&h->mapO, h->O, 2 * N, N, L));
     TRY(make_map(&h->mapD, h->Dinv, (int64_t)h->nblk * CHOL_NB, CHOL_NB, CHOL_NB));
     for (int i = 0; i < 5; ++i) {
         cudaError_t e = cudaEventCreate(&h->ev[i]);
@@ -333,7 +358,7 @@ int pfsm_destroy(pfsm_handle_t h) {
     if (cur != h->device) cudaSetDevice(h->device);
     cudaDeviceSynchronize();
     void* ptrs[] = {h->W, h->S, h->O, h->Dinv, h->Gws, h->eps, h->resid, h->gdiag, h->rotcnt, h->nrm_g, h->jw_bar, h->slice_tab, h->krange, h->info, h->chain_cnt,
-                    h->A_stage, h->V_stage, h->lam_stage, h->Ap, h->LT, h->DinvT,
+                    h->A_stage, h->V_stage, h->lam_stage, h->Ap, h->LT, h->DinvT, h->padA, h->padB, h->padV, h->Ub,
                     h->tri.d, h->tri.e, h->tri.tau, h->tri.pbuf, h->tri.vbuf, h->tri.rowbuf, h->tri.colbuf, h->tri.colk, h->tri.lam, h->tri.zscale,
                     h->tri.f[0], h->tri.f[1], h->tri.f[2], h->tri.f[3], h->tri.f[4], h->tri.piv,
                     h->sbw.VW, h->sbw.WV, h->sbw.ypart, h->sbw.y, h->sbw.base, h->sbw.dots, h->sbw.yv, h->sbw.sbar};
@@ -377,7 +402,7 @@ static int launch_jacobi_t(pfsm_ctx* h, const double* A, double* V, cudaStream_t
     attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
-    PFSM_CUDA(cudaLaunchKernelEx(&cfg, jacobi_batched_kernel<EPL>, A, h->N, h->M, tab, h->Gws, V, h->eps,
+    PFSM_CUDA(cudaLaunchKernelEx(&cfg, jacobi_batched_kernel<EPL>, A, h->ld, h->M, tab, h->Gws, V, h->eps,
                                  h->rotcnt, h->info, s0));
     return 0;
 }
@@ -404,7 +429,7 @@ static int launch_jacobi_smem_t(pfsm_ctx* h, const double* A, double* V, cudaStr
     attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
-    PFSM_CUDA(cudaLaunchKernelEx(&cfg, jacobi_smem_kernel<EPL, HALF>, A, h->N, h->M, (int32_t)h->jac_hloc, tab,
+    PFSM_CUDA(cudaLaunchKernelEx(&cfg, jacobi_smem_kernel<EPL, HALF>, A, h->ld, h->M, (int32_t)h->jac_hloc, tab,
                                  h->nrm_g, V, h->eps, h->rotcnt, h->info, s0, compact));
     return 0;
 }
@@ -550,7 +575,7 @@ static int launch_jacobi_wide_t(pfsm_ctx* h, const double* A, double* V, cudaStr
     attr[0].val.cooperative = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
-    PFSM_CUDA(cudaLaunchKernelEx(&cfg, jacobi_wide_kernel<EPT>, A, h->N, h->M, tab, h->Gws, h->nrm_g, V, h->eps,
+    PFSM_CUDA(cudaLaunchKernelEx(&cfg, jacobi_wide_kernel<EPT>, A, h->ld, h->M, tab, h->Gws, h->nrm_g, V, h->eps,
                                  h->rotcnt, h->info, s0, ns, h->jw_bar));
     return 0;
 }
@@ -587,7 +612,7 @@ static int launch_sytrd_blocked(pfsm_ctx* h, const double* A, cudaStream_t st, i
     int rc;
     if ((rc = ensure_blocked_ws(h))) return rc;
     if (!precopied) {
-        sytrd_copy_kernel<<<dim3((unsigned)M, (unsigned)ns), 256, 0, st>>>(A, h->N, M, tab, h->Gws, s0);
+        sytrd_copy_kernel<<<dim3((unsigned)M, (unsigned)ns), 256, 0, st>>>(A, h->ld, M, tab, h->Gws, s0);
         PFSM_CUDA(cudaGetLastError());
     }
     const int nbk = (M + 31) / 32;
@@ -735,7 +760,7 @@ static int launch_tridiag(pfsm_ctx* h, const double* A, double* V, cudaStream_t 
             attr[0].val.clusterDim.z = 1;
             cfg.attrs = attr;
             cfg.numAttrs = 1;
-            PFSM_CUDA(cudaLaunchKernelEx(&cfg, sytrd_dsmem_kernel, A, h->N, (int32_t)M, tab, h->Gws, h->tri, h->P, s0, (int32_t)dsC, precopied));
+            PFSM_CUDA(cudaLaunchKernelEx(&cfg, sytrd_dsmem_kernel, A, h->ld, (int32_t)M, tab, h->Gws, h->tri, h->P, s0, (int32_t)dsC, precopied));
         } else {
         auto kern = half ? sytrd_half_kernel : (cluster ? sytrd_kernel<true> : sytrd_kernel<false>);
         PFSM_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
@@ -765,7 +790,7 @@ static int launch_tridiag(pfsm_ctx* h, const double* A, double* V, cudaStream_t 
         }
         cfg.attrs = attr;
         cfg.numAttrs = 1;
-        PFSM_CUDA(cudaLaunchKernelEx(&cfg, kern, A, h->N, (int32_t)M, tab, h->Gws, h->tri, h->P, s0, ns, (int32_t)C,
+        PFSM_CUDA(cudaLaunchKernelEx(&cfg, kern, A, h->ld, (int32_t)M, tab, h->Gws, h->tri, h->P, s0, ns, (int32_t)C,
                                      h->jw_bar, precopied));
     }
         }
@@ -776,15 +801,15 @@ static int launch_tridiag(pfsm_ctx* h, const double* A, double* V, cudaStream_t 
     const dim3 g2b((unsigned)((h->m + TRI_THREADS / 32 - 1) / (TRI_THREADS / 32)), (unsigned)ns);
     tri_bisect_kernel<<<g2b, TRI_THREADS, smem2, st>>>((int32_t)M, tab, h->tri, s0);
     PFSM_CUDA(cudaGetLastError());
-    tri_invit_kernel<<<g2, TRI_THREADS, smem2, st>>>(h->N, (int32_t)M, tab, h->tri, s0, h->info);
+    tri_invit_kernel<<<g2, TRI_THREADS, smem2, st>>>(h->ld, (int32_t)M, tab, h->tri, s0, h->info);
     PFSM_CUDA(cudaGetLastError());
-    tri_cluster_kernel<<<(unsigned)ns, TRC_THREADS, 0, st>>>(h->N, (int32_t)M, tab, h->tri, s0);
+    tri_cluster_kernel<<<(unsigned)ns, TRC_THREADS, 0, st>>>(h->ld, (int32_t)M, tab, h->tri, s0);
     PFSM_CUDA(cudaGetLastError());
     {
         const int ept = (M + BT_THREADS - 1) / BT_THREADS;
         const int nvec = ept <= 8 ? 8 : 4;
         const dim3 g3((unsigned)((h->m + nvec - 1) / nvec), (unsigned)ns);
-#define PFSM_BT(E, NVEC) tri_backtransform_kernel<E, NVEC><<<g3, BT_THREADS, 0, st>>>(h->N, (int32_t)M, tab, h->Gws, h->tri, V, h->eps, s0)
+#define PFSM_BT(E, NVEC) tri_backtransform_kernel<E, NVEC><<<g3, BT_THREADS, 0, st>>>(h->ld, (int32_t)M, tab, h->Gws, h->tri, V, h->eps, s0)
         if (ept <= 1) PFSM_BT(1, 8);
         else if (ept <= 2) PFSM_BT(2, 8);
         else if (ept <= 4) PFSM_BT(4, 8);
@@ -845,7 +870,7 @@ static int launch_jacobi(pfsm_ctx* h, const double* A, double* V, cudaStream_t s
 // update is applied once per PAIR of panels with K = 256, halving how often every C tile is read and re-written.
 // b0, b1: only the bottom rows [N + b0, N + b1) are transformed (a rank of the sharded solve owns a row block of Z).
 static int stacked_cholesky(pfsm_ctx* h, bool factor, cudaStream_t st, int32_t b0 = 0, int32_t b1 = -1) {
-    const int64_t N = h->N;
+    const int64_t N = h->N, L = h->ld;
     const int32_t n = (int32_t)N;
     if (b1 < 0) b1 = n;
     const bool whole = factor && b0 == 0 && b1 == n;  // top and bottom rows form one contiguous row range
@@ -860,14 +885,14 @@ static int stacked_cholesky(pfsm_ctx* h, bool factor, cudaStream_t st, int32_t b
         if (nr <= 0) return 0;
         const int32_t k0 = k * CHOL_NB, nb = (int32_t)std::min<int64_t>(CHOL_NB, N - k0);
         GemmParams pp = base_params();
-        pp.C = h->O; pp.ldc = N; pp.cr0 = r0; pp.cc0 = k0; pp.mr = nr; pp.nc = nb;
+        pp.C = h->O; pp.ldc = L; pp.cr0 = r0; pp.cc0 = k0; pp.mr = nr; pp.nc = nb;
         pp.xr0 = r0; pp.xk0 = k0; pp.yr0 = k * CHOL_NB; pp.yk0 = 0; pp.klen = nb;
         return launch_gemm<EPI_PLAIN>(h, h->mapS, h->mapD, h->mapO, pp, cs);
     };
     auto factor_panel = [&](int32_t k) -> int {
         const int32_t k0 = k * CHOL_NB, nb = (int32_t)std::min<int64_t>(CHOL_NB, N - k0);
         if (factor) {
-            chol_diag_kernel<<<1, CHOL_THREADS, CHOL_SMEM, cs>>>(h->S, h->O, N, k0, nb,
+            chol_diag_kernel<<<1, CHOL_THREADS, CHOL_SMEM, cs>>>(h->S, h->O, L, k0, nb,
                                                                  h->Dinv + (size_t)k * CHOL_NB * CHOL_NB, h->gdiag, h->info);
             PFSM_CUDA(cudaGetLastError());
         }
@@ -879,7 +904,7 @@ static int stacked_cholesky(pfsm_ctx* h, bool factor, cudaStream_t st, int32_t b
     auto update_rows = [&](int32_t r0, int32_t nr, int32_t c0, int32_t ncols, int32_t kk0, int32_t klen, int lower) -> int {
         if (ncols <= 0 || nr <= 0) return 0;
         GemmParams pt = base_params();
-        pt.C = h->S; pt.ldc = N; pt.cr0 = r0; pt.cc0 = c0; pt.mr = nr; pt.nc = ncols;
+        pt.C = h->S; pt.ldc = L; pt.cr0 = r0; pt.cc0 = c0; pt.mr = nr; pt.nc = ncols;
         pt.xr0 = r0; pt.yr0 = c0; pt.xk0 = kk0; pt.yk0 = kk0; pt.klen = klen; pt.lower = lower;
         return launch_gemm<EPI_SUB>(h, h->mapO, h->mapO, h->mapS, pt, cs);
     };
@@ -946,25 +971,25 @@ static int stacked_cholesky(pfsm_ctx* h, bool factor, cudaStream_t st, int32_t b
 // to it (row-block counters, see the step-3 loop) and starts on the SMs that wave leaves idle.
 static int run_step4_once(pfsm_ctx* h, const CUtensorMap& mapV, double* V, cudaStream_t st,
                           const int32_t* wait_cnt = nullptr, int32_t wait_target = 0) {
-    const int64_t N = h->N;
+    const int64_t N = h->N, L = h->ld;
     const int32_t n = (int32_t)N;
     int rc;
     const dim3 tb(32, 8), tg((unsigned)((N + 31) / 32), (unsigned)((N + 31) / 32));
     GemmParams p = base_params();
-    p.C = h->S; p.ldc = N; p.mr = n; p.nc = n; p.klen = n; p.lower = 2;
+    p.C = h->S; p.ldc = L; p.mr = n; p.nc = n; p.klen = n; p.lower = 2;
     p.wait_cnt = wait_cnt; p.wait_target = wait_target;
     if (wait_cnt) {
         if ((rc = launch_gemm<EPI_PLAIN>(h, mapV, mapV, h->mapS, p, st, true))) return rc;
     }
-    transpose_kernel<<<tg, tb, 0, st>>>(V, N, h->S + (size_t)N * N, N, n, n);
+    transpose_kernel<<<tg, tb, 0, st>>>(V, L, h->S + (size_t)N * L, L, n, n);
     PFSM_CUDA(cudaGetLastError());
     if (!wait_cnt) {
         if ((rc = launch_gemm<EPI_PLAIN>(h, mapV, mapV, h->mapS, p, st))) return rc;
     }
-    extract_diag_kernel<<<(unsigned)((N + 255) / 256), 256, 0, st>>>(h->S, N, n, h->gdiag);
+    extract_diag_kernel<<<(unsigned)((N + 255) / 256), 256, 0, st>>>(h->S, L, n, h->gdiag);
     PFSM_CUDA(cudaGetLastError());
     if ((rc = stacked_cholesky(h, true, st))) return rc;
-    transpose_kernel<<<tg, tb, 0, st>>>(h->O + (size_t)N * N, N, V, N, n, n);
+    transpose_kernel<<<tg, tb, 0, st>>>(h->O + (size_t)N * L, L, V, L, n, n);
     PFSM_CUDA(cudaGetLastError());
     return 0;
 }
@@ -988,7 +1013,7 @@ static int launch_rayleigh(pfsm_ctx* h, const double* V, double* lambda_out, int
     const size_t in_flight = (size_t)h->sms * 8 * 16 * (size_t)h->N;
     const size_t smem = in_flight > ((size_t)48 << 20) ? RAY_CAP_SMEM : 0;
     if (smem) PFSM_CUDA(cudaFuncSetAttribute(rayleigh_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    rayleigh_kernel<<<(unsigned)rows, RAY_THREADS, smem, st>>>(V, h->W, h->N, lambda_out, h->resid, r0);
+    rayleigh_kernel<<<(unsigned)rows, RAY_THREADS, smem, st>>>(V, h->W, h->ld, h->N, lambda_out, h->resid, r0);
     PFSM_CUDA(cudaGetLastError());
     return 0;
 }
@@ -996,12 +1021,12 @@ static int launch_rayleigh(pfsm_ctx* h, const double* V, double* lambda_out, int
 // ---- step 5 (reading R11): T = V A, Rayleigh quotients and residual norms ----
 static int run_step5(pfsm_ctx* h, const CUtensorMap& mapV, const CUtensorMap& mapA, double* V, double* lambda_out,
                      cudaStream_t st) {
-    const int64_t N = h->N;
+    const int64_t N = h->N, L = h->ld;
     const int32_t n = (int32_t)N;
     int rc;
     {
         GemmParams p = base_params();
-        p.C = h->W; p.ldc = N; p.mr = n; p.nc = n; p.klen = n;
+        p.C = h->W; p.ldc = L; p.mr = n; p.nc = n; p.klen = n;
         if ((rc = launch_gemm<EPI_PLAIN>(h, mapV, mapA, h->mapW, p, st))) return rc;
         if ((rc = launch_rayleigh(h, V, lambda_out, 0, n, st))) return rc;
     }
@@ -1016,7 +1041,7 @@ static int run_step5(pfsm_ctx* h, const CUtensorMap& mapV, const CUtensorMap& ma
 // its own row range (rows / BM row blocks).  *last_cnt = the counters of the last update (nullptr when not chained).
 static int run_step3(pfsm_ctx* h, const CUtensorMap& mapV, const CUtensorMap& mapA, double* V, int32_t r0, int32_t rows,
                      cudaStream_t st, const int32_t** last_cnt) {
-    const int64_t N = h->N;
+    const int64_t N = h->N, L = h->ld;
     const int32_t n = (int32_t)N;
     const int32_t nrb = (rows + BM - 1) / BM, ncb = (n + BN - 1) / BN;
     const bool chain = h->chain && h->iters > 0;
@@ -1025,12 +1050,12 @@ static int run_step3(pfsm_ctx* h, const CUtensorMap& mapV, const CUtensorMap& ma
     if (chain) PFSM_CUDA(cudaMemsetAsync(h->chain_cnt, 0, (size_t)2 * h->iters * nrb * sizeof(int32_t), st));
     for (int it = 0; it < h->iters; ++it) {
         GemmParams p = base_params();  // W = V A - diag(eps) V   (row-major view; A symmetric)
-        p.C = h->W; p.ldc = N; p.cr0 = r0; p.xr0 = r0; p.mr = rows; p.nc = n; p.klen = n;
+        p.C = h->W; p.ldc = L; p.cr0 = r0; p.xr0 = r0; p.mr = rows; p.nc = n; p.klen = n;
         p.krange = (it == 0) ? h->krange + r0 / BM : nullptr;  // start vectors are zero outside their window
-        p.E1 = V; p.ld1 = N; p.eps = h->eps;
+        p.E1 = V; p.ld1 = L; p.eps = h->eps;
         GemmParams q = base_params();  // V <- V - alpha (W A - diag(eps) W)
-        q.C = V; q.ldc = N; q.cr0 = r0; q.xr0 = r0; q.mr = rows; q.nc = n; q.klen = n;
-        q.E1 = h->W; q.ld1 = N; q.E2 = V; q.ld2 = N; q.eps = h->eps; q.alpha = h->alpha;
+        q.C = V; q.ldc = L; q.cr0 = r0; q.xr0 = r0; q.mr = rows; q.nc = n; q.klen = n;
+        q.E1 = h->W; q.ld1 = L; q.E2 = V; q.ld2 = L; q.eps = h->eps; q.alpha = h->alpha;
         if (chain) {
             int32_t* c0 = h->chain_cnt + (size_t)(2 * it) * nrb;
             p.signal_cnt = c0;
@@ -1047,7 +1072,8 @@ static int run_step3(pfsm_ctx* h, const CUtensorMap& mapV, const CUtensorMap& ma
 
 // band != nullptr: packed copy of the P diagonal blocks for step 2 (A itself may still be in flight on the side
 // stream; `a_ready` is waited for before step 3 reads it)
-static int solve_impl(pfsm_handle_t h, const double* A, double* V, double* lambda_out, void* stream, int32_t last_step,
+// A, V: leading dimension h->ld (the caller's own matrices when N is even, staged copies when it is odd)
+static int solve_core(pfsm_handle_t h, const double* A, double* V, double* lambda_out, void* stream, int32_t last_step,
                       const double* band, cudaEvent_t a_ready) {
     if (!h) return -1;
     if (int rc_dev = check_device(h)) return rc_dev;
@@ -1056,19 +1082,19 @@ static int solve_impl(pfsm_handle_t h, const double* A, double* V, double* lambd
     if (last_step < 2 || last_step > 5) return -6;
     if (last_step == 5 && (!lambda_out || ((uintptr_t)lambda_out & 7))) return -4;
     cudaStream_t st = (cudaStream_t)stream;
-    const int64_t N = h->N;
+    const int64_t N = h->N, L = h->ld;
     const int32_t n = (int32_t)N;
     int rc;
     CUtensorMap mapA, mapV;
-    if ((rc = make_map(&mapA, A, N, N, N))) return rc;
-    if ((rc = make_map(&mapV, V, N, N, N))) return rc;
+    if ((rc = make_map(&mapA, A, N, N, L))) return rc;
+    if ((rc = make_map(&mapV, V, N, N, L))) return rc;
     const bool tm = h->timing;
     h->ev_valid = false;
 
     // ---- step 2: batched submatrix eigensolves -> shifts and zero-padded start vectors ----
     if (tm) PFSM_CUDA(cudaEventRecord(h->ev[0], st));
     if (!h->keep_info) PFSM_CUDA(cudaMemsetAsync(h->info, 0xFF, sizeof(unsigned long long), st));
-    PFSM_CUDA(cudaMemsetAsync(V, 0, (size_t)N * N * sizeof(double), st));
+    PFSM_CUDA(cudaMemsetAsync(V, 0, (size_t)N * L * sizeof(double), st));
     if ((rc = launch_jacobi(h, band ? band : A, V, st, 0, -1, band ? 1 : 0))) return rc;
     if (band) PFSM_CUDA(cudaStreamWaitEvent(st, a_ready, 0));
     if (tm) PFSM_CUDA(cudaEventRecord(h->ev[1], st));
@@ -1098,71 +1124,90 @@ static int solve_impl(pfsm_handle_t h, const double* A, double* V, double* lambd
 
 int pfsm_solve_partial(pfsm_handle_t h, const double* A, double* V, double* lambda_out, void* stream,
                        int32_t last_step) {
-    return solve_impl(h, A, V, lambda_out, stream, last_step, nullptr, nullptr);
+    if (!h) return -1;
+    if (h->ld == h->N) return solve_core(h, A, V, lambda_out, stream, last_step, nullptr, nullptr);
+    if (int rc_dev = check_device(h)) return rc_dev;
+    if (!A || ((uintptr_t)A & 7)) return -2;
+    if (!V || ((uintptr_t)V & 7)) return -3;
+    cudaStream_t st = (cudaStream_t)stream;
+    double *Au, *Vu;
+    int rc;
+    if ((rc = stage_in(h, A, &h->padA, &Au, st))) return rc;
+    if ((rc = stage_in(h, V, &h->padV, &Vu, st, false))) return rc;
+    if ((rc = solve_core(h, Au, Vu, lambda_out, stream, last_step, nullptr, nullptr))) return rc;
+    return stage_out(h, Vu, V, st);
 }
 
 int pfsm_orthonormalize(pfsm_handle_t h, double* V_inout, void* stream) {
     if (!h) return -1;
     if (int rc_dev = check_device(h)) return rc_dev;
-    if (!V_inout || ((uintptr_t)V_inout & 15)) return -2;
+    if (!V_inout || ((uintptr_t)V_inout & (h->ld == h->N ? 15 : 7))) return -2;
     CUtensorMap mapV;
     int rc;
-    if ((rc = make_map(&mapV, V_inout, h->N, h->N, h->N))) return rc;
     cudaStream_t st = (cudaStream_t)stream;
+    double* Vu;
+    if ((rc = stage_in(h, V_inout, &h->padV, &Vu, st))) return rc;
+    if ((rc = make_map(&mapV, Vu, h->N, h->N, h->ld))) return rc;
     h->ev_valid = false;
     PFSM_CUDA(cudaMemsetAsync(h->info, 0xFF, sizeof(unsigned long long), st));
-    return run_step4(h, mapV, V_inout, st);
+    if ((rc = run_step4(h, mapV, Vu, st))) return rc;
+    return stage_out(h, Vu, V_inout, st);
 }
 
 int pfsm_rayleigh(pfsm_handle_t h, const double* A, const double* V, double* lambda_out, void* stream) {
     if (!h) return -1;
     if (int rc_dev = check_device(h)) return rc_dev;
-    if (!A || ((uintptr_t)A & 15)) return -2;
-    if (!V || ((uintptr_t)V & 15)) return -3;
+    const uintptr_t am = (h->ld == h->N) ? 15 : 7;
+    if (!A || ((uintptr_t)A & am)) return -2;
+    if (!V || ((uintptr_t)V & am)) return -3;
     if (!lambda_out || ((uintptr_t)lambda_out & 7)) return -4;
     CUtensorMap mapA, mapV;
     int rc;
-    if ((rc = make_map(&mapA, A, h->N, h->N, h->N))) return rc;
-    if ((rc = make_map(&mapV, V, h->N, h->N, h->N))) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    double *Au, *Vu;
+    if ((rc = stage_in(h, A, &h->padA, &Au, st))) return rc;
+    if ((rc = stage_in(h, V, &h->padV, &Vu, st))) return rc;
+    if ((rc = make_map(&mapA, Au, h->N, h->N, h->ld))) return rc;
+    if ((rc = make_map(&mapV, Vu, h->N, h->N, h->ld))) return rc;
     h->ev_valid = false;
-    return run_step5(h, mapV, mapA, const_cast<double*>(V), lambda_out, (cudaStream_t)stream);
+    return run_step5(h, mapV, mapA, Vu, lambda_out, st);
 }
 
 // ---- Row G (BASELINE.json configs[4], Eq. 13): A x = lambda S x reduced by Cholesky(S) ----
 static int ensure_generalized(pfsm_ctx* h) {
     if (h->Ap) return 0;
-    const int64_t N = h->N;
-    const size_t n2 = (size_t)N * N * sizeof(double);
+    const int64_t N = h->N, L = h->ld;
+    const size_t n2 = (size_t)N * L * sizeof(double);
     int rc;
     if ((rc = dev_alloc(h, (void**)&h->Ap, n2))) return rc;
     if ((rc = dev_alloc(h, (void**)&h->LT, n2))) return rc;
     if ((rc = dev_alloc(h, (void**)&h->DinvT, (size_t)h->nblk * CHOL_NB * CHOL_NB * sizeof(double)))) return rc;
-    if ((rc = make_map(&h->mapAp, h->Ap, N, N, N))) return rc;
-    if ((rc = make_map(&h->mapLT, h->LT, N, N, N))) return rc;
+    if ((rc = make_map(&h->mapAp, h->Ap, N, N, L))) return rc;
+    if ((rc = make_map(&h->mapLT, h->LT, N, N, L))) return rc;
     if ((rc = make_map(&h->mapDT, h->DinvT, (int64_t)h->nblk * CHOL_NB, CHOL_NB, CHOL_NB))) return rc;
     return 0;
 }
 
 // S = L L^T;  Ap = L^-1 A L^-T (symmetrized);  keeps L^T and the transposed inverted diagonal blocks for the
 // back-transformation.  Two passes of the stacked Cholesky: [S ; A] -> A L^-T, then [.; (A L^-T)^T] -> L^-1 A L^-T.
-static int run_generalized_reduce(pfsm_ctx* h, const double* A, const double* S_in, double* Ap_out, cudaStream_t st) {
-    const int64_t N = h->N;
+// A, S_in: the caller's matrices (leading dimension N); Ap_out: leading dimension ldo
+static int run_generalized_reduce(pfsm_ctx* h, const double* A, const double* S_in, double* Ap_out, int64_t ldo, cudaStream_t st) {
+    const int64_t N = h->N, L = h->ld;
     const int32_t n = (int32_t)N;
-    const size_t n2 = (size_t)N * N * sizeof(double);
     int rc;
     const dim3 tb(32, 8), tg((unsigned)((N + 31) / 32), (unsigned)((N + 31) / 32));
     PFSM_CUDA(cudaMemsetAsync(h->info, 0xFF, sizeof(unsigned long long), st));
-    PFSM_CUDA(cudaMemcpyAsync(h->S, S_in, n2, cudaMemcpyDeviceToDevice, st));
-    PFSM_CUDA(cudaMemcpyAsync(h->S + (size_t)N * N, A, n2, cudaMemcpyDeviceToDevice, st));
-    extract_diag_kernel<<<(unsigned)((N + 255) / 256), 256, 0, st>>>(h->S, N, n, h->gdiag);
+    if ((rc = copy_mat(h->S, L, S_in, N, N, st))) return rc;
+    if ((rc = copy_mat(h->S + (size_t)N * L, L, A, N, N, st))) return rc;
+    extract_diag_kernel<<<(unsigned)((N + 255) / 256), 256, 0, st>>>(h->S, L, n, h->gdiag);
     PFSM_CUDA(cudaGetLastError());
     if ((rc = stacked_cholesky(h, true, st))) return rc;                       // O = [L ; A L^-T]
-    transpose_kernel<<<tg, tb, 0, st>>>(h->O + (size_t)N * N, N, h->S + (size_t)N * N, N, n, n);  // (A L^-T)^T = L^-1 A
+    transpose_kernel<<<tg, tb, 0, st>>>(h->O + (size_t)N * L, L, h->S + (size_t)N * L, L, n, n);  // (A L^-T)^T = L^-1 A
     PFSM_CUDA(cudaGetLastError());
     if ((rc = stacked_cholesky(h, false, st))) return rc;                      // O bottom = L^-1 A L^-T
-    symmetrize_kernel<<<tg, tb, 0, st>>>(h->O + (size_t)N * N, N, Ap_out, N, n);
+    symmetrize_kernel<<<tg, tb, 0, st>>>(h->O + (size_t)N * L, L, Ap_out, ldo, n);
     PFSM_CUDA(cudaGetLastError());
-    transpose_kernel<<<tg, tb, 0, st>>>(h->O, N, h->LT, N, n, n);
+    transpose_kernel<<<tg, tb, 0, st>>>(h->O, L, h->LT, L, n, n);
     PFSM_CUDA(cudaGetLastError());
     transpose_blocks_kernel<<<dim3(4, 4, (unsigned)h->nblk), tb, 0, st>>>(h->Dinv, h->DinvT);
     PFSM_CUDA(cudaGetLastError());
@@ -1170,60 +1215,64 @@ static int run_generalized_reduce(pfsm_ctx* h, const double* A, const double* S_
 }
 
 // X = L^-T V, in the row-major view X_rm = V_rm L^-1: block back-substitution from the last panel to the first,
-// X_k = R_k L_kk^-1, then R[:, c] -= X_k L[k, c] for the column blocks c < k.  R = V in place, X collected in W.
+// X_k = R_k L_kk^-1, then R[:, c] -= X_k L[k, c] for the column blocks c < k.  All in place in V: the tile that forms
+// X_k[r] reads exactly the block R_k[r] it overwrites (every read of the main loop precedes the epilogue's stores), and
+// column block k is not touched again, so no second matrix and no final copy are needed.
 static int run_generalized_back(pfsm_ctx* h, double* V, cudaStream_t st) {
-    const int64_t N = h->N;
+    const int64_t N = h->N, L = h->ld;
     const int32_t n = (int32_t)N;
     int rc;
     CUtensorMap mapV;
-    if ((rc = make_map(&mapV, V, N, N, N))) return rc;
+    if ((rc = make_map(&mapV, V, N, N, L))) return rc;
     for (int32_t k = h->nblk - 1; k >= 0; --k) {
         const int32_t k0 = k * CHOL_NB, nb = (int32_t)std::min<int64_t>(CHOL_NB, N - k0);
         GemmParams pp = base_params();
-        pp.C = h->W; pp.ldc = N; pp.cr0 = 0; pp.cc0 = k0; pp.mr = n; pp.nc = nb;
+        pp.C = V; pp.ldc = L; pp.cr0 = 0; pp.cc0 = k0; pp.mr = n; pp.nc = nb;
         pp.xr0 = 0; pp.xk0 = k0; pp.yr0 = k * CHOL_NB; pp.yk0 = 0; pp.klen = nb;
-        if ((rc = launch_gemm<EPI_PLAIN>(h, mapV, h->mapDT, h->mapW, pp, st))) return rc;
+        if ((rc = launch_gemm<EPI_PLAIN>(h, mapV, h->mapDT, mapV, pp, st))) return rc;
         if (k0 > 0) {
             GemmParams pt = base_params();
-            pt.C = V; pt.ldc = N; pt.cr0 = 0; pt.cc0 = 0; pt.mr = n; pt.nc = k0;
+            pt.C = V; pt.ldc = L; pt.cr0 = 0; pt.cc0 = 0; pt.mr = n; pt.nc = k0;
             pt.xr0 = 0; pt.xk0 = k0; pt.yr0 = 0; pt.yk0 = k0; pt.klen = nb;
-            if ((rc = launch_gemm<EPI_SUB>(h, h->mapW, h->mapLT, mapV, pt, st))) return rc;
+            if ((rc = launch_gemm<EPI_SUB>(h, mapV, h->mapLT, mapV, pt, st))) return rc;
         }
     }
-    PFSM_CUDA(cudaMemcpyAsync(V, h->W, (size_t)N * N * sizeof(double), cudaMemcpyDeviceToDevice, st));
     return 0;
 }
 
 int pfsm_generalized_reduce(pfsm_handle_t h, const double* A, const double* S, double* Ap_out, void* stream) {
     if (!h) return -1;
     if (int rc_dev = check_device(h)) return rc_dev;
-    if (!A || ((uintptr_t)A & 15)) return -2;
-    if (!S || ((uintptr_t)S & 15)) return -3;
-    if (!Ap_out || ((uintptr_t)Ap_out & 15)) return -4;
+    if (!A || ((uintptr_t)A & 7)) return -2;
+    if (!S || ((uintptr_t)S & 7)) return -3;
+    if (!Ap_out || ((uintptr_t)Ap_out & 7)) return -4;
     int rc;
     if ((rc = ensure_generalized(h))) return rc;
     h->ev_valid = false;
-    return run_generalized_reduce(h, A, S, Ap_out, (cudaStream_t)stream);
+    return run_generalized_reduce(h, A, S, Ap_out, h->N, (cudaStream_t)stream);
 }
 
 int pfsm_solve_generalized(pfsm_handle_t h, const double* A, const double* S, double* X_out, double* lambda_out,
                            void* stream) {
     if (!h) return -1;
     if (int rc_dev = check_device(h)) return rc_dev;
-    if (!A || ((uintptr_t)A & 15)) return -2;
-    if (!S || ((uintptr_t)S & 15)) return -3;
-    if (!X_out || ((uintptr_t)X_out & 15)) return -4;
+    if (!A || ((uintptr_t)A & 7)) return -2;
+    if (!S || ((uintptr_t)S & 7)) return -3;
+    if (!X_out || ((uintptr_t)X_out & (h->ld == h->N ? 15 : 7))) return -4;
     if (!lambda_out || ((uintptr_t)lambda_out & 7)) return -5;
     int rc;
     if ((rc = ensure_generalized(h))) return rc;
     cudaStream_t st = (cudaStream_t)stream;
-    if ((rc = run_generalized_reduce(h, A, S, h->Ap, st))) return rc;
+    double* Xu;
+    if ((rc = stage_in(h, X_out, &h->padV, &Xu, st, false))) return rc;
+    if ((rc = run_generalized_reduce(h, A, S, h->Ap, h->ld, st))) return rc;
     // the reduction's status (S not positive definite) must survive the solve's own reset of info
     h->keep_info = true;
-    rc = pfsm_solve_partial(h, h->Ap, X_out, lambda_out, stream, 5);
+    rc = solve_core(h, h->Ap, Xu, lambda_out, stream, 5, nullptr, nullptr);
     h->keep_info = false;
     if (rc) return rc;
-    return run_generalized_back(h, X_out, st);
+    if ((rc = run_generalized_back(h, Xu, st))) return rc;
+    return stage_out(h, Xu, X_out, st);
 }
 
 // ---- SCF-sequence mode: A is the subspace matrix of a step whose solution is close to the
@@ -1232,40 +1281,45 @@ int pfsm_solve_generalized(pfsm_handle_t h, const double* A, const double* S, do
 int pfsm_solve_warm(pfsm_handle_t h, const double* A, double* V_inout, double* lambda_out, void* stream) {
     if (!h) return -1;
     if (int rc_dev = check_device(h)) return rc_dev;
-    if (!A || ((uintptr_t)A & 15)) return -2;
-    if (!V_inout || ((uintptr_t)V_inout & 15)) return -3;
+    const uintptr_t am = (h->ld == h->N) ? 15 : 7;
+    if (!A || ((uintptr_t)A & am)) return -2;
+    if (!V_inout || ((uintptr_t)V_inout & am)) return -3;
     if (!lambda_out || ((uintptr_t)lambda_out & 7)) return -4;
     int rc;
     if ((rc = ensure_generalized(h))) return rc;  // Ap and LT double as A' and V_prev^T
     cudaStream_t st = (cudaStream_t)stream;
-    const int64_t N = h->N;
+    const int64_t N = h->N, L = h->ld;
     const int32_t n = (int32_t)N;
-    CUtensorMap mapA, mapV;
-    if ((rc = make_map(&mapA, A, N, N, N))) return rc;
-    if ((rc = make_map(&mapV, V_inout, N, N, N))) return rc;
+    if (!h->Ub && (rc = dev_alloc(h, (void**)&h->Ub, (size_t)N * L * sizeof(double)))) return rc;  // U of the rotated problem
+    double *Au, *Vu;
+    if ((rc = stage_in(h, A, &h->padA, &Au, st))) return rc;
+    if ((rc = stage_in(h, V_inout, &h->padV, &Vu, st))) return rc;
+    CUtensorMap mapA, mapV, mapU;
+    if ((rc = make_map(&mapA, Au, N, N, L))) return rc;
+    if ((rc = make_map(&mapV, Vu, N, N, L))) return rc;
+    if ((rc = make_map(&mapU, h->Ub, N, N, L))) return rc;
     const dim3 tb(32, 8), tg((unsigned)((N + 31) / 32), (unsigned)((N + 31) / 32));
     {   // W = V_prev A  (row-major view: row i = (A v_i)^T)
         GemmParams p = base_params();
-        p.C = h->W; p.ldc = N; p.mr = n; p.nc = n; p.klen = n;
+        p.C = h->W; p.ldc = L; p.mr = n; p.nc = n; p.klen = n;
         if ((rc = launch_gemm<EPI_PLAIN>(h, mapV, mapA, h->mapW, p, st))) return rc;
     }
     {   // A'[i][j] = v_i . (A v_j), into S's top half, then symmetrized into Ap
         GemmParams p = base_params();
-        p.C = h->S; p.ldc = N; p.mr = n; p.nc = n; p.klen = n;
+        p.C = h->S; p.ldc = L; p.mr = n; p.nc = n; p.klen = n;
         if ((rc = launch_gemm<EPI_PLAIN>(h, mapV, h->mapW, h->mapS, p, st))) return rc;
-        symmetrize_kernel<<<tg, tb, 0, st>>>(h->S, N, h->Ap, N, n);
+        symmetrize_kernel<<<tg, tb, 0, st>>>(h->S, L, h->Ap, L, n);
         PFSM_CUDA(cudaGetLastError());
     }
-    transpose_kernel<<<tg, tb, 0, st>>>(V_inout, N, h->LT, N, n, n);  // V_prev^T, K-contiguous for the rotation back
+    transpose_kernel<<<tg, tb, 0, st>>>(Vu, L, h->LT, L, n, n);  // V_prev^T, K-contiguous for the rotation back
     PFSM_CUDA(cudaGetLastError());
-    if ((rc = pfsm_solve_partial(h, h->Ap, V_inout, lambda_out, stream, 5))) return rc;  // U, lambda
-    {   // V = V_prev U: row i of the result = sum_k U[i][k] V_prev[k][:]
+    if ((rc = solve_core(h, h->Ap, h->Ub, lambda_out, stream, 5, nullptr, nullptr))) return rc;  // U, lambda
+    {   // V = V_prev U: row i of the result = sum_k U[i][k] V_prev[k][:], written over V_prev (LT keeps its transpose)
         GemmParams p = base_params();
-        p.C = h->W; p.ldc = N; p.mr = n; p.nc = n; p.klen = n;
-        if ((rc = launch_gemm<EPI_PLAIN>(h, mapV, h->mapLT, h->mapW, p, st))) return rc;
+        p.C = Vu; p.ldc = L; p.mr = n; p.nc = n; p.klen = n;
+        if ((rc = launch_gemm<EPI_PLAIN>(h, mapU, h->mapLT, mapV, p, st))) return rc;
     }
-    PFSM_CUDA(cudaMemcpyAsync(V_inout, h->W, (size_t)N * N * sizeof(double), cudaMemcpyDeviceToDevice, st));
-    return 0;
+    return stage_out(h, Vu, V_inout, st);
 }
 
 // ---- f2: the paper's own generalized -> standard conversion (Eq. 14-15; reading R19):
@@ -1277,38 +1331,41 @@ int pfsm_standard_form_eq14(pfsm_handle_t h, const double* A, const double* B, d
                             int32_t symmetrize, void* stream) {
     if (!h) return -1;
     if (int rc_dev = check_device(h)) return rc_dev;
-    if (!A || ((uintptr_t)A & 15)) return -2;
-    if (!B || ((uintptr_t)B & 15)) return -3;
-    if (!Z_out || ((uintptr_t)Z_out & 15)) return -4;
+    const uintptr_t am = (h->ld == h->N) ? 15 : 7;
+    if (!A || ((uintptr_t)A & am)) return -2;
+    if (!B || ((uintptr_t)B & am)) return -3;
+    if (!Z_out || ((uintptr_t)Z_out & 7)) return -4;
     if (niter < 0) return -5;
     cudaStream_t st = (cudaStream_t)stream;
-    const int64_t N = h->N;
+    const int64_t N = h->N, L = h->ld;
     const int32_t n = (int32_t)N;
-    const size_t n2 = (size_t)N * N * sizeof(double);
     int rc;
+    double *Au, *Bu;
+    if ((rc = stage_in(h, A, &h->padA, &Au, st))) return rc;
+    if ((rc = stage_in(h, B, &h->padB, &Bu, st))) return rc;
     CUtensorMap mapB;
-    if ((rc = make_map(&mapB, B, N, N, N))) return rc;
+    if ((rc = make_map(&mapB, Bu, N, N, L))) return rc;
     inv_diag_kernel<<<(unsigned)((N + 255) / 256), 256, 0, st>>>(B, N, n, h->gdiag);
     PFSM_CUDA(cudaGetLastError());
     double* cur = h->W;       // Y_n
     double* nxt = h->S;       // Y_{n+1} (top half of S)
     const CUtensorMap* mcur = &h->mapW;
     const CUtensorMap* mnxt = &h->mapS;
-    PFSM_CUDA(cudaMemcpyAsync(cur, A, n2, cudaMemcpyDeviceToDevice, st));
+    if ((rc = copy_mat(cur, L, A, N, N, st))) return rc;
     for (int it = 0; it < niter; ++it) {
         GemmParams p = base_params();
-        p.C = nxt; p.ldc = N; p.mr = n; p.nc = n; p.klen = n;
-        p.E1 = A; p.ld1 = N; p.E2 = cur; p.ld2 = N; p.eps = h->gdiag;
+        p.C = nxt; p.ldc = L; p.mr = n; p.nc = n; p.klen = n;
+        p.E1 = Au; p.ld1 = L; p.E2 = cur; p.ld2 = L; p.eps = h->gdiag;
         if ((rc = launch_gemm<EPI_JSTEP>(h, *mcur, mapB, *mnxt, p, st))) return rc;
         std::swap(cur, nxt);
         std::swap(mcur, mnxt);
     }
     if (symmetrize) {
         const dim3 tb(32, 8), tg((unsigned)((N + 31) / 32), (unsigned)((N + 31) / 32));
-        symmetrize_kernel<<<tg, tb, 0, st>>>(cur, N, Z_out, N, n);   // (Y + Y^T)/2 = (Z + Z^T)/2
+        symmetrize_kernel<<<tg, tb, 0, st>>>(cur, L, Z_out, N, n);   // (Y + Y^T)/2 = (Z + Z^T)/2
     } else {
         // column-major Z is the same memory as row-major Y = Z^T
-        PFSM_CUDA(cudaMemcpyAsync(Z_out, cur, n2, cudaMemcpyDeviceToDevice, st));
+        if ((rc = copy_mat(Z_out, N, cur, L, N, st))) return rc;
     }
     PFSM_CUDA(cudaGetLastError());
     return 0;
@@ -1325,7 +1382,7 @@ int pfsm_standard_form_eq14(pfsm_handle_t h, const double* A, const double* B, d
 //   phase 4: V = (V^T R^-1)^T, step 5 on the own rows              -> all-gather lambda
 int pfsm_set_shard(pfsm_handle_t h, int32_t rank, int32_t world) {
     if (!h) return -1;
-    if (world < 1 || h->N % h->P != 0 || h->P % world != 0 || (h->N / world) % BM != 0) return -3;
+    if (world < 1 || (h->N & 1) || h->N % h->P != 0 || h->P % world != 0 || (h->N / world) % BM != 0) return -3;
     if (rank < 0 || rank >= world) return -2;
     h->sh_rank = rank;
     h->sh_world = world;
@@ -1336,7 +1393,7 @@ int pfsm_shard_buffer(pfsm_handle_t h, int32_t which, double** ptr) {
     if (!h) return -1;
     if (!ptr) return -3;
     if (which == 0) *ptr = h->S;                                   // G: N x N (row block = own rows)
-    else if (which == 1) *ptr = h->O + (size_t)h->N * h->N;        // V^T R^-1: N x N (row block = own components)
+    else if (which == 1) *ptr = h->O + (size_t)h->N * h->ld;       // V^T R^-1: N x N (row block = own components)
     else return -2;
     return 0;
 }
@@ -1349,14 +1406,14 @@ int pfsm_shard_phase(pfsm_handle_t h, int32_t phase, const double* A, double* V,
     if (!V || ((uintptr_t)V & 15)) return -4;
     if (phase == 4 && !lambda_out) return -5;
     cudaStream_t st = (cudaStream_t)stream;
-    const int64_t N = h->N;
+    const int64_t N = h->N, L = h->ld;
     const int32_t n = (int32_t)N;
     const int32_t rows = n / h->sh_world, r0 = h->sh_rank * rows;
     const int32_t ns = h->P / h->sh_world, s0 = h->sh_rank * ns;
     int rc;
     CUtensorMap mapA, mapV;
-    if ((rc = make_map(&mapV, V, N, N, N))) return rc;
-    if (A && (rc = make_map(&mapA, A, N, N, N))) return rc;
+    if ((rc = make_map(&mapV, V, N, N, L))) return rc;
+    if (A && (rc = make_map(&mapA, A, N, N, L))) return rc;
     const dim3 tb(32, 8), tg((unsigned)((N + 31) / 32), (unsigned)((N + 31) / 32));
     h->ev_valid = false;
     if (phase == 1) {
@@ -1366,19 +1423,19 @@ int pfsm_shard_phase(pfsm_handle_t h, int32_t phase, const double* A, double* V,
         if ((rc = run_step3(h, mapV, mapA, V, r0, rows, st, nullptr))) return rc;
     } else if (phase == 2) {
         GemmParams p = base_params();  // G[r0:r1, :] = V[r0:r1, :] V^T
-        p.C = h->S; p.ldc = N; p.cr0 = r0; p.mr = rows; p.nc = n; p.xr0 = r0; p.klen = n;
+        p.C = h->S; p.ldc = L; p.cr0 = r0; p.mr = rows; p.nc = n; p.xr0 = r0; p.klen = n;
         if ((rc = launch_gemm<EPI_PLAIN>(h, mapV, mapV, h->mapS, p, st))) return rc;
     } else if (phase == 3) {
-        transpose_kernel<<<tg, tb, 0, st>>>(V, N, h->S + (size_t)N * N, N, n, n);
+        transpose_kernel<<<tg, tb, 0, st>>>(V, L, h->S + (size_t)N * L, L, n, n);
         PFSM_CUDA(cudaGetLastError());
-        extract_diag_kernel<<<(unsigned)((N + 255) / 256), 256, 0, st>>>(h->S, N, n, h->gdiag);
+        extract_diag_kernel<<<(unsigned)((N + 255) / 256), 256, 0, st>>>(h->S, L, n, h->gdiag);
         PFSM_CUDA(cudaGetLastError());
         if ((rc = stacked_cholesky(h, true, st, r0, r0 + rows))) return rc;
     } else {
-        transpose_kernel<<<tg, tb, 0, st>>>(h->O + (size_t)N * N, N, V, N, n, n);
+        transpose_kernel<<<tg, tb, 0, st>>>(h->O + (size_t)N * L, L, V, L, n, n);
         PFSM_CUDA(cudaGetLastError());
         GemmParams p = base_params();
-        p.C = h->W; p.ldc = N; p.cr0 = r0; p.mr = rows; p.nc = n; p.xr0 = r0; p.klen = n;
+        p.C = h->W; p.ldc = L; p.cr0 = r0; p.mr = rows; p.nc = n; p.xr0 = r0; p.klen = n;
         if ((rc = launch_gemm<EPI_PLAIN>(h, mapV, mapA, h->mapW, p, st))) return rc;
         if ((rc = launch_rayleigh(h, V, lambda_out, r0, rows, st))) return rc;
     }
@@ -1392,15 +1449,15 @@ int pfsm_solve(pfsm_handle_t h, const double* A, double* V_inout, double* lambda
 // A = A^T: only the lower block triangle (256-row blocks, each with its columns up to the end of its diagonal block)
 // crosses PCIe, 52 % of 8 N^2 bytes at N = 8192; the upper part is mirrored on the device (0.2 ms).
 static int upload_symmetric(pfsm_ctx* h, const double* A_host, cudaStream_t s) {
-    const int64_t N = h->N, RB = 256;
+    const int64_t N = h->N, L = h->ld, RB = 256;
     for (int64_t r0 = 0; r0 < N; r0 += RB) {
         const int64_t rows = std::min<int64_t>(RB, N - r0), width = std::min<int64_t>(N, r0 + RB);
-        PFSM_CUDA(cudaMemcpy2DAsync(h->A_stage + (size_t)r0 * N, (size_t)N * sizeof(double), A_host + (size_t)r0 * N,
+        PFSM_CUDA(cudaMemcpy2DAsync(h->A_stage + (size_t)r0 * L, (size_t)L * sizeof(double), A_host + (size_t)r0 * N,
                                     (size_t)N * sizeof(double), (size_t)width * sizeof(double), (size_t)rows,
                                     cudaMemcpyHostToDevice, s));
     }
     const dim3 tb(32, 8), tg((unsigned)((N + 31) / 32), (unsigned)((N + 31) / 32));
-    mirror_lower_kernel<<<tg, tb, 0, s>>>(h->A_stage, N, (int32_t)N, (int32_t)RB);
+    mirror_lower_kernel<<<tg, tb, 0, s>>>(h->A_stage, L, (int32_t)N, (int32_t)RB);
     PFSM_CUDA(cudaGetLastError());
     return 0;
 }
@@ -1411,7 +1468,7 @@ int pfsm_solve_host(pfsm_handle_t h, const double* A_host, double* V_host, doubl
     if (!A_host) return -2;
     if (!V_host) return -3;
     if (!lambda_host) return -4;
-    const size_t n2 = (size_t)h->N * h->N * sizeof(double);
+    const size_t n2 = (size_t)h->N * h->ld * sizeof(double);
     if (!h->A_stage) {
         int rc;
         if ((rc = dev_alloc(h, (void**)&h->A_stage, n2))) return rc;
@@ -1434,18 +1491,25 @@ int pfsm_solve_host(pfsm_handle_t h, const double* A_host, double* V_host, doubl
         PFSM_CUDA(cudaStreamWaitEvent(h->side, h->ev_fork, 0));
         if ((rc = upload_symmetric(h, A_host, h->side))) return rc;
         PFSM_CUDA(cudaEventRecord(h->ev_rest, h->side));
-        rc = solve_impl(h, h->A_stage, h->V_stage, h->lam_stage, stream, 4, h->Gws, h->ev_rest);  // steps 2-4: V is final
+        rc = solve_core(h, h->A_stage, h->V_stage, h->lam_stage, stream, 4, h->Gws, h->ev_rest);  // steps 2-4: V is final
     } else {
         if ((rc = upload_symmetric(h, A_host, st))) return rc;
-        rc = pfsm_solve_partial(h, h->A_stage, h->V_stage, h->lam_stage, stream, 4);
+        rc = solve_core(h, h->A_stage, h->V_stage, h->lam_stage, stream, 4, nullptr, nullptr);
     }
     if (rc) return rc;
     // V goes back to the host on the side stream while step 5 (which only reads V) computes lambda
     PFSM_CUDA(cudaEventRecord(h->ev_fork, st));
     PFSM_CUDA(cudaStreamWaitEvent(h->side, h->ev_fork, 0));
-    PFSM_CUDA(cudaMemcpyAsync(V_host, h->V_stage, n2, cudaMemcpyDeviceToHost, h->side));
+    PFSM_CUDA(cudaMemcpy2DAsync(V_host, (size_t)h->N * sizeof(double), h->V_stage, (size_t)h->ld * sizeof(double),
+                                (size_t)h->N * sizeof(double), (size_t)h->N, cudaMemcpyDeviceToHost, h->side));
     PFSM_CUDA(cudaEventRecord(h->ev_chain, h->side));
-    if ((rc = pfsm_rayleigh(h, h->A_stage, h->V_stage, h->lam_stage, stream))) return rc;
+    {   // step 5 on the staged (leading dimension ld) matrices
+        CUtensorMap mapA, mapV;
+        if ((rc = make_map(&mapA, h->A_stage, h->N, h->N, h->ld))) return rc;
+        if ((rc = make_map(&mapV, h->V_stage, h->N, h->N, h->ld))) return rc;
+        h->ev_valid = false;
+        if ((rc = run_step5(h, mapV, mapA, h->V_stage, h->lam_stage, st))) return rc;
+    }
     PFSM_CUDA(cudaMemcpyAsync(lambda_host, h->lam_stage, h->N * sizeof(double), cudaMemcpyDeviceToHost, st));
     PFSM_CUDA(cudaStreamWaitEvent(st, h->ev_chain, 0));  // join: the caller's stream covers both copies
     return 0;
@@ -1458,7 +1522,8 @@ int pfsm_get_info(pfsm_handle_t h, void* stream, int64_t* info) {
     unsigned long long v = 0;
     PFSM_CUDA(cudaMemcpyAsync(&v, h->info, sizeof(v), cudaMemcpyDeviceToHost, (cudaStream_t)stream));
     PFSM_CUDA(cudaStreamSynchronize((cudaStream_t)stream));
-    *info = (v == ULLONG_MAX) ? 0 : (int64_t)v;
+    // (the step-2 kernels form their code from the leading dimension: ld + s + 1)
+    *info = (v == ULLONG_MAX) ? 0 : ((int64_t)v > h->ld ? (int64_t)v - (h->ld - h->N) : (int64_t)v);
     return 0;
 }
 
@@ -1477,7 +1542,7 @@ int pfsm_check_validity(pfsm_handle_t h, void* stream, double resid_tol, int32_t
     PFSM_CUDA(cudaMemcpyAsync(&mx, h->gdiag, sizeof(double), cudaMemcpyDeviceToHost, st));
     PFSM_CUDA(cudaMemcpyAsync(&v, h->info, sizeof(v), cudaMemcpyDeviceToHost, st));
     PFSM_CUDA(cudaStreamSynchronize(st));
-    const int64_t info = (v == ~0ULL) ? 0 : (int64_t)v;
+    const int64_t info = (v == ~0ULL) ? 0 : ((int64_t)v > h->ld ? (int64_t)v - (h->ld - h->N) : (int64_t)v);
     *use_standard_solver = (info != 0 || !(mx <= resid_tol)) ? 1 : 0;
     if (max_resid_out) *max_resid_out = mx;
     if (info_out) *info_out = info;

@@ -52,7 +52,6 @@ def test_create_rejects_bad_arguments_before_touching_cuda():
     h = ctypes.c_void_p()
     assert lib.pfsm_create(None, 256, 4, 16, 3, 0.5) == -1
     assert lib.pfsm_create(ctypes.byref(h), 1, 1, 0, 1, 0.5) == -2      # N < 2
-    assert lib.pfsm_create(ctypes.byref(h), 255, 5, 0, 1, 0.5) == -2    # N odd
     assert lib.pfsm_create(ctypes.byref(h), 256, 0, 16, 3, 0.5) == -3   # P < 1
     assert lib.pfsm_create(ctypes.byref(h), 256, 257, 0, 3, 0.5) == -3  # P > N would leave a slice empty (reading R14)
     assert lib.pfsm_create(ctypes.byref(h), 256, 4, -1, 3, 0.5) == -4

@@ -95,6 +95,9 @@ SMALL_CASES = [
     (500, 7, 20, 3, 1e-3, 16.0),     # slices of 71 / 72, M = 112, tiles straddle uneven slice boundaries
     (64, 64, 3, 1, 1e-3, 4.0),       # one eigenpair per slice
     (48, 48, 0, 2, 1e-3, 4.0),       # M = 1: every submatrix is one diagonal entry
+    (255, 5, 8, 2, 1e-3, 12.0),      # odd N: the library works on a leading dimension of N + 1 internally (m = 51, M = 67)
+    (1001, 7, 20, 3, 1e-3, 16.0),    # odd N, several 128-tiles, m = 143, M = 183
+    (3, 1, 0, 1, 1e-1, 1.0),         # smallest odd problem
     (66, 64, 2, 2, 1e-3, 4.0),       # slices of 1 and 2
 ]
 
@@ -354,7 +357,7 @@ def test_breakdown_is_flagged_for_dependent_vectors():
     assert g["info"] != 0 or g["resid"].max() > 100 * gg["resid"].max()
 
 
-@pytest.mark.parametrize("N", [64, 200, 258, 384])
+@pytest.mark.parametrize("N", [64, 200, 258, 384, 131, 257])   # (odd N: staged through a padded copy)
 def test_step4_alone_matches_gram_schmidt(N):
     # step 4 on arbitrary (well-conditioned) vectors: Cholesky-QR == modified Gram-Schmidt (uniqueness of
     # thin QR with positive diagonal R, reading R10 / pin P11)
@@ -390,8 +393,8 @@ def test_step4_flags_dependent_vectors():
     h.destroy()
 
 
-def test_step5_alone_matches_definition():
-    N = 320
+@pytest.mark.parametrize("N", [320, 321])
+def test_step5_alone_matches_definition(N):
     p = gen.small_problem(N, 0.05, 10.0, seed=33)
     X = gen.normal(19, gen.STREAM_TEST, 0, N * N).reshape(N, N)
     X /= np.linalg.norm(X, axis=1, keepdims=True)
@@ -412,13 +415,16 @@ def test_solve_is_deterministic_and_ignores_v_input():
     assert np.array_equal(a["lam"], b["lam"]) and np.array_equal(a["Vr"], b["Vr"])
 
 
-@pytest.mark.parametrize("case", ["config0", "config1", "wide"])
+@pytest.mark.parametrize("case", ["config0", "config1", "wide", "odd"])
 def test_host_buffer_entry_point_matches_device_entry_point(case):
     # config 0: shared-memory Jacobi, config 1: tridiagonal route -- both with the diagonal blocks uploaded ahead of A;
     # wide: M = 700 (blocks as large as A: plain upload)
     if case == "wide":
         p = gen.small_problem(1000, 1e-3, 24.0, seed=808)
         N, P, w, iters = 1000, 2, 100, 2
+    elif case == "odd":
+        p = gen.small_problem(777, 1e-3, 24.0, seed=809)
+        N, P, w, iters = 777, 7, 20, 2
     else:
         p = gen.problem(int(case[-1]))
         N, P, w, iters = p.cfg.N, p.cfg.P, p.cfg.window, p.cfg.iters
@@ -669,7 +675,7 @@ def gpu_generalized(A, S, P, w, iters, alpha):
     return out
 
 
-@pytest.mark.parametrize("N,P,w,iters", [(192, 4, 12, 2), (300, 5, 10, 3), (384, 3, 40, 2)])
+@pytest.mark.parametrize("N,P,w,iters", [(192, 4, 12, 2), (300, 5, 10, 3), (384, 3, 40, 2), (275, 5, 10, 2)])
 def test_generalized_small_against_oracle(N, P, w, iters):
     p = gen.small_problem(N, 2e-3, 12.0, seed=600 + N)
     S = gen.banded_symmetric(N, np.ones(N), 1e-2, 6.0, 600 + N, gen.STREAM_S)
@@ -756,9 +762,9 @@ def gpu_warm(A, Vr_prev, P, w, iters, alpha):
     return out
 
 
-@pytest.mark.parametrize("P", [4, 2])    # M = 144 (Jacobi in step 2) and M = 240 (the tridiagonal route)
-def test_warm_start_sequence_matches_oracle(P):
-    N, w, iters = 384, 24, 3
+@pytest.mark.parametrize("N,P", [(384, 4), (384, 2), (385, 5)])    # M = 144, M = 240; odd N (M = 125)
+def test_warm_start_sequence_matches_oracle(N, P):
+    w, iters = 24, 3
     d = np.sort(gen.uniform(83, gen.STREAM_TEST, 0, N) * 2 - 1)
     X = gen.normal(83, gen.STREAM_TEST, 10_000, N * N).reshape(N, N)
     Q, _ = np.linalg.qr(X)
@@ -834,7 +840,7 @@ def test_solve_is_cuda_graph_capturable(big):
 
 
 # ------------------------------------------------------------------ f2: the paper's Eq. 14-15 conversion
-@pytest.mark.parametrize("N,niter", [(256, 1), (300, 3), (384, 6)])
+@pytest.mark.parametrize("N,niter", [(256, 1), (300, 3), (384, 6), (301, 3)])
 def test_eq14_iteration_matches_oracle(N, niter):
     p = gen.small_problem(N, 2e-3, 12.0, seed=900 + N)
     B = gen.banded_symmetric(N, np.ones(N), 1e-2, 6.0, 900 + N, gen.STREAM_S)
