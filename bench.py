@@ -27,7 +27,7 @@ FP64_NOMINAL_RATIO = 45.0 / 2250.0  # guide's nominal B200 FP64-tensor : bf16-te
 # dram__bytes_read.sum + dram__bytes_write.sum per full-k gemm_tn_kernel launch.  NOT measured in this run: ncu cannot
 # run inside a timed bench, so the figure is copied from a committed `ncu --set full` capture of the same kernel at the
 # same config (config index -> (bytes, file)); configs without a capture report null.
-NCU_TRAFFIC_PER_GEMM_LAUNCH = {4: (8.14e9 + 0.53e9, "profiles/r01c_ncu_full_gemm_final.md")}
+NCU_TRAFFIC_PER_GEMM_LAUNCH = {4: (8.126e9 + 0.528e9, "profiles/r02_ncu_full_gemm.md")}
 
 
 def algorithmic_flops(N: int, M: int, iters: int) -> dict:

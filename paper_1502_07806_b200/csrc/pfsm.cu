@@ -581,6 +581,17 @@ static int launch_jacobi_wide_t(pfsm_ctx* h, const double* A, double* V, cudaStr
 }
 }  // extern "C++"
 
+// Does step 2 of `ns` slices take the blocked tridiagonalization?  (See launch_tridiag for the measurements behind the rule.)
+static bool uses_blocked_sytrd(const pfsm_ctx* h, int32_t ns) {
+    const int64_t M = h->M;
+    if (!h->tridiag || (M % 2) != 0 || M < 4) return false;  // (M even: the tensor maps need a 16-byte pitch)
+    if (h->opt_sytrd_storage == 3) return true;
+    if (h->opt_sytrd_storage != 0) return false;
+    int l2b = 0;
+    if (cudaDeviceGetAttribute(&l2b, cudaDevAttrL2CacheSize, h->device) != cudaSuccess) return false;
+    return (size_t)ns * M * M * sizeof(double) > (size_t)l2b + (size_t)l2b / 2;
+}
+
 // ---- Blocked tridiagonalization (sytrd_blocked.cuh): per panel of SB_NB columns one cooperative launch of
 // sytrd_panel_kernel (C CTAs per slice, per-slice barriers) and one batched rank-2NB trailing update on the DMMA pipe.
 static int ensure_blocked_ws(pfsm_ctx* h) {
@@ -665,11 +676,7 @@ static int launch_tridiag(pfsm_ctx* h, const double* A, double* V, cudaStream_t 
     // column halves the HBM traffic of the lower-triangle kernel but costs two slice barriers and more O(M) work per column,
     // so it wins once the batch is well beyond L2 (step 2, full / lower / blocked: 1536 x 8 = 151 MB 45 / 42 / 42 ms,
     // 2048 x 8 = 268 MB 96 / 80 / 69, 2048 x 16 = 537 MB 163 / 120 / 83; 2048 x 4 = 134 MB 60 / 61 / 75).
-    int l2b = 0;
-    PFSM_CUDA(cudaDeviceGetAttribute(&l2b, cudaDevAttrL2CacheSize, h->device));
-    const bool blocked_ok = (M % 2 == 0) && M >= 4;
-    const bool blocked = blocked_ok && (h->opt_sytrd_storage == 3 ||
-                                        (h->opt_sytrd_storage == 0 && (size_t)ns * M * M * sizeof(double) > (size_t)l2b + (size_t)l2b / 2));
+    const bool blocked = uses_blocked_sytrd(h, ns);
     if (blocked) {
         int rcb;
         if ((rcb = launch_sytrd_blocked(h, A, st, s0, ns, precopied))) return rcb;
@@ -1656,7 +1663,15 @@ int64_t pfsm_launches_per_solve(pfsm_handle_t h) {
             if (cn0 >= h->N) continue;
             trailing += (h->lookahead && npairs >= 3 && cn1 < h->N) ? 2 : 1;
         }
-        const int64_t step2 = h->tridiag ? 5 : 1;  // tridiagonal route: sytrd, bisection, inverse iteration, cluster pass, back-transformation
+        // tridiagonal route: tridiagonalization, bisection, inverse iteration, cluster pass, back-transformation; the blocked
+        // tridiagonalization is a copy, one panel kernel per 32 columns and one trailing update per panel but the last
+        int64_t step2 = h->tridiag ? 5 : 1;
+        if (uses_blocked_sytrd(h, h->P)) {
+            const int64_t panels = (h->M - 1 + SB_NB - 1) / SB_NB, waves = (h->P + h->sms - 1) / h->sms;
+            int64_t gemms = 0;
+            for (int64_t k0 = 0; k0 < h->M - 1; k0 += SB_NB) gemms += (k0 + SB_NB < h->M - 1) ? 1 : 0;
+            step2 = 4 + 1 + waves * (panels + gemms);
+        }
         return step2 + 2 * (int64_t)h->iters + h->cholqr_passes * (2 + 1 + 1 + 2 * nb + pairs + trailing) + 2;
     }
 }

@@ -343,27 +343,12 @@ sytrd_panel_kernel(double* __restrict__ Gws, int32_t M, TriWs ws, SbWs sb, int32
         {
             double* yo = sb.y + ((size_t)(j & 1) * P + s) * M;
             double* bo = sb.base + ((size_t)(j & 1) * P + s) * M;
-            if (tid < 2 * SB_NB) {  // coefficients: the panel dots (sums over the CTAs, fixed order), row k+1 of V and W
-                const int t = tid & 31;
-                double a = 0.0;
-                if (j > 0 && t < j) {
-                    for (int q0 = 0; q0 < C; q0 += 8) {
-                        double x[8];
-#pragma unroll
-                        for (int u = 0; u < 8; ++u) x[u] = (q0 + u < C) ? __ldcg(dots + (size_t)(q0 + u) * (2 * SB_NB) + tid) : 0.0;
-#pragma unroll
-                        for (int u = 0; u < 8; ++u) a += x[u];
-                    }
-                }
-                coef[tid] = a;  // [0, 32): V^T v;  [32, 64): W^T v
-                coef[2 * SB_NB + tid] = (j > 0 && t < j) ? __ldcg(VW + (size_t)(k + 1) * (2 * SB_NB) + tid) : 0.0;  // V[k+1][t], W[k+1][t]
-            }
-            __syncthreads();
-            // a pair of threads per row: the even one takes the V half of the row's panel entries, the odd one the W half;
-            // every load of a row is issued before its first use
+            // a pair of threads per row: the even one takes the V half of the row's panel entries, the odd one the W half.
+            // Every load of a row is issued before its first use, and the loads of the first group of rows go out together
+            // with those of the coefficients (panel dots, row k+1 of V and W): one L2 round trip serves both.
             double yvacc = 0.0;
             const int half = tid & 1, rs = tid >> 1;
-            for (int rbg = rb_first; rbg < nbk; rbg += 8 * C) {
+            for (int rbg = rb_first; rbg < nbk || rbg == rb_first; rbg += 8 * C) {
                 const int i = 32 * (rbg + (rs >> 5) * C) + (rs & 31);
                 const bool ok = i > k && i < M;
                 const double* row = VW + (size_t)(ok ? i : 0) * (2 * SB_NB) + half * SB_NB;
@@ -384,6 +369,24 @@ sytrd_panel_kernel(double* __restrict__ Gws, int32_t M, TriWs ws, SbWs sb, int32
                     } else {
                         extra = (k + 1 < M) ? __ldg(G + (size_t)i * M + k + 1) : 0.0;
                     }
+                }
+                if (rbg == rb_first) {
+                    if (tid < 2 * SB_NB) {  // coefficients: the panel dots (sums over the CTAs, fixed order), row k+1 of V and W
+                        const int t = tid & 31;
+                        double a = 0.0;
+                        if (j > 0 && t < j) {
+                            for (int q0 = 0; q0 < C; q0 += 8) {
+                                double xx[8];
+#pragma unroll
+                                for (int u = 0; u < 8; ++u) xx[u] = (q0 + u < C) ? __ldcg(dots + (size_t)(q0 + u) * (2 * SB_NB) + tid) : 0.0;
+#pragma unroll
+                                for (int u = 0; u < 8; ++u) a += xx[u];
+                            }
+                        }
+                        coef[tid] = a;  // [0, 32): V^T v;  [32, 64): W^T v
+                        coef[2 * SB_NB + tid] = (j > 0 && t < j) ? __ldcg(VW + (size_t)(k + 1) * (2 * SB_NB) + tid) : 0.0;  // V[k+1][t], W[k+1][t]
+                    }
+                    __syncthreads();
                 }
                 // even: s1 += V[i][t] (W^T v)[t], s2 += V[i][t] W[k+1][t];  odd: s1 += W[i][t] (V^T v)[t], s2 += W[i][t] V[k+1][t]
                 const double* c1 = coef + (half ? 0 : SB_NB);
