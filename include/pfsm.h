@@ -63,8 +63,8 @@ typedef struct pfsm_ctx* pfsm_handle_t; /* opaque */
  *   P       number of spectral slices; 1 <= P <= N.  Slice s holds eigen-indices floor(s N / P) .. floor((s+1) N / P) - 1:
  *           N/P of them when P divides N (the paper writes m = N/P), else floor(N/P) or ceil(N/P) (reading R14)
  *   window  halo rows/columns added on each side of a slice's diagonal block; >= 0.
- *           M = min(N, ceil(N/P) + 2*window), the order of every submatrix, must be <= 4096 in this version (else -4; the
- *           paper ran "M <= 3000").  Step 2 is a Householder tridiagonalization + multi-section + inverse
+ *           M = min(N, ceil(N/P) + 2*window), the order of every submatrix, must be <= 8192 in this version (else -4; the
+ *           paper ran "M <= 3000"; 4096 < M <= 8192 always takes the lower-triangle tridiagonalization).  Step 2 is a Householder tridiagonalization + multi-section + inverse
  *           iteration (with re-orthogonalization inside tight eigenvalue clusters) + back-transformation of the slice's own
  *           eigenpairs: the submatrix resident in its cluster's distributed shared memory for small M (the BASELINE
  *           configs), L2- or HBM-resident up to the paper's wide windows, gamma = M/N = 0.2-0.3, where

@@ -133,6 +133,9 @@ struct pfsm_ctx {
     int32_t opt_sytrd_grid = 0;        // 1: grid barrier instead of clusters for small M
 };
 
+// largest submatrix order: the tridiagonal route's back-transformation keeps M / 256 <= 32 doubles per thread and vector
+constexpr int64_t PFSM_MAX_M = 8192;
+
 static int dev_alloc(pfsm_ctx* h, void** p, size_t bytes) {
     PFSM_CUDA(cudaMalloc(p, bytes));
     h->bytes += bytes;
@@ -261,7 +264,7 @@ int pfsm_create(pfsm_handle_t* out, int64_t N, int32_t P, int32_t window, int32_
     if (!std::isfinite(alpha) || !(alpha > 0.0)) return -6;
     const int64_t m = (N + P - 1) / P;  // largest slice; all slices have N / P eigenpairs when P divides N (R14)
     const int64_t M = std::min<int64_t>(N, m + 2 * (int64_t)window);
-    if (M > JW_MAX_M) return -4;
+    if (M > PFSM_MAX_M) return -4;
 
     pfsm_ctx* h = new pfsm_ctx();
     h->N = N; h->ld = N + (N & 1); h->P = P; h->window = window; h->iters = iters; h->alpha = alpha;
@@ -495,7 +498,7 @@ static void choose_jacobi_layout(pfsm_ctx* h) {
     h->jac_cs = 0;
     h->jac_hloc = 0;
     h->jac_half = false;
-    h->jac_wide = h->opt_route == 3;  // option step2_route = 3: the persistent-grid Jacobi kernel at any M
+    h->jac_wide = h->opt_route == 3 && h->M <= JW_MAX_M;  // option step2_route = 3: the persistent-grid Jacobi kernel (M <= 4096)
     // Route of step 2.  Tridiagonalization + bisection + inverse iteration + back-transformation costs ~M latency-bound
     // columns; the Jacobi kernels cost sweeps x (M - 1) rounds.  With the submatrix resident in the cluster's distributed
     // shared memory (sytrd_dsmem_kernel) the tridiagonal route wins at every size measured (step 2, Jacobi -> tridiagonal):
@@ -584,7 +587,7 @@ static int launch_jacobi_wide_t(pfsm_ctx* h, const double* A, double* V, cudaStr
 // Does step 2 of `ns` slices take the blocked tridiagonalization?  (See launch_tridiag for the measurements behind the rule.)
 static bool uses_blocked_sytrd(const pfsm_ctx* h, int32_t ns) {
     const int64_t M = h->M;
-    if (!h->tridiag || (M % 2) != 0 || M < 4) return false;  // (M even: the tensor maps need a 16-byte pitch)
+    if (!h->tridiag || (M % 2) != 0 || M < 4 || M > 4096) return false;  // (M even: 16-byte pitch of the tensor maps; M <= 8 x 512 rows per thread)
     if (h->opt_sytrd_storage == 3) return true;
     if (h->opt_sytrd_storage != 0) return false;
     int l2b = 0;
@@ -688,7 +691,8 @@ static int launch_tridiag(pfsm_ctx* h, const double* A, double* V, cudaStream_t 
         // L2 resident: 11 -> 17 ms, so full storage is kept there)
         int l2 = 0;
         PFSM_CUDA(cudaDeviceGetAttribute(&l2, cudaDevAttrL2CacheSize, h->device));
-        const bool half = h->opt_sytrd_storage != 1 && (h->opt_sytrd_storage == 2 || (size_t)ns * M * M * sizeof(double) > (size_t)l2);
+        // (the full-storage kernel holds row k in 8 registers per thread: M <= 4096; beyond, the lower-triangle kernel)
+        const bool half = M > 4096 || (h->opt_sytrd_storage != 1 && (h->opt_sytrd_storage == 2 || (size_t)ns * M * M * sizeof(double) > (size_t)l2));
         // Small submatrices (a column is latency bound): the CTAs of a slice form a cluster and use its barrier
         const bool small = !half && M <= 768 && h->opt_sytrd_grid != 1;
         bool cluster = small;
@@ -814,7 +818,7 @@ static int launch_tridiag(pfsm_ctx* h, const double* A, double* V, cudaStream_t 
     PFSM_CUDA(cudaGetLastError());
     {
         const int ept = (M + BT_THREADS - 1) / BT_THREADS;
-        const int nvec = ept <= 8 ? 8 : 4;
+        const int nvec = ept <= 8 ? 8 : (ept <= 16 ? 4 : 2);
         const dim3 g3((unsigned)((h->m + nvec - 1) / nvec), (unsigned)ns);
 #define PFSM_BT(E, NVEC) tri_backtransform_kernel<E, NVEC><<<g3, BT_THREADS, 0, st>>>(h->ld, (int32_t)M, tab, h->Gws, h->tri, V, h->eps, s0)
         if (ept <= 1) PFSM_BT(1, 8);
@@ -823,7 +827,9 @@ static int launch_tridiag(pfsm_ctx* h, const double* A, double* V, cudaStream_t 
         else if (ept <= 6) PFSM_BT(6, 8);
         else if (ept <= 8) PFSM_BT(8, 8);
         else if (ept <= 12) PFSM_BT(12, 4);
-        else PFSM_BT(16, 4);
+        else if (ept <= 16) PFSM_BT(16, 4);
+        else if (ept <= 24) PFSM_BT(24, 2);
+        else PFSM_BT(32, 2);
 #undef PFSM_BT
         PFSM_CUDA(cudaGetLastError());
     }

@@ -958,7 +958,7 @@ tri_cluster_kernel(int64_t N, int32_t M, SliceTable tab, TriWs ws, int32_t s_off
 // ---------------------------------------------------------------------------------------------
 constexpr int BT_THREADS = 256;
 
-template <int EPT, int NV>  // NV = 8 or 4; BT_THREADS = 256 (8 warps) is assumed by the cross-warp sum
+template <int EPT, int NV>  // NV = 8, 4 or 2; BT_THREADS = 256 (8 warps) is assumed by the cross-warp sum
 __global__ void __launch_bounds__(BT_THREADS, 1)
 tri_backtransform_kernel(int64_t N, int32_t M, SliceTable tab, const double* __restrict__ Gws, TriWs ws,
                          double* __restrict__ V, double* __restrict__ eps, int32_t s_off) {
@@ -982,7 +982,7 @@ tri_backtransform_kernel(int64_t N, int32_t M, SliceTable tab, const double* __r
     const double* G = Gws + (size_t)s * M * M;
     const double* tau = ws.tau + (size_t)s * M;
     // reflectors k, k-1, .., k-D+1 in flight: at small M one reflector's arithmetic is shorter than an L2 round trip
-    constexpr int D = EPT <= 2 ? 4 : (EPT <= 4 ? 3 : 2);
+    constexpr int D = EPT <= 2 ? 4 : (EPT <= 4 ? 3 : (EPT <= 16 ? 2 : 1));
     double vq[D][EPT];
     int k = M - 3;
 #pragma unroll
@@ -1039,11 +1039,16 @@ tri_backtransform_kernel(int64_t N, int32_t M, SliceTable tab, const double* __r
             t = pb[lane >> 3][lane & 7] + pb[(lane >> 3) + 4][lane & 7];
             t += __shfl_xor_sync(0xffffffffu, t, 8);
             t += __shfl_xor_sync(0xffffffffu, t, 16);
-        } else {
+        } else if (NV == 4) {
             t = pb[lane >> 2][lane & 3];
             t += __shfl_xor_sync(0xffffffffu, t, 4);
             t += __shfl_xor_sync(0xffffffffu, t, 8);
             t += __shfl_xor_sync(0xffffffffu, t, 16);
+        } else {  // NV == 2: lanes 0..15 hold warp (lane >> 1), value (lane & 1)
+            t = (lane < 16) ? pb[lane >> 1][lane & 1] : 0.0;
+            t += __shfl_xor_sync(0xffffffffu, t, 2);
+            t += __shfl_xor_sync(0xffffffffu, t, 4);
+            t += __shfl_xor_sync(0xffffffffu, t, 8);
         }
         t *= tk;
 #pragma unroll

@@ -55,7 +55,7 @@ def test_create_rejects_bad_arguments_before_touching_cuda():
     assert lib.pfsm_create(ctypes.byref(h), 256, 0, 16, 3, 0.5) == -3   # P < 1
     assert lib.pfsm_create(ctypes.byref(h), 256, 257, 0, 3, 0.5) == -3  # P > N would leave a slice empty (reading R14)
     assert lib.pfsm_create(ctypes.byref(h), 256, 4, -1, 3, 0.5) == -4
-    assert lib.pfsm_create(ctypes.byref(h), 16384, 2, 0, 3, 0.5) == -4  # M = 8192 > 4096 unsupported in this version
+    assert lib.pfsm_create(ctypes.byref(h), 32768, 2, 0, 3, 0.5) == -4  # M = 16384 > 8192 unsupported in this version
     assert lib.pfsm_create(ctypes.byref(h), 256, 4, 16, -1, 0.5) == -5
     assert lib.pfsm_create(ctypes.byref(h), 256, 4, 16, 3, 0.0) == -6
     assert lib.pfsm_create(ctypes.byref(h), 256, 4, 16, 3, float("nan")) == -6

@@ -275,11 +275,12 @@ def test_tridiagonal_route_on_exact_multiplets(mult):
     assert g["resid"].max() < 1e-11 * nF
 
 
-@pytest.mark.parametrize("N", [3000, 4096])
+@pytest.mark.parametrize("N", [3000, 4096, 5000, 8192])
 def test_submatrix_order_up_to_the_library_limit(N):
-    # P = 1: the submatrix is A itself, M = N = 3000 ("M <= 3000") and 4096 (the library limit: 16 rows
-    # per thread in the back-transformation, 8 prologue rows per thread in the tridiagonalization).  The oracle's Jacobi
-    # would need hours, so step 2 is checked against its definition: eigenvalues vs LAPACK, residuals, orthonormality
+    # P = 1: the submatrix is A itself, M = N = 3000 ("M <= 3000"), 4096 (the largest order the full-storage,
+    # blocked and persistent-grid-Jacobi kernels take), 5000 and 8192 (the library limit: the lower-triangle
+    # tridiagonalization and 24-32 rows per thread in the back-transformation).  PROPERTY-checked, not oracle-checked: the
+    # oracle's Jacobi would need hours, so step 2 is held to its definition -- eigenvalues vs LAPACK, residuals, orthonormality
     p = gen.small_problem(N, 1e-3, 48.0, seed=6000 + N)
     g2 = gpu_solve(p.A, 1, 0, 1, p.alpha, last_step=2)
     assert g2["info"] == 0
