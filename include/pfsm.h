@@ -212,7 +212,7 @@ int pfsm_check_validity(pfsm_handle_t h, void* stream, double resid_tol, int32_t
 
 /* Largest number of Jacobi sweeps any slice's submatrix eigensolve (step 2) used in the last solve;
  * synchronizes `stream`.  The last sweep is the one that found nothing left to rotate.  Reads 1 when step 2 took
- * the tridiagonal route (M > 160), which has no sweeps. */
+ * the tridiagonal route (the default from M = 16 on), which has no sweeps. */
 int pfsm_get_step2_sweeps(pfsm_handle_t h, void* stream, int32_t* max_sweeps);
 
 /* Device pointer to the N residual norms r_i = ||A v_i - lambda_i v_i||_2 of the last solve (step 5). */

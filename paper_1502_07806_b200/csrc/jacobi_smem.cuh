@@ -1,5 +1,5 @@
 // jacobi_smem.cuh -- step 2, shared-memory resident: one thread-block CLUSTER per slice.  Product path for
-// submatrix orders M <= 160 (BASELINE config 0); second route (PFSM_JACOBI=1) up to M ~ 480.
+// submatrix orders M < 16; second route (option step2_route = 1) up to M ~ 480.
 //
 // Same mathematics as jacobi_batched_kernel (one-sided Jacobi on G = B_s + sigma I, eigenvectors = normalized
 // columns, mu = ||g|| - sigma), but the columns of G never leave shared memory.  The Mp = 2 h columns (M padded

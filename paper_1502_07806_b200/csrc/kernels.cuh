@@ -1,8 +1,8 @@
 // kernels.cuh -- the non-GEMM kernels of the PFSM path (sm_100a):
-//   jacobi_batched_kernel   step 2, second route (PFSM_JACOBI=1) for submatrices too large for shared memory: a cluster
+//   jacobi_batched_kernel   step 2, second route (option step2_route = 1) for submatrices too large for shared memory: a cluster
 //                           of CTAs per slice, one-sided (Hestenes) Jacobi on the slice's shifted submatrix kept in L2,
 //                           round-robin parallel ordering, a warp per column pair.  (The product path of step 2 is
-//                           jacobi_smem.cuh up to M = 160 and tridiag_eig.cuh above.)
+//                           tridiag_eig.cuh from M = 16 on, jacobi_smem.cuh below.)
 //   chol_diag_kernel        step 4: Cholesky factor + inverse of one 128 x 128 diagonal block
 //   extract_diag_kernel     step 4: diag(V^T V) for the breakdown threshold
 //   transpose_kernel        step 4: V <-> V^T staging for the stacked Cholesky-QR

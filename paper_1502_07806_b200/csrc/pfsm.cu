@@ -87,7 +87,7 @@ struct pfsm_ctx {
     unsigned int* jw_bar = nullptr;  // grid-barrier counter of the wide-window Jacobi (M > 512)
     double* nrm_g = nullptr;  // P x (M + 16): final column norms of the shared-memory Jacobi
     bool jac_wide = false;             // persistent-grid Jacobi (jacobi_wide.cuh): option step2_route = 3, at any M
-    bool tridiag = false;              // tridiagonalization route (tridiag_eig.cuh): default for M > 160, step2_route = 2 at any M
+    bool tridiag = false;              // tridiagonalization route (tridiag_eig.cuh): default for M >= 16, step2_route = 2 at any M
     TriWs tri{};                       // its workspace
     SbWs sbw{};                        // workspace of the blocked tridiagonalization (sytrd_blocked.cuh), allocated on first use
     CUtensorMap mapG, mapVW, mapWV;    //   its tensor maps: the stacked submatrices (P M x M) and panel operands (P M x 2 NB)

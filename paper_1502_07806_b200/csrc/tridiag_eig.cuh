@@ -1,5 +1,5 @@
-// tridiag_eig.cuh -- step 2 as a batched dense symmetric eigensolver in four kernels: the product path for
-// submatrix orders 160 < M <= 4096, i.e. BASELINE configs 1-4 (M = 192-256) and the paper's wide windows (gamma = M/N = 0.2-0.3,
+// tridiag_eig.cuh -- step 2 as a batched dense symmetric eigensolver in five kernels: the product path for
+// submatrix orders 16 <= M <= 8192, i.e. all BASELINE configs (M = 96-256) and the paper's wide windows (gamma = M/N = 0.2-0.3,
 // "M <= 3000").  Only the slice's m of the M eigenpairs of B_s are wanted (local ascending ranks
 // off .. off+m-1), which this route exploits:
 //
@@ -8,18 +8,23 @@
 //                           column k, so the trailing matrix is read and written once per column (16 (M-k)^2 bytes).
 //                           CLUSTER (M <= 768): one thread-block cluster per slice, cluster barrier per column -- latency bound;
 //                           otherwise ONE persistent cooperative grid, C CTAs per slice, grid barrier per column.
+//   sytrd_dsmem_kernel      the same with the submatrix resident in the distributed shared memory of the slice's cluster: the
+//                           default for small M (all BASELINE configs), no global-memory access on the per-column chain
+//   (sytrd_blocked.cuh)     the blocked variant with DMMA trailing updates: the default once the batch is well beyond L2
 //   sytrd_half_kernel       the same on the lower triangle only (half the bytes, two grid barriers per column): used when the
 //                           batch 8 P M^2 exceeds L2, where the tridiagonalization is HBM bound
 //   tri_bisect_kernel       eigenvalue of rank off+t of T by 33-way multi-section on the Sturm count, one warp per eigenvalue
 //   tri_invit_kernel        its eigenvector by inverse iteration: LU of T - lambda I with partial pivoting, three
 //                           solves from a counter-based random start, one thread per eigenvector, factors stored
 //                           [row][vector] so that a warp's accesses coalesce
-//   tri_backtransform_kernel  y = H_0 H_1 ... H_{M-3} z, eight (four) eigenvectors per CTA held in registers, each
+//   tri_cluster_kernel      re-orthogonalization + re-iteration inside eigenvalue clusters tighter than 1e-7 ||T|| (dstein's scheme)
+//   tri_backtransform_kernel  y = H_0 H_1 ... H_{M-3} z, eight (four, two) eigenvectors per CTA held in registers, each
 //                           reflector read once per CTA, written zero-padded into V
 //
-// Eigenvalues closer than 10 eps |lambda| get shifts pushed apart as LAPACK's dstein does; there is no
-// re-orthogonalization inside clusters: step 4 orthonormalizes all N vectors anyway, and vectors of a
-// tight cluster that come out numerically dependent are flagged there (info = index of the dependent vector).
+// Eigenvalues closer than 10 eps max(|lambda|, 1e-3 ||T||) get shifts pushed apart as LAPACK's dstein does; vectors of runs
+// of eigenvalues closer than 1e-7 ||T|| are re-orthogonalized and re-iterated (tri_cluster_kernel); wider gaps leave at most
+// 2e-9 of non-orthogonality, which step 4 removes (it orthonormalizes all N vectors anyway).  A vector whose
+// last solve did not converge flags its slice (info = N + s + 1).
 // Every reduction has a fixed order: results are bitwise reproducible.
 #pragma once
 #include <cuda_runtime.h>
