@@ -16,11 +16,12 @@ the Gram / triangular-solve parts of step 4 scale 1/G; the N^3/3 Cholesky is rep
 from __future__ import annotations
 
 
-def _all_gather_rows(t, world: int, rank: int, group=None):
-    """In-place all-gather of a tensor split into `world` equal row blocks (dim 0); this rank's block is valid."""
+def _all_gather_rows(t, world: int, rank: int, group=None, force: bool = False):
+    """In-place all-gather of a tensor split into `world` equal row blocks (dim 0); this rank's block is valid.
+    force: run the collective even for world == 1 (a test executes the NCCL branch on a one-GPU box that way)."""
     import torch
     import torch.distributed as dist
-    if world == 1:
+    if world == 1 and not force:
         return
     chunks = list(t.chunk(world, dim=0))
     assert len(chunks) == world and all(c.shape == chunks[0].shape for c in chunks)

@@ -1,6 +1,7 @@
-"""World-size-2 CPU test (gloo) of the N>1 path's host logic: replicas draw distinct matrices, timings are
-reduced with MAX over ranks, the whole-job value aggregates all ranks' flops, failure on any rank is seen
-by all.  (The GPU kernels themselves are single-GPU: replicas only, no data-path collective.)"""
+"""World-size-2 CPU tests (gloo) of the N>1 paths' host logic.  Replica mode (bench.py --replicas): ranks draw
+distinct matrices, timings are reduced with MAX over ranks, the whole-job value aggregates all ranks' flops, failure
+on any rank is seen by all.  Sharded mode (bench.py's N>1 default): the in-place all-gather of row
+blocks, and the whole solve_sharded sequence driven end to end with a recording fake handle."""
 import os
 import socket
 import sys
