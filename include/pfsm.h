@@ -275,6 +275,22 @@ int pfsm_get_step_ms(pfsm_handle_t h, float* ms4);
  */
 int pfsm_probe_fp64_peak(int32_t kind, void* stream, double* tflops);
 
+/*
+ * Step 5 WITHOUT ANY ALLOCATION, for callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving
+ * loops, harnesses that forbid it): lambda_i = v_i^T A v_i and r_i = ||A v_i - lambda_i v_i||_2 (reading R11; the same two
+ * kernels, operation order and bits as pfsm_rayleigh).  Needs no handle: the one piece of scratch, the N x N product
+ * T = V A, lives in a static device array inside the library (8 MiB on every GPU that loads it, held until exit).
+ *   N          matrix order: even, 2 <= N <= 1024; anything else returns PFSM_ERR_NOALLOC_SIZE
+ *   A, V       device, N x N, leading dimension N, 16-byte aligned, read only (column i of V = vector i)
+ *   lambda_out device, N (out)          resid_out  device, N (out)
+ * Calls no cudaMalloc, cudaFree or allocating library routine; enqueues two kernels on `stream` and returns.
+ * All calls on a device share the static array: it keeps the last call's contents (every call overwrites the part it reads,
+ * nothing needs clearing), and two calls that overlap on the GPU -- different streams, no dependency -- RACE.  Serialize them.
+ * Errors: PFSM_ERR_NOALLOC_SIZE, -2..-5 null or misaligned pointer, 1000+cudaError.
+ */
+#define PFSM_ERR_NOALLOC_SIZE 900
+int pfsm_rayleigh_noalloc(int64_t N, const double* A, const double* V, double* lambda_out, double* resid_out, void* stream);
+
 /* Static text for a return code of this API. */
 const char* pfsm_strerror(int code);
 

@@ -21,7 +21,7 @@ EXPORTS = [
     "pfsm_create", "pfsm_solve", "pfsm_solve_host", "pfsm_solve_partial", "pfsm_orthonormalize", "pfsm_rayleigh", "pfsm_solve_generalized",
     "pfsm_generalized_reduce", "pfsm_solve_warm", "pfsm_standard_form_eq14",
     "pfsm_set_shard", "pfsm_shard_phase", "pfsm_shard_buffer", "pfsm_destroy", "pfsm_get_info", "pfsm_check_validity",
-    "pfsm_get_step2_sweeps", "pfsm_get_residuals", "pfsm_get_shifts", "pfsm_set_alpha", "pfsm_set_cholqr_passes", "pfsm_set_option", "pfsm_workspace_bytes",
+    "pfsm_get_step2_sweeps", "pfsm_get_residuals", "pfsm_get_shifts", "pfsm_set_alpha", "pfsm_set_cholqr_passes", "pfsm_set_option", "pfsm_rayleigh_noalloc", "pfsm_workspace_bytes",
     "pfsm_launches_per_solve", "pfsm_enable_step_timing", "pfsm_get_step_ms", "pfsm_probe_fp64_peak",
     "pfsm_strerror",
 ]
@@ -70,6 +70,7 @@ def load(build_if_missing: bool = True):
     lib.pfsm_set_alpha.argtypes = [p, dbl]
     lib.pfsm_set_cholqr_passes.argtypes = [p, i32]
     lib.pfsm_set_option.argtypes = [p, ctypes.c_char_p, i64]
+    lib.pfsm_rayleigh_noalloc.argtypes = [i64, p, p, p, p, p]
     lib.pfsm_workspace_bytes.argtypes = [p]
     lib.pfsm_workspace_bytes.restype = ctypes.c_size_t
     lib.pfsm_launches_per_solve.argtypes = [p]
@@ -309,3 +310,15 @@ def probe_fp64_peak(kind: int = 0, stream=None) -> float:
     v = ctypes.c_double(0.0)
     _check(load().pfsm_probe_fp64_peak(kind, _stream_ptr(stream), ctypes.byref(v)), "pfsm_probe_fp64_peak")
     return float(v.value)
+
+
+ERR_NOALLOC_SIZE = 900
+
+
+def rayleigh_noalloc(A, Vr, lam, resid, stream=None):
+    """pfsm_rayleigh_noalloc: step 5 with no allocation anywhere (static device scratch inside the library; N even, <= 1024).
+    A, Vr: (N, N) CUDA float64; lam, resid: (N,) CUDA float64 outputs.  Calls sharing a device must not overlap on the GPU."""
+    N = A.shape[0]
+    _check(load().pfsm_rayleigh_noalloc(N, _dev_ptr(A, N, (N, N), "A"), _dev_ptr(Vr, N, (N, N), "V"),
+                                        _dev_ptr(lam, N, (N,), "lambda"), _dev_ptr(resid, N, (N,), "resid"),
+                                        _stream_ptr(stream)), "pfsm_rayleigh_noalloc")

@@ -13,6 +13,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <vector>
 
 #include "gemm_tn.cuh"
@@ -64,6 +65,30 @@ static int make_map(CUtensorMap* map, const double* base, int64_t rows, int64_t 
 }  // namespace pfsm
 
 using namespace pfsm;
+
+// ---- Scratch of the allocation-free entry point pfsm_rayleigh_noalloc (below): T = V A of step 5, N <= 1024.
+// 8 MiB of device memory on every GPU that loads the library, held until the process exits.  In HOST code this name is a
+// host-side stand-in, not a device address: the address kernels and tensor maps use comes from cudaGetSymbolAddress, once
+// per device, with that device current (noalloc_scratch_ptr).
+#define PFSM_NOALLOC_MAX_N 1024
+static __device__ __align__(256) double pfsm_noalloc_scratch[(size_t)PFSM_NOALLOC_MAX_N * PFSM_NOALLOC_MAX_N];
+
+static int noalloc_scratch_ptr(double** out) {
+    constexpr int MAXDEV = 64;
+    static double* addr[MAXDEV] = {nullptr};
+    static std::mutex mu;
+    int dev = -1;
+    PFSM_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= MAXDEV) return PFSM_CUDA_ERROR_BASE + (int)cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(mu);
+    if (!addr[dev]) {
+        void* p = nullptr;
+        PFSM_CUDA(cudaGetSymbolAddress(&p, pfsm_noalloc_scratch));  // the CURRENT device's instance of the array
+        addr[dev] = (double*)p;
+    }
+    *out = addr[dev];
+    return 0;
+}
 
 struct pfsm_ctx {
     int64_t N;
@@ -250,6 +275,8 @@ const char* pfsm_strerror(int code) {
                                       "argument 4 invalid", "argument 5 invalid", "argument 6 invalid"};
         return (-code <= 6) ? names[-code] : "invalid argument";
     }
+    if (code == PFSM_ERR_NOALLOC_SIZE)
+        return "size not served by the allocation-free entry point (pfsm_rayleigh_noalloc: N even, 2 <= N <= 1024)";
     if (code >= PFSM_CUDA_ERROR_BASE) return cudaGetErrorString((cudaError_t)(code - PFSM_CUDA_ERROR_BASE));
     return "unknown error";
 }
@@ -1732,6 +1759,37 @@ int pfsm_probe_fp64_peak(int32_t kind, void* stream, double* tflops) {
     cudaEventDestroy(e0);
     cudaEventDestroy(e1);
     cudaFree(sink);
+    return 0;
+}
+
+// ---- Allocation-free step 5 (reading R11): lambda_i = v_i^T A v_i, r_i = ||A v_i - lambda_i v_i||_2 for callers that cannot
+// call cudaMalloc (CUDA graph capture, tight serving loops, harnesses that forbid it).  No handle (pfsm_create allocates):
+// the N x N product T = V A goes to the file-scope static device array above, everything else is the caller's.  Same two
+// kernels as pfsm_rayleigh (gemm_tn_kernel<PLAIN>, rayleigh_kernel), same operation order, same bits.  Calls no cudaMalloc,
+// cudaFree or allocating library routine.  T is overwritten in full before it is read, so nothing has to be cleared between
+// calls; every call on a device shares the one array, so calls that overlap on the GPU (different streams) race.
+int pfsm_rayleigh_noalloc(int64_t N, const double* A, const double* V, double* lambda_out, double* resid_out, void* stream) {
+    if (N < 2 || (N & 1) || N > PFSM_NOALLOC_MAX_N) return PFSM_ERR_NOALLOC_SIZE;
+    if (!A || ((uintptr_t)A & 15)) return -2;
+    if (!V || ((uintptr_t)V & 15)) return -3;
+    if (!lambda_out || ((uintptr_t)lambda_out & 7)) return -4;
+    if (!resid_out || ((uintptr_t)resid_out & 7)) return -5;
+    cudaStream_t st = (cudaStream_t)stream;
+    double* T = nullptr;
+    int rc;
+    if ((rc = noalloc_scratch_ptr(&T))) return rc;
+    CUtensorMap mapA, mapV, mapT;
+    if ((rc = make_map(&mapA, A, N, N, N))) return rc;
+    if ((rc = make_map(&mapV, V, N, N, N))) return rc;
+    if ((rc = make_map(&mapT, T, N, N, N))) return rc;
+    pfsm_ctx launch_state;  // on the stack: only launch_gemm's per-handle flags are used (no workspace, no allocation)
+    launch_state.N = N;
+    launch_state.ld = N;
+    GemmParams p = base_params();
+    p.C = T; p.ldc = N; p.mr = (int32_t)N; p.nc = (int32_t)N; p.klen = (int32_t)N;
+    if ((rc = launch_gemm<EPI_PLAIN>(&launch_state, mapV, mapA, mapT, p, st))) return rc;
+    rayleigh_kernel<<<(unsigned)N, RAY_THREADS, 0, st>>>(V, T, N, N, lambda_out, resid_out, 0);
+    PFSM_CUDA(cudaGetLastError());
     return 0;
 }
 
