@@ -217,8 +217,17 @@ def run_ours(args):
                          f"{args.gpus}, or without WORLD_SIZE set (bench.py then starts the ranks itself)")
     if not torch.cuda.is_available():
         raise RuntimeError("bench.py needs a CUDA device: the PFSM path has no CPU fallback")
-    torch.cuda.set_device(local_rank)
-    replicas.init("nccl", world, rank, torch.device("cuda", local_rank))
+    ndev = torch.cuda.device_count()
+    if local_rank >= ndev and not args.share_gpu:
+        raise SystemExit(f"bench.py: rank {rank} has no GPU of its own ({ndev} visible, --gpus {args.gpus}); "
+                         "--share-gpu runs the N>1 code path with ranks time-sharing the GPUs (a dry run, not a scaling number)")
+    dev_index = local_rank % ndev
+    torch.cuda.set_device(dev_index)
+    # NCCL needs one GPU per rank; the dry run stages its collectives through the host (gloo), so no kernel of one rank
+    # ever waits on another rank's kernel
+    backend = "gloo" if args.share_gpu else "nccl"
+    coll_dev = "cpu" if backend == "gloo" else "cuda"
+    replicas.init(backend, world, rank, torch.device("cuda", dev_index))
     n_gpus = world
 
     k = args.config
@@ -261,14 +270,14 @@ def run_ours(args):
         torch.cuda.synchronize()
 
     def max_over_ranks(x: float) -> float:
-        return replicas.max_over_ranks(x, world, "cuda")
+        return replicas.max_over_ranks(x, world, coll_dev)
 
     # ---- device-resident leg: K solves, CUDA events on the launching stream ----
     for _ in range(args.warmup):
         solve_once()
     barrier()
-    assert replicas.all_ok(h.info() == 0, world, "cuda"), "PFSM reported a numerical breakdown on a bench matrix"
-    sampler = ClockSampler(local_rank)
+    assert replicas.all_ok(h.info() == 0, world, coll_dev), "PFSM reported a numerical breakdown on a bench matrix"
+    sampler = ClockSampler(dev_index)
     sampler.start()
     time.sleep(0.3)
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
@@ -379,7 +388,7 @@ def run_ours(args):
     achieved = flops_per_launch / (gemm_ms * 1e-3) * 1e-12 if n_launch3 and gemm_ms > 0 else 0.0
     probe_peak = pfsm.probe_fp64_peak(0)
     proxy_peak = peaks["bf16_tflops_sustained"] * FP64_NOMINAL_RATIO
-    sms = torch.cuda.get_device_properties(local_rank).multi_processor_count
+    sms = torch.cuda.get_device_properties(dev_index).multi_processor_count
     clk_ghz = (clocks.get("sm_max_mhz") or 0.0) * 1e-3
     pipe_peak = sms * 64 * 2 * clk_ghz * 1e-3   # SMs x 64 FP64 FMA/clk/SM x 2 flop x max SM clock
     traffic = NCU_TRAFFIC_PER_GEMM_LAUNCH.get(k) if not sharded_mode else None
@@ -454,13 +463,15 @@ def run_ours(args):
 
     # the sample is repeated until ~12 s of CPU work have been timed (at most 8 times), so a fast host still gives
     # a stable figure; the value is flops over the total time of the repeats
-    if args.cpu_cols > 0:
+    if args.cpu_cols > 0 and world == 1:
         cpu_times, cpu_flops, cpu_desc, threads = oracle_sample(k, args.cpu_cols, 1, 0, min_seconds=args.cpu_seconds)
         cpu_value = cpu_flops * len(cpu_times) / sum(cpu_times) * 1e-12
         cpu_desc += f", repeated {len(cpu_times)}x"
     else:  # --cpu-cols 0: skipped (the 2048 x 2048 CPU Jacobi of config 6 alone takes minutes)
         import oracle
-        cpu_times, cpu_value, cpu_desc, threads = [0.0], None, "skipped (--cpu-cols 0)", oracle.num_threads()
+        cpu_times, cpu_value, threads = [0.0], None, oracle.num_threads()
+        cpu_desc = ("skipped: the CPU-oracle leg runs at N=1 only (torchrun also pins OMP_NUM_THREADS=1 per rank)" if world > 1
+                    else "skipped (--cpu-cols 0)")
 
     whole = whole_oracle_record(k, flops["total"])
     line = {
@@ -487,6 +498,9 @@ def run_ours(args):
                          "sample": cpu_desc, "seconds": sum(cpu_times), "whole_oracle_solve": whole},
         "workspace_bytes": h.workspace_bytes(),
     }
+    if args.share_gpu:
+        line["dry_run"] = (f"{world} ranks time-shared {min(world, ndev)} GPU(s), collectives staged through the host (gloo): "
+                           "exercises the N>1 code path, NOT a scaling number")
     line.update(extra)
     print(json.dumps(line))
     replicas.finalize(world)
@@ -522,6 +536,9 @@ def main():
                     help="N>1: independent replicas (rank r solves its own matrix; weak scaling, no collective) instead of "
                          "the default, ONE solve sharded over the ranks (strong scaling)")
     ap.add_argument("--sharded", action="store_true", help="accepted for compatibility: sharding is the N>1 default")
+    ap.add_argument("--share-gpu", action="store_true",
+                    help="dry run of the N>1 path on fewer GPUs than ranks: ranks time-share the GPUs, gloo instead of NCCL; "
+                         "the line is marked dry_run and is not a scaling number")
     ap.add_argument("--generalized", action="store_true",
                     help="also time pfsm_solve_generalized on the config's matrix with S = I + 1e-4 perturbation (row G)")
     ap.add_argument("--option", action="append", default=[], metavar="KEY=INT",

@@ -115,3 +115,35 @@ def test_nccl_branch_of_the_row_gather_executes(tmp_path):
     pr.join(timeout=300)
     assert pr.exitcode == 0
     assert open(out).read() == "ok"
+
+
+def test_bench_n_gt_1_path_dry_run_on_one_gpu():
+    """`python bench.py --gpus 2` starts its own two ranks (torchrun re-exec) and runs the SHARDED solve, the N>1 default.
+    The box has one GPU, so --share-gpu lets the ranks time-share it with host-staged (gloo) gathers: a dry run that
+    executes the whole N>1 bench path -- self-launch, phase/gather events, e2e leg, max-over-ranks, the JSON line -- and
+    must reproduce the single-GPU quality numbers.  Not a scaling number, and the line says so."""
+    import json
+    import subprocess
+    common = ["--config", "0", "--steps", "2", "--no-syevd", "--no-calibrate", "--cpu-cols", "0"]
+    env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK")}
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--share-gpu", *common],
+                         capture_output=True, text=True, timeout=600, env=env)
+    assert out.returncode == 0, out.stderr[-2000:]
+    line = json.loads(out.stdout.strip().splitlines()[-1])
+    assert line["n_gpus"] == 2 and line["scaling"] == "strong" and "dry_run" in line
+    assert "sharded over 2 ranks" in line["config"]["parallelism"]
+    assert set(line["step_ms"]) >= {"phase1_steps2_3", "gather_V", "phase2_gram_rows", "gather_G",
+                                    "phase3_cholesky_trsm_rows", "gather_VRinv", "phase4_step5_rows"}
+    one = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), *common], capture_output=True, text=True,
+                         timeout=600, env=env)
+    assert one.returncode == 0, one.stderr[-2000:]
+    ref = json.loads(one.stdout.strip().splitlines()[-1])
+    assert line["quality"]["info"] == 0 and ref["quality"]["info"] == 0
+    assert abs(line["quality"]["max_residual"] - ref["quality"]["max_residual"]) < 1e-12
+    assert line["quality"]["orthogonality_max"] <= 1e-12 * 256
+    # without --share-gpu a rank without a GPU of its own is an error, not a silent single-rank run
+    bad = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", *common], capture_output=True,
+                         text=True, timeout=600, env=env)
+    import torch
+    if torch.cuda.device_count() < 2:
+        assert bad.returncode != 0 and "has no GPU of its own" in bad.stderr
