@@ -841,8 +841,20 @@ static int launch_tridiag(pfsm_ctx* h, const double* A, double* V, cudaStream_t 
     PFSM_CUDA(cudaGetLastError());
     tri_invit_kernel<<<g2, TRI_THREADS, smem2, st>>>(h->ld, (int32_t)M, tab, h->tri, s0, h->info);
     PFSM_CUDA(cudaGetLastError());
-    tri_cluster_kernel<<<(unsigned)ns, TRC_THREADS, 0, st>>>(h->ld, (int32_t)M, tab, h->tri, s0);
-    PFSM_CUDA(cudaGetLastError());
+    {   // re-orthogonalization inside tight eigenvalue clusters: the runs of a slice are dealt to CX CTAs
+        const bool staged = M <= TRC_STAGED_MAX_M;
+        const size_t smem3 = tri_cluster_smem_bytes(M, h->m, staged);
+        const int cx = std::max(1, std::min(64, (2 * h->sms) / std::max(1, ns)));
+        const dim3 g4((unsigned)cx, (unsigned)ns);
+        if (staged) {
+            PFSM_CUDA(cudaFuncSetAttribute(tri_cluster_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem3));
+            tri_cluster_kernel<true><<<g4, TRC_THREADS, smem3, st>>>(h->ld, (int32_t)M, tab, h->tri, s0, h->m);
+        } else {
+            PFSM_CUDA(cudaFuncSetAttribute(tri_cluster_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem3));
+            tri_cluster_kernel<false><<<g4, TRC_THREADS, smem3, st>>>(h->ld, (int32_t)M, tab, h->tri, s0, h->m);
+        }
+        PFSM_CUDA(cudaGetLastError());
+    }
     {
         const int ept = (M + BT_THREADS - 1) / BT_THREADS;
         const int nvec = ept <= 8 ? 8 : (ept <= 16 ? 4 : 2);

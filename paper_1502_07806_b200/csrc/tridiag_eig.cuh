@@ -842,14 +842,27 @@ tri_invit_kernel(int64_t N, int32_t M, SliceTable tab, TriWs ws, int32_t s_off, 
 // ---------------------------------------------------------------------------------------------
 // Eigenvalue clusters (LAPACK dstein's re-orthogonalization, restricted to the gaps that need it).  Inverse iteration
 // without it delivers the vectors of a pair with gap g to eps ||T|| / g; for g below TRI_CLUSTER_TOL ||T|| two vectors can
-// come out numerically parallel, and step 4 would then orthonormalize noise.  One CTA per slice walks its eigenvalues;
-// for every run of consecutive eigenvalues closer than that, members 2, 3, .. are -- one after the other -- orthogonalized
-// against the earlier members (modified Gram-Schmidt), normalized and put through one more inverse-iteration solve with
-// their own stored LU factors, three times, ending on an orthogonalization.  The dot products run over the CTA (fixed
-// order), the solve is the serial recurrence on one thread; clusters this tight are rare (exact degeneracies).
+// come out numerically parallel, and step 4 would then orthonormalize noise.  For every run of consecutive eigenvalues
+// closer than that, members 2, 3, .. are -- one after the other -- orthogonalized against the earlier members (modified
+// Gram-Schmidt), normalized and put through one more inverse-iteration solve with their own stored LU factors, three
+// times, ending on an orthogonalization.  Runs are independent: the CX CTAs of a slice (grid.x) take them round-robin;
+// inside a run the members follow each other on one CTA.  The dot products run over the CTA (fixed order); the solve is
+// the serial recurrence on one thread, from SHARED memory (STAGED: the vector and its LU factors are staged there once
+// per member, 41 M bytes; the global-memory version pays an L2 round trip per row and is kept for M > 4096).  Exactly
+// degenerate spectra (the paper's diamond cell is "highly degenerate") put every vector through this pass:
+// step 2 of a 13-fold degenerate 256 x 256 matrix took 24 ms with one CTA per slice and global-memory solves, against 1.3 ms
+// for a generic spectrum.
+// Dynamic shared memory: lam[mmax] doubles; STAGED: + z, 1/U_ii, U_i,i+1, U_i,i+2, L multipliers [M] doubles, pivots [M] bytes.
 // ---------------------------------------------------------------------------------------------
 constexpr double TRI_CLUSTER_TOL = 1e-7;
 constexpr int TRC_THREADS = 256;
+constexpr int TRC_STAGED_MAX_M = 4096;
+
+constexpr int TRC_CHUNK = 1024;  // rows per staging chunk of the solve when M > TRC_STAGED_MAX_M
+
+inline size_t tri_cluster_smem_bytes(int M, int mmax, bool staged) {
+    return (size_t)mmax * 8 + (size_t)(staged ? M : TRC_CHUNK) * 41 + 16;
+}
 
 __device__ __forceinline__ double trc_block_sum(double v, double* red) {
     v = warp_sum(v);
@@ -862,10 +875,21 @@ __device__ __forceinline__ double trc_block_sum(double v, double* red) {
     return t;
 }
 
+template <bool STAGED>
 __global__ void __launch_bounds__(TRC_THREADS)
-tri_cluster_kernel(int64_t N, int32_t M, SliceTable tab, TriWs ws, int32_t s_off) {
+tri_cluster_kernel(int64_t N, int32_t M, SliceTable tab, TriWs ws, int32_t s_off, int32_t mmax) {
+    extern __shared__ double trc_sm[];
+    double* lam_s = trc_sm;                          // the slice's eigenvalues
+    const int SL = STAGED ? M : TRC_CHUNK;           // rows the staging arrays hold
+    double* zs = trc_sm + mmax;                      // STAGED: the member's vector and LU factors; else one chunk of them
+    double* f0 = zs + SL;
+    double* f1 = f0 + SL;
+    double* f2 = f1 + SL;
+    double* f3 = f2 + SL;
+    unsigned char* pvs = reinterpret_cast<unsigned char*>(f3 + SL);
     __shared__ double red[TRC_THREADS / 32];
-    const int s = s_off + blockIdx.x, tid = threadIdx.x;
+    const int s = s_off + blockIdx.y, tid = threadIdx.x;
+    const int cta = blockIdx.x, CX = gridDim.x;
     const size_t so = (size_t)s * M;
     const int m = tab.cnt[s], g0 = tab.g0[s];
     double tmax = 0.0;
@@ -873,6 +897,7 @@ tri_cluster_kernel(int64_t N, int32_t M, SliceTable tab, TriWs ws, int32_t s_off
         const double ei = (i < M - 1) ? ws.e[so + i] : 0.0;
         tmax = fmax(tmax, fabs(ws.d[so + i]) + 2.0 * fabs(ei));
     }
+    for (int t = tid; t < m; t += TRC_THREADS) lam_s[t] = ws.lam[g0 + t];
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) tmax = fmax(tmax, __shfl_xor_sync(0xffffffffu, tmax, o));
     __syncthreads();
@@ -881,27 +906,43 @@ tri_cluster_kernel(int64_t N, int32_t M, SliceTable tab, TriWs ws, int32_t s_off
     for (int w = 0; w < TRC_THREADS / 32; ++w) tmax = fmax(tmax, red[w]);
     const double gaptol = TRI_CLUSTER_TOL * tmax;
     const size_t st = (size_t)N;
-    int start = 0;  // first member of the current run
+    int start = 0;   // first member of the current run
+    int runid = -1;  // index of the current run among the runs with at least two members
+    // every thread walks the (shared-memory) eigenvalue list the same way: all branches below are block-uniform
     for (int t = 1; t < m; ++t) {
-        if (ws.lam[g0 + t] - ws.lam[g0 + t - 1] > gaptol) {
+        if (lam_s[t] - lam_s[t - 1] > gaptol) {
             start = t;
             continue;
         }
+        if (t == start + 1) ++runid;
+        if (runid % CX != cta) continue;
         // eigenvalue t belongs to the run [start, t]: orthogonalize its vector against members start .. t-1
         const size_t g = (size_t)g0 + t;
-        double* z = ws.f[4] + g;
+        double* zg = ws.f[4] + g;
+        if (STAGED) {
+            for (int i = tid; i < M; i += TRC_THREADS) {
+                zs[i] = zg[i * st];
+                f0[i] = ws.f[0][g + i * st];
+                f1[i] = ws.f[1][g + i * st];
+                f2[i] = ws.f[2][g + i * st];
+                f3[i] = ws.f[3][g + i * st];
+                pvs[i] = ws.piv[g + i * st];
+            }
+            __syncthreads();
+        }
+        auto Z = [&](int i) -> double& { return STAGED ? zs[i] : zg[i * st]; };
         for (int it = 0; it < 3; ++it) {
             for (int b = start; b < t; ++b) {
                 const double* zb = ws.f[4] + g0 + b;
                 const double sb_ = ws.zscale[g0 + b];
                 double acc = 0.0;
-                for (int i = tid; i < M; i += TRC_THREADS) acc = fma(z[i * st], zb[i * st] * sb_, acc);
+                for (int i = tid; i < M; i += TRC_THREADS) acc = fma(Z(i), zb[i * st] * sb_, acc);
                 const double dot = trc_block_sum(acc, red);
-                for (int i = tid; i < M; i += TRC_THREADS) z[i * st] = fma(-dot, zb[i * st] * sb_, z[i * st]);
+                for (int i = tid; i < M; i += TRC_THREADS) Z(i) = fma(-dot, zb[i * st] * sb_, Z(i));
                 __syncthreads();
             }
             double mx = 0.0;  // scaled 2-norm (the vector carries the growth of the solves)
-            for (int i = tid; i < M; i += TRC_THREADS) mx = fmax(mx, fabs(z[i * st]));
+            for (int i = tid; i < M; i += TRC_THREADS) mx = fmax(mx, fabs(Z(i)));
 #pragma unroll
             for (int o = 16; o > 0; o >>= 1) mx = fmax(mx, __shfl_xor_sync(0xffffffffu, mx, o));
             __syncthreads();
@@ -911,43 +952,104 @@ tri_cluster_kernel(int64_t N, int32_t M, SliceTable tab, TriWs ws, int32_t s_off
             const double inv = (mx > 0.0) ? 1.0 / mx : 1.0;
             double acc = 0.0;
             for (int i = tid; i < M; i += TRC_THREADS) {
-                const double q = z[i * st] * inv;
+                const double q = Z(i) * inv;
                 acc = fma(q, q, acc);
             }
             const double nrm = sqrt(trc_block_sum(acc, red));
             const double sc = (nrm > 0.0) ? inv / nrm : 1.0;
-            for (int i = tid; i < M; i += TRC_THREADS) z[i * st] *= sc;
+            for (int i = tid; i < M; i += TRC_THREADS) Z(i) *= sc;
             __syncthreads();
             if (it == 2) break;
-            if (tid == 0) {  // one more solve with this vector's own factors (the tri_invit_kernel recurrences)
+            // one more solve with this vector's own factors (the tri_invit_kernel recurrences), by thread 0 from shared memory
+            if (STAGED) {
+                if (tid == 0) {
+                    double bi = zs[0];
+                    for (int i = 0; i < M - 1; ++i) {
+                        const double bn = zs[i + 1], f = f3[i];
+                        if (pvs[i]) {
+                            zs[i] = bn;
+                            bi = fma(-f, bn, bi);
+                        } else {
+                            zs[i] = bi;
+                            bi = fma(-f, bi, bn);
+                        }
+                    }
+                    double x1 = bi * f0[M - 1], x2 = 0.0;
+                    zs[M - 1] = x1;
+                    for (int i = M - 2; i >= 0; --i) {
+                        const double xi = (zs[i] - f1[i] * x1 - f2[i] * x2) * f0[i];
+                        zs[i] = xi;
+                        x2 = x1;
+                        x1 = xi;
+                    }
+                }
+            } else {
+                // M > TRC_STAGED_MAX_M: the vector stays in global memory; the solve walks it in chunks of TRC_CHUNK rows
+                // that all threads stage in (operands) and out (results), so that the recurrence never waits on global memory
                 const double* uinv = ws.f[0] + g;
                 const double* u1 = ws.f[1] + g;
                 const double* u2 = ws.f[2] + g;
                 const double* lm = ws.f[3] + g;
                 const unsigned char* pv = ws.piv + g;
-                double bi = z[0];
-                for (int i = 0; i < M - 1; ++i) {
-                    const double bn = z[(size_t)(i + 1) * st], f = lm[i * st];
-                    if (pv[i * st]) {
-                        z[i * st] = bn;
-                        bi = fma(-f, bn, bi);
-                    } else {
-                        z[i * st] = bi;
-                        bi = fma(-f, bi, bn);
+                double bi = zg[0], x1 = 0.0, x2 = 0.0;  // (thread 0's copies carry the recurrences across chunks)
+                for (int i0 = 0; i0 < M - 1; i0 += TRC_CHUNK) {  // forward: L^-1 P^T
+                    const int n = min(TRC_CHUNK, M - 1 - i0);
+                    for (int j = tid; j < n; j += TRC_THREADS) {
+                        f0[j] = zg[(size_t)(i0 + j + 1) * st];
+                        f3[j] = lm[(size_t)(i0 + j) * st];
+                        pvs[j] = pv[(size_t)(i0 + j) * st];
                     }
+                    __syncthreads();
+                    if (tid == 0) {
+                        for (int j = 0; j < n; ++j) {
+                            const double bn = f0[j], f = f3[j];
+                            if (pvs[j]) {
+                                zs[j] = bn;
+                                bi = fma(-f, bn, bi);
+                            } else {
+                                zs[j] = bi;
+                                bi = fma(-f, bi, bn);
+                            }
+                        }
+                    }
+                    __syncthreads();
+                    for (int j = tid; j < n; j += TRC_THREADS) zg[(size_t)(i0 + j) * st] = zs[j];
+                    __syncthreads();
                 }
-                double x1 = bi * uinv[(size_t)(M - 1) * st], x2 = 0.0;
-                z[(size_t)(M - 1) * st] = x1;
-                for (int i = M - 2; i >= 0; --i) {
-                    const double xi = (z[i * st] - u1[i * st] * x1 - u2[i * st] * x2) * uinv[i * st];
-                    z[i * st] = xi;
-                    x2 = x1;
-                    x1 = xi;
+                if (tid == 0) {
+                    x1 = bi * uinv[(size_t)(M - 1) * st];
+                    zg[(size_t)(M - 1) * st] = x1;
+                }
+                for (int i1 = M - 2; i1 >= 0; i1 -= TRC_CHUNK) {  // backward: U^-1, rows i1, i1 - 1, ..
+                    const int n = min(TRC_CHUNK, i1 + 1);
+                    for (int j = tid; j < n; j += TRC_THREADS) {
+                        const size_t i = (size_t)(i1 - j);
+                        f3[j] = zg[i * st];
+                        f0[j] = uinv[i * st];
+                        f1[j] = u1[i * st];
+                        f2[j] = u2[i * st];
+                    }
+                    __syncthreads();
+                    if (tid == 0) {
+                        for (int j = 0; j < n; ++j) {
+                            const double xi = (f3[j] - f1[j] * x1 - f2[j] * x2) * f0[j];
+                            zs[j] = xi;
+                            x2 = x1;
+                            x1 = xi;
+                        }
+                    }
+                    __syncthreads();
+                    for (int j = tid; j < n; j += TRC_THREADS) zg[(size_t)(i1 - j) * st] = zs[j];
+                    __syncthreads();
                 }
             }
             __syncthreads();
         }
+        if (STAGED) {
+            for (int i = tid; i < M; i += TRC_THREADS) zg[i * st] = zs[i];
+        }
         if (tid == 0) ws.zscale[g] = 1.0;
+        __threadfence();  // the next member of the run (same CTA) reads this vector from global memory
         __syncthreads();
     }
 }

@@ -249,6 +249,29 @@ def test_tridiagonal_route_on_near_degenerate_gaps(storage, monkeypatch):
         assert g["resid"].max() < 1e-11 * nA
 
 
+@pytest.mark.parametrize("n", [1100, 2100])
+def test_cluster_pass_on_exact_doubles_at_large_submatrix_orders(n):
+    # A = blockdiag(B, B), P = 1: one submatrix of order M = 2n whose every eigenvalue is exactly double, so EVERY vector
+    # goes through the re-orthogonalization pass (reading R25) -- with its solves staged in shared memory as a whole
+    # (M = 2200) and in chunks (M = 4200 > 4096).  Property-checked (the oracle's Jacobi would need far too long): eigenvalues vs
+    # LAPACK on B, residuals, and orthonormality of the start vectors themselves, pairs included.
+    B = gen.small_problem(n, 1e-3, 24.0, seed=4300 + n).A
+    N = 2 * n
+    A = np.zeros((N, N))
+    A[:n, :n] = B
+    A[n:, n:] = B
+    mu = np.repeat(np.linalg.eigvalsh(B), 2)
+    nA = np.linalg.norm(A)
+    g2 = gpu_solve(A, 1, 0, 1, 0.5 / np.abs(mu).max() ** 2, last_step=2)
+    assert g2["info"] == 0
+    assert np.abs(g2["eps"] - mu).max() <= 1e-12 * nA
+    Y = torch.from_numpy(g2["Vr"]).cuda()
+    dA = torch.from_numpy(A).cuda()
+    R = Y @ dA - torch.from_numpy(g2["eps"]).cuda()[:, None] * Y
+    assert R.abs().max().item() <= 1e-12 * nA
+    assert (Y @ Y.T - torch.eye(N, dtype=torch.float64, device="cuda")).abs().max().item() < 1e-7
+
+
 @pytest.mark.parametrize("mult", [3, 13])
 def test_tridiagonal_route_on_exact_multiplets(mult):
     # A = Q diag(d) Q^T with every eigenvalue repeated `mult` times (13 = the multiplet size of BASELINE config 2,
