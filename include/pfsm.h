@@ -245,6 +245,8 @@ int pfsm_set_cholqr_passes(pfsm_handle_t h, int32_t passes);
  *   "sytrd_grid_barrier"     small M (<= 768): 0 = submatrix resident in the cluster's distributed shared memory when it
  *                            fits (default), 2 = L2-resident submatrix with cluster barriers, 1 = with the grid barrier
  *   "cholesky_lookahead"     default 1; 0: step 4 on one stream                                    [PAPER.md:94-96]
+ *   "cholesky_group"         panels (of 128 columns) per trailing update of step 4: 0 auto (4 from N = 6144 on, while more than
+ *                            24 panels remain, else 2), 2, 4
  *   "chain_launches"         default 1; 0: the step-3 / step-4 GEMMs in plain stream order (same bits)
  *   "cholqr_passes"          as pfsm_set_cholqr_passes (1 | 2)
  * May allocate workspace (a newly selected route).  Errors: -1 handle, -2 unknown key, -3 value out of range,

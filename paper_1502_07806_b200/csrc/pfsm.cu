@@ -156,6 +156,7 @@ struct pfsm_ctx {
     int32_t opt_jacobi_full = 0;       // 1: no half-CTA layout
     int32_t opt_sytrd_storage = 0;     // 0 auto, 1 full storage, 2 lower triangle
     int32_t opt_sytrd_grid = 0;        // 1: grid barrier instead of clusters for small M
+    int32_t opt_chol_group = 0;        // panels per trailing update of step 4: 0 auto, 2, 4
 };
 
 // largest submatrix order: the tridiagonal route's back-transformation keeps M / 256 <= 32 doubles per thread and vector
@@ -914,6 +915,19 @@ static int launch_jacobi(pfsm_ctx* h, const double* A, double* V, cudaStream_t s
     return launch_jacobi_t<16>(h, A, V, st, s0, ns);
 }
 
+// Groups of panels of the stacked Cholesky (see stacked_cholesky): boundaries in panel units, last entry = nblk.
+static std::vector<int32_t> chol_group_bounds(const pfsm_ctx* h) {
+    std::vector<int32_t> gb;
+    const int32_t big = h->opt_chol_group ? h->opt_chol_group : (h->nblk >= 48 ? 4 : 2);
+    const int32_t tail = 24;  // panels at the end that stay in pairs (measured flat between 16 and 24 at N = 8192)
+    for (int32_t k = 0; k < h->nblk;) {
+        gb.push_back(k);
+        k += (big > 2 && h->nblk - k > tail) ? big : 2;
+    }
+    gb.push_back(h->nblk);
+    return gb;
+}
+
 // ---- Stacked right-looking Cholesky on S = [G ; Z] (2N x N, row-major view): O = [L ; Z L^-T] with G = L L^T.
 // The panel step O[r,k] = S[r,k] L_kk^-T and the trailing update S[r,c] -= O[r,k] O[c,k]^T run over every row
 // below the diagonal block, so the triangular solve of the bottom rows is folded into the factorization's GEMMs.
@@ -966,20 +980,31 @@ static int stacked_cholesky(pfsm_ctx* h, bool factor, cudaStream_t st, int32_t b
         int r = factor ? update_rows(c0, n - c0, c0, ncols, kk0, klen, lower) : 0;
         return r ? r : update_rows(n + b0, b1 - b0, c0, ncols, kk0, klen, 0);
     };
-    const int32_t npairs = (h->nblk + 1) / 2;
-    auto pair_c0 = [&](int32_t p) { return std::min<int32_t>(n, 2 * p * CHOL_NB); };  // first column of pair p
-    // the serial chain of pair p: factor its first panel, bring the second panel's columns up to date, factor it
-    auto chain = [&](int32_t p) -> int {
-        const int32_t k = 2 * p, k0 = k * CHOL_NB;
-        int r = factor_panel(k);
-        if (r || k + 1 >= h->nblk) return r;
-        const int32_t k1 = k0 + CHOL_NB, nb1 = (int32_t)std::min<int64_t>(CHOL_NB, N - k1);
-        if ((r = update(k1, nb1, k0, CHOL_NB, 0))) return r;  // second panel's columns only, K = 128
-        return factor_panel(k + 1);
+    // Panels are factored one by one, but the big trailing update is applied once per GROUP of panels (K = 128 x group
+    // size), which divides how often every C tile is read and re-written: groups of opt_chol_group panels (4: K = 512)
+    // while many panels remain, pairs near the end, where the serial chain of a group is no longer hidden by its bulk update.
+    const std::vector<int32_t> gb = chol_group_bounds(h);  // first panel of each group; last entry = nblk
+    const int32_t npairs = (int32_t)gb.size() - 1;         // number of groups
+    auto pair_c0 = [&](int32_t p) {                        // first column of group p
+        return std::min<int32_t>(n, gb[std::min<size_t>((size_t)p, gb.size() - 1)] * CHOL_NB);
     };
-    // columns [c0, c1) of the trailing matrix updated with pair p's panels (K = 256)
+    // the serial chain of group p: for each of its panels, bring the panel's columns up to date with the group's earlier
+    // panels (left-looking inside the group, K = 128 .. 384), then factor it
+    auto chain = [&](int32_t p) -> int {
+        const int32_t kb = gb[p], ke = gb[p + 1];
+        for (int32_t k = kb; k < ke; ++k) {
+            int r;
+            if (k > kb) {
+                const int32_t k1 = k * CHOL_NB, nb1 = (int32_t)std::min<int64_t>(CHOL_NB, N - k1);
+                if ((r = update(k1, nb1, kb * CHOL_NB, (k - kb) * CHOL_NB, 0))) return r;
+            }
+            if ((r = factor_panel(k))) return r;
+        }
+        return 0;
+    };
+    // columns [c0, c1) of the trailing matrix updated with group p's panels
     auto trailing = [&](int32_t p, int32_t c0, int32_t c1) -> int {
-        const int32_t k0 = 2 * p * CHOL_NB, kend = pair_c0(p + 1);
+        const int32_t k0 = pair_c0(p), kend = pair_c0(p + 1);
         return update(c0, c1 - c0, k0, kend - k0, 1);
     };
     if (whole && h->lookahead && npairs >= 3) {
@@ -1665,6 +1690,9 @@ int pfsm_set_option(pfsm_handle_t h, const char* key, int64_t value) {
     } else if (!strcmp(key, "sytrd_grid_barrier")) {
         if (value < 0 || value > 2) return -3;
         h->opt_sytrd_grid = (int32_t)value;
+    } else if (!strcmp(key, "cholesky_group")) {
+        if (value != 0 && value != 2 && value != 4) return -3;
+        h->opt_chol_group = (int32_t)value;
     } else if (!strcmp(key, "cholesky_lookahead")) {
         if (!is01(value)) return -3;
         h->lookahead = value != 0;
@@ -1699,14 +1727,18 @@ int64_t pfsm_launches_per_solve(pfsm_handle_t h) {
     if (!h) return 0;
     // jacobi + 2 iters GEMMs + (2 transposes + Gram + diag extract + per panel: diag, panel, trailing (none after the last)) + GEMM + rayleigh
     {
-        const int64_t nb = h->nblk, pairs = nb / 2, npairs = (nb + 1) / 2;
-        // per panel: chol_diag + panel GEMM; per pair of panels: inner update; trailing updates: one per pair with
-        // columns left, split in two (next pair's columns / the rest) when the look-ahead schedule is active
-        int64_t trailing = 0;
-        for (int64_t p = 0; p < npairs; ++p) {
-            const int64_t cn0 = std::min<int64_t>(h->N, 2 * (p + 1) * CHOL_NB), cn1 = std::min<int64_t>(h->N, 2 * (p + 2) * CHOL_NB);
+        const int64_t nb = h->nblk;
+        // per panel: chol_diag + panel GEMM; inside a group one inner update per panel after its first; trailing updates: one
+        // per group with columns left, split in two (next group's columns / the rest) when the look-ahead schedule is active
+        const std::vector<int32_t> gb = chol_group_bounds(h);
+        const int64_t ngroups = (int64_t)gb.size() - 1;
+        int64_t trailing = 0, pairs = 0;  // pairs = inner updates
+        for (int64_t g = 0; g < ngroups; ++g) {
+            pairs += gb[g + 1] - gb[g] - 1;
+            const int64_t cn0 = std::min<int64_t>(h->N, (int64_t)gb[g + 1] * CHOL_NB);
+            const int64_t cn1 = std::min<int64_t>(h->N, (int64_t)gb[std::min<size_t>((size_t)g + 2, gb.size() - 1)] * CHOL_NB);
             if (cn0 >= h->N) continue;
-            trailing += (h->lookahead && npairs >= 3 && cn1 < h->N) ? 2 : 1;
+            trailing += (h->lookahead && ngroups >= 3 && cn1 < h->N) ? 2 : 1;
         }
         // tridiagonal route: tridiagonalization, bisection, inverse iteration, cluster pass, back-transformation; the blocked
         // tridiagonalization is a copy, one panel kernel per 32 columns and one trailing update per panel but the last

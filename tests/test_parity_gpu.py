@@ -381,6 +381,30 @@ def test_breakdown_is_flagged_for_dependent_vectors():
     assert g["info"] != 0 or g["resid"].max() > 100 * gg["resid"].max()
 
 
+@pytest.mark.parametrize("group", [2, 4])
+def test_step4_panel_groups_match_gram_schmidt(group):
+    # step 4 at a size with a tail: N = 3700 = 28 full panels + 116 columns, so with groups of 4 the schedule mixes groups of
+    # four panels (K = 512 trailing updates, inner updates with K = 128, 256, 384), pairs and a ragged last panel; both
+    # groupings must deliver THE Gram-Schmidt basis (uniqueness of QR), checked against the oracle on a leading block of columns
+    N = 3700
+    X = gen.normal(23, gen.STREAM_TEST, 0, N * N).reshape(N, N) + 4 * np.sqrt(N) * np.eye(N)
+    h = pfsm.Handle(N, 1, 0, 0, 1.0, options={"cholesky_group": group})
+    dV = dev(X)
+    h.orthonormalize(dV)
+    assert h.info() == 0
+    Vg = dV.cpu().numpy()
+    dVg = torch.from_numpy(Vg).cuda()
+    assert (dVg @ dVg.T - torch.eye(N, dtype=torch.float64, device="cuda")).abs().max().item() <= 1e-12 * N
+    R = dVg @ dev(X).T                                        # V_out^T X = R: upper triangular, positive diagonal
+    assert torch.tril(R, -1).abs().max().item() < 1e-9 * np.sqrt(N) * 4
+    assert (torch.diagonal(R) > 0).all()
+    ncol = 300
+    Vo, info = oracle.step4_mgs(X, ncol)                      # Gram-Schmidt of the first columns does not depend on the rest
+    assert info == 0
+    assert np.abs(Vg[:ncol] - Vo[:ncol]).max() < 1e-12
+    h.destroy()
+
+
 @pytest.mark.parametrize("N", [64, 200, 258, 384, 131, 257])   # (odd N: staged through a padded copy)
 def test_step4_alone_matches_gram_schmidt(N):
     # step 4 on arbitrary (well-conditioned) vectors: Cholesky-QR == modified Gram-Schmidt (uniqueness of
