@@ -180,6 +180,28 @@ int pfsm_set_shard(pfsm_handle_t h, int32_t rank, int32_t world);
 int pfsm_shard_phase(pfsm_handle_t h, int32_t phase, const double* A, double* V, double* lambda_out, void* stream);
 int pfsm_shard_buffer(pfsm_handle_t h, int32_t which, double** device_ptr);
 
+/*
+ * PEER-WRITE MODE of the sharded solve: the exchange fused into the kernels that produce the data.  Instead of the caller
+ * all-gathering after each phase, every rank stores its share of a phase's result straight into the other ranks' buffers:
+ * the GEMM epilogues of phases 1-3 write each finished C tile to all ranks (peer device memory over NVLink / NVSwitch), a
+ * small copy kernel does the same for lambda and the residuals.  The caller then only needs a BARRIER between the phases
+ * (all ranks' phase-k work complete before anyone starts phase k+1) and one after phase 4 -- the paper's MPI_Allgatherv
+ * disappears into the product's own stores.  Results are those of the gather mode, bit for bit.
+ *   pfsm_ipc_export   owner process: 64-byte CUDA IPC handle of the allocation that holds `dev_ptr`, and dev_ptr's byte
+ *                     offset in it (the handle travels to the other ranks as plain bytes, e.g. by all_gather_object)
+ *   pfsm_ipc_open     peer process: maps that allocation (enabling peer access on first use); *base_out is what
+ *                     pfsm_ipc_close takes, *ptr_out = base + offset is the usable device pointer
+ *   pfsm_set_shard_peers(h, which, peer_ptrs, npeer)   after pfsm_set_shard: the other ranks' buffer `which`
+ *                     (0: V, 1: pfsm_shard_buffer 0, 2: pfsm_shard_buffer 1, 3: lambda_out, 4: the residuals), npeer =
+ *                     world - 1 mapped pointers in any order (npeer = 0 clears).  The mode is on once all five are set.
+ * Every rank must pass the SAME V and lambda_out buffers to pfsm_shard_phase that its peers registered.  world <= 8.
+ * Errors: -k for argument k; 1000+cudaError (e.g. the allocation cannot be shared: not from cudaMalloc).
+ */
+int pfsm_ipc_export(const void* dev_ptr, void* handle64, int64_t* offset);
+int pfsm_ipc_open(const void* handle64, int64_t offset, void** base_out, void** ptr_out);
+int pfsm_ipc_close(void* base);
+int pfsm_set_shard_peers(pfsm_handle_t h, int32_t which, void* const* peer_ptrs, int32_t npeer);
+
 /* Release the handle and its workspace (synchronizes the device).  NULL is a no-op returning 0. */
 int pfsm_destroy(pfsm_handle_t h);
 

@@ -21,7 +21,8 @@ EXPORTS = [
     "pfsm_create", "pfsm_solve", "pfsm_solve_host", "pfsm_solve_partial", "pfsm_orthonormalize", "pfsm_rayleigh", "pfsm_solve_generalized",
     "pfsm_generalized_reduce", "pfsm_solve_warm", "pfsm_standard_form_eq14",
     "pfsm_set_shard", "pfsm_shard_phase", "pfsm_shard_buffer", "pfsm_destroy", "pfsm_get_info", "pfsm_check_validity",
-    "pfsm_get_step2_sweeps", "pfsm_get_residuals", "pfsm_get_shifts", "pfsm_set_alpha", "pfsm_set_cholqr_passes", "pfsm_set_option", "pfsm_rayleigh_noalloc", "pfsm_workspace_bytes",
+    "pfsm_get_step2_sweeps", "pfsm_get_residuals", "pfsm_get_shifts", "pfsm_set_alpha", "pfsm_set_cholqr_passes", "pfsm_set_option", "pfsm_rayleigh_noalloc", "pfsm_ipc_export", "pfsm_ipc_open", "pfsm_ipc_close",
+    "pfsm_set_shard_peers", "pfsm_workspace_bytes",
     "pfsm_launches_per_solve", "pfsm_enable_step_timing", "pfsm_get_step_ms", "pfsm_probe_fp64_peak",
     "pfsm_strerror",
 ]
@@ -71,6 +72,10 @@ def load(build_if_missing: bool = True):
     lib.pfsm_set_cholqr_passes.argtypes = [p, i32]
     lib.pfsm_set_option.argtypes = [p, ctypes.c_char_p, i64]
     lib.pfsm_rayleigh_noalloc.argtypes = [i64, p, p, p, p, p]
+    lib.pfsm_ipc_export.argtypes = [p, p, ctypes.POINTER(i64)]
+    lib.pfsm_ipc_open.argtypes = [p, i64, ctypes.POINTER(p), ctypes.POINTER(p)]
+    lib.pfsm_ipc_close.argtypes = [p]
+    lib.pfsm_set_shard_peers.argtypes = [p, i32, ctypes.POINTER(p), i32]
     lib.pfsm_workspace_bytes.argtypes = [p]
     lib.pfsm_workspace_bytes.restype = ctypes.c_size_t
     lib.pfsm_launches_per_solve.argtypes = [p]
@@ -187,6 +192,10 @@ class Handle:
         lp = _dev_ptr(lam, N, (N,), "lambda") if lam is not None else None
         _check(self._lib.pfsm_shard_phase(self._h, phase, ap, _dev_ptr(Vr, N, (N, N), "V"), lp, _stream_ptr(stream)),
                "pfsm_shard_phase")
+
+    def set_shard_peers(self, which: int, ptrs):
+        arr = (ctypes.c_void_p * max(1, len(ptrs)))(*ptrs)
+        _check(self._lib.pfsm_set_shard_peers(self._h, which, arr, len(ptrs)), "pfsm_set_shard_peers")
 
     def shard_buffer(self, which: int):
         """Zero-copy (N, N) tensor view of a handle-owned exchange buffer (0: G, 1: V^T R^-1)."""
@@ -322,3 +331,22 @@ def rayleigh_noalloc(A, Vr, lam, resid, stream=None):
     _check(load().pfsm_rayleigh_noalloc(N, _dev_ptr(A, N, (N, N), "A"), _dev_ptr(Vr, N, (N, N), "V"),
                                         _dev_ptr(lam, N, (N,), "lambda"), _dev_ptr(resid, N, (N,), "resid"),
                                         _stream_ptr(stream)), "pfsm_rayleigh_noalloc")
+
+
+def ipc_export(t):
+    """(64-byte handle, byte offset) of the CUDA allocation that holds tensor `t` -- plain Python values for all_gather_object."""
+    buf = ctypes.create_string_buffer(64)
+    off = ctypes.c_int64()
+    _check(load().pfsm_ipc_export(t.data_ptr(), buf, ctypes.byref(off)), "pfsm_ipc_export")
+    return bytes(buf.raw), int(off.value)
+
+
+def ipc_open(handle: bytes, offset: int):
+    """Maps another process's allocation; returns (base, ptr) as ints (pfsm_ipc_close takes base)."""
+    base, ptr = ctypes.c_void_p(), ctypes.c_void_p()
+    _check(load().pfsm_ipc_open(handle, offset, ctypes.byref(base), ctypes.byref(ptr)), "pfsm_ipc_open")
+    return int(base.value), int(ptr.value)
+
+
+def ipc_close(base: int):
+    _check(load().pfsm_ipc_close(base), "pfsm_ipc_close")

@@ -34,6 +34,7 @@ constexpr int GEMM_CONSUMER_WARPS = 8;
 constexpr int GEMM_THREADS = GEMM_CONSUMER_WARPS * 32;       // 256 threads x 255 registers = the whole file
 constexpr int GEMM_PREFETCH = GEMM_STAGES - 2;               // k-blocks in flight ahead of the math
 constexpr int TILE_BYTES = BM * BK * 8;                       // 16 KiB per operand per stage
+constexpr int GEMM_MAX_PEERS = 7;                              // other ranks of one NVSwitch node (8 GPUs)
 constexpr int GEMM_SMEM = GEMM_STAGES * 2 * TILE_BYTES + 1024 /*align*/ + 256 /*barriers*/;
 
 enum Epilogue : int {
@@ -74,6 +75,12 @@ struct GemmParams {
     // grid = nbatch * tiles_per_batch; batch b shifts the X / Y / C row origins by b * bxs / b * bys / b * bcs rows of the
     // same tensor maps (the slices' matrices are stacked row-wise).  nbatch <= 1: a single product.
     int32_t nbatch, tiles_per_batch, bxs, bys, bcs;
+    // Fused compute + all-gather (gemm_tn_kernel<EPI, true> only; the sharded solve): every C tile is also
+    // stored, at the same coordinates, into the buffers of npeer other ranks -- peer device memory mapped through CUDA IPC
+    // (NVLink / NVSwitch P2P stores), so the exchange the paper does with MPI_Allgatherv rides on the
+    // product's own epilogue, tile by tile, instead of following it as a separate collective.
+    double* peerC[GEMM_MAX_PEERS];
+    int32_t npeer;
 };
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -164,7 +171,7 @@ inline int64_t gemm_num_tiles(int32_t ntr, int32_t ntc, int lower) {
     return t;
 }
 
-template <int EPI>
+template <int EPI, bool PEER = false>
 __global__ void __launch_bounds__(GEMM_THREADS, 1)
 gemm_tn_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CUtensorMap mapY,
                const __grid_constant__ CUtensorMap mapC, const GemmParams p) {
@@ -342,9 +349,13 @@ gemm_tn_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__
                         v1 = w[i][j].y - v1;
                     }
                     *reinterpret_cast<double2*>(p.C + o + 8 * j) = make_double2(v0, v1);
+                    if (PEER) {
+                        for (int q = 0; q < p.npeer; ++q) *reinterpret_cast<double2*>(p.peerC[q] + o + 8 * j) = make_double2(v0, v1);
+                    }
                 }
             }
         }
+        if (PEER) __threadfence_system();  // peer stores: visible to the other devices before this grid is seen complete
         signal_done();
         return;
     }
@@ -398,8 +409,18 @@ gemm_tn_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__
                 *reinterpret_cast<double2*>(cp) = make_double2(v0, v1);
             else
                 cp[0] = v0;
+            if (PEER) {
+                for (int q = 0; q < p.npeer; ++q) {
+                    double* pp = p.peerC[q] + ar * p.ldc + ac;
+                    if (pair)
+                        *reinterpret_cast<double2*>(pp) = make_double2(v0, v1);
+                    else
+                        pp[0] = v0;
+                }
+            }
         }
     }
+    if (PEER) __threadfence_system();
     signal_done();
 }
 

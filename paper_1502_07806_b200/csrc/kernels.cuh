@@ -580,6 +580,21 @@ rayleigh_kernel(const double* __restrict__ V, const double* __restrict__ T, int6
     }
 }
 
+// Peer-write mode of the sharded solve: copies `count` doubles of this rank's result into the same place of every other
+// rank's buffer (peer device memory mapped through CUDA IPC).  Used for what no GEMM epilogue produces: lambda and the
+// residuals (N / world doubles each), and the start vectors when there are no folded-spectrum iterations.
+struct PeerPtrs {
+    double* p[GEMM_MAX_PEERS];
+    int32_t n;
+};
+__global__ void peer_copy_kernel(const double* __restrict__ src, int64_t count, PeerPtrs dst) {
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < count; i += (int64_t)gridDim.x * blockDim.x) {
+        const double v = src[i];
+        for (int q = 0; q < dst.n; ++q) dst.p[q][i] = v;
+    }
+    __threadfence_system();
+}
+
 // max_i r[i] (NaN counts as +inf) -> out[0]; one CTA, fixed order.  The validity guard of PAPER.md:98-100.
 __global__ void __launch_bounds__(1024) max_residual_kernel(const double* __restrict__ r, int64_t N, double* __restrict__ out) {
     __shared__ double red[32];

@@ -144,6 +144,11 @@ struct pfsm_ctx {
     int32_t cholqr_passes = 1;         // 2 = CholeskyQR2 (re-orthonormalize once; reading R10)
     bool jac_half = false;             // shared-memory Jacobi with 512-thread CTAs, two per SM (jacobi_smem.cuh)
     int32_t sh_rank = 0, sh_world = 1;  // sharded solve: this handle works on rows [sh_rank, sh_rank+1) * N / sh_world
+    // peer-write mode of the sharded solve (pfsm_set_shard_peers): the other ranks' copies of V, buffer 0 (G), buffer 1
+    // (V^T R^-1), lambda and the residuals, mapped into this process; npeer = 0: the caller all-gathers instead
+    double* peer_buf[5][GEMM_MAX_PEERS] = {};
+    int32_t npeer = 0;
+    bool gemm_attr_peer[5] = {false, false, false, false, false};
     // per-handle launch state (function attributes are per device/context, so nothing here is a process-wide static)
     int sms = 0;                       // multiprocessors of h->device
     bool gemm_attr[5] = {false, false, false, false, false};  // MaxDynamicSharedMemorySize set for gemm_tn_kernel<EPI>
@@ -196,7 +201,7 @@ static int stage_out(pfsm_ctx* h, const double* use, double* dst, cudaStream_t s
 }
 
 // mc: tensor map of the matrix C lives in (used by the SUB / UPDATE epilogues to prefetch the C tile into L2)
-template <int EPI>
+template <int EPI, bool PEER = false>
 // pdl: launch with programmatic stream serialization -- the grid may become resident while the previous gemm_tn_kernel
 // in the stream drains its last wave; p.wait_cnt must then carry the real dependency (GemmParams).
 static int launch_gemm(pfsm_ctx* h, const CUtensorMap& mx, const CUtensorMap& my, const CUtensorMap& mc, GemmParams p,
@@ -208,9 +213,10 @@ static int launch_gemm(pfsm_ctx* h, const CUtensorMap& mx, const CUtensorMap& my
     if (tiles1 <= 0) return 0;
     p.tiles_per_batch = (int32_t)tiles1;
     const int64_t tiles = tiles1 * (p.nbatch > 1 ? p.nbatch : 1);
-    if (!h->gemm_attr[EPI]) {
-        PFSM_CUDA(cudaFuncSetAttribute(gemm_tn_kernel<EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, GEMM_SMEM));
-        h->gemm_attr[EPI] = true;
+    bool& attr_done = PEER ? h->gemm_attr_peer[EPI] : h->gemm_attr[EPI];
+    if (!attr_done) {
+        PFSM_CUDA((cudaFuncSetAttribute(gemm_tn_kernel<EPI, PEER>, cudaFuncAttributeMaxDynamicSharedMemorySize, GEMM_SMEM)));
+        attr_done = true;
     }
     if (pdl && h->pdl_ok) {
         cudaLaunchConfig_t cfg;
@@ -224,14 +230,14 @@ static int launch_gemm(pfsm_ctx* h, const CUtensorMap& mx, const CUtensorMap& my
         at[0].val.programmaticStreamSerializationAllowed = 1;
         cfg.attrs = at;
         cfg.numAttrs = 1;
-        const cudaError_t e = cudaLaunchKernelEx(&cfg, gemm_tn_kernel<EPI>, mx, my, mc, p);
+        const cudaError_t e = cudaLaunchKernelEx(&cfg, gemm_tn_kernel<EPI, PEER>, mx, my, mc, p);
         if (e == cudaSuccess) return 0;
         // only "attribute not supported" falls back to plain stream order (always correct); anything else is a real error
         if (e != cudaErrorNotSupported) return PFSM_CUDA_ERROR_BASE + (int)e;
         cudaGetLastError();
         h->pdl_ok = false;
     }
-    gemm_tn_kernel<EPI><<<(unsigned)tiles, GEMM_THREADS, GEMM_SMEM, st>>>(mx, my, mc, p);
+    gemm_tn_kernel<EPI, PEER><<<(unsigned)tiles, GEMM_THREADS, GEMM_SMEM, st>>>(mx, my, mc, p);
     PFSM_CUDA(cudaGetLastError());
     return 0;
 }
@@ -935,7 +941,8 @@ static std::vector<int32_t> chol_group_bounds(const pfsm_ctx* h) {
 // the bottom rows [N, 2N).  Two-level blocking: 128-wide panels are factored one by one, but the big trailing
 // update is applied once per PAIR of panels with K = 256, halving how often every C tile is read and re-written.
 // b0, b1: only the bottom rows [N + b0, N + b1) are transformed (a rank of the sharded solve owns a row block of Z).
-static int stacked_cholesky(pfsm_ctx* h, bool factor, cudaStream_t st, int32_t b0 = 0, int32_t b1 = -1) {
+// peer_bottom: the transformed bottom rows are also stored into the other ranks' copies of O (peer-write mode).
+static int stacked_cholesky(pfsm_ctx* h, bool factor, cudaStream_t st, int32_t b0 = 0, int32_t b1 = -1, bool peer_bottom = false) {
     const int64_t N = h->N, L = h->ld;
     const int32_t n = (int32_t)N;
     if (b1 < 0) b1 = n;
@@ -953,6 +960,11 @@ static int stacked_cholesky(pfsm_ctx* h, bool factor, cudaStream_t st, int32_t b
         GemmParams pp = base_params();
         pp.C = h->O; pp.ldc = L; pp.cr0 = r0; pp.cc0 = k0; pp.mr = nr; pp.nc = nb;
         pp.xr0 = r0; pp.xk0 = k0; pp.yr0 = k * CHOL_NB; pp.yk0 = 0; pp.klen = nb;
+        if (peer_bottom && h->npeer > 0 && r0 >= n) {  // (peer_buf[2] points at the peer's row N of O: same coordinates as h->O)
+            pp.npeer = h->npeer;
+            for (int i = 0; i < h->npeer; ++i) pp.peerC[i] = h->peer_buf[2][i] - (size_t)N * L;
+            return launch_gemm<EPI_PLAIN, true>(h, h->mapS, h->mapD, h->mapO, pp, cs);
+        }
         return launch_gemm<EPI_PLAIN>(h, h->mapS, h->mapD, h->mapO, pp, cs);
     };
     auto factor_panel = [&](int32_t k) -> int {
@@ -1116,8 +1128,9 @@ static int run_step5(pfsm_ctx* h, const CUtensorMap& mapV, const CUtensorMap& ma
 // blocks were finished waves ago) fill the idle SMs.  Hazards: tile (i, j) of GEMM g+1 overwrites what only tiles (i, .)
 // of GEMM g read, and it starts after all of those have signalled.  A rank of the sharded solve runs the same chain on
 // its own row range (rows / BM row blocks).  *last_cnt = the counters of the last update (nullptr when not chained).
+// peers: the last update also stores its rows of V into the other ranks' V (peer-write mode of the sharded solve).
 static int run_step3(pfsm_ctx* h, const CUtensorMap& mapV, const CUtensorMap& mapA, double* V, int32_t r0, int32_t rows,
-                     cudaStream_t st, const int32_t** last_cnt) {
+                     cudaStream_t st, const int32_t** last_cnt, bool peers = false) {
     const int64_t N = h->N, L = h->ld;
     const int32_t n = (int32_t)N;
     const int32_t nrb = (rows + BM - 1) / BM, ncb = (n + BN - 1) / BN;
@@ -1141,7 +1154,11 @@ static int run_step3(pfsm_ctx* h, const CUtensorMap& mapV, const CUtensorMap& ma
             if (it > 0) { p.wait_cnt = c0 - nrb; p.wait_target = ncb; }
         }
         if ((rc = launch_gemm<EPI_SHIFT>(h, mapV, mapA, h->mapW, p, st, chain && it > 0))) return rc;
-        if ((rc = launch_gemm<EPI_UPDATE>(h, h->mapW, mapA, mapV, q, st, chain))) return rc;
+        if (peers && h->npeer > 0 && it == h->iters - 1) {
+            q.npeer = h->npeer;
+            for (int i = 0; i < h->npeer; ++i) q.peerC[i] = h->peer_buf[0][i];
+            if ((rc = launch_gemm<EPI_UPDATE, true>(h, h->mapW, mapA, mapV, q, st, chain))) return rc;
+        } else if ((rc = launch_gemm<EPI_UPDATE>(h, h->mapW, mapA, mapV, q, st, chain))) return rc;
     }
     if (chain && last_cnt) *last_cnt = h->chain_cnt + (size_t)(2 * h->iters - 1) * nrb;
     return 0;
@@ -1457,12 +1474,25 @@ int pfsm_standard_form_eq14(pfsm_handle_t h, const double* A, const double* B, d
 //   phase 3: Cholesky of G (replicated, N^3/3) + triangular solve of the own rows of V^T (N^3/G)
 //                                                                  -> all-gather rows of V^T R^-1 (buffer 1)
 //   phase 4: V = (V^T R^-1)^T, step 5 on the own rows              -> all-gather lambda
+// copies count doubles at src into buffer `which` of every peer, at element offset `off` of that buffer
+static int peer_copy(pfsm_ctx* h, int which, const double* src, size_t off, int64_t count, cudaStream_t st) {
+    PeerPtrs d;
+    d.n = h->npeer;
+    for (int i = 0; i < GEMM_MAX_PEERS; ++i) d.p[i] = i < h->npeer ? h->peer_buf[which][i] + off : nullptr;
+    const int blocks = (int)std::min<int64_t>((count + 255) / 256, (int64_t)h->sms * 8);
+    peer_copy_kernel<<<blocks, 256, 0, st>>>(src, count, d);
+    PFSM_CUDA(cudaGetLastError());
+    return 0;
+}
+
 int pfsm_set_shard(pfsm_handle_t h, int32_t rank, int32_t world) {
     if (!h) return -1;
     if (world < 1 || (h->N & 1) || h->N % h->P != 0 || h->P % world != 0 || (h->N / world) % BM != 0) return -3;
     if (rank < 0 || rank >= world) return -2;
     h->sh_rank = rank;
     h->sh_world = world;
+    h->npeer = 0;
+    memset(h->peer_buf, 0, sizeof(h->peer_buf));
     return 0;
 }
 
@@ -1497,17 +1527,22 @@ int pfsm_shard_phase(pfsm_handle_t h, int32_t phase, const double* A, double* V,
         PFSM_CUDA(cudaMemsetAsync(h->info, 0xFF, sizeof(unsigned long long), st));
         PFSM_CUDA(cudaMemsetAsync(V + (size_t)r0 * N, 0, (size_t)rows * N * sizeof(double), st));
         if ((rc = launch_jacobi(h, A, V, st, s0, ns))) return rc;
-        if ((rc = run_step3(h, mapV, mapA, V, r0, rows, st, nullptr))) return rc;
+        if ((rc = run_step3(h, mapV, mapA, V, r0, rows, st, nullptr, true))) return rc;
+        if (h->npeer > 0 && h->iters == 0 && (rc = peer_copy(h, 0, V + (size_t)r0 * L, (size_t)r0 * L, (int64_t)rows * L, st))) return rc;
     } else if (phase == 2) {
         GemmParams p = base_params();  // G[r0:r1, :] = V[r0:r1, :] V^T
         p.C = h->S; p.ldc = L; p.cr0 = r0; p.mr = rows; p.nc = n; p.xr0 = r0; p.klen = n;
-        if ((rc = launch_gemm<EPI_PLAIN>(h, mapV, mapV, h->mapS, p, st))) return rc;
+        if (h->npeer > 0) {  // ... stored into every rank's G as the tiles finish
+            p.npeer = h->npeer;
+            for (int i = 0; i < h->npeer; ++i) p.peerC[i] = h->peer_buf[1][i];
+            if ((rc = launch_gemm<EPI_PLAIN, true>(h, mapV, mapV, h->mapS, p, st))) return rc;
+        } else if ((rc = launch_gemm<EPI_PLAIN>(h, mapV, mapV, h->mapS, p, st))) return rc;
     } else if (phase == 3) {
         transpose_kernel<<<tg, tb, 0, st>>>(V, L, h->S + (size_t)N * L, L, n, n);
         PFSM_CUDA(cudaGetLastError());
         extract_diag_kernel<<<(unsigned)((N + 255) / 256), 256, 0, st>>>(h->S, L, n, h->gdiag);
         PFSM_CUDA(cudaGetLastError());
-        if ((rc = stacked_cholesky(h, true, st, r0, r0 + rows))) return rc;
+        if ((rc = stacked_cholesky(h, true, st, r0, r0 + rows, true))) return rc;
     } else {
         transpose_kernel<<<tg, tb, 0, st>>>(h->O + (size_t)N * L, L, V, L, n, n);
         PFSM_CUDA(cudaGetLastError());
@@ -1515,7 +1550,75 @@ int pfsm_shard_phase(pfsm_handle_t h, int32_t phase, const double* A, double* V,
         p.C = h->W; p.ldc = L; p.cr0 = r0; p.mr = rows; p.nc = n; p.xr0 = r0; p.klen = n;
         if ((rc = launch_gemm<EPI_PLAIN>(h, mapV, mapA, h->mapW, p, st))) return rc;
         if ((rc = launch_rayleigh(h, V, lambda_out, r0, rows, st))) return rc;
+        if (h->npeer > 0) {
+            if ((rc = peer_copy(h, 3, lambda_out + r0, (size_t)r0, rows, st))) return rc;
+            if ((rc = peer_copy(h, 4, h->resid + r0, (size_t)r0, rows, st))) return rc;
+        }
     }
+    return 0;
+}
+
+// ---- Peer-write mode of the sharded solve: instead of all-gathering after each phase, every rank stores its share of
+// a phase's result straight into the other ranks' buffers -- from the epilogue of the GEMM that produces it
+// (gemm_tn_kernel<EPI, true>), tile by tile over NVLink / NVSwitch -- and the ranks only synchronize between phases.
+// The other ranks' buffers are ordinary device allocations of their processes, mapped here through CUDA IPC:
+//   pfsm_ipc_export  (owner)  handle + byte offset of a device pointer inside its allocation
+//   pfsm_ipc_open    (peer)   maps the allocation (lazily enabling peer access) and returns base and pointer
+//   pfsm_set_shard_peers      registers, per buffer, the world - 1 mapped pointers of the other ranks
+int pfsm_ipc_export(const void* dev_ptr, void* handle64, int64_t* offset) {
+    if (!dev_ptr) return -1;
+    if (!handle64) return -2;
+    if (!offset) return -3;
+    static_assert(sizeof(cudaIpcMemHandle_t) == 64, "handle size");
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    PFSM_CUDA(cudaGetDriverEntryPoint("cuMemGetAddressRange", &fn, cudaEnableDefault, &q));
+    if (q != cudaDriverEntryPointSuccess || !fn) return PFSM_CUDA_ERROR_BASE + (int)cudaErrorNotSupported;
+    CUdeviceptr base = 0;
+    size_t size = 0;
+    if (((CUresult(*)(CUdeviceptr*, size_t*, CUdeviceptr))fn)(&base, &size, (CUdeviceptr)dev_ptr) != CUDA_SUCCESS)
+        return PFSM_CUDA_ERROR_BASE + (int)cudaErrorInvalidValue;
+    cudaIpcMemHandle_t hd;
+    PFSM_CUDA(cudaIpcGetMemHandle(&hd, (void*)base));
+    memcpy(handle64, &hd, 64);
+    *offset = (int64_t)((CUdeviceptr)dev_ptr - base);
+    return 0;
+}
+
+int pfsm_ipc_open(const void* handle64, int64_t offset, void** base_out, void** ptr_out) {
+    if (!handle64) return -1;
+    if (offset < 0) return -2;
+    if (!base_out) return -3;
+    if (!ptr_out) return -4;
+    cudaIpcMemHandle_t hd;
+    memcpy(&hd, handle64, 64);
+    void* base = nullptr;
+    PFSM_CUDA(cudaIpcOpenMemHandle(&base, hd, cudaIpcMemLazyEnablePeerAccess));
+    *base_out = base;
+    *ptr_out = (char*)base + offset;
+    return 0;
+}
+
+int pfsm_ipc_close(void* base) {
+    if (!base) return -1;
+    PFSM_CUDA(cudaIpcCloseMemHandle(base));
+    return 0;
+}
+
+int pfsm_set_shard_peers(pfsm_handle_t h, int32_t which, void* const* peer_ptrs, int32_t npeer) {
+    if (!h) return -1;
+    if (which < 0 || which > 4) return -2;
+    if (npeer < 0 || npeer > GEMM_MAX_PEERS || npeer != (npeer ? h->sh_world - 1 : 0)) return -4;
+    if (npeer > 0 && !peer_ptrs) return -3;
+    for (int i = 0; i < npeer; ++i)
+        if (!peer_ptrs[i] || ((uintptr_t)peer_ptrs[i] & 7)) return -3;
+    for (int i = 0; i < GEMM_MAX_PEERS; ++i) h->peer_buf[which][i] = i < npeer ? (double*)peer_ptrs[i] : nullptr;
+    // peer-write mode is on once all five buffers are registered (and off again when any is cleared)
+    int32_t all = h->sh_world - 1;
+    for (int b = 0; b < 5; ++b)
+        for (int i = 0; i < h->sh_world - 1; ++i)
+            if (!h->peer_buf[b][i]) all = 0;
+    h->npeer = all;
     return 0;
 }
 

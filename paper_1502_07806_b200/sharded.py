@@ -10,7 +10,12 @@ phases run in libpfsm (pfsm_shard_phase); this module only sequences them with t
     phase 4  step 5 on the own rows                    -> all-gather lambda, residuals
 
 With the NCCL backend the gathers run GPU to GPU over NVLink/NVSwitch on the solve's stream; with gloo (CPU tests,
-or several ranks time-sharing one GPU) they are staged through host memory.  Flop split per rank: steps 2, 3, 5 and
+or several ranks time-sharing one GPU) they are staged through host memory.
+
+PEER-WRITE MODE (setup_peers, then solve_sharded(..., peers=...)): no gathers at all.  Each rank maps the other ranks' V, G,
+V^T R^-1, lambda and residual buffers through CUDA IPC once; from then on the GEMM epilogues of phases 1-3 store every
+finished tile into all ranks' buffers (peer memory over NVLink / NVSwitch, overlapped with the product tile by tile) and
+only a barrier separates the phases.  Same results as the gather mode, bit for bit.  Flop split per rank: steps 2, 3, 5 and
 the Gram / triangular-solve parts of step 4 scale 1/G; the N^3/3 Cholesky is replicated (2 % of the flops).
 """
 from __future__ import annotations
@@ -64,3 +69,73 @@ def solve_sharded(h, A, Vr, lam, group=None, mark=None):
     _all_gather_rows(lam, world, rank, group)
     _all_gather_rows(h.residuals_view(), world, rank, group)
     mark("gather_lambda_resid")
+
+
+class Peers:
+    """The other ranks' buffers of one sharded solve, mapped into this process (see setup_peers)."""
+
+    def __init__(self, bases, group):
+        self.bases = bases       # IPC mappings to close
+        self.group = group
+        self.token = None        # 1-element CUDA tensor for the stream-ordered NCCL barrier
+
+    def close(self):
+        from . import ipc_close
+        for b in self.bases:
+            ipc_close(b)
+        self.bases = []
+
+
+def setup_peers(h, Vr, lam, group=None):
+    """Collective, once per (handle, Vr, lam): exchanges CUDA IPC handles of the five exchanged buffers (V, G, V^T R^-1,
+    lambda, residuals), maps the other ranks' copies and registers them with the handle (pfsm_set_shard_peers).  Vr and lam
+    must be the tensors later passed to solve_sharded.  Returns a Peers object (keep it alive; close() unmaps)."""
+    import torch.distributed as dist
+    from . import ipc_export, ipc_open
+    world = dist.get_world_size(group)
+    rank = dist.get_rank(group)
+    mine = [ipc_export(t) for t in (Vr, h.shard_buffer(0), h.shard_buffer(1), lam, h.residuals_view())]
+    everyone = [None] * world
+    dist.all_gather_object(everyone, mine, group=group)
+    bases = []
+    opened = {}                 # one mapping per (rank, allocation): several buffers may live in one allocation
+    for which in range(5):
+        ptrs = []
+        for r in range(world):
+            if r == rank:
+                continue
+            handle, off = everyone[r][which]
+            key = (r, handle)
+            if key not in opened:
+                base, _ = ipc_open(handle, 0)
+                opened[key] = base
+                bases.append(base)
+            ptrs.append(opened[key] + off)
+        h.set_shard_peers(which, ptrs)
+    return Peers(bases, group)
+
+
+def _phase_barrier(peers):
+    """All ranks' work of the phase (their peer stores included) is complete before anyone goes on.  NCCL: a one-element
+    all-reduce on the solve's stream (stream-ordered, no host synchronization); gloo: device synchronize + host barrier."""
+    import torch
+    import torch.distributed as dist
+    if dist.get_backend(peers.group) == "nccl":
+        if peers.token is None:
+            peers.token = torch.zeros(1, device="cuda")
+        dist.all_reduce(peers.token, group=peers.group)
+    else:
+        torch.cuda.synchronize()
+        dist.barrier(group=peers.group)
+
+
+def solve_sharded_peer_writes(h, A, Vr, lam, peers, mark=None):
+    """The sharded solve in peer-write mode: four compute phases, a barrier after each, no gather.  Collective."""
+    mark = mark or (lambda label: None)
+    mark("start")
+    for phase, label in ((1, "phase1_steps2_3"), (2, "phase2_gram_rows"), (3, "phase3_cholesky_trsm_rows"),
+                         (4, "phase4_step5_rows")):
+        h.shard_phase(phase, A if phase in (1, 4) else None, Vr, lam if phase == 4 else None)
+        mark(label)
+        _phase_barrier(peers)
+        mark("barrier_after_phase%d" % phase)

@@ -147,3 +147,57 @@ def test_bench_n_gt_1_path_dry_run_on_one_gpu():
     import torch
     if torch.cuda.device_count() < 2:
         assert bad.returncode != 0 and "has no GPU of its own" in bad.stderr
+
+
+def _peer_worker(rank, world, port, N, P, w, iters, out_dir):
+    sys.path.insert(0, ROOT)
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), WORLD_SIZE=str(world), RANK=str(rank))
+    import torch
+    import torch.distributed as dist
+
+    import paper_1502_07806_b200 as pfsm
+    import pfsm_inputs as gen
+    from paper_1502_07806_b200 import sharded
+    dist.init_process_group("gloo", world_size=world, rank=rank)
+    torch.cuda.set_device(0)
+    p = gen.small_problem(N, 1e-3, 16.0, seed=4242)
+    h = pfsm.Handle(N, P, w, iters, p.alpha)
+    h.set_shard(rank, world)
+    dA = torch.from_numpy(p.A).cuda()
+    dV = torch.full((N, N), float("nan"), dtype=torch.float64, device="cuda")
+    dl = torch.full((N,), float("nan"), dtype=torch.float64, device="cuda")
+    peers = sharded.setup_peers(h, dV, dl)                 # CUDA IPC: the other process's buffers, mapped here
+    for rep in range(2):                                   # twice: the second solve starts on top of the first one's buffers
+        sharded.solve_sharded_peer_writes(h, dA, dV, dl, peers)
+    torch.cuda.synchronize()
+    np.savez(os.path.join(out_dir, f"peer{rank}.npz"), lam=dl.cpu().numpy(), V=dV.cpu().numpy(),
+             res=h.residuals().cpu().numpy(), info=h.info())
+    dist.barrier()
+    peers.close()
+    h.destroy()
+    dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("N,P,w,iters", [(512, 4, 16, 2), (768, 6, 24, 3), (512, 4, 16, 0)])
+def test_peer_write_mode_equals_gather_mode(tmp_path, N, P, w, iters):
+    """Peer-write mode of the sharded solve: the GEMM epilogues store every finished tile into the other rank's buffers
+    (mapped through CUDA IPC) and only barriers separate the phases.  Two processes time-share the one GPU -- IPC works
+    between processes on one device, and no kernel of one rank waits on the other (phases are separated by a device
+    synchronize + host barrier) -- so the whole mechanism (handle export / open, peer registration, the PEER epilogues of
+    the UPDATE / Gram / panel GEMMs, the copy kernel for lambda and residuals, and for iters = 0 the start vectors) runs
+    here exactly as it would across NVLink.  Must equal the gather mode bit for bit, on every rank."""
+    world = 2
+    ctx = mp.get_context("spawn")
+    for target, port in ((_worker, _free_port()), (_peer_worker, _free_port())):
+        procs = [ctx.Process(target=target, args=(r, world, port, N, P, w, iters, str(tmp_path))) for r in range(world)]
+        for pr in procs:
+            pr.start()
+        for pr in procs:
+            pr.join(timeout=300)
+            assert pr.exitcode == 0
+    for r in range(world):
+        g = np.load(os.path.join(str(tmp_path), f"rank{r}.npz"))      # gather mode (host-staged gloo gathers)
+        q = np.load(os.path.join(str(tmp_path), f"peer{r}.npz"))      # peer-write mode
+        assert int(g["info"]) == 0 and int(q["info"]) == 0
+        assert np.array_equal(q["lam"], g["lam"]) and np.array_equal(q["V"], g["V"]) and np.array_equal(q["res"], g["res"])
+        assert not np.isnan(q["V"]).any() and not np.isnan(q["lam"]).any()
