@@ -192,12 +192,14 @@ def run_reference(args):
     return 0
 
 
-def workload_config(c, n_gpus: int, sharded: bool = False, opts=None) -> dict:
+def workload_config(c, n_gpus: int, sharded: bool = False, opts=None, peer_writes: bool = False) -> dict:
     origin = f"BASELINE.json configs[{c.index}]" if c.index <= 4 else "extra (SURVEY 8(f) f4)"
     return {"workload": f"{origin}: {c.name}, synthetic A = D + E",
             "N": c.N, "P": c.P, "window": c.window, "M": c.M, "iters": c.iters,
             "alpha": "0.5/max|d|^2", "replicas": 1 if sharded else n_gpus, "options": opts or "defaults (product path)",
-            "parallelism": (f"one solve sharded over {n_gpus} ranks (slices -> ranks, 4 all-gathers around step 4)" if sharded
+            "parallelism": ((f"one solve sharded over {n_gpus} ranks (slices -> ranks; peer-write mode: GEMM epilogues store into the "
+                             "other ranks' buffers, barriers between the 4 phases)" if peer_writes else
+                             f"one solve sharded over {n_gpus} ranks (slices -> ranks, 4 all-gathers around step 4)") if sharded
                             else ("single GPU" if n_gpus == 1 else f"replicas x{n_gpus} (independent solves, no collective)")),
             "l2_policy": f"inputs larger than L2 (A, V, W are {8 * c.N * c.N / 2**20:.0f} MiB each vs 126 MB L2)"
             if 8 * c.N * c.N > 126e6 else "L2 flushed between timed iterations (256 MiB write)"}
@@ -247,9 +249,17 @@ def run_ours(args):
         from paper_1502_07806_b200 import sharded
         h.set_shard(rank, world)
 
+    peers = None   # --peer-writes: the other ranks' buffers mapped through CUDA IPC (set up below, once dV / dl exist)
+
+    def run_sharded(mark=None):
+        if peers is not None:
+            sharded.solve_sharded_peer_writes(h, dA, dV, dl, peers, mark=mark)
+        else:
+            sharded.solve_sharded(h, dA, dV, dl, mark=mark)
+
     def solve_once():
         if sharded_mode:
-            sharded.solve_sharded(h, dA, dV, dl)
+            run_sharded()
         else:
             h.solve(dA, dV, dl)
 
@@ -260,6 +270,8 @@ def run_ours(args):
     dA = A_host.cuda()
     dV = torch.empty((N, N), dtype=torch.float64, device="cuda")
     dl = torch.empty((N,), dtype=torch.float64, device="cuda")
+    if sharded_mode and args.peer_writes:
+        peers = sharded.setup_peers(h, dV, dl)
     flush = None
     if 8 * N * N <= 126e6:
         flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
@@ -306,7 +318,7 @@ def run_ours(args):
             e.record(stream)
             marks.append((label, e))
         for i in range(args.steps):
-            sharded.solve_sharded(h, dA, dV, dl, mark=mark)
+            run_sharded(mark=mark)
         torch.cuda.synchronize()
         per = len(marks) // args.steps
         for i in range(args.steps):
@@ -340,7 +352,7 @@ def run_ours(args):
     def e2e_once():
         if sharded_mode:
             dA.copy_(A_host, non_blocking=True)
-            sharded.solve_sharded(h, dA, dV, dl)
+            run_sharded()
             V_host.copy_(dV, non_blocking=True)
             lam_host.copy_(dl, non_blocking=True)
         else:
@@ -479,7 +491,7 @@ def run_ours(args):
         "value": value, "unit": "TFLOP/s", "n_gpus": n_gpus, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "strong" if sharded_mode else "weak",
         "vs_baseline": None,
-        "dtype": "f64", "data": "synthetic", "config": workload_config(c, n_gpus, sharded_mode, opts),
+        "dtype": "f64", "data": "synthetic", "config": workload_config(c, n_gpus, sharded_mode, opts, peers is not None),
         "solve_ms": {"median": float(np.median(solve_ms)), "best": float(min(solve_ms))},
         "step_ms": ({"step2_submatrix_eig": step_ms[0], "step3_folded_spectrum": step_ms[1],
                      "step4_cholesky_qr": step_ms[2], "step5_rayleigh": step_ms[3],
@@ -536,6 +548,9 @@ def main():
                     help="N>1: independent replicas (rank r solves its own matrix; weak scaling, no collective) instead of "
                          "the default, ONE solve sharded over the ranks (strong scaling)")
     ap.add_argument("--sharded", action="store_true", help="accepted for compatibility: sharding is the N>1 default")
+    ap.add_argument("--peer-writes", action="store_true",
+                    help="N>1 sharded solve in peer-write mode: GEMM epilogues store their tiles into the other ranks' buffers "
+                         "(CUDA IPC peer memory over NVLink), barriers instead of all-gathers")
     ap.add_argument("--share-gpu", action="store_true",
                     help="dry run of the N>1 path on fewer GPUs than ranks: ranks time-share the GPUs, gloo instead of NCCL; "
                          "the line is marked dry_run and is not a scaling number")

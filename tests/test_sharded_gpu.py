@@ -138,6 +138,13 @@ def test_bench_n_gt_1_path_dry_run_on_one_gpu():
                          timeout=600, env=env)
     assert one.returncode == 0, one.stderr[-2000:]
     ref = json.loads(one.stdout.strip().splitlines()[-1])
+    # the same run in peer-write mode (GEMM epilogues store into the other rank's buffers through CUDA IPC; barriers, no gathers)
+    pw = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--share-gpu", "--peer-writes", *common],
+                        capture_output=True, text=True, timeout=600, env=env)
+    assert pw.returncode == 0, pw.stderr[-2000:]
+    pwl = json.loads(pw.stdout.strip().splitlines()[-1])
+    assert "peer-write mode" in pwl["config"]["parallelism"] and "barrier_after_phase3" in pwl["step_ms"]
+    assert pwl["quality"] == line["quality"]                 # bit-for-bit the gather mode's result
     assert line["quality"]["info"] == 0 and ref["quality"]["info"] == 0
     assert abs(line["quality"]["max_residual"] - ref["quality"]["max_residual"]) < 1e-12
     assert line["quality"]["orthogonality_max"] <= 1e-12 * 256
