@@ -125,7 +125,8 @@ def _phase_barrier(peers):
             peers.token = torch.zeros(1, device="cuda")
         dist.all_reduce(peers.token, group=peers.group)
     else:
-        torch.cuda.synchronize()
+        if torch.cuda.is_available():
+            torch.cuda.synchronize()
         dist.barrier(group=peers.group)
 
 

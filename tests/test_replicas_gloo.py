@@ -187,3 +187,87 @@ def test_sharded_solve_sequencing_gloo():
     for rank, calls, V, lam, resid, G in res:
         assert calls == [(1, True, False), (2, False, False), (3, False, False), (4, True, True)]
         assert lam == want_lam and resid == want_res and G == want_G and V == want_V
+
+
+class _PeerWritingHandle:
+    """Stands in for pfsm.Handle in PEER-WRITE mode on a CPU-only box.  The ranks' buffers are shared-memory tensors, so a
+    phase can do what the library's PEER epilogues do: store its own row block into EVERY rank's copy.  Before it works,
+    each phase asserts that all ranks' rows of the previous phase have arrived in its OWN copy -- which only holds if
+    solve_sharded_peer_writes puts a barrier after every phase."""
+
+    def __init__(self, rank, world, bufs):
+        self.rank, self.world, self.bufs = rank, world, bufs      # bufs[name][r] = rank r's copy (shared memory)
+        self.calls = []
+
+    def _own(self, n):
+        rows = n // self.world
+        return slice(self.rank * rows, (self.rank + 1) * rows)
+
+    def _write_all(self, name, value):
+        for r in range(self.world):
+            t = self.bufs[name][r]
+            t[self._own(t.shape[0])] = value
+
+    def shard_phase(self, phase, A, Vr, lam, stream=None):
+        import time
+
+        import torch
+        mine = {k: v[self.rank] for k, v in self.bufs.items()}
+        self.calls.append((phase, A is not None, lam is not None))
+        if self.rank == 1:
+            time.sleep(0.2)                                        # a slow rank: without barriers the fast one would run ahead
+        if phase == 1:
+            self._write_all("V", 100.0 + self.rank)
+        elif phase == 2:
+            assert not torch.isnan(mine["V"]).any(), "phase 2 started before every rank's rows of V had arrived"
+            self._write_all("G", 200.0 + self.rank)
+        elif phase == 3:
+            assert not torch.isnan(mine["G"]).any(), "phase 3 started before every rank's rows of G had arrived"
+            self._write_all("O", 300.0 + self.rank)
+        elif phase == 4:
+            assert not torch.isnan(mine["O"]).any(), "phase 4 started before every rank's rows of V^T R^-1 had arrived"
+            self._write_all("lam", 400.0 + self.rank)
+
+
+def _peer_sequence_worker(rank, world, port, bufs, q):
+    sys.path.insert(0, ROOT)
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), WORLD_SIZE=str(world), RANK=str(rank))
+    import torch
+    import torch.distributed as dist
+    from paper_1502_07806_b200 import sharded
+    dist.init_process_group("gloo", world_size=world, rank=rank)
+    h = _PeerWritingHandle(rank, world, bufs)
+    peers = sharded.Peers([], None)
+    A = torch.zeros((8, 8), dtype=torch.float64)
+    labels = []
+    sharded.solve_sharded_peer_writes(h, A, bufs["V"][rank], bufs["lam"][rank], peers, mark=labels.append)
+    # after the last barrier every rank's lambda is complete in every copy
+    q.put((rank, h.calls, labels, bufs["lam"][rank].tolist()))
+    dist.destroy_process_group()
+
+
+def test_peer_write_solve_sequencing_gloo():
+    """solve_sharded_peer_writes end to end on CPU, world size 2: phases 1-4 in order, A only where the library reads it, a
+    barrier after EVERY phase (a slow rank's stores have landed before the fast rank's next phase reads them; the one after
+    phase 4 makes lambda complete everywhere before the call returns)."""
+    import torch
+    world, N = 2, 8
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    bufs = {name: [torch.full(shape, float("nan"), dtype=torch.float64).share_memory_() for _ in range(world)]
+            for name, shape in (("V", (N, N)), ("G", (N, N)), ("O", (N, N)), ("lam", (N,)))}
+    procs = [ctx.Process(target=_peer_sequence_worker, args=(r, world, port, bufs, q)) for r in range(world)]
+    for p in procs:
+        p.start()
+    res = sorted(q.get(timeout=120) for _ in range(world))
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    want_labels = ["start"]
+    for k, name in ((1, "phase1_steps2_3"), (2, "phase2_gram_rows"), (3, "phase3_cholesky_trsm_rows"), (4, "phase4_step5_rows")):
+        want_labels += [name, "barrier_after_phase%d" % k]
+    for rank, calls, labels, lam in res:
+        assert calls == [(1, True, False), (2, False, False), (3, False, False), (4, True, True)]
+        assert labels == want_labels
+        assert lam == [400.0] * 4 + [401.0] * 4
