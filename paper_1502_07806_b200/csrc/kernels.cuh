@@ -300,10 +300,9 @@ chol_diag_kernel(const double* __restrict__ S, double* __restrict__ Lout, int64_
                     if (lane == 0) atomicMin(info, (unsigned long long)(k0 + j0 + j + 1));
                     piv = 1.0;
                 }
-                double rd = rsqrt(piv);
+                const double rd = rsqrt(piv);  // (1 ulp; the scaling below sits on the serial chain, so no refinement there)
                 double d = piv * rd;
-                d = fma(fma(-d, d, piv), 0.5 * rd, d);  // one Newton step: d = sqrt(piv) to the last bit or two
-                rd = fma(fma(-d, rd, 1.0), rd, rd);     // and rd = 1/d
+                d = fma(fma(-d, d, piv), 0.5 * rd, d);  // off the chain: d = sqrt(piv) to the last bit or two (only lane j keeps it)
                 r[j] = (lane == j) ? d : r[j] * rd;
                 if (lane == j) idiag[j0 + j] = rd;
 #pragma unroll
